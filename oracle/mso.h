@@ -1,0 +1,139 @@
+/* mso.h -- CPU ORACLE for the MLP-Splatting forward render (arxiv/paper_2606_03877).
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may load it.  It shares no
+ * source, header, table or helper with the CUDA path (paper_2606_03877_b200/csrc/,
+ * include/mlpsplat.h); it was written from PAPER.md and BASELINE.json's north_star
+ * (NS) before any kernel existed.
+ *
+ * What it computes (citations: P:NN = /root/reference/PAPER.md line NN):
+ *   scene      N primitives (mu, s, unit quaternion q, own MLP)            P:74-76 (Sec.3.1)
+ *   support    ellipsoid { x : |x-mu|^2_Lambda <= 1 },
+ *              Lambda = R diag(s^2)^-1 R^T                                  P:84, NS, Q5
+ *   interval   ray/ellipsoid chord [t_in, t_out], K midpoint samples       NS (c), Q1,Q7
+ *   MLP input  u = S^-1 R^T (p - mu); [u, sin(2^l pi u), cos(2^l pi u)]_l
+ *              [, world-frame unit d]                                       P:101 Eq.5, Q2,Q3,Q15
+ *   MLP        (Linear+ReLU) x n_hidden, Linear; rgb = sigmoid,
+ *              sigma = softplus, extra channels linear                      P:105, Eq.18-19
+ *   composite  alpha = 1-exp(-sigma*delta), T_j = prod_{l<j}(1-alpha_l),
+ *              C = sum_j T_j alpha_j c_j, front to back over all samples of
+ *              the ray sorted by (t, primitive id, k); stop after the sample
+ *              that brings T below t_stop                                   P:113-115 Eq.6, Eq.14
+ *   binning    conservative screen-tile lists of projected supports,
+ *              sorted by (tile, entry depth, primitive id)                  P:119, NS (a),(b)
+ *
+ * Precision: every geometric decision (projection, tile range, intersection,
+ * sample t, sample order, local coordinate u) is evaluated in IEEE fp32,
+ * round-to-nearest, NO fused multiply-add, in the operation order written in
+ * mso.c -- because NS demands bit-exact tile
+ * lists, interval counts and sample order.  The MLP and the compositing sum run
+ * in fp64 from the given float32 weight values.
+ *
+ * Parity pins: tests/test_oracle_pins.py (closed forms, invariants, brute force,
+ * torch fp64 MLP).  Unpinned: nothing on the render path; dataset-level quality
+ * metrics (PSNR/mIoU) are out of scope ("parity unpinned").
+ */
+#ifndef MSO_H
+#define MSO_H
+#include <stdint.h>
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mso_scene mso_scene;
+
+typedef struct {
+  int32_t n;             /* primitives */
+  const float *center;   /* [n][3] */
+  const float *quat;     /* [n][4] (w,x,y,z), normalised here */
+  const float *scale;    /* [n][3] ellipsoid semi-axes > 0 */
+} mso_prims;
+
+typedef struct {
+  int32_t n_freq;        /* L of Eq.5 */
+  int32_t use_viewdir;   /* append raw world-frame unit d after the encoding  */
+  int32_t n_hidden;      /* hidden Linear+ReLU layers                                  */
+  int32_t width;         /* hidden width                                               */
+  int32_t n_feat;        /* linear channels after [r,g,b,sigma] */
+  const float *weights;  /* [n][params]: per layer W[in][out] row-major, then b[out]   */
+} mso_mlp;
+
+typedef struct {
+  float fx, fy, cx, cy;
+  float c2w[12];         /* 3x4 row-major; camera x right, y down, z forward */
+  float t_near;
+} mso_camera;
+
+typedef struct {
+  int32_t K;             /* midpoint samples per interval (NS (c)) */
+  float   t_stop;        /* early termination: stop once T < t_stop (NS (e): 1e-4) */
+  int32_t tile;          /* tile edge in pixels for binned mode; 0 = brute force (no binning) */
+  int32_t n_threads;     /* OpenMP threads; <= 0 = all cores */
+} mso_opts;
+
+typedef struct {
+  int64_t n_pixels;
+  int64_t n_intervals;         /* (ray, primitive) hits */
+  int64_t n_samples;           /* n_intervals * K */
+  int64_t n_mlp_evals;         /* samples actually evaluated (fewer if rays terminated early) */
+  int64_t n_terminated;        /* rays stopped by T < t_stop */
+  int64_t n_pairs;             /* (tile, primitive) keys; 0 in brute mode */
+  double  min_T;               /* smallest final transmittance over the rendered pixels */
+} mso_stats;
+
+enum { MSO_OK = 0, MSO_ERR_ARG = -1, MSO_ERR_MEM = -2, MSO_ERR_CAP = -3 };
+
+int  mso_scene_create(const mso_prims *, const mso_mlp *, mso_scene **out);
+void mso_scene_destroy(mso_scene *);
+
+/* Renders pixels pix[0..n_pix) (linear index y*W+x), or all H*W pixels in raster
+ * order when pix == NULL.  Outputs are fp64: rgb[n][3], alpha[n], feat[n][n_feat]
+ * (feat may be NULL).  stats may be NULL. */
+int mso_render(const mso_scene *, const mso_camera *, int H, int W, const mso_opts *,
+               const int32_t *pix, int64_t n_pix,
+               double *out_rgb, double *out_alpha, double *out_feat, mso_stats *stats);
+
+/* ---- parity artefacts (NS: "tile lists, interval counts and sample ordering bit-exact") ---- */
+
+/* Sorted (tile, z_entry bits, primitive) keys.  tile_offsets[tiles+1]; prim_ids/zbits[cap].
+ * Returns MSO_ERR_CAP (with *n set) if cap is too small; call with cap = 0 to size. */
+int mso_tile_lists(const mso_scene *, const mso_camera *, int H, int W, int tile,
+                   int64_t *tile_offsets, int32_t *prim_ids, uint32_t *zbits,
+                   size_t cap, size_t *n);
+
+/* Per-pixel hit counts for the whole image (binned if opts->tile > 0). hit_count[H*W]. */
+int mso_hit_counts(const mso_scene *, const mso_camera *, int H, int W, const mso_opts *,
+                   int32_t *hit_count);
+
+/* Intervals of one pixel, sorted by primitive id: prim, t_in, delta = (t_out - t_in)/K. */
+int mso_ray_intervals(const mso_scene *, const mso_camera *, int H, int W, const mso_opts *,
+                      int32_t pixel, int32_t *prim, float *t_in, float *delta,
+                      size_t cap, size_t *n);
+
+/* All samples of one pixel in compositing order (not truncated by early termination). */
+int mso_ray_samples(const mso_scene *, const mso_camera *, int H, int W, const mso_opts *,
+                    int32_t pixel, int32_t *prim, int32_t *k, float *t,
+                    size_t cap, size_t *n);
+
+/* ---- pieces exposed so tests can pin them one by one ---- */
+
+/* world->unit-sphere frame A = diag(1/s) R^T and its inverse-ish M = R diag(s), both [n][9]. */
+int mso_prim_frames(const mso_scene *, float *A, float *M);
+/* ray of pixel (x, y): origin o[3], unit direction d[3]. */
+int mso_ray(const mso_camera *, int x, int y, float *o, float *d);
+/* screen-space AABB of one primitive: rect = {px0, px1, py0, py1} inclusive; *visible = 0 if culled. */
+int mso_project(const mso_scene *, const mso_camera *, int H, int W, int32_t prim,
+                int32_t *visible, int32_t *rect, float *z_entry);
+/* MLP of one primitive at local coordinate u (and world direction d): raw[out_dim] and
+ * act[out_dim] = (sigmoid rgb, softplus sigma, linear features). */
+int mso_mlp_eval(const mso_scene *, int32_t prim, const float *u, const float *d,
+                 double *raw, double *act);
+/* encoded input vector x[in_dim] for (u, d). */
+int mso_encode(const mso_scene *, const float *u, const float *d, double *x);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
