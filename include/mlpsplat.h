@@ -1,0 +1,161 @@
+/* mlpsplat.h -- C ABI of the B200-native MLP-Splatting forward render
+ * (arxiv/paper_2606_03877; BASELINE.json north_star = NS).  P:NN = PAPER.md line NN.
+ *
+ * The library renders a scene of N spatially bounded primitives, each an independent
+ * compact MLP (Sec.3 / 3.1): per camera ray it finds the ray/ellipsoid support
+ * intervals, takes K midpoint samples in each, evaluates the hit primitive's own MLP at
+ * every sample (positional encoding P:101 Eq.5 -> Linear+ReLU -> rgb = sigmoid,
+ * sigma = softplus P:105) and alpha-composites all samples of the ray front to back,
+ * alpha = 1 - exp(-sigma*delta), C = sum_j T_j alpha_j c_j (Eq.6
+ * Eq.14), stopping once T < t_stop.  Stages (NS (a)-(e)): projection + tile keys,
+ * device radix sort, per-tile intersection, grouped per-primitive MLP (fp32 SIMT or bf16
+ * tcgen05 tensor cores), per-ray merge + composite.  DESIGN.md Sec.1 lists every reading
+ * of the paper this ABI fixes (Q1-Q27); Sec.2 the canonical fp32 order of the geometry.
+ *
+ * Conventions
+ *  - Every function returns MS_OK (0) or a negative MS_ERR_*; nothing aborts, throws or prints.
+ *  - "host" / "device" on a pointer says where the memory lives.  Inputs of ms_scene_create
+ *    are host pointers and are copied; the caller keeps ownership.  Render outputs are
+ *    DEVICE pointers owned by the caller (ms_render_host: host pointers).
+ *  - One CUDA device (the current one at ms_scene_create); there is no CPU fallback.
+ *  - A scene handle is not thread-safe; use one handle per host thread / stream.
+ */
+#ifndef MLPSPLAT_H
+#define MLPSPLAT_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  MS_OK = 0,
+  MS_ERR_INVALID_ARG = -1,       /* NULL / out-of-range argument, zero quaternion, scale <= 0 */
+  MS_ERR_OUT_OF_MEMORY = -2,     /* host or device allocation failed */
+  MS_ERR_CUDA = -3,              /* a CUDA call or kernel failed (ms_error_string has no detail; see ms_last_cuda_error) */
+  MS_ERR_UNSUPPORTED_SHAPE = -4, /* MLP shape / key width outside what the kernels cover */
+  MS_ERR_CAPACITY = -5           /* a caller-provided debug buffer is too small (*n holds the need) */
+};
+
+typedef struct ms_scene ms_scene; /* opaque; owns every device allocation it makes */
+
+/* Primitive parameterisation: centre mu, unit quaternion q, ellipsoid semi-axes s.
+ * The support of primitive i is { x : |x - mu|^2_Lambda <= 1 }, Lambda = R(q) diag(s^2)^-1 R(q)^T
+ * (Q5). */
+typedef struct {
+  int32_t n;           /* number of primitives, >= 1 */
+  const float *center; /* host [n][3] */
+  const float *quat;   /* host [n][4], order (w,x,y,z), Hamilton; normalised by the library (Q6) */
+  const float *scale;  /* host [n][3], semi-axes > 0 */
+} ms_prims;
+
+enum { MS_F32 = 0, MS_BF16 = 1 };
+
+/* One MLP per primitive, all of the same shape.  Input (Q2,Q3,Q15):
+ *   x = [u, sin(2^0 pi u), cos(2^0 pi u), ..., sin(2^(L-1) pi u), cos(2^(L-1) pi u)] [, d]
+ * u = local coordinate of the sample in the primitive's unit-sphere frame (3 values; each
+ * sin/cos block is 3 wide: x,y,z), d = unit world-frame ray direction.  in_dim = 3 + 6L (+3).
+ * n_hidden x (Linear(width) + ReLU), then Linear(4 + n_feat): outputs [r,g,b,sigma,feat...];
+ * rgb = sigmoid, sigma = softplus, feat linear (Q16).
+ * weights: host float32 [n][P]; per primitive, for each layer in order: W[in][out] row-major
+ * (input index slowest), then b[out].  P = sum(in*out + out).
+ * dtype = MS_BF16 declares that the contractions run with bf16 operands on tensor cores:
+ * weight matrices are rounded to bf16 (round-to-nearest-even; a no-op if already
+ * representable), biases stay fp32 (Q18).  dtype = MS_F32 keeps everything fp32. */
+typedef struct {
+  int32_t n_freq;      /* L >= 0 */
+  int32_t use_viewdir; /* 0 / 1 */
+  int32_t n_hidden;    /* 1..4 */
+  int32_t width;       /* hidden width, 1..128 (tensor path: 64 or 128) */
+  int32_t n_feat;      /* 0..60 */
+  int32_t dtype;       /* MS_F32 | MS_BF16 */
+  const float *weights;
+  size_t n_weights;    /* must equal n * P */
+} ms_mlp;
+
+/* Pinhole camera (Q14): pixel (x,y), row 0 on top, looks along
+ * d_cam = ((x+0.5-cx)/fx, (y+0.5-cy)/fy, 1); c2w = 3x4 row-major [R|t], camera axes
+ * x right, y down, z forward; the ray is o = t, d = normalise(R d_cam). */
+typedef struct {
+  float fx, fy, cx, cy;
+  float c2w[12];
+  float t_near; /* >= 0; intervals are clipped to t >= t_near (Q13) */
+} ms_camera;
+
+enum { MS_PATH_AUTO = 0, MS_PATH_FP32 = 1, MS_PATH_BF16_TC = 2 };
+enum {
+  MS_FLAG_KEEP_DEBUG = 1, /* keep the intermediate buffers of the last view for ms_debug_* */
+  MS_FLAG_STAGE_TIMES = 2 /* record CUDA events between stages (ms_last_stage_ms) */
+};
+
+typedef struct {
+  int32_t K;      /* midpoint samples per interval, 1..64 (NS (c)) */
+  float t_stop;   /* early termination threshold on T (NS (e): 1e-4); 0 disables */
+  int32_t tile;   /* tile edge in pixels: 8, 16 or 32; 0 = default 16 (Q10) */
+  int32_t path;   /* MS_PATH_*; AUTO = BF16_TC when dtype is MS_BF16 and the shape is covered, else FP32 */
+  void *stream;   /* cudaStream_t to enqueue on; NULL = the legacy default stream */
+  int32_t flags;  /* MS_FLAG_* */
+} ms_opts;
+
+typedef struct {
+  int64_t n_visible;   /* primitives with a non-empty screen AABB */
+  int64_t n_pairs;     /* (tile, primitive) keys */
+  int64_t n_intervals; /* (ray, primitive) hits */
+  int64_t n_samples;   /* n_intervals * K = MLP evaluations */
+  int64_t n_blocks;    /* 128-sample row blocks fed to the MLP stage */
+  int64_t scratch_bytes;
+} ms_stats;
+
+enum { MS_STAGE_BIN = 0, MS_STAGE_SORT, MS_STAGE_ISECT, MS_STAGE_MLP, MS_STAGE_COMPOSITE, MS_N_STAGES };
+
+/* Builds the device-resident scene: uploads primitives, derives per primitive (in canonical
+ * fp32) A = diag(1/s) R^T and M = R diag(s), and packs the weights for the
+ * MLP kernels.  Synchronises the device. */
+int ms_scene_create(const ms_prims *prims, const ms_mlp *mlp, ms_scene **out);
+int ms_scene_destroy(ms_scene *scene);
+
+/* Renders one view into DEVICE buffers out_rgb [H][W][3], out_alpha [H][W] and, if the MLP has
+ * n_feat > 0 and out_feat != NULL, out_feat [H][W][n_feat]; all float32.  rgb / feat are
+ * premultiplied sums (no background term, Q14); alpha = 1 - T.  Work is enqueued on
+ * opts->stream; the call synchronises that stream twice internally to size its scratch
+ * buffers (pair and interval counts), not at the end: outputs are ready once the stream is. */
+int ms_render(ms_scene *scene, const ms_camera *camera, int32_t H, int32_t W, const ms_opts *opts,
+              float *out_rgb, float *out_alpha, float *out_feat);
+
+/* n_views cameras (host array), outputs [n_views][H][W][...] (CFG5: 8 poses). */
+int ms_render_batch(ms_scene *scene, const ms_camera *cameras, int32_t n_views, int32_t H, int32_t W,
+                    const ms_opts *opts, float *out_rgb, float *out_alpha, float *out_feat);
+
+/* Same as ms_render_batch with HOST output buffers (pinned or pageable): renders into
+ * library-owned device buffers, copies the results back and synchronises the stream. */
+int ms_render_host(ms_scene *scene, const ms_camera *cameras, int32_t n_views, int32_t H, int32_t W,
+                   const ms_opts *opts, float *host_rgb, float *host_alpha, float *host_feat);
+
+/* Counts of the last view rendered on this scene (valid once the stream is idle). */
+int ms_last_stats(ms_scene *scene, ms_stats *out);
+/* Device time of each stage of the last view rendered with MS_FLAG_STAGE_TIMES, in ms,
+ * ms[MS_N_STAGES].  Synchronises the recorded events. */
+int ms_last_stage_ms(ms_scene *scene, float *ms);
+
+/* ---- parity introspection: valid after a render with MS_FLAG_KEEP_DEBUG (last view) ---- */
+/* Sorted tile lists: tile_offsets host [tiles+1], prim_ids / zbits host [cap]. */
+int ms_debug_tile_lists(ms_scene *scene, int64_t *tile_offsets, int32_t *prim_ids, uint32_t *zbits,
+                        size_t cap, size_t *n);
+/* Per-ray hit lists in tile-list order: hit_offsets host [H*W+1]; prim / t_in / delta host [cap]. */
+int ms_debug_intervals(ms_scene *scene, int64_t *hit_offsets, int32_t *prim, float *t_in, float *delta,
+                       size_t cap, size_t *n);
+/* Compositing order of one ray (all samples, not truncated): prim / k / t host [cap]. */
+int ms_debug_sample_order(ms_scene *scene, int32_t ray, int32_t *prim, int32_t *k, float *t,
+                          size_t cap, size_t *n);
+/* Derived per-primitive frames, host [n][9] each (row-major A, M). */
+int ms_debug_prim_frames(ms_scene *scene, float *A, float *M);
+
+const char *ms_error_string(int code);
+/* cudaError_t of the last failing CUDA call on this scene (0 if none). */
+int ms_last_cuda_error(ms_scene *scene);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

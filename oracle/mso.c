@@ -633,3 +633,35 @@ int mso_ray_samples(const mso_scene *s, const mso_camera *cam, int H, int W, con
   raybuf_free(&rb);
   return MSO_OK;
 }
+
+/* Intervals of every pixel (each ray's list sorted by primitive id): offsets[H*W+1]. */
+int mso_intervals_all(const mso_scene *s, const mso_camera *cam, int H, int W, const mso_opts *opt,
+                      int64_t *offsets, int32_t *prim, float *t_in, float *delta, size_t cap, size_t *n) {
+  if (!s || !cam || !opt || !offsets || opt->K <= 0) return MSO_ERR_ARG;
+  tlists_t tl; memset(&tl, 0, sizeof(tl));
+  if (opt->tile > 0) { int rc = tlists_build(s, cam, H, W, opt->tile, &tl); if (rc) return rc; }
+  const tlists_t *tlp = opt->tile > 0 ? &tl : NULL;
+  raybuf_t rb; memset(&rb, 0, sizeof(rb));
+  size_t tot = 0;
+  int rc = MSO_OK;
+  for (int64_t q = 0; q < (int64_t)H * W; ++q) {
+    float o[3], d[3];
+    offsets[q] = (int64_t)tot;
+    long nh = gather_hits(s, cam, tlp, opt->tile, W, (int)q, opt->K, o, d, &rb);
+    if (nh < 0) { rc = MSO_ERR_MEM; break; }
+    qsort(rb.hits, (size_t)nh, sizeof(hit_t), hit_cmp_prim);
+    for (long j = 0; j < nh; ++j, ++tot) {
+      if (tot < cap) {
+        if (prim) prim[tot] = rb.hits[j].prim;
+        if (t_in) t_in[tot] = rb.hits[j].t_in;
+        if (delta) delta[tot] = rb.hits[j].delta;
+      }
+    }
+  }
+  offsets[(int64_t)H * W] = (int64_t)tot;
+  if (n) *n = tot;
+  raybuf_free(&rb);
+  tlists_free(&tl);
+  if (rc == MSO_OK && tot > cap) rc = MSO_ERR_CAP;
+  return rc;
+}

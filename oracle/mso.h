@@ -112,6 +112,12 @@ int mso_ray_intervals(const mso_scene *, const mso_camera *, int H, int W, const
                       int32_t pixel, int32_t *prim, float *t_in, float *delta,
                       size_t cap, size_t *n);
 
+/* Intervals of every pixel (each ray's list sorted by primitive id): offsets[H*W+1].
+ * Call with cap = 0 to size (*n), then again. */
+int mso_intervals_all(const mso_scene *, const mso_camera *, int H, int W, const mso_opts *,
+                      int64_t *offsets, int32_t *prim, float *t_in, float *delta,
+                      size_t cap, size_t *n);
+
 /* All samples of one pixel in compositing order (not truncated by early termination). */
 int mso_ray_samples(const mso_scene *, const mso_camera *, int H, int W, const mso_opts *,
                     int32_t pixel, int32_t *prim, int32_t *k, float *t,

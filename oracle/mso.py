@@ -164,6 +164,25 @@ class OracleScene:
             raise RuntimeError(f"mso_ray_intervals failed: {rc}")
         return prim[:n.value], t_in[:n.value], delta[:n.value]
 
+    def intervals_all(self, cam, H, W, K, tile=16):
+        """(offsets[H*W+1], prim, t_in, delta), each ray's hits sorted by primitive id."""
+        off = np.zeros(H * W + 1, np.int64)
+        n = C.c_size_t(0)
+        o = _Opts(K, 1e-4, tile, 1)
+        c = _cam(cam)
+        rc = lib().mso_intervals_all(self._h, C.byref(c), H, W, C.byref(o), _ptr(off), None, None,
+                                     None, C.c_size_t(0), C.byref(n))
+        if rc not in (0, -3):
+            raise RuntimeError(f"mso_intervals_all failed: {rc}")
+        prim = np.zeros(max(n.value, 1), np.int32)
+        t_in = np.zeros(max(n.value, 1), np.float32)
+        delta = np.zeros(max(n.value, 1), np.float32)
+        rc = lib().mso_intervals_all(self._h, C.byref(c), H, W, C.byref(o), _ptr(off), _ptr(prim),
+                                     _ptr(t_in), _ptr(delta), C.c_size_t(prim.size), C.byref(n))
+        if rc != 0:
+            raise RuntimeError(f"mso_intervals_all failed: {rc}")
+        return off, prim[:n.value], t_in[:n.value], delta[:n.value]
+
     def ray_samples(self, cam, H, W, K, pixel, tile=16):
         cap = self.n * K
         prim = np.zeros(cap, np.int32)

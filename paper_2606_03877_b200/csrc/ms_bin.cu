@@ -1,0 +1,187 @@
+// ms_bin.cu -- scene prep and stage (a): projection of each ellipsoid support to a
+// conservative screen-space AABB and emission of (tile | z_entry | prim) keys
+// ("conservative overlap tests based on their projected support regions";
+//  P:148 "AABB-tile-frustum intersection test"; NS (a)).  All arithmetic is the canonical
+// fp32 sequence of DESIGN.md Sec.2.  Bytes: N*(3+9+9)*4 in, P*8 out -- negligible.
+#include "ms_internal.cuh"
+
+namespace {
+
+// P:74 / P:84: q -> R (Hamilton, (w,x,y,z)); A = diag(1/s) R^T; M = R diag(s)
+__global__ void prep_prims_kernel(int n, const float *__restrict__ quat, const float *__restrict__ scale,
+                                  float *__restrict__ A, float *__restrict__ M, int *__restrict__ bad) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  float w = quat[4 * i], x = quat[4 * i + 1], y = quat[4 * i + 2], z = quat[4 * i + 3];
+  float s0 = scale[3 * i], s1 = scale[3 * i + 1], s2 = scale[3 * i + 2];
+  float n2 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(w, w), __fmul_rn(x, x)), __fmul_rn(y, y)), __fmul_rn(z, z));
+  if (!(n2 > 0.0f) || isinf(n2) || !(s0 > 0.0f) || !(s1 > 0.0f) || !(s2 > 0.0f)) {
+    atomicExch(bad, 1);
+    return;
+  }
+  float nrm = __fsqrt_rn(n2);
+  w = __fdiv_rn(w, nrm); x = __fdiv_rn(x, nrm); y = __fdiv_rn(y, nrm); z = __fdiv_rn(z, nrm);
+  float xx = __fmul_rn(x, x), yy = __fmul_rn(y, y), zz = __fmul_rn(z, z);
+  float xy = __fmul_rn(x, y), xz = __fmul_rn(x, z), yz = __fmul_rn(y, z);
+  float wx = __fmul_rn(w, x), wy = __fmul_rn(w, y), wz = __fmul_rn(w, z);
+  float R[9];
+  R[0] = __fsub_rn(1.0f, __fmul_rn(2.0f, __fadd_rn(yy, zz)));
+  R[1] = __fmul_rn(2.0f, __fsub_rn(xy, wz));
+  R[2] = __fmul_rn(2.0f, __fadd_rn(xz, wy));
+  R[3] = __fmul_rn(2.0f, __fadd_rn(xy, wz));
+  R[4] = __fsub_rn(1.0f, __fmul_rn(2.0f, __fadd_rn(xx, zz)));
+  R[5] = __fmul_rn(2.0f, __fsub_rn(yz, wx));
+  R[6] = __fmul_rn(2.0f, __fsub_rn(xz, wy));
+  R[7] = __fmul_rn(2.0f, __fadd_rn(yz, wx));
+  R[8] = __fsub_rn(1.0f, __fmul_rn(2.0f, __fadd_rn(xx, yy)));
+  float s[3] = {s0, s1, s2};
+#pragma unroll
+  for (int r = 0; r < 3; ++r)
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      A[9 * i + 3 * r + c] = __fdiv_rn(R[3 * c + r], s[r]);
+      M[9 * i + 3 * r + c] = __fmul_rn(R[3 * r + c], s[c]);
+    }
+}
+
+__device__ __forceinline__ void axis_bounds(const float *rx, float cxv, const float *rz, float czv, float zz,
+                                            float focal, float centre, float *lo, float *hi) {
+  float xz = __fsub_rn(ms_dot3(rx[0], rx[1], rx[2], rz[0], rz[1], rz[2]), __fmul_rn(cxv, czv));
+  float xx = __fsub_rn(ms_dot3(rx[0], rx[1], rx[2], rx[0], rx[1], rx[2]), __fmul_rn(cxv, cxv));
+  float m = __fdiv_rn(xz, zz);
+  float q = __fsub_rn(__fmul_rn(m, m), __fdiv_rn(xx, zz));
+  float h = __fsqrt_rn(q > 0.0f ? q : 0.0f);
+  *lo = __fadd_rn(__fmul_rn(focal, __fsub_rn(m, h)), centre);
+  *hi = __fadd_rn(__fmul_rn(focal, __fadd_rn(m, h)), centre);
+}
+
+__device__ __forceinline__ int clamp_lo(float v, int n) {
+  float f = floorf(v);
+  if (!(f > 0.0f)) return 0;
+  if (f > (float)n) return n;
+  return (int)f;
+}
+__device__ __forceinline__ int clamp_hi(float v, int n) {
+  float f = ceilf(v);
+  if (!(f < (float)(n - 1))) return n - 1;
+  if (f < 0.0f) return -1;
+  return (int)f;
+}
+
+__global__ void project_kernel(int n, const float *__restrict__ center, const float *__restrict__ A,
+                               const float *__restrict__ M, MsCam cam, int tile, uint32_t *__restrict__ tile_count,
+                               int4 *__restrict__ rect, float *__restrict__ z_entry, float *__restrict__ oprime) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const float *mu = center + 3 * i;
+  const float *Mi = M + 9 * i;
+  const float *Ai = A + 9 * i;
+  // o' = A (o - mu), reused by every ray of this view (stage (c))
+  {
+    float v0 = __fsub_rn(cam.o[0], mu[0]), v1 = __fsub_rn(cam.o[1], mu[1]), v2 = __fsub_rn(cam.o[2], mu[2]);
+    oprime[3 * i + 0] = ms_dot3(Ai[0], Ai[1], Ai[2], v0, v1, v2);
+    oprime[3 * i + 1] = ms_dot3(Ai[3], Ai[4], Ai[5], v0, v1, v2);
+    oprime[3 * i + 2] = ms_dot3(Ai[6], Ai[7], Ai[8], v0, v1, v2);
+  }
+  float v0 = __fsub_rn(mu[0], cam.o[0]), v1 = __fsub_rn(mu[1], cam.o[1]), v2 = __fsub_rn(mu[2], cam.o[2]);
+  const float *r = cam.r;
+  float cv[3], Mc[9];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    cv[a] = ms_dot3(r[a], r[3 + a], r[6 + a], v0, v1, v2);
+#pragma unroll
+    for (int j = 0; j < 3; ++j) Mc[3 * a + j] = ms_dot3(r[a], r[3 + a], r[6 + a], Mi[j], Mi[3 + j], Mi[6 + j]);
+  }
+  float rz2 = ms_dot3(Mc[6], Mc[7], Mc[8], Mc[6], Mc[7], Mc[8]);
+  float rz = __fsqrt_rn(rz2);
+  float z_lo = __fsub_rn(cv[2], rz);
+  float z_hi = __fadd_rn(cv[2], rz);
+  int4 rc = make_int4(0, 0, -1, -1);
+  uint32_t cnt = 0;
+  float ze = 0.0f;
+  if (z_hi > 0.0f) {
+    ze = z_lo > 0.0f ? z_lo : 0.0f;
+    int px0, px1, py0, py1;
+    if (z_lo <= __fmul_rn(0.01f, rz)) {
+      px0 = 0; px1 = cam.W - 1; py0 = 0; py1 = cam.H - 1;
+    } else {
+      float zz = __fsub_rn(rz2, __fmul_rn(cv[2], cv[2]));
+      float xl, xh, yl, yh;
+      axis_bounds(Mc, cv[0], Mc + 6, cv[2], zz, cam.fx, cam.cx, &xl, &xh);
+      axis_bounds(Mc + 3, cv[1], Mc + 6, cv[2], zz, cam.fy, cam.cy, &yl, &yh);
+      px0 = clamp_lo(__fsub_rn(xl, 0.5f), cam.W);
+      px1 = clamp_hi(__fsub_rn(xh, 0.5f), cam.W);
+      py0 = clamp_lo(__fsub_rn(yl, 0.5f), cam.H);
+      py1 = clamp_hi(__fsub_rn(yh, 0.5f), cam.H);
+    }
+    if (px0 <= px1 && py0 <= py1) {
+      rc = make_int4(px0 / tile, py0 / tile, px1 / tile, py1 / tile);
+      cnt = (uint32_t)(rc.z - rc.x + 1) * (uint32_t)(rc.w - rc.y + 1);
+    }
+  }
+  tile_count[i] = cnt;
+  rect[i] = rc;
+  z_entry[i] = ze;
+}
+
+// one warp per primitive; emission order: tile rows, then columns (row-major inside the rect)
+__global__ void emit_keys_kernel(int n, const uint32_t *__restrict__ emit_off, const int4 *__restrict__ rect,
+                                 const float *__restrict__ z_entry, int tiles_x, int prim_bits,
+                                 uint64_t *__restrict__ keys) {
+  int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  int lane = threadIdx.x & 31;
+  if (i >= n) return;
+  uint32_t beg = emit_off[i], cnt = emit_off[i + 1] - beg;
+  if (cnt == 0) return;
+  int4 rc = rect[i];
+  int tw = rc.z - rc.x + 1;
+  uint64_t low = ((uint64_t)__float_as_uint(z_entry[i]) << prim_bits) | (uint64_t)(uint32_t)i;
+  for (uint32_t j = lane; j < cnt; j += 32) {
+    int ty = rc.y + (int)(j / (uint32_t)tw), tx = rc.x + (int)(j % (uint32_t)tw);
+    uint64_t t = (uint64_t)(uint32_t)(ty * tiles_x + tx);
+    keys[beg + j] = (t << (32 + prim_bits)) | low;
+  }
+}
+
+__global__ void tile_ranges_kernel(const uint64_t *__restrict__ keys, uint32_t n_pairs, int n_tiles, int shift,
+                                   uint32_t *__restrict__ tile_start) {
+  uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_pairs) return;
+  int t = (int)(keys[i] >> shift);
+  int prev = i == 0 ? -1 : (int)(keys[i - 1] >> shift);
+  for (int u = prev + 1; u <= t; ++u) tile_start[u] = i;
+  if (i == n_pairs - 1)
+    for (int u = t + 1; u <= n_tiles; ++u) tile_start[u] = n_pairs;
+}
+
+}  // namespace
+
+cudaError_t ms_prep_prims(int n, const float *center, const float *quat, const float *scale, float *A, float *M,
+                          int *bad, cudaStream_t s) {
+  (void)center;
+  prep_prims_kernel<<<(n + 127) / 128, 128, 0, s>>>(n, quat, scale, A, M, bad);
+  return cudaGetLastError();
+}
+
+cudaError_t ms_project(int n, const float *center, const float *A, const float *M, MsCam cam, int tile, int tiles_x,
+                       int tiles_y, uint32_t *tile_count, int4 *rect, float *z_entry, float *oprime, cudaStream_t s) {
+  (void)tiles_x; (void)tiles_y;
+  project_kernel<<<(n + 127) / 128, 128, 0, s>>>(n, center, A, M, cam, tile, tile_count, rect, z_entry, oprime);
+  return cudaGetLastError();
+}
+
+cudaError_t ms_emit_keys(int n, const uint32_t *emit_off, const int4 *rect, const float *z_entry, int tiles_x,
+                         int prim_bits, uint64_t *keys, cudaStream_t s) {
+  long threads = (long)n * 32;
+  emit_keys_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, s>>>(n, emit_off, rect, z_entry, tiles_x, prim_bits,
+                                                                    keys);
+  return cudaGetLastError();
+}
+
+cudaError_t ms_tile_ranges(const uint64_t *keys, size_t n_pairs, int n_tiles, int prim_bits, uint32_t *tile_start,
+                           cudaStream_t s) {
+  if (n_pairs == 0) return cudaMemsetAsync(tile_start, 0, (size_t)(n_tiles + 1) * sizeof(uint32_t), s);
+  tile_ranges_kernel<<<(unsigned)((n_pairs + 255) / 256), 256, 0, s>>>(keys, (uint32_t)n_pairs, n_tiles,
+                                                                      32 + prim_bits, tile_start);
+  return cudaGetLastError();
+}

@@ -1,0 +1,182 @@
+// ms_internal.cuh -- shared declarations of the CUDA path (never included by oracle/).
+// Canonical fp32 geometry: every operation below is an explicit
+// round-to-nearest intrinsic, so nvcc can never contract a multiply and an add into an FMA.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/mlpsplat.h"
+
+#define MS_MAX_WIDTH 128
+#define MS_MAX_IN 64
+#define MS_MAX_OUT 64
+#define MS_MAX_K 64
+#define MS_ROWS 128  // samples per MLP row block (one TMEM lane / one thread per sample)
+
+struct MsCam {
+  float fx, fy, cx, cy;
+  float r[9];  // c2w rotation, row-major
+  float o[3];  // eye
+  float t_near;
+  int W, H;
+};
+
+// interval of one (ray, primitive) hit in the primitive-major list consumed by stage (d)
+struct __align__(16) MsInterval {
+  int ray;      // y*W + x
+  float t_in;
+  float delta;  // (t_out - t_in)/K
+  int slot;     // global hit index = ray_off[ray] + h ; sample k lives at staging[slot*K + k]
+  float dx, dy, dz;  // unit world-frame ray direction (canonical)
+  int pad;
+};
+
+// hit of one ray (ray-major list consumed by stage (e))
+struct __align__(16) MsHit {
+  int prim;
+  float t_in;
+  float delta;
+  int pad;
+};
+
+struct MsMlpShape {
+  int n_freq, use_viewdir, n_hidden, width, n_feat;
+  int in_dim, out_dim, n_layers, params;
+};
+
+// ---------------------------------------------------------------------------------------------
+// canonical fp32 primitives
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ float ms_dot3(float a0, float a1, float a2, float b0, float b1, float b2) {
+  return __fadd_rn(__fadd_rn(__fmul_rn(a0, b0), __fmul_rn(a1, b1)), __fmul_rn(a2, b2));
+}
+
+__device__ __forceinline__ void ms_camera_ray(const MsCam &c, int x, int y, float *d) {
+  float px = __fadd_rn((float)x, 0.5f);
+  float py = __fadd_rn((float)y, 0.5f);
+  float dcx = __fdiv_rn(__fsub_rn(px, c.cx), c.fx);
+  float dcy = __fdiv_rn(__fsub_rn(py, c.cy), c.fy);
+  float wx = __fadd_rn(__fadd_rn(__fmul_rn(c.r[0], dcx), __fmul_rn(c.r[1], dcy)), c.r[2]);
+  float wy = __fadd_rn(__fadd_rn(__fmul_rn(c.r[3], dcx), __fmul_rn(c.r[4], dcy)), c.r[5]);
+  float wz = __fadd_rn(__fadd_rn(__fmul_rn(c.r[6], dcx), __fmul_rn(c.r[7], dcy)), c.r[8]);
+  float n2 = __fadd_rn(__fadd_rn(__fmul_rn(wx, wx), __fmul_rn(wy, wy)), __fmul_rn(wz, wz));
+  float nrm = __fsqrt_rn(n2);
+  d[0] = __fdiv_rn(wx, nrm);
+  d[1] = __fdiv_rn(wy, nrm);
+  d[2] = __fdiv_rn(wz, nrm);
+}
+
+// ray / ellipsoid chord in the unit-sphere frame; op = A (o - mu) is per primitive per view.
+__device__ __forceinline__ bool ms_intersect(const float *A, const float *op, const float *d, float t_near,
+                                             float Kf, float *t_in, float *delta) {
+  float d0 = ms_dot3(A[0], A[1], A[2], d[0], d[1], d[2]);
+  float d1 = ms_dot3(A[3], A[4], A[5], d[0], d[1], d[2]);
+  float d2 = ms_dot3(A[6], A[7], A[8], d[0], d[1], d[2]);
+  float a = ms_dot3(d0, d1, d2, d0, d1, d2);
+  float b = ms_dot3(op[0], op[1], op[2], d0, d1, d2);
+  float c = __fsub_rn(ms_dot3(op[0], op[1], op[2], op[0], op[1], op[2]), 1.0f);
+  float disc = __fsub_rn(__fmul_rn(b, b), __fmul_rn(a, c));
+  if (!(disc > 0.0f)) return false;
+  float sq = __fsqrt_rn(disc);
+  float nb = -b;
+  float t0 = __fdiv_rn(__fsub_rn(nb, sq), a);
+  float t1 = __fdiv_rn(__fadd_rn(nb, sq), a);
+  if (!(t1 > t_near)) return false;
+  float ti = t0 > t_near ? t0 : t_near;
+  float dl = __fdiv_rn(__fsub_rn(t1, ti), Kf);
+  if (!(dl > 0.0f)) return false;
+  *t_in = ti;
+  *delta = dl;
+  return true;
+}
+
+__device__ __forceinline__ float ms_sample_t(float t_in, float delta, int k) {
+  float kf = __fadd_rn((float)k, 0.5f);
+  return __fadd_rn(t_in, __fmul_rn(kf, delta));
+}
+
+// u = A ((o + t d) - mu)
+__device__ __forceinline__ void ms_sample_u(const float *A, const float *mu, const float *o, const float *d,
+                                            float t, float *u) {
+  float w0 = __fsub_rn(__fadd_rn(o[0], __fmul_rn(t, d[0])), mu[0]);
+  float w1 = __fsub_rn(__fadd_rn(o[1], __fmul_rn(t, d[1])), mu[1]);
+  float w2 = __fsub_rn(__fadd_rn(o[2], __fmul_rn(t, d[2])), mu[2]);
+  u[0] = ms_dot3(A[0], A[1], A[2], w0, w1, w2);
+  u[1] = ms_dot3(A[3], A[4], A[5], w0, w1, w2);
+  u[2] = ms_dot3(A[6], A[7], A[8], w0, w1, w2);
+}
+
+// ---------------------------------------------------------------------------------------------
+// host-side launchers (one per stage file)
+// ---------------------------------------------------------------------------------------------
+// ms_scan.cu: out[i] = sum_{j<i} in[j] for i in [0, n]; out has n+1 entries. scratch >= ms_scan_scratch_elems(n).
+size_t ms_scan_scratch_elems(size_t n);
+cudaError_t ms_exclusive_scan_u32(const uint32_t *in, uint32_t *out, size_t n, uint32_t *scratch, cudaStream_t s);
+
+// ms_sort.cu: LSD radix sort of 64-bit keys on bits [0, n_bits). Result ends in *result (either a or b).
+size_t ms_sort_scratch_elems(size_t n);
+cudaError_t ms_radix_sort_u64(uint64_t *a, uint64_t *b, size_t n, int n_bits, uint32_t *scratch,
+                              uint64_t **result, cudaStream_t s);
+
+// ms_bin.cu
+cudaError_t ms_prep_prims(int n, const float *center, const float *quat, const float *scale, float *A, float *M,
+                          int *bad, cudaStream_t s);
+cudaError_t ms_project(int n, const float *center, const float *A, const float *M, MsCam cam, int tile,
+                       int tiles_x, int tiles_y, uint32_t *tile_count, int4 *rect, float *z_entry, float *oprime,
+                       cudaStream_t s);
+cudaError_t ms_emit_keys(int n, const uint32_t *emit_off, const int4 *rect, const float *z_entry, int tiles_x,
+                         int prim_bits, uint64_t *keys, cudaStream_t s);
+cudaError_t ms_tile_ranges(const uint64_t *keys, size_t n_pairs, int n_tiles, int prim_bits, uint32_t *tile_start,
+                           cudaStream_t s);
+
+// ms_isect.cu
+struct MsIsectArgs {
+  MsCam cam;
+  int tile, tiles_x, n_tiles, K, prim_bits;
+  const uint64_t *keys;        // sorted
+  const uint32_t *tile_start;  // [n_tiles+1]
+  const float *A;              // [N][9]
+  const float *oprime;         // [N][3]
+  const int4 *rect;            // [N] tile rect (tx0, ty0, tx1, ty1)
+  const uint32_t *emit_off;    // [N+1]
+  uint32_t *pair_hits;         // [P]   (count pass: out)   indexed by emission index
+  uint32_t *ray_hits;          // [R]   (count pass: out)
+  const uint32_t *pair_off;    // [P+1] (fill pass: in)
+  const uint32_t *ray_off;     // [R+1] (fill pass: in)
+  MsInterval *intervals;       // [n_hits] primitive-major (fill pass: out)
+  MsHit *hits;                 // [n_hits] ray-major       (fill pass: out)
+};
+cudaError_t ms_isect_count(const MsIsectArgs &a, cudaStream_t s);
+cudaError_t ms_isect_fill(const MsIsectArgs &a, cudaStream_t s);
+// per-primitive interval starts and 128-row block counts
+cudaError_t ms_prim_blocks(int n, const uint32_t *emit_off, const uint32_t *pair_off, int K, uint32_t *prim_start,
+                           uint32_t *prim_blocks, cudaStream_t s);
+
+// ms_mlp_f32.cu
+struct MsMlpArgs {
+  MsMlpShape shape;
+  MsCam cam;
+  int K, n_prims;
+  const float *center, *A;
+  const float *weights_f32;       // [N][params]
+  const uint32_t *prim_start;     // [N+1] interval offsets
+  const uint32_t *blk_off;        // [N+1] row-block offsets
+  uint32_t n_blocks;
+  const MsInterval *intervals;
+  float4 *staging;                // [n_hits*K] (r,g,b,e)
+  float *staging_feat;            // [n_hits*K][n_feat] or NULL
+};
+cudaError_t ms_mlp_f32(const MsMlpArgs &a, cudaStream_t s);
+
+// ms_composite.cu
+struct MsCompositeArgs {
+  int n_rays, K, n_feat;
+  float t_stop;
+  const uint32_t *ray_off;  // [R+1]
+  const MsHit *hits;
+  const float4 *staging;
+  const float *staging_feat;
+  float *cur_t;             // [n_hits] scratch
+  float *out_rgb, *out_alpha, *out_feat;
+};
+cudaError_t ms_composite(const MsCompositeArgs &a, cudaStream_t s);
+cudaError_t ms_sample_order(const MsCompositeArgs &a, int ray, int *prim, int *k, float *t, cudaStream_t s);

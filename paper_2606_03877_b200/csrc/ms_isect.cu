@@ -1,0 +1,106 @@
+// ms_isect.cu -- stage (c): per-tile ray/ellipsoid intersection (NS (c)).  One CTA per tile,
+// one thread per pixel; the CTA walks the tile's sorted list and every thread tests its ray
+// against the primitive (canonical fp32 chord).  Two passes:
+//   count: hits per ray and hits per (tile, primitive) pair
+//   fill : after two exclusive scans, each hit is written twice --
+//          ray-major   hits[ray_off[ray] + h]           (stage (e) merges these per ray)
+//          prim-major  intervals[pair_off[pair] + rank]  (stage (d) batches samples by primitive)
+// The prim-major order is (primitive, tile row-major inside its rect, pixel index in tile):
+// deterministic, no atomics.  Bytes: ~48 B written per hit; reads are L1/L2-resident lists.
+#include "ms_internal.cuh"
+
+namespace {
+
+template <bool FILL>
+__global__ void isect_kernel(MsIsectArgs a) {
+  __shared__ uint32_t wtot[2][32];
+  const int T = a.tile;
+  const int tile_id = blockIdx.x;
+  const int tile_x = tile_id % a.tiles_x, tile_y = tile_id / a.tiles_x;
+  const int lx = threadIdx.x % T, ly = threadIdx.x / T;
+  const int x = tile_x * T + lx, y = tile_y * T + ly;
+  const bool valid = x < a.cam.W && y < a.cam.H;
+  const int ray = y * a.cam.W + x;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int n_warps = (blockDim.x + 31) >> 5;
+  const uint32_t lt = (1u << lane) - 1u;
+  float d[3] = {0.f, 0.f, 1.f};
+  if (valid) ms_camera_ray(a.cam, x, y, d);
+  const float Kf = (float)a.K;
+  const uint64_t pmask = (1ull << a.prim_bits) - 1ull;
+  const uint32_t beg = a.tile_start[tile_id], end = a.tile_start[tile_id + 1];
+  uint32_t my_hits = 0;
+  uint32_t ray_base = 0;
+  if (FILL && valid) ray_base = a.ray_off[ray];
+  for (uint32_t j = beg; j < end; ++j) {
+    const int prim = (int)(a.keys[j] & pmask);
+    const float *A = a.A + 9 * (size_t)prim;
+    const float *op = a.oprime + 3 * (size_t)prim;
+    float Al[9], ol[3];
+#pragma unroll
+    for (int q = 0; q < 9; ++q) Al[q] = __ldg(A + q);
+#pragma unroll
+    for (int q = 0; q < 3; ++q) ol[q] = __ldg(op + q);
+    float t_in = 0.f, delta = 0.f;
+    const bool hit = valid && ms_intersect(Al, ol, d, a.cam.t_near, Kf, &t_in, &delta);
+    const int4 rc = a.rect[prim];
+    const uint32_t emit = a.emit_off[prim] + (uint32_t)((tile_y - rc.y) * (rc.z - rc.x + 1) + (tile_x - rc.x));
+    if (!FILL) {
+      const int cnt = __syncthreads_count(hit);
+      if (threadIdx.x == 0) a.pair_hits[emit] = (uint32_t)cnt;
+    } else {
+      const uint32_t ballot = __ballot_sync(0xffffffffu, hit);
+      const int buf = (int)(j & 1u);
+      if (lane == 0) wtot[buf][warp] = __popc(ballot);
+      __syncthreads();
+      if (hit) {
+        uint32_t rank = __popc(ballot & lt);
+        for (int w = 0; w < warp; ++w) rank += wtot[buf][w];
+        (void)n_warps;
+        const uint32_t slot = ray_base + my_hits;
+        MsInterval iv;
+        iv.ray = ray; iv.t_in = t_in; iv.delta = delta; iv.slot = (int)slot;
+        iv.dx = d[0]; iv.dy = d[1]; iv.dz = d[2]; iv.pad = 0;
+        a.intervals[a.pair_off[emit] + rank] = iv;
+        MsHit h;
+        h.prim = prim; h.t_in = t_in; h.delta = delta; h.pad = 0;
+        a.hits[slot] = h;
+      }
+    }
+    my_hits += hit ? 1u : 0u;
+  }
+  if (!FILL && valid) a.ray_hits[ray] = my_hits;
+}
+
+__global__ void prim_blocks_kernel(int n, const uint32_t *__restrict__ emit_off, const uint32_t *__restrict__ pair_off,
+                                   int K, uint32_t *__restrict__ prim_start, uint32_t *__restrict__ prim_blocks) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i > n) return;
+  uint32_t s = pair_off[emit_off[i]];
+  prim_start[i] = s;
+  if (i < n) {
+    uint32_t e = pair_off[emit_off[i + 1]];
+    uint64_t samples = (uint64_t)(e - s) * (uint64_t)K;
+    prim_blocks[i] = (uint32_t)((samples + MS_ROWS - 1) / MS_ROWS);
+  }
+}
+
+}  // namespace
+
+cudaError_t ms_isect_count(const MsIsectArgs &a, cudaStream_t s) {
+  if (a.n_tiles == 0) return cudaSuccess;
+  isect_kernel<false><<<a.n_tiles, a.tile * a.tile, 0, s>>>(a);
+  return cudaGetLastError();
+}
+
+cudaError_t ms_isect_fill(const MsIsectArgs &a, cudaStream_t s) {
+  if (a.n_tiles == 0) return cudaSuccess;
+  isect_kernel<true><<<a.n_tiles, a.tile * a.tile, 0, s>>>(a);
+  return cudaGetLastError();
+}
+
+cudaError_t ms_prim_blocks(int n, const uint32_t *emit_off, const uint32_t *pair_off, int K, uint32_t *prim_start,
+                           uint32_t *prim_blocks, cudaStream_t s) {
+  prim_blocks_kernel<<<(n + 1 + 127) / 128, 128, 0, s>>>(n, emit_off, pair_off, K, prim_start, prim_blocks);
+  return cudaGetLastError();
+}

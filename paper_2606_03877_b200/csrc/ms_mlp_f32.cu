@@ -1,0 +1,93 @@
+// ms_mlp_f32.cu -- stage (d), fp32 SIMT path (NS: "rgb/alpha within 1e-5 max abs for the fp32
+// path"; CFG1).  One CTA = one 128-sample row block of ONE primitive, whose fp32 weights are
+// staged in shared memory once per CTA; one thread = one sample: canonical u,
+// positional encoding Eq.5 with exact-argument sincospif(2^l u), Linear+ReLU layers with
+// fp32 FMA accumulation, rgb = sigmoid, sigma = softplus, e = exp(-sigma*delta).
+// This path is the accuracy reference on the device; the throughput path is ms_mlp_tc.cu.
+#include "ms_internal.cuh"
+
+namespace {
+
+__device__ __forceinline__ int find_prim(const uint32_t *__restrict__ blk_off, int n, uint32_t b) {
+  int lo = 0, hi = n;  // largest p with blk_off[p] <= b
+  while (hi - lo > 1) {
+    int mid = (lo + hi) >> 1;
+    if (blk_off[mid] <= b) lo = mid; else hi = mid;
+  }
+  return lo;
+}
+
+__global__ void __launch_bounds__(MS_ROWS) mlp_f32_kernel(MsMlpArgs a) {
+  extern __shared__ float w_s[];
+  __shared__ int s_prim;
+  const MsMlpShape &sh = a.shape;
+  if (threadIdx.x == 0) s_prim = find_prim(a.blk_off, a.n_prims, blockIdx.x);
+  __syncthreads();
+  const int prim = s_prim;
+  const float *wg = a.weights_f32 + (size_t)prim * sh.params;
+  for (int i = threadIdx.x; i < sh.params; i += blockDim.x) w_s[i] = wg[i];
+  __syncthreads();
+
+  const uint32_t first = a.prim_start[prim], count = a.prim_start[prim + 1] - first;
+  const uint64_t s = (uint64_t)(blockIdx.x - a.blk_off[prim]) * MS_ROWS + threadIdx.x;
+  const uint32_t j = (uint32_t)(s / (uint32_t)a.K);
+  const int k = (int)(s % (uint32_t)a.K);
+  if (j >= count) return;
+  const MsInterval iv = a.intervals[first + j];
+  const float d[3] = {iv.dx, iv.dy, iv.dz};
+  const float t = ms_sample_t(iv.t_in, iv.delta, k);
+  float u[3];
+  ms_sample_u(a.A + 9 * (size_t)prim, a.center + 3 * (size_t)prim, a.cam.o, d, t, u);
+
+  float ha[MS_MAX_WIDTH], hb[MS_MAX_WIDTH];
+  int n_in = 0;
+  ha[n_in++] = u[0]; ha[n_in++] = u[1]; ha[n_in++] = u[2];
+  float scale = 1.0f;
+  for (int l = 0; l < sh.n_freq; ++l) {
+    float sv[3], cv[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) sincospif(scale * u[c], &sv[c], &cv[c]);  // 2^l u is exact
+    ha[n_in++] = sv[0]; ha[n_in++] = sv[1]; ha[n_in++] = sv[2];
+    ha[n_in++] = cv[0]; ha[n_in++] = cv[1]; ha[n_in++] = cv[2];
+    scale *= 2.0f;
+  }
+  if (sh.use_viewdir) { ha[n_in++] = d[0]; ha[n_in++] = d[1]; ha[n_in++] = d[2]; }
+
+  float *src = ha, *dst = hb;
+  const float *w = w_s;
+  for (int l = 0; l < sh.n_layers; ++l) {
+    const bool last = l == sh.n_layers - 1;
+    const int n_out = last ? sh.out_dim : sh.width;
+    const float *bias = w + n_in * n_out;
+    for (int o = 0; o < n_out; ++o) {
+      float acc = bias[o];
+      for (int i = 0; i < n_in; ++i) acc = fmaf(src[i], w[i * n_out + o], acc);
+      dst[o] = last ? acc : fmaxf(acc, 0.0f);
+    }
+    w = bias + n_out;
+    n_in = n_out;
+    float *tmp = src; src = dst; dst = tmp;
+  }
+  const float *raw = src;
+  float4 r;
+  r.x = 1.0f / (1.0f + expf(-raw[0]));
+  r.y = 1.0f / (1.0f + expf(-raw[1]));
+  r.z = 1.0f / (1.0f + expf(-raw[2]));
+  const float sigma = fmaxf(raw[3], 0.0f) + log1pf(expf(-fabsf(raw[3])));
+  r.w = expf(-sigma * iv.delta);  // e = 1 - alpha
+  const size_t out = (size_t)(uint32_t)iv.slot * (size_t)a.K + (size_t)k;
+  a.staging[out] = r;
+  if (a.staging_feat)
+    for (int c = 0; c < sh.n_feat; ++c) a.staging_feat[out * sh.n_feat + c] = raw[4 + c];
+}
+
+}  // namespace
+
+cudaError_t ms_mlp_f32(const MsMlpArgs &a, cudaStream_t s) {
+  if (a.n_blocks == 0) return cudaSuccess;
+  size_t smem = (size_t)a.shape.params * sizeof(float);
+  cudaError_t e = cudaFuncSetAttribute(mlp_f32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  mlp_f32_kernel<<<a.n_blocks, MS_ROWS, smem, s>>>(a);
+  return cudaGetLastError();
+}

@@ -1,0 +1,96 @@
+// ms_scan.cu -- device exclusive scan of uint32 counts (used by stages (a), (c), (d) to turn
+// per-primitive / per-pair / per-ray counts into offsets).  HBM-bound, one read + one write
+// per element per level; levels shrink by 2048x.
+#include "ms_internal.cuh"
+
+namespace {
+
+constexpr int SCAN_THREADS = 256;
+constexpr int SCAN_ITEMS = 8;
+constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
+
+// Local exclusive scan of one tile; the tile total goes to sums[blockIdx.x] (or out[n] if sums == NULL).
+__global__ void __launch_bounds__(SCAN_THREADS) scan_tile_kernel(const uint32_t *__restrict__ in,
+                                                                 uint32_t *__restrict__ out, size_t n,
+                                                                 uint32_t *__restrict__ sums) {
+  __shared__ uint32_t warp_tot[SCAN_THREADS / 32];
+  size_t base = (size_t)blockIdx.x * SCAN_TILE + (size_t)threadIdx.x * SCAN_ITEMS;
+  uint32_t v[SCAN_ITEMS];
+  uint32_t tsum = 0;
+#pragma unroll
+  for (int i = 0; i < SCAN_ITEMS; ++i) {
+    v[i] = (base + i < n) ? in[base + i] : 0u;
+    tsum += v[i];
+  }
+  int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  uint32_t inc = tsum;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    uint32_t o = __shfl_up_sync(0xffffffffu, inc, d);
+    if (lane >= d) inc += o;
+  }
+  if (lane == 31) warp_tot[warp] = inc;
+  __syncthreads();
+  if (warp == 0) {
+    uint32_t w = lane < SCAN_THREADS / 32 ? warp_tot[lane] : 0u;
+#pragma unroll
+    for (int d = 1; d < SCAN_THREADS / 32; d <<= 1) {
+      uint32_t o = __shfl_up_sync(0xffffffffu, w, d);
+      if (lane >= d) w += o;
+    }
+    if (lane < SCAN_THREADS / 32) warp_tot[lane] = w;  // inclusive over warps
+  }
+  __syncthreads();
+  uint32_t excl = inc - tsum + (warp > 0 ? warp_tot[warp - 1] : 0u);
+#pragma unroll
+  for (int i = 0; i < SCAN_ITEMS; ++i) {
+    if (base + i < n) out[base + i] = excl;
+    excl += v[i];
+  }
+  if (threadIdx.x == SCAN_THREADS - 1) {
+    uint32_t total = warp_tot[SCAN_THREADS / 32 - 1];
+    if (sums) sums[blockIdx.x] = total;
+    else out[n] = total;
+  }
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) scan_add_kernel(uint32_t *__restrict__ out, size_t n,
+                                                                const uint32_t *__restrict__ sums_scan,
+                                                                uint32_t n_tiles) {
+  uint32_t add = sums_scan[blockIdx.x];
+  size_t base = (size_t)blockIdx.x * SCAN_TILE + (size_t)threadIdx.x * SCAN_ITEMS;
+#pragma unroll
+  for (int i = 0; i < SCAN_ITEMS; ++i)
+    if (base + i < n) out[base + i] += add;
+  if (blockIdx.x == 0 && threadIdx.x == 0) out[n] = sums_scan[n_tiles];
+}
+
+}  // namespace
+
+size_t ms_scan_scratch_elems(size_t n) {
+  size_t tot = 0;
+  while (n > SCAN_TILE) {
+    size_t nb = (n + SCAN_TILE - 1) / SCAN_TILE;
+    tot += 2 * (nb + 1);
+    n = nb;
+  }
+  return tot + 8;
+}
+
+cudaError_t ms_exclusive_scan_u32(const uint32_t *in, uint32_t *out, size_t n, uint32_t *scratch, cudaStream_t s) {
+  if (n == 0) return cudaMemsetAsync(out, 0, sizeof(uint32_t), s);
+  size_t nb = (n + SCAN_TILE - 1) / SCAN_TILE;
+  if (nb == 1) {
+    scan_tile_kernel<<<1, SCAN_THREADS, 0, s>>>(in, out, n, nullptr);
+    return cudaGetLastError();
+  }
+  uint32_t *sums = scratch;            // [nb]
+  uint32_t *sums_scan = scratch + nb + 1;  // [nb+1]
+  scan_tile_kernel<<<(unsigned)nb, SCAN_THREADS, 0, s>>>(in, out, n, sums);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  e = ms_exclusive_scan_u32(sums, sums_scan, nb, scratch + 2 * (nb + 1), s);
+  if (e != cudaSuccess) return e;
+  scan_add_kernel<<<(unsigned)nb, SCAN_THREADS, 0, s>>>(out, n, sums_scan, (uint32_t)nb);
+  return cudaGetLastError();
+}

@@ -1,0 +1,111 @@
+// ms_sort.cu -- stage (b): device LSD radix sort of the 64-bit (tile | z_entry bits | prim)
+// keys (NS (b); the paper sorts per tile inside one 256-thread block).
+// 8-bit digits, stable; only the bits actually used are sorted.  Each pass: per-block digit
+// histogram -> exclusive scan (digit-major, block-minor) -> stable scatter.  The key set is
+// <= ~0.5 M keys (L2-resident), so this stage is launch-latency-bound, not HBM-bound.
+#include "ms_internal.cuh"
+
+namespace {
+
+constexpr int RS_THREADS = 256;
+constexpr int RS_WARPS = RS_THREADS / 32;
+constexpr int RS_ITEMS = 8;
+constexpr int RS_TILE = RS_THREADS * RS_ITEMS;
+
+__global__ void __launch_bounds__(RS_THREADS) radix_hist_kernel(const uint64_t *__restrict__ keys, size_t n, int shift,
+                                                                uint32_t *__restrict__ counts, uint32_t n_blocks) {
+  __shared__ uint32_t hist[256];
+  hist[threadIdx.x] = 0;
+  __syncthreads();
+  size_t base = (size_t)blockIdx.x * RS_TILE;
+#pragma unroll
+  for (int r = 0; r < RS_ITEMS; ++r) {
+    size_t i = base + (size_t)r * RS_THREADS + threadIdx.x;
+    if (i < n) atomicAdd(&hist[(uint32_t)(keys[i] >> shift) & 255u], 1u);
+  }
+  __syncthreads();
+  counts[(size_t)threadIdx.x * n_blocks + blockIdx.x] = hist[threadIdx.x];
+}
+
+// Key order inside a block: warp w owns keys [w*32*ITEMS, (w+1)*32*ITEMS), visited in rounds of 32.
+__global__ void __launch_bounds__(RS_THREADS) radix_scatter_kernel(const uint64_t *__restrict__ keys,
+                                                                   uint64_t *__restrict__ out, size_t n, int shift,
+                                                                   const uint32_t *__restrict__ offsets,
+                                                                   uint32_t n_blocks) {
+  __shared__ uint32_t wc[RS_WARPS][256];
+  for (int i = threadIdx.x; i < RS_WARPS * 256; i += RS_THREADS) (&wc[0][0])[i] = 0;
+  __syncthreads();
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const uint32_t lt = (1u << lane) - 1u;
+  size_t base = (size_t)blockIdx.x * RS_TILE + (size_t)warp * 32 * RS_ITEMS;
+  uint64_t key[RS_ITEMS];
+  uint32_t rank[RS_ITEMS];
+#pragma unroll
+  for (int r = 0; r < RS_ITEMS; ++r) {
+    size_t i = base + (size_t)r * 32 + lane;
+    bool valid = i < n;
+    key[r] = valid ? keys[i] : 0ull;
+    uint32_t d = valid ? ((uint32_t)(key[r] >> shift) & 255u) : 256u;
+    uint32_t peers = __match_any_sync(0xffffffffu, d);
+    uint32_t prior = valid ? wc[warp][d] : 0u;
+    __syncwarp();
+    if (valid && (peers & lt) == 0u) wc[warp][d] = prior + __popc(peers);
+    __syncwarp();
+    rank[r] = prior + __popc(peers & lt);
+  }
+  __syncthreads();
+  {  // thread t owns digit t: exclusive prefix over warps + global offset of (digit, block)
+    uint32_t run = offsets[(size_t)threadIdx.x * n_blocks + blockIdx.x];
+#pragma unroll
+    for (int w = 0; w < RS_WARPS; ++w) {
+      uint32_t c = wc[w][threadIdx.x];
+      wc[w][threadIdx.x] = run;
+      run += c;
+    }
+  }
+  __syncthreads();
+#pragma unroll
+  for (int r = 0; r < RS_ITEMS; ++r) {
+    size_t i = base + (size_t)r * 32 + lane;
+    if (i < n) {
+      uint32_t d = (uint32_t)(key[r] >> shift) & 255u;
+      out[wc[warp][d] + rank[r]] = key[r];
+    }
+  }
+}
+
+}  // namespace
+
+size_t ms_sort_scratch_elems(size_t n) {
+  size_t nb = (n + RS_TILE - 1) / RS_TILE;
+  if (nb == 0) nb = 1;
+  size_t m = 256 * nb;
+  return 2 * (m + 1) + ms_scan_scratch_elems(m) + 8;
+}
+
+cudaError_t ms_radix_sort_u64(uint64_t *a, uint64_t *b, size_t n, int n_bits, uint32_t *scratch, uint64_t **result,
+                              cudaStream_t s) {
+  *result = a;
+  if (n <= 1 || n_bits <= 0) return cudaSuccess;
+  size_t nb = (n + RS_TILE - 1) / RS_TILE;
+  size_t m = 256 * nb;
+  uint32_t *counts = scratch;
+  uint32_t *offsets = scratch + m + 1;
+  uint32_t *scan_scratch = scratch + 2 * (m + 1);
+  uint64_t *src = a, *dst = b;
+  for (int shift = 0; shift < n_bits; shift += 8) {
+    radix_hist_kernel<<<(unsigned)nb, RS_THREADS, 0, s>>>(src, n, shift, counts, (uint32_t)nb);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    e = ms_exclusive_scan_u32(counts, offsets, m, scan_scratch, s);
+    if (e != cudaSuccess) return e;
+    radix_scatter_kernel<<<(unsigned)nb, RS_THREADS, 0, s>>>(src, dst, n, shift, offsets, (uint32_t)nb);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    uint64_t *t = src;
+    src = dst;
+    dst = t;
+  }
+  *result = src;
+  return cudaSuccess;
+}
