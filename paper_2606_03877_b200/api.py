@@ -125,11 +125,15 @@ class Scene:
 
     def close(self):
         h = getattr(self, "_h", None)
-        if h:
+        if h and _lib is not None:
             _lib.ms_scene_destroy(h)
-            self._h = None
+        self._h = None
 
-    __del__ = close
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
     def _check(self, rc: int, where: str):
         if rc != 0:
