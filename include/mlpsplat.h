@@ -105,6 +105,7 @@ typedef struct {
   int64_t n_samples;   /* n_intervals * K = MLP evaluations */
   int64_t n_blocks;    /* 128-sample row blocks fed to the MLP stage */
   int64_t scratch_bytes;
+  int64_t n_launches;  /* kernels launched for this view (all stages) */
 } ms_stats;
 
 enum { MS_STAGE_BIN = 0, MS_STAGE_SORT, MS_STAGE_ISECT, MS_STAGE_MLP, MS_STAGE_COMPOSITE, MS_N_STAGES };
@@ -137,6 +138,12 @@ int ms_last_stats(ms_scene *scene, ms_stats *out);
 /* Device time of each stage of the last view rendered with MS_FLAG_STAGE_TIMES, in ms,
  * ms[MS_N_STAGES].  Synchronises the recorded events. */
 int ms_last_stage_ms(ms_scene *scene, float *ms);
+
+/* Sum of the per-stage device times (ms_sum[MS_N_STAGES], ms) over every view rendered with
+ * MS_FLAG_STAGE_TIMES since the last reset, and the number of views summed.  The library reads a
+ * view's events at the start of the next render (or in this call): one event wait per view, on
+ * work the next render has to wait for anyway.  reset != 0 clears the sums. */
+int ms_stage_accum(ms_scene *scene, double *ms_sum, int64_t *n_views, int32_t reset);
 
 /* ---- parity introspection: valid after a render with MS_FLAG_KEEP_DEBUG (last view) ---- */
 /* Sorted tile lists: tile_offsets host [tiles+1], prim_ids / zbits host [cap]. */

@@ -21,7 +21,7 @@ FLAG_KEEP_DEBUG, FLAG_STAGE_TIMES = 1, 2
 STAGES = ("bin", "sort", "isect", "mlp", "composite")
 
 EXPORTS = ["ms_scene_create", "ms_scene_destroy", "ms_render", "ms_render_batch", "ms_render_host",
-           "ms_last_stats", "ms_last_stage_ms", "ms_debug_tile_lists", "ms_debug_intervals",
+           "ms_last_stats", "ms_last_stage_ms", "ms_stage_accum", "ms_debug_tile_lists", "ms_debug_intervals",
            "ms_debug_sample_order", "ms_debug_prim_frames", "ms_error_string", "ms_last_cuda_error"]
 
 
@@ -47,7 +47,8 @@ class _Opts(C.Structure):
 
 class _Stats(C.Structure):
     _fields_ = [("n_visible", C.c_int64), ("n_pairs", C.c_int64), ("n_intervals", C.c_int64),
-                ("n_samples", C.c_int64), ("n_blocks", C.c_int64), ("scratch_bytes", C.c_int64)]
+                ("n_samples", C.c_int64), ("n_blocks", C.c_int64), ("scratch_bytes", C.c_int64),
+                ("n_launches", C.c_int64)]
 
 
 def _load() -> C.CDLL:
@@ -94,6 +95,7 @@ class Stats:
     n_samples: int
     n_blocks: int
     scratch_bytes: int
+    n_launches: int
 
 
 class Scene:
@@ -200,12 +202,20 @@ class Scene:
     def stats(self) -> Stats:
         st = _Stats()
         self._check(_lib.ms_last_stats(self._h, C.byref(st)), "ms_last_stats")
-        return Stats(st.n_pairs, st.n_intervals, st.n_samples, st.n_blocks, st.scratch_bytes)
+        return Stats(st.n_pairs, st.n_intervals, st.n_samples, st.n_blocks, st.scratch_bytes, st.n_launches)
 
     def stage_ms(self) -> dict[str, float]:
         ms = (C.c_float * len(STAGES))()
         self._check(_lib.ms_last_stage_ms(self._h, ms), "ms_last_stage_ms")
         return {k: float(v) for k, v in zip(STAGES, ms)}
+
+    def stage_accum(self, reset: bool = False):
+        """(sum of per-stage ms over the views rendered with FLAG_STAGE_TIMES, number of views)."""
+        ms = (C.c_double * len(STAGES))()
+        n = C.c_int64(0)
+        self._check(_lib.ms_stage_accum(self._h, ms, C.byref(n), C.c_int32(1 if reset else 0)),
+                    "ms_stage_accum")
+        return {k: float(v) for k, v in zip(STAGES, ms)}, int(n.value)
 
     def debug_tile_lists(self, n_tiles: int):
         n = C.c_size_t(0)

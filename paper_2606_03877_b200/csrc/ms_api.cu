@@ -11,6 +11,8 @@
 #include "ms_internal.cuh"
 #include "ms_mlp_tc.cuh"
 
+thread_local long long ms_launch_count = 0;
+
 namespace {
 
 struct Buf {
@@ -37,6 +39,9 @@ struct ms_scene {
   uint32_t *pinned = nullptr;  // [4] host-pinned readback
   cudaEvent_t ev[MS_N_STAGES + 1] = {};
   bool ev_valid = false;
+  bool ev_pending = false;         // events of the last view not yet added to stage_sum
+  double stage_sum[MS_N_STAGES] = {};
+  int64_t stage_views = 0;
   // last view
   ms_stats stats{};
   bool debug_valid = false;
@@ -112,6 +117,22 @@ float round_bf16(float f) {
   return f;
 }
 
+// Adds the stage times of the previous view to the running sums.  Called right after a stream
+// synchronisation (so the events have completed) -- never adds a synchronisation of its own.
+void harvest_stage_times(ms_scene *sc) {
+  if (!sc->ev_pending) return;
+  sc->ev_pending = false;
+  for (int i = 0; i < MS_N_STAGES; ++i) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, sc->ev[i], sc->ev[i + 1]) != cudaSuccess) {
+      (void)cudaGetLastError();
+      return;
+    }
+    sc->stage_sum[i] += ms;
+  }
+  sc->stage_views += 1;
+}
+
 MsCam make_cam(const ms_camera *c, int H, int W) {
   MsCam m;
   m.fx = c->fx; m.fy = c->fy; m.cx = c->cx; m.cy = c->cy;
@@ -147,9 +168,14 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   if (path != MS_PATH_BF16_TC && path != MS_PATH_FP32) return MS_ERR_INVALID_ARG;
 
   const bool timing = (opts->flags & MS_FLAG_STAGE_TIMES) != 0;
-  sc->ev_valid = false;
   sc->debug_valid = false;
   const MsCam cam = make_cam(camera, H, W);
+  const long long launches0 = ms_launch_count;
+  if (sc->ev_pending) {  // the previous view's events must be read before they are re-recorded
+    CK(cudaEventSynchronize(sc->ev[MS_N_STAGES]));
+    harvest_stage_times(sc);
+  }
+  sc->ev_valid = false;
 
   // ---- (a) projection + key emit ----------------------------------------------------------
   if (timing) CK(cudaEventRecord(sc->ev[0], st));
@@ -249,7 +275,9 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   if (timing) {
     CK(cudaEventRecord(sc->ev[5], st));
     sc->ev_valid = true;
+    sc->ev_pending = true;
   }
+  sc->stats.n_launches = (int64_t)(ms_launch_count - launches0);
 
   sc->stats.n_pairs = (int64_t)P;
   sc->stats.n_intervals = (int64_t)n_hits;
@@ -451,6 +479,22 @@ int ms_last_stage_ms(ms_scene *sc, float *ms) {
   if (!sc || !ms || !sc->ev_valid) return MS_ERR_INVALID_ARG;
   CK(cudaEventSynchronize(sc->ev[MS_N_STAGES]));
   for (int i = 0; i < MS_N_STAGES; ++i) CK(cudaEventElapsedTime(&ms[i], sc->ev[i], sc->ev[i + 1]));
+  return MS_OK;
+}
+
+int ms_stage_accum(ms_scene *sc, double *ms_sum, int64_t *n_views, int32_t reset) {
+  if (!sc) return MS_ERR_INVALID_ARG;
+  if (sc->ev_pending) {
+    CK(cudaEventSynchronize(sc->ev[MS_N_STAGES]));
+    harvest_stage_times(sc);
+  }
+  if (ms_sum)
+    for (int i = 0; i < MS_N_STAGES; ++i) ms_sum[i] = sc->stage_sum[i];
+  if (n_views) *n_views = sc->stage_views;
+  if (reset) {
+    for (int i = 0; i < MS_N_STAGES; ++i) sc->stage_sum[i] = 0.0;
+    sc->stage_views = 0;
+  }
   return MS_OK;
 }
 

@@ -160,6 +160,7 @@ cudaError_t ms_prep_prims(int n, const float *center, const float *quat, const f
                           int *bad, cudaStream_t s) {
   (void)center;
   prep_prims_kernel<<<(n + 127) / 128, 128, 0, s>>>(n, quat, scale, A, M, bad);
+  MS_LAUNCHED();
   return cudaGetLastError();
 }
 
@@ -167,6 +168,7 @@ cudaError_t ms_project(int n, const float *center, const float *A, const float *
                        int tiles_y, uint32_t *tile_count, int4 *rect, float *z_entry, float *oprime, cudaStream_t s) {
   (void)tiles_x; (void)tiles_y;
   project_kernel<<<(n + 127) / 128, 128, 0, s>>>(n, center, A, M, cam, tile, tile_count, rect, z_entry, oprime);
+  MS_LAUNCHED();
   return cudaGetLastError();
 }
 
@@ -175,6 +177,7 @@ cudaError_t ms_emit_keys(int n, const uint32_t *emit_off, const int4 *rect, cons
   long threads = (long)n * 32;
   emit_keys_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, s>>>(n, emit_off, rect, z_entry, tiles_x, prim_bits,
                                                                     keys);
+  MS_LAUNCHED();
   return cudaGetLastError();
 }
 
@@ -183,5 +186,6 @@ cudaError_t ms_tile_ranges(const uint64_t *keys, size_t n_pairs, int n_tiles, in
   if (n_pairs == 0) return cudaMemsetAsync(tile_start, 0, (size_t)(n_tiles + 1) * sizeof(uint32_t), s);
   tile_ranges_kernel<<<(unsigned)((n_pairs + 255) / 256), 256, 0, s>>>(keys, (uint32_t)n_pairs, n_tiles,
                                                                       32 + prim_bits, tile_start);
+  MS_LAUNCHED();
   return cudaGetLastError();
 }

@@ -86,10 +86,12 @@ cudaError_t ms_composite(const MsCompositeArgs &a, cudaStream_t s) {
   if (!feat) composite_kernel<0, false><<<grid, 128, 0, s>>>(a, 0, nullptr, nullptr, nullptr);
   else if (a.n_feat == 32) composite_kernel<32, false><<<grid, 128, 0, s>>>(a, 0, nullptr, nullptr, nullptr);
   else composite_kernel<-1, false><<<grid, 128, 0, s>>>(a, 0, nullptr, nullptr, nullptr);
+  MS_LAUNCHED();
   return cudaGetLastError();
 }
 
 cudaError_t ms_sample_order(const MsCompositeArgs &a, int ray, int *prim, int *k, float *t, cudaStream_t s) {
   composite_kernel<0, true><<<1, 32, 0, s>>>(a, ray, prim, k, t);
+  MS_LAUNCHED();
   return cudaGetLastError();
 }

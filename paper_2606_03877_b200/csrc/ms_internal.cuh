@@ -105,6 +105,10 @@ __device__ __forceinline__ void ms_sample_u(const float *A, const float *mu, con
   u[2] = ms_dot3(A[6], A[7], A[8], w0, w1, w2);
 }
 
+// kernels launched so far by this host thread (bench.py reports the per-step count)
+extern thread_local long long ms_launch_count;
+#define MS_LAUNCHED() (++ms_launch_count)
+
 // ---------------------------------------------------------------------------------------------
 // host-side launchers (one per stage file)
 // ---------------------------------------------------------------------------------------------

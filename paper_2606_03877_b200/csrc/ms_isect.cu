@@ -90,17 +90,20 @@ __global__ void prim_blocks_kernel(int n, const uint32_t *__restrict__ emit_off,
 cudaError_t ms_isect_count(const MsIsectArgs &a, cudaStream_t s) {
   if (a.n_tiles == 0) return cudaSuccess;
   isect_kernel<false><<<a.n_tiles, a.tile * a.tile, 0, s>>>(a);
+  MS_LAUNCHED();
   return cudaGetLastError();
 }
 
 cudaError_t ms_isect_fill(const MsIsectArgs &a, cudaStream_t s) {
   if (a.n_tiles == 0) return cudaSuccess;
   isect_kernel<true><<<a.n_tiles, a.tile * a.tile, 0, s>>>(a);
+  MS_LAUNCHED();
   return cudaGetLastError();
 }
 
 cudaError_t ms_prim_blocks(int n, const uint32_t *emit_off, const uint32_t *pair_off, int K, uint32_t *prim_start,
                            uint32_t *prim_blocks, cudaStream_t s) {
   prim_blocks_kernel<<<(n + 1 + 127) / 128, 128, 0, s>>>(n, emit_off, pair_off, K, prim_start, prim_blocks);
+  MS_LAUNCHED();
   return cudaGetLastError();
 }

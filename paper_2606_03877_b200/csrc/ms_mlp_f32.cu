@@ -89,5 +89,6 @@ cudaError_t ms_mlp_f32(const MsMlpArgs &a, cudaStream_t s) {
   cudaError_t e = cudaFuncSetAttribute(mlp_f32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   mlp_f32_kernel<<<a.n_blocks, MS_ROWS, smem, s>>>(a);
+  MS_LAUNCHED();
   return cudaGetLastError();
 }

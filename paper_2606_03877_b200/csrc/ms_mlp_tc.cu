@@ -571,5 +571,6 @@ cudaError_t ms_mlp_tc(const MsTcWeights &w, const MsMlpArgs &a, cudaStream_t s) 
   if (e != cudaSuccess) return e;
   unsigned grid = a.n_blocks < (uint32_t)n_sm ? a.n_blocks : (unsigned)n_sm;
   fn<<<grid, TC_THREADS, smem, s>>>(p);
+  MS_LAUNCHED();
   return cudaGetLastError();
 }

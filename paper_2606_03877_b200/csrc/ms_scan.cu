@@ -82,15 +82,18 @@ cudaError_t ms_exclusive_scan_u32(const uint32_t *in, uint32_t *out, size_t n, u
   size_t nb = (n + SCAN_TILE - 1) / SCAN_TILE;
   if (nb == 1) {
     scan_tile_kernel<<<1, SCAN_THREADS, 0, s>>>(in, out, n, nullptr);
+  MS_LAUNCHED();
     return cudaGetLastError();
   }
   uint32_t *sums = scratch;            // [nb]
   uint32_t *sums_scan = scratch + nb + 1;  // [nb+1]
   scan_tile_kernel<<<(unsigned)nb, SCAN_THREADS, 0, s>>>(in, out, n, sums);
+  MS_LAUNCHED();
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   e = ms_exclusive_scan_u32(sums, sums_scan, nb, scratch + 2 * (nb + 1), s);
   if (e != cudaSuccess) return e;
   scan_add_kernel<<<(unsigned)nb, SCAN_THREADS, 0, s>>>(out, n, sums_scan, (uint32_t)nb);
+  MS_LAUNCHED();
   return cudaGetLastError();
 }

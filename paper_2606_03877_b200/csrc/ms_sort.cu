@@ -95,11 +95,13 @@ cudaError_t ms_radix_sort_u64(uint64_t *a, uint64_t *b, size_t n, int n_bits, ui
   uint64_t *src = a, *dst = b;
   for (int shift = 0; shift < n_bits; shift += 8) {
     radix_hist_kernel<<<(unsigned)nb, RS_THREADS, 0, s>>>(src, n, shift, counts, (uint32_t)nb);
+  MS_LAUNCHED();
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     e = ms_exclusive_scan_u32(counts, offsets, m, scan_scratch, s);
     if (e != cudaSuccess) return e;
     radix_scatter_kernel<<<(unsigned)nb, RS_THREADS, 0, s>>>(src, dst, n, shift, offsets, (uint32_t)nb);
+  MS_LAUNCHED();
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     uint64_t *t = src;
