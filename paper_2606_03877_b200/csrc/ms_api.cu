@@ -34,7 +34,7 @@ struct ms_scene {
   MsTcWeights tc{};  // packed bf16 image for the tensor path (may be empty)
   // per-view scratch
   Buf tile_count, emit_off, rect, z_entry, oprime, keys_a, keys_b, sort_scratch, tile_start, pair_hits, pair_off,
-      ray_hits, ray_off, scan_scratch, prim_start, prim_blocks, blk_off, intervals, hits, cur, staging, staging_feat,
+      ray_hits, ray_off, scan_scratch, prim_start, prim_blocks, blk_off, intervals, hits, staging, staging_feat,
       host_rgb, host_alpha, host_feat, dbg;
   uint32_t *pinned = nullptr;  // [4] host-pinned readback
   cudaEvent_t ev[MS_N_STAGES + 1] = {};
@@ -95,7 +95,7 @@ size_t scratch_total(const ms_scene *sc) {
   const Buf *all[] = {&sc->tile_count, &sc->emit_off, &sc->rect, &sc->z_entry, &sc->oprime, &sc->keys_a, &sc->keys_b,
                       &sc->sort_scratch, &sc->tile_start, &sc->pair_hits, &sc->pair_off, &sc->ray_hits, &sc->ray_off,
                       &sc->scan_scratch, &sc->prim_start, &sc->prim_blocks, &sc->blk_off, &sc->intervals, &sc->hits,
-                      &sc->cur, &sc->staging, &sc->staging_feat};
+                      &sc->staging, &sc->staging_feat};
   size_t t = 0;
   for (const Buf *b : all) t += b->cap;
   return t;
@@ -244,7 +244,6 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   const bool want_feat = sc->shape.n_feat > 0 && out_feat != nullptr;
   ENS(sc->intervals, (n_hits + 1) * sizeof(MsInterval));
   ENS(sc->hits, (n_hits + 1) * sizeof(MsHit));
-  ENS(sc->cur, (n_hits + 1) * sizeof(float2));
   ENS(sc->staging, (n_samples + 1) * sizeof(float4));
   if (want_feat) ENS(sc->staging_feat, (n_samples + 1) * (size_t)sc->shape.n_feat * 4);
   ia.intervals = (MsInterval *)sc->intervals.p;
@@ -269,7 +268,6 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   ca.n_rays = R; ca.K = K; ca.n_feat = sc->shape.n_feat; ca.t_stop = opts->t_stop;
   ca.ray_off = (uint32_t *)sc->ray_off.p; ca.hits = (MsHit *)sc->hits.p; ca.staging = (float4 *)sc->staging.p;
   ca.staging_feat = want_feat ? (float *)sc->staging_feat.p : nullptr;
-  ca.cur_t = (float *)sc->cur.p;
   ca.out_rgb = out_rgb; ca.out_alpha = out_alpha; ca.out_feat = want_feat ? out_feat : nullptr;
   CK(ms_composite(ca, st));
   if (timing) {
@@ -416,7 +414,7 @@ int ms_scene_destroy(ms_scene *sc) {
   Buf *all[] = {&sc->tile_count, &sc->emit_off, &sc->rect, &sc->z_entry, &sc->oprime, &sc->keys_a, &sc->keys_b,
                 &sc->sort_scratch, &sc->tile_start, &sc->pair_hits, &sc->pair_off, &sc->ray_hits, &sc->ray_off,
                 &sc->scan_scratch, &sc->prim_start, &sc->prim_blocks, &sc->blk_off, &sc->intervals, &sc->hits,
-                &sc->cur, &sc->staging, &sc->staging_feat, &sc->host_rgb, &sc->host_alpha, &sc->host_feat, &sc->dbg};
+                &sc->staging, &sc->staging_feat, &sc->host_rgb, &sc->host_alpha, &sc->host_feat, &sc->dbg};
   for (Buf *b : all) free_buf(*b);
   if (sc->pinned) cudaFreeHost(sc->pinned);
   for (int i = 0; i <= MS_N_STAGES; ++i)
@@ -556,7 +554,6 @@ int ms_debug_sample_order(ms_scene *sc, int32_t ray, int32_t *prim, int32_t *k, 
   memset(&ca, 0, sizeof(ca));
   ca.n_rays = sc->dbg_H * sc->dbg_W; ca.K = sc->dbg_K; ca.n_feat = 0; ca.t_stop = 0.f;
   ca.ray_off = (uint32_t *)sc->ray_off.p; ca.hits = (MsHit *)sc->hits.p; ca.staging = (float4 *)sc->staging.p;
-  ca.cur_t = (float *)sc->cur.p;
   CK(ms_sample_order(ca, ray, dp, dk, dt, 0));
   CK(cudaDeviceSynchronize());
   if (prim) CK(cudaMemcpy(prim, dp, ns * 4, cudaMemcpyDeviceToHost));

@@ -1,97 +1,245 @@
 // ms_composite.cu -- stage (e): per-ray merge of the hit intervals' sample streams in
 // (t, primitive id, k) order and front-to-back compositing (Eq.6, Eq.14):
 //   w = T (1 - e); C += w rgb; F += w feat; T <- T e; stop once T < t_stop (NS (e), Q9).
-// Each stream t_k = t_in + (k + 1/2) delta is already sorted in k (fp32 rounding is monotone),
-// so a cursor per hit and a min-selection over the ray's hits reproduces the full sort.
-// One thread per ray; cursor state lives in a global scratch array (8 B per hit) so any number
-// of hits per ray is handled.  HBM-bound: reads 16 B (+ 4 n_feat B) per sample.
+//
+// One warp per ray.  Each stream t_k = t_in + (k + 1/2) delta is non-decreasing in k (fp32 rounding
+// is monotone), so the position of a sample in the merged order has a closed form: its own k plus,
+// for every other hit of the ray, the number of that hit's samples that precede (t, prim) -- 0 or K
+// when the two t-ranges do not overlap (two compares), else a binary search over k.  No cursors, no
+// sort.  The ray's staged samples (16 B each, contiguous) are fetched by cp.async while the ranks are
+// computed; 32 merged samples at a time are composited with a warp product scan.  Features are
+// accumulated channel-per-lane, one coalesced 128 B row per sample.
+// HBM-bound by design: reads 16 B (+ 4 n_feat B) per sample and 16 B per hit, once.
 #include "ms_internal.cuh"
-#include <math_constants.h>
 
 namespace {
 
-template <int NF, bool DEBUG>
-__global__ void __launch_bounds__(128) composite_kernel(MsCompositeArgs a, int dbg_ray, int *dbg_prim, int *dbg_k,
-                                                        float *dbg_t) {
-  int ray = DEBUG ? dbg_ray : (int)(blockIdx.x * blockDim.x + threadIdx.x);
-  if (ray >= a.n_rays || (DEBUG && (blockIdx.x != 0 || threadIdx.x != 0))) return;
+constexpr int CW = 4;        // warps (rays) per CTA
+constexpr int CAP = 448;     // samples per window (a ray with more is processed in rank windows)
+constexpr int HCAP = 32;     // hits cached in shared memory per ray (one per lane)
+constexpr unsigned FULL = 0xffffffffu;
+
+struct WarpSmem {
+  float4 val[CAP];      // (r, g, b, e) of the window's samples; .w is overwritten by the weight w
+  uint32_t ord[CAP];    // ord[rank - r0] = sample index s = h*K + k inside the ray
+  float4 key[HCAP];     // (t of sample 0, t of sample K-1, prim bits, unused)
+  float2 geo[HCAP];     // (t_in, delta)
+  uint2 pre[HCAP];      // (samples of streams entirely before this one, mask of streams that overlap it)
+};
+
+__device__ __forceinline__ bool precedes(float t2, float t, bool tie_lt) { return t2 < t || (t2 == t && tie_lt); }
+
+// number of samples of stream (ti2, dl2, first tf, last tl, prim p2) that precede (t, prim)
+__device__ __forceinline__ uint32_t count_before(float tf, float tl, float ti2, float dl2, int p2, float t, int prim, int K) {
+  const bool tie_lt = p2 < prim;
+  if (!precedes(tf, t, tie_lt)) return 0u;
+  if (precedes(tl, t, tie_lt)) return (uint32_t)K;
+  int lo = 0, hi = K - 1;  // precedes(lo) holds, precedes(hi) does not
+  while (hi - lo > 1) {
+    const int mid = (lo + hi) >> 1;
+    if (precedes(ms_sample_t(ti2, dl2, mid), t, tie_lt)) lo = mid; else hi = mid;
+  }
+  return (uint32_t)hi;
+}
+
+// rank of sample (h, k) in the order (t, prim, k).  n <= HCAP: stream-level classification in
+// sm.pre (streams entirely before / after need no per-sample work); else every stream is tested.
+__device__ __forceinline__ uint32_t sample_rank(const WarpSmem &sm, const MsHit *__restrict__ hits, int n, int K, int h,
+                                                int k, float *t_out) {
+  if (n <= HCAP) {
+    const float t = ms_sample_t(sm.geo[h].x, sm.geo[h].y, k);
+    const int prim = __float_as_int(sm.key[h].z);
+    *t_out = t;
+    const uint2 pr = sm.pre[h];
+    uint32_t rank = (uint32_t)k + pr.x;
+    uint32_t m = pr.y;
+    while (m) {
+      const int h2 = __ffs(m) - 1;
+      m &= m - 1;
+      const float4 q = sm.key[h2];
+      const float2 g = sm.geo[h2];
+      rank += count_before(q.x, q.y, g.x, g.y, __float_as_int(q.z), t, prim, K);
+    }
+    return rank;
+  }
+  const MsHit me = hits[h];
+  const float t = ms_sample_t(me.t_in, me.delta, k);
+  *t_out = t;
+  uint32_t rank = (uint32_t)k;
+  for (int h2 = 0; h2 < n; ++h2) {
+    if (h2 == h) continue;
+    const MsHit g = hits[h2];
+    rank += count_before(ms_sample_t(g.t_in, g.delta, 0), ms_sample_t(g.t_in, g.delta, K - 1), g.t_in, g.delta, g.prim, t,
+                         me.prim, K);
+  }
+  return rank;
+}
+
+__device__ __forceinline__ void cp_async16(void *dst_smem, const void *src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(dst_smem)), "l"(src)
+               : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+// n <= HCAP: lane h caches hit h and classifies every other stream against it
+__device__ __forceinline__ void load_hits(WarpSmem &sm, const MsHit *__restrict__ hits, int n, int K, int lane) {
+  if (n > HCAP) return;
+  float tf = 0.f, tl = 0.f;
+  int prim = 0;
+  if (lane < n) {
+    const MsHit g = hits[lane];
+    tf = ms_sample_t(g.t_in, g.delta, 0); tl = ms_sample_t(g.t_in, g.delta, K - 1); prim = g.prim;
+    sm.key[lane] = make_float4(tf, tl, __int_as_float(prim), 0.f);
+    sm.geo[lane] = make_float2(g.t_in, g.delta);
+  }
+  __syncwarp();
+  if (lane < n) {
+    uint32_t before = 0, mask = 0;
+    for (int h2 = 0; h2 < n; ++h2) {
+      const float4 q = sm.key[h2];
+      const bool tie_lt = __float_as_int(q.z) < prim;
+      const bool all_before = precedes(q.y, tf, tie_lt);    // its last sample precedes my first
+      const bool some_before = precedes(q.x, tl, tie_lt);   // its first sample precedes my last
+      before += all_before ? (uint32_t)K : 0u;
+      mask |= (some_before && !all_before && h2 != lane) ? (1u << h2) : 0u;
+    }
+    sm.pre[lane] = make_uint2(before, mask);
+  }
+}
+
+template <int FEAT>  // 0: rgb/alpha only; 1: + features
+__global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
+  __shared__ WarpSmem s_all[CW];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int ray = (int)(blockIdx.x * CW + warp);
+  if (ray >= a.n_rays) return;
+  WarpSmem &sm = s_all[warp];
+  const uint32_t off = a.ray_off[ray];
+  const int n = (int)(a.ray_off[ray + 1] - off);
+  const int K = a.K, nf = a.n_feat;
+  float T = 1.0f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
+  float F[MS_MAX_OUT / 32] = {0.f, 0.f};
+  if (n > 0) {
+    const MsHit *hits = a.hits + off;
+    const float4 *stg = a.staging + (size_t)off * (size_t)K;
+    const uint32_t S = (uint32_t)n * (uint32_t)K;
+    const bool single = S <= (uint32_t)CAP;
+    if (single)
+      for (uint32_t s = lane; s < S; s += 32) cp_async16(&sm.val[s], stg + s);  // in flight during the rank pass
+    load_hits(sm, hits, n, K, lane);
+    __syncwarp();
+    bool stopped = false;
+    for (uint32_t r0 = 0; r0 < S && !stopped; r0 += CAP) {
+      const uint32_t cnt = S - r0 < (uint32_t)CAP ? S - r0 : (uint32_t)CAP;
+      // ---- rank pass: ord[] (and, for a multi-window ray, val[] by rank) ----
+      int h = lane / K, k = lane - h * K;
+      const int dh = 32 / K, dk = 32 - dh * K;
+      for (uint32_t s = lane; s < S; s += 32) {
+        float t;
+        const uint32_t rk = sample_rank(sm, hits, n, K, h, k, &t) - r0;
+        if (rk < cnt) {
+          sm.ord[rk] = s;
+          if (!single) sm.val[rk] = stg[s];
+        }
+        h += dh; k += dk;
+        if (k >= K) { k -= K; ++h; }
+      }
+      if (single) cp_async_wait_all();
+      __syncwarp();
+      // ---- composite the window, 32 merged samples per step ----
+      uint32_t done = cnt;  // samples of this window that carry a weight
+      for (uint32_t base = 0; base < cnt; base += 32) {
+        const uint32_t r = base + lane;
+        const bool valid = r < cnt;
+        uint32_t slot = 0;
+        float4 v = make_float4(0.f, 0.f, 0.f, 1.f);
+        if (valid) {
+          slot = single ? sm.ord[r] : r;
+          v = sm.val[slot];
+        }
+        float p = v.w;  // inclusive product scan of e over the lanes
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+          const float q = __shfl_up_sync(FULL, p, o);
+          if (lane >= o) p *= q;
+        }
+        float excl = __shfl_up_sync(FULL, p, 1);
+        if (lane == 0) excl = 1.0f;
+        const float T_after = T * p;
+        const unsigned stop = __ballot_sync(FULL, valid && T_after < a.t_stop);
+        const int last = stop ? __ffs(stop) - 1 : 31;          // Q9: the stopping sample still contributes
+        float w = (valid && lane <= last) ? (T * excl) * (1.0f - v.w) : 0.f;
+        C0 = fmaf(w, v.x, C0); C1 = fmaf(w, v.y, C1); C2 = fmaf(w, v.z, C2);
+        if (FEAT && valid) sm.val[slot].w = w;
+        T = __shfl_sync(FULL, T_after, last);
+        if (stop) { stopped = true; done = base + (uint32_t)last + 1; break; }
+      }
+      if (FEAT) {
+        __syncwarp();
+        const float *fbase = a.staging_feat + (size_t)off * (size_t)K * (size_t)nf;
+        for (uint32_t r = 0; r < done; ++r) {
+          const uint32_t s = sm.ord[r];
+          const float w = sm.val[single ? s : r].w;
+#pragma unroll
+          for (int q = 0; q < MS_MAX_OUT / 32; ++q) {
+            const int c = lane + 32 * q;
+            if (c < nf) F[q] = fmaf(w, __ldg(fbase + (size_t)s * (size_t)nf + c), F[q]);
+          }
+        }
+      }
+      __syncwarp();
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      C0 += __shfl_xor_sync(FULL, C0, o);
+      C1 += __shfl_xor_sync(FULL, C1, o);
+      C2 += __shfl_xor_sync(FULL, C2, o);
+    }
+  }
+  if (lane < 3) a.out_rgb[3 * (size_t)ray + lane] = lane == 0 ? C0 : (lane == 1 ? C1 : C2);
+  if (lane == 3) a.out_alpha[ray] = 1.0f - T;
+  if (FEAT) {
+#pragma unroll
+    for (int q = 0; q < MS_MAX_OUT / 32; ++q) {
+      const int c = lane + 32 * q;
+      if (c < nf) a.out_feat[(size_t)ray * nf + c] = F[q];
+    }
+  }
+}
+
+// parity introspection: the merged order of one ray, written by rank (NS: "sample ordering bit-exact")
+__global__ void sample_order_kernel(MsCompositeArgs a, int ray, int *dbg_prim, int *dbg_k, float *dbg_t) {
+  __shared__ WarpSmem sm;
+  const int lane = threadIdx.x;
   const uint32_t off = a.ray_off[ray];
   const int n = (int)(a.ray_off[ray + 1] - off);
   const int K = a.K;
-  const int nf = NF >= 0 ? NF : a.n_feat;
-  float T = 1.0f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
-  float F[NF > 0 ? NF : (NF < 0 ? MS_MAX_OUT : 1)];
-#pragma unroll
-  for (int c = 0; c < (NF > 0 ? NF : (NF < 0 ? MS_MAX_OUT : 1)); ++c) F[c] = 0.f;
   const MsHit *hits = a.hits + off;
-  float2 *cur = reinterpret_cast<float2 *>(a.cur_t) + off;  // (t of the next sample, its k)
-  for (int h = 0; h < n; ++h) cur[h] = make_float2(ms_sample_t(hits[h].t_in, hits[h].delta, 0), __int_as_float(0));
-  const long total = (long)n * K;
-  for (long it = 0; it < total; ++it) {
-    int best = -1, best_prim = 0;
-    float bt = CUDART_INF_F;
-    for (int h = 0; h < n; ++h) {
-      const float t = cur[h].x;  // +inf once the stream is exhausted
-      if (t < bt) {
-        bt = t; best = h; best_prim = -1;
-      } else if (t == bt && best >= 0) {
-        if (best_prim < 0) best_prim = hits[best].prim;
-        const int p = hits[h].prim;
-        if (p < best_prim) { best = h; best_prim = p; }
-      }
-    }
-    if (best < 0) break;  // only if some t is NaN/inf; cannot happen for finite inputs
-    const MsHit hb = hits[best];
-    const int k = __float_as_int(cur[best].y);
-    cur[best] = make_float2(k + 1 < K ? ms_sample_t(hb.t_in, hb.delta, k + 1) : CUDART_INF_F, __int_as_float(k + 1));
-    if (DEBUG) {
-      dbg_prim[it] = hb.prim; dbg_k[it] = k; dbg_t[it] = bt;
-      continue;
-    }
-    const size_t s = (size_t)(off + (uint32_t)best) * (size_t)K + (size_t)k;
-    const float4 v = a.staging[s];
-    const float w = T * (1.0f - v.w);
-    C0 = fmaf(w, v.x, C0); C1 = fmaf(w, v.y, C1); C2 = fmaf(w, v.z, C2);
-    if (NF != 0 && a.staging_feat) {
-      const float *f = a.staging_feat + s * (size_t)nf;
-      if (NF > 0) {
-#pragma unroll
-        for (int c = 0; c < (NF > 0 ? NF : 1); c += 4) {
-          const float4 q = *reinterpret_cast<const float4 *>(f + c);
-          F[c] = fmaf(w, q.x, F[c]); F[c + 1] = fmaf(w, q.y, F[c + 1]);
-          F[c + 2] = fmaf(w, q.z, F[c + 2]); F[c + 3] = fmaf(w, q.w, F[c + 3]);
-        }
-      } else {
-        for (int c = 0; c < nf; ++c) F[c] = fmaf(w, f[c], F[c]);
-      }
-    }
-    T *= v.w;
-    if (T < a.t_stop) break;
+  load_hits(sm, hits, n, K, lane);
+  __syncwarp();
+  const uint32_t S = (uint32_t)n * (uint32_t)K;
+  for (uint32_t s = lane; s < S; s += 32) {
+    const int h = (int)(s / (uint32_t)K), k = (int)(s - (uint32_t)h * (uint32_t)K);
+    float t;
+    const uint32_t rk = sample_rank(sm, hits, n, K, h, k, &t);
+    dbg_prim[rk] = hits[h].prim; dbg_k[rk] = k; dbg_t[rk] = t;
   }
-  if (DEBUG) return;
-  a.out_rgb[3 * (size_t)ray + 0] = C0;
-  a.out_rgb[3 * (size_t)ray + 1] = C1;
-  a.out_rgb[3 * (size_t)ray + 2] = C2;
-  a.out_alpha[ray] = 1.0f - T;
-  if (NF != 0 && a.out_feat)
-    for (int c = 0; c < nf; ++c) a.out_feat[(size_t)ray * nf + c] = F[c];
 }
 
 }  // namespace
 
 cudaError_t ms_composite(const MsCompositeArgs &a, cudaStream_t s) {
   if (a.n_rays == 0) return cudaSuccess;
-  unsigned grid = (unsigned)((a.n_rays + 127) / 128);
+  const unsigned grid = (unsigned)((a.n_rays + CW - 1) / CW);
   const bool feat = a.n_feat > 0 && a.out_feat && a.staging_feat;
-  if (!feat) composite_kernel<0, false><<<grid, 128, 0, s>>>(a, 0, nullptr, nullptr, nullptr);
-  else if (a.n_feat == 32) composite_kernel<32, false><<<grid, 128, 0, s>>>(a, 0, nullptr, nullptr, nullptr);
-  else composite_kernel<-1, false><<<grid, 128, 0, s>>>(a, 0, nullptr, nullptr, nullptr);
+  if (!feat) composite_kernel<0><<<grid, CW * 32, 0, s>>>(a);
+  else composite_kernel<1><<<grid, CW * 32, 0, s>>>(a);
   MS_LAUNCHED();
   return cudaGetLastError();
 }
 
 cudaError_t ms_sample_order(const MsCompositeArgs &a, int ray, int *prim, int *k, float *t, cudaStream_t s) {
-  composite_kernel<0, true><<<1, 32, 0, s>>>(a, ray, prim, k, t);
+  sample_order_kernel<<<1, 32, 0, s>>>(a, ray, prim, k, t);
   MS_LAUNCHED();
   return cudaGetLastError();
 }

@@ -179,7 +179,6 @@ struct MsCompositeArgs {
   const MsHit *hits;
   const float4 *staging;
   const float *staging_feat;
-  float *cur_t;             // [n_hits] scratch
   float *out_rgb, *out_alpha, *out_feat;
 };
 cudaError_t ms_composite(const MsCompositeArgs &a, cudaStream_t s);
