@@ -15,9 +15,7 @@
 //   head           D[128 x NOUT] = h . Wh^T ; rgb = sigmoid, sigma = softplus, e = exp(-sigma delta)
 // Accumulators never leave TMEM between layers; activations never touch shared or global memory.
 //
-// Warp roles (320 threads): warp 0 weight loader + TMEM owner, warp 1 MMA issuer (one lane),
-// warps 2-5 and 6-9 two epilogue groups that ping-pong two row blocks so the tensor pipe works on
-// one block while the other is in its CUDA-core phase.  All hand-offs are mbarriers.
+// Warp roles and the pipeline are described above the kernel.
 #include <cuda_bf16.h>
 
 #include <vector>
@@ -26,9 +24,6 @@
 
 namespace {
 
-constexpr int TC_THREADS = 320;
-constexpr int TC_GROUP_THREADS = 128;
-constexpr uint32_t TC_MIN_SMEM = 116 * 1024;  // > half of the SM's shared memory: one CTA per SM (it owns all 512 TMEM columns)
 
 // ---------------------------------------------------------------------------------------------
 // PTX wrappers (validated one by one against a CPU GEMM on B200 before this kernel was written)
@@ -144,6 +139,11 @@ __host__ __device__ inline TcLayout tc_layout(int k1, int width, int nh, int nou
   return L;
 }
 
+// byte offset of layer l's W^T inside the image (l = nh: head) -- closed form of TcLayout::off_w
+__device__ __forceinline__ uint32_t tc_off_w(int k1, int width, int l) {
+  return l == 0 ? 0u : (uint32_t)(k1 * width * 2 + (l - 1) * width * width * 2);
+}
+
 struct TcParams {
   MsCam cam;
   int K, n_prims, in_dim, n_feat, nh, k1;
@@ -235,27 +235,71 @@ __device__ __forceinline__ void encode_row(const float *u, const float *d, uint8
   }
 }
 
-template <int NFREQ, int VIEWDIR, int WIDTH, int NOUT>
+// ---------------------------------------------------------------------------------------------
+// kernel
+// ---------------------------------------------------------------------------------------------
+// Warp roles (448 threads):
+//   warp 0       weight loader (one lane) + TMEM owner
+//   warp 1       MMA issuer (one lane)
+//   warps 2-5    FB group: encodes row blocks into the A1 ring (runs ahead of the tensor pipe) and,
+//                three blocks later, reads the head accumulator, applies sigmoid / softplus / exp
+//                and stores the sample
+//   warps 6-13   HE group: hidden-layer epilogue, D (fp32, TMEM) -> +bias, relu, bf16 -> A (TMEM);
+//                two warps per TMEM lane quarter, each on one half of the columns
+// NSLOT row blocks are in flight in the tensor pipe (slot s: D at column s*3W/2, A at +W); the head
+// accumulators live in NHS small regions after the slots, so a slot is released to the next block as
+// soon as its last hidden epilogue is done.  The MMA warp and the HE group walk the same static
+// round-robin schedule (visit v of slot s = layer v % nh of the slot's block v / nh); all hand-offs
+// are mbarriers, the tensor pipe completes in issue order.
+constexpr int TC_THREADS = 448;
+constexpr int TC_NA1 = 4;    // A1 ring stages
+constexpr int TC_LAG = 3;    // head epilogue of block i runs after the encode of block i + TC_LAG
+constexpr uint32_t TC_MIN_SMEM = 116 * 1024;  // > half of the SM's shared memory: one CTA per SM (it owns all 512 TMEM columns)
+
+struct __align__(16) TcMeta {  // per (A1 stage, row): what the head epilogue needs of the sample
+  float delta;
+  uint32_t slot;   // global hit index; sample k lives at staging[slot*K + k]
+  uint32_t k;      // 0xffffffff: padding row
+  uint32_t pad;
+};
+
+template <int NOUT> struct TcHeadSlots { static constexpr int value = NOUT <= 16 ? 4 : 2; };
+
+__device__ __forceinline__ void tmem_ld4(uint32_t taddr, uint32_t *r) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+               : "r"(taddr));
+}
+
+template <int NFREQ, int VIEWDIR, int WIDTH, int NOUT, int NSLOT>
 __global__ void __launch_bounds__(TC_THREADS, 1) mlp_tc_kernel(const TcParams p) {
   constexpr int K1 = ((3 + 6 * NFREQ + 3 * VIEWDIR) + 15) / 16 * 16;
+  constexpr int NHS = TcHeadSlots<NOUT>::value;
+  constexpr int SLOT_COLS = WIDTH + WIDTH / 2;
+  constexpr int HEAD_COL0 = NSLOT * SLOT_COLS;
+  static_assert(HEAD_COL0 + NHS * NOUT <= 512, "TMEM columns");
+  static_assert(TC_LAG <= TC_NA1 + NSLOT + NHS - 1 && TC_LAG >= NSLOT - 1, "pipeline depths (see DESIGN.md Sec.6)");
+  constexpr uint32_t A1_BYTES = MS_ROWS * K1 * 2;
   extern __shared__ __align__(1024) uint8_t smem[];
-  // [ weight image | A1[0] | A1[1] ]
-  __shared__ uint64_t bars[8];
+  // [ weight image | A1 ring | meta ring ]
+  __shared__ uint64_t bars[2 + 2 * TC_NA1 + 2 * NSLOT + 2 * NHS];
   __shared__ uint32_t tmem_base_s;
   const TcLayout L = tc_layout(K1, WIDTH, p.nh, NOUT);
   uint8_t *s_img = smem;
   uint8_t *s_a1 = smem + L.bytes;
-  constexpr uint32_t A1_BYTES = MS_ROWS * K1 * 2;
+  TcMeta *s_meta = reinterpret_cast<TcMeta *>(s_a1 + TC_NA1 * A1_BYTES);
   const uint32_t bar_w_full = smem_u32(&bars[0]), bar_w_free = smem_u32(&bars[1]);
-  const uint32_t bar_a_full0 = smem_u32(&bars[2]);  // [2], [3]
-  const uint32_t bar_d_full0 = smem_u32(&bars[4]);  // [4], [5]
+  const uint32_t bar_a1_full = smem_u32(&bars[2]), bar_a1_free = bar_a1_full + 8 * TC_NA1;
+  const uint32_t bar_d_full = bar_a1_free + 8 * TC_NA1, bar_a_ready = bar_d_full + 8 * NSLOT;
+  const uint32_t bar_h_full = bar_a_ready + 8 * NSLOT, bar_h_free = bar_h_full + 8 * NHS;
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   if (tid == 0) {
     mbar_init(bar_w_full, 1);
-    mbar_init(bar_w_free, 9);  // 8 epilogue warps + the MMA warp's commit
-    mbar_init(bar_a_full0, 4); mbar_init(bar_a_full0 + 8, 4);
-    mbar_init(bar_d_full0, 1); mbar_init(bar_d_full0 + 8, 1);
+    mbar_init(bar_w_free, 13);  // MMA commit + 8 HE warps + 4 FB warps
+    for (int i = 0; i < TC_NA1; ++i) { mbar_init(bar_a1_full + 8 * i, 4); mbar_init(bar_a1_free + 8 * i, 1); }
+    for (int i = 0; i < NSLOT; ++i) { mbar_init(bar_d_full + 8 * i, 1); mbar_init(bar_a_ready + 8 * i, 8); }
+    for (int i = 0; i < NHS; ++i) { mbar_init(bar_h_full + 8 * i, 1); mbar_init(bar_h_free + 8 * i, 4); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 0) {
@@ -288,165 +332,215 @@ __global__ void __launch_bounds__(TC_THREADS, 1) mlp_tc_kernel(const TcParams p)
     if (lane == 0) {
       SegWalk w(p.blk_off, p.n_prims, b0, b1);
       int prim; uint32_t first, count, seg = 0;
-      uint32_t pa[2] = {0, 0};
+      uint32_t run0 = 0;                 // running index of the segment's first block (ring positions)
+      uint32_t pa = 0;                   // bit s: parity of the next a_ready[s] completion
       const uint32_t idesc_w = umma_idesc(WIDTH), idesc_o = umma_idesc(NOUT);
       const uint32_t img = smem_u32(s_img);
       while (w.next(prim, first, count)) {
         mbar_wait(bar_w_full, seg & 1);
-        const uint32_t iters = (count + 1) >> 1;
-        for (uint32_t it = 0; it < iters; ++it) {
-          for (int l = 0; l <= nh; ++l) {
+        tc_fence_after();
+        const uint32_t maxv = ((count + NSLOT - 1) / NSLOT) * (uint32_t)nh;
+        for (uint32_t v = 0, j = 0, l = 0; v <= maxv; ++v) {
 #pragma unroll
-            for (int g = 0; g < 2; ++g) {
-              if (2 * it + g >= count) continue;
-              mbar_wait(bar_a_full0 + 8 * g, pa[g]);
-              pa[g] ^= 1;
-              tc_fence_after();
-              const uint32_t d_tmem = tmem + 256 * g;
-              const uint32_t a_tmem = tmem + 256 * g + 128;
-              if (l == 0) {
-                const uint32_t a1 = smem_u32(s_a1) + g * A1_BYTES;
+          for (int s = 0; s < NSLOT; ++s) {
+            const uint32_t n_s = (count + NSLOT - 1 - s) / NSLOT;
+            if (v > n_s * (uint32_t)nh) continue;
+            const uint32_t d_tmem = tmem + s * SLOT_COLS, a_tmem = d_tmem + WIDTH;
+            if (l == 0) {
+              if (j > 0) {  // head of the slot's previous block
+                const uint32_t run = run0 + (j - 1) * NSLOT + s, hs = run % NHS;
+                mbar_wait(bar_a_ready + 8 * s, (pa >> s) & 1u);
+                pa ^= 1u << s;
+                mbar_wait(bar_h_free + 8 * hs, ((run / NHS) & 1u) ^ 1u);
+                tc_fence_after();
 #pragma unroll
-                for (int j = 0; j < K1 / 16; ++j) {
-                  uint64_t da = umma_desc(a1 + j * 2 * (MS_ROWS * 16), MS_ROWS * 16, 128);
-                  uint64_t db = umma_desc(img + L.off_w[0] + j * 2 * (WIDTH * 16), WIDTH * 16, 128);
-                  mma_ss(d_tmem, da, db, idesc_w, j > 0);
+                for (int q = 0; q < WIDTH / 16; ++q) {
+                  uint64_t db = umma_desc(img + tc_off_w(K1, WIDTH, nh) + q * 2 * (NOUT * 16), NOUT * 16, 128);
+                  mma_ts(tmem + HEAD_COL0 + hs * NOUT, a_tmem + q * 8, db, idesc_o, q > 0);
                 }
-              } else if (l < nh) {
-#pragma unroll
-                for (int j = 0; j < WIDTH / 16; ++j) {
-                  uint64_t db = umma_desc(img + L.off_w[l] + j * 2 * (WIDTH * 16), WIDTH * 16, 128);
-                  mma_ts(d_tmem, a_tmem + j * 8, db, idesc_w, j > 0);
-                }
-              } else {
-#pragma unroll
-                for (int j = 0; j < WIDTH / 16; ++j) {
-                  uint64_t db = umma_desc(img + L.off_w[nh] + j * 2 * (NOUT * 16), NOUT * 16, 128);
-                  mma_ts(d_tmem, a_tmem + j * 8, db, idesc_o, j > 0);
-                }
+                mma_commit(bar_h_full + 8 * hs);
               }
-              mma_commit(bar_d_full0 + 8 * g);
+              if (j < n_s) {  // layer 1 of the slot's next block: A from the A1 ring
+                const uint32_t run = run0 + j * NSLOT + s, st = run % TC_NA1;
+                mbar_wait(bar_a1_full + 8 * st, (run / TC_NA1) & 1u);
+                tc_fence_after();
+                const uint32_t a1 = smem_u32(s_a1) + st * A1_BYTES;
+#pragma unroll
+                for (int q = 0; q < K1 / 16; ++q) {
+                  uint64_t da = umma_desc(a1 + q * 2 * (MS_ROWS * 16), MS_ROWS * 16, 128);
+                  uint64_t db = umma_desc(img + q * 2 * (WIDTH * 16), WIDTH * 16, 128);
+                  mma_ss(d_tmem, da, db, idesc_w, q > 0);
+                }
+                mma_commit(bar_a1_free + 8 * st);
+                mma_commit(bar_d_full + 8 * s);
+              }
+            } else {
+              mbar_wait(bar_a_ready + 8 * s, (pa >> s) & 1u);
+              pa ^= 1u << s;
+              tc_fence_after();
+#pragma unroll
+              for (int q = 0; q < WIDTH / 16; ++q) {
+                uint64_t db = umma_desc(img + tc_off_w(K1, WIDTH, (int)l) + q * 2 * (WIDTH * 16), WIDTH * 16, 128);
+                mma_ts(d_tmem, a_tmem + q * 8, db, idesc_w, q > 0);
+              }
+              mma_commit(bar_d_full + 8 * s);
             }
           }
+          if (++l == (uint32_t)nh) { l = 0; ++j; }
         }
         mma_commit(bar_w_free);  // arrives once every MMA of this segment has read its weights
+        run0 += count;
         ++seg;
       }
     }
-  } else {
-    // ===== epilogue groups: g = 0 (warps 2-5), g = 1 (warps 6-9) =====
-    const int g = (warp - 2) >> 2;
-    const int quarter = warp & 3;                  // TMEM lanes this warp may touch: 32*quarter .. +31
-    const int row = quarter * 32 + lane;           // sample row inside the block = TMEM lane
+  } else if (warp >= 6) {
+    // ===== HE group: hidden-layer epilogues =====
+    const int quarter = warp & 3;                 // TMEM lanes this warp may touch: 32*quarter .. +31
+    const int ch = (warp - 6) >> 2;               // column half
+    constexpr int HC = WIDTH / 2;                 // columns per warp
     const uint32_t lane_addr = (uint32_t)(quarter * 32) << 16;
-    const uint32_t d_tmem = tmem + 256 * g + lane_addr;
-    const uint32_t a_tmem = tmem + 256 * g + 128 + lane_addr;
-    const uint32_t bar_a = bar_a_full0 + 8 * g, bar_d = bar_d_full0 + 8 * g;
-    uint8_t *a1_row = s_a1 + g * A1_BYTES + row * 16;
-    const float *bias_s = reinterpret_cast<const float *>(s_img + L.off_bias);
-    uint32_t pd = 0;
+    const float *bias_s = reinterpret_cast<const float *>(s_img + L.off_bias) + ch * HC;
+    uint32_t pd = 0;                              // bit s: parity of the next d_full[s] completion
     SegWalk w(p.blk_off, p.n_prims, b0, b1);
     int prim; uint32_t first, count, seg = 0;
-    const uint32_t K = (uint32_t)p.K;
     while (w.next(prim, first, count)) {
-      mbar_wait(bar_w_full, seg & 1);              // biases live in the weight image
-      const uint32_t iv_first = p.prim_start[prim], iv_count = p.prim_start[prim + 1] - iv_first;
-      float Al[9], mu[3];
+      mbar_wait(bar_w_full, seg & 1);             // biases live in the weight image
+      const uint32_t maxv = ((count + NSLOT - 1) / NSLOT) * (uint32_t)nh;
+      for (uint32_t v = 0, l = 0; v < maxv; ++v) {
 #pragma unroll
-      for (int q = 0; q < 9; ++q) Al[q] = __ldg(p.A + 9 * (size_t)prim + q);
-#pragma unroll
-      for (int q = 0; q < 3; ++q) mu[q] = __ldg(p.center + 3 * (size_t)prim + q);
-      for (uint32_t i = (uint32_t)g; i < count; i += 2) {
-        // ---- stage 0: sample -> u -> encoding -> smem (A operand of layer 1) ----
-        const uint64_t s = (uint64_t)(first + i) * MS_ROWS + (uint32_t)row;
-        const uint32_t j = (uint32_t)(s / K);
-        const uint32_t k = (uint32_t)(s - (uint64_t)j * K);
-        const bool valid = j < iv_count;
-        float delta = 0.f;
-        size_t out_idx = 0;
-        {
-          float u[3] = {0.f, 0.f, 0.f}, d[3] = {0.f, 0.f, 0.f};
-          if (valid) {
-            const float4 *ivp = reinterpret_cast<const float4 *>(p.intervals + iv_first + j);
-            const float4 q0 = __ldg(ivp), q1 = __ldg(ivp + 1);
-            const float t = ms_sample_t(q0.y, q0.z, (int)k);
-            delta = q0.z;
-            out_idx = (size_t)(uint32_t)__float_as_int(q0.w) * K + k;
-            d[0] = q1.x; d[1] = q1.y; d[2] = q1.z;
-            ms_sample_u(Al, mu, p.cam.o, d, t, u);
-          }
-          encode_row<NFREQ, VIEWDIR, K1>(u, d, a1_row);
-        }
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        __syncwarp();
-        if (lane == 0) mbar_arrive(bar_a);
-        // ---- hidden layers: D -> +bias, relu, bf16 -> TMEM (A operand of the next layer) ----
-        for (int l = 0; l < nh; ++l) {
-          mbar_wait(bar_d, pd);
-          pd ^= 1;
+        for (int s = 0; s < NSLOT; ++s) {
+          const uint32_t n_s = (count + NSLOT - 1 - s) / NSLOT;
+          if (v >= n_s * (uint32_t)nh) continue;
+          const uint32_t d_tmem = tmem + s * SLOT_COLS + lane_addr + ch * HC;
+          const uint32_t a_tmem = tmem + s * SLOT_COLS + WIDTH + lane_addr + ch * (HC / 2);
+          const float4 *b4 = reinterpret_cast<const float4 *>(bias_s + l * WIDTH);
+          mbar_wait(bar_d_full + 8 * s, (pd >> s) & 1u);
+          pd ^= 1u << s;
           tc_fence_after();
-          const float *b = bias_s + l * WIDTH;
+          uint32_t r[HC];
 #pragma unroll
-          for (int c0 = 0; c0 < WIDTH; c0 += 32) {
-            uint32_t r[32], o[16];
-            tmem_ld32(d_tmem + c0, r);
-            tmem_ld_wait();
+          for (int c0 = 0; c0 < HC; c0 += 32) tmem_ld32(d_tmem + c0, r + c0);
+          tmem_ld_wait();
 #pragma unroll
-            for (int q = 0; q < 16; ++q) {
-              const float2 bb = *reinterpret_cast<const float2 *>(b + c0 + 2 * q);
-              o[q] = relu_pack_bf16(__uint_as_float(r[2 * q]) + bb.x, __uint_as_float(r[2 * q + 1]) + bb.y);
+          for (int c0 = 0; c0 < HC; c0 += 32) {
+            uint32_t o[16];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+              const float4 bb = b4[(c0 >> 2) + q];
+              o[2 * q] = relu_pack_bf16(__uint_as_float(r[c0 + 4 * q]) + bb.x, __uint_as_float(r[c0 + 4 * q + 1]) + bb.y);
+              o[2 * q + 1] = relu_pack_bf16(__uint_as_float(r[c0 + 4 * q + 2]) + bb.z, __uint_as_float(r[c0 + 4 * q + 3]) + bb.w);
             }
             tmem_st16(a_tmem + c0 / 2, o);
           }
           tmem_st_wait();
           tc_fence_before();
           __syncwarp();
-          if (lane == 0) mbar_arrive(bar_a);
+          if (lane == 0) mbar_arrive(bar_a_ready + 8 * s);
         }
-        // ---- head: raw -> rgb = sigmoid, sigma = softplus, e = exp(-sigma delta) ----
-        mbar_wait(bar_d, pd);
-        pd ^= 1;
-        tc_fence_after();
-        {
-          const float *b = bias_s + nh * WIDTH;
-          uint32_t r[16];
-          tmem_ld16(d_tmem, r);
-          tmem_ld_wait();
+        if (++l == (uint32_t)nh) l = 0;
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar_w_free);
+      ++seg;
+    }
+  } else {
+    // ===== FB group: encode (front) + head epilogue (back) =====
+    const int quarter = warp & 3;
+    const int row = quarter * 32 + lane;          // sample row inside the block = TMEM lane
+    const uint32_t lane_addr = (uint32_t)(quarter * 32) << 16;
+    const uint32_t K = (uint32_t)p.K;
+    const uint32_t dj = MS_ROWS / K, dk = MS_ROWS - dj * K;
+    uint32_t run0 = 0;
+    SegWalk w(p.blk_off, p.n_prims, b0, b1);
+    int prim; uint32_t first, count, seg = 0;
+    while (w.next(prim, first, count)) {
+      const uint32_t iv_first = p.prim_start[prim], iv_count = p.prim_start[prim + 1] - iv_first;
+      float Al[9], mu[3];
+#pragma unroll
+      for (int q = 0; q < 9; ++q) Al[q] = __ldg(p.A + 9 * (size_t)prim + q);
+#pragma unroll
+      for (int q = 0; q < 3; ++q) mu[q] = __ldg(p.center + 3 * (size_t)prim + q);
+      const float *bias_h = reinterpret_cast<const float *>(s_img + L.off_bias) + nh * WIDTH;
+      // interval index j and sample index k of this thread's row in block i; advanced by 128 samples per block
+      const uint64_t s0 = (uint64_t)first * MS_ROWS + (uint32_t)row;
+      uint32_t j = (uint32_t)(s0 / K), k = (uint32_t)(s0 - (uint64_t)j * K);
+      float4 q0 = make_float4(0.f, 0.f, 0.f, 0.f), q1 = q0;   // interval record of the block about to be encoded
+      if (j < iv_count) {
+        const float4 *ivp = reinterpret_cast<const float4 *>(p.intervals + iv_first + j);
+        q0 = __ldg(ivp); q1 = __ldg(ivp + 1);
+      }
+      for (uint32_t i = 0; i < count + TC_LAG; ++i) {
+        if (i < count) {
+          // ---- front: sample -> u -> encoding -> A1 ring ----
+          const uint32_t run = run0 + i, st = run % TC_NA1;
+          const bool valid = j < iv_count;
+          const float4 c0 = q0, c1 = q1;
+          const uint32_t kk = k;
+          // prefetch the next block's interval record
+          k += dk; j += dj;
+          if (k >= K) { k -= K; ++j; }
+          if (i + 1 < count && j < iv_count) {
+            const float4 *ivp = reinterpret_cast<const float4 *>(p.intervals + iv_first + j);
+            q0 = __ldg(ivp); q1 = __ldg(ivp + 1);
+          }
+          float u[3] = {0.f, 0.f, 0.f}, d[3] = {0.f, 0.f, 0.f};
+          TcMeta m;
+          m.delta = 0.f; m.slot = 0; m.k = 0xffffffffu; m.pad = 0;
           if (valid) {
-            const float r0 = __uint_as_float(r[0]) + b[0], r1 = __uint_as_float(r[1]) + b[1];
-            const float r2 = __uint_as_float(r[2]) + b[2], r3 = __uint_as_float(r[3]) + b[3];
+            const float t = ms_sample_t(c0.y, c0.z, (int)kk);
+            m.delta = c0.z; m.slot = (uint32_t)__float_as_int(c0.w); m.k = kk;
+            d[0] = c1.x; d[1] = c1.y; d[2] = c1.z;
+            ms_sample_u(Al, mu, p.cam.o, d, t, u);
+          }
+          mbar_wait(bar_a1_free + 8 * st, ((run / TC_NA1) & 1u) ^ 1u);
+          encode_row<NFREQ, VIEWDIR, K1>(u, d, s_a1 + st * A1_BYTES + row * 16);
+          s_meta[st * MS_ROWS + row] = m;
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+          __syncwarp();
+          if (lane == 0) mbar_arrive(bar_a1_full + 8 * st);
+        }
+        if (i >= TC_LAG) {
+          // ---- back: raw -> rgb = sigmoid, sigma = softplus, e = exp(-sigma delta) ----
+          const uint32_t run = run0 + i - TC_LAG, hs = run % NHS;
+          const TcMeta m = s_meta[(run % TC_NA1) * MS_ROWS + row];
+          if (i == TC_LAG) mbar_wait(bar_w_full, seg & 1);   // head biases live in the weight image
+          mbar_wait(bar_h_full + 8 * hs, (run / NHS) & 1u);
+          tc_fence_after();
+          const uint32_t h_tmem = tmem + HEAD_COL0 + hs * NOUT + lane_addr;
+          uint32_t r[NOUT];
+          if (NOUT <= 16 && p.staging_feat == nullptr) {
+            tmem_ld4(h_tmem, r);
+          } else {
+#pragma unroll
+            for (int c0 = 0; c0 < NOUT; c0 += 16) tmem_ld16(h_tmem + c0, r + c0);
+          }
+          tmem_ld_wait();
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(bar_h_free + 8 * hs);
+          if (m.k != 0xffffffffu) {
+            const size_t out_idx = (size_t)m.slot * K + m.k;
+            const float r0 = __uint_as_float(r[0]) + bias_h[0], r1 = __uint_as_float(r[1]) + bias_h[1];
+            const float r2 = __uint_as_float(r[2]) + bias_h[2], r3 = __uint_as_float(r[3]) + bias_h[3];
             float4 v;
             v.x = __fdividef(1.0f, 1.0f + __expf(-r0));
             v.y = __fdividef(1.0f, 1.0f + __expf(-r1));
             v.z = __fdividef(1.0f, 1.0f + __expf(-r2));
             const float sigma = fmaxf(r3, 0.0f) + __logf(1.0f + __expf(-fabsf(r3)));
-            v.w = __expf(-sigma * delta);
+            v.w = __expf(-sigma * m.delta);
             p.staging[out_idx] = v;
             if (p.staging_feat) {
               float *f = p.staging_feat + out_idx * (size_t)p.n_feat;
 #pragma unroll
-              for (int c = 4; c < 16; ++c)
-                if (c - 4 < p.n_feat) f[c - 4] = __uint_as_float(r[c]) + b[c];
-            }
-          }
-          if (NOUT > 16) {
-#pragma unroll
-            for (int c0 = 16; c0 < NOUT; c0 += 16) {
-              tmem_ld16(d_tmem + c0, r);
-              tmem_ld_wait();
-              if (valid && p.staging_feat) {
-                float *f = p.staging_feat + out_idx * (size_t)p.n_feat;
-#pragma unroll
-                for (int c = 0; c < 16; ++c)
-                  if (c0 + c - 4 < p.n_feat) f[c0 + c - 4] = __uint_as_float(r[c]) + b[c0 + c];
-              }
+              for (int c = 4; c < NOUT; ++c)
+                if (c - 4 < p.n_feat) f[c - 4] = __uint_as_float(r[c]) + bias_h[c];
             }
           }
         }
-        tc_fence_before();  // the next block's layer-1 MMA overwrites D: order our loads before the arrive
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(bar_w_free);
+      run0 += count;
       ++seg;
     }
   }
@@ -480,7 +574,7 @@ void pack_wT(const float *W, int in, int out, int k_pad, int n_pad, uint8_t *dst
 using KernelFn = void (*)(const TcParams);
 
 template <int NFREQ, int VIEWDIR, int WIDTH, int NOUT>
-KernelFn kernel_ptr() { return mlp_tc_kernel<NFREQ, VIEWDIR, WIDTH, NOUT>; }
+KernelFn kernel_ptr() { return mlp_tc_kernel<NFREQ, VIEWDIR, WIDTH, NOUT, 2>; }
 
 KernelFn select_kernel(int n_freq, int viewdir, int width, int nout) {
 #define MS_TC_CASE(F, V, W, O) \
@@ -559,7 +653,7 @@ cudaError_t ms_mlp_tc(const MsTcWeights &w, const MsMlpArgs &a, cudaStream_t s) 
   p.center = a.center; p.A = a.A; p.prim_start = a.prim_start; p.blk_off = a.blk_off; p.intervals = a.intervals;
   p.image = (const uint8_t *)w.image; p.image_bytes = (uint32_t)w.bytes_per_prim;
   p.staging = a.staging; p.staging_feat = a.staging_feat;
-  size_t smem = w.bytes_per_prim + 2 * (size_t)MS_ROWS * w.k1_pad * 2;
+  size_t smem = w.bytes_per_prim + TC_NA1 * ((size_t)MS_ROWS * w.k1_pad * 2 + MS_ROWS * sizeof(TcMeta));
   if (smem < TC_MIN_SMEM) smem = TC_MIN_SMEM;
   static int n_sm = 0;
   if (n_sm == 0) {
