@@ -8,15 +8,22 @@
 // the primitive changes (a handful of times per frame per CTA) -- one 1-D bulk async copy
 // (cp.async.bulk, mbarrier complete_tx) of a host-prepacked shared-memory image.
 //
-// Per row block:   x = posenc(u) (bf16, smem, K-major no-swizzle core-matrix layout)
-//   layer 1        D[128 x W]  = x . W1^T            tcgen05.mma SS  (A, B from shared memory)
-//   epilogue       h = relu(D + b) -> bf16 -> TMEM   tcgen05.ld / cvt.rn.relu.bf16x2 / tcgen05.st
-//   layers 2..NH   D = h . Wl^T                      tcgen05.mma TS  (A from tensor memory)
-//   head           D[128 x NOUT] = h . Wh^T ; rgb = sigmoid, sigma = softplus, e = exp(-sigma delta)
-// Accumulators never leave TMEM between layers; activations never touch shared or global memory.
+// Per row block:   x = [posenc(u), 1, 1] (bf16, smem, K-major no-swizzle core-matrix layout)
+//   layer 1        D[128 x W]  = x . [W1; b1_hi; b1_lo]^T      tcgen05.mma SS  (A, B from shared memory)
+//   epilogue       h = relu(D) -> bf16 -> TMEM                 tcgen05.ld / cvt.rn.relu.bf16x2 / tcgen05.st
+//   layers 2..NH   D = [h, 1, 1] . [Wl; bl_hi; bl_lo]^T        tcgen05.mma TS  (A from tensor memory)
+//   head           D[128 x NOUT] = [h, 1, 1] . [Wh; bh_hi; bh_lo]^T ; rgb = sigmoid, sigma = softplus,
+//                  e = exp(-sigma delta)
+// The bias rides in the contraction: every A operand carries two constant 1 columns and every
+// weight matrix two extra K rows holding the bias split into bf16 hi + lo parts (b = hi + lo to
+// 2^-17 relative; products with 1 are exact, accumulation is fp32), so the hidden epilogue is
+// load / relu-pack / store only.  Accumulators never leave TMEM between layers; activations
+// never touch shared or global memory.
 //
 // Warp roles and the pipeline are described above the kernel.
 #include <cuda_bf16.h>
+
+#include <string.h>
 
 #include <vector>
 
@@ -62,18 +69,28 @@ __device__ __forceinline__ uint64_t umma_desc(uint32_t addr, uint32_t lbo, uint3
 __host__ __device__ constexpr uint32_t umma_idesc(int n) {
   return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
 }
+// The MMA warp stays converged; one elected lane issues.  (Issued from a divergent `if (lane == 0)`
+// block, every tcgen05.mma costs ~95 cycles: ptxas wraps it in a per-lane R2UR loop.  Converged +
+// unrolled, the issue cost is ~20-30 cycles; measured on B200.)
 __device__ __forceinline__ void mma_ss(uint32_t d_tmem, uint64_t a, uint64_t b, uint32_t idesc, uint32_t acc) {
-  asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\ntcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n}\n" ::"r"(d_tmem),
-               "l"(a), "l"(b), "r"(idesc), "r"(acc)
-               : "memory");
+  asm volatile(
+      "{\n.reg .pred p, e;\nelect.sync _|e, 0xffffffff;\nsetp.ne.b32 p, %4, 0;\n"
+      "@e tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n}\n" ::"r"(d_tmem),
+      "l"(a), "l"(b), "r"(idesc), "r"(acc)
+      : "memory");
 }
 __device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b, uint32_t idesc, uint32_t acc) {
-  asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\ntcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n}\n" ::"r"(d_tmem),
-               "r"(a_tmem), "l"(b), "r"(idesc), "r"(acc)
-               : "memory");
+  asm volatile(
+      "{\n.reg .pred p, e;\nelect.sync _|e, 0xffffffff;\nsetp.ne.b32 p, %4, 0;\n"
+      "@e tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n}\n" ::"r"(d_tmem),
+      "r"(a_tmem), "l"(b), "r"(idesc), "r"(acc)
+      : "memory");
 }
 __device__ __forceinline__ void mma_commit(uint32_t bar) {
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+  asm volatile(
+      "{\n.reg .pred e;\nelect.sync _|e, 0xffffffff;\n"
+      "@e tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n}\n" ::"r"(bar)
+      : "memory");
 }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -104,6 +121,16 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t *r) {
       : "memory");
 }
 __device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t *r) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"r"(taddr), "r"(r[0]), "r"(r[1]),
+               "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])
+               : "memory");
+}
+__device__ __forceinline__ void tmem_ld4(uint32_t taddr, uint32_t *r) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+               : "r"(taddr));
+}
 
 // relu + round-to-nearest-even to bf16, two values per register: lo = element k, hi = element k+1
 __device__ __forceinline__ uint32_t relu_pack_bf16(float lo, float hi) {
@@ -117,42 +144,42 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
   return d;
 }
 
+
 // ---------------------------------------------------------------------------------------------
 // image layout (bytes), shared by the host packer and the kernel
 // ---------------------------------------------------------------------------------------------
+// Layer 0:  [W1; b1_hi; b1_lo; 0...]^T,  K = k1 = pad16(in_dim + 2), N = width
+// Layer l:  [Wl; bl_hi; bl_lo; 0...]^T,  K = width + 16,             N = width   (l = 1..nh-1)
+// Head:     [Wh; bh_hi; bh_lo; 0...]^T,  K = width + 16,             N = nout (padded)
+// Each as the UMMA B operand, K-major without swizzle: element (n, k) at 16-byte chunk (k/8) of an
+// [N rows x 16 B] slab, row n, position k%8.
 struct TcLayout {
-  int k1, width, nh, nout;
-  uint32_t off_w[6];   // W^T of layer l (l = 0..nh-1 hidden, nh = head)
-  uint32_t off_bias;   // fp32 biases: nh x width, then nout
+  uint32_t off_w[6];   // layer l (l = 0..nh-1 hidden, nh = head)
   uint32_t bytes;      // multiple of 128
 };
 
-__host__ __device__ inline TcLayout tc_layout(int k1, int width, int nh, int nout) {
-  TcLayout L;
-  L.k1 = k1; L.width = width; L.nh = nh; L.nout = nout;
-  uint32_t o = 0;
-  L.off_w[0] = o; o += (uint32_t)(k1 * width * 2);
-  for (int l = 1; l < nh; ++l) { L.off_w[l] = o; o += (uint32_t)(width * width * 2); }
-  L.off_w[nh] = o; o += (uint32_t)(nout * width * 2);
-  L.off_bias = o; o += (uint32_t)((nh * width + nout) * 4);
-  L.bytes = (o + 127u) & ~127u;
-  return L;
+__host__ __device__ constexpr uint32_t tc_off_w(int k1, int width, int l) {
+  return l == 0 ? 0u : (uint32_t)(k1 * width * 2 + (l - 1) * (width + 16) * width * 2);
+}
+__host__ __device__ constexpr uint32_t tc_image_bytes(int k1, int width, int nh, int nout) {
+  return (tc_off_w(k1, width, nh) + (uint32_t)((width + 16) * nout * 2) + 127u) & ~127u;
 }
 
-// byte offset of layer l's W^T inside the image (l = nh: head) -- closed form of TcLayout::off_w
-__device__ __forceinline__ uint32_t tc_off_w(int k1, int width, int l) {
-  return l == 0 ? 0u : (uint32_t)(k1 * width * 2 + (l - 1) * width * width * 2);
+inline TcLayout tc_layout(int k1, int width, int nh, int nout) {
+  TcLayout L;
+  for (int l = 0; l <= nh; ++l) L.off_w[l] = tc_off_w(k1, width, l);
+  L.bytes = tc_image_bytes(k1, width, nh, nout);
+  return L;
 }
 
 struct TcParams {
   MsCam cam;
-  int K, n_prims, in_dim, n_feat, nh, k1;
+  int K, n_prims, n_feat;
   uint32_t n_blocks;
   const float *center, *A;
   const uint32_t *prim_start, *blk_off;
   const MsInterval *intervals;
   const uint8_t *image;
-  uint32_t image_bytes;
   float4 *staging;
   float *staging_feat;
 };
@@ -166,7 +193,8 @@ __device__ __forceinline__ int find_prim(const uint32_t *__restrict__ blk_off, i
   return lo;
 }
 
-// Segment walk: the CTA's block range [b0, b1) cut at primitive boundaries.
+// Segment walk: the CTA's block range [b0, b1) cut at primitive boundaries.  Every role walks the
+// same segments (a pure function of blk_off), so no role has to tell another what comes next.
 struct SegWalk {
   const uint32_t *blk_off;
   uint32_t cur, b1;
@@ -192,13 +220,13 @@ struct SegWalk {
 };
 
 // positional encoding of one sample into K-major bf16 chunks (16 B each), Eq.5 with identity
-// first (Q3): [u, sin(2^l pi u) xyz, cos(2^l pi u) xyz]_l [, d].  sin/cos of level 0 from the SFU on
-// the exact product pi*u (|u| <= 1), higher levels by the double-angle recurrence in fp32; the
-// RESULT is rounded to bf16 (never the argument: S:H8).
+// first (Q3): [u, sin(2^l pi u) xyz, cos(2^l pi u) xyz]_l [, d], then the two bias columns (1, 1).
+// sin/cos of level 0 from the SFU on the exact product pi*u (|u| <= 1), higher levels by the
+// double-angle recurrence in fp32; the RESULT is rounded to bf16 (never the argument: S:H8).
 template <int NFREQ, int VIEWDIR, int K1>
 __device__ __forceinline__ void encode_row(const float *u, const float *d, uint8_t *dst_row /* + chunk*2048 */) {
   constexpr int IN = 3 + 6 * NFREQ + 3 * VIEWDIR;
-  static_assert(IN <= K1, "padded input too small");
+  static_assert(IN + 2 <= K1, "padded input too small");
   float x[K1];
 #pragma unroll
   for (int i = 0; i < K1; ++i) x[i] = 0.0f;
@@ -224,6 +252,7 @@ __device__ __forceinline__ void encode_row(const float *u, const float *d, uint8
   if (VIEWDIR) {
     x[3 + 6 * NFREQ + 0] = d[0]; x[3 + 6 * NFREQ + 1] = d[1]; x[3 + 6 * NFREQ + 2] = d[2];
   }
+  x[IN] = 1.0f; x[IN + 1] = 1.0f;   // bias columns
 #pragma unroll
   for (int ch = 0; ch < K1 / 8; ++ch) {
     uint4 v;
@@ -238,56 +267,43 @@ __device__ __forceinline__ void encode_row(const float *u, const float *d, uint8
 // ---------------------------------------------------------------------------------------------
 // kernel
 // ---------------------------------------------------------------------------------------------
-// Warp roles (448 threads):
+// Warp roles (576 threads, one CTA per SM):
 //   warp 0       weight loader (one lane) + TMEM owner
-//   warp 1       MMA issuer (one lane)
-//   warps 2-5    FB group: encodes row blocks into the A1 ring (runs ahead of the tensor pipe) and,
-//                three blocks later, reads the head accumulator, applies sigmoid / softplus / exp
-//                and stores the sample
-//   warps 6-13   HE group: hidden-layer epilogue, D (fp32, TMEM) -> +bias, relu, bf16 -> A (TMEM);
-//                two warps per TMEM lane quarter, each on one half of the columns
-// NSLOT row blocks are in flight in the tensor pipe (slot s: D at column s*3W/2, A at +W); the head
-// accumulators live in NHS small regions after the slots, so a slot is released to the next block as
-// soon as its last hidden epilogue is done.  The MMA warp and the HE group walk the same static
-// round-robin schedule (visit v of slot s = layer v % nh of the slot's block v / nh); all hand-offs
-// are mbarriers, the tensor pipe completes in issue order.
-constexpr int TC_THREADS = 448;
+//   warp 1       MMA issuer: converged warp, one elected lane issues (see mma_ss)
+//   warps 2-5    EN: sample -> u -> encoding -> A1 ring in shared memory (runs ahead of the tensor pipe)
+//   warps 6-9    HD: head accumulator -> sigmoid / softplus / exp -> staging store
+//   warps 10-17  HE: hidden-layer epilogue, D (fp32, TMEM) -> relu, bf16 -> A (TMEM); two warps per
+//                TMEM lane quarter, each on one half of the columns
+// Every role walks the same static schedule (SegWalk + the (j, layer, slot) loop nest below), so all
+// hand-offs are plain mbarriers: EN -a1_full-> MMA -d_full-> HE -a_ready-> MMA ... -h_full-> HD,
+// and back: MMA commit -a1_free-> EN, HD -h_free-> MMA.  NSLOT row blocks are in flight in the
+// tensor pipe (slot s: D at column s*SLOT_COLS, A at +W, the two constant 1 columns at +3W/2); the
+// head accumulators live in NHS small regions after the slots, so a slot is released to its next
+// block as soon as the block's head MMA is issued.  The tensor pipe completes in issue order.
+constexpr int TC_THREADS = 576;
 constexpr int TC_NA1 = 4;    // A1 ring stages
-constexpr int TC_LAG = 3;    // head epilogue of block i runs after the encode of block i + TC_LAG
 constexpr uint32_t TC_MIN_SMEM = 116 * 1024;  // > half of the SM's shared memory: one CTA per SM (it owns all 512 TMEM columns)
 
-struct __align__(16) TcMeta {  // per (A1 stage, row): what the head epilogue needs of the sample
-  float delta;
-  uint32_t slot;   // global hit index; sample k lives at staging[slot*K + k]
-  uint32_t k;      // 0xffffffff: padding row
-  uint32_t pad;
-};
-
 template <int NOUT> struct TcHeadSlots { static constexpr int value = NOUT <= 16 ? 4 : 2; };
+template <int WIDTH> struct TcSlots { static constexpr int value = WIDTH <= 64 ? 4 : 2; };
 
-__device__ __forceinline__ void tmem_ld4(uint32_t taddr, uint32_t *r) {
-  asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
-               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
-               : "r"(taddr));
-}
-
-template <int NFREQ, int VIEWDIR, int WIDTH, int NOUT, int NSLOT>
+template <int NFREQ, int VIEWDIR, int WIDTH, int NOUT, int NH>
 __global__ void __launch_bounds__(TC_THREADS, 1) mlp_tc_kernel(const TcParams p) {
-  constexpr int K1 = ((3 + 6 * NFREQ + 3 * VIEWDIR) + 15) / 16 * 16;
+  constexpr int IN = 3 + 6 * NFREQ + 3 * VIEWDIR;
+  constexpr int K1 = (IN + 2 + 15) / 16 * 16;
+  constexpr int NSLOT = TcSlots<WIDTH>::value;
   constexpr int NHS = TcHeadSlots<NOUT>::value;
-  constexpr int SLOT_COLS = WIDTH + WIDTH / 2;
+  constexpr int SLOT_COLS = WIDTH + WIDTH / 2 + 8;
   constexpr int HEAD_COL0 = NSLOT * SLOT_COLS;
   static_assert(HEAD_COL0 + NHS * NOUT <= 512, "TMEM columns");
-  static_assert(TC_LAG <= TC_NA1 + NSLOT + NHS - 1 && TC_LAG >= NSLOT - 1, "pipeline depths (see DESIGN.md Sec.6)");
   constexpr uint32_t A1_BYTES = MS_ROWS * K1 * 2;
+  constexpr uint32_t IMG_BYTES = tc_image_bytes(K1, WIDTH, NH, NOUT);
   extern __shared__ __align__(1024) uint8_t smem[];
-  // [ weight image | A1 ring | meta ring ]
+  // [ weight image | A1 ring ]
   __shared__ uint64_t bars[2 + 2 * TC_NA1 + 2 * NSLOT + 2 * NHS];
   __shared__ uint32_t tmem_base_s;
-  const TcLayout L = tc_layout(K1, WIDTH, p.nh, NOUT);
   uint8_t *s_img = smem;
-  uint8_t *s_a1 = smem + L.bytes;
-  TcMeta *s_meta = reinterpret_cast<TcMeta *>(s_a1 + TC_NA1 * A1_BYTES);
+  uint8_t *s_a1 = smem + IMG_BYTES;
   const uint32_t bar_w_full = smem_u32(&bars[0]), bar_w_free = smem_u32(&bars[1]);
   const uint32_t bar_a1_full = smem_u32(&bars[2]), bar_a1_free = bar_a1_full + 8 * TC_NA1;
   const uint32_t bar_d_full = bar_a1_free + 8 * TC_NA1, bar_a_ready = bar_d_full + 8 * NSLOT;
@@ -296,7 +312,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) mlp_tc_kernel(const TcParams p)
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   if (tid == 0) {
     mbar_init(bar_w_full, 1);
-    mbar_init(bar_w_free, 13);  // MMA commit + 8 HE warps + 4 FB warps
+    mbar_init(bar_w_free, 1);
     for (int i = 0; i < TC_NA1; ++i) { mbar_init(bar_a1_full + 8 * i, 4); mbar_init(bar_a1_free + 8 * i, 1); }
     for (int i = 0; i < NSLOT; ++i) { mbar_init(bar_d_full + 8 * i, 1); mbar_init(bar_a_ready + 8 * i, 8); }
     for (int i = 0; i < NHS; ++i) { mbar_init(bar_h_full + 8 * i, 1); mbar_init(bar_h_free + 8 * i, 4); }
@@ -310,10 +326,19 @@ __global__ void __launch_bounds__(TC_THREADS, 1) mlp_tc_kernel(const TcParams p)
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = tmem_base_s;
+  if (warp >= 10 && warp < 14) {  // the two constant 1 columns (bf16 pair 1,1 then zeros) of every slot's A operand
+    uint32_t ones[8] = {0x3f803f80u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
+#pragma unroll
+    for (int s = 0; s < NSLOT; ++s)
+      tmem_st8(tmem + s * SLOT_COLS + WIDTH + WIDTH / 2 + ((uint32_t)((warp & 3) * 32) << 16), ones);
+    tmem_st_wait();
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
 
   const uint32_t b0 = (uint32_t)(((uint64_t)p.n_blocks * blockIdx.x) / gridDim.x);
   const uint32_t b1 = (uint32_t)(((uint64_t)p.n_blocks * (blockIdx.x + 1)) / gridDim.x);
-  const int nh = p.nh;
 
   if (warp == 0) {
     // ===== weight loader: one bulk async copy per segment =====
@@ -322,41 +347,43 @@ __global__ void __launch_bounds__(TC_THREADS, 1) mlp_tc_kernel(const TcParams p)
       int prim; uint32_t first, count, seg = 0;
       while (w.next(prim, first, count)) {
         if (seg > 0) mbar_wait(bar_w_free, (seg - 1) & 1);
-        mbar_expect_tx(bar_w_full, p.image_bytes);
-        bulk_g2s(smem_u32(s_img), p.image + (size_t)prim * p.image_bytes, p.image_bytes, bar_w_full);
+        mbar_expect_tx(bar_w_full, IMG_BYTES);
+        bulk_g2s(smem_u32(s_img), p.image + (size_t)prim * IMG_BYTES, IMG_BYTES, bar_w_full);
         ++seg;
       }
     }
   } else if (warp == 1) {
-    // ===== MMA issuer =====
-    if (lane == 0) {
-      SegWalk w(p.blk_off, p.n_prims, b0, b1);
-      int prim; uint32_t first, count, seg = 0;
-      uint32_t run0 = 0;                 // running index of the segment's first block (ring positions)
-      uint32_t pa = 0;                   // bit s: parity of the next a_ready[s] completion
-      const uint32_t idesc_w = umma_idesc(WIDTH), idesc_o = umma_idesc(NOUT);
-      const uint32_t img = smem_u32(s_img);
-      while (w.next(prim, first, count)) {
-        mbar_wait(bar_w_full, seg & 1);
-        tc_fence_after();
-        const uint32_t maxv = ((count + NSLOT - 1) / NSLOT) * (uint32_t)nh;
-        for (uint32_t v = 0, j = 0, l = 0; v <= maxv; ++v) {
+    // ===== MMA issuer (all 32 lanes walk the schedule; mma_* elect one lane) =====
+    SegWalk w(p.blk_off, p.n_prims, b0, b1);
+    int prim; uint32_t first, count, seg = 0;
+    uint32_t run0 = 0;                 // running index of the segment's first block (ring positions)
+    uint32_t pa = 0;                   // bit s: parity of the next a_ready[s] completion
+    constexpr uint32_t idesc_w = umma_idesc(WIDTH), idesc_o = umma_idesc(NOUT);
+    const uint32_t img = smem_u32(s_img);
+    const uint32_t a1_base = smem_u32(s_a1);
+    while (w.next(prim, first, count)) {
+      mbar_wait(bar_w_full, seg & 1);
+      tc_fence_after();
+      const uint32_t jmax = (count + NSLOT - 1) / NSLOT;
+      for (uint32_t j = 0; j <= jmax; ++j) {
+#pragma unroll
+        for (int l = 0; l < NH; ++l) {
 #pragma unroll
           for (int s = 0; s < NSLOT; ++s) {
             const uint32_t n_s = (count + NSLOT - 1 - s) / NSLOT;
-            if (v > n_s * (uint32_t)nh) continue;
             const uint32_t d_tmem = tmem + s * SLOT_COLS, a_tmem = d_tmem + WIDTH;
             if (l == 0) {
-              if (j > 0) {  // head of the slot's previous block
+              if (j > 0 && j <= n_s) {  // head of the slot's previous block
                 const uint32_t run = run0 + (j - 1) * NSLOT + s, hs = run % NHS;
                 mbar_wait(bar_a_ready + 8 * s, (pa >> s) & 1u);
                 pa ^= 1u << s;
                 mbar_wait(bar_h_free + 8 * hs, ((run / NHS) & 1u) ^ 1u);
                 tc_fence_after();
+                const uint32_t h_tmem = tmem + HEAD_COL0 + hs * NOUT;
 #pragma unroll
-                for (int q = 0; q < WIDTH / 16; ++q) {
-                  uint64_t db = umma_desc(img + tc_off_w(K1, WIDTH, nh) + q * 2 * (NOUT * 16), NOUT * 16, 128);
-                  mma_ts(tmem + HEAD_COL0 + hs * NOUT, a_tmem + q * 8, db, idesc_o, q > 0);
+                for (int q = 0; q <= WIDTH / 16; ++q) {
+                  const uint64_t db = umma_desc(img + tc_off_w(K1, WIDTH, NH) + q * 2 * (NOUT * 16), NOUT * 16, 128);
+                  mma_ts(h_tmem, a_tmem + q * 8, db, idesc_o, q > 0);
                 }
                 mma_commit(bar_h_full + 8 * hs);
               }
@@ -364,87 +391,80 @@ __global__ void __launch_bounds__(TC_THREADS, 1) mlp_tc_kernel(const TcParams p)
                 const uint32_t run = run0 + j * NSLOT + s, st = run % TC_NA1;
                 mbar_wait(bar_a1_full + 8 * st, (run / TC_NA1) & 1u);
                 tc_fence_after();
-                const uint32_t a1 = smem_u32(s_a1) + st * A1_BYTES;
+                const uint32_t a1 = a1_base + st * A1_BYTES;
 #pragma unroll
                 for (int q = 0; q < K1 / 16; ++q) {
-                  uint64_t da = umma_desc(a1 + q * 2 * (MS_ROWS * 16), MS_ROWS * 16, 128);
-                  uint64_t db = umma_desc(img + q * 2 * (WIDTH * 16), WIDTH * 16, 128);
+                  const uint64_t da = umma_desc(a1 + q * 2 * (MS_ROWS * 16), MS_ROWS * 16, 128);
+                  const uint64_t db = umma_desc(img + q * 2 * (WIDTH * 16), WIDTH * 16, 128);
                   mma_ss(d_tmem, da, db, idesc_w, q > 0);
                 }
                 mma_commit(bar_a1_free + 8 * st);
                 mma_commit(bar_d_full + 8 * s);
               }
-            } else {
+            } else if (j < n_s) {
               mbar_wait(bar_a_ready + 8 * s, (pa >> s) & 1u);
               pa ^= 1u << s;
               tc_fence_after();
 #pragma unroll
-              for (int q = 0; q < WIDTH / 16; ++q) {
-                uint64_t db = umma_desc(img + tc_off_w(K1, WIDTH, (int)l) + q * 2 * (WIDTH * 16), WIDTH * 16, 128);
+              for (int q = 0; q <= WIDTH / 16; ++q) {
+                const uint64_t db = umma_desc(img + tc_off_w(K1, WIDTH, l) + q * 2 * (WIDTH * 16), WIDTH * 16, 128);
                 mma_ts(d_tmem, a_tmem + q * 8, db, idesc_w, q > 0);
               }
               mma_commit(bar_d_full + 8 * s);
             }
           }
-          if (++l == (uint32_t)nh) { l = 0; ++j; }
         }
-        mma_commit(bar_w_free);  // arrives once every MMA of this segment has read its weights
-        run0 += count;
-        ++seg;
+      }
+      mma_commit(bar_w_free);  // arrives once every MMA of this segment has read its weights
+      run0 += count;
+      ++seg;
+    }
+    if (seg > 0) mbar_wait(bar_w_free, (seg - 1) & 1);  // no asynchronous arrive may outlive the CTA
+  } else if (warp >= 10) {
+    // ===== HE: hidden-layer epilogues =====
+    const int quarter = warp & 3;                 // TMEM lanes this warp may touch: 32*quarter .. +31
+    const int ch = (warp - 10) >> 2;              // column half
+    constexpr int HC = WIDTH / 2;                 // columns per warp
+    const uint32_t lane_addr = (uint32_t)(quarter * 32) << 16;
+    uint32_t pd = 0;                              // bit s: parity of the next d_full[s] completion
+    SegWalk w(p.blk_off, p.n_prims, b0, b1);
+    int prim; uint32_t first, count;
+    while (w.next(prim, first, count)) {
+      const uint32_t jmax = (count + NSLOT - 1) / NSLOT;
+      for (uint32_t j = 0; j < jmax; ++j) {
+#pragma unroll 1
+        for (int l = 0; l < NH; ++l) {
+#pragma unroll
+          for (int s = 0; s < NSLOT; ++s) {
+            const uint32_t n_s = (count + NSLOT - 1 - s) / NSLOT;
+            if (j >= n_s) continue;
+            const uint32_t d_tmem = tmem + s * SLOT_COLS + lane_addr + ch * HC;
+            const uint32_t a_tmem = tmem + s * SLOT_COLS + WIDTH + lane_addr + ch * (HC / 2);
+            mbar_wait(bar_d_full + 8 * s, (pd >> s) & 1u);
+            pd ^= 1u << s;
+            tc_fence_after();
+            uint32_t r[HC];
+#pragma unroll
+            for (int c0 = 0; c0 < HC; c0 += 32) tmem_ld32(d_tmem + c0, r + c0);
+            tmem_ld_wait();
+#pragma unroll
+            for (int c0 = 0; c0 < HC; c0 += 32) {
+              uint32_t o[16];
+#pragma unroll
+              for (int q = 0; q < 16; ++q)
+                o[q] = relu_pack_bf16(__uint_as_float(r[c0 + 2 * q]), __uint_as_float(r[c0 + 2 * q + 1]));
+              tmem_st16(a_tmem + c0 / 2, o);
+            }
+            tmem_st_wait();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_a_ready + 8 * s);
+          }
+        }
       }
     }
   } else if (warp >= 6) {
-    // ===== HE group: hidden-layer epilogues =====
-    const int quarter = warp & 3;                 // TMEM lanes this warp may touch: 32*quarter .. +31
-    const int ch = (warp - 6) >> 2;               // column half
-    constexpr int HC = WIDTH / 2;                 // columns per warp
-    const uint32_t lane_addr = (uint32_t)(quarter * 32) << 16;
-    const float *bias_s = reinterpret_cast<const float *>(s_img + L.off_bias) + ch * HC;
-    uint32_t pd = 0;                              // bit s: parity of the next d_full[s] completion
-    SegWalk w(p.blk_off, p.n_prims, b0, b1);
-    int prim; uint32_t first, count, seg = 0;
-    while (w.next(prim, first, count)) {
-      mbar_wait(bar_w_full, seg & 1);             // biases live in the weight image
-      const uint32_t maxv = ((count + NSLOT - 1) / NSLOT) * (uint32_t)nh;
-      for (uint32_t v = 0, l = 0; v < maxv; ++v) {
-#pragma unroll
-        for (int s = 0; s < NSLOT; ++s) {
-          const uint32_t n_s = (count + NSLOT - 1 - s) / NSLOT;
-          if (v >= n_s * (uint32_t)nh) continue;
-          const uint32_t d_tmem = tmem + s * SLOT_COLS + lane_addr + ch * HC;
-          const uint32_t a_tmem = tmem + s * SLOT_COLS + WIDTH + lane_addr + ch * (HC / 2);
-          const float4 *b4 = reinterpret_cast<const float4 *>(bias_s + l * WIDTH);
-          mbar_wait(bar_d_full + 8 * s, (pd >> s) & 1u);
-          pd ^= 1u << s;
-          tc_fence_after();
-          uint32_t r[HC];
-#pragma unroll
-          for (int c0 = 0; c0 < HC; c0 += 32) tmem_ld32(d_tmem + c0, r + c0);
-          tmem_ld_wait();
-#pragma unroll
-          for (int c0 = 0; c0 < HC; c0 += 32) {
-            uint32_t o[16];
-#pragma unroll
-            for (int q = 0; q < 8; ++q) {
-              const float4 bb = b4[(c0 >> 2) + q];
-              o[2 * q] = relu_pack_bf16(__uint_as_float(r[c0 + 4 * q]) + bb.x, __uint_as_float(r[c0 + 4 * q + 1]) + bb.y);
-              o[2 * q + 1] = relu_pack_bf16(__uint_as_float(r[c0 + 4 * q + 2]) + bb.z, __uint_as_float(r[c0 + 4 * q + 3]) + bb.w);
-            }
-            tmem_st16(a_tmem + c0 / 2, o);
-          }
-          tmem_st_wait();
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive(bar_a_ready + 8 * s);
-        }
-        if (++l == (uint32_t)nh) l = 0;
-      }
-      __syncwarp();
-      if (lane == 0) mbar_arrive(bar_w_free);
-      ++seg;
-    }
-  } else {
-    // ===== FB group: encode (front) + head epilogue (back) =====
+    // ===== HD: head epilogue: raw -> rgb = sigmoid, sigma = softplus, e = exp(-sigma delta) =====
     const int quarter = warp & 3;
     const int row = quarter * 32 + lane;          // sample row inside the block = TMEM lane
     const uint32_t lane_addr = (uint32_t)(quarter * 32) << 16;
@@ -452,7 +472,77 @@ __global__ void __launch_bounds__(TC_THREADS, 1) mlp_tc_kernel(const TcParams p)
     const uint32_t dj = MS_ROWS / K, dk = MS_ROWS - dj * K;
     uint32_t run0 = 0;
     SegWalk w(p.blk_off, p.n_prims, b0, b1);
-    int prim; uint32_t first, count, seg = 0;
+    int prim; uint32_t first, count;
+    while (w.next(prim, first, count)) {
+      const uint32_t iv_first = p.prim_start[prim], iv_count = p.prim_start[prim + 1] - iv_first;
+      const uint64_t s0 = (uint64_t)first * MS_ROWS + (uint32_t)row;
+      uint32_t j = (uint32_t)(s0 / K), k = (uint32_t)(s0 - (uint64_t)j * K);
+      float4 q0 = make_float4(0.f, 0.f, 0.f, 0.f);   // (ray, t_in, delta, slot) of the row's interval
+      if (j < iv_count) q0 = __ldg(reinterpret_cast<const float4 *>(p.intervals + iv_first + j));
+      for (uint32_t i = 0; i < count; ++i) {
+        const uint32_t run = run0 + i, hs = run % NHS;
+        const bool valid = j < iv_count;
+        const float delta = q0.z;
+        const size_t out_idx = (size_t)(uint32_t)__float_as_int(q0.w) * K + k;
+        k += dk; j += dj;
+        if (k >= K) { k -= K; ++j; }
+        if (i + 1 < count && j < iv_count) q0 = __ldg(reinterpret_cast<const float4 *>(p.intervals + iv_first + j));
+        mbar_wait(bar_h_full + 8 * hs, (run / NHS) & 1u);
+        tc_fence_after();
+        const uint32_t h_tmem = tmem + HEAD_COL0 + hs * NOUT + lane_addr;
+        uint32_t r[NOUT > 16 ? 36 : 4];
+        const bool feat = NOUT > 16 && p.staging_feat != nullptr;
+        if constexpr (NOUT > 16) {
+          if (feat) {
+            tmem_ld16(h_tmem, r);
+            tmem_ld16(h_tmem + 16, r + 16);
+            tmem_ld4(h_tmem + 32, r + 32);
+          } else {
+            tmem_ld4(h_tmem, r);
+          }
+        } else {
+          tmem_ld4(h_tmem, r);
+        }
+        tmem_ld_wait();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_h_free + 8 * hs);
+        if (valid) {
+          const float r0 = __uint_as_float(r[0]), r1 = __uint_as_float(r[1]);
+          const float r2 = __uint_as_float(r[2]), r3 = __uint_as_float(r[3]);
+          float4 v;
+          v.x = __fdividef(1.0f, 1.0f + __expf(-r0));
+          v.y = __fdividef(1.0f, 1.0f + __expf(-r1));
+          v.z = __fdividef(1.0f, 1.0f + __expf(-r2));
+          const float sigma = fmaxf(r3, 0.0f) + __logf(1.0f + __expf(-fabsf(r3)));
+          v.w = __expf(-sigma * delta);
+          p.staging[out_idx] = v;
+          if constexpr (NOUT > 16) if (feat) {
+            float *f = p.staging_feat + out_idx * (size_t)p.n_feat;
+            if (p.n_feat == 32) {
+#pragma unroll
+              for (int c = 0; c < 8; ++c)
+                reinterpret_cast<float4 *>(f)[c] =
+                    make_float4(__uint_as_float(r[4 + 4 * c]), __uint_as_float(r[5 + 4 * c]),
+                                __uint_as_float(r[6 + 4 * c]), __uint_as_float(r[7 + 4 * c]));
+            } else {
+#pragma unroll
+              for (int c = 0; c < 32; ++c)
+                if (c < p.n_feat) f[c] = __uint_as_float(r[4 + c]);
+            }
+          }
+        }
+      }
+      run0 += count;
+    }
+  } else {
+    // ===== EN: sample -> u -> encoding -> A1 ring =====
+    const int row = (warp - 2) * 32 + lane;
+    const uint32_t K = (uint32_t)p.K;
+    const uint32_t dj = MS_ROWS / K, dk = MS_ROWS - dj * K;
+    uint32_t run0 = 0;
+    SegWalk w(p.blk_off, p.n_prims, b0, b1);
+    int prim; uint32_t first, count;
     while (w.next(prim, first, count)) {
       const uint32_t iv_first = p.prim_start[prim], iv_count = p.prim_start[prim + 1] - iv_first;
       float Al[9], mu[3];
@@ -460,7 +550,6 @@ __global__ void __launch_bounds__(TC_THREADS, 1) mlp_tc_kernel(const TcParams p)
       for (int q = 0; q < 9; ++q) Al[q] = __ldg(p.A + 9 * (size_t)prim + q);
 #pragma unroll
       for (int q = 0; q < 3; ++q) mu[q] = __ldg(p.center + 3 * (size_t)prim + q);
-      const float *bias_h = reinterpret_cast<const float *>(s_img + L.off_bias) + nh * WIDTH;
       // interval index j and sample index k of this thread's row in block i; advanced by 128 samples per block
       const uint64_t s0 = (uint64_t)first * MS_ROWS + (uint32_t)row;
       uint32_t j = (uint32_t)(s0 / K), k = (uint32_t)(s0 - (uint64_t)j * K);
@@ -469,79 +558,31 @@ __global__ void __launch_bounds__(TC_THREADS, 1) mlp_tc_kernel(const TcParams p)
         const float4 *ivp = reinterpret_cast<const float4 *>(p.intervals + iv_first + j);
         q0 = __ldg(ivp); q1 = __ldg(ivp + 1);
       }
-      for (uint32_t i = 0; i < count + TC_LAG; ++i) {
-        if (i < count) {
-          // ---- front: sample -> u -> encoding -> A1 ring ----
-          const uint32_t run = run0 + i, st = run % TC_NA1;
-          const bool valid = j < iv_count;
-          const float4 c0 = q0, c1 = q1;
-          const uint32_t kk = k;
-          // prefetch the next block's interval record
-          k += dk; j += dj;
-          if (k >= K) { k -= K; ++j; }
-          if (i + 1 < count && j < iv_count) {
-            const float4 *ivp = reinterpret_cast<const float4 *>(p.intervals + iv_first + j);
-            q0 = __ldg(ivp); q1 = __ldg(ivp + 1);
-          }
-          float u[3] = {0.f, 0.f, 0.f}, d[3] = {0.f, 0.f, 0.f};
-          TcMeta m;
-          m.delta = 0.f; m.slot = 0; m.k = 0xffffffffu; m.pad = 0;
-          if (valid) {
-            const float t = ms_sample_t(c0.y, c0.z, (int)kk);
-            m.delta = c0.z; m.slot = (uint32_t)__float_as_int(c0.w); m.k = kk;
-            d[0] = c1.x; d[1] = c1.y; d[2] = c1.z;
-            ms_sample_u(Al, mu, p.cam.o, d, t, u);
-          }
-          mbar_wait(bar_a1_free + 8 * st, ((run / TC_NA1) & 1u) ^ 1u);
-          encode_row<NFREQ, VIEWDIR, K1>(u, d, s_a1 + st * A1_BYTES + row * 16);
-          s_meta[st * MS_ROWS + row] = m;
-          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-          __syncwarp();
-          if (lane == 0) mbar_arrive(bar_a1_full + 8 * st);
+      for (uint32_t i = 0; i < count; ++i) {
+        const uint32_t run = run0 + i, st = run % TC_NA1;
+        const bool valid = j < iv_count;
+        const float4 c0 = q0, c1 = q1;
+        const uint32_t kk = k;
+        // prefetch the next block's interval record
+        k += dk; j += dj;
+        if (k >= K) { k -= K; ++j; }
+        if (i + 1 < count && j < iv_count) {
+          const float4 *ivp = reinterpret_cast<const float4 *>(p.intervals + iv_first + j);
+          q0 = __ldg(ivp); q1 = __ldg(ivp + 1);
         }
-        if (i >= TC_LAG) {
-          // ---- back: raw -> rgb = sigmoid, sigma = softplus, e = exp(-sigma delta) ----
-          const uint32_t run = run0 + i - TC_LAG, hs = run % NHS;
-          const TcMeta m = s_meta[(run % TC_NA1) * MS_ROWS + row];
-          if (i == TC_LAG) mbar_wait(bar_w_full, seg & 1);   // head biases live in the weight image
-          mbar_wait(bar_h_full + 8 * hs, (run / NHS) & 1u);
-          tc_fence_after();
-          const uint32_t h_tmem = tmem + HEAD_COL0 + hs * NOUT + lane_addr;
-          uint32_t r[NOUT];
-          if (NOUT <= 16 && p.staging_feat == nullptr) {
-            tmem_ld4(h_tmem, r);
-          } else {
-#pragma unroll
-            for (int c0 = 0; c0 < NOUT; c0 += 16) tmem_ld16(h_tmem + c0, r + c0);
-          }
-          tmem_ld_wait();
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive(bar_h_free + 8 * hs);
-          if (m.k != 0xffffffffu) {
-            const size_t out_idx = (size_t)m.slot * K + m.k;
-            const float r0 = __uint_as_float(r[0]) + bias_h[0], r1 = __uint_as_float(r[1]) + bias_h[1];
-            const float r2 = __uint_as_float(r[2]) + bias_h[2], r3 = __uint_as_float(r[3]) + bias_h[3];
-            float4 v;
-            v.x = __fdividef(1.0f, 1.0f + __expf(-r0));
-            v.y = __fdividef(1.0f, 1.0f + __expf(-r1));
-            v.z = __fdividef(1.0f, 1.0f + __expf(-r2));
-            const float sigma = fmaxf(r3, 0.0f) + __logf(1.0f + __expf(-fabsf(r3)));
-            v.w = __expf(-sigma * m.delta);
-            p.staging[out_idx] = v;
-            if (p.staging_feat) {
-              float *f = p.staging_feat + out_idx * (size_t)p.n_feat;
-#pragma unroll
-              for (int c = 4; c < NOUT; ++c)
-                if (c - 4 < p.n_feat) f[c - 4] = __uint_as_float(r[c]) + bias_h[c];
-            }
-          }
+        float u[3] = {0.f, 0.f, 0.f}, d[3] = {0.f, 0.f, 0.f};
+        if (valid) {
+          const float t = ms_sample_t(c0.y, c0.z, (int)kk);
+          d[0] = c1.x; d[1] = c1.y; d[2] = c1.z;
+          ms_sample_u(Al, mu, p.cam.o, d, t, u);
         }
+        mbar_wait(bar_a1_free + 8 * st, ((run / TC_NA1) & 1u) ^ 1u);
+        encode_row<NFREQ, VIEWDIR, K1>(u, d, s_a1 + st * A1_BYTES + row * 16);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_a1_full + 8 * st);
       }
-      __syncwarp();
-      if (lane == 0) mbar_arrive(bar_w_free);
       run0 += count;
-      ++seg;
     }
   }
   tc_fence_before();
@@ -552,56 +593,66 @@ __global__ void __launch_bounds__(TC_THREADS, 1) mlp_tc_kernel(const TcParams p)
 // ---------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------
-uint16_t bf16_bits(float f) {  // values are already bf16-representable (ms_api.cu rounds them)
+float bf16_round(float f) {  // RNE to a bf16-representable value
   uint32_t u;
   memcpy(&u, &f, 4);
+  if ((u & 0x7f800000u) == 0x7f800000u) return f;
   uint32_t lsb = (u >> 16) & 1u;
-  u += 0x7fffu + lsb;
+  u = (u + 0x7fffu + lsb) & 0xffff0000u;
+  memcpy(&f, &u, 4);
+  return f;
+}
+uint16_t bf16_bits(float f) {  // of a bf16-representable value
+  uint32_t u;
+  memcpy(&u, &f, 4);
   return (uint16_t)(u >> 16);
 }
 
-// W [in][out] row-major -> W^T as B operand: element (n = out, k = in) at chunk (k/8) slab
-// [rows x 16 B], row n, position k%8.
-void pack_wT(const float *W, int in, int out, int k_pad, int n_pad, uint8_t *dst) {
+// W [in][out] row-major and b [out] -> [W; b_hi; b_lo; 0]^T as B operand: element (n = out, k) at
+// chunk (k/8) slab [n_pad rows x 16 B], row n, position k%8.  Rows k = in, in+1 carry the bias.
+void pack_wT(const float *W, const float *b, int in, int out, int k_pad, int n_pad, uint8_t *dst) {
   uint16_t *d = reinterpret_cast<uint16_t *>(dst);
   for (int k = 0; k < k_pad; ++k)
     for (int n = 0; n < n_pad; ++n) {
-      float v = (k < in && n < out) ? W[(size_t)k * out + n] : 0.0f;
+      float v = 0.0f;
+      if (n < out) {
+        if (k < in) v = bf16_round(W[(size_t)k * out + n]);
+        else if (k == in) v = bf16_round(b[n]);
+        else if (k == in + 1) v = bf16_round(b[n] - bf16_round(b[n]));
+      }
       d[(size_t)(k / 8) * (n_pad * 8) + (size_t)n * 8 + (k % 8)] = bf16_bits(v);
     }
 }
 
 using KernelFn = void (*)(const TcParams);
 
-template <int NFREQ, int VIEWDIR, int WIDTH, int NOUT>
-KernelFn kernel_ptr() { return mlp_tc_kernel<NFREQ, VIEWDIR, WIDTH, NOUT, 2>; }
-
-KernelFn select_kernel(int n_freq, int viewdir, int width, int nout) {
-#define MS_TC_CASE(F, V, W, O) \
-  if (n_freq == F && viewdir == V && width == W && nout == O) return kernel_ptr<F, V, W, O>();
-  MS_TC_CASE(4, 0, 64, 16)
-  MS_TC_CASE(4, 1, 64, 16)
-  MS_TC_CASE(4, 1, 64, 48)
-  MS_TC_CASE(4, 0, 64, 48)
-  MS_TC_CASE(6, 0, 128, 16)
-  MS_TC_CASE(6, 1, 128, 16)
-  MS_TC_CASE(4, 0, 128, 16)
-  MS_TC_CASE(4, 1, 128, 16)
-  MS_TC_CASE(6, 0, 64, 16)
-  MS_TC_CASE(6, 0, 128, 48)
+KernelFn select_kernel(int n_freq, int viewdir, int width, int nout, int nh) {
+#define MS_TC_CASE(F, V, W, O, H) \
+  if (n_freq == F && viewdir == V && width == W && nout == O && nh == H) return mlp_tc_kernel<F, V, W, O, H>;
+  MS_TC_CASE(4, 0, 64, 16, 3)
+  MS_TC_CASE(4, 1, 64, 16, 3)
+  MS_TC_CASE(4, 1, 64, 48, 3)
+  MS_TC_CASE(4, 0, 64, 48, 3)
+  MS_TC_CASE(6, 0, 128, 16, 3)
+  MS_TC_CASE(6, 1, 128, 16, 3)
+  MS_TC_CASE(4, 0, 128, 16, 3)
+  MS_TC_CASE(4, 1, 128, 16, 3)
+  MS_TC_CASE(6, 0, 64, 16, 3)
+  MS_TC_CASE(4, 0, 64, 16, 2)
+  MS_TC_CASE(6, 0, 128, 16, 2)
 #undef MS_TC_CASE
   return nullptr;
 }
 
-int nout_pad(int out_dim) { return out_dim <= 16 ? 16 : (out_dim <= 48 ? 48 : 0); }
+int nout_pad(int out_dim) { return out_dim <= 16 ? 16 : (out_dim <= 36 ? 48 : 0); }
 
 }  // namespace
 
 int ms_tc_pack(const MsMlpShape &sh, int n_prims, const float *weights, MsTcWeights *out) {
   out->valid = false;
   const int nout = nout_pad(sh.out_dim);
-  if (nout == 0 || !select_kernel(sh.n_freq, sh.use_viewdir, sh.width, nout)) return MS_OK;  // shape not covered
-  const int k1 = (sh.in_dim + 15) / 16 * 16;
+  if (nout == 0 || !select_kernel(sh.n_freq, sh.use_viewdir, sh.width, nout, sh.n_hidden)) return MS_OK;  // shape not covered
+  const int k1 = (sh.in_dim + 2 + 15) / 16 * 16;
   const TcLayout L = tc_layout(k1, sh.width, sh.n_hidden, nout);
   std::vector<uint8_t> img;
   try {
@@ -612,14 +663,12 @@ int ms_tc_pack(const MsMlpShape &sh, int n_prims, const float *weights, MsTcWeig
   for (int i = 0; i < n_prims; ++i) {
     const float *w = weights + (size_t)i * sh.params;
     uint8_t *dst = img.data() + (size_t)i * L.bytes;
-    float *bias = reinterpret_cast<float *>(dst + L.off_bias);
     int in = sh.in_dim;
     for (int l = 0; l <= sh.n_hidden; ++l) {
       const bool last = l == sh.n_hidden;
       const int o = last ? sh.out_dim : sh.width;
-      pack_wT(w, in, o, l == 0 ? k1 : sh.width, last ? nout : sh.width, dst + L.off_w[l]);
       const float *b = w + (size_t)in * o;
-      for (int q = 0; q < o; ++q) bias[l * sh.width + q] = b[q];
+      pack_wT(w, b, in, o, l == 0 ? k1 : sh.width + 16, last ? nout : sh.width, dst + L.off_w[l]);
       w = b + o;
       in = o;
     }
@@ -645,15 +694,14 @@ void ms_tc_free(MsTcWeights *w) {
 cudaError_t ms_mlp_tc(const MsTcWeights &w, const MsMlpArgs &a, cudaStream_t s) {
   if (a.n_blocks == 0) return cudaSuccess;
   if (!w.valid) return cudaErrorNotSupported;
-  KernelFn fn = select_kernel(a.shape.n_freq, a.shape.use_viewdir, a.shape.width, w.n_out_pad);
+  KernelFn fn = select_kernel(a.shape.n_freq, a.shape.use_viewdir, a.shape.width, w.n_out_pad, a.shape.n_hidden);
   if (!fn) return cudaErrorNotSupported;
   TcParams p;
-  p.cam = a.cam; p.K = a.K; p.n_prims = a.n_prims; p.in_dim = a.shape.in_dim; p.n_feat = a.shape.n_feat;
-  p.nh = a.shape.n_hidden; p.k1 = w.k1_pad; p.n_blocks = a.n_blocks;
+  p.cam = a.cam; p.K = a.K; p.n_prims = a.n_prims; p.n_feat = a.shape.n_feat; p.n_blocks = a.n_blocks;
   p.center = a.center; p.A = a.A; p.prim_start = a.prim_start; p.blk_off = a.blk_off; p.intervals = a.intervals;
-  p.image = (const uint8_t *)w.image; p.image_bytes = (uint32_t)w.bytes_per_prim;
+  p.image = (const uint8_t *)w.image;
   p.staging = a.staging; p.staging_feat = a.staging_feat;
-  size_t smem = w.bytes_per_prim + TC_NA1 * ((size_t)MS_ROWS * w.k1_pad * 2 + MS_ROWS * sizeof(TcMeta));
+  size_t smem = w.bytes_per_prim + TC_NA1 * ((size_t)MS_ROWS * w.k1_pad * 2);
   if (smem < TC_MIN_SMEM) smem = TC_MIN_SMEM;
   static int n_sm = 0;
   if (n_sm == 0) {
