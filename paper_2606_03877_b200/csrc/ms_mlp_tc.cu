@@ -267,32 +267,39 @@ __device__ __forceinline__ void encode_row(const float *u, const float *d, uint8
 // ---------------------------------------------------------------------------------------------
 // kernel
 // ---------------------------------------------------------------------------------------------
-// Warp roles (576 threads, one CTA per SM):
-//   warp 0       weight loader (one lane) + TMEM owner
-//   warp 1       MMA issuer: converged warp, one elected lane issues (see mma_ss)
-//   warps 2-5    EN: sample -> u -> encoding -> A1 ring in shared memory (runs ahead of the tensor pipe)
-//   warps 6-9    HD: head accumulator -> sigmoid / softplus / exp -> staging store
-//   warps 10-17  HE: hidden-layer epilogue, D (fp32, TMEM) -> relu, bf16 -> A (TMEM); two warps per
-//                TMEM lane quarter, each on one half of the columns
-// Every role walks the same static schedule (SegWalk + the (j, layer, slot) loop nest below), so all
+// Warp roles (17 + NSLOT warps, one CTA per SM):
+//   warp 0            weight loader (one lane) + TMEM owner
+//   warps 1..NSLOT    MMA issuers, one per slot: a converged warp, one elected lane issues (see mma_ss).
+//                     One warp per slot because the issue path is latency-bound: ~45 cycles per
+//                     tcgen05.mma (four R2UR each) and ~90 per mbarrier try_wait, 30 MMAs and 6 waits
+//                     per block -- more than the 1416 tensor cycles the block needs
+//   next 4 warps      EN: sample -> u -> encoding -> A1 ring in shared memory (runs ahead of the tensor pipe)
+//   next 4 warps      HD: head accumulator -> sigmoid / softplus / exp -> staging store
+//   last 8 warps      HE: hidden-layer epilogue, D (fp32, TMEM) -> relu, bf16 -> A (TMEM); two warps per
+//                     TMEM lane quarter, each on one half of the columns
+// Every role walks the same static schedule (SegWalk; block i of a segment runs in slot i % NSLOT), so all
 // hand-offs are plain mbarriers: EN -a1_full-> MMA -d_full-> HE -a_ready-> MMA ... -h_full-> HD,
 // and back: MMA commit -a1_free-> EN, HD -h_free-> MMA.  NSLOT row blocks are in flight in the
 // tensor pipe (slot s: D at column s*SLOT_COLS, A at +W, the two constant 1 columns at +3W/2); the
-// head accumulators live in NHS small regions after the slots, so a slot is released to its next
-// block as soon as the block's head MMA is issued.  The tensor pipe completes in issue order.
-constexpr int TC_THREADS = 576;
+// head accumulators live in HPS small regions per slot after the slots (private to the slot's MMA
+// warp, so every mbarrier has one producer and one consumer walking it in order), and a slot is
+// released to its next block as soon as the block's head MMA is issued.  The tensor pipe completes in issue order.
+constexpr int TC_WARPS_FIXED = 1 + 4 + 4 + 8;   // loader, EN, HD, HE; plus one MMA warp per slot
 constexpr int TC_NA1 = 4;    // A1 ring stages
 constexpr uint32_t TC_MIN_SMEM = 116 * 1024;  // > half of the SM's shared memory: one CTA per SM (it owns all 512 TMEM columns)
 
-template <int NOUT> struct TcHeadSlots { static constexpr int value = NOUT <= 16 ? 4 : 2; };
-template <int WIDTH> struct TcSlots { static constexpr int value = WIDTH <= 64 ? 4 : 2; };
+// slots in flight and head accumulator regions per slot, fitted to the 512 TMEM columns
+__host__ __device__ constexpr int tc_slots(int width, int nout) { return width > 64 ? 2 : (nout <= 16 ? 4 : 3); }
+__host__ __device__ constexpr int tc_heads_per_slot(int width) { return width > 64 ? 2 : 1; }
 
 template <int NFREQ, int VIEWDIR, int WIDTH, int NOUT, int NH>
-__global__ void __launch_bounds__(TC_THREADS, 1) mlp_tc_kernel(const TcParams p) {
+__global__ void __launch_bounds__(32 * (TC_WARPS_FIXED + tc_slots(WIDTH, NOUT)), 1) mlp_tc_kernel(const TcParams p) {
   constexpr int IN = 3 + 6 * NFREQ + 3 * VIEWDIR;
   constexpr int K1 = (IN + 2 + 15) / 16 * 16;
-  constexpr int NSLOT = TcSlots<WIDTH>::value;
-  constexpr int NHS = TcHeadSlots<NOUT>::value;
+  constexpr int NSLOT = tc_slots(WIDTH, NOUT);
+  constexpr int HPS = tc_heads_per_slot(WIDTH);   // head regions per slot (private to the slot's MMA warp)
+  constexpr int NHS = NSLOT * HPS;
+  constexpr int W_EN = 1 + NSLOT, W_HD = W_EN + 4, W_HE = W_HD + 4;   // first warp of each group
   constexpr int SLOT_COLS = WIDTH + WIDTH / 2 + 8;
   constexpr int HEAD_COL0 = NSLOT * SLOT_COLS;
   static_assert(HEAD_COL0 + NHS * NOUT <= 512, "TMEM columns");
@@ -312,7 +319,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) mlp_tc_kernel(const TcParams p)
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   if (tid == 0) {
     mbar_init(bar_w_full, 1);
-    mbar_init(bar_w_free, 1);
+    mbar_init(bar_w_free, NSLOT);
     for (int i = 0; i < TC_NA1; ++i) { mbar_init(bar_a1_full + 8 * i, 4); mbar_init(bar_a1_free + 8 * i, 1); }
     for (int i = 0; i < NSLOT; ++i) { mbar_init(bar_d_full + 8 * i, 1); mbar_init(bar_a_ready + 8 * i, 8); }
     for (int i = 0; i < NHS; ++i) { mbar_init(bar_h_full + 8 * i, 1); mbar_init(bar_h_free + 8 * i, 4); }
@@ -326,7 +333,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) mlp_tc_kernel(const TcParams p)
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = tmem_base_s;
-  if (warp >= 10 && warp < 14) {  // the two constant 1 columns (bf16 pair 1,1 then zeros) of every slot's A operand
+  if (warp >= W_HE && warp < W_HE + 4) {  // the two constant 1 columns (bf16 pair 1,1 then zeros) of every slot's A operand
     uint32_t ones[8] = {0x3f803f80u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
 #pragma unroll
     for (int s = 0; s < NSLOT; ++s)
@@ -352,78 +359,76 @@ __global__ void __launch_bounds__(TC_THREADS, 1) mlp_tc_kernel(const TcParams p)
         ++seg;
       }
     }
-  } else if (warp == 1) {
-    // ===== MMA issuer (all 32 lanes walk the schedule; mma_* elect one lane) =====
+  } else if (warp <= NSLOT) {
+    // ===== MMA issuer of slot s = warp - 1 (all 32 lanes walk the schedule; mma_* elect one lane) =====
+    const int s = warp - 1;
     SegWalk w(p.blk_off, p.n_prims, b0, b1);
     int prim; uint32_t first, count, seg = 0;
     uint32_t run0 = 0;                 // running index of the segment's first block (ring positions)
-    uint32_t pa = 0;                   // bit s: parity of the next a_ready[s] completion
+    uint32_t pa = 0;                   // parity of the next a_ready[s] completion
+    uint32_t cnt = 0;                  // heads this warp has issued: head region s*HPS + cnt%HPS, use cnt/HPS
     constexpr uint32_t idesc_w = umma_idesc(WIDTH), idesc_o = umma_idesc(NOUT);
     const uint32_t img = smem_u32(s_img);
     const uint32_t a1_base = smem_u32(s_a1);
+    const uint32_t d_tmem = tmem + s * SLOT_COLS, a_tmem = d_tmem + WIDTH;
+    const uint32_t bar_a_ready_s = bar_a_ready + 8 * s, bar_d_full_s = bar_d_full + 8 * s;
     while (w.next(prim, first, count)) {
       mbar_wait(bar_w_full, seg & 1);
       tc_fence_after();
-      const uint32_t jmax = (count + NSLOT - 1) / NSLOT;
-      for (uint32_t j = 0; j <= jmax; ++j) {
+      const uint32_t n_s = (count + NSLOT - 1 - s) / NSLOT;   // blocks of this segment that run in slot s
+      for (uint32_t j = 0; j <= n_s; ++j) {
+        if (j > 0) {  // head of the slot's previous block
+          const uint32_t hs = s * HPS + cnt % HPS;
+          mbar_wait(bar_a_ready_s, pa);
+          pa ^= 1u;
+          mbar_wait(bar_h_free + 8 * hs, ((cnt / HPS) & 1u) ^ 1u);
+          ++cnt;
+          tc_fence_after();
+          const uint32_t h_tmem = tmem + HEAD_COL0 + hs * NOUT;
 #pragma unroll
-        for (int l = 0; l < NH; ++l) {
-#pragma unroll
-          for (int s = 0; s < NSLOT; ++s) {
-            const uint32_t n_s = (count + NSLOT - 1 - s) / NSLOT;
-            const uint32_t d_tmem = tmem + s * SLOT_COLS, a_tmem = d_tmem + WIDTH;
-            if (l == 0) {
-              if (j > 0 && j <= n_s) {  // head of the slot's previous block
-                const uint32_t run = run0 + (j - 1) * NSLOT + s, hs = run % NHS;
-                mbar_wait(bar_a_ready + 8 * s, (pa >> s) & 1u);
-                pa ^= 1u << s;
-                mbar_wait(bar_h_free + 8 * hs, ((run / NHS) & 1u) ^ 1u);
-                tc_fence_after();
-                const uint32_t h_tmem = tmem + HEAD_COL0 + hs * NOUT;
-#pragma unroll
-                for (int q = 0; q <= WIDTH / 16; ++q) {
-                  const uint64_t db = umma_desc(img + tc_off_w(K1, WIDTH, NH) + q * 2 * (NOUT * 16), NOUT * 16, 128);
-                  mma_ts(h_tmem, a_tmem + q * 8, db, idesc_o, q > 0);
-                }
-                mma_commit(bar_h_full + 8 * hs);
-              }
-              if (j < n_s) {  // layer 1 of the slot's next block: A from the A1 ring
-                const uint32_t run = run0 + j * NSLOT + s, st = run % TC_NA1;
-                mbar_wait(bar_a1_full + 8 * st, (run / TC_NA1) & 1u);
-                tc_fence_after();
-                const uint32_t a1 = a1_base + st * A1_BYTES;
-#pragma unroll
-                for (int q = 0; q < K1 / 16; ++q) {
-                  const uint64_t da = umma_desc(a1 + q * 2 * (MS_ROWS * 16), MS_ROWS * 16, 128);
-                  const uint64_t db = umma_desc(img + q * 2 * (WIDTH * 16), WIDTH * 16, 128);
-                  mma_ss(d_tmem, da, db, idesc_w, q > 0);
-                }
-                mma_commit(bar_a1_free + 8 * st);
-                mma_commit(bar_d_full + 8 * s);
-              }
-            } else if (j < n_s) {
-              mbar_wait(bar_a_ready + 8 * s, (pa >> s) & 1u);
-              pa ^= 1u << s;
-              tc_fence_after();
-#pragma unroll
-              for (int q = 0; q <= WIDTH / 16; ++q) {
-                const uint64_t db = umma_desc(img + tc_off_w(K1, WIDTH, l) + q * 2 * (WIDTH * 16), WIDTH * 16, 128);
-                mma_ts(d_tmem, a_tmem + q * 8, db, idesc_w, q > 0);
-              }
-              mma_commit(bar_d_full + 8 * s);
-            }
+          for (int q = 0; q <= WIDTH / 16; ++q) {
+            const uint64_t db = umma_desc(img + tc_off_w(K1, WIDTH, NH) + q * 2 * (NOUT * 16), NOUT * 16, 128);
+            mma_ts(h_tmem, a_tmem + q * 8, db, idesc_o, q > 0);
           }
+          mma_commit(bar_h_full + 8 * hs);
+        }
+        if (j == n_s) break;
+        {  // layer 1 of the slot's next block: A from the A1 ring
+          const uint32_t run = run0 + j * NSLOT + s, st = run % TC_NA1;
+          mbar_wait(bar_a1_full + 8 * st, (run / TC_NA1) & 1u);
+          tc_fence_after();
+          const uint32_t a1 = a1_base + st * A1_BYTES;
+#pragma unroll
+          for (int q = 0; q < K1 / 16; ++q) {
+            const uint64_t da = umma_desc(a1 + q * 2 * (MS_ROWS * 16), MS_ROWS * 16, 128);
+            const uint64_t db = umma_desc(img + q * 2 * (WIDTH * 16), WIDTH * 16, 128);
+            mma_ss(d_tmem, da, db, idesc_w, q > 0);
+          }
+          mma_commit(bar_a1_free + 8 * st);
+          mma_commit(bar_d_full_s);
+        }
+#pragma unroll
+        for (int l = 1; l < NH; ++l) {
+          mbar_wait(bar_a_ready_s, pa);
+          pa ^= 1u;
+          tc_fence_after();
+#pragma unroll
+          for (int q = 0; q <= WIDTH / 16; ++q) {
+            const uint64_t db = umma_desc(img + tc_off_w(K1, WIDTH, l) + q * 2 * (WIDTH * 16), WIDTH * 16, 128);
+            mma_ts(d_tmem, a_tmem + q * 8, db, idesc_w, q > 0);
+          }
+          mma_commit(bar_d_full_s);
         }
       }
-      mma_commit(bar_w_free);  // arrives once every MMA of this segment has read its weights
+      mma_commit(bar_w_free);  // arrives once every MMA this warp issued in the segment has read its weights
       run0 += count;
       ++seg;
     }
     if (seg > 0) mbar_wait(bar_w_free, (seg - 1) & 1);  // no asynchronous arrive may outlive the CTA
-  } else if (warp >= 10) {
+  } else if (warp >= W_HE) {
     // ===== HE: hidden-layer epilogues =====
     const int quarter = warp & 3;                 // TMEM lanes this warp may touch: 32*quarter .. +31
-    const int ch = (warp - 10) >> 2;              // column half
+    const int ch = (warp - W_HE) >> 2;              // column half
     constexpr int HC = WIDTH / 2;                 // columns per warp
     const uint32_t lane_addr = (uint32_t)(quarter * 32) << 16;
     uint32_t pd = 0;                              // bit s: parity of the next d_full[s] completion
@@ -463,14 +468,16 @@ __global__ void __launch_bounds__(TC_THREADS, 1) mlp_tc_kernel(const TcParams p)
         }
       }
     }
-  } else if (warp >= 6) {
+  } else if (warp >= W_HD) {
     // ===== HD: head epilogue: raw -> rgb = sigmoid, sigma = softplus, e = exp(-sigma delta) =====
     const int quarter = warp & 3;
     const int row = quarter * 32 + lane;          // sample row inside the block = TMEM lane
     const uint32_t lane_addr = (uint32_t)(quarter * 32) << 16;
     const uint32_t K = (uint32_t)p.K;
     const uint32_t dj = MS_ROWS / K, dk = MS_ROWS - dj * K;
-    uint32_t run0 = 0;
+    uint32_t cum[NSLOT];                          // blocks each slot has taken in earlier segments
+#pragma unroll
+    for (int s = 0; s < NSLOT; ++s) cum[s] = 0;
     SegWalk w(p.blk_off, p.n_prims, b0, b1);
     int prim; uint32_t first, count;
     while (w.next(prim, first, count)) {
@@ -480,14 +487,18 @@ __global__ void __launch_bounds__(TC_THREADS, 1) mlp_tc_kernel(const TcParams p)
       float4 q0 = make_float4(0.f, 0.f, 0.f, 0.f);   // (ray, t_in, delta, slot) of the row's interval
       if (j < iv_count) q0 = __ldg(reinterpret_cast<const float4 *>(p.intervals + iv_first + j));
       for (uint32_t i = 0; i < count; ++i) {
-        const uint32_t run = run0 + i, hs = run % NHS;
+        const uint32_t slot = i % NSLOT;
+        uint32_t cnt = i / NSLOT;                   // the slot's head counter for this block (see the MMA warp)
+#pragma unroll
+        for (int s = 0; s < NSLOT; ++s) cnt += slot == (uint32_t)s ? cum[s] : 0u;
+        const uint32_t hs = slot * HPS + cnt % HPS;
         const bool valid = j < iv_count;
         const float delta = q0.z;
         const size_t out_idx = (size_t)(uint32_t)__float_as_int(q0.w) * K + k;
         k += dk; j += dj;
         if (k >= K) { k -= K; ++j; }
         if (i + 1 < count && j < iv_count) q0 = __ldg(reinterpret_cast<const float4 *>(p.intervals + iv_first + j));
-        mbar_wait(bar_h_full + 8 * hs, (run / NHS) & 1u);
+        mbar_wait(bar_h_full + 8 * hs, (cnt / HPS) & 1u);
         tc_fence_after();
         const uint32_t h_tmem = tmem + HEAD_COL0 + hs * NOUT + lane_addr;
         uint32_t r[NOUT > 16 ? 36 : 4];
@@ -533,11 +544,12 @@ __global__ void __launch_bounds__(TC_THREADS, 1) mlp_tc_kernel(const TcParams p)
           }
         }
       }
-      run0 += count;
+#pragma unroll
+      for (int s = 0; s < NSLOT; ++s) cum[s] += (count + NSLOT - 1 - s) / NSLOT;
     }
   } else {
     // ===== EN: sample -> u -> encoding -> A1 ring =====
-    const int row = (warp - 2) * 32 + lane;
+    const int row = (warp - W_EN) * 32 + lane;
     const uint32_t K = (uint32_t)p.K;
     const uint32_t dj = MS_ROWS / K, dk = MS_ROWS - dj * K;
     uint32_t run0 = 0;
@@ -712,7 +724,8 @@ cudaError_t ms_mlp_tc(const MsTcWeights &w, const MsMlpArgs &a, cudaStream_t s) 
   cudaError_t e = cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   unsigned grid = a.n_blocks < (uint32_t)n_sm ? a.n_blocks : (unsigned)n_sm;
-  fn<<<grid, TC_THREADS, smem, s>>>(p);
+  const int threads = 32 * (TC_WARPS_FIXED + tc_slots(a.shape.width, w.n_out_pad));
+  fn<<<grid, threads, smem, s>>>(p);
   MS_LAUNCHED();
   return cudaGetLastError();
 }
