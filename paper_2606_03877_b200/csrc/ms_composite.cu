@@ -34,12 +34,15 @@ __device__ __forceinline__ uint32_t count_before(float tf, float tl, float ti2, 
   const bool tie_lt = p2 < prim;
   if (!precedes(tf, t, tie_lt)) return 0u;
   if (precedes(tl, t, tie_lt)) return (uint32_t)K;
-  int lo = 0, hi = K - 1;  // precedes(lo) holds, precedes(hi) does not
-  while (hi - lo > 1) {
-    const int mid = (lo + hi) >> 1;
-    if (precedes(ms_sample_t(ti2, dl2, mid), t, tie_lt)) lo = mid; else hi = mid;
-  }
-  return (uint32_t)hi;
+  // precedes(sample 0) holds, precedes(sample K-1) does not: the count c is in [1, K-1].  The stream
+  // is an arithmetic progression, so c ~ (t - t_in2)/delta2 + 1/2; the estimate is then corrected
+  // against the canonical fp32 sample positions (usually one test on each side), so the result is
+  // exactly the count the definition gives.
+  int c = __float2int_rn(__fdividef(t - ti2, dl2));
+  c = c < 1 ? 1 : (c > K - 1 ? K - 1 : c);
+  while (c > 1 && !precedes(ms_sample_t(ti2, dl2, c - 1), t, tie_lt)) --c;
+  while (c < K - 1 && precedes(ms_sample_t(ti2, dl2, c), t, tie_lt)) ++c;
+  return (uint32_t)c;
 }
 
 // rank of sample (h, k) in the order (t, prim, k).  n <= HCAP: stream-level classification in
@@ -119,6 +122,7 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
   const int K = a.K, nf = a.n_feat;
   float T = 1.0f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
   float F[MS_MAX_OUT / 32] = {0.f, 0.f};
+  float4 F4 = make_float4(0.f, 0.f, 0.f, 0.f);   // n_feat == 32: channels 4*(lane%8)..+3 of the samples of lane group lane/8
   if (n > 0) {
     const MsHit *hits = a.hits + off;
     const float4 *stg = a.staging + (size_t)off * (size_t)K;
@@ -177,13 +181,39 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
       if (FEAT) {
         __syncwarp();
         const float *fbase = a.staging_feat + (size_t)off * (size_t)K * (size_t)nf;
-        for (uint32_t r = 0; r < done; ++r) {
-          const uint32_t s = sm.ord[r];
-          const float w = sm.val[single ? s : r].w;
+        if (nf == 32) {
+          // lane group g = lane/8 takes sample r+g, lane%8 takes channels 4*(lane%8)..+3: one warp
+          // load covers four 128 B rows; four loads in flight per lane before the FMAs.
+          const int g = lane >> 3, c4 = lane & 7;
+          for (uint32_t r = 0; r < done; r += 16) {
+            float4 f[4];
+            float wv[4];
 #pragma unroll
-          for (int q = 0; q < MS_MAX_OUT / 32; ++q) {
-            const int c = lane + 32 * q;
-            if (c < nf) F[q] = fmaf(w, __ldg(fbase + (size_t)s * (size_t)nf + c), F[q]);
+            for (int q = 0; q < 4; ++q) {
+              const uint32_t rr = r + 4 * q + g;
+              f[q] = make_float4(0.f, 0.f, 0.f, 0.f);
+              wv[q] = 0.f;
+              if (rr < done) {
+                const uint32_t s = sm.ord[rr];
+                wv[q] = sm.val[single ? s : rr].w;
+                f[q] = __ldg(reinterpret_cast<const float4 *>(fbase + (size_t)s * 32) + c4);
+              }
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              F4.x = fmaf(wv[q], f[q].x, F4.x); F4.y = fmaf(wv[q], f[q].y, F4.y);
+              F4.z = fmaf(wv[q], f[q].z, F4.z); F4.w = fmaf(wv[q], f[q].w, F4.w);
+            }
+          }
+        } else {
+          for (uint32_t r = 0; r < done; ++r) {
+            const uint32_t s = sm.ord[r];
+            const float w = sm.val[single ? s : r].w;
+#pragma unroll
+            for (int q = 0; q < MS_MAX_OUT / 32; ++q) {
+              const int c = lane + 32 * q;
+              if (c < nf) F[q] = fmaf(w, __ldg(fbase + (size_t)s * (size_t)nf + c), F[q]);
+            }
           }
         }
       }
@@ -199,10 +229,19 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
   if (lane < 3) a.out_rgb[3 * (size_t)ray + lane] = lane == 0 ? C0 : (lane == 1 ? C1 : C2);
   if (lane == 3) a.out_alpha[ray] = 1.0f - T;
   if (FEAT) {
+    if (nf == 32) {
 #pragma unroll
-    for (int q = 0; q < MS_MAX_OUT / 32; ++q) {
-      const int c = lane + 32 * q;
-      if (c < nf) a.out_feat[(size_t)ray * nf + c] = F[q];
+      for (int o = 8; o < 32; o <<= 1) {
+        F4.x += __shfl_xor_sync(FULL, F4.x, o); F4.y += __shfl_xor_sync(FULL, F4.y, o);
+        F4.z += __shfl_xor_sync(FULL, F4.z, o); F4.w += __shfl_xor_sync(FULL, F4.w, o);
+      }
+      if (lane < 8) reinterpret_cast<float4 *>(a.out_feat + (size_t)ray * 32)[lane] = F4;
+    } else {
+#pragma unroll
+      for (int q = 0; q < MS_MAX_OUT / 32; ++q) {
+        const int c = lane + 32 * q;
+        if (c < nf) a.out_feat[(size_t)ray * nf + c] = F[q];
+      }
     }
   }
 }
