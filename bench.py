@@ -164,21 +164,18 @@ def run_reference(args, cfg):
 # ------------------------------------------------------------------------------------------------
 def run_ours(args, cfg):
     import torch
-    import torch.distributed as dist
     from paper_2606_03877_b200 import api
+    from paper_2606_03877_b200 import dist as msdist
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, local, world = msdist.env_rank_world()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the render has no CPU fallback")
     torch.cuda.set_device(local)
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        msdist.init("nccl", torch.device("cuda", local))
 
     def barrier():
-        if world > 1:
-            dist.barrier()
+        msdist.barrier()
         torch.cuda.synchronize()
 
     peaks = load_peaks()
@@ -222,13 +219,9 @@ def run_ours(args, cfg):
     barrier()
     e2e_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
 
-    t = torch.tensor([ms_total, e2e_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_total, e2e_ms = float(t[0]), float(t[1])
+    ms_total, e2e_ms = msdist.max_over_ranks([ms_total, e2e_ms], "cuda")
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
+        msdist.shutdown()
         return
 
     ms_step = ms_total / args.steps
@@ -271,8 +264,7 @@ def run_ours(args, cfg):
         line["cpu_baseline"] = {k: v for k, v in time_oracle(cfg, sc, cams, args.cpu_seconds).items()
                                 if k in ("value", "unit", "cores", "kind", "sample", "samples_per_s")}
     print(json.dumps(line), flush=True)
-    if world > 1:
-        dist.destroy_process_group()
+    msdist.shutdown()
 
 
 def main():
