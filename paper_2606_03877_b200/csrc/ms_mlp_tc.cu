@@ -267,13 +267,15 @@ __device__ __forceinline__ void encode_row(const float *u, const float *d, uint8
 // ---------------------------------------------------------------------------------------------
 // kernel
 // ---------------------------------------------------------------------------------------------
-// Warp roles (17 + NSLOT warps, one CTA per SM):
-//   warp 0            weight loader (one lane) + TMEM owner
-//   warps 1..NSLOT    MMA issuers, one per slot: a converged warp, one elected lane issues (see mma_ss).
+// Warp roles (one CTA per SM):
+//   warp NSLOT        head MMA issuer (N = NOUT MMAs of every block, in block order); also the weight
+//                     loader (one bulk copy per segment) and the TMEM owner
+//   warps 0..NSLOT-1  MMA issuers, one per slot: a converged warp, one elected lane issues (see mma_ss).
 //                     One warp per slot because the issue path is latency-bound: ~45 cycles per
 //                     tcgen05.mma (four R2UR each) and ~90 per mbarrier try_wait, 30 MMAs and 6 waits
 //                     per block -- more than the 1416 tensor cycles the block needs
-//   next 4 warps      EN: sample -> u -> encoding -> A1 ring in shared memory (runs ahead of the tensor pipe)
+//   next 4 or 8 warps EN: sample -> u -> encoding -> A1 ring in shared memory (runs ahead of the tensor pipe);
+//                     two groups taking alternate blocks when the MLP is 64 wide
 //   next 4 warps      HD: head accumulator -> sigmoid / softplus / exp -> staging store
 //   last 8 warps      HE: hidden-layer epilogue, D (fp32, TMEM) -> relu, bf16 -> A (TMEM); two warps per
 //                     TMEM lane quarter, each on one half of the columns
@@ -284,22 +286,34 @@ __device__ __forceinline__ void encode_row(const float *u, const float *d, uint8
 // head accumulators live in HPS small regions per slot after the slots (private to the slot's MMA
 // warp, so every mbarrier has one producer and one consumer walking it in order), and a slot is
 // released to its next block as soon as the block's head MMA is issued.  The tensor pipe completes in issue order.
-constexpr int TC_WARPS_FIXED = 1 + 4 + 4 + 8;   // loader, EN, HD, HE; plus one MMA warp per slot
-constexpr int TC_NA1 = 4;    // A1 ring stages
 constexpr uint32_t TC_MIN_SMEM = 116 * 1024;  // > half of the SM's shared memory: one CTA per SM (it owns all 512 TMEM columns)
 
 // slots in flight and head accumulator regions per slot, fitted to the 512 TMEM columns
 __host__ __device__ constexpr int tc_slots(int width, int nout) { return width > 64 ? 2 : (nout <= 16 ? 4 : 3); }
 __host__ __device__ constexpr int tc_heads_per_slot(int width) { return width > 64 ? 2 : 1; }
+// EN warp groups (4 warps each, group g encodes the blocks with run % groups == g) and A1 ring stages:
+// a 64-wide MLP needs < 500 tensor cycles per block, less than one warp needs to encode its 32 rows
+__host__ __device__ constexpr int tc_en_groups(int width) { return width > 64 ? 1 : 2; }
+__host__ __device__ constexpr int tc_a1_stages(int width) { return width > 64 ? 4 : 8; }
+// HE warp groups: 128 wide -- one group of 8 warps (64 columns each) serves both slots in turn;
+// 64 wide -- groups of 4 warps (a whole row of 64 columns each), group g serving the slots s % groups == g
+__host__ __device__ constexpr int tc_he_groups(int width, int nout) { return width > 64 ? 1 : (nout <= 16 ? 2 : 1); }
+__host__ __device__ constexpr int tc_he_warps(int, int) { return 8; }
+__host__ __device__ constexpr int tc_warps(int width, int nout) {
+  return tc_slots(width, nout) + 1 + 4 * tc_en_groups(width) + 4 + tc_he_warps(width, nout);
+}
+// warps: one MMA warp per slot, head MMA warp (also weight loader and TMEM owner), EN groups, 4 HD, HE groups
 
 template <int NFREQ, int VIEWDIR, int WIDTH, int NOUT, int NH>
-__global__ void __launch_bounds__(32 * (TC_WARPS_FIXED + tc_slots(WIDTH, NOUT)), 1) mlp_tc_kernel(const TcParams p) {
+__global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(const TcParams p) {
   constexpr int IN = 3 + 6 * NFREQ + 3 * VIEWDIR;
   constexpr int K1 = (IN + 2 + 15) / 16 * 16;
   constexpr int NSLOT = tc_slots(WIDTH, NOUT);
   constexpr int HPS = tc_heads_per_slot(WIDTH);   // head regions per slot (private to the slot's MMA warp)
   constexpr int NHS = NSLOT * HPS;
-  constexpr int W_EN = 1 + NSLOT, W_HD = W_EN + 4, W_HE = W_HD + 4;   // first warp of each group
+  constexpr int NEG = tc_en_groups(WIDTH), TC_NA1 = tc_a1_stages(WIDTH), NG = tc_he_groups(WIDTH, NOUT), HEW = tc_he_warps(WIDTH, NOUT) / NG;   // HE groups, warps per group
+  static_assert(TC_NA1 % NEG == 0, "every ring stage belongs to one EN group");
+  constexpr int W_HM = NSLOT, W_EN = W_HM + 1, W_HD = W_EN + 4 * NEG, W_HE = W_HD + 4;   // first warp of each group
   constexpr int SLOT_COLS = WIDTH + WIDTH / 2 + 8;
   constexpr int HEAD_COL0 = NSLOT * SLOT_COLS;
   static_assert(HEAD_COL0 + NHS * NOUT <= 512, "TMEM columns");
@@ -307,25 +321,26 @@ __global__ void __launch_bounds__(32 * (TC_WARPS_FIXED + tc_slots(WIDTH, NOUT)),
   constexpr uint32_t IMG_BYTES = tc_image_bytes(K1, WIDTH, NH, NOUT);
   extern __shared__ __align__(1024) uint8_t smem[];
   // [ weight image | A1 ring ]
-  __shared__ uint64_t bars[2 + 2 * TC_NA1 + 2 * NSLOT + 2 * NHS];
+  __shared__ uint64_t bars[2 + 2 * TC_NA1 + 3 * NSLOT + 2 * NHS];
   __shared__ uint32_t tmem_base_s;
   uint8_t *s_img = smem;
   uint8_t *s_a1 = smem + IMG_BYTES;
   const uint32_t bar_w_full = smem_u32(&bars[0]), bar_w_free = smem_u32(&bars[1]);
   const uint32_t bar_a1_full = smem_u32(&bars[2]), bar_a1_free = bar_a1_full + 8 * TC_NA1;
   const uint32_t bar_d_full = bar_a1_free + 8 * TC_NA1, bar_a_ready = bar_d_full + 8 * NSLOT;
-  const uint32_t bar_h_full = bar_a_ready + 8 * NSLOT, bar_h_free = bar_h_full + 8 * NHS;
+  const uint32_t bar_a3_ready = bar_a_ready + 8 * NSLOT;   // the block's last epilogue is done: input of the head
+  const uint32_t bar_h_full = bar_a3_ready + 8 * NSLOT, bar_h_free = bar_h_full + 8 * NHS;
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   if (tid == 0) {
     mbar_init(bar_w_full, 1);
-    mbar_init(bar_w_free, NSLOT);
+    mbar_init(bar_w_free, NSLOT + 1);
     for (int i = 0; i < TC_NA1; ++i) { mbar_init(bar_a1_full + 8 * i, 4); mbar_init(bar_a1_free + 8 * i, 1); }
-    for (int i = 0; i < NSLOT; ++i) { mbar_init(bar_d_full + 8 * i, 1); mbar_init(bar_a_ready + 8 * i, 8); }
+    for (int i = 0; i < NSLOT; ++i) { mbar_init(bar_d_full + 8 * i, 1); mbar_init(bar_a_ready + 8 * i, HEW); mbar_init(bar_a3_ready + 8 * i, HEW); }
     for (int i = 0; i < NHS; ++i) { mbar_init(bar_h_full + 8 * i, 1); mbar_init(bar_h_free + 8 * i, 4); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (warp == 0) {
+  if (warp == W_HM) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)), "r"(512));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
@@ -347,27 +362,14 @@ __global__ void __launch_bounds__(32 * (TC_WARPS_FIXED + tc_slots(WIDTH, NOUT)),
   const uint32_t b0 = (uint32_t)(((uint64_t)p.n_blocks * blockIdx.x) / gridDim.x);
   const uint32_t b1 = (uint32_t)(((uint64_t)p.n_blocks * (blockIdx.x + 1)) / gridDim.x);
 
-  if (warp == 0) {
-    // ===== weight loader: one bulk async copy per segment =====
-    if (lane == 0) {
-      SegWalk w(p.blk_off, p.n_prims, b0, b1);
-      int prim; uint32_t first, count, seg = 0;
-      while (w.next(prim, first, count)) {
-        if (seg > 0) mbar_wait(bar_w_free, (seg - 1) & 1);
-        mbar_expect_tx(bar_w_full, IMG_BYTES);
-        bulk_g2s(smem_u32(s_img), p.image + (size_t)prim * IMG_BYTES, IMG_BYTES, bar_w_full);
-        ++seg;
-      }
-    }
-  } else if (warp <= NSLOT) {
-    // ===== MMA issuer of slot s = warp - 1 (all 32 lanes walk the schedule; mma_* elect one lane) =====
-    const int s = warp - 1;
+  if (warp < NSLOT) {
+    // ===== MMA issuer of slot s = warp (all 32 lanes walk the schedule; mma_* elect one lane) =====
+    const int s = warp;
     SegWalk w(p.blk_off, p.n_prims, b0, b1);
     int prim; uint32_t first, count, seg = 0;
     uint32_t run0 = 0;                 // running index of the segment's first block (ring positions)
     uint32_t pa = 0;                   // parity of the next a_ready[s] completion
-    uint32_t cnt = 0;                  // heads this warp has issued: head region s*HPS + cnt%HPS, use cnt/HPS
-    constexpr uint32_t idesc_w = umma_idesc(WIDTH), idesc_o = umma_idesc(NOUT);
+    constexpr uint32_t idesc_w = umma_idesc(WIDTH);
     const uint32_t img = smem_u32(s_img);
     const uint32_t a1_base = smem_u32(s_a1);
     const uint32_t d_tmem = tmem + s * SLOT_COLS, a_tmem = d_tmem + WIDTH;
@@ -377,20 +379,9 @@ __global__ void __launch_bounds__(32 * (TC_WARPS_FIXED + tc_slots(WIDTH, NOUT)),
       tc_fence_after();
       const uint32_t n_s = (count + NSLOT - 1 - s) / NSLOT;   // blocks of this segment that run in slot s
       for (uint32_t j = 0; j <= n_s; ++j) {
-        if (j > 0) {  // head of the slot's previous block
-          const uint32_t hs = s * HPS + cnt % HPS;
+        if (j > 0) {  // the previous block's last epilogue has read D (its head is the head warp's business)
           mbar_wait(bar_a_ready_s, pa);
           pa ^= 1u;
-          mbar_wait(bar_h_free + 8 * hs, ((cnt / HPS) & 1u) ^ 1u);
-          ++cnt;
-          tc_fence_after();
-          const uint32_t h_tmem = tmem + HEAD_COL0 + hs * NOUT;
-#pragma unroll
-          for (int q = 0; q <= WIDTH / 16; ++q) {
-            const uint64_t db = umma_desc(img + tc_off_w(K1, WIDTH, NH) + q * 2 * (NOUT * 16), NOUT * 16, 128);
-            mma_ts(h_tmem, a_tmem + q * 8, db, idesc_o, q > 0);
-          }
-          mma_commit(bar_h_full + 8 * hs);
         }
         if (j == n_s) break;
         {  // layer 1 of the slot's next block: A from the A1 ring
@@ -425,13 +416,71 @@ __global__ void __launch_bounds__(32 * (TC_WARPS_FIXED + tc_slots(WIDTH, NOUT)),
       ++seg;
     }
     if (seg > 0) mbar_wait(bar_w_free, (seg - 1) & 1);  // no asynchronous arrive may outlive the CTA
+  } else if (warp == W_HM) {
+    // ===== head MMA issuer: the N = NOUT head MMAs are issue-bound (~25 cycles each for a few cycles
+    // of tensor work); from a warp of their own they slip into the pipe between the slots' wide MMAs
+    // It is also the weight loader: one bulk async copy of the next primitive's image once every
+    // MMA of the segment has read the current one (w_free), issued by lane 0.
+    SegWalk w(p.blk_off, p.n_prims, b0, b1), wl(p.blk_off, p.n_prims, b0, b1);
+    int prim; uint32_t first, count, seg = 0;
+    constexpr uint32_t idesc_o = umma_idesc(NOUT);
+    const uint32_t img = smem_u32(s_img);
+    uint32_t cum[NSLOT];                          // blocks each slot has taken in earlier segments
+#pragma unroll
+    for (int s = 0; s < NSLOT; ++s) cum[s] = 0;
+    {
+      int lp; uint32_t lf, lc;
+      if (wl.next(lp, lf, lc) && lane == 0) {
+        mbar_expect_tx(bar_w_full, IMG_BYTES);
+        bulk_g2s(img, p.image + (size_t)lp * IMG_BYTES, IMG_BYTES, bar_w_full);
+      }
+      __syncwarp();
+    }
+    while (w.next(prim, first, count)) {
+      mbar_wait(bar_w_full, seg & 1);
+      for (uint32_t i = 0; i < count; ++i) {
+        const uint32_t slot = i % NSLOT;
+        uint32_t cnt = i / NSLOT;                   // the slot's block counter (uses of its barriers)
+#pragma unroll
+        for (int s = 0; s < NSLOT; ++s) cnt += slot == (uint32_t)s ? cum[s] : 0u;
+        const uint32_t hs = slot * HPS + cnt % HPS;
+        mbar_wait(bar_a3_ready + 8 * slot, cnt & 1u);
+        mbar_wait(bar_h_free + 8 * hs, ((cnt / HPS) & 1u) ^ 1u);
+        tc_fence_after();
+        const uint32_t a_tmem = tmem + slot * SLOT_COLS + WIDTH;
+        const uint32_t h_tmem = tmem + HEAD_COL0 + hs * NOUT;
+#pragma unroll
+        for (int q = 0; q <= WIDTH / 16; ++q) {
+          const uint64_t db = umma_desc(img + tc_off_w(K1, WIDTH, NH) + q * 2 * (NOUT * 16), NOUT * 16, 128);
+          mma_ts(h_tmem, a_tmem + q * 8, db, idesc_o, q > 0);
+        }
+        mma_commit(bar_h_full + 8 * hs);
+      }
+      mma_commit(bar_w_free);
+#pragma unroll
+      for (int s = 0; s < NSLOT; ++s) cum[s] += (count + NSLOT - 1 - s) / NSLOT;
+      mbar_wait(bar_w_free, seg & 1);             // every MMA of the segment is done with the image
+      {
+        int lp; uint32_t lf, lc;
+        if (wl.next(lp, lf, lc) && lane == 0) {
+          mbar_expect_tx(bar_w_full, IMG_BYTES);
+          bulk_g2s(img, p.image + (size_t)lp * IMG_BYTES, IMG_BYTES, bar_w_full);
+        }
+        __syncwarp();
+      }
+      ++seg;
+    }
   } else if (warp >= W_HE) {
     // ===== HE: hidden-layer epilogues =====
     const int quarter = warp & 3;                 // TMEM lanes this warp may touch: 32*quarter .. +31
-    const int ch = (warp - W_HE) >> 2;              // column half
-    constexpr int HC = WIDTH / 2;                 // columns per warp
+    const int grp = (warp - W_HE) / HEW;            // this warp serves the slots with s % NG == grp
+    const int ch = ((warp - W_HE) % HEW) >> 2;      // column group
+    constexpr int HC = WIDTH / (HEW / 4);         // columns per warp (64)
     const uint32_t lane_addr = (uint32_t)(quarter * 32) << 16;
     uint32_t pd = 0;                              // bit s: parity of the next d_full[s] completion
+    uint32_t cum[NSLOT];                          // blocks each slot has taken in earlier segments
+#pragma unroll
+    for (int s = 0; s < NSLOT; ++s) cum[s] = 0;
     SegWalk w(p.blk_off, p.n_prims, b0, b1);
     int prim; uint32_t first, count;
     while (w.next(prim, first, count)) {
@@ -442,31 +491,57 @@ __global__ void __launch_bounds__(32 * (TC_WARPS_FIXED + tc_slots(WIDTH, NOUT)),
 #pragma unroll
           for (int s = 0; s < NSLOT; ++s) {
             const uint32_t n_s = (count + NSLOT - 1 - s) / NSLOT;
-            if (j >= n_s) continue;
+            if (j >= n_s || s % NG != grp) continue;
             const uint32_t d_tmem = tmem + s * SLOT_COLS + lane_addr + ch * HC;
             const uint32_t a_tmem = tmem + s * SLOT_COLS + WIDTH + lane_addr + ch * (HC / 2);
             mbar_wait(bar_d_full + 8 * s, (pd >> s) & 1u);
             pd ^= 1u << s;
             tc_fence_after();
-            uint32_t r[HC];
+            const uint32_t prev = cum[s] + j;       // blocks the slot has finished before this one
+            if constexpr (WIDTH > 64) {
+              uint32_t r[HC];
 #pragma unroll
-            for (int c0 = 0; c0 < HC; c0 += 32) tmem_ld32(d_tmem + c0, r + c0);
-            tmem_ld_wait();
+              for (int c0 = 0; c0 < HC; c0 += 32) tmem_ld32(d_tmem + c0, r + c0);
+              tmem_ld_wait();
+              if (l == 0 && prev > 0) {             // A still feeds the previous block's head MMAs
+                mbar_wait(bar_h_full + 8 * (s * HPS + (prev - 1) % HPS), ((prev - 1) / HPS) & 1u);
+                tc_fence_after();
+              }
 #pragma unroll
-            for (int c0 = 0; c0 < HC; c0 += 32) {
-              uint32_t o[16];
+              for (int c0 = 0; c0 < HC; c0 += 32) {
+                uint32_t o[16];
 #pragma unroll
-              for (int q = 0; q < 16; ++q)
-                o[q] = relu_pack_bf16(__uint_as_float(r[c0 + 2 * q]), __uint_as_float(r[c0 + 2 * q + 1]));
-              tmem_st16(a_tmem + c0 / 2, o);
+                for (int q = 0; q < 16; ++q)
+                  o[q] = relu_pack_bf16(__uint_as_float(r[c0 + 2 * q]), __uint_as_float(r[c0 + 2 * q + 1]));
+                tmem_st16(a_tmem + c0 / 2, o);
+              }
+            } else {                                // 72-register budget: 32 columns at a time
+#pragma unroll
+              for (int c0 = 0; c0 < HC; c0 += 32) {
+                uint32_t r[32], o[16];
+                tmem_ld32(d_tmem + c0, r);
+                tmem_ld_wait();
+#pragma unroll
+                for (int q = 0; q < 16; ++q) o[q] = relu_pack_bf16(__uint_as_float(r[2 * q]), __uint_as_float(r[2 * q + 1]));
+                if (c0 == 0 && l == 0 && prev > 0) {
+                  mbar_wait(bar_h_full + 8 * (s * HPS + (prev - 1) % HPS), ((prev - 1) / HPS) & 1u);
+                  tc_fence_after();
+                }
+                tmem_st16(a_tmem + c0 / 2, o);
+              }
             }
             tmem_st_wait();
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive(bar_a_ready + 8 * s);
+            if (lane == 0) {
+              mbar_arrive(bar_a_ready + 8 * s);
+              if (l == NH - 1) mbar_arrive(bar_a3_ready + 8 * s);
+            }
           }
         }
       }
+#pragma unroll
+      for (int s = 0; s < NSLOT; ++s) cum[s] += (count + NSLOT - 1 - s) / NSLOT;
     }
   } else if (warp >= W_HD) {
     // ===== HD: head epilogue: raw -> rgb = sigmoid, sigma = softplus, e = exp(-sigma delta) =====
@@ -549,9 +624,10 @@ __global__ void __launch_bounds__(32 * (TC_WARPS_FIXED + tc_slots(WIDTH, NOUT)),
     }
   } else {
     // ===== EN: sample -> u -> encoding -> A1 ring =====
-    const int row = (warp - W_EN) * 32 + lane;
+    const int row = ((warp - W_EN) & 3) * 32 + lane;
+    const uint32_t grp = (uint32_t)(warp - W_EN) >> 2;   // this group encodes the blocks with run % NEG == grp
     const uint32_t K = (uint32_t)p.K;
-    const uint32_t dj = MS_ROWS / K, dk = MS_ROWS - dj * K;
+    const uint32_t dj = (NEG * MS_ROWS) / K, dk = NEG * MS_ROWS - dj * K;   // NEG blocks ahead
     uint32_t run0 = 0;
     SegWalk w(p.blk_off, p.n_prims, b0, b1);
     int prim; uint32_t first, count;
@@ -563,14 +639,15 @@ __global__ void __launch_bounds__(32 * (TC_WARPS_FIXED + tc_slots(WIDTH, NOUT)),
 #pragma unroll
       for (int q = 0; q < 3; ++q) mu[q] = __ldg(p.center + 3 * (size_t)prim + q);
       // interval index j and sample index k of this thread's row in block i; advanced by 128 samples per block
-      const uint64_t s0 = (uint64_t)first * MS_ROWS + (uint32_t)row;
+      const uint32_t i0 = (grp + NEG - run0 % NEG) % NEG;   // first block of the segment that is this group's
+      const uint64_t s0 = (uint64_t)(first + i0) * MS_ROWS + (uint32_t)row;
       uint32_t j = (uint32_t)(s0 / K), k = (uint32_t)(s0 - (uint64_t)j * K);
       float4 q0 = make_float4(0.f, 0.f, 0.f, 0.f), q1 = q0;   // interval record of the block about to be encoded
       if (j < iv_count) {
         const float4 *ivp = reinterpret_cast<const float4 *>(p.intervals + iv_first + j);
         q0 = __ldg(ivp); q1 = __ldg(ivp + 1);
       }
-      for (uint32_t i = 0; i < count; ++i) {
+      for (uint32_t i = i0; i < count; i += NEG) {
         const uint32_t run = run0 + i, st = run % TC_NA1;
         const bool valid = j < iv_count;
         const float4 c0 = q0, c1 = q1;
@@ -578,7 +655,7 @@ __global__ void __launch_bounds__(32 * (TC_WARPS_FIXED + tc_slots(WIDTH, NOUT)),
         // prefetch the next block's interval record
         k += dk; j += dj;
         if (k >= K) { k -= K; ++j; }
-        if (i + 1 < count && j < iv_count) {
+        if (i + NEG < count && j < iv_count) {
           const float4 *ivp = reinterpret_cast<const float4 *>(p.intervals + iv_first + j);
           q0 = __ldg(ivp); q1 = __ldg(ivp + 1);
         }
@@ -599,7 +676,7 @@ __global__ void __launch_bounds__(32 * (TC_WARPS_FIXED + tc_slots(WIDTH, NOUT)),
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512));
+  if (warp == W_HM) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512));
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -713,7 +790,7 @@ cudaError_t ms_mlp_tc(const MsTcWeights &w, const MsMlpArgs &a, cudaStream_t s) 
   p.center = a.center; p.A = a.A; p.prim_start = a.prim_start; p.blk_off = a.blk_off; p.intervals = a.intervals;
   p.image = (const uint8_t *)w.image;
   p.staging = a.staging; p.staging_feat = a.staging_feat;
-  size_t smem = w.bytes_per_prim + TC_NA1 * ((size_t)MS_ROWS * w.k1_pad * 2);
+  size_t smem = w.bytes_per_prim + tc_a1_stages(a.shape.width) * ((size_t)MS_ROWS * w.k1_pad * 2);
   if (smem < TC_MIN_SMEM) smem = TC_MIN_SMEM;
   static int n_sm = 0;
   if (n_sm == 0) {
@@ -724,7 +801,7 @@ cudaError_t ms_mlp_tc(const MsTcWeights &w, const MsMlpArgs &a, cudaStream_t s) 
   cudaError_t e = cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   unsigned grid = a.n_blocks < (uint32_t)n_sm ? a.n_blocks : (unsigned)n_sm;
-  const int threads = 32 * (TC_WARPS_FIXED + tc_slots(a.shape.width, w.n_out_pad));
+  const int threads = 32 * tc_warps(a.shape.width, w.n_out_pad);
   fn<<<grid, threads, smem, s>>>(p);
   MS_LAUNCHED();
   return cudaGetLastError();
