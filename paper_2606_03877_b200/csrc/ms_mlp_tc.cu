@@ -286,6 +286,7 @@ __device__ __forceinline__ void encode_row(const float *u, const float *d, uint8
 // head accumulators live in HPS small regions per slot after the slots (private to the slot's MMA
 // warp, so every mbarrier has one producer and one consumer walking it in order), and a slot is
 // released to its next block as soon as the block's head MMA is issued.  The tensor pipe completes in issue order.
+constexpr uint32_t TC_HD_ROW = 144;           // bytes per row of the HD transpose buffers (128 + 16: conflict-free)
 constexpr uint32_t TC_MIN_SMEM = 116 * 1024;  // > half of the SM's shared memory: one CTA per SM (it owns all 512 TMEM columns)
 
 // slots in flight and head accumulator regions per slot, fitted to the 512 TMEM columns
@@ -320,11 +321,12 @@ __global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(c
   constexpr uint32_t A1_BYTES = MS_ROWS * K1 * 2;
   constexpr uint32_t IMG_BYTES = tc_image_bytes(K1, WIDTH, NH, NOUT);
   extern __shared__ __align__(1024) uint8_t smem[];
-  // [ weight image | A1 ring ]
+  // [ weight image | A1 ring | HD transpose buffers (wide head only) ]
   __shared__ uint64_t bars[2 + 2 * TC_NA1 + 3 * NSLOT + 2 * NHS];
   __shared__ uint32_t tmem_base_s;
   uint8_t *s_img = smem;
   uint8_t *s_a1 = smem + IMG_BYTES;
+  uint8_t *s_hd = s_a1 + TC_NA1 * A1_BYTES;
   const uint32_t bar_w_full = smem_u32(&bars[0]), bar_w_free = smem_u32(&bars[1]);
   const uint32_t bar_a1_full = smem_u32(&bars[2]), bar_a1_free = bar_a1_full + 8 * TC_NA1;
   const uint32_t bar_d_full = bar_a1_free + 8 * TC_NA1, bar_a_ready = bar_d_full + 8 * NSLOT;
@@ -603,20 +605,33 @@ __global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(c
           const float sigma = fmaxf(r3, 0.0f) + __logf(1.0f + __expf(-fabsf(r3)));
           v.w = __expf(-sigma * delta);
           p.staging[out_idx] = v;
-          if constexpr (NOUT > 16) if (feat) {
+          if constexpr (NOUT > 16) if (feat && p.n_feat != 32) {
             float *f = p.staging_feat + out_idx * (size_t)p.n_feat;
-            if (p.n_feat == 32) {
 #pragma unroll
-              for (int c = 0; c < 8; ++c)
-                reinterpret_cast<float4 *>(f)[c] =
-                    make_float4(__uint_as_float(r[4 + 4 * c]), __uint_as_float(r[5 + 4 * c]),
-                                __uint_as_float(r[6 + 4 * c]), __uint_as_float(r[7 + 4 * c]));
-            } else {
-#pragma unroll
-              for (int c = 0; c < 32; ++c)
-                if (c < p.n_feat) f[c] = __uint_as_float(r[4 + c]);
-            }
+            for (int c = 0; c < 32; ++c)
+              if (c < p.n_feat) f[c] = __uint_as_float(r[4 + c]);
           }
+        }
+        if constexpr (NOUT > 16) if (feat && p.n_feat == 32) {
+          // 32 feature channels = one 128 B row per sample.  A lane storing its own row touches 32 lines
+          // per instruction (one LSU wavefront each -- measured: HD was the slowest role of CFG5);
+          // transposed through shared memory, eight lanes store one row and an instruction touches 4.
+          float4 *buf = reinterpret_cast<float4 *>(s_hd + (warp - W_HD) * (32 * TC_HD_ROW));
+#pragma unroll
+          for (int c = 0; c < 8; ++c)
+            *reinterpret_cast<float4 *>(reinterpret_cast<uint8_t *>(buf) + lane * TC_HD_ROW + c * 16) =
+                make_float4(__uint_as_float(r[4 + 4 * c]), __uint_as_float(r[5 + 4 * c]),
+                            __uint_as_float(r[6 + 4 * c]), __uint_as_float(r[7 + 4 * c]));
+          __syncwarp();
+          const unsigned long long my = valid ? (unsigned long long)out_idx : ~0ull;
+#pragma unroll
+          for (int it = 0; it < 8; ++it) {
+            const int rr = it * 4 + (lane >> 3);
+            const unsigned long long idx = __shfl_sync(0xffffffffu, my, rr);
+            const float4 v = *reinterpret_cast<const float4 *>(reinterpret_cast<const uint8_t *>(buf) + rr * TC_HD_ROW + (lane & 7) * 16);
+            if (idx != ~0ull) reinterpret_cast<float4 *>(p.staging_feat + (size_t)idx * 32)[lane & 7] = v;
+          }
+          __syncwarp();
         }
       }
 #pragma unroll
@@ -791,6 +806,7 @@ cudaError_t ms_mlp_tc(const MsTcWeights &w, const MsMlpArgs &a, cudaStream_t s) 
   p.image = (const uint8_t *)w.image;
   p.staging = a.staging; p.staging_feat = a.staging_feat;
   size_t smem = w.bytes_per_prim + tc_a1_stages(a.shape.width) * ((size_t)MS_ROWS * w.k1_pad * 2);
+  if (w.n_out_pad > 16) smem += 4 * 32 * TC_HD_ROW;
   if (smem < TC_MIN_SMEM) smem = TC_MIN_SMEM;
   static int n_sm = 0;
   if (n_sm == 0) {
