@@ -118,3 +118,74 @@ def test_tc_path_refuses_uncovered_shapes():
     with pytest.raises(api.MsError) as e:
         gs.render(cam, 64, 64, 8, path=api.PATH_BF16_TC)
     assert e.value.code == -4
+
+
+@pytest.mark.parametrize("K", [1, 5, 24, 64])
+@pytest.mark.parametrize("seed", [0, 3])
+def test_tc_ragged_blocks_and_eye_inside_cloud(K, seed):
+    """K that does not divide the 128-row block (ragged tails, intervals split across blocks),
+    K = 1 and the maximum K = 64, on scenes whose eye sits inside the primitive cloud (t_near
+    clamps, full-image AABBs); odd image size; a two-hidden-layer tensor shape (NH = 2)."""
+    api = _api()
+    mlp = synth.MLPSpec(4, 0, 2, 64, 0, True)
+    sc, cam, cfg = synth.random_tiny_scene(seed, n=20, mlp=mlp)
+    H, W = 37, 53
+    cam = synth.pinhole(W, H, cfg.fov_deg, cam.c2w)
+    orc = mso.OracleScene(sc)
+    gs = api.Scene(sc)
+    rgb, alpha, _ = gs.render(cam, H, W, K, path=api.PATH_BF16_TC, flags=api.FLAG_KEEP_DEBUG)
+    torch.cuda.synchronize()
+    o_rgb, o_alpha, _, st = orc.render(cam, H, W, K)
+    assert check_structures(gs, orc, cam, H, W, K, 16, n_order_rays=6) == st.n_intervals
+    assert_bf16_bar(rgb.cpu().numpy().reshape(-1, 3), alpha.cpu().numpy().reshape(-1), o_rgb, o_alpha)
+
+
+def test_tc_dense_scene_early_termination():
+    """pin P9 through the tensor path: opaque 128-wide scene, rays stop at T < 1e-4 (Q9, Q25)."""
+    api = _api()
+    cfg = synth.SceneConfig("dense_tc", 7, 48, 1.0, 0.3, 0.8, synth.MLPSpec(6, 0, 2, 128, 0, True),
+                            96, 80, 50.0, 3.0, 8, sigma_bias=8.0)
+    sc, cam = synth.make_scene(cfg), synth.make_cameras(cfg)[0]
+    gs = api.Scene(sc)
+    rgb, alpha, _ = gs.render(cam, cfg.height, cfg.width, cfg.K, path=api.PATH_BF16_TC)
+    torch.cuda.synchronize()
+    o_rgb, o_alpha, _, st = mso.OracleScene(sc).render(cam, cfg.height, cfg.width, cfg.K)
+    assert st.n_terminated > 200
+    assert_bf16_bar(rgb.cpu().numpy().reshape(-1, 3), alpha.cpu().numpy().reshape(-1), o_rgb, o_alpha)
+    assert float(alpha.max()) >= 1.0 - 1e-4 - 1e-6        # terminated rays: alpha = 1 - T, T < t_stop
+
+
+def test_tc_bias_rides_in_the_contraction():
+    """Biases that are not bf16-representable and span five orders of magnitude: the hi + lo bias
+    rows of the contraction must reproduce them to fp32-level accuracy, so the
+    tensor path stays as close to the oracle as it is with the generator's zero biases."""
+    api = _api()
+    cfg = synth.shrink(synth.CONFIGS["cfg2"], 96, 64)
+    sc, cam = synth.make_scene(cfg), synth.make_cameras(cfg)[0]
+    rng = np.random.default_rng(11)
+    w = sc.weights.copy()
+    off = 0
+    for i, o in cfg.mlp.layer_dims:
+        off += i * o
+        w[:, off:off + o] += (rng.uniform(-1, 1, (w.shape[0], o)) *
+                              10.0 ** rng.uniform(-4, 0, (w.shape[0], o))).astype(np.float32) * 0.3
+        off += o
+    sc2 = synth.custom_scene(sc.center, sc.quat, sc.scale, w, cfg.mlp)
+    gs = api.Scene(sc2)
+    rgb, alpha, _ = gs.render(cam, 64, 96, cfg.K, path=api.PATH_BF16_TC)
+    torch.cuda.synchronize()
+    o_rgb, o_alpha, _, _ = mso.OracleScene(sc2).render(cam, 64, 96, cfg.K)
+    assert_bf16_bar(rgb.cpu().numpy().reshape(-1, 3), alpha.cpu().numpy().reshape(-1), o_rgb, o_alpha)
+
+
+def test_tc_repeated_renders_are_deterministic():
+    """The warp-specialised pipeline has no data race: ten renders of one view are bitwise equal."""
+    api = _api()
+    cfg = synth.shrink(synth.CONFIGS["cfg4"], 320, 180)
+    sc, cam = synth.make_scene(cfg), synth.make_cameras(cfg)[0]
+    gs = api.Scene(sc)
+    ref = [t.clone() for t in gs.render(cam, 180, 320, cfg.K)[:2]]
+    for _ in range(9):
+        rgb, alpha, _ = gs.render(cam, 180, 320, cfg.K)
+        torch.cuda.synchronize()
+        assert torch.equal(rgb, ref[0]) and torch.equal(alpha, ref[1])
