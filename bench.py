@@ -31,6 +31,9 @@ import numpy as np  # noqa: E402
 from paper_2606_03877_b200 import synth  # noqa: E402
 
 UNIT = "Mpixels/s"
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed
+# `ncu --set full` capture of this very command (profiles/r1c_summary.md); null where none was taken.
+NCU_TRAFFIC_BYTES = {"cfg4": 0.843211264e9 + 7.445789e9}
 METRIC = "render throughput (Mpixels/s; MLP samples/s and roofline fraction alongside)"
 
 
@@ -252,7 +255,9 @@ def run_ours(args, cfg):
                 "note": "ms_render_host: camera in (kernel parameters), rgb/alpha(/feat) copied to pinned host memory"},
         "gpu_launches": launches,
         "roofline": {"bound": "tensor", "kernel": "mlp_tc_kernel (stage d)", "achieved": achieved, "peak": peak,
-                     "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                     "unit": "TFLOP/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg.name),
+                     "traffic_unit": "bytes per launch (ncu dram read + write, profiles/r1c_summary.md)",
+                     "algorithmic_bytes": n_samples_view * 16 + st.n_intervals * 32,
                      "peak_kind": f"bf16 dense, sustained, of {peaks['source']}",
                      "frac_of_burst_peak": achieved / peaks["bf16_tflops"],
                      "algorithmic_flop_per_sample": cfg.mlp.flop_per_sample,
