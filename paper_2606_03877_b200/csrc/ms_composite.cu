@@ -6,9 +6,10 @@
 // is monotone), so the position of a sample in the merged order has a closed form: its own k plus,
 // for every other hit of the ray, the number of that hit's samples that precede (t, prim) -- 0 or K
 // when the two t-ranges do not overlap (two compares), else a binary search over k.  No cursors, no
-// sort.  The ray's staged samples (16 B each, contiguous) are fetched by cp.async while the ranks are
-// computed; 32 merged samples at a time are composited with a warp product scan.  Features are
-// accumulated channel-per-lane, one coalesced 128 B row per sample.
+// sort.  The ray's staged samples (16 B each, one contiguous run) are gathered in merged order
+// straight from global memory -- only the order (4 B per sample) lives in shared memory, so 40+
+// warps fit per SM; 32 merged samples at a time are composited with a warp product scan.  Features
+// (32 channels): four 128 B rows per warp load.
 // HBM-bound by design: reads 16 B (+ 4 n_feat B) per sample and 16 B per hit, once.
 #include "ms_internal.cuh"
 
@@ -20,7 +21,6 @@ constexpr int HCAP = 32;     // hits cached in shared memory per ray (one per la
 constexpr unsigned FULL = 0xffffffffu;
 
 struct WarpSmem {
-  float4 val[CAP];      // (r, g, b, e) of the window's samples; .w is overwritten by the weight w
   uint32_t ord[CAP];    // ord[rank - r0] = sample index s = h*K + k inside the ray
   float4 key[HCAP];     // (t of sample 0, t of sample K-1, prim bits, unused)
   float2 geo[HCAP];     // (t_in, delta)
@@ -78,12 +78,6 @@ __device__ __forceinline__ uint32_t sample_rank(const WarpSmem &sm, const MsHit 
   return rank;
 }
 
-__device__ __forceinline__ void cp_async16(void *dst_smem, const void *src) {
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(dst_smem)), "l"(src)
-               : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
-
 // n <= HCAP: lane h caches hit h and classifies every other stream against it
 __device__ __forceinline__ void load_hits(WarpSmem &sm, const MsHit *__restrict__ hits, int n, int K, int lane) {
   if (n > HCAP) return;
@@ -113,6 +107,7 @@ __device__ __forceinline__ void load_hits(WarpSmem &sm, const MsHit *__restrict_
 template <int FEAT>  // 0: rgb/alpha only; 1: + features
 __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
   __shared__ WarpSmem s_all[CW];
+  __shared__ float s_w[FEAT ? CW : 1][FEAT ? CAP : 1];   // weight of the window's r-th merged sample (features only)
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int ray = (int)(blockIdx.x * CW + warp);
   if (ray >= a.n_rays) return;
@@ -127,9 +122,6 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
     const MsHit *hits = a.hits + off;
     const float4 *stg = a.staging + (size_t)off * (size_t)K;
     const uint32_t S = (uint32_t)n * (uint32_t)K;
-    const bool single = S <= (uint32_t)CAP;
-    if (single)
-      for (uint32_t s = lane; s < S; s += 32) cp_async16(&sm.val[s], stg + s);  // in flight during the rank pass
     load_hits(sm, hits, n, K, lane);
     __syncwarp();
     bool stopped = false;
@@ -141,14 +133,10 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
       for (uint32_t s = lane; s < S; s += 32) {
         float t;
         const uint32_t rk = sample_rank(sm, hits, n, K, h, k, &t) - r0;
-        if (rk < cnt) {
-          sm.ord[rk] = s;
-          if (!single) sm.val[rk] = stg[s];
-        }
+        if (rk < cnt) sm.ord[rk] = s;
         h += dh; k += dk;
         if (k >= K) { k -= K; ++h; }
       }
-      if (single) cp_async_wait_all();
       __syncwarp();
       // ---- composite the window, 32 merged samples per step ----
       uint32_t done = cnt;  // samples of this window that carry a weight
@@ -158,8 +146,8 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
         uint32_t slot = 0;
         float4 v = make_float4(0.f, 0.f, 0.f, 1.f);
         if (valid) {
-          slot = single ? sm.ord[r] : r;
-          v = sm.val[slot];
+          slot = sm.ord[r];
+          v = __ldg(stg + slot);   // 16 B gather inside the ray's contiguous staging run (read once: L1 keeps the lines)
         }
         float p = v.w;  // inclusive product scan of e over the lanes
 #pragma unroll
@@ -174,7 +162,7 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
         const int last = stop ? __ffs(stop) - 1 : 31;          // Q9: the stopping sample still contributes
         float w = (valid && lane <= last) ? (T * excl) * (1.0f - v.w) : 0.f;
         C0 = fmaf(w, v.x, C0); C1 = fmaf(w, v.y, C1); C2 = fmaf(w, v.z, C2);
-        if (FEAT && valid) sm.val[slot].w = w;
+        if (FEAT && valid) s_w[FEAT ? warp : 0][FEAT ? r : 0] = w;
         T = __shfl_sync(FULL, T_after, last);
         if (stop) { stopped = true; done = base + (uint32_t)last + 1; break; }
       }
@@ -195,7 +183,7 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
               wv[q] = 0.f;
               if (rr < done) {
                 const uint32_t s = sm.ord[rr];
-                wv[q] = sm.val[single ? s : rr].w;
+                wv[q] = s_w[FEAT ? warp : 0][FEAT ? rr : 0];
                 f[q] = __ldg(reinterpret_cast<const float4 *>(fbase + (size_t)s * 32) + c4);
               }
             }
@@ -208,7 +196,7 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
         } else {
           for (uint32_t r = 0; r < done; ++r) {
             const uint32_t s = sm.ord[r];
-            const float w = sm.val[single ? s : r].w;
+            const float w = s_w[FEAT ? warp : 0][FEAT ? r : 0];
 #pragma unroll
             for (int q = 0; q < MS_MAX_OUT / 32; ++q) {
               const int c = lane + 32 * q;
