@@ -118,12 +118,16 @@ def time_oracle(cfg, sc, cams, target_s: float, seed: int = 0):
     H, W = cfg.height, cfg.width
     rng = np.random.default_rng(seed)
     cores = os.cpu_count() or 1
-    n0 = min(H * W, 256)
-    pix = rng.choice(H * W, n0, replace=False).astype(np.int32)
-    t = time.perf_counter()
-    orc.render(cams[0], H, W, cfg.K, pixels=pix, tile=cfg.tile)
-    dt0 = max(time.perf_counter() - t, 1e-4)
-    n = int(min(H * W, max(n0, n0 * target_s / dt0)))
+    # two calibration passes: 256 pixels (dominated by the per-call tile-list build), then ~1/8 of the target
+    n, rate = min(H * W, 256), None
+    for _ in range(2):
+        if rate is not None:
+            n = int(min(H * W, max(256, rate * target_s / 8.0)))
+        pix = rng.choice(H * W, n, replace=False).astype(np.int32)
+        t = time.perf_counter()
+        orc.render(cams[0], H, W, cfg.K, pixels=pix, tile=cfg.tile)
+        rate = n / max(time.perf_counter() - t, 1e-4)          # pixels per second
+    n = int(min(H * W, max(256, rate * target_s)))
     pix = rng.choice(H * W, n, replace=False).astype(np.int32)
     t = time.perf_counter()
     _, _, _, st = orc.render(cams[0], H, W, cfg.K, pixels=pix, tile=cfg.tile)
