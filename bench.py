@@ -246,8 +246,10 @@ def run_ours(args, cfg):
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16" if cfg.mlp.bf16 else "f32", "data": "synthetic",
         "config": {"workload": workload_desc(cfg), "parallelism": f"replicas x{world}, no collective",
-                   "l2": "inputs larger than L2 (weights %.0f MB, per-view staging %.1f GB)" %
-                         (sc.weights.nbytes / 2 / 1e6, n_samples_view * 16 / 1e9),
+                   "l2": ("inputs larger than L2 (weights %.0f MB, per-view staging %.1f GB)" if
+                          sc.weights.nbytes / 2 + n_samples_view * 16 > 126e6 else
+                          "working set below L2 (weights %.1f MB, per-view staging %.3f GB): no flush, config is launch-bound")
+                         % (sc.weights.nbytes / 2 / 1e6, n_samples_view * 16 / 1e9),
                    "tile": cfg.tile, "t_stop": cfg.t_stop},
         "samples_per_s": world * n_samples_view * V / (ms_step * 1e-3),
         "counts_per_view": {"pairs": st.n_pairs, "intervals": st.n_intervals, "samples": st.n_samples,
@@ -258,7 +260,8 @@ def run_ours(args, cfg):
                 "h2d_bytes_per_step": 64 * V, "d2h_bytes_per_step": out_bytes * V, "ms_per_step": e2e_ms,
                 "note": "ms_render_host: camera in (kernel parameters), rgb/alpha(/feat) copied to pinned host memory"},
         "gpu_launches": launches,
-        "roofline": {"bound": "tensor", "kernel": "mlp_tc_kernel (stage d)", "achieved": achieved, "peak": peak,
+        "roofline": {"bound": "tensor" if cfg.mlp.bf16 else "alu",
+                     "kernel": "mlp_tc_kernel (stage d)" if cfg.mlp.bf16 else "mlp_f32_kernel (stage d, fp32 SIMT accuracy path; peak quoted is the bf16 tensor peak)", "achieved": achieved, "peak": peak,
                      "unit": "TFLOP/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg.name),
                      "traffic_unit": "bytes per launch (ncu dram read + write, profiles/r1c_summary.md)",
                      "algorithmic_bytes": n_samples_view * 16 + st.n_intervals * 32,
