@@ -8,7 +8,8 @@
 // when the two t-ranges do not overlap (two compares), else a binary search over k.  No cursors, no
 // sort.  The ray's staged samples (16 B each, one contiguous run) are gathered in merged order
 // straight from global memory -- only the order (4 B per sample) lives in shared memory, so 40+
-// warps fit per SM; 32 merged samples at a time are composited with a warp product scan.  Features
+// warps fit per SM; each lane composites a run of consecutive merged samples, one warp product
+// scan per window links the runs.  Features
 // (32 channels): four 128 B rows per warp load.
 // HBM-bound by design: reads 16 B (+ 4 n_feat B) per sample and 16 B per hit, once.
 #include "ms_internal.cuh"
@@ -138,34 +139,44 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
         if (k >= K) { k -= K; ++h; }
       }
       __syncwarp();
-      // ---- composite the window, 32 merged samples per step ----
-      uint32_t done = cnt;  // samples of this window that carry a weight
-      for (uint32_t base = 0; base < cnt; base += 32) {
-        const uint32_t r = base + lane;
-        const bool valid = r < cnt;
-        uint32_t slot = 0;
-        float4 v = make_float4(0.f, 0.f, 0.f, 1.f);
-        if (valid) {
-          slot = sm.ord[r];
-          v = __ldg(stg + slot);   // 16 B gather inside the ray's contiguous staging run (read once: L1 keeps the lines)
-        }
-        float p = v.w;  // inclusive product scan of e over the lanes
+      // ---- composite the window: lane l takes the l-th run of CH consecutive merged samples ----
+      // One product scan over the lanes' run products gives every lane its entry transmittance; the
+      // run itself is sequential (T <- T e).  The first sample, in merged order, whose T drops
+      // below t_stop still contributes (Q9); every later one contributes nothing.
+      const uint32_t CH = (cnt + 31u) >> 5;
+      const uint32_t rb = lane * CH < cnt ? lane * CH : cnt, re = rb + CH < cnt ? rb + CH : cnt;
+      float pl = 1.0f;
+      for (uint32_t r = rb; r < re; ++r) pl *= __ldg(&stg[sm.ord[r]].w);
+      float p = pl;  // inclusive product scan of the run products over the lanes
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-          const float q = __shfl_up_sync(FULL, p, o);
-          if (lane >= o) p *= q;
-        }
-        float excl = __shfl_up_sync(FULL, p, 1);
-        if (lane == 0) excl = 1.0f;
-        const float T_after = T * p;
-        const unsigned stop = __ballot_sync(FULL, valid && T_after < a.t_stop);
-        const int last = stop ? __ffs(stop) - 1 : 31;          // Q9: the stopping sample still contributes
-        float w = (valid && lane <= last) ? (T * excl) * (1.0f - v.w) : 0.f;
-        C0 = fmaf(w, v.x, C0); C1 = fmaf(w, v.y, C1); C2 = fmaf(w, v.z, C2);
-        if (FEAT && valid) s_w[FEAT ? warp : 0][FEAT ? r : 0] = w;
-        T = __shfl_sync(FULL, T_after, last);
-        if (stop) { stopped = true; done = base + (uint32_t)last + 1; break; }
+      for (int o = 1; o < 32; o <<= 1) {
+        const float q = __shfl_up_sync(FULL, p, o);
+        if (lane >= o) p *= q;
       }
+      float Tl = __shfl_up_sync(FULL, p, 1);
+      Tl = lane == 0 ? T : T * Tl;                 // transmittance in front of the lane's first sample
+      float c0 = 0.f, c1 = 0.f, c2 = 0.f;
+      uint32_t lstop = 0xffffffffu;                // the lane's first sample that crosses the threshold
+      for (uint32_t r = rb; r < re && lstop == 0xffffffffu; ++r) {
+        const float4 v = __ldg(stg + sm.ord[r]);   // 16 B gather inside the ray's contiguous staging run (second touch: L1)
+        const float w = Tl * (1.0f - v.w);
+        c0 = fmaf(w, v.x, c0); c1 = fmaf(w, v.y, c1); c2 = fmaf(w, v.z, c2);
+        if (FEAT) s_w[FEAT ? warp : 0][FEAT ? r : 0] = w;
+        Tl *= v.w;
+        if (Tl < a.t_stop) lstop = r;
+      }
+      const unsigned stop = __ballot_sync(FULL, lstop != 0xffffffffu);
+      uint32_t done = cnt;                         // samples of this window that carry a weight
+      if (stop) {
+        const int ls = __ffs(stop) - 1;            // runs are in merged order: the lowest lane stops first
+        if (lane > ls) { c0 = 0.f; c1 = 0.f; c2 = 0.f; }
+        done = __shfl_sync(FULL, lstop, ls) + 1u;
+        T = __shfl_sync(FULL, Tl, ls);
+        stopped = true;
+      } else {
+        T = __shfl_sync(FULL, Tl, 31);             // lane 31 leaves with T times the product of the whole window
+      }
+      C0 += c0; C1 += c1; C2 += c2;
       if (FEAT) {
         __syncwarp();
         const float *fbase = a.staging_feat + (size_t)off * (size_t)K * (size_t)nf;
