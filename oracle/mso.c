@@ -24,7 +24,7 @@
  * ---------------------------------------------------------------------------------------- */
 struct mso_scene {
   int32_t n;
-  int32_t n_freq, use_viewdir, n_hidden, width, n_feat;
+  int32_t n_freq, use_viewdir, n_hidden, width, n_feat, mode;
   int32_t in_dim, out_dim, n_layers, params;
   float *center;  /* [n][3] */
   float *A;       /* [n][9] world -> unit-sphere frame: diag(1/s) R^T    (Lambda = A^T A) */
@@ -61,12 +61,15 @@ int mso_scene_create(const mso_prims *p, const mso_mlp *m, mso_scene **out) {
   if (!p || !m || !out || p->n <= 0 || !p->center || !p->quat || !p->scale || !m->weights)
     return MSO_ERR_ARG;
   if (m->n_freq < 0 || m->n_hidden < 1 || m->width < 1 || m->n_feat < 0) return MSO_ERR_ARG;
+  if (m->mode != MSO_MODE_LOCAL && m->mode != MSO_MODE_CONTACT) return MSO_ERR_ARG;
+  if (m->mode == MSO_MODE_CONTACT && (m->n_freq < 1 || m->use_viewdir)) return MSO_ERR_ARG;
   mso_scene *s = (mso_scene *)calloc(1, sizeof(*s));
   if (!s) return MSO_ERR_MEM;
   s->n = p->n;
   s->n_freq = m->n_freq; s->use_viewdir = m->use_viewdir ? 1 : 0;
   s->n_hidden = m->n_hidden; s->width = m->width; s->n_feat = m->n_feat;
-  s->in_dim = 3 + 6 * m->n_freq + (s->use_viewdir ? 3 : 0);
+  s->mode = m->mode;
+  s->in_dim = m->mode == MSO_MODE_CONTACT ? 12 * m->n_freq : 3 + 6 * m->n_freq + (s->use_viewdir ? 3 : 0);
   s->out_dim = 4 + m->n_feat;
   s->n_layers = m->n_hidden + 1;
   int params = 0, in = s->in_dim;
@@ -318,10 +321,16 @@ static int intersect(const mso_scene *s, int i, const float *o, const float *d,
   float delta = (t1 - t_in) / (float)K;
   if (!(delta > 0.0f)) return 0;
   h->prim = i; h->t_in = t_in; h->delta = delta;
+  if (s->mode == MSO_MODE_CONTACT) {
+    /* Eq.2: t* = max(0, d^T Lambda (mu - o) / d^T Lambda d) = max(-b/a, .); the hit keeps
+     * (t*, chord length): K = 1, so delta above IS the chord length t1 - max(t0, t_near). */
+    float ts = (-b) / a;
+    h->t_in = ts > t_near ? ts : t_near;
+  }
   return 1;
 }
 
-static inline float sample_t(float t_in, float delta, int k) {
+static inline float sample_t(float t_in, float delta, int k) {   /* MSO_MODE_LOCAL; contact mode: the sample IS t_in = t* */
   float kf = (float)k + 0.5f;
   float off = kf * delta;
   return t_in + off;
@@ -351,6 +360,26 @@ static void encode(const mso_scene *s, const float *u, const float *d, double *x
     for (int a = 0; a < 3; ++a) x[j++] = cos(f * (double)u[a]);
   }
   if (s->use_viewdir) for (int a = 0; a < 3; ++a) x[j++] = (double)d[a];
+}
+
+/* Contact-point input (Eq.3-5): p* = o + t* d, delta = mu - p*, z = [d; delta];
+ * gamma(z): per scalar z_j, per level l: sin(2^l pi z_j), cos(2^l pi z_j).  Also returns
+ * r2 = |p* - mu|^2_Lambda = |A (p* - mu)|^2 for the falloff.  p* and A (p* - mu) in
+ * canonical fp32 (the same sample_u as the local mode), the rest fp64. */
+static void encode_contact(const mso_scene *s, int i, const float *o, const float *d, float t, double *x, double *r2) {
+  const float *mu = s->center + 3 * i;
+  float p0 = o[0] + t * d[0], p1 = o[1] + t * d[1], p2 = o[2] + t * d[2];
+  float z[6] = {d[0], d[1], d[2], mu[0] - p0, mu[1] - p1, mu[2] - p2};
+  int j = 0;
+  for (int c = 0; c < 6; ++c)
+    for (int l = 0; l < s->n_freq; ++l) {
+      double f = ldexp(MSO_PI, l);
+      x[j++] = sin(f * (double)z[c]);
+      x[j++] = cos(f * (double)z[c]);
+    }
+  float u[3];
+  sample_u(s, i, o, d, t, u);
+  *r2 = (double)u[0] * u[0] + (double)u[1] * u[1] + (double)u[2] * u[2];
 }
 
 #define MSO_MAXW 1024
@@ -390,13 +419,13 @@ static void activate(const mso_scene *s, const double *raw, double *act) {
 }
 
 int mso_encode(const mso_scene *s, const float *u, const float *d, double *x) {
-  if (!s || !u || !x || (s->use_viewdir && !d)) return MSO_ERR_ARG;
+  if (!s || !u || !x || (s->use_viewdir && !d) || s->mode != MSO_MODE_LOCAL) return MSO_ERR_ARG;
   encode(s, u, d, x);
   return MSO_OK;
 }
 
 int mso_mlp_eval(const mso_scene *s, int32_t prim, const float *u, const float *d, double *raw, double *act) {
-  if (!s || prim < 0 || prim >= s->n || !u || (s->use_viewdir && !d)) return MSO_ERR_ARG;
+  if (!s || prim < 0 || prim >= s->n || !u || (s->use_viewdir && !d) || s->mode != MSO_MODE_LOCAL) return MSO_ERR_ARG;
   if (s->in_dim > MSO_MAXW || s->width > MSO_MAXW || s->out_dim > MSO_MAXW) return MSO_ERR_ARG;
   double x[MSO_MAXW], r[MSO_MAXW], a[MSO_MAXW];
   encode(s, u, d, x);
@@ -458,7 +487,7 @@ static long gather_hits(const mso_scene *s, const mso_camera *cam, const tlists_
   return (long)nh;
 }
 
-static long build_samples(long nh, int K, raybuf_t *rb) {
+static long build_samples(const mso_scene *s, long nh, int K, raybuf_t *rb) {
   size_t ns = (size_t)nh * (size_t)K;
   if (ns > rb->scap) {
     samp_t *s2 = (samp_t *)realloc(rb->samps, ns * sizeof(samp_t));
@@ -468,7 +497,8 @@ static long build_samples(long nh, int K, raybuf_t *rb) {
   size_t j = 0;
   for (long h = 0; h < nh; ++h)
     for (int k = 0; k < K; ++k) {
-      rb->samps[j].t = sample_t(rb->hits[h].t_in, rb->hits[h].delta, k);
+      rb->samps[j].t = s->mode == MSO_MODE_CONTACT ? rb->hits[h].t_in   /* the contact point t* itself */
+                                                   : sample_t(rb->hits[h].t_in, rb->hits[h].delta, k);
       rb->samps[j].prim = rb->hits[h].prim; rb->samps[j].k = k; rb->samps[j].hit = (int32_t)h;
       ++j;
     }
@@ -476,11 +506,28 @@ static long build_samples(long nh, int K, raybuf_t *rb) {
   return (long)ns;
 }
 
+/* contact mode: input vector, raw outputs, activations and |p*-mu|^2_Lambda at o + t d (for the pins) */
+int mso_contact_eval(const mso_scene *s, int32_t prim, const float *o, const float *d, float t,
+                     double *x_out, double *raw, double *act, double *r2_out) {
+  if (!s || prim < 0 || prim >= s->n || !o || !d || s->mode != MSO_MODE_CONTACT) return MSO_ERR_ARG;
+  if (s->in_dim > MSO_MAXW || s->width > MSO_MAXW || s->out_dim > MSO_MAXW) return MSO_ERR_ARG;
+  double x[MSO_MAXW], r[MSO_MAXW], a[MSO_MAXW], r2;
+  encode_contact(s, prim, o, d, t, x, &r2);
+  mlp_forward(s, prim, x, r);
+  activate(s, r, a);
+  if (x_out) memcpy(x_out, x, (size_t)s->in_dim * sizeof(double));
+  if (raw) memcpy(raw, r, (size_t)s->out_dim * sizeof(double));
+  if (act) memcpy(act, a, (size_t)s->out_dim * sizeof(double));
+  if (r2_out) *r2_out = r2;
+  return MSO_OK;
+}
+
 int mso_render(const mso_scene *s, const mso_camera *cam, int H, int W, const mso_opts *opt,
                const int32_t *pix, int64_t n_pix, double *out_rgb, double *out_alpha,
                double *out_feat, mso_stats *stats) {
   if (!s || !cam || !opt || H <= 0 || W <= 0 || opt->K <= 0 || opt->tile < 0 || !out_rgb || !out_alpha)
     return MSO_ERR_ARG;
+  if (s->mode == MSO_MODE_CONTACT && opt->K != 1) return MSO_ERR_ARG;
   if (s->in_dim > MSO_MAXW || s->width > MSO_MAXW || s->out_dim > MSO_MAXW) return MSO_ERR_ARG;
   if (!pix) n_pix = (int64_t)H * W;
   tlists_t tl; memset(&tl, 0, sizeof(tl));
@@ -509,7 +556,7 @@ int mso_render(const mso_scene *s, const mso_camera *cam, int H, int W, const ms
       int pixel = pix ? pix[q] : (int)q;
       float o[3], d[3];
       long nh = gather_hits(s, cam, tlp, opt->tile, W, pixel, K, o, d, &rb);
-      long ns = nh >= 0 ? build_samples(nh, K, &rb) : -1;
+      long ns = nh >= 0 ? build_samples(s, nh, K, &rb) : -1;
       if (ns < 0) {
 #ifdef _OPENMP
 #pragma omp atomic write
@@ -524,13 +571,23 @@ int mso_render(const mso_scene *s, const mso_camera *cam, int H, int W, const ms
       if (F) for (int c = 0; c < nf; ++c) F[c] = 0.0;
       for (long j = 0; j < ns; ++j) {
         const samp_t *sp = &rb.samps[j];
-        float u[3];
-        sample_u(s, sp->prim, o, d, sp->t, u);
-        encode(s, u, d, x);
-        mlp_forward(s, sp->prim, x, raw);
-        activate(s, raw, act);
+        double e;                                                     /* 1 - alpha */
+        if (s->mode == MSO_MODE_CONTACT) {
+          double r2;
+          encode_contact(s, sp->prim, o, d, sp->t, x, &r2);
+          mlp_forward(s, sp->prim, x, raw);
+          activate(s, raw, act);
+          /* alpha = (1 - exp(-sigma l)) g,  g = exp(-(9/2) r2)   (readings: mso.h header) */
+          e = 1.0 - (1.0 - exp(-act[3] * (double)rb.hits[sp->hit].delta)) * exp(-4.5 * r2);
+        } else {
+          float u[3];
+          sample_u(s, sp->prim, o, d, sp->t, u);
+          encode(s, u, d, x);
+          mlp_forward(s, sp->prim, x, raw);
+          activate(s, raw, act);
+          e = exp(-act[3] * (double)rb.hits[sp->hit].delta);
+        }
         ++tot_evals;
-        double e = exp(-act[3] * (double)rb.hits[sp->hit].delta);   /* 1 - alpha */
         double w = T * (1.0 - e);
         C[0] += w * act[0]; C[1] += w * act[1]; C[2] += w * act[2];
         if (F) for (int c = 0; c < nf; ++c) F[c] += w * act[4 + c];
@@ -595,7 +652,7 @@ static int one_ray(const mso_scene *s, const mso_camera *cam, int H, int W, cons
   *nh = gather_hits(s, cam, opt->tile > 0 ? &tl : NULL, opt->tile, W, pixel, opt->K, o, d, rb);
   tlists_free(&tl);
   if (*nh < 0) return MSO_ERR_MEM;
-  if (ns) { *ns = build_samples(*nh, opt->K, rb); if (*ns < 0) return MSO_ERR_MEM; }
+  if (ns) { *ns = build_samples(s, *nh, opt->K, rb); if (*ns < 0) return MSO_ERR_MEM; }
   return MSO_OK;
 }
 

@@ -22,6 +22,18 @@
  *   binning    conservative screen-tile lists of projected supports,
  *              sorted by (tile, entry depth, primitive id)                  P:119, NS (a),(b)
  *
+ * Contact-point mode (mso_mlp.mode = MSO_MODE_CONTACT; the paper's own variant, S:Sec.8(f) NEXT-1):
+ *   one evaluation per hit (K must be 1) at the soft contact point
+ *   t* = max(d^T Lambda (mu-o) / d^T Lambda d, t_near), p* = o + t* d        P:80-86 Eq.1-2
+ *   residual delta = mu - p*, MLP input gamma([d; delta]): per scalar z_j
+ *   (d_x,d_y,d_z,delta_x,delta_y,delta_z), per level l: sin(2^l pi z_j), cos(2^l pi z_j)
+ *   -> 12 L dims, no identity                                                P:89-103 Eq.3-5
+ *   alpha = (1 - exp(-sigma l)) g, l = chord length of the ray in the support (reading of the
+ *   undefined "effective integration length"), g = exp(-(9/2) |p*-mu|^2_Lambda)
+ *   (reading of the "Gaussian falloff" whose formula the paper omits: the support
+ *   boundary |.|_Lambda = 1 sits at three standard deviations); samples ordered by (t*, primitive id).
+ *   Both readings are listed in DESIGN.md Sec.11.
+ *
  * Precision: every geometric decision (projection, tile range, intersection,
  * sample t, sample order, local coordinate u) is evaluated in IEEE fp32,
  * round-to-nearest, NO fused multiply-add, in the operation order written in
@@ -58,7 +70,10 @@ typedef struct {
   int32_t width;         /* hidden width                                               */
   int32_t n_feat;        /* linear channels after [r,g,b,sigma] */
   const float *weights;  /* [n][params]: per layer W[in][out] row-major, then b[out]   */
+  int32_t mode;          /* MSO_MODE_LOCAL (0) | MSO_MODE_CONTACT (1)                  */
 } mso_mlp;
+
+enum { MSO_MODE_LOCAL = 0, MSO_MODE_CONTACT = 1 };
 
 typedef struct {
   float fx, fy, cx, cy;
@@ -136,6 +151,9 @@ int mso_project(const mso_scene *, const mso_camera *, int H, int W, int32_t pri
  * act[out_dim] = (sigmoid rgb, softplus sigma, linear features). */
 int mso_mlp_eval(const mso_scene *, int32_t prim, const float *u, const float *d,
                  double *raw, double *act);
+/* contact mode only: x[in_dim], raw[out_dim], act[out_dim], |p*-mu|^2_Lambda of primitive prim at o + t d */
+int mso_contact_eval(const mso_scene *, int32_t prim, const float *o, const float *d, float t,
+                     double *x, double *raw, double *act, double *r2);
 /* encoded input vector x[in_dim] for (u, d). */
 int mso_encode(const mso_scene *, const float *u, const float *d, double *x);
 

@@ -20,7 +20,7 @@ class _Prims(C.Structure):
 
 class _MLP(C.Structure):
     _fields_ = [("n_freq", C.c_int32), ("use_viewdir", C.c_int32), ("n_hidden", C.c_int32),
-                ("width", C.c_int32), ("n_feat", C.c_int32), ("weights", C.c_void_p)]
+                ("width", C.c_int32), ("n_feat", C.c_int32), ("weights", C.c_void_p), ("mode", C.c_int32)]
 
 
 class _Camera(C.Structure):
@@ -84,7 +84,7 @@ class OracleScene:
         self.n = int(self._keep[0].shape[0])
         p = _Prims(self.n, _ptr(self._keep[0]), _ptr(self._keep[1]), _ptr(self._keep[2]))
         m = _MLP(scene.mlp.n_freq, scene.mlp.use_viewdir, scene.mlp.n_hidden, scene.mlp.width,
-                 scene.mlp.n_feat, _ptr(self._keep[3]))
+                 scene.mlp.n_feat, _ptr(self._keep[3]), int(getattr(scene.mlp, "mode", 0)))
         h = C.c_void_p()
         rc = lib().mso_scene_create(C.byref(p), C.byref(m), C.byref(h))
         if rc != 0:
@@ -224,6 +224,20 @@ class OracleScene:
         if rc != 0:
             raise RuntimeError(f"mso_mlp_eval failed: {rc}")
         return raw, act
+
+    def contact_eval(self, prim, o, d, t):
+        """contact mode: (x, raw, act, r2) of primitive prim at o + t d."""
+        o = np.ascontiguousarray(o, np.float32)
+        d = np.ascontiguousarray(d, np.float32)
+        x = np.zeros(self.mlp.in_dim, np.float64)
+        raw = np.zeros(self.mlp.out_dim, np.float64)
+        act = np.zeros(self.mlp.out_dim, np.float64)
+        r2 = C.c_double()
+        rc = lib().mso_contact_eval(self._h, C.c_int32(prim), _ptr(o), _ptr(d), C.c_float(t), _ptr(x), _ptr(raw),
+                                    _ptr(act), C.byref(r2))
+        if rc != 0:
+            raise RuntimeError(f"mso_contact_eval failed: {rc}")
+        return x, raw, act, r2.value
 
     def encode(self, u, d=None):
         u = np.ascontiguousarray(u, np.float32)

@@ -32,6 +32,9 @@ from dataclasses import dataclass, field, replace
 import numpy as np
 
 
+MODE_LOCAL, MODE_CONTACT = 0, 1
+
+
 @dataclass(frozen=True)
 class MLPSpec:
     n_freq: int          # L of Eq.5
@@ -40,9 +43,12 @@ class MLPSpec:
     width: int           # hidden width
     n_feat: int          # extra linear output channels after [r,g,b,sigma]
     bf16: bool           # weights are bf16-representable values
+    mode: int = 0        # 0: north-star input (local coords, K samples); 1: the paper's contact-point input (S:§8(f) NEXT-1)
 
     @property
     def in_dim(self) -> int:
+        if self.mode == MODE_CONTACT:
+            return 12 * self.n_freq            # gamma([d; delta]) of Eq.4-5: 6 scalars x 2L, no identity
         return 3 + 6 * self.n_freq + (3 if self.use_viewdir else 0)
 
     @property
@@ -98,6 +104,10 @@ CONFIGS: dict[str, SceneConfig] = {
     "cfg5": SceneConfig("cfg5", 2, 1024, 2.0, 0.05, 0.5,
                         MLPSpec(4, 1, 3, 64, 32, True), 1920, 1080, 60.0, 5.0, 16,
                         n_views=8),
+    # S:§8(f) NEXT-1, the paper's own variant: one evaluation per (ray, primitive) at
+    # the contact point, 72-32-32-4 fp32 MLPs on gamma([d; delta]); N in the paper's range (Table 6).
+    "next1": SceneConfig("next1", 6, 2048, 2.0, 0.05, 0.5,
+                         MLPSpec(6, 0, 2, 32, 0, False, MODE_CONTACT), 1280, 720, 60.0, 5.0, 1),
 }
 
 
