@@ -51,6 +51,7 @@ typedef struct {
 } ms_prims;
 
 enum { MS_F32 = 0, MS_BF16 = 1 };
+enum { MS_MODE_LOCAL = 0, MS_MODE_CONTACT = 1 };
 
 /* One MLP per primitive, all of the same shape.  Input (Q2,Q3,Q15):
  *   x = [u, sin(2^0 pi u), cos(2^0 pi u), ..., sin(2^(L-1) pi u), cos(2^(L-1) pi u)] [, d]
@@ -62,7 +63,17 @@ enum { MS_F32 = 0, MS_BF16 = 1 };
  * (input index slowest), then b[out].  P = sum(in*out + out).
  * dtype = MS_BF16 declares that the contractions run with bf16 operands on tensor cores:
  * weight matrices are rounded to bf16 (round-to-nearest-even; a no-op if already
- * representable), biases stay fp32 (Q18).  dtype = MS_F32 keeps everything fp32. */
+ * representable), biases stay fp32 (Q18).  dtype = MS_F32 keeps everything fp32.
+ *
+ * mode = MS_MODE_CONTACT selects the paper's own interaction model (S:Sec.8(f) NEXT-1)
+ * instead of the north-star's K samples per chord: ONE evaluation per (ray, primitive) hit, at
+ * the soft contact point t* = max(d^T Lambda (mu - o) / d^T Lambda d, t_near), p* = o + t* d
+ * (Eq.1-2).  Input x = gamma([d; delta]), delta = mu - p* (Eq.3-5): for scalar j of
+ * (d_x,d_y,d_z,delta_x,delta_y,delta_z) and level l, x[2L j + 2l] = sin(2^l pi z_j),
+ * x[2L j + 2l + 1] = cos(2^l pi z_j); in_dim = 12 L, no identity, use_viewdir must be 0.
+ * alpha = (1 - exp(-sigma l)) g with l = the chord length of the ray inside the support and
+ * g = exp(-(9/2) |p* - mu|^2_Lambda) (readings of P:105); hits are
+ * composited in the order of (t*, primitive id).  ms_opts.K must be 1; fp32 path only. */
 typedef struct {
   int32_t n_freq;      /* L >= 0 */
   int32_t use_viewdir; /* 0 / 1 */
@@ -72,6 +83,7 @@ typedef struct {
   int32_t dtype;       /* MS_F32 | MS_BF16 */
   const float *weights;
   size_t n_weights;    /* must equal n * P */
+  int32_t mode;        /* MS_MODE_LOCAL | MS_MODE_CONTACT */
 } ms_mlp;
 
 /* Pinhole camera (Q14): pixel (x,y), row 0 on top, looks along

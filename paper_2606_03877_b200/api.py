@@ -32,7 +32,7 @@ class _Prims(C.Structure):
 class _MLP(C.Structure):
     _fields_ = [("n_freq", C.c_int32), ("use_viewdir", C.c_int32), ("n_hidden", C.c_int32),
                 ("width", C.c_int32), ("n_feat", C.c_int32), ("dtype", C.c_int32),
-                ("weights", C.c_void_p), ("n_weights", C.c_size_t)]
+                ("weights", C.c_void_p), ("n_weights", C.c_size_t), ("mode", C.c_int32)]
 
 
 class _Camera(C.Structure):
@@ -118,7 +118,7 @@ class Scene:
         self.dtype = dtype
         p = _Prims(self.n, _ptr(center), _ptr(quat), _ptr(scale))
         m = _MLP(scene.mlp.n_freq, scene.mlp.use_viewdir, scene.mlp.n_hidden, scene.mlp.width,
-                 scene.mlp.n_feat, dtype, _ptr(weights), weights.size)
+                 scene.mlp.n_feat, dtype, _ptr(weights), weights.size, int(getattr(scene.mlp, "mode", 0)))
         h = C.c_void_p()
         rc = _lib.ms_scene_create(C.byref(p), C.byref(m), C.byref(h))
         if rc != 0:

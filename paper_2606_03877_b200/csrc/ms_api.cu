@@ -219,6 +219,7 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   ENS(sc->blk_off, (size_t)(N + 2) * 4);
   MsIsectArgs ia;
   ia.cam = cam; ia.tile = tile; ia.tiles_x = tiles_x; ia.n_tiles = n_tiles; ia.K = K; ia.prim_bits = prim_bits;
+  ia.contact = sc->shape.mode == MS_MODE_CONTACT;
   ia.keys = sorted; ia.tile_start = (uint32_t *)sc->tile_start.p; ia.A = sc->A; ia.oprime = (float *)sc->oprime.p;
   ia.rect = (int4 *)sc->rect.p; ia.emit_off = (uint32_t *)sc->emit_off.p;
   ia.pair_hits = (uint32_t *)sc->pair_hits.p; ia.ray_hits = (uint32_t *)sc->ray_hits.p;
@@ -266,6 +267,7 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   if (timing) CK(cudaEventRecord(sc->ev[4], st));
   MsCompositeArgs ca;
   ca.n_rays = R; ca.K = K; ca.n_feat = sc->shape.n_feat; ca.t_stop = opts->t_stop;
+  ca.contact = sc->shape.mode == MS_MODE_CONTACT;
   ca.ray_off = (uint32_t *)sc->ray_off.p; ca.hits = (MsHit *)sc->hits.p; ca.staging = (float4 *)sc->staging.p;
   ca.staging_feat = want_feat ? (float *)sc->staging_feat.p : nullptr;
   ca.out_rgb = out_rgb; ca.out_alpha = out_alpha; ca.out_feat = want_feat ? out_feat : nullptr;
@@ -295,6 +297,7 @@ int check_render_args(ms_scene *sc, const ms_camera *cams, int n_views, int H, i
                       const void *alpha) {
   if (!sc || !cams || !o || !rgb || !alpha || n_views < 1 || H < 1 || W < 1) return MS_ERR_INVALID_ARG;
   if (o->K < 1 || o->K > MS_MAX_K || !(o->t_stop >= 0.0f)) return MS_ERR_INVALID_ARG;
+  if (sc->shape.mode == MS_MODE_CONTACT && o->K != 1) return MS_ERR_INVALID_ARG;   // one evaluation per hit
   if (o->tile != 0 && o->tile != 8 && o->tile != 16 && o->tile != 32) return MS_ERR_INVALID_ARG;
   for (int v = 0; v < n_views; ++v)
     if (!(cams[v].fx > 0.f) || !(cams[v].fy > 0.f) || !(cams[v].t_near >= 0.f)) return MS_ERR_INVALID_ARG;
@@ -321,7 +324,10 @@ int ms_scene_create(const ms_prims *prims, const ms_mlp *mlp, ms_scene **out) {
   MsMlpShape sh;
   sh.n_freq = mlp->n_freq; sh.use_viewdir = mlp->use_viewdir ? 1 : 0; sh.n_hidden = mlp->n_hidden;
   sh.width = mlp->width; sh.n_feat = mlp->n_feat;
-  sh.in_dim = 3 + 6 * sh.n_freq + (sh.use_viewdir ? 3 : 0);
+  if (mlp->mode != MS_MODE_LOCAL && mlp->mode != MS_MODE_CONTACT) return MS_ERR_INVALID_ARG;
+  if (mlp->mode == MS_MODE_CONTACT && (mlp->n_freq < 1 || mlp->use_viewdir)) return MS_ERR_INVALID_ARG;
+  sh.mode = mlp->mode;
+  sh.in_dim = sh.mode == MS_MODE_CONTACT ? 12 * sh.n_freq : 3 + 6 * sh.n_freq + (sh.use_viewdir ? 3 : 0);
   sh.out_dim = 4 + sh.n_feat;
   sh.n_layers = sh.n_hidden + 1;
   if (sh.width > MS_MAX_WIDTH || sh.in_dim > MS_MAX_IN || sh.out_dim > MS_MAX_OUT) return MS_ERR_UNSUPPORTED_SHAPE;
@@ -395,7 +401,7 @@ int ms_scene_create(const ms_prims *prims, const ms_mlp *mlp, ms_scene **out) {
     if (!isfinite(prims->center[i])) return fail(MS_ERR_INVALID_ARG);
   CKC(cudaMallocHost(&sc->pinned, 16));
   for (int i = 0; i <= MS_N_STAGES; ++i) CKC(cudaEventCreate(&sc->ev[i]));
-  if (mlp->dtype == MS_BF16) {
+  if (mlp->dtype == MS_BF16 && sh.mode == MS_MODE_LOCAL) {   // the contact-point mode runs on the fp32 path only
     rc = ms_tc_pack(sh, sc->n, w.data(), &sc->tc);  // leaves tc.valid = false if the shape is not covered
     if (rc != MS_OK) return fail(rc);
   }
@@ -553,6 +559,7 @@ int ms_debug_sample_order(ms_scene *sc, int32_t ray, int32_t *prim, int32_t *k, 
   MsCompositeArgs ca;
   memset(&ca, 0, sizeof(ca));
   ca.n_rays = sc->dbg_H * sc->dbg_W; ca.K = sc->dbg_K; ca.n_feat = 0; ca.t_stop = 0.f;
+  ca.contact = sc->shape.mode == MS_MODE_CONTACT;
   ca.ray_off = (uint32_t *)sc->ray_off.p; ca.hits = (MsHit *)sc->hits.p; ca.staging = (float4 *)sc->staging.p;
   CK(ms_sample_order(ca, ray, dp, dk, dt, 0));
   CK(cudaDeviceSynchronize());

@@ -49,9 +49,9 @@ __device__ __forceinline__ uint32_t count_before(float tf, float tl, float ti2, 
 // rank of sample (h, k) in the order (t, prim, k).  n <= HCAP: stream-level classification in
 // sm.pre (streams entirely before / after need no per-sample work); else every stream is tested.
 __device__ __forceinline__ uint32_t sample_rank(const WarpSmem &sm, const MsHit *__restrict__ hits, int n, int K, int h,
-                                                int k, float *t_out) {
+                                                int k, float *t_out, int contact) {
   if (n <= HCAP) {
-    const float t = ms_sample_t(sm.geo[h].x, sm.geo[h].y, k);
+    const float t = ms_sample_tm(sm.geo[h].x, sm.geo[h].y, k, contact);
     const int prim = __float_as_int(sm.key[h].z);
     *t_out = t;
     const uint2 pr = sm.pre[h];
@@ -67,26 +67,26 @@ __device__ __forceinline__ uint32_t sample_rank(const WarpSmem &sm, const MsHit 
     return rank;
   }
   const MsHit me = hits[h];
-  const float t = ms_sample_t(me.t_in, me.delta, k);
+  const float t = ms_sample_tm(me.t_in, me.delta, k, contact);
   *t_out = t;
   uint32_t rank = (uint32_t)k;
   for (int h2 = 0; h2 < n; ++h2) {
     if (h2 == h) continue;
     const MsHit g = hits[h2];
-    rank += count_before(ms_sample_t(g.t_in, g.delta, 0), ms_sample_t(g.t_in, g.delta, K - 1), g.t_in, g.delta, g.prim, t,
+    rank += count_before(ms_sample_tm(g.t_in, g.delta, 0, contact), ms_sample_tm(g.t_in, g.delta, K - 1, contact), g.t_in, g.delta, g.prim, t,
                          me.prim, K);
   }
   return rank;
 }
 
 // n <= HCAP: lane h caches hit h and classifies every other stream against it
-__device__ __forceinline__ void load_hits(WarpSmem &sm, const MsHit *__restrict__ hits, int n, int K, int lane) {
+__device__ __forceinline__ void load_hits(WarpSmem &sm, const MsHit *__restrict__ hits, int n, int K, int lane, int contact) {
   if (n > HCAP) return;
   float tf = 0.f, tl = 0.f;
   int prim = 0;
   if (lane < n) {
     const MsHit g = hits[lane];
-    tf = ms_sample_t(g.t_in, g.delta, 0); tl = ms_sample_t(g.t_in, g.delta, K - 1); prim = g.prim;
+    tf = ms_sample_tm(g.t_in, g.delta, 0, contact); tl = ms_sample_tm(g.t_in, g.delta, K - 1, contact); prim = g.prim;
     sm.key[lane] = make_float4(tf, tl, __int_as_float(prim), 0.f);
     sm.geo[lane] = make_float2(g.t_in, g.delta);
   }
@@ -123,7 +123,7 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
     const MsHit *hits = a.hits + off;
     const float4 *stg = a.staging + (size_t)off * (size_t)K;
     const uint32_t S = (uint32_t)n * (uint32_t)K;
-    load_hits(sm, hits, n, K, lane);
+    load_hits(sm, hits, n, K, lane, a.contact);
     __syncwarp();
     bool stopped = false;
     for (uint32_t r0 = 0; r0 < S && !stopped; r0 += CAP) {
@@ -133,7 +133,7 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
       const int dh = 32 / K, dk = 32 - dh * K;
       for (uint32_t s = lane; s < S; s += 32) {
         float t;
-        const uint32_t rk = sample_rank(sm, hits, n, K, h, k, &t) - r0;
+        const uint32_t rk = sample_rank(sm, hits, n, K, h, k, &t, a.contact) - r0;
         if (rk < cnt) sm.ord[rk] = s;
         h += dh; k += dk;
         if (k >= K) { k -= K; ++h; }
@@ -253,13 +253,13 @@ __global__ void sample_order_kernel(MsCompositeArgs a, int ray, int *dbg_prim, i
   const int n = (int)(a.ray_off[ray + 1] - off);
   const int K = a.K;
   const MsHit *hits = a.hits + off;
-  load_hits(sm, hits, n, K, lane);
+  load_hits(sm, hits, n, K, lane, a.contact);
   __syncwarp();
   const uint32_t S = (uint32_t)n * (uint32_t)K;
   for (uint32_t s = lane; s < S; s += 32) {
     const int h = (int)(s / (uint32_t)K), k = (int)(s - (uint32_t)h * (uint32_t)K);
     float t;
-    const uint32_t rk = sample_rank(sm, hits, n, K, h, k, &t);
+    const uint32_t rk = sample_rank(sm, hits, n, K, h, k, &t, a.contact);
     dbg_prim[rk] = hits[h].prim; dbg_k[rk] = k; dbg_t[rk] = t;
   }
 }

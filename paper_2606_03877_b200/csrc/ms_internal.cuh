@@ -7,7 +7,7 @@
 #include "../../include/mlpsplat.h"
 
 #define MS_MAX_WIDTH 128
-#define MS_MAX_IN 64
+#define MS_MAX_IN 80
 #define MS_MAX_OUT 64
 #define MS_MAX_K 64
 #define MS_ROWS 128  // samples per MLP row block (one TMEM lane / one thread per sample)
@@ -41,6 +41,7 @@ struct __align__(16) MsHit {
 struct MsMlpShape {
   int n_freq, use_viewdir, n_hidden, width, n_feat;
   int in_dim, out_dim, n_layers, params;
+  int mode;  // MS_MODE_LOCAL | MS_MODE_CONTACT
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -66,8 +67,10 @@ __device__ __forceinline__ void ms_camera_ray(const MsCam &c, int x, int y, floa
 }
 
 // ray / ellipsoid chord in the unit-sphere frame; op = A (o - mu) is per primitive per view.
+// contact != 0 (MS_MODE_CONTACT, K = 1): *t_in is the contact point t* = max(-b/a, t_near) of Eq.2
+// and *delta the chord length inside the support.
 __device__ __forceinline__ bool ms_intersect(const float *A, const float *op, const float *d, float t_near,
-                                             float Kf, float *t_in, float *delta) {
+                                             float Kf, float *t_in, float *delta, int contact = 0) {
   float d0 = ms_dot3(A[0], A[1], A[2], d[0], d[1], d[2]);
   float d1 = ms_dot3(A[3], A[4], A[5], d[0], d[1], d[2]);
   float d2 = ms_dot3(A[6], A[7], A[8], d[0], d[1], d[2]);
@@ -84,6 +87,10 @@ __device__ __forceinline__ bool ms_intersect(const float *A, const float *op, co
   float ti = t0 > t_near ? t0 : t_near;
   float dl = __fdiv_rn(__fsub_rn(t1, ti), Kf);
   if (!(dl > 0.0f)) return false;
+  if (contact) {
+    const float ts = __fdiv_rn(nb, a);
+    ti = ts > t_near ? ts : t_near;
+  }
   *t_in = ti;
   *delta = dl;
   return true;
@@ -92,6 +99,10 @@ __device__ __forceinline__ bool ms_intersect(const float *A, const float *op, co
 __device__ __forceinline__ float ms_sample_t(float t_in, float delta, int k) {
   float kf = __fadd_rn((float)k, 0.5f);
   return __fadd_rn(t_in, __fmul_rn(kf, delta));
+}
+// sample position of either mode: the contact point itself in MS_MODE_CONTACT
+__device__ __forceinline__ float ms_sample_tm(float t_in, float delta, int k, int contact) {
+  return contact ? t_in : ms_sample_t(t_in, delta, k);
 }
 
 // u = A ((o + t d) - mu)
@@ -135,7 +146,7 @@ cudaError_t ms_tile_ranges(const uint64_t *keys, size_t n_pairs, int n_tiles, in
 // ms_isect.cu
 struct MsIsectArgs {
   MsCam cam;
-  int tile, tiles_x, n_tiles, K, prim_bits;
+  int tile, tiles_x, n_tiles, K, prim_bits, contact;
   const uint64_t *keys;        // sorted
   const uint32_t *tile_start;  // [n_tiles+1]
   const float *A;              // [N][9]
@@ -173,7 +184,7 @@ cudaError_t ms_mlp_f32(const MsMlpArgs &a, cudaStream_t s);
 
 // ms_composite.cu
 struct MsCompositeArgs {
-  int n_rays, K, n_feat;
+  int n_rays, K, n_feat, contact;
   float t_stop;
   const uint32_t *ray_off;  // [R+1]
   const MsHit *hits;

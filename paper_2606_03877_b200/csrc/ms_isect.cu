@@ -42,7 +42,7 @@ __global__ void isect_kernel(MsIsectArgs a) {
 #pragma unroll
     for (int q = 0; q < 3; ++q) ol[q] = __ldg(op + q);
     float t_in = 0.f, delta = 0.f;
-    const bool hit = valid && ms_intersect(Al, ol, d, a.cam.t_near, Kf, &t_in, &delta);
+    const bool hit = valid && ms_intersect(Al, ol, d, a.cam.t_near, Kf, &t_in, &delta, a.contact);
     const int4 rc = a.rect[prim];
     const uint32_t emit = a.emit_off[prim] + (uint32_t)((tile_y - rc.y) * (rc.z - rc.x + 1) + (tile_x - rc.x));
     if (!FILL) {

@@ -35,12 +35,28 @@ __global__ void __launch_bounds__(MS_ROWS) mlp_f32_kernel(MsMlpArgs a) {
   if (j >= count) return;
   const MsInterval iv = a.intervals[first + j];
   const float d[3] = {iv.dx, iv.dy, iv.dz};
-  const float t = ms_sample_t(iv.t_in, iv.delta, k);
+  const bool contact = sh.mode == MS_MODE_CONTACT;
+  const float t = ms_sample_tm(iv.t_in, iv.delta, k, contact);
   float u[3];
   ms_sample_u(a.A + 9 * (size_t)prim, a.center + 3 * (size_t)prim, a.cam.o, d, t, u);
 
   float ha[MS_MAX_WIDTH], hb[MS_MAX_WIDTH];
   int n_in = 0;
+  if (contact) {
+    // P:89-103 Eq.3-5: z = [d; mu - p*], x[2L j + 2l] = sin(2^l pi z_j), x[2L j + 2l + 1] = cos(2^l pi z_j)
+    const float *mu = a.center + 3 * (size_t)prim;
+    float z[6] = {d[0], d[1], d[2], 0.f, 0.f, 0.f};
+#pragma unroll
+    for (int c = 0; c < 3; ++c) z[3 + c] = __fsub_rn(mu[c], __fadd_rn(a.cam.o[c], __fmul_rn(t, d[c])));
+    for (int c = 0; c < 6; ++c) {
+      float scale = 1.0f;
+      for (int l = 0; l < sh.n_freq; ++l) {
+        sincospif(scale * z[c], &ha[n_in], &ha[n_in + 1]);  // 2^l z is exact
+        n_in += 2;
+        scale *= 2.0f;
+      }
+    }
+  } else {
   ha[n_in++] = u[0]; ha[n_in++] = u[1]; ha[n_in++] = u[2];
   float scale = 1.0f;
   for (int l = 0; l < sh.n_freq; ++l) {
@@ -52,6 +68,7 @@ __global__ void __launch_bounds__(MS_ROWS) mlp_f32_kernel(MsMlpArgs a) {
     scale *= 2.0f;
   }
   if (sh.use_viewdir) { ha[n_in++] = d[0]; ha[n_in++] = d[1]; ha[n_in++] = d[2]; }
+  }
 
   float *src = ha, *dst = hb;
   const float *w = w_s;
@@ -75,6 +92,10 @@ __global__ void __launch_bounds__(MS_ROWS) mlp_f32_kernel(MsMlpArgs a) {
   r.z = 1.0f / (1.0f + expf(-raw[2]));
   const float sigma = fmaxf(raw[3], 0.0f) + log1pf(expf(-fabsf(raw[3])));
   r.w = expf(-sigma * iv.delta);  // e = 1 - alpha
+  if (contact) {  // alpha = (1 - exp(-sigma l)) g, g = exp(-(9/2) |p* - mu|^2_Lambda)  (include/mlpsplat.h)
+    const float r2 = u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
+    r.w = 1.0f - (1.0f - r.w) * expf(-4.5f * r2);
+  }
   const size_t out = (size_t)(uint32_t)iv.slot * (size_t)a.K + (size_t)k;
   a.staging[out] = r;
   if (a.staging_feat)

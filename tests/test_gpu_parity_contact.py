@@ -1,0 +1,65 @@
+"""GPU parity, contact-point mode (S:Sec.8(f) NEXT-1; the paper's own variant P:80-105): the CUDA
+render through the C ABI against the oracle's contact mode on the same seeded inputs.  Same bar as
+the fp32 path: tile lists, hit lists (t*, chord length) and the per-ray order bit-exact; rgb/alpha
+within 1e-5 max abs."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import mso
+from paper_2606_03877_b200 import synth
+from test_gpu_parity_fp32 import TOL_FP32, render_both
+
+pytestmark = pytest.mark.gpu
+
+
+def _api():
+    from paper_2606_03877_b200 import api
+    return api
+
+
+@pytest.mark.parametrize("W,H,tile", [(160, 90, 16), (97, 61, 8), (64, 36, 32)])
+def test_next1_shrunk(W, H, tile):
+    cfg = synth.shrink(synth.CONFIGS["next1"], W, H)
+    sc, cam = synth.make_scene(cfg), synth.make_cameras(cfg)[0]
+    g, o, st = render_both(sc, cam, H, W, 1, tile=tile)
+    assert st.n_intervals > 2 * W * H and st.n_samples == st.n_intervals
+    assert np.abs(g[0] - o[0]).max() <= TOL_FP32 and np.abs(g[1] - o[1]).max() <= TOL_FP32
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_contact_eye_inside_cloud(seed):
+    """t* clamps to t_near when the eye is inside a support; supports straddle the eye plane."""
+    mlp = synth.MLPSpec(3, 0, 1, 16, 0, False, synth.MODE_CONTACT)
+    sc, cam, cfg = synth.random_tiny_scene(seed, n=16, mlp=mlp)
+    g, o, st = render_both(sc, cam, cfg.height, cfg.width, 1, tile=8)
+    assert st.n_intervals > 0
+    assert np.abs(g[0] - o[0]).max() <= TOL_FP32 and np.abs(g[1] - o[1]).max() <= TOL_FP32
+
+
+def test_next1_full_size_sampled_pixels():
+    """The bench configuration at its full 1280x720 size; the oracle computes a seeded pixel sample."""
+    api = _api()
+    cfg = synth.CONFIGS["next1"]
+    sc, cam = synth.make_scene(cfg), synth.make_cameras(cfg)[0]
+    gs = api.Scene(sc)
+    rgb, alpha, _ = gs.render(cam, cfg.height, cfg.width, 1)
+    torch.cuda.synchronize()
+    pix = np.random.default_rng(2).choice(cfg.width * cfg.height, 20000, replace=False).astype(np.int32)
+    o_rgb, o_alpha, _, st = mso.OracleScene(sc).render(cam, cfg.height, cfg.width, 1, pixels=pix)
+    assert st.n_intervals > 3 * len(pix)
+    assert np.abs(rgb.cpu().numpy().reshape(-1, 3)[pix] - o_rgb).max() <= TOL_FP32
+    assert np.abs(alpha.cpu().numpy().reshape(-1)[pix] - o_alpha).max() <= TOL_FP32
+    a = alpha.cpu().numpy()
+    assert a.min() >= 0 and a.max() <= 1 and (rgb.cpu().numpy() <= a[..., None] + 1e-6).all()
+
+
+def test_contact_mode_argument_checks():
+    api = _api()
+    cfg = synth.shrink(synth.CONFIGS["next1"], 32, 18)
+    sc, cam = synth.make_scene(cfg), synth.make_cameras(cfg)[0]
+    gs = api.Scene(sc)
+    with pytest.raises(api.MsError):
+        gs.render(cam, 18, 32, 4)                                   # K samples per chord is the other mode
+    with pytest.raises(api.MsError):
+        gs.render(cam, 18, 32, 1, path=api.PATH_BF16_TC)            # fp32 path only
