@@ -102,14 +102,151 @@ __global__ void __launch_bounds__(MS_ROWS) mlp_f32_kernel(MsMlpArgs a) {
     for (int c = 0; c < sh.n_feat; ++c) a.staging_feat[out * sh.n_feat + c] = raw[4 + c];
 }
 
+
+// 32-wide MLPs (CFG1 27-32-32-4; the paper's own 72-32-32-4): the same arithmetic in the same
+// order as mlp_f32_kernel (acc = b; acc = fma(x_i, W[i][o], acc) for i ascending), but the 32
+// accumulators and activations live in registers and the encoded input is fed one element at a time
+// as it is produced, each with one broadcast row of W1 (8 x LDS.128) -- no local-memory arrays.
+template <int NH>
+__global__ void __launch_bounds__(MS_ROWS) mlp_f32_w32_kernel(MsMlpArgs a) {
+  extern __shared__ __align__(16) float w_s[];
+  __shared__ int s_prim;
+  const MsMlpShape &sh = a.shape;
+  if (threadIdx.x == 0) s_prim = find_prim(a.blk_off, a.n_prims, blockIdx.x);
+  __syncthreads();
+  const int prim = s_prim;
+  {
+    const float4 *wg = reinterpret_cast<const float4 *>(a.weights_f32 + (size_t)prim * sh.params);   // params % 4 == 0 for these shapes
+    float4 *ws4 = reinterpret_cast<float4 *>(w_s);
+    for (int i = threadIdx.x; i < sh.params / 4; i += blockDim.x) ws4[i] = __ldg(wg + i);
+  }
+  __syncthreads();
+
+  const uint32_t first = a.prim_start[prim], count = a.prim_start[prim + 1] - first;
+  const uint64_t s = (uint64_t)(blockIdx.x - a.blk_off[prim]) * MS_ROWS + threadIdx.x;
+  const uint32_t j = (uint32_t)(s / (uint32_t)a.K);
+  const int k = (int)(s % (uint32_t)a.K);
+  if (j >= count) return;
+  const MsInterval iv = a.intervals[first + j];
+  const float d[3] = {iv.dx, iv.dy, iv.dz};
+  const bool contact = sh.mode == MS_MODE_CONTACT;
+  const float t = ms_sample_tm(iv.t_in, iv.delta, k, contact);
+  float u[3];
+  ms_sample_u(a.A + 9 * (size_t)prim, a.center + 3 * (size_t)prim, a.cam.o, d, t, u);
+
+  float acc[32];
+  const int n_in = sh.in_dim;
+  {
+    const float4 *b4 = reinterpret_cast<const float4 *>(w_s + n_in * 32);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) { const float4 v = b4[q]; acc[4 * q] = v.x; acc[4 * q + 1] = v.y; acc[4 * q + 2] = v.z; acc[4 * q + 3] = v.w; }
+  }
+  int row = 0;
+  auto feed = [&](float x) {   // acc += x * W1[row][:]
+    const float4 *wr = reinterpret_cast<const float4 *>(w_s + row * 32);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+      const float4 v = wr[q];
+      acc[4 * q] = fmaf(x, v.x, acc[4 * q]); acc[4 * q + 1] = fmaf(x, v.y, acc[4 * q + 1]);
+      acc[4 * q + 2] = fmaf(x, v.z, acc[4 * q + 2]); acc[4 * q + 3] = fmaf(x, v.w, acc[4 * q + 3]);
+    }
+    ++row;
+  };
+  if (contact) {
+    // P:89-103 Eq.3-5: z = [d; mu - p*], x[2L j + 2l] = sin(2^l pi z_j), x[2L j + 2l + 1] = cos(2^l pi z_j)
+    const float *mu = a.center + 3 * (size_t)prim;
+    float z[6] = {d[0], d[1], d[2], 0.f, 0.f, 0.f};
+#pragma unroll
+    for (int c = 0; c < 3; ++c) z[3 + c] = __fsub_rn(mu[c], __fadd_rn(a.cam.o[c], __fmul_rn(t, d[c])));
+#pragma unroll
+    for (int c = 0; c < 6; ++c) {
+      float scale = 1.0f;
+      for (int l = 0; l < sh.n_freq; ++l) {
+        float sv, cv;
+        sincospif(scale * z[c], &sv, &cv);  // 2^l z is exact
+        feed(sv); feed(cv);
+        scale *= 2.0f;
+      }
+    }
+  } else {
+    feed(u[0]); feed(u[1]); feed(u[2]);
+    float scale = 1.0f;
+    for (int l = 0; l < sh.n_freq; ++l) {
+      float sv[3], cv[3];
+#pragma unroll
+      for (int c = 0; c < 3; ++c) sincospif(scale * u[c], &sv[c], &cv[c]);  // 2^l u is exact
+      feed(sv[0]); feed(sv[1]); feed(sv[2]);
+      feed(cv[0]); feed(cv[1]); feed(cv[2]);
+      scale *= 2.0f;
+    }
+    if (sh.use_viewdir) { feed(d[0]); feed(d[1]); feed(d[2]); }
+  }
+  float h[32];
+#pragma unroll
+  for (int o = 0; o < 32; ++o) h[o] = fmaxf(acc[o], 0.0f);
+  const float *w = w_s + n_in * 32 + 32;
+#pragma unroll
+  for (int l = 1; l < NH; ++l) {
+    const float4 *b4 = reinterpret_cast<const float4 *>(w + 32 * 32);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) { const float4 v = b4[q]; acc[4 * q] = v.x; acc[4 * q + 1] = v.y; acc[4 * q + 2] = v.z; acc[4 * q + 3] = v.w; }
+#pragma unroll
+    for (int i = 0; i < 32; ++i) {
+      const float4 *wr = reinterpret_cast<const float4 *>(w + i * 32);
+#pragma unroll
+      for (int q = 0; q < 8; ++q) {
+        const float4 v = wr[q];
+        acc[4 * q] = fmaf(h[i], v.x, acc[4 * q]); acc[4 * q + 1] = fmaf(h[i], v.y, acc[4 * q + 1]);
+        acc[4 * q + 2] = fmaf(h[i], v.z, acc[4 * q + 2]); acc[4 * q + 3] = fmaf(h[i], v.w, acc[4 * q + 3]);
+      }
+    }
+#pragma unroll
+    for (int o = 0; o < 32; ++o) h[o] = fmaxf(acc[o], 0.0f);
+    w += 32 * 32 + 32;
+  }
+  // head: raw[o] = b[o] + sum_i h[i] Wh[i][o]
+  const int n_out = sh.out_dim;
+  const float *bh = w + 32 * n_out;
+  float raw4[4];
+#pragma unroll
+  for (int o = 0; o < 4; ++o) {
+    float r = bh[o];
+#pragma unroll
+    for (int i = 0; i < 32; ++i) r = fmaf(h[i], w[i * n_out + o], r);
+    raw4[o] = r;
+  }
+  float4 r;
+  r.x = 1.0f / (1.0f + expf(-raw4[0]));
+  r.y = 1.0f / (1.0f + expf(-raw4[1]));
+  r.z = 1.0f / (1.0f + expf(-raw4[2]));
+  const float sigma = fmaxf(raw4[3], 0.0f) + log1pf(expf(-fabsf(raw4[3])));
+  r.w = expf(-sigma * iv.delta);  // e = 1 - alpha
+  if (contact) {  // alpha = (1 - exp(-sigma l)) g, g = exp(-(9/2) |p* - mu|^2_Lambda)  (include/mlpsplat.h)
+    const float r2 = u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
+    r.w = 1.0f - (1.0f - r.w) * expf(-4.5f * r2);
+  }
+  const size_t out = (size_t)(uint32_t)iv.slot * (size_t)a.K + (size_t)k;
+  a.staging[out] = r;
+  if (a.staging_feat)
+    for (int c = 0; c < sh.n_feat; ++c) {
+      float f = bh[4 + c];
+#pragma unroll
+      for (int i = 0; i < 32; ++i) f = fmaf(h[i], w[i * n_out + 4 + c], f);
+      a.staging_feat[out * sh.n_feat + c] = f;
+    }
+}
+
 }  // namespace
 
 cudaError_t ms_mlp_f32(const MsMlpArgs &a, cudaStream_t s) {
   if (a.n_blocks == 0) return cudaSuccess;
   size_t smem = (size_t)a.shape.params * sizeof(float);
-  cudaError_t e = cudaFuncSetAttribute(mlp_f32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  void (*fn)(MsMlpArgs) = mlp_f32_kernel;
+  if (a.shape.width == 32 && a.shape.params % 4 == 0 && a.shape.n_hidden >= 1 && a.shape.n_hidden <= 3)
+    fn = a.shape.n_hidden == 1 ? mlp_f32_w32_kernel<1> : (a.shape.n_hidden == 2 ? mlp_f32_w32_kernel<2> : mlp_f32_w32_kernel<3>);
+  cudaError_t e = cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  mlp_f32_kernel<<<a.n_blocks, MS_ROWS, smem, s>>>(a);
+  fn<<<a.n_blocks, MS_ROWS, smem, s>>>(a);
   MS_LAUNCHED();
   return cudaGetLastError();
 }
