@@ -107,8 +107,11 @@ __global__ void __launch_bounds__(MS_ROWS) mlp_f32_kernel(MsMlpArgs a) {
 // order as mlp_f32_kernel (acc = b; acc = fma(x_i, W[i][o], acc) for i ascending), but the 32
 // accumulators and activations live in registers and the encoded input is fed one element at a time
 // as it is produced, each with one broadcast row of W1 (8 x LDS.128) -- no local-memory arrays.
-template <int NH>
-__global__ void __launch_bounds__(MS_ROWS) mlp_f32_w32_kernel(MsMlpArgs a) {
+// Each thread carries SPT = 2 samples (rows r and r + 64 of the block) so that a weight row loaded
+// from shared memory feeds 64 FMAs: with one sample per thread the kernel was bound by the
+// shared-memory wavefronts of the broadcast loads (84 % of peak, profiles/r1e_summary.md).
+template <int NH, int SPT>
+__global__ void __launch_bounds__(MS_ROWS / SPT) mlp_f32_w32_kernel(MsMlpArgs a) {
   extern __shared__ __align__(16) float w_s[];
   __shared__ int s_prim;
   const MsMlpShape &sh = a.shape;
@@ -123,117 +126,164 @@ __global__ void __launch_bounds__(MS_ROWS) mlp_f32_w32_kernel(MsMlpArgs a) {
   __syncthreads();
 
   const uint32_t first = a.prim_start[prim], count = a.prim_start[prim + 1] - first;
-  const uint64_t s = (uint64_t)(blockIdx.x - a.blk_off[prim]) * MS_ROWS + threadIdx.x;
-  const uint32_t j = (uint32_t)(s / (uint32_t)a.K);
-  const int k = (int)(s % (uint32_t)a.K);
-  if (j >= count) return;
-  const MsInterval iv = a.intervals[first + j];
-  const float d[3] = {iv.dx, iv.dy, iv.dz};
   const bool contact = sh.mode == MS_MODE_CONTACT;
-  const float t = ms_sample_tm(iv.t_in, iv.delta, k, contact);
-  float u[3];
-  ms_sample_u(a.A + 9 * (size_t)prim, a.center + 3 * (size_t)prim, a.cam.o, d, t, u);
+  const float *mu = a.center + 3 * (size_t)prim;
+  bool live[SPT];
+  int kk[SPT];
+  MsInterval iv[SPT];
+  float u[SPT][3], z[SPT][6];
+#pragma unroll
+  for (int q = 0; q < SPT; ++q) {
+    const uint64_t s = (uint64_t)(blockIdx.x - a.blk_off[prim]) * MS_ROWS + threadIdx.x + q * (MS_ROWS / SPT);
+    const uint32_t j = (uint32_t)(s / (uint32_t)a.K);
+    kk[q] = (int)(s % (uint32_t)a.K);
+    live[q] = j < count;
+    iv[q] = a.intervals[first + (live[q] ? j : 0u)];   // a dead row recomputes interval 0 and stores nothing
+    const float d[3] = {iv[q].dx, iv[q].dy, iv[q].dz};
+    const float t = ms_sample_tm(iv[q].t_in, iv[q].delta, kk[q], contact);
+    ms_sample_u(a.A + 9 * (size_t)prim, mu, a.cam.o, d, t, u[q]);
+    // P:89-103 Eq.3-5: z = [d; mu - p*]
+    z[q][0] = d[0]; z[q][1] = d[1]; z[q][2] = d[2];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) z[q][3 + c] = __fsub_rn(mu[c], __fadd_rn(a.cam.o[c], __fmul_rn(t, d[c])));
+  }
+  if (count == 0) return;
 
-  float acc[32];
+  float acc[SPT][32];
   const int n_in = sh.in_dim;
   {
     const float4 *b4 = reinterpret_cast<const float4 *>(w_s + n_in * 32);
 #pragma unroll
-    for (int q = 0; q < 8; ++q) { const float4 v = b4[q]; acc[4 * q] = v.x; acc[4 * q + 1] = v.y; acc[4 * q + 2] = v.z; acc[4 * q + 3] = v.w; }
+    for (int q = 0; q < 8; ++q) {
+      const float4 v = b4[q];
+#pragma unroll
+      for (int p = 0; p < SPT; ++p) { acc[p][4 * q] = v.x; acc[p][4 * q + 1] = v.y; acc[p][4 * q + 2] = v.z; acc[p][4 * q + 3] = v.w; }
+    }
   }
   int row = 0;
-  auto feed = [&](float x) {   // acc += x * W1[row][:]
+  auto feed = [&](const float (&x)[SPT]) {   // acc[p] += x[p] * W1[row][:]
     const float4 *wr = reinterpret_cast<const float4 *>(w_s + row * 32);
 #pragma unroll
     for (int q = 0; q < 8; ++q) {
       const float4 v = wr[q];
-      acc[4 * q] = fmaf(x, v.x, acc[4 * q]); acc[4 * q + 1] = fmaf(x, v.y, acc[4 * q + 1]);
-      acc[4 * q + 2] = fmaf(x, v.z, acc[4 * q + 2]); acc[4 * q + 3] = fmaf(x, v.w, acc[4 * q + 3]);
+#pragma unroll
+      for (int p = 0; p < SPT; ++p) {
+        acc[p][4 * q] = fmaf(x[p], v.x, acc[p][4 * q]); acc[p][4 * q + 1] = fmaf(x[p], v.y, acc[p][4 * q + 1]);
+        acc[p][4 * q + 2] = fmaf(x[p], v.z, acc[p][4 * q + 2]); acc[p][4 * q + 3] = fmaf(x[p], v.w, acc[p][4 * q + 3]);
+      }
     }
     ++row;
   };
   if (contact) {
-    // P:89-103 Eq.3-5: z = [d; mu - p*], x[2L j + 2l] = sin(2^l pi z_j), x[2L j + 2l + 1] = cos(2^l pi z_j)
-    const float *mu = a.center + 3 * (size_t)prim;
-    float z[6] = {d[0], d[1], d[2], 0.f, 0.f, 0.f};
-#pragma unroll
-    for (int c = 0; c < 3; ++c) z[3 + c] = __fsub_rn(mu[c], __fadd_rn(a.cam.o[c], __fmul_rn(t, d[c])));
+    // x[2L j + 2l] = sin(2^l pi z_j), x[2L j + 2l + 1] = cos(2^l pi z_j)
 #pragma unroll
     for (int c = 0; c < 6; ++c) {
       float scale = 1.0f;
       for (int l = 0; l < sh.n_freq; ++l) {
-        float sv, cv;
-        sincospif(scale * z[c], &sv, &cv);  // 2^l z is exact
+        float sv[SPT], cv[SPT];
+#pragma unroll
+        for (int p = 0; p < SPT; ++p) sincospif(scale * z[p][c], &sv[p], &cv[p]);  // 2^l z is exact
         feed(sv); feed(cv);
         scale *= 2.0f;
       }
     }
   } else {
-    feed(u[0]); feed(u[1]); feed(u[2]);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      float x[SPT];
+#pragma unroll
+      for (int p = 0; p < SPT; ++p) x[p] = u[p][c];
+      feed(x);
+    }
     float scale = 1.0f;
     for (int l = 0; l < sh.n_freq; ++l) {
-      float sv[3], cv[3];
+      float sv[3][SPT], cv[3][SPT];
 #pragma unroll
-      for (int c = 0; c < 3; ++c) sincospif(scale * u[c], &sv[c], &cv[c]);  // 2^l u is exact
+      for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int p = 0; p < SPT; ++p) sincospif(scale * u[p][c], &sv[c][p], &cv[c][p]);  // 2^l u is exact
       feed(sv[0]); feed(sv[1]); feed(sv[2]);
       feed(cv[0]); feed(cv[1]); feed(cv[2]);
       scale *= 2.0f;
     }
-    if (sh.use_viewdir) { feed(d[0]); feed(d[1]); feed(d[2]); }
-  }
-  float h[32];
+    if (sh.use_viewdir) {
 #pragma unroll
-  for (int o = 0; o < 32; ++o) h[o] = fmaxf(acc[o], 0.0f);
+      for (int c = 0; c < 3; ++c) {
+        float x[SPT];
+#pragma unroll
+        for (int p = 0; p < SPT; ++p) x[p] = z[p][c];
+        feed(x);
+      }
+    }
+  }
+  float h[SPT][32];
+#pragma unroll
+  for (int p = 0; p < SPT; ++p)
+#pragma unroll
+    for (int o = 0; o < 32; ++o) h[p][o] = fmaxf(acc[p][o], 0.0f);
   const float *w = w_s + n_in * 32 + 32;
 #pragma unroll
   for (int l = 1; l < NH; ++l) {
     const float4 *b4 = reinterpret_cast<const float4 *>(w + 32 * 32);
 #pragma unroll
-    for (int q = 0; q < 8; ++q) { const float4 v = b4[q]; acc[4 * q] = v.x; acc[4 * q + 1] = v.y; acc[4 * q + 2] = v.z; acc[4 * q + 3] = v.w; }
+    for (int q = 0; q < 8; ++q) {
+      const float4 v = b4[q];
+#pragma unroll
+      for (int p = 0; p < SPT; ++p) { acc[p][4 * q] = v.x; acc[p][4 * q + 1] = v.y; acc[p][4 * q + 2] = v.z; acc[p][4 * q + 3] = v.w; }
+    }
 #pragma unroll
     for (int i = 0; i < 32; ++i) {
       const float4 *wr = reinterpret_cast<const float4 *>(w + i * 32);
 #pragma unroll
       for (int q = 0; q < 8; ++q) {
         const float4 v = wr[q];
-        acc[4 * q] = fmaf(h[i], v.x, acc[4 * q]); acc[4 * q + 1] = fmaf(h[i], v.y, acc[4 * q + 1]);
-        acc[4 * q + 2] = fmaf(h[i], v.z, acc[4 * q + 2]); acc[4 * q + 3] = fmaf(h[i], v.w, acc[4 * q + 3]);
+#pragma unroll
+        for (int p = 0; p < SPT; ++p) {
+          acc[p][4 * q] = fmaf(h[p][i], v.x, acc[p][4 * q]); acc[p][4 * q + 1] = fmaf(h[p][i], v.y, acc[p][4 * q + 1]);
+          acc[p][4 * q + 2] = fmaf(h[p][i], v.z, acc[p][4 * q + 2]); acc[p][4 * q + 3] = fmaf(h[p][i], v.w, acc[p][4 * q + 3]);
+        }
       }
     }
 #pragma unroll
-    for (int o = 0; o < 32; ++o) h[o] = fmaxf(acc[o], 0.0f);
+    for (int p = 0; p < SPT; ++p)
+#pragma unroll
+      for (int o = 0; o < 32; ++o) h[p][o] = fmaxf(acc[p][o], 0.0f);
     w += 32 * 32 + 32;
   }
   // head: raw[o] = b[o] + sum_i h[i] Wh[i][o]
   const int n_out = sh.out_dim;
   const float *bh = w + 32 * n_out;
-  float raw4[4];
 #pragma unroll
-  for (int o = 0; o < 4; ++o) {
-    float r = bh[o];
+  for (int p = 0; p < SPT; ++p) {
+    if (!live[p]) continue;
+    float raw4[4];
 #pragma unroll
-    for (int i = 0; i < 32; ++i) r = fmaf(h[i], w[i * n_out + o], r);
-    raw4[o] = r;
-  }
-  float4 r;
-  r.x = 1.0f / (1.0f + expf(-raw4[0]));
-  r.y = 1.0f / (1.0f + expf(-raw4[1]));
-  r.z = 1.0f / (1.0f + expf(-raw4[2]));
-  const float sigma = fmaxf(raw4[3], 0.0f) + log1pf(expf(-fabsf(raw4[3])));
-  r.w = expf(-sigma * iv.delta);  // e = 1 - alpha
-  if (contact) {  // alpha = (1 - exp(-sigma l)) g, g = exp(-(9/2) |p* - mu|^2_Lambda)  (include/mlpsplat.h)
-    const float r2 = u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
-    r.w = 1.0f - (1.0f - r.w) * expf(-4.5f * r2);
-  }
-  const size_t out = (size_t)(uint32_t)iv.slot * (size_t)a.K + (size_t)k;
-  a.staging[out] = r;
-  if (a.staging_feat)
-    for (int c = 0; c < sh.n_feat; ++c) {
-      float f = bh[4 + c];
+    for (int o = 0; o < 4; ++o) {
+      float r = bh[o];
 #pragma unroll
-      for (int i = 0; i < 32; ++i) f = fmaf(h[i], w[i * n_out + 4 + c], f);
-      a.staging_feat[out * sh.n_feat + c] = f;
+      for (int i = 0; i < 32; ++i) r = fmaf(h[p][i], w[i * n_out + o], r);
+      raw4[o] = r;
     }
+    float4 r;
+    r.x = 1.0f / (1.0f + expf(-raw4[0]));
+    r.y = 1.0f / (1.0f + expf(-raw4[1]));
+    r.z = 1.0f / (1.0f + expf(-raw4[2]));
+    const float sigma = fmaxf(raw4[3], 0.0f) + log1pf(expf(-fabsf(raw4[3])));
+    r.w = expf(-sigma * iv[p].delta);  // e = 1 - alpha
+    if (contact) {  // alpha = (1 - exp(-sigma l)) g, g = exp(-(9/2) |p* - mu|^2_Lambda)  (include/mlpsplat.h)
+      const float r2 = u[p][0] * u[p][0] + u[p][1] * u[p][1] + u[p][2] * u[p][2];
+      r.w = 1.0f - (1.0f - r.w) * expf(-4.5f * r2);
+    }
+    const size_t out = (size_t)(uint32_t)iv[p].slot * (size_t)a.K + (size_t)kk[p];
+    a.staging[out] = r;
+    if (a.staging_feat)
+      for (int c = 0; c < sh.n_feat; ++c) {
+        float f = bh[4 + c];
+#pragma unroll
+        for (int i = 0; i < 32; ++i) f = fmaf(h[p][i], w[i * n_out + 4 + c], f);
+        a.staging_feat[out * sh.n_feat + c] = f;
+      }
+  }
 }
 
 }  // namespace
@@ -242,11 +292,14 @@ cudaError_t ms_mlp_f32(const MsMlpArgs &a, cudaStream_t s) {
   if (a.n_blocks == 0) return cudaSuccess;
   size_t smem = (size_t)a.shape.params * sizeof(float);
   void (*fn)(MsMlpArgs) = mlp_f32_kernel;
-  if (a.shape.width == 32 && a.shape.params % 4 == 0 && a.shape.n_hidden >= 1 && a.shape.n_hidden <= 3)
-    fn = a.shape.n_hidden == 1 ? mlp_f32_w32_kernel<1> : (a.shape.n_hidden == 2 ? mlp_f32_w32_kernel<2> : mlp_f32_w32_kernel<3>);
+  int threads = MS_ROWS;
+  if (a.shape.width == 32 && a.shape.params % 4 == 0 && a.shape.n_hidden >= 1 && a.shape.n_hidden <= 3) {
+    fn = a.shape.n_hidden == 1 ? mlp_f32_w32_kernel<1, 2> : (a.shape.n_hidden == 2 ? mlp_f32_w32_kernel<2, 2> : mlp_f32_w32_kernel<3, 2>);
+    threads = MS_ROWS / 2;
+  }
   cudaError_t e = cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  fn<<<a.n_blocks, MS_ROWS, smem, s>>>(a);
+  fn<<<a.n_blocks, threads, smem, s>>>(a);
   MS_LAUNCHED();
   return cudaGetLastError();
 }

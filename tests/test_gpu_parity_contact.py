@@ -63,3 +63,21 @@ def test_contact_mode_argument_checks():
         gs.render(cam, 18, 32, 4)                                   # K samples per chord is the other mode
     with pytest.raises(api.MsError):
         gs.render(cam, 18, 32, 1, path=api.PATH_BF16_TC)            # fp32 path only
+
+
+def test_contact_dense_scene_early_termination_and_t_near():
+    """Opaque primitives (sigma-bias 8): rays stop at T < 1e-4 in contact mode too; and a camera with
+    t_near > 0 (t* clamps to t_near, supports in front of it only)."""
+    from dataclasses import replace
+    cfg = synth.SceneConfig("dense_c", 9, 64, 1.0, 0.3, 0.8, synth.MLPSpec(4, 0, 2, 32, 0, False, synth.MODE_CONTACT),
+                            96, 80, 50.0, 3.0, 1, sigma_bias=8.0)
+    sc, cam = synth.make_scene(cfg), synth.make_cameras(cfg)[0]
+    g, o, st = render_both(sc, cam, cfg.height, cfg.width, 1)
+    assert st.n_terminated > 100
+    d = np.maximum(np.abs(g[0] - o[0]).max(axis=1), np.abs(g[1] - o[1]))
+    assert (d > TOL_FP32).sum() <= 2 and d.max() < 1.5e-4          # DESIGN.md Q25: stop decision fp32 vs fp64
+    cam2 = replace(cam, t_near=2.6)
+    g2, o2, st2 = render_both(sc, cam2, cfg.height, cfg.width, 1)
+    assert 0 < st2.n_intervals < st.n_intervals
+    d2 = np.maximum(np.abs(g2[0] - o2[0]).max(axis=1), np.abs(g2[1] - o2[1]))
+    assert (d2 > TOL_FP32).sum() <= 2 and d2.max() < 1.5e-4
