@@ -25,6 +25,8 @@
 struct mso_scene {
   int32_t n;
   int32_t n_freq, use_viewdir, n_hidden, width, n_feat, mode;
+  int32_t c_f;           /* Eq.7 slot embeddings: width (0 = none) */
+  float *slots;          /* [n][4][c_f] */
   int32_t in_dim, out_dim, n_layers, params;
   float *center;  /* [n][3] */
   float *A;       /* [n][9] world -> unit-sphere frame: diag(1/s) R^T    (Lambda = A^T A) */
@@ -105,9 +107,42 @@ int mso_scene_create(const mso_prims *p, const mso_mlp *m, mso_scene **out) {
   return MSO_OK;
 }
 
+int mso_scene_set_slots(mso_scene *s, int32_t c_f, const float *emb) {
+  if (!s || c_f < 1 || !emb || s->mode != MSO_MODE_CONTACT || s->n_feat != 0) return MSO_ERR_ARG;
+  float *p = (float *)malloc((size_t)s->n * 4 * (size_t)c_f * sizeof(float));
+  if (!p) return MSO_ERR_MEM;
+  memcpy(p, emb, (size_t)s->n * 4 * (size_t)c_f * sizeof(float));
+  free(s->slots);
+  s->slots = p; s->c_f = c_f;
+  return MSO_OK;
+}
+
+/* Eq.7: u = clip(R^T delta / s) = clip(A delta), g = softmax_k(a_k^T u) over the tetrahedral frame */
+static void slot_gates(const mso_scene *s, int i, const float *delta, double *g) {
+  static const double TET[4][3] = {{1, 1, 1}, {1, -1, -1}, {-1, 1, -1}, {-1, -1, 1}};
+  const float *A = s->A + 9 * i;
+  double u[3], z[4], m = -1e300, sum = 0.0;
+  for (int r = 0; r < 3; ++r) {
+    double v = (double)A[3 * r] * delta[0] + (double)A[3 * r + 1] * delta[1] + (double)A[3 * r + 2] * delta[2];
+    u[r] = v < -1.0 ? -1.0 : (v > 1.0 ? 1.0 : v);
+  }
+  for (int k = 0; k < 4; ++k) {
+    z[k] = (TET[k][0] * u[0] + TET[k][1] * u[1] + TET[k][2] * u[2]) / sqrt(3.0);
+    if (z[k] > m) m = z[k];
+  }
+  for (int k = 0; k < 4; ++k) { g[k] = exp(z[k] - m); sum += g[k]; }
+  for (int k = 0; k < 4; ++k) g[k] /= sum;
+}
+
+int mso_slot_gates(const mso_scene *s, int32_t prim, const float *delta, double *g) {
+  if (!s || prim < 0 || prim >= s->n || !delta || !g) return MSO_ERR_ARG;
+  slot_gates(s, prim, delta, g);
+  return MSO_OK;
+}
+
 void mso_scene_destroy(mso_scene *s) {
   if (!s) return;
-  free(s->center); free(s->A); free(s->M); free(s->weights);
+  free(s->center); free(s->A); free(s->M); free(s->weights); free(s->slots);
   free(s);
 }
 
@@ -366,10 +401,12 @@ static void encode(const mso_scene *s, const float *u, const float *d, double *x
  * gamma(z): per scalar z_j, per level l: sin(2^l pi z_j), cos(2^l pi z_j).  Also returns
  * r2 = |p* - mu|^2_Lambda = |A (p* - mu)|^2 for the falloff.  p* and A (p* - mu) in
  * canonical fp32 (the same sample_u as the local mode), the rest fp64. */
-static void encode_contact(const mso_scene *s, int i, const float *o, const float *d, float t, double *x, double *r2) {
+static void encode_contact(const mso_scene *s, int i, const float *o, const float *d, float t, double *x, double *r2,
+                           float *delta_out) {
   const float *mu = s->center + 3 * i;
   float p0 = o[0] + t * d[0], p1 = o[1] + t * d[1], p2 = o[2] + t * d[2];
   float z[6] = {d[0], d[1], d[2], mu[0] - p0, mu[1] - p1, mu[2] - p2};
+  if (delta_out) { delta_out[0] = z[3]; delta_out[1] = z[4]; delta_out[2] = z[5]; }
   int j = 0;
   for (int c = 0; c < 6; ++c)
     for (int l = 0; l < s->n_freq; ++l) {
@@ -512,7 +549,7 @@ int mso_contact_eval(const mso_scene *s, int32_t prim, const float *o, const flo
   if (!s || prim < 0 || prim >= s->n || !o || !d || s->mode != MSO_MODE_CONTACT) return MSO_ERR_ARG;
   if (s->in_dim > MSO_MAXW || s->width > MSO_MAXW || s->out_dim > MSO_MAXW) return MSO_ERR_ARG;
   double x[MSO_MAXW], r[MSO_MAXW], a[MSO_MAXW], r2;
-  encode_contact(s, prim, o, d, t, x, &r2);
+  encode_contact(s, prim, o, d, t, x, &r2, NULL);
   mlp_forward(s, prim, x, r);
   activate(s, r, a);
   if (x_out) memcpy(x_out, x, (size_t)s->in_dim * sizeof(double));
@@ -538,7 +575,7 @@ int mso_render(const mso_scene *s, const mso_camera *cam, int H, int W, const ms
   const tlists_t *tlp = opt->tile > 0 ? &tl : NULL;
   const int K = opt->K;
   const double t_stop = (double)opt->t_stop;
-  const int nf = s->n_feat;
+  const int nf = s->c_f ? s->c_f : s->n_feat;
   int64_t tot_hits = 0, tot_evals = 0, tot_term = 0;
   double min_T = 1.0;
   int failed = 0;
@@ -572,9 +609,10 @@ int mso_render(const mso_scene *s, const mso_camera *cam, int H, int W, const ms
       for (long j = 0; j < ns; ++j) {
         const samp_t *sp = &rb.samps[j];
         double e;                                                     /* 1 - alpha */
+        float dlt[3] = {0.f, 0.f, 0.f};
         if (s->mode == MSO_MODE_CONTACT) {
           double r2;
-          encode_contact(s, sp->prim, o, d, sp->t, x, &r2);
+          encode_contact(s, sp->prim, o, d, sp->t, x, &r2, dlt);
           mlp_forward(s, sp->prim, x, raw);
           activate(s, raw, act);
           /* alpha = (1 - exp(-sigma l)) g,  g = exp(-(9/2) r2)   (readings: mso.h header) */
@@ -590,7 +628,18 @@ int mso_render(const mso_scene *s, const mso_camera *cam, int H, int W, const ms
         ++tot_evals;
         double w = T * (1.0 - e);
         C[0] += w * act[0]; C[1] += w * act[1]; C[2] += w * act[2];
-        if (F) for (int c = 0; c < nf; ++c) F[c] += w * act[4 + c];
+        if (F && s->c_f) {                                            /* Eq.7: f_i = sum_k g_ik e_ik, F += T alpha f_i */
+          double g[4];
+          slot_gates(s, sp->prim, dlt, g);
+          const float *e0 = s->slots + (size_t)sp->prim * 4 * (size_t)nf;
+          for (int c = 0; c < nf; ++c) {
+            double f = 0.0;
+            for (int k = 0; k < 4; ++k) f += g[k] * (double)e0[(size_t)k * nf + c];
+            F[c] += w * f;
+          }
+        } else if (F) {
+          for (int c = 0; c < nf; ++c) F[c] += w * act[4 + c];
+        }
         T = T * e;
         if (T < t_stop) { ++tot_term; break; }                       /* P:437; NS (e) */
       }

@@ -33,6 +33,9 @@
  *   (reading of the "Gaussian falloff" whose formula the paper omits: the support
  *   boundary |.|_Lambda = 1 sits at three standard deviations); samples ordered by (t*, primitive id).
  *   Both readings are listed in DESIGN.md Sec.11.
+ *   Slot features (mso_scene_set_slots; S:Sec.8(f) NEXT-2; Eq.7): u = clip_[-1,1]^3(R^T delta / s),
+ *   g_k = softmax_k(a_k^T u) over the canonical tetrahedral frame a_k = (1,1,1), (1,-1,-1), (-1,1,-1),
+ *   (-1,-1,1), each / sqrt(3); f = sum_k g_k e_k in R^{C_f}; F = sum_i T_i alpha_i f_i (same weights as colour).
  *
  * Precision: every geometric decision (projection, tile range, intersection,
  * sample t, sample order, local coordinate u) is evaluated in IEEE fp32,
@@ -101,6 +104,10 @@ typedef struct {
 enum { MSO_OK = 0, MSO_ERR_ARG = -1, MSO_ERR_MEM = -2, MSO_ERR_CAP = -3 };
 
 int  mso_scene_create(const mso_prims *, const mso_mlp *, mso_scene **out);
+/* contact mode, n_feat == 0: attach slot embeddings emb[n][4][c_f] (copied); mso_render then writes feat[n_pix][c_f] */
+int  mso_scene_set_slots(mso_scene *, int32_t c_f, const float *emb);
+/* gates g[4] of primitive prim for the residual delta = mu - p* (world frame) */
+int  mso_slot_gates(const mso_scene *, int32_t prim, const float *delta, double *g);
 void mso_scene_destroy(mso_scene *);
 
 /* Renders pixels pix[0..n_pix) (linear index y*W+x), or all H*W pixels in raster

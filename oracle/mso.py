@@ -90,6 +90,15 @@ class OracleScene:
         if rc != 0:
             raise ValueError(f"mso_scene_create failed: {rc}")
         self._h = h
+        self.c_f = 0
+        slots = getattr(scene, "slots", None)
+        if slots is not None:
+            emb = np.ascontiguousarray(slots, np.float32)
+            assert emb.shape[:2] == (self.n, 4)
+            rc = lib().mso_scene_set_slots(self._h, C.c_int32(emb.shape[2]), _ptr(emb))
+            if rc != 0:
+                raise ValueError(f"mso_scene_set_slots failed: {rc}")
+            self.c_f = int(emb.shape[2])
 
     def __del__(self):
         h = getattr(self, "_h", None)
@@ -108,7 +117,7 @@ class OracleScene:
             n = H * W
         rgb = np.zeros((n, 3), np.float64)
         alpha = np.zeros((n,), np.float64)
-        nf = self.mlp.n_feat
+        nf = self.c_f or self.mlp.n_feat
         feat = np.zeros((n, nf), np.float64) if (nf and want_feat) else None
         st = _Stats()
         o = _Opts(K, t_stop, tile, n_threads)
@@ -224,6 +233,14 @@ class OracleScene:
         if rc != 0:
             raise RuntimeError(f"mso_mlp_eval failed: {rc}")
         return raw, act
+
+    def slot_gates(self, prim, delta):
+        g = np.zeros(4, np.float64)
+        dl = np.ascontiguousarray(delta, np.float32)
+        rc = lib().mso_slot_gates(self._h, C.c_int32(prim), _ptr(dl), _ptr(g))
+        if rc != 0:
+            raise RuntimeError(f"mso_slot_gates failed: {rc}")
+        return g
 
     def contact_eval(self, prim, o, d, t):
         """contact mode: (x, raw, act, r2) of primitive prim at o + t d."""

@@ -89,6 +89,7 @@ class SceneConfig:
     sigma_bias: float = 0.5
     t_stop: float = 1e-4
     tile: int = 16
+    c_f: int = 0         # C_f of Eq.7: four slot embeddings of this width per primitive (0 = none)
 
 
 CONFIGS: dict[str, SceneConfig] = {
@@ -108,6 +109,10 @@ CONFIGS: dict[str, SceneConfig] = {
     # the contact point, 72-32-32-4 fp32 MLPs on gamma([d; delta]); N in the paper's range (Table 6).
     "next1": SceneConfig("next1", 6, 2048, 2.0, 0.05, 0.5,
                          MLPSpec(6, 0, 2, 32, 0, False, MODE_CONTACT), 1280, 720, 60.0, 5.0, 1),
+    # S:§8(f) NEXT-2: the same scene with the paper's feature model (Eq.7): 4 slot embeddings of
+    # C_f = 512 per primitive, gated by a tetrahedral frame, composited with the colour weights.
+    "next2": SceneConfig("next2", 6, 2048, 2.0, 0.05, 0.5,
+                         MLPSpec(6, 0, 2, 32, 0, False, MODE_CONTACT), 1280, 720, 60.0, 5.0, 1, c_f=512),
 }
 
 
@@ -140,6 +145,7 @@ class Scene:
     scale: np.ndarray    # [N,3] f32 semi-axes
     weights: np.ndarray  # [N, params_per_prim] f32 values
     mlp: MLPSpec
+    slots: np.ndarray | None = None   # [N, 4, C_f] f32 slot embeddings e_ik of Eq.7, contact mode only
 
     @property
     def n(self) -> int:
@@ -185,10 +191,11 @@ def make_scene(cfg: SceneConfig) -> Scene:
     log_s = rng.uniform(math.log(cfg.s_min), math.log(cfg.s_max), size=(n, 3))
     scale = np.exp(log_s)
     weights = draw_weights(rng, n, cfg.mlp, cfg.sigma_bias)
+    slots = rng.normal(size=(n, 4, cfg.c_f)).astype(np.float32) if cfg.c_f else None   # drawn last: earlier draws unchanged
     return Scene(np.ascontiguousarray(center, dtype=np.float32),
                  np.ascontiguousarray(q, dtype=np.float32),
                  np.ascontiguousarray(scale, dtype=np.float32),
-                 weights, cfg.mlp)
+                 weights, cfg.mlp, slots)
 
 
 def look_at(eye, target=(0.0, 0.0, 0.0), up=(0.0, 1.0, 0.0)) -> np.ndarray:
@@ -252,12 +259,13 @@ def constant_mlp_weights(mlp: MLPSpec, raw_out: np.ndarray) -> np.ndarray:
     return np.concatenate(blob).astype(np.float32)
 
 
-def custom_scene(center, quat, scale, weights, mlp: MLPSpec) -> Scene:
+def custom_scene(center, quat, scale, weights, mlp: MLPSpec, slots=None) -> Scene:
     return Scene(np.ascontiguousarray(center, dtype=np.float32).reshape(-1, 3),
                  np.ascontiguousarray(quat, dtype=np.float32).reshape(-1, 4),
                  np.ascontiguousarray(scale, dtype=np.float32).reshape(-1, 3),
                  np.ascontiguousarray(weights, dtype=np.float32).reshape(
-                     -1, mlp.params_per_prim), mlp)
+                     -1, mlp.params_per_prim), mlp,
+                 None if slots is None else np.ascontiguousarray(slots, dtype=np.float32))
 
 
 def dense_scene(seed: int = 7, n: int = 48, sigma_bias: float = 8.0) -> tuple[Scene, SceneConfig]:
