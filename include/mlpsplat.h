@@ -126,6 +126,14 @@ enum { MS_STAGE_BIN = 0, MS_STAGE_SORT, MS_STAGE_ISECT, MS_STAGE_MLP, MS_STAGE_C
  * fp32) A = diag(1/s) R^T and M = R diag(s), and packs the weights for the
  * MLP kernels.  Synchronises the device. */
 int ms_scene_create(const ms_prims *prims, const ms_mlp *mlp, ms_scene **out);
+/* Eq.7 slot features (S:Sec.8(f) NEXT-2), MS_MODE_CONTACT scenes with n_feat == 0 only:
+ * attaches four slot embeddings per primitive, emb = host float32 [n][4][c_f] (copied), c_f a multiple
+ * of 128, <= 512 (the paper: 512).  Renders then write out_feat[H][W][c_f]:
+ *   u = clip_[-1,1]^3(R^T delta / s), g_k = softmax_k(a_k^T u) over the canonical tetrahedral frame
+ *   a_k = (1,1,1), (1,-1,-1), (-1,1,-1), (-1,-1,1), each / sqrt(3); f = sum_k g_k e_k;
+ *   F = sum_i T_i alpha_i f_i (the colour weights).  Synchronises the device. */
+int ms_scene_set_slots(ms_scene *scene, int32_t c_f, const float *emb);
+
 int ms_scene_destroy(ms_scene *scene);
 
 /* Renders one view into DEVICE buffers out_rgb [H][W][3], out_alpha [H][W] and, if the MLP has

@@ -20,7 +20,7 @@ PATH_AUTO, PATH_FP32, PATH_BF16_TC = 0, 1, 2
 FLAG_KEEP_DEBUG, FLAG_STAGE_TIMES = 1, 2
 STAGES = ("bin", "sort", "isect", "mlp", "composite")
 
-EXPORTS = ["ms_scene_create", "ms_scene_destroy", "ms_render", "ms_render_batch", "ms_render_host",
+EXPORTS = ["ms_scene_create", "ms_scene_set_slots", "ms_scene_destroy", "ms_render", "ms_render_batch", "ms_render_host",
            "ms_last_stats", "ms_last_stage_ms", "ms_stage_accum", "ms_debug_tile_lists", "ms_debug_intervals",
            "ms_debug_sample_order", "ms_debug_prim_frames", "ms_error_string", "ms_last_cuda_error"]
 
@@ -61,6 +61,7 @@ def _load() -> C.CDLL:
         getattr(lib, name)  # fail loudly on a stale library
     lib.ms_error_string.restype = C.c_char_p
     lib.ms_scene_destroy.argtypes = [C.c_void_p]
+    lib.ms_scene_set_slots.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
     return lib
 
 
@@ -124,6 +125,16 @@ class Scene:
         if rc != 0:
             raise MsError(rc, "ms_scene_create")
         self._h = h
+        self.c_f = 0                                   # Eq.7 slot features (ms_scene_set_slots)
+        slots = getattr(scene, "slots", None)
+        if slots is not None:
+            emb = np.ascontiguousarray(slots, np.float32)
+            if emb.ndim != 3 or emb.shape[:2] != (self.n, 4):
+                raise ValueError("slots must be [n][4][c_f]")
+            rc = _lib.ms_scene_set_slots(self._h, int(emb.shape[2]), _ptr(emb))
+            if rc != 0:
+                raise MsError(rc, "ms_scene_set_slots")
+            self.c_f = int(emb.shape[2])
 
     def close(self):
         h = getattr(self, "_h", None)
@@ -150,7 +161,7 @@ class Scene:
     def render(self, cam, H, W, K, *, t_stop=1e-4, tile=16, path=PATH_AUTO, flags=0, out=None,
                want_feat=True, stream=None):
         """One view -> (rgb [H,W,3], alpha [H,W], feat [H,W,F] | None) float32 CUDA tensors."""
-        nf = self.mlp.n_feat if want_feat else 0
+        nf = (self.c_f or self.mlp.n_feat) if want_feat else 0
         if out is None:
             rgb = torch.empty((H, W, 3), dtype=torch.float32, device="cuda")
             alpha = torch.empty((H, W), dtype=torch.float32, device="cuda")
@@ -166,7 +177,7 @@ class Scene:
     def render_batch(self, cams, H, W, K, *, t_stop=1e-4, tile=16, path=PATH_AUTO, flags=0, out=None,
                      want_feat=True, stream=None):
         V = len(cams)
-        nf = self.mlp.n_feat if want_feat else 0
+        nf = (self.c_f or self.mlp.n_feat) if want_feat else 0
         if out is None:
             rgb = torch.empty((V, H, W, 3), dtype=torch.float32, device="cuda")
             alpha = torch.empty((V, H, W), dtype=torch.float32, device="cuda")
@@ -184,7 +195,7 @@ class Scene:
                     want_feat=True, stream=None):
         """End-to-end entry: HOST (pinned) output buffers, device->host copies inside the call."""
         V = len(cams)
-        nf = self.mlp.n_feat if want_feat else 0
+        nf = (self.c_f or self.mlp.n_feat) if want_feat else 0
         if out is None:
             rgb = torch.empty((V, H, W, 3), dtype=torch.float32).pin_memory()
             alpha = torch.empty((V, H, W), dtype=torch.float32).pin_memory()

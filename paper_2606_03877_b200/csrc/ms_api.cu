@@ -32,9 +32,11 @@ struct ms_scene {
   float *center = nullptr, *quat = nullptr, *scale = nullptr, *A = nullptr, *M = nullptr;
   float *weights_f32 = nullptr;
   MsTcWeights tc{};  // packed bf16 image for the tensor path (may be empty)
+  int slot_cf = 0;           // Eq.7 slot embeddings: width C_f (0 = none)
+  float *slots = nullptr;    // device [N][4][slot_cf]
   // per-view scratch
   Buf tile_count, emit_off, rect, z_entry, oprime, keys_a, keys_b, sort_scratch, tile_start, pair_hits, pair_off,
-      ray_hits, ray_off, scan_scratch, prim_start, prim_blocks, blk_off, intervals, hits, staging, staging_feat,
+      ray_hits, ray_off, scan_scratch, prim_start, prim_blocks, blk_off, intervals, hits, staging, staging_feat, staging_gate,
       host_rgb, host_alpha, host_feat, dbg;
   uint32_t *pinned = nullptr;  // [4] host-pinned readback
   cudaEvent_t ev[MS_N_STAGES + 1] = {};
@@ -95,7 +97,7 @@ size_t scratch_total(const ms_scene *sc) {
   const Buf *all[] = {&sc->tile_count, &sc->emit_off, &sc->rect, &sc->z_entry, &sc->oprime, &sc->keys_a, &sc->keys_b,
                       &sc->sort_scratch, &sc->tile_start, &sc->pair_hits, &sc->pair_off, &sc->ray_hits, &sc->ray_off,
                       &sc->scan_scratch, &sc->prim_start, &sc->prim_blocks, &sc->blk_off, &sc->intervals, &sc->hits,
-                      &sc->staging, &sc->staging_feat};
+                      &sc->staging, &sc->staging_feat, &sc->staging_gate};
   size_t t = 0;
   for (const Buf *b : all) t += b->cap;
   return t;
@@ -247,6 +249,8 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   ENS(sc->hits, (n_hits + 1) * sizeof(MsHit));
   ENS(sc->staging, (n_samples + 1) * sizeof(float4));
   if (want_feat) ENS(sc->staging_feat, (n_samples + 1) * (size_t)sc->shape.n_feat * 4);
+  const bool want_slots = sc->slot_cf > 0 && out_feat != nullptr;   // Eq.7 features (contact mode, K = 1)
+  if (want_slots) ENS(sc->staging_gate, (n_samples + 1) * sizeof(float4));
   ia.intervals = (MsInterval *)sc->intervals.p;
   ia.hits = (MsHit *)sc->hits.p;
   CK(ms_isect_fill(ia, st));
@@ -260,6 +264,7 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   ma.intervals = (MsInterval *)sc->intervals.p;
   ma.staging = (float4 *)sc->staging.p;
   ma.staging_feat = want_feat ? (float *)sc->staging_feat.p : nullptr;
+  ma.staging_gate = want_slots ? (float4 *)sc->staging_gate.p : nullptr;
   if (path == MS_PATH_BF16_TC) CK(ms_mlp_tc(sc->tc, ma, st));
   else CK(ms_mlp_f32(ma, st));
 
@@ -270,7 +275,9 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   ca.contact = sc->shape.mode == MS_MODE_CONTACT;
   ca.ray_off = (uint32_t *)sc->ray_off.p; ca.hits = (MsHit *)sc->hits.p; ca.staging = (float4 *)sc->staging.p;
   ca.staging_feat = want_feat ? (float *)sc->staging_feat.p : nullptr;
-  ca.out_rgb = out_rgb; ca.out_alpha = out_alpha; ca.out_feat = want_feat ? out_feat : nullptr;
+  ca.gates = want_slots ? (const float4 *)sc->staging_gate.p : nullptr;
+  ca.slots = sc->slots; ca.c_f = sc->slot_cf;
+  ca.out_rgb = out_rgb; ca.out_alpha = out_alpha; ca.out_feat = (want_feat || want_slots) ? out_feat : nullptr;
   CK(ms_composite(ca, st));
   if (timing) {
     CK(cudaEventRecord(sc->ev[5], st));
@@ -412,15 +419,32 @@ int ms_scene_create(const ms_prims *prims, const ms_mlp *mlp, ms_scene **out) {
 #undef CKC
 }
 
+int ms_scene_set_slots(ms_scene *sc, int32_t c_f, const float *emb) {
+  if (!sc || !emb || c_f < 1) return MS_ERR_INVALID_ARG;
+  if (sc->shape.mode != MS_MODE_CONTACT || sc->shape.n_feat != 0) return MS_ERR_INVALID_ARG;
+  if (c_f % 128 != 0 || c_f > 512) return MS_ERR_UNSUPPORTED_SHAPE;   // one float4 per lane per 128 channels
+  const size_t bytes = (size_t)sc->n * 4 * (size_t)c_f * sizeof(float);
+  float *d = nullptr;
+  cudaError_t e = cudaMalloc(&d, bytes);
+  if (e != cudaSuccess) { (void)cudaGetLastError(); sc->last_cuda = (int)e; return MS_ERR_OUT_OF_MEMORY; }
+  e = cudaMemcpy(d, emb, bytes, cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) { cudaFree(d); sc->last_cuda = (int)e; return MS_ERR_CUDA; }
+  cudaFree(sc->slots);
+  sc->slots = d;
+  sc->slot_cf = c_f;
+  return MS_OK;
+}
+
 int ms_scene_destroy(ms_scene *sc) {
   if (!sc) return MS_OK;
   cudaFree(sc->center); cudaFree(sc->quat); cudaFree(sc->scale); cudaFree(sc->A); cudaFree(sc->M);
   cudaFree(sc->weights_f32);
+  cudaFree(sc->slots);
   ms_tc_free(&sc->tc);
   Buf *all[] = {&sc->tile_count, &sc->emit_off, &sc->rect, &sc->z_entry, &sc->oprime, &sc->keys_a, &sc->keys_b,
                 &sc->sort_scratch, &sc->tile_start, &sc->pair_hits, &sc->pair_off, &sc->ray_hits, &sc->ray_off,
                 &sc->scan_scratch, &sc->prim_start, &sc->prim_blocks, &sc->blk_off, &sc->intervals, &sc->hits,
-                &sc->staging, &sc->staging_feat, &sc->host_rgb, &sc->host_alpha, &sc->host_feat, &sc->dbg};
+                &sc->staging, &sc->staging_feat, &sc->staging_gate, &sc->host_rgb, &sc->host_alpha, &sc->host_feat, &sc->dbg};
   for (Buf *b : all) free_buf(*b);
   if (sc->pinned) cudaFreeHost(sc->pinned);
   for (int i = 0; i <= MS_N_STAGES; ++i)
@@ -444,7 +468,7 @@ int ms_render_batch(ms_scene *sc, const ms_camera *cams, int32_t n_views, int32_
   const size_t px = (size_t)H * W;
   for (int v = 0; v < n_views; ++v) {
     rc = render_view(sc, cams + v, H, W, opts, out_rgb + v * px * 3, out_alpha + v * px,
-                     out_feat ? out_feat + v * px * sc->shape.n_feat : nullptr);
+                     out_feat ? out_feat + v * px * (size_t)(sc->slot_cf ? sc->slot_cf : sc->shape.n_feat) : nullptr);
     if (rc != MS_OK) return rc;
   }
   return MS_OK;
@@ -456,7 +480,7 @@ int ms_render_host(ms_scene *sc, const ms_camera *cams, int32_t n_views, int32_t
   if (rc != MS_OK) return rc;
   cudaStream_t st = (cudaStream_t)opts->stream;
   const size_t px = (size_t)H * W;
-  const int nf = sc->shape.n_feat;
+  const int nf = sc->slot_cf ? sc->slot_cf : sc->shape.n_feat;
   const bool feat = nf > 0 && host_feat;
   ENS(sc->host_rgb, px * 12);
   ENS(sc->host_alpha, px * 4);

@@ -105,7 +105,7 @@ __device__ __forceinline__ void load_hits(WarpSmem &sm, const MsHit *__restrict_
   }
 }
 
-template <int FEAT>  // 0: rgb/alpha only; 1: + features
+template <int FEAT>  // 0: rgb/alpha only; 1: + linear head features; 2: + Eq.7 slot features (contact mode, K = 1)
 __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
   __shared__ WarpSmem s_all[CW];
   __shared__ float s_w[FEAT ? CW : 1][FEAT ? CAP : 1];   // weight of the window's r-th merged sample (features only)
@@ -119,6 +119,9 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
   float T = 1.0f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
   float F[MS_MAX_OUT / 32] = {0.f, 0.f};
   float4 F4 = make_float4(0.f, 0.f, 0.f, 0.f);   // n_feat == 32: channels 4*(lane%8)..+3 of the samples of lane group lane/8
+  float4 Fs[4];                                  // slot features: channels 4*(lane + 32 q)..+3, q < c_f/128
+#pragma unroll
+  for (int q = 0; q < 4; ++q) Fs[q] = make_float4(0.f, 0.f, 0.f, 0.f);
   if (n > 0) {
     const MsHit *hits = a.hits + off;
     const float4 *stg = a.staging + (size_t)off * (size_t)K;
@@ -177,7 +180,31 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
         T = __shfl_sync(FULL, Tl, 31);             // lane 31 leaves with T times the product of the whole window
       }
       C0 += c0; C1 += c1; C2 += c2;
-      if (FEAT) {
+      if (FEAT == 2) {
+        // Eq.7: f_i = sum_k g_ik e_ik, F += (T_i alpha_i) f_i.  One hit per merged sample (K = 1):
+        // every lane takes 4 channels per 128 of the primitive's four embedding rows (coalesced 512 B loads).
+        __syncwarp();
+        const float4 *gates = a.gates + off;
+        const int cf4 = a.c_f >> 2, nq = a.c_f >> 7;
+        for (uint32_t r = 0; r < done; ++r) {
+          const uint32_t s = sm.ord[r];
+          const float w = s_w[FEAT ? warp : 0][FEAT ? r : 0];
+          const float4 g = __ldg(gates + s);
+          const float4 *e = reinterpret_cast<const float4 *>(a.slots + (size_t)__ldg(&hits[s].prim) * 4 * (size_t)a.c_f) + lane;
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            if (q < nq) {
+              const float4 e0 = __ldg(e + 32 * q), e1 = __ldg(e + cf4 + 32 * q), e2 = __ldg(e + 2 * cf4 + 32 * q),
+                           e3 = __ldg(e + 3 * cf4 + 32 * q);
+              Fs[q].x = fmaf(w, fmaf(g.w, e3.x, fmaf(g.z, e2.x, fmaf(g.y, e1.x, g.x * e0.x))), Fs[q].x);
+              Fs[q].y = fmaf(w, fmaf(g.w, e3.y, fmaf(g.z, e2.y, fmaf(g.y, e1.y, g.x * e0.y))), Fs[q].y);
+              Fs[q].z = fmaf(w, fmaf(g.w, e3.z, fmaf(g.z, e2.z, fmaf(g.y, e1.z, g.x * e0.z))), Fs[q].z);
+              Fs[q].w = fmaf(w, fmaf(g.w, e3.w, fmaf(g.z, e2.w, fmaf(g.y, e1.w, g.x * e0.w))), Fs[q].w);
+            }
+          }
+        }
+      }
+      if (FEAT == 1) {
         __syncwarp();
         const float *fbase = a.staging_feat + (size_t)off * (size_t)K * (size_t)nf;
         if (nf == 32) {
@@ -227,7 +254,13 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
   }
   if (lane < 3) a.out_rgb[3 * (size_t)ray + lane] = lane == 0 ? C0 : (lane == 1 ? C1 : C2);
   if (lane == 3) a.out_alpha[ray] = 1.0f - T;
-  if (FEAT) {
+  if (FEAT == 2) {
+    const int nq = a.c_f >> 7;
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+      if (q < nq) reinterpret_cast<float4 *>(a.out_feat + (size_t)ray * a.c_f)[lane + 32 * q] = Fs[q];
+  }
+  if (FEAT == 1) {
     if (nf == 32) {
 #pragma unroll
       for (int o = 8; o < 32; o <<= 1) {
@@ -270,7 +303,9 @@ cudaError_t ms_composite(const MsCompositeArgs &a, cudaStream_t s) {
   if (a.n_rays == 0) return cudaSuccess;
   const unsigned grid = (unsigned)((a.n_rays + CW - 1) / CW);
   const bool feat = a.n_feat > 0 && a.out_feat && a.staging_feat;
-  if (!feat) composite_kernel<0><<<grid, CW * 32, 0, s>>>(a);
+  const bool slots = a.c_f > 0 && a.out_feat && a.gates && a.slots && a.K == 1;
+  if (slots) composite_kernel<2><<<grid, CW * 32, 0, s>>>(a);
+  else if (!feat) composite_kernel<0><<<grid, CW * 32, 0, s>>>(a);
   else composite_kernel<1><<<grid, CW * 32, 0, s>>>(a);
   MS_LAUNCHED();
   return cudaGetLastError();

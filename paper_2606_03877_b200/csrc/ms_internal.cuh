@@ -116,6 +116,18 @@ __device__ __forceinline__ void ms_sample_u(const float *A, const float *mu, con
   u[2] = ms_dot3(A[6], A[7], A[8], w0, w1, w2);
 }
 
+// Eq.7: slot gates g = softmax_k(a_k^T u_s), u_s = clip(R^T delta / s) = clip(-u) with
+// u = A (p* - mu) the local coordinate of the contact point; a_k the canonical tetrahedral frame.
+__device__ __forceinline__ float4 ms_slot_gates(const float *u) {
+  const float c = 0.57735026918962576f;  // 1/sqrt(3)
+  const float x = fminf(fmaxf(-u[0], -1.0f), 1.0f), y = fminf(fmaxf(-u[1], -1.0f), 1.0f), z = fminf(fmaxf(-u[2], -1.0f), 1.0f);
+  const float z0 = (x + y + z) * c, z1 = (x - y - z) * c, z2 = (-x + y - z) * c, z3 = (-x - y + z) * c;
+  const float m = fmaxf(fmaxf(z0, z1), fmaxf(z2, z3));
+  const float e0 = expf(z0 - m), e1 = expf(z1 - m), e2 = expf(z2 - m), e3 = expf(z3 - m);
+  const float inv = 1.0f / (e0 + e1 + e2 + e3);
+  return make_float4(e0 * inv, e1 * inv, e2 * inv, e3 * inv);
+}
+
 // kernels launched so far by this host thread (bench.py reports the per-step count)
 extern thread_local long long ms_launch_count;
 #define MS_LAUNCHED() (++ms_launch_count)
@@ -179,6 +191,7 @@ struct MsMlpArgs {
   const MsInterval *intervals;
   float4 *staging;                // [n_hits*K] (r,g,b,e)
   float *staging_feat;            // [n_hits*K][n_feat] or NULL
+  float4 *staging_gate;           // [n_hits] slot gates g_k of Eq.7 (contact mode) or NULL
 };
 cudaError_t ms_mlp_f32(const MsMlpArgs &a, cudaStream_t s);
 
@@ -190,6 +203,9 @@ struct MsCompositeArgs {
   const MsHit *hits;
   const float4 *staging;
   const float *staging_feat;
+  const float4 *gates;   // [n_hits] slot gates (Eq.7) or NULL
+  const float *slots;    // [N][4][c_f] slot embeddings
+  int c_f;
   float *out_rgb, *out_alpha, *out_feat;
 };
 cudaError_t ms_composite(const MsCompositeArgs &a, cudaStream_t s);

@@ -98,6 +98,7 @@ __global__ void __launch_bounds__(MS_ROWS) mlp_f32_kernel(MsMlpArgs a) {
   }
   const size_t out = (size_t)(uint32_t)iv.slot * (size_t)a.K + (size_t)k;
   a.staging[out] = r;
+  if (a.staging_gate) a.staging_gate[out] = ms_slot_gates(u);
   if (a.staging_feat)
     for (int c = 0; c < sh.n_feat; ++c) a.staging_feat[out * sh.n_feat + c] = raw[4 + c];
 }
@@ -276,6 +277,7 @@ __global__ void __launch_bounds__(MS_ROWS / SPT) mlp_f32_w32_kernel(MsMlpArgs a)
     }
     const size_t out = (size_t)(uint32_t)iv[p].slot * (size_t)a.K + (size_t)kk[p];
     a.staging[out] = r;
+    if (a.staging_gate) a.staging_gate[out] = ms_slot_gates(u[p]);
     if (a.staging_feat)
       for (int c = 0; c < sh.n_feat; ++c) {
         float f = bh[4 + c];

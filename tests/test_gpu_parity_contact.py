@@ -81,3 +81,36 @@ def test_contact_dense_scene_early_termination_and_t_near():
     assert 0 < st2.n_intervals < st.n_intervals
     d2 = np.maximum(np.abs(g2[0] - o2[0]).max(axis=1), np.abs(g2[1] - o2[1]))
     assert (d2 > TOL_FP32).sum() <= 2 and d2.max() < 1.5e-4
+
+
+@pytest.mark.parametrize("c_f,W,H", [(128, 96, 54), (512, 64, 36)])
+def test_next2_slot_features(c_f, W, H):
+    """Eq.7 slot features (S:Sec.8(f) NEXT-2): gates, embeddings and the colour weights; C_f = 512 is the
+    paper's width.  Features are linear in O(1) embeddings: 1e-5 relative to their range."""
+    from dataclasses import replace
+    api = _api()
+    cfg = synth.shrink(replace(synth.CONFIGS["next2"], c_f=c_f), W, H)
+    sc, cam = synth.make_scene(cfg), synth.make_cameras(cfg)[0]
+    gs = api.Scene(sc)
+    rgb, alpha, feat = gs.render(cam, H, W, 1)
+    torch.cuda.synchronize()
+    o_rgb, o_alpha, o_feat, st = mso.OracleScene(sc).render(cam, H, W, 1)
+    assert feat.shape == (H, W, c_f) and gs.stats().n_intervals == st.n_intervals
+    assert np.abs(rgb.cpu().numpy().reshape(-1, 3) - o_rgb).max() <= TOL_FP32
+    assert np.abs(alpha.cpu().numpy().reshape(-1) - o_alpha).max() <= TOL_FP32
+    scale = max(1.0, np.abs(o_feat).max())
+    assert np.abs(feat.cpu().numpy().reshape(-1, c_f) - o_feat).max() <= TOL_FP32 * scale
+
+
+def test_slot_argument_checks():
+    api = _api()
+    from dataclasses import replace
+    cfg = synth.shrink(replace(synth.CONFIGS["next2"], c_f=96), 32, 18)        # not a multiple of 128
+    with pytest.raises(api.MsError) as e:
+        api.Scene(synth.make_scene(cfg))
+    assert e.value.code == -4
+    cfg2 = synth.shrink(synth.CONFIGS["cfg1"], 32, 18)                          # not a contact-mode scene
+    sc2 = synth.make_scene(cfg2)
+    sc2.slots = np.zeros((sc2.n, 4, 128), np.float32)
+    with pytest.raises(api.MsError):
+        api.Scene(sc2)
