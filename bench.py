@@ -242,7 +242,8 @@ def run_ours(args, cfg):
     if not cfg.mlp.bf16:
         # fp32 SIMT path: 148 SMs x 128 FMA lanes x 2 FLOP at the top SM clock (guide's unit counts)
         peak = 148 * 128 * 2 * 1.965e9 / 1e12
-    out_bytes = H * W * (16 + 4 * cfg.mlp.n_feat)
+    feat_w = cfg.c_f or cfg.mlp.n_feat                  # Eq.7 slot features or the widened head
+    out_bytes = H * W * (16 + 4 * feat_w)
     frame_floor_ms = max(flops_view / (peak * 1e12), out_bytes / (peaks["hbm_gbs"] * 1e9)) * 1e3
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -276,6 +277,18 @@ def run_ours(args, cfg):
         "frame_roofline": {"floor_ms_per_view": frame_floor_ms, "frac": frame_floor_ms * V / ms_step,
                            "note": "slower of MLP FLOPs at the bf16 peak and output bytes at the HBM peak, over the whole step"},
     }
+    comp_ms = stage_sum["composite"] / max(1, n_views_timed)
+    if cfg.c_f and comp_ms > mlp_ms:
+        # Eq.7 slot features: stage (e) dominates and is memory-bound.  Algorithmic bytes per view: staging,
+        # gates and hit records once per hit (16 B each), the embeddings once, the outputs once.
+        alg = st.n_intervals * 48 + sc.slots.nbytes + out_bytes
+        ach = alg / (comp_ms * 1e-3) / 1e9
+        line["roofline"] = {"bound": "hbm", "kernel": "composite_kernel<2> (stage e, slot features)", "achieved": ach,
+                            "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"], "traffic": None,
+                            "peak_kind": f"HBM copy bandwidth, of {peaks['source']}", "algorithmic_bytes": alg,
+                            "kernel_ms": comp_ms, "kernel_share_of_step": comp_ms * V / ms_step,
+                            "note": "the kernel re-reads each hit's four embedding rows (16 * c_f B per hit) through L1/L2; "
+                                    "that traffic is not algorithmic"}
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = {k: v for k, v in time_oracle(cfg, sc, cams, args.cpu_seconds).items()
                                 if k in ("value", "unit", "cores", "kind", "sample", "samples_per_s")}
