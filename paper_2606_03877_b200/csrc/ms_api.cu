@@ -408,7 +408,7 @@ int ms_scene_create(const ms_prims *prims, const ms_mlp *mlp, ms_scene **out) {
     if (!isfinite(prims->center[i])) return fail(MS_ERR_INVALID_ARG);
   CKC(cudaMallocHost(&sc->pinned, 16));
   for (int i = 0; i <= MS_N_STAGES; ++i) CKC(cudaEventCreate(&sc->ev[i]));
-  if (mlp->dtype == MS_BF16 && sh.mode == MS_MODE_LOCAL) {   // the contact-point mode runs on the fp32 path only
+  if (mlp->dtype == MS_BF16) {
     rc = ms_tc_pack(sh, sc->n, w.data(), &sc->tc);  // leaves tc.valid = false if the shape is not covered
     if (rc != MS_OK) return fail(rc);
   }

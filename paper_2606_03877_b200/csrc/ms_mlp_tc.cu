@@ -264,6 +264,41 @@ __device__ __forceinline__ void encode_row(const float *u, const float *d, uint8
   }
 }
 
+// Contact-point input (MS_MODE_CONTACT; Eq.3-5): z = [d; mu - p*], x[2L j + 2l] = sin(2^l pi z_j),
+// x[2L j + 2l + 1] = cos(2^l pi z_j), then the two bias columns.  Two scalars fill 4L values = whole
+// 16-byte chunks (L even), so the row is produced and stored pair by pair (24 live values, not 80).
+template <int NFREQ, int K1>
+__device__ __forceinline__ void encode_contact_row(const float *z, uint8_t *dst_row /* + chunk*2048 */) {
+  constexpr int IN = 12 * NFREQ, PER = 4 * NFREQ;
+  static_assert(PER % 8 == 0 && IN + 2 <= K1 && K1 == IN + 8, "contact layout");
+#pragma unroll
+  for (int jp = 0; jp < 3; ++jp) {
+    float x[PER];
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const float arg = 3.14159265358979323846f * z[2 * jp + h];
+      float sv = __sinf(arg), cv = __cosf(arg);
+#pragma unroll
+      for (int l = 0; l < NFREQ; ++l) {
+        x[2 * NFREQ * h + 2 * l] = sv;
+        x[2 * NFREQ * h + 2 * l + 1] = cv;
+        const float s2 = 2.0f * sv * cv, c2 = fmaf(-2.0f * sv, sv, 1.0f);
+        sv = s2; cv = c2;
+      }
+    }
+#pragma unroll
+    for (int c = 0; c < PER / 8; ++c) {
+      uint4 v;
+      v.x = pack_bf16(x[8 * c + 0], x[8 * c + 1]);
+      v.y = pack_bf16(x[8 * c + 2], x[8 * c + 3]);
+      v.z = pack_bf16(x[8 * c + 4], x[8 * c + 5]);
+      v.w = pack_bf16(x[8 * c + 6], x[8 * c + 7]);
+      *reinterpret_cast<uint4 *>(dst_row + (jp * (PER / 8) + c) * (MS_ROWS * 16)) = v;
+    }
+  }
+  *reinterpret_cast<uint4 *>(dst_row + (IN / 8) * (MS_ROWS * 16)) = make_uint4(0x3f803f80u, 0u, 0u, 0u);   // bias columns (1, 1)
+}
+
 // ---------------------------------------------------------------------------------------------
 // kernel
 // ---------------------------------------------------------------------------------------------
@@ -305,9 +340,9 @@ __host__ __device__ constexpr int tc_warps(int width, int nout) {
 }
 // warps: one MMA warp per slot, head MMA warp (also weight loader and TMEM owner), EN groups, 4 HD, HE groups
 
-template <int NFREQ, int VIEWDIR, int WIDTH, int NOUT, int NH>
+template <int NFREQ, int VIEWDIR, int WIDTH, int NOUT, int NH, int CONTACT = 0>
 __global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(const TcParams p) {
-  constexpr int IN = 3 + 6 * NFREQ + 3 * VIEWDIR;
+  constexpr int IN = CONTACT ? 12 * NFREQ : 3 + 6 * NFREQ + 3 * VIEWDIR;   // CONTACT: gamma([d; delta]) of the paper's own mode
   constexpr int K1 = (IN + 2 + 15) / 16 * 16;
   constexpr int NSLOT = tc_slots(WIDTH, NOUT);
   constexpr int HPS = tc_heads_per_slot(WIDTH);   // head regions per slot (private to the slot's MMA warp)
@@ -562,7 +597,18 @@ __global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(c
       const uint64_t s0 = (uint64_t)first * MS_ROWS + (uint32_t)row;
       uint32_t j = (uint32_t)(s0 / K), k = (uint32_t)(s0 - (uint64_t)j * K);
       float4 q0 = make_float4(0.f, 0.f, 0.f, 0.f);   // (ray, t_in, delta, slot) of the row's interval
-      if (j < iv_count) q0 = __ldg(reinterpret_cast<const float4 *>(p.intervals + iv_first + j));
+      float4 q1 = q0;                                // CONTACT: (d, -) of the row's interval, for the falloff
+      if (j < iv_count) {
+        q0 = __ldg(reinterpret_cast<const float4 *>(p.intervals + iv_first + j));
+        if (CONTACT) q1 = __ldg(reinterpret_cast<const float4 *>(p.intervals + iv_first + j) + 1);
+      }
+      float Al[9], mu[3];
+      if (CONTACT) {
+#pragma unroll
+        for (int q = 0; q < 9; ++q) Al[q] = __ldg(p.A + 9 * (size_t)prim + q);
+#pragma unroll
+        for (int q = 0; q < 3; ++q) mu[q] = __ldg(p.center + 3 * (size_t)prim + q);
+      }
       for (uint32_t i = 0; i < count; ++i) {
         const uint32_t slot = i % NSLOT;
         uint32_t cnt = i / NSLOT;                   // the slot's head counter for this block (see the MMA warp)
@@ -572,9 +618,19 @@ __global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(c
         const bool valid = j < iv_count;
         const float delta = q0.z;
         const size_t out_idx = (size_t)(uint32_t)__float_as_int(q0.w) * K + k;
+        float fall = 1.0f;                           // CONTACT: g = exp(-(9/2) |p* - mu|^2_Lambda)
+        if (CONTACT && valid) {
+          const float dd[3] = {q1.x, q1.y, q1.z};
+          float uu[3];
+          ms_sample_u(Al, mu, p.cam.o, dd, q0.y, uu);
+          fall = __expf(-4.5f * (uu[0] * uu[0] + uu[1] * uu[1] + uu[2] * uu[2]));
+        }
         k += dk; j += dj;
         if (k >= K) { k -= K; ++j; }
-        if (i + 1 < count && j < iv_count) q0 = __ldg(reinterpret_cast<const float4 *>(p.intervals + iv_first + j));
+        if (i + 1 < count && j < iv_count) {
+          q0 = __ldg(reinterpret_cast<const float4 *>(p.intervals + iv_first + j));
+          if (CONTACT) q1 = __ldg(reinterpret_cast<const float4 *>(p.intervals + iv_first + j) + 1);
+        }
         mbar_wait(bar_h_full + 8 * hs, (cnt / HPS) & 1u);
         tc_fence_after();
         const uint32_t h_tmem = tmem + HEAD_COL0 + hs * NOUT + lane_addr;
@@ -604,6 +660,7 @@ __global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(c
           v.z = __fdividef(1.0f, 1.0f + __expf(-r2));
           const float sigma = fmaxf(r3, 0.0f) + __logf(1.0f + __expf(-fabsf(r3)));
           v.w = __expf(-sigma * delta);
+          if (CONTACT) v.w = 1.0f - (1.0f - v.w) * fall;   // alpha = (1 - exp(-sigma l)) g
           p.staging[out_idx] = v;
           if constexpr (NOUT > 16) if (feat && p.n_feat != 32) {
             float *f = p.staging_feat + out_idx * (size_t)p.n_feat;
@@ -675,13 +732,23 @@ __global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(c
           q0 = __ldg(ivp); q1 = __ldg(ivp + 1);
         }
         float u[3] = {0.f, 0.f, 0.f}, d[3] = {0.f, 0.f, 0.f};
+        float z[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};   // CONTACT: [d; mu - p*]
         if (valid) {
-          const float t = ms_sample_t(c0.y, c0.z, (int)kk);
+          const float t = ms_sample_tm(c0.y, c0.z, (int)kk, CONTACT);
           d[0] = c1.x; d[1] = c1.y; d[2] = c1.z;
-          ms_sample_u(Al, mu, p.cam.o, d, t, u);
+          if (CONTACT) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+              z[c] = d[c];
+              z[3 + c] = __fsub_rn(mu[c], __fadd_rn(p.cam.o[c], __fmul_rn(t, d[c])));
+            }
+          } else {
+            ms_sample_u(Al, mu, p.cam.o, d, t, u);
+          }
         }
         mbar_wait(bar_a1_free + 8 * st, ((run / TC_NA1) & 1u) ^ 1u);
-        encode_row<NFREQ, VIEWDIR, K1>(u, d, s_a1 + st * A1_BYTES + row * 16);
+        if constexpr (CONTACT) encode_contact_row<NFREQ, K1>(z, s_a1 + st * A1_BYTES + row * 16);
+        else encode_row<NFREQ, VIEWDIR, K1>(u, d, s_a1 + st * A1_BYTES + row * 16);
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_a1_full + 8 * st);
@@ -730,7 +797,11 @@ void pack_wT(const float *W, const float *b, int in, int out, int k_pad, int n_p
 
 using KernelFn = void (*)(const TcParams);
 
-KernelFn select_kernel(int n_freq, int viewdir, int width, int nout, int nh) {
+KernelFn select_kernel(int n_freq, int viewdir, int width, int nout, int nh, int contact) {
+  if (contact) {   // the paper's own shape: gamma([d; delta]) 72-d, 32 wide, two hidden layers
+    if (n_freq == 6 && viewdir == 0 && width == 32 && nout == 16 && nh == 2) return mlp_tc_kernel<6, 0, 32, 16, 2, 1>;
+    return nullptr;
+  }
 #define MS_TC_CASE(F, V, W, O, H) \
   if (n_freq == F && viewdir == V && width == W && nout == O && nh == H) return mlp_tc_kernel<F, V, W, O, H>;
   MS_TC_CASE(4, 0, 64, 16, 3)
@@ -755,7 +826,7 @@ int nout_pad(int out_dim) { return out_dim <= 16 ? 16 : (out_dim <= 36 ? 48 : 0)
 int ms_tc_pack(const MsMlpShape &sh, int n_prims, const float *weights, MsTcWeights *out) {
   out->valid = false;
   const int nout = nout_pad(sh.out_dim);
-  if (nout == 0 || !select_kernel(sh.n_freq, sh.use_viewdir, sh.width, nout, sh.n_hidden)) return MS_OK;  // shape not covered
+  if (nout == 0 || !select_kernel(sh.n_freq, sh.use_viewdir, sh.width, nout, sh.n_hidden, sh.mode == MS_MODE_CONTACT)) return MS_OK;  // shape not covered
   const int k1 = (sh.in_dim + 2 + 15) / 16 * 16;
   const TcLayout L = tc_layout(k1, sh.width, sh.n_hidden, nout);
   std::vector<uint8_t> img;
@@ -798,7 +869,8 @@ void ms_tc_free(MsTcWeights *w) {
 cudaError_t ms_mlp_tc(const MsTcWeights &w, const MsMlpArgs &a, cudaStream_t s) {
   if (a.n_blocks == 0) return cudaSuccess;
   if (!w.valid) return cudaErrorNotSupported;
-  KernelFn fn = select_kernel(a.shape.n_freq, a.shape.use_viewdir, a.shape.width, w.n_out_pad, a.shape.n_hidden);
+  KernelFn fn = select_kernel(a.shape.n_freq, a.shape.use_viewdir, a.shape.width, w.n_out_pad, a.shape.n_hidden,
+                              a.shape.mode == MS_MODE_CONTACT);
   if (!fn) return cudaErrorNotSupported;
   TcParams p;
   p.cam = a.cam; p.K = a.K; p.n_prims = a.n_prims; p.n_feat = a.shape.n_feat; p.n_blocks = a.n_blocks;

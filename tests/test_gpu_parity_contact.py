@@ -62,7 +62,7 @@ def test_contact_mode_argument_checks():
     with pytest.raises(api.MsError):
         gs.render(cam, 18, 32, 4)                                   # K samples per chord is the other mode
     with pytest.raises(api.MsError):
-        gs.render(cam, 18, 32, 1, path=api.PATH_BF16_TC)            # fp32 path only
+        gs.render(cam, 18, 32, 1, path=api.PATH_BF16_TC)            # fp32 weights: no tensor image was packed
 
 
 def test_contact_dense_scene_early_termination_and_t_near():
@@ -114,3 +114,37 @@ def test_slot_argument_checks():
     sc2.slots = np.zeros((sc2.n, 4, 128), np.float32)
     with pytest.raises(api.MsError):
         api.Scene(sc2)
+
+
+@pytest.mark.parametrize("W,H", [(160, 90), (97, 61)])
+def test_next1_tensor_path(W, H):
+    """Contact-point mode on the tcgen05 path (bf16 weights, 72-32-32-4): structures bit-exact,
+    rgb/alpha at the bf16 bar of the north star (3e-3 max, 5e-4 mean per channel)."""
+    from test_gpu_parity_bf16 import assert_bf16_bar
+    from test_gpu_parity_fp32 import check_structures
+    api = _api()
+    cfg = synth.shrink(synth.CONFIGS["next1b"], W, H)
+    sc, cam = synth.make_scene(cfg), synth.make_cameras(cfg)[0]
+    orc = mso.OracleScene(sc)
+    gs = api.Scene(sc)
+    rgb, alpha, _ = gs.render(cam, H, W, 1, path=api.PATH_BF16_TC, flags=api.FLAG_KEEP_DEBUG)
+    torch.cuda.synchronize()
+    o_rgb, o_alpha, _, st = orc.render(cam, H, W, 1)
+    assert check_structures(gs, orc, cam, H, W, 1, 16, n_order_rays=8) == st.n_intervals
+    assert_bf16_bar(rgb.cpu().numpy().reshape(-1, 3), alpha.cpu().numpy().reshape(-1), o_rgb, o_alpha)
+    rgb32, alpha32, _ = gs.render(cam, H, W, 1, path=api.PATH_FP32)       # same scene, fp32 path: far tighter
+    torch.cuda.synchronize()
+    assert np.abs(rgb32.cpu().numpy().reshape(-1, 3) - o_rgb).max() <= TOL_FP32
+
+
+def test_next1b_full_size_sampled_pixels():
+    from test_gpu_parity_bf16 import assert_bf16_bar
+    api = _api()
+    cfg = synth.CONFIGS["next1b"]
+    sc, cam = synth.make_scene(cfg), synth.make_cameras(cfg)[0]
+    gs = api.Scene(sc)
+    rgb, alpha, _ = gs.render(cam, cfg.height, cfg.width, 1)               # AUTO -> tensor path
+    torch.cuda.synchronize()
+    pix = np.random.default_rng(4).choice(cfg.width * cfg.height, 20000, replace=False).astype(np.int32)
+    o_rgb, o_alpha, _, _ = mso.OracleScene(sc).render(cam, cfg.height, cfg.width, 1, pixels=pix)
+    assert_bf16_bar(rgb.cpu().numpy().reshape(-1, 3)[pix], alpha.cpu().numpy().reshape(-1)[pix], o_rgb, o_alpha)
