@@ -182,6 +182,7 @@ struct TcParams {
   const uint8_t *image;
   float4 *staging;
   float *staging_feat;
+  float4 *staging_gate;   // CONTACT + Eq.7 slot features: the four gates of every hit, or NULL
 };
 
 __device__ __forceinline__ int find_prim(const uint32_t *__restrict__ blk_off, int n, uint32_t b) {
@@ -624,6 +625,7 @@ __global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(c
           float uu[3];
           ms_sample_u(Al, mu, p.cam.o, dd, q0.y, uu);
           fall = __expf(-4.5f * (uu[0] * uu[0] + uu[1] * uu[1] + uu[2] * uu[2]));
+          if (p.staging_gate) p.staging_gate[out_idx] = ms_slot_gates(uu);   // Eq.7 gates for stage (e)
         }
         k += dk; j += dj;
         if (k >= K) { k -= K; ++j; }
@@ -876,7 +878,7 @@ cudaError_t ms_mlp_tc(const MsTcWeights &w, const MsMlpArgs &a, cudaStream_t s) 
   p.cam = a.cam; p.K = a.K; p.n_prims = a.n_prims; p.n_feat = a.shape.n_feat; p.n_blocks = a.n_blocks;
   p.center = a.center; p.A = a.A; p.prim_start = a.prim_start; p.blk_off = a.blk_off; p.intervals = a.intervals;
   p.image = (const uint8_t *)w.image;
-  p.staging = a.staging; p.staging_feat = a.staging_feat;
+  p.staging = a.staging; p.staging_feat = a.staging_feat; p.staging_gate = a.staging_gate;
   size_t smem = w.bytes_per_prim + tc_a1_stages(a.shape.width) * ((size_t)MS_ROWS * w.k1_pad * 2);
   if (w.n_out_pad > 16) smem += 4 * 32 * TC_HD_ROW;
   if (smem < TC_MIN_SMEM) smem = TC_MIN_SMEM;

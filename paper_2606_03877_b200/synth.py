@@ -114,6 +114,8 @@ CONFIGS: dict[str, SceneConfig] = {
     # next1 with bf16 weights: the same mode on the tcgen05 path (32-wide MLPs), at the bf16 parity bar
     "next1b": SceneConfig("next1b", 6, 2048, 2.0, 0.05, 0.5,
                           MLPSpec(6, 0, 2, 32, 0, True, MODE_CONTACT), 1280, 720, 60.0, 5.0, 1),
+    "next2b": SceneConfig("next2b", 6, 2048, 2.0, 0.05, 0.5,
+                          MLPSpec(6, 0, 2, 32, 0, True, MODE_CONTACT), 1280, 720, 60.0, 5.0, 1, c_f=512),
     "next2": SceneConfig("next2", 6, 2048, 2.0, 0.05, 0.5,
                          MLPSpec(6, 0, 2, 32, 0, False, MODE_CONTACT), 1280, 720, 60.0, 5.0, 1, c_f=512),
 }

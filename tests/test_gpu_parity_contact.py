@@ -148,3 +148,21 @@ def test_next1b_full_size_sampled_pixels():
     pix = np.random.default_rng(4).choice(cfg.width * cfg.height, 20000, replace=False).astype(np.int32)
     o_rgb, o_alpha, _, _ = mso.OracleScene(sc).render(cam, cfg.height, cfg.width, 1, pixels=pix)
     assert_bf16_bar(rgb.cpu().numpy().reshape(-1, 3)[pix], alpha.cpu().numpy().reshape(-1)[pix], o_rgb, o_alpha)
+
+
+def test_next2_slot_features_tensor_path():
+    """Slot features with the MLPs on the tensor path: the gates come from the canonical fp32 geometry,
+    the weights T alpha from bf16 MLPs -> the bf16 bar, relative to the features' range."""
+    from dataclasses import replace
+    from test_gpu_parity_bf16 import TOL_MAX, TOL_MEAN, assert_bf16_bar
+    api = _api()
+    cfg = synth.shrink(replace(synth.CONFIGS["next2b"], c_f=128), 96, 54)
+    sc, cam = synth.make_scene(cfg), synth.make_cameras(cfg)[0]
+    gs = api.Scene(sc)
+    rgb, alpha, feat = gs.render(cam, 54, 96, 1)                            # AUTO -> tensor path
+    torch.cuda.synchronize()
+    o_rgb, o_alpha, o_feat, _ = mso.OracleScene(sc).render(cam, 54, 96, 1)
+    assert_bf16_bar(rgb.cpu().numpy().reshape(-1, 3), alpha.cpu().numpy().reshape(-1), o_rgb, o_alpha)
+    d = np.abs(feat.cpu().numpy().reshape(-1, 128) - o_feat)
+    scale = max(1.0, np.abs(o_feat).max())
+    assert d.max() <= TOL_MAX * scale and np.all(d.mean(axis=0) <= TOL_MEAN * scale)
