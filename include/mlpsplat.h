@@ -73,7 +73,8 @@ enum { MS_MODE_LOCAL = 0, MS_MODE_CONTACT = 1 };
  * x[2L j + 2l + 1] = cos(2^l pi z_j); in_dim = 12 L, no identity, use_viewdir must be 0.
  * alpha = (1 - exp(-sigma l)) g with l = the chord length of the ray inside the support and
  * g = exp(-(9/2) |p* - mu|^2_Lambda) (readings of P:105); hits are
- * composited in the order of (t*, primitive id).  ms_opts.K must be 1; fp32 path only. */
+ * composited in the order of (t*, primitive id).  ms_opts.K must be 1.  Paths: fp32 for any shape;
+ * the tensor path for dtype = MS_BF16 with the paper's shape (L = 6, width 32, two hidden layers, n_feat 0). */
 typedef struct {
   int32_t n_freq;      /* L >= 0 */
   int32_t use_viewdir; /* 0 / 1 */
