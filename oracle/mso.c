@@ -26,6 +26,7 @@ struct mso_scene {
   int32_t n;
   int32_t n_freq, use_viewdir, n_hidden, width, n_feat, mode;
   int32_t c_f;           /* Eq.7 slot embeddings: width (0 = none) */
+  int32_t order;         /* MSO_ORDER_EXACT | MSO_ORDER_TILE (contact mode, binned only) */
   float *slots;          /* [n][4][c_f] */
   int32_t in_dim, out_dim, n_layers, params;
   float *center;  /* [n][3] */
@@ -107,6 +108,13 @@ int mso_scene_create(const mso_prims *p, const mso_mlp *m, mso_scene **out) {
   return MSO_OK;
 }
 
+int mso_scene_set_order(mso_scene *s, int32_t order) {
+  if (!s || (order != MSO_ORDER_EXACT && order != MSO_ORDER_TILE)) return MSO_ERR_ARG;
+  if (order == MSO_ORDER_TILE && s->mode != MSO_MODE_CONTACT) return MSO_ERR_ARG;
+  s->order = order;
+  return MSO_OK;
+}
+
 int mso_scene_set_slots(mso_scene *s, int32_t c_f, const float *emb) {
   if (!s || c_f < 1 || !emb || s->mode != MSO_MODE_CONTACT || s->n_feat != 0) return MSO_ERR_ARG;
   float *p = (float *)malloc((size_t)s->n * 4 * (size_t)c_f * sizeof(float));
@@ -156,9 +164,8 @@ int mso_prim_frames(const mso_scene *s, float *A, float *M) {
 /* ------------------------------------------------------------------------------------------
  * Camera ray (Q14: pixel centres at +0.5, row 0 on top, OpenCV frame)
  * ---------------------------------------------------------------------------------------- */
-static void camera_ray(const mso_camera *c, int x, int y, float *o, float *d) {
-  float px = (float)x + 0.5f;
-  float py = (float)y + 0.5f;
+/* ray through the image point (px, py) in pixel units; pixel (x, y) has its centre at (x + 0.5, y + 0.5) */
+static void point_ray(const mso_camera *c, float px, float py, float *o, float *d) {
   float dcx = (px - c->cx) / c->fx;
   float dcy = (py - c->cy) / c->fy;
   const float *m = c->c2w;   /* rows: [r00 r01 r02 tx] ... */
@@ -169,6 +176,10 @@ static void camera_ray(const mso_camera *c, int x, int y, float *o, float *d) {
   float nrm = sqrtf(n2);
   d[0] = wx / nrm; d[1] = wy / nrm; d[2] = wz / nrm;
   o[0] = m[3]; o[1] = m[7]; o[2] = m[11];
+}
+
+static void camera_ray(const mso_camera *c, int x, int y, float *o, float *d) {
+  point_ray(c, (float)x + 0.5f, (float)y + 0.5f, o, d);
 }
 
 int mso_ray(const mso_camera *c, int x, int y, float *o, float *d) {
@@ -276,6 +287,26 @@ typedef struct { int tiles_x, tiles_y; int64_t *offsets; tkey_t *keys; size_t n;
 
 static void tlists_free(tlists_t *t) { free(t->offsets); free(t->keys); memset(t, 0, sizeof(*t)); }
 
+/* "a representative virtual ray passing through the tile center" orders the tile's primitives
+ * for every pixel of the tile: t*_{i,c} of Eq.2 for the ray through the centre point of tile (a, b). */
+static float tile_center_tstar(const mso_scene *s, const mso_camera *cam, int i, int a, int b, int tile) {
+  float o[3], d[3];
+  point_ray(cam, (float)(a * tile) + 0.5f * (float)tile, (float)(b * tile) + 0.5f * (float)tile, o, d);
+  const float *A = s->A + 9 * i;
+  const float *mu = s->center + 3 * i;
+  float v0 = o[0] - mu[0], v1 = o[1] - mu[1], v2 = o[2] - mu[2];
+  float o0 = dot3(A[0], A[1], A[2], v0, v1, v2);
+  float o1 = dot3(A[3], A[4], A[5], v0, v1, v2);
+  float o2 = dot3(A[6], A[7], A[8], v0, v1, v2);
+  float d0 = dot3(A[0], A[1], A[2], d[0], d[1], d[2]);
+  float d1 = dot3(A[3], A[4], A[5], d[0], d[1], d[2]);
+  float d2 = dot3(A[6], A[7], A[8], d[0], d[1], d[2]);
+  float aa = dot3(d0, d1, d2, d0, d1, d2);
+  float bb = dot3(o0, o1, o2, d0, d1, d2);
+  float ts = (-bb) / aa;
+  return ts > 0.0f ? ts : 0.0f;
+}
+
 static int tlists_build(const mso_scene *s, const mso_camera *cam, int H, int W, int tile, tlists_t *out) {
   memset(out, 0, sizeof(*out));
   int tx = (W + tile - 1) / tile, ty = (H + tile - 1) / tile;
@@ -295,6 +326,7 @@ static int tlists_build(const mso_scene *s, const mso_camera *cam, int H, int W,
           if (!k2) { free(keys); return MSO_ERR_MEM; }
           keys = k2;
         }
+        if (s->order == MSO_ORDER_TILE) { float tc = tile_center_tstar(s, cam, i, a, b, tile); memcpy(&zb, &tc, 4); }
         keys[n].tile = (uint32_t)(b * tx + a); keys[n].zbits = zb; keys[n].prim = i; ++n;
       }
   }
@@ -539,7 +571,7 @@ static long build_samples(const mso_scene *s, long nh, int K, raybuf_t *rb) {
       rb->samps[j].prim = rb->hits[h].prim; rb->samps[j].k = k; rb->samps[j].hit = (int32_t)h;
       ++j;
     }
-  qsort(rb->samps, ns, sizeof(samp_t), samp_cmp);
+  if (s->order != MSO_ORDER_TILE) qsort(rb->samps, ns, sizeof(samp_t), samp_cmp);   /* tile order: the tile list's order as it is */
   return (long)ns;
 }
 
@@ -565,6 +597,7 @@ int mso_render(const mso_scene *s, const mso_camera *cam, int H, int W, const ms
   if (!s || !cam || !opt || H <= 0 || W <= 0 || opt->K <= 0 || opt->tile < 0 || !out_rgb || !out_alpha)
     return MSO_ERR_ARG;
   if (s->mode == MSO_MODE_CONTACT && opt->K != 1) return MSO_ERR_ARG;
+  if (s->order == MSO_ORDER_TILE && opt->tile <= 0) return MSO_ERR_ARG;   /* the shared order is a property of the tiling */
   if (s->in_dim > MSO_MAXW || s->width > MSO_MAXW || s->out_dim > MSO_MAXW) return MSO_ERR_ARG;
   if (!pix) n_pix = (int64_t)H * W;
   tlists_t tl; memset(&tl, 0, sizeof(tl));

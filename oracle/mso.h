@@ -77,6 +77,7 @@ typedef struct {
 } mso_mlp;
 
 enum { MSO_MODE_LOCAL = 0, MSO_MODE_CONTACT = 1 };
+enum { MSO_ORDER_EXACT = 0, MSO_ORDER_TILE = 1 };
 
 typedef struct {
   float fx, fy, cx, cy;
@@ -104,6 +105,11 @@ typedef struct {
 enum { MSO_OK = 0, MSO_ERR_ARG = -1, MSO_ERR_MEM = -2, MSO_ERR_CAP = -3 };
 
 int  mso_scene_create(const mso_prims *, const mso_mlp *, mso_scene **out);
+/* contact mode: MSO_ORDER_TILE composites every pixel of a tile in ONE shared order, that of the contact
+ * points t*_{i,c} of the virtual ray through the tile centre (ties by primitive id) -- the paper's
+ * approximation (about 2x faster, -0.35 dB there).  Binned mode only; the tile lists are then sorted by
+ * (tile, t*_{i,c}, primitive id).  Default MSO_ORDER_EXACT: per-ray order by (t*, primitive id). */
+int  mso_scene_set_order(mso_scene *, int32_t order);
 /* contact mode, n_feat == 0: attach slot embeddings emb[n][4][c_f] (copied); mso_render then writes feat[n_pix][c_f] */
 int  mso_scene_set_slots(mso_scene *, int32_t c_f, const float *emb);
 /* gates g[4] of primitive prim for the residual delta = mu - p* (world frame) */

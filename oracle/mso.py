@@ -234,6 +234,12 @@ class OracleScene:
             raise RuntimeError(f"mso_mlp_eval failed: {rc}")
         return raw, act
 
+    def set_order(self, order: int):
+        """0: exact per-ray order; 1: the paper's shared per-tile order of the tile-centre ray (contact mode)."""
+        rc = lib().mso_scene_set_order(self._h, C.c_int32(order))
+        if rc != 0:
+            raise ValueError(f"mso_scene_set_order failed: {rc}")
+
     def slot_gates(self, prim, delta):
         g = np.zeros(4, np.float64)
         dl = np.ascontiguousarray(delta, np.float32)

@@ -157,3 +157,61 @@ def test_binned_equals_brute_force_and_invariants():
     assert st.n_samples == st.n_intervals                       # one evaluation per (ray, primitive)
     with pytest.raises(Exception):
         orc.render(cam, 54, 96, 2)                              # K samples per interval is the other mode
+
+
+def test_tile_centre_order_pins():
+    """P:109 / P:148 shared per-tile order (MSO_ORDER_TILE): (i) alpha = 1 - prod(1 - alpha_i) does not depend on
+    the order; (ii) the tile lists are sorted by Eq.2's t* of the tile-centre ray, recomputed from the
+    Lambda quadratic in fp64; (iii) a pixel's colour equals an independent fp64 re-compositing of its
+    hits in tile-list order; (iv) one primitive: identical to the exact order."""
+    cfg = synth.shrink(synth.CONFIGS["next1"], 96, 54)
+    sc, cam = synth.make_scene(cfg), synth.make_cameras(cfg)[0]
+    H, W, T = 54, 96, 8
+    orc = mso.OracleScene(sc)
+    rgb_e, alpha_e, _, st_e = orc.render(cam, H, W, 1, tile=T)
+    orc.set_order(1)
+    rgb_t, alpha_t, _, st_t = orc.render(cam, H, W, 1, tile=T)
+    assert st_t.n_intervals == st_e.n_intervals
+    assert np.abs(alpha_t - alpha_e).max() <= 1e-12                        # (i)
+    assert np.abs(rgb_t - rgb_e).max() > 1e-3                              # and the colours do differ
+    off, prim, zb = orc.tile_lists(cam, H, W, T)
+    tiles_x = (W + T - 1) // T
+    checked = 0
+    for t in range(0, len(off) - 1, 5):                                    # (ii)
+        ids = prim[off[t]:off[t + 1]]
+        if len(ids) < 2:
+            continue
+        o, d = ray64(cam, (t % tiles_x) * T + T / 2 - 0.5, (t // tiles_x) * T + T / 2 - 0.5)   # ray64 adds the half pixel
+        ts = []
+        for i in ids:
+            L, _ = lam(sc.quat[i], sc.scale[i])
+            ts.append(max(0.0, d @ L @ (sc.center[i].astype(np.float64) - o) / (d @ L @ d)))
+        ts = np.array(ts)
+        assert np.all(np.diff(ts) >= -1e-4 * np.maximum(1.0, ts[1:]))
+        assert np.abs(zb[off[t]:off[t + 1]].view(np.float32) - ts).max() <= 1e-4 * max(1.0, ts.max())
+        checked += 1
+    assert checked > 10
+    for pixel in (W * 20 + 31, W * 33 + 70, W * 41 + 12):                  # (iii)
+        x, y = pixel % W, pixel // W
+        t = (y // T) * tiles_x + x // T
+        order = list(prim[off[t]:off[t + 1]])
+        hp, ht, hl = orc.ray_intervals(cam, H, W, 1, pixel, tile=T)
+        hits = sorted(zip(hp, ht, hl), key=lambda h: order.index(h[0]))
+        o32, d32 = mso.ray(cam, x, y)
+        Tr, C = 1.0, np.zeros(3)
+        for p, tstar, chord in hits:
+            _, _, act, r2 = orc.contact_eval(int(p), o32, d32, float(tstar))
+            a = (1.0 - math.exp(-act[3] * float(chord))) * math.exp(-4.5 * r2)
+            C += Tr * a * act[:3]
+            Tr *= 1.0 - a
+        assert len(hits) >= 2 and np.abs(C - rgb_t[pixel]).max() <= 1e-12 and abs((1 - Tr) - alpha_t[pixel]) <= 1e-12
+    w = synth.constant_mlp_weights(MLP_C, [0.3, -0.2, 0.1, 0.7])           # (iv)
+    one = synth.custom_scene([[0, 0, 0]], [[1, 0, 0, 0]], [[0.8, 0.5, 0.6]], w[None], MLP_C)
+    cam1 = synth.pinhole(32, 24, 50.0, synth.look_at([0.5, 0.4, 3.0]))
+    o1 = mso.OracleScene(one)
+    a = o1.render(cam1, 24, 32, 1, tile=8)
+    o1.set_order(1)
+    b = o1.render(cam1, 24, 32, 1, tile=8)
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+    with pytest.raises(Exception):
+        o1.render(cam1, 24, 32, 1, tile=0)                                 # the shared order needs tiles
