@@ -99,7 +99,11 @@ typedef struct {
 enum { MS_PATH_AUTO = 0, MS_PATH_FP32 = 1, MS_PATH_BF16_TC = 2 };
 enum {
   MS_FLAG_KEEP_DEBUG = 1, /* keep the intermediate buffers of the last view for ms_debug_* */
-  MS_FLAG_STAGE_TIMES = 2 /* record CUDA events between stages (ms_last_stage_ms) */
+  MS_FLAG_STAGE_TIMES = 2, /* record CUDA events between stages (ms_last_stage_ms) */
+  MS_FLAG_TILE_ORDER = 4   /* MS_MODE_CONTACT only: composite every pixel of a tile in ONE shared order, that of the
+                              contact points t*_{i,c} of the virtual ray through the tile centre (the
+                              paper's approximation), instead of the exact per-ray order; the tile lists are
+                              then sorted by (tile, t*_{i,c}, primitive id) */
 };
 
 typedef struct {

@@ -18,6 +18,7 @@ _LIB_PATH = os.path.join(_HERE, "libmlpsplat.so")
 MS_F32, MS_BF16 = 0, 1
 PATH_AUTO, PATH_FP32, PATH_BF16_TC = 0, 1, 2
 FLAG_KEEP_DEBUG, FLAG_STAGE_TIMES = 1, 2
+FLAG_TILE_ORDER = 4     # contact mode: the paper's shared per-tile order instead of the exact per-ray order
 STAGES = ("bin", "sort", "isect", "mlp", "composite")
 
 EXPORTS = ["ms_scene_create", "ms_scene_set_slots", "ms_scene_destroy", "ms_render", "ms_render_batch", "ms_render_host",

@@ -50,6 +50,7 @@ struct ms_scene {
   int dbg_H = 0, dbg_W = 0, dbg_tile = 0, dbg_K = 0, dbg_prim_bits = 0, dbg_n_tiles = 0;
   uint64_t *dbg_keys = nullptr;
   float dbg_t_stop = 0.f;
+  int dbg_tile_order = 0;
 };
 
 namespace {
@@ -202,8 +203,9 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   ENS(sc->pair_hits, (P + 1) * 4);
   ENS(sc->pair_off, (P + 2) * 4);
   if (ms_scan_scratch_elems(P) + 16 > sc->scan_scratch.cap / 4) ENS(sc->scan_scratch, (ms_scan_scratch_elems(P) + 16) * 4);
+  const int tile_order = (opts->flags & MS_FLAG_TILE_ORDER) != 0;
   CK(ms_emit_keys(N, (uint32_t *)sc->emit_off.p, (int4 *)sc->rect.p, (float *)sc->z_entry.p, tiles_x, prim_bits,
-                  (uint64_t *)sc->keys_a.p, st));
+                  (uint64_t *)sc->keys_a.p, tile_order, cam, tile, sc->A, (float *)sc->oprime.p, st));
 
   // ---- (b) radix sort + tile ranges -------------------------------------------------------
   if (timing) CK(cudaEventRecord(sc->ev[1], st));
@@ -273,6 +275,7 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   MsCompositeArgs ca;
   ca.n_rays = R; ca.K = K; ca.n_feat = sc->shape.n_feat; ca.t_stop = opts->t_stop;
   ca.contact = sc->shape.mode == MS_MODE_CONTACT;
+  ca.tile_order = tile_order;
   ca.ray_off = (uint32_t *)sc->ray_off.p; ca.hits = (MsHit *)sc->hits.p; ca.staging = (float4 *)sc->staging.p;
   ca.staging_feat = want_feat ? (float *)sc->staging_feat.p : nullptr;
   ca.gates = want_slots ? (const float4 *)sc->staging_gate.p : nullptr;
@@ -296,6 +299,7 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
     sc->debug_valid = true;
     sc->dbg_H = H; sc->dbg_W = W; sc->dbg_tile = tile; sc->dbg_K = K; sc->dbg_prim_bits = prim_bits;
     sc->dbg_n_tiles = n_tiles; sc->dbg_keys = sorted; sc->dbg_t_stop = opts->t_stop;
+    sc->dbg_tile_order = tile_order;
   }
   return MS_OK;
 }
@@ -305,6 +309,7 @@ int check_render_args(ms_scene *sc, const ms_camera *cams, int n_views, int H, i
   if (!sc || !cams || !o || !rgb || !alpha || n_views < 1 || H < 1 || W < 1) return MS_ERR_INVALID_ARG;
   if (o->K < 1 || o->K > MS_MAX_K || !(o->t_stop >= 0.0f)) return MS_ERR_INVALID_ARG;
   if (sc->shape.mode == MS_MODE_CONTACT && o->K != 1) return MS_ERR_INVALID_ARG;   // one evaluation per hit
+  if ((o->flags & MS_FLAG_TILE_ORDER) && sc->shape.mode != MS_MODE_CONTACT) return MS_ERR_INVALID_ARG;
   if (o->tile != 0 && o->tile != 8 && o->tile != 16 && o->tile != 32) return MS_ERR_INVALID_ARG;
   for (int v = 0; v < n_views; ++v)
     if (!(cams[v].fx > 0.f) || !(cams[v].fy > 0.f) || !(cams[v].t_near >= 0.f)) return MS_ERR_INVALID_ARG;
@@ -584,6 +589,7 @@ int ms_debug_sample_order(ms_scene *sc, int32_t ray, int32_t *prim, int32_t *k, 
   memset(&ca, 0, sizeof(ca));
   ca.n_rays = sc->dbg_H * sc->dbg_W; ca.K = sc->dbg_K; ca.n_feat = 0; ca.t_stop = 0.f;
   ca.contact = sc->shape.mode == MS_MODE_CONTACT;
+  ca.tile_order = sc->dbg_tile_order;
   ca.ray_off = (uint32_t *)sc->ray_off.p; ca.hits = (MsHit *)sc->hits.p; ca.staging = (float4 *)sc->staging.p;
   CK(ms_sample_order(ca, ray, dp, dk, dt, 0));
   CK(cudaDeviceSynchronize());

@@ -127,7 +127,8 @@ __global__ void project_kernel(int n, const float *__restrict__ center, const fl
 // one warp per primitive; emission order: tile rows, then columns (row-major inside the rect)
 __global__ void emit_keys_kernel(int n, const uint32_t *__restrict__ emit_off, const int4 *__restrict__ rect,
                                  const float *__restrict__ z_entry, int tiles_x, int prim_bits,
-                                 uint64_t *__restrict__ keys) {
+                                 uint64_t *__restrict__ keys, int tile_order, MsCam cam, int tile,
+                                 const float *__restrict__ A, const float *__restrict__ oprime) {
   int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   int lane = threadIdx.x & 31;
   if (i >= n) return;
@@ -139,6 +140,13 @@ __global__ void emit_keys_kernel(int n, const uint32_t *__restrict__ emit_off, c
   for (uint32_t j = lane; j < cnt; j += 32) {
     int ty = rc.y + (int)(j / (uint32_t)tw), tx = rc.x + (int)(j % (uint32_t)tw);
     uint64_t t = (uint64_t)(uint32_t)(ty * tiles_x + tx);
+    if (tile_order) {  // order of the contact points of the virtual ray through the tile centre
+      float d[3];
+      ms_point_ray(cam, __fadd_rn((float)(tx * tile), __fmul_rn(0.5f, (float)tile)),
+                   __fadd_rn((float)(ty * tile), __fmul_rn(0.5f, (float)tile)), d);
+      const float tc = ms_contact_t(A + 9 * (size_t)i, oprime + 3 * (size_t)i, d);
+      low = ((uint64_t)__float_as_uint(tc) << prim_bits) | (uint64_t)(uint32_t)i;
+    }
     keys[beg + j] = (t << (32 + prim_bits)) | low;
   }
 }
@@ -173,10 +181,11 @@ cudaError_t ms_project(int n, const float *center, const float *A, const float *
 }
 
 cudaError_t ms_emit_keys(int n, const uint32_t *emit_off, const int4 *rect, const float *z_entry, int tiles_x,
-                         int prim_bits, uint64_t *keys, cudaStream_t s) {
+                         int prim_bits, uint64_t *keys, int tile_order, MsCam cam, int tile, const float *A,
+                         const float *oprime, cudaStream_t s) {
   long threads = (long)n * 32;
   emit_keys_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, s>>>(n, emit_off, rect, z_entry, tiles_x, prim_bits,
-                                                                    keys);
+                                                                    keys, tile_order, cam, tile, A, oprime);
   MS_LAUNCHED();
   return cudaGetLastError();
 }

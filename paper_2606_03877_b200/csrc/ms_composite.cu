@@ -136,7 +136,7 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
       const int dh = 32 / K, dk = 32 - dh * K;
       for (uint32_t s = lane; s < S; s += 32) {
         float t;
-        const uint32_t rk = sample_rank(sm, hits, n, K, h, k, &t, a.contact) - r0;
+        const uint32_t rk = (a.tile_order ? s : sample_rank(sm, hits, n, K, h, k, &t, a.contact)) - r0;
         if (rk < cnt) sm.ord[rk] = s;
         h += dh; k += dk;
         if (k >= K) { k -= K; ++h; }
@@ -292,7 +292,8 @@ __global__ void sample_order_kernel(MsCompositeArgs a, int ray, int *dbg_prim, i
   for (uint32_t s = lane; s < S; s += 32) {
     const int h = (int)(s / (uint32_t)K), k = (int)(s - (uint32_t)h * (uint32_t)K);
     float t;
-    const uint32_t rk = sample_rank(sm, hits, n, K, h, k, &t, a.contact);
+    uint32_t rk = sample_rank(sm, hits, n, K, h, k, &t, a.contact);
+    if (a.tile_order) rk = s;   // the shared per-tile order: the hits as stage (c) wrote them
     dbg_prim[rk] = hits[h].prim; dbg_k[rk] = k; dbg_t[rk] = t;
   }
 }

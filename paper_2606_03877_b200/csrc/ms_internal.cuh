@@ -51,9 +51,8 @@ __device__ __forceinline__ float ms_dot3(float a0, float a1, float a2, float b0,
   return __fadd_rn(__fadd_rn(__fmul_rn(a0, b0), __fmul_rn(a1, b1)), __fmul_rn(a2, b2));
 }
 
-__device__ __forceinline__ void ms_camera_ray(const MsCam &c, int x, int y, float *d) {
-  float px = __fadd_rn((float)x, 0.5f);
-  float py = __fadd_rn((float)y, 0.5f);
+// ray through the image point (px, py) in pixel units; pixel (x, y) has its centre at (x + 0.5, y + 0.5)
+__device__ __forceinline__ void ms_point_ray(const MsCam &c, float px, float py, float *d) {
   float dcx = __fdiv_rn(__fsub_rn(px, c.cx), c.fx);
   float dcy = __fdiv_rn(__fsub_rn(py, c.cy), c.fy);
   float wx = __fadd_rn(__fadd_rn(__fmul_rn(c.r[0], dcx), __fmul_rn(c.r[1], dcy)), c.r[2]);
@@ -64,6 +63,21 @@ __device__ __forceinline__ void ms_camera_ray(const MsCam &c, int x, int y, floa
   d[0] = __fdiv_rn(wx, nrm);
   d[1] = __fdiv_rn(wy, nrm);
   d[2] = __fdiv_rn(wz, nrm);
+}
+
+__device__ __forceinline__ void ms_camera_ray(const MsCam &c, int x, int y, float *d) {
+  ms_point_ray(c, __fadd_rn((float)x, 0.5f), __fadd_rn((float)y, 0.5f), d);
+}
+
+// Eq.2's t* = max(-b/a, 0) of primitive (A, op = A (o - mu)) for the ray direction d (the tile-centre order)
+__device__ __forceinline__ float ms_contact_t(const float *A, const float *op, const float *d) {
+  float d0 = ms_dot3(A[0], A[1], A[2], d[0], d[1], d[2]);
+  float d1 = ms_dot3(A[3], A[4], A[5], d[0], d[1], d[2]);
+  float d2 = ms_dot3(A[6], A[7], A[8], d[0], d[1], d[2]);
+  float a = ms_dot3(d0, d1, d2, d0, d1, d2);
+  float b = ms_dot3(op[0], op[1], op[2], d0, d1, d2);
+  float ts = __fdiv_rn(-b, a);
+  return ts > 0.0f ? ts : 0.0f;
 }
 
 // ray / ellipsoid chord in the unit-sphere frame; op = A (o - mu) is per primitive per view.
@@ -150,8 +164,10 @@ cudaError_t ms_prep_prims(int n, const float *center, const float *quat, const f
 cudaError_t ms_project(int n, const float *center, const float *A, const float *M, MsCam cam, int tile,
                        int tiles_x, int tiles_y, uint32_t *tile_count, int4 *rect, float *z_entry, float *oprime,
                        cudaStream_t s);
+// tile_order != 0: the depth field of the key is t*_{i,c} of the tile-centre ray (needs cam, tile, A, oprime)
 cudaError_t ms_emit_keys(int n, const uint32_t *emit_off, const int4 *rect, const float *z_entry, int tiles_x,
-                         int prim_bits, uint64_t *keys, cudaStream_t s);
+                         int prim_bits, uint64_t *keys, int tile_order, MsCam cam, int tile, const float *A,
+                         const float *oprime, cudaStream_t s);
 cudaError_t ms_tile_ranges(const uint64_t *keys, size_t n_pairs, int n_tiles, int prim_bits, uint32_t *tile_start,
                            cudaStream_t s);
 
@@ -198,6 +214,7 @@ cudaError_t ms_mlp_f32(const MsMlpArgs &a, cudaStream_t s);
 // ms_composite.cu
 struct MsCompositeArgs {
   int n_rays, K, n_feat, contact;
+  int tile_order;        // contact mode: the hits are already in the tile's shared order -- no per-ray merge
   float t_stop;
   const uint32_t *ray_off;  // [R+1]
   const MsHit *hits;
