@@ -193,9 +193,11 @@ def run_ours(args, cfg):
     stream = torch.cuda.Stream()
     out = None
     with torch.cuda.stream(stream):
-        out = gs.render_batch(cams, H, W, K)          # allocates outputs + scratch
+        extra_flags = api.FLAG_TILE_ORDER if args.tile_order else 0
+        tile_kw = {"tile": args.tile} if args.tile else {}
+        out = gs.render_batch(cams, H, W, K, flags=extra_flags, **tile_kw)          # allocates outputs + scratch
         for _ in range(args.warmup):
-            gs.render_batch(cams, H, W, K, out=out)
+            gs.render_batch(cams, H, W, K, out=out, flags=extra_flags, **tile_kw)
     barrier()
     gs.stage_accum(reset=True)
     sampler = ClockSampler(local)
@@ -207,7 +209,7 @@ def run_ours(args, cfg):
     with torch.cuda.stream(stream):
         ev0.record(stream)
         for _ in range(args.steps):
-            gs.render_batch(cams, H, W, K, out=out, flags=api.FLAG_STAGE_TIMES)
+            gs.render_batch(cams, H, W, K, out=out, flags=api.FLAG_STAGE_TIMES | extra_flags, **tile_kw)
             launches += gs.stats().n_launches * V
         ev1.record(stream)
     barrier()
@@ -217,12 +219,12 @@ def run_ours(args, cfg):
     st = gs.stats()                                     # counts of the last view
 
     # ---- e2e: the same steps through ms_render_host (pinned HOST outputs, D2H inside) ----
-    host_out = gs.render_host(cams, H, W, K, stream=stream.cuda_stream)
+    host_out = gs.render_host(cams, H, W, K, stream=stream.cuda_stream, flags=extra_flags, **tile_kw)
     barrier()
     t0 = time.perf_counter()
     e2e_steps = max(1, min(args.steps, 10))
     for _ in range(e2e_steps):
-        gs.render_host(cams, H, W, K, out=host_out, stream=stream.cuda_stream)   # synchronises the stream itself
+        gs.render_host(cams, H, W, K, out=host_out, stream=stream.cuda_stream, flags=extra_flags, **tile_kw)   # synchronises the stream itself
     barrier()
     e2e_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
 
@@ -254,7 +256,8 @@ def run_ours(args, cfg):
                           sc.weights.nbytes / 2 + n_samples_view * 16 > 126e6 else
                           "working set below L2 (weights %.1f MB, per-view staging %.3f GB): no flush, config is launch-bound")
                          % (sc.weights.nbytes / 2 / 1e6, n_samples_view * 16 / 1e9),
-                   "tile": cfg.tile, "t_stop": cfg.t_stop},
+                   "tile": args.tile or cfg.tile, "t_stop": cfg.t_stop,
+                   "order": "tile-centre shared order (P:109)" if args.tile_order else "exact per-ray order"},
         "samples_per_s": world * n_samples_view * V / (ms_step * 1e-3),
         "counts_per_view": {"pairs": st.n_pairs, "intervals": st.n_intervals, "samples": st.n_samples,
                             "row_blocks": st.n_blocks, "scratch_GB": st.scratch_bytes / 1e9},
@@ -305,6 +308,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--tile-order", action="store_true",
+                    help="contact-mode configs: the paper's shared per-tile order (P:109) instead of the exact per-ray order")
+    ap.add_argument("--tile", type=int, default=0, help="tile edge override (8, 16, 32)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                                  # timing rule: W >= 3
