@@ -36,7 +36,7 @@ struct ms_scene {
   float *slots = nullptr;    // device [N][4][slot_cf]
   // per-view scratch
   Buf tile_count, emit_off, rect, z_entry, oprime, keys_a, keys_b, sort_scratch, tile_start, pair_hits, pair_off,
-      ray_hits, ray_off, scan_scratch, prim_start, prim_blocks, blk_off, intervals, hits, staging, staging_feat, staging_gate,
+      ray_hits, ray_off, scan_scratch, prim_start, prim_blocks, blk_off, intervals, hits, staging, staging_feat, staging_gate, staging_coef,
       host_rgb, host_alpha, host_feat, dbg;
   uint32_t *pinned = nullptr;  // [4] host-pinned readback
   cudaEvent_t ev[MS_N_STAGES + 1] = {};
@@ -98,7 +98,7 @@ size_t scratch_total(const ms_scene *sc) {
   const Buf *all[] = {&sc->tile_count, &sc->emit_off, &sc->rect, &sc->z_entry, &sc->oprime, &sc->keys_a, &sc->keys_b,
                       &sc->sort_scratch, &sc->tile_start, &sc->pair_hits, &sc->pair_off, &sc->ray_hits, &sc->ray_off,
                       &sc->scan_scratch, &sc->prim_start, &sc->prim_blocks, &sc->blk_off, &sc->intervals, &sc->hits,
-                      &sc->staging, &sc->staging_feat, &sc->staging_gate};
+                      &sc->staging, &sc->staging_feat, &sc->staging_gate, &sc->staging_coef};
   size_t t = 0;
   for (const Buf *b : all) t += b->cap;
   return t;
@@ -253,6 +253,7 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   if (want_feat) ENS(sc->staging_feat, (n_samples + 1) * (size_t)sc->shape.n_feat * 4);
   const bool want_slots = sc->slot_cf > 0 && out_feat != nullptr;   // Eq.7 features (contact mode, K = 1)
   if (want_slots) ENS(sc->staging_gate, (n_samples + 1) * sizeof(float4));
+  if (want_slots) ENS(sc->staging_coef, (n_samples + 1) * sizeof(float4));
   ia.intervals = (MsInterval *)sc->intervals.p;
   ia.hits = (MsHit *)sc->hits.p;
   CK(ms_isect_fill(ia, st));
@@ -279,6 +280,7 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   ca.ray_off = (uint32_t *)sc->ray_off.p; ca.hits = (MsHit *)sc->hits.p; ca.staging = (float4 *)sc->staging.p;
   ca.staging_feat = want_feat ? (float *)sc->staging_feat.p : nullptr;
   ca.gates = want_slots ? (const float4 *)sc->staging_gate.p : nullptr;
+  ca.coef = want_slots ? (float4 *)sc->staging_coef.p : nullptr;
   ca.slots = sc->slots; ca.c_f = sc->slot_cf;
   ca.out_rgb = out_rgb; ca.out_alpha = out_alpha; ca.out_feat = (want_feat || want_slots) ? out_feat : nullptr;
   CK(ms_composite(ca, st));
@@ -449,7 +451,7 @@ int ms_scene_destroy(ms_scene *sc) {
   Buf *all[] = {&sc->tile_count, &sc->emit_off, &sc->rect, &sc->z_entry, &sc->oprime, &sc->keys_a, &sc->keys_b,
                 &sc->sort_scratch, &sc->tile_start, &sc->pair_hits, &sc->pair_off, &sc->ray_hits, &sc->ray_off,
                 &sc->scan_scratch, &sc->prim_start, &sc->prim_blocks, &sc->blk_off, &sc->intervals, &sc->hits,
-                &sc->staging, &sc->staging_feat, &sc->staging_gate, &sc->host_rgb, &sc->host_alpha, &sc->host_feat, &sc->dbg};
+                &sc->staging, &sc->staging_feat, &sc->staging_gate, &sc->staging_coef, &sc->host_rgb, &sc->host_alpha, &sc->host_feat, &sc->dbg};
   for (Buf *b : all) free_buf(*b);
   if (sc->pinned) cudaFreeHost(sc->pinned);
   for (int i = 0; i <= MS_N_STAGES; ++i)

@@ -119,14 +119,13 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
   float T = 1.0f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
   float F[MS_MAX_OUT / 32] = {0.f, 0.f};
   float4 F4 = make_float4(0.f, 0.f, 0.f, 0.f);   // n_feat == 32: channels 4*(lane%8)..+3 of the samples of lane group lane/8
-  float4 Fs[4];                                  // slot features: channels 4*(lane + 32 q)..+3, q < c_f/128
-#pragma unroll
-  for (int q = 0; q < 4; ++q) Fs[q] = make_float4(0.f, 0.f, 0.f, 0.f);
   if (n > 0) {
     const MsHit *hits = a.hits + off;
     const float4 *stg = a.staging + (size_t)off * (size_t)K;
     const uint32_t S = (uint32_t)n * (uint32_t)K;
     load_hits(sm, hits, n, K, lane, a.contact);
+    if (FEAT == 2 && S > (uint32_t)CAP)   // a ray that stops early leaves its later windows unvisited: their coefficients are 0
+      for (uint32_t s = lane; s < S; s += 32) a.coef[off + s] = make_float4(0.f, 0.f, 0.f, 0.f);
     __syncwarp();
     bool stopped = false;
     for (uint32_t r0 = 0; r0 < S && !stopped; r0 += CAP) {
@@ -181,27 +180,16 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
       }
       C0 += c0; C1 += c1; C2 += c2;
       if (FEAT == 2) {
-        // Eq.7: f_i = sum_k g_ik e_ik, F += (T_i alpha_i) f_i.  One hit per merged sample (K = 1):
-        // every lane takes 4 channels per 128 of the primitive's four embedding rows (coalesced 512 B loads).
+        // Eq.7: F = sum_i (T_i alpha_i) sum_k g_ik e_ik.  This kernel only turns every hit's gates into
+        // its coefficients (T alpha) g_k; slot_feature_kernel sums the embeddings (the sum's order is free).
         __syncwarp();
         const float4 *gates = a.gates + off;
-        const int cf4 = a.c_f >> 2, nq = a.c_f >> 7;
-        for (uint32_t r = 0; r < done; ++r) {
+        float4 *coef = a.coef + off;
+        for (uint32_t r = lane; r < cnt; r += 32) {
           const uint32_t s = sm.ord[r];
-          const float w = s_w[FEAT ? warp : 0][FEAT ? r : 0];
+          const float w = r < done ? s_w[FEAT ? warp : 0][FEAT ? r : 0] : 0.0f;
           const float4 g = __ldg(gates + s);
-          const float4 *e = reinterpret_cast<const float4 *>(a.slots + (size_t)__ldg(&hits[s].prim) * 4 * (size_t)a.c_f) + lane;
-#pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            if (q < nq) {
-              const float4 e0 = __ldg(e + 32 * q), e1 = __ldg(e + cf4 + 32 * q), e2 = __ldg(e + 2 * cf4 + 32 * q),
-                           e3 = __ldg(e + 3 * cf4 + 32 * q);
-              Fs[q].x = fmaf(w, fmaf(g.w, e3.x, fmaf(g.z, e2.x, fmaf(g.y, e1.x, g.x * e0.x))), Fs[q].x);
-              Fs[q].y = fmaf(w, fmaf(g.w, e3.y, fmaf(g.z, e2.y, fmaf(g.y, e1.y, g.x * e0.y))), Fs[q].y);
-              Fs[q].z = fmaf(w, fmaf(g.w, e3.z, fmaf(g.z, e2.z, fmaf(g.y, e1.z, g.x * e0.z))), Fs[q].z);
-              Fs[q].w = fmaf(w, fmaf(g.w, e3.w, fmaf(g.z, e2.w, fmaf(g.y, e1.w, g.x * e0.w))), Fs[q].w);
-            }
-          }
+          coef[s] = make_float4(w * g.x, w * g.y, w * g.z, w * g.w);
         }
       }
       if (FEAT == 1) {
@@ -254,12 +242,6 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
   }
   if (lane < 3) a.out_rgb[3 * (size_t)ray + lane] = lane == 0 ? C0 : (lane == 1 ? C1 : C2);
   if (lane == 3) a.out_alpha[ray] = 1.0f - T;
-  if (FEAT == 2) {
-    const int nq = a.c_f >> 7;
-#pragma unroll
-    for (int q = 0; q < 4; ++q)
-      if (q < nq) reinterpret_cast<float4 *>(a.out_feat + (size_t)ray * a.c_f)[lane + 32 * q] = Fs[q];
-  }
   if (FEAT == 1) {
     if (nf == 32) {
 #pragma unroll
@@ -276,6 +258,107 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
       }
     }
   }
+}
+
+// Eq.7 features: F[ray] = sum over the ray's hits of coef_k e_k[prim], coef = (T alpha) g from
+// composite_kernel<2>.  The sum's order is free, so one warp takes R = 4 consecutive rays of a row and walks the
+// UNION of their primitives: the four embedding rows of a primitive (16 c_f bytes, the whole cost of this
+// stage) are loaded once and used for every ray of the group that hits it -- neighbouring rays share most
+// of their primitives (a 2 x 2 pixel block instead of 4 in a row measured no better).  Lane l holds channels 4 (l + 32 q)..+3; lane j also holds hit j of each ray.
+template <int R>
+__global__ void __launch_bounds__(CW * 32) slot_feature_kernel(MsCompositeArgs a) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const long long grp = (long long)blockIdx.x * CW + warp;
+  if (grp * R >= a.n_rays) return;
+  long long ray_of[R];
+#pragma unroll
+  for (int r = 0; r < R; ++r) ray_of[r] = grp * R + r < a.n_rays ? grp * R + r : -1;
+  const int cf4 = a.c_f >> 2, nq = a.c_f >> 7;
+  float4 F[R][4];
+  int prim[R], nh[R];
+  uint32_t off[R], used[R];
+  float4 cf[R];
+  bool big = false;
+#pragma unroll
+  for (int r = 0; r < R; ++r) {
+#pragma unroll
+    for (int q = 0; q < 4; ++q) F[r][q] = make_float4(0.f, 0.f, 0.f, 0.f);
+    const bool live = ray_of[r] >= 0;
+    off[r] = live ? a.ray_off[ray_of[r]] : 0u;
+    nh[r] = live ? (int)(a.ray_off[ray_of[r] + 1] - off[r]) : 0;
+    big |= nh[r] > 32;
+    used[r] = 0u;
+    prim[r] = -1;
+    cf[r] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (lane < nh[r] && nh[r] <= 32) {
+      prim[r] = __ldg(&a.hits[off[r] + lane].prim);
+      cf[r] = __ldg(a.coef + off[r] + lane);
+    }
+  }
+  auto add = [&](float4 (&Fr)[4], const float4 c, const float4 *e) {
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+      if (q < nq) {
+        const float4 e0 = __ldg(e + 32 * q), e1 = __ldg(e + cf4 + 32 * q), e2 = __ldg(e + 2 * cf4 + 32 * q),
+                     e3 = __ldg(e + 3 * cf4 + 32 * q);
+        Fr[q].x += fmaf(c.w, e3.x, fmaf(c.z, e2.x, fmaf(c.y, e1.x, c.x * e0.x)));
+        Fr[q].y += fmaf(c.w, e3.y, fmaf(c.z, e2.y, fmaf(c.y, e1.y, c.x * e0.y)));
+        Fr[q].z += fmaf(c.w, e3.z, fmaf(c.z, e2.z, fmaf(c.y, e1.z, c.x * e0.z)));
+        Fr[q].w += fmaf(c.w, e3.w, fmaf(c.z, e2.w, fmaf(c.y, e1.w, c.x * e0.w)));
+      }
+  };
+  if (!big) {
+#pragma unroll
+    for (int ra = 0; ra < R; ++ra) {
+      for (int j = 0; j < nh[ra]; ++j) {
+        if ((used[ra] >> j) & 1u) continue;
+        const int p = __shfl_sync(FULL, prim[ra], j);
+        const float4 *e = reinterpret_cast<const float4 *>(a.slots + (size_t)p * 4 * (size_t)a.c_f) + lane;
+        float4 c[R];          // coefficients of this primitive in the rays of the group that hit it (0 otherwise)
+#pragma unroll
+        for (int rb = 0; rb < R; ++rb) {
+          c[rb] = make_float4(0.f, 0.f, 0.f, 0.f);
+          if (rb < ra) continue;
+          int jb = j;
+          if (rb > ra) {
+            const unsigned m = __ballot_sync(FULL, prim[rb] == p) & ~used[rb];
+            if (!m) continue;
+            jb = __ffs(m) - 1;
+            used[rb] |= 1u << jb;
+          }
+          c[rb] = make_float4(__shfl_sync(FULL, cf[rb].x, jb), __shfl_sync(FULL, cf[rb].y, jb),
+                              __shfl_sync(FULL, cf[rb].z, jb), __shfl_sync(FULL, cf[rb].w, jb));
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+          if (q < nq) {
+            const float4 e0 = __ldg(e + 32 * q), e1 = __ldg(e + cf4 + 32 * q), e2 = __ldg(e + 2 * cf4 + 32 * q),
+                         e3 = __ldg(e + 3 * cf4 + 32 * q);
+#pragma unroll
+            for (int rb = 0; rb < R; ++rb) {
+              if (rb < ra) continue;
+              F[rb][q].x += fmaf(c[rb].w, e3.x, fmaf(c[rb].z, e2.x, fmaf(c[rb].y, e1.x, c[rb].x * e0.x)));
+              F[rb][q].y += fmaf(c[rb].w, e3.y, fmaf(c[rb].z, e2.y, fmaf(c[rb].y, e1.y, c[rb].x * e0.y)));
+              F[rb][q].z += fmaf(c[rb].w, e3.z, fmaf(c[rb].z, e2.z, fmaf(c[rb].y, e1.z, c[rb].x * e0.z)));
+              F[rb][q].w += fmaf(c[rb].w, e3.w, fmaf(c[rb].z, e2.w, fmaf(c[rb].y, e1.w, c[rb].x * e0.w)));
+            }
+          }
+      }
+    }
+  } else {  // a ray with more than 32 hits: no sharing, every ray on its own
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+      for (int j = 0; j < nh[r]; ++j) {
+        const int p = __ldg(&a.hits[off[r] + j].prim);
+        add(F[r], __ldg(a.coef + off[r] + j), reinterpret_cast<const float4 *>(a.slots + (size_t)p * 4 * (size_t)a.c_f) + lane);
+      }
+  }
+#pragma unroll
+  for (int r = 0; r < R; ++r)
+    if (ray_of[r] >= 0)
+#pragma unroll
+      for (int q = 0; q < 4; ++q)
+        if (q < nq) reinterpret_cast<float4 *>(a.out_feat + (size_t)ray_of[r] * a.c_f)[lane + 32 * q] = F[r][q];
 }
 
 // parity introspection: the merged order of one ray, written by rank (NS: "sample ordering bit-exact")
@@ -304,11 +387,17 @@ cudaError_t ms_composite(const MsCompositeArgs &a, cudaStream_t s) {
   if (a.n_rays == 0) return cudaSuccess;
   const unsigned grid = (unsigned)((a.n_rays + CW - 1) / CW);
   const bool feat = a.n_feat > 0 && a.out_feat && a.staging_feat;
-  const bool slots = a.c_f > 0 && a.out_feat && a.gates && a.slots && a.K == 1;
+  const bool slots = a.c_f > 0 && a.out_feat && a.gates && a.coef && a.slots && a.K == 1;
   if (slots) composite_kernel<2><<<grid, CW * 32, 0, s>>>(a);
   else if (!feat) composite_kernel<0><<<grid, CW * 32, 0, s>>>(a);
   else composite_kernel<1><<<grid, CW * 32, 0, s>>>(a);
   MS_LAUNCHED();
+  if (slots) {
+    constexpr int R = 4;
+    const long long groups = ((long long)a.n_rays + R - 1) / R;
+    slot_feature_kernel<R><<<(unsigned)((groups + CW - 1) / CW), CW * 32, 0, s>>>(a);
+    MS_LAUNCHED();
+  }
   return cudaGetLastError();
 }
 

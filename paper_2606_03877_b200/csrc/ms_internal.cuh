@@ -221,6 +221,7 @@ struct MsCompositeArgs {
   const float4 *staging;
   const float *staging_feat;
   const float4 *gates;   // [n_hits] slot gates (Eq.7) or NULL
+  float4 *coef;          // [n_hits] (T alpha) g_k per hit: composite_kernel<2> -> slot_feature_kernel
   const float *slots;    // [N][4][c_f] slot embeddings
   int c_f;
   float *out_rgb, *out_alpha, *out_feat;
