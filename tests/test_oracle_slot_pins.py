@@ -86,3 +86,18 @@ def test_next2_binned_equals_brute_and_colour_unchanged():
     # |F| <= alpha * max_k |e_k| channel-wise (convex gate, weights sum to alpha)
     bound = np.abs(sc.slots).max()
     assert (np.abs(feat) <= alpha[:, None] * bound + 1e-9).all()
+
+
+def test_next2_crop_matches_stored_oracle_snapshot():
+    """regression snapshot written by tests/golden/make_golden.py (calls only oracle/)."""
+    import json
+    import os
+    g = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "next2_oracle.json")))
+    cfg = synth.shrink(synth.replace(synth.CONFIGS["next2"], c_f=8), 96, 54)
+    sc, cam = synth.make_scene(cfg), synth.make_cameras(cfg)[0]
+    rgb, alpha, feat, st = mso.OracleScene(sc).render(cam, 54, 96, 1)
+    assert st.n_intervals == g["n_intervals"] and st.n_pairs == g["n_pairs"]
+    pix = np.array(g["pixels"])
+    np.testing.assert_allclose(rgb[pix], np.array(g["rgb"]), atol=1e-11)
+    np.testing.assert_allclose(alpha[pix], np.array(g["alpha"]), atol=1e-11)
+    np.testing.assert_allclose(feat[pix], np.array(g["feat"]), atol=1e-11)
