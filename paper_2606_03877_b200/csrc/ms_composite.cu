@@ -123,6 +123,50 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
     const MsHit *hits = a.hits + off;
     const float4 *stg = a.staging + (size_t)off * (size_t)K;
     const uint32_t S = (uint32_t)n * (uint32_t)K;
+    if (FEAT != 1 && K == 1 && n <= 32) {
+      // One sample per hit and at most one hit per lane (the contact-point mode's usual ray): lane j holds hit j,
+      // its rank is the number of hits that precede it in (t, prim) order, one product scan composites the ray.
+      float t = 0.f;
+      int prim = 0x7fffffff;
+      if (lane < n) {
+        const MsHit g = hits[lane];
+        t = ms_sample_tm(g.t_in, g.delta, 0, a.contact);
+        prim = g.prim;
+      }
+      uint32_t rank = 0;
+      for (int j = 0; j < n; ++j) {
+        const float t2 = __shfl_sync(FULL, t, j);
+        const int p2 = __shfl_sync(FULL, prim, j);
+        rank += (j != lane && precedes(t2, t, p2 < prim)) ? 1u : 0u;
+      }
+      if (a.tile_order) rank = (uint32_t)lane;      // the shared per-tile order: the hits as stage (c) wrote them
+      if (lane < n) sm.ord[rank] = (uint32_t)lane;
+      __syncwarp();
+      const bool valid = lane < n;
+      uint32_t slot = 0;
+      float4 v = make_float4(0.f, 0.f, 0.f, 1.f);
+      if (valid) {
+        slot = sm.ord[lane];
+        v = __ldg(stg + slot);
+      }
+      float p = v.w;  // inclusive product scan of e over the lanes
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const float q = __shfl_up_sync(FULL, p, o);
+        if (lane >= o) p *= q;
+      }
+      float excl = __shfl_up_sync(FULL, p, 1);
+      if (lane == 0) excl = 1.0f;
+      const unsigned stop = __ballot_sync(FULL, valid && p < a.t_stop);
+      const int last = stop ? __ffs(stop) - 1 : 31;          // Q9: the stopping sample still contributes
+      const float w = (valid && lane <= last) ? excl * (1.0f - v.w) : 0.f;
+      C0 = w * v.x; C1 = w * v.y; C2 = w * v.z;
+      T = __shfl_sync(FULL, p, stop ? last : 31);
+      if (FEAT == 2 && valid) {
+        const float4 g = __ldg(a.gates + off + slot);
+        a.coef[off + slot] = make_float4(w * g.x, w * g.y, w * g.z, w * g.w);
+      }
+    } else {
     load_hits(sm, hits, n, K, lane, a.contact);
     if (FEAT == 2 && S > (uint32_t)CAP)   // a ray that stops early leaves its later windows unvisited: their coefficients are 0
       for (uint32_t s = lane; s < S; s += 32) a.coef[off + s] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -232,6 +276,7 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
         }
       }
       __syncwarp();
+    }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
