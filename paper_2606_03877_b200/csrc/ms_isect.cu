@@ -11,9 +11,17 @@
 
 namespace {
 
+constexpr int IS_CHUNK = 32;   // primitives of the tile list staged in shared memory at a time
+
 template <bool FILL>
 __global__ void isect_kernel(MsIsectArgs a) {
-  __shared__ uint32_t wtot[2][32];
+  // The tile's list is walked in chunks of 32 primitives whose frames (A, o') and pair slots are staged
+  // in shared memory by the first 32 threads: no dependent global load and no block barrier per primitive.
+  __shared__ float sA[IS_CHUNK][12];        // A (9), o' = A (o - mu) (3)
+  __shared__ int sPrim[IS_CHUNK];
+  __shared__ uint32_t sEmit[IS_CHUNK];      // emission index of the (tile, primitive) pair
+  __shared__ uint32_t sBase[IS_CHUNK];      // FILL: pair_off[emit]
+  __shared__ uint32_t sCnt[IS_CHUNK][33];   // hits of the pair per warp (count pass: [c][32] = total)
   const int T = a.tile;
   const int tile_id = blockIdx.x;
   const int tile_x = tile_id % a.tiles_x, tile_y = tile_id / a.tiles_x;
@@ -22,7 +30,6 @@ __global__ void isect_kernel(MsIsectArgs a) {
   const bool valid = x < a.cam.W && y < a.cam.H;
   const int ray = y * a.cam.W + x;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int n_warps = (blockDim.x + 31) >> 5;
   const uint32_t lt = (1u << lane) - 1u;
   float d[3] = {0.f, 0.f, 1.f};
   if (valid) ms_camera_ray(a.cam, x, y, d);
@@ -32,42 +39,66 @@ __global__ void isect_kernel(MsIsectArgs a) {
   uint32_t my_hits = 0;
   uint32_t ray_base = 0;
   if (FILL && valid) ray_base = a.ray_off[ray];
-  for (uint32_t j = beg; j < end; ++j) {
-    const int prim = (int)(a.keys[j] & pmask);
-    const float *A = a.A + 9 * (size_t)prim;
-    const float *op = a.oprime + 3 * (size_t)prim;
-    float Al[9], ol[3];
+  for (uint32_t base = beg; base < end; base += IS_CHUNK) {
+    const int nc = (int)(end - base < (uint32_t)IS_CHUNK ? end - base : (uint32_t)IS_CHUNK);
+    __syncthreads();                        // the previous chunk is done with the staging arrays
+    if ((int)threadIdx.x < nc) {
+      const int c = threadIdx.x;
+      const int prim = (int)(a.keys[base + c] & pmask);
+      const float *A = a.A + 9 * (size_t)prim;
+      const float *op = a.oprime + 3 * (size_t)prim;
 #pragma unroll
-    for (int q = 0; q < 9; ++q) Al[q] = __ldg(A + q);
+      for (int q = 0; q < 9; ++q) sA[c][q] = __ldg(A + q);
 #pragma unroll
-    for (int q = 0; q < 3; ++q) ol[q] = __ldg(op + q);
-    float t_in = 0.f, delta = 0.f;
-    const bool hit = valid && ms_intersect(Al, ol, d, a.cam.t_near, Kf, &t_in, &delta, a.contact);
-    const int4 rc = a.rect[prim];
-    const uint32_t emit = a.emit_off[prim] + (uint32_t)((tile_y - rc.y) * (rc.z - rc.x + 1) + (tile_x - rc.x));
-    if (!FILL) {
-      const int cnt = __syncthreads_count(hit);
-      if (threadIdx.x == 0) a.pair_hits[emit] = (uint32_t)cnt;
-    } else {
+      for (int q = 0; q < 3; ++q) sA[c][9 + q] = __ldg(op + q);
+      const int4 rc = a.rect[prim];
+      const uint32_t emit = a.emit_off[prim] + (uint32_t)((tile_y - rc.y) * (rc.z - rc.x + 1) + (tile_x - rc.x));
+      sPrim[c] = prim;
+      sEmit[c] = emit;
+      if (FILL) sBase[c] = a.pair_off[emit];
+      if (!FILL) sCnt[c][32] = 0u;
+    }
+    __syncthreads();
+    // pass 1 over the chunk: which primitives does this ray hit; hits per (primitive, warp)
+    uint32_t hitmask = 0;
+    for (int c = 0; c < nc; ++c) {
+      float t_in, delta;
+      const bool hit = valid && ms_intersect(sA[c], sA[c] + 9, d, a.cam.t_near, Kf, &t_in, &delta, a.contact);
       const uint32_t ballot = __ballot_sync(0xffffffffu, hit);
-      const int buf = (int)(j & 1u);
-      if (lane == 0) wtot[buf][warp] = __popc(ballot);
-      __syncthreads();
-      if (hit) {
-        uint32_t rank = __popc(ballot & lt);
-        for (int w = 0; w < warp; ++w) rank += wtot[buf][w];
-        (void)n_warps;
-        const uint32_t slot = ray_base + my_hits;
-        MsInterval iv;
-        iv.ray = ray; iv.t_in = t_in; iv.delta = delta; iv.slot = (int)slot;
-        iv.dx = d[0]; iv.dy = d[1]; iv.dz = d[2]; iv.pad = 0;
-        a.intervals[a.pair_off[emit] + rank] = iv;
-        MsHit h;
-        h.prim = prim; h.t_in = t_in; h.delta = delta; h.pad = 0;
-        a.hits[slot] = h;
+      hitmask |= hit ? (1u << c) : 0u;
+      if (lane == 0 && ballot) {
+        if (FILL) sCnt[c][warp] = __popc(ballot);
+        else atomicAdd(&sCnt[c][32], (uint32_t)__popc(ballot));
+      } else if (FILL && lane == 0) {
+        sCnt[c][warp] = 0u;
       }
     }
-    my_hits += hit ? 1u : 0u;
+    __syncthreads();
+    if (!FILL) {
+      if ((int)threadIdx.x < nc) a.pair_hits[sEmit[threadIdx.x]] = sCnt[threadIdx.x][32];
+      my_hits += __popc(hitmask);
+    } else {
+      // pass 2: the hits are written in list order; rank inside the pair = hits of lower warps + lower lanes
+      for (int c = 0; c < nc; ++c) {
+        const bool hit = (hitmask >> c) & 1u;
+        const uint32_t ballot = __ballot_sync(0xffffffffu, hit);
+        if (hit) {
+          float t_in = 0.f, delta = 0.f;
+          ms_intersect(sA[c], sA[c] + 9, d, a.cam.t_near, Kf, &t_in, &delta, a.contact);
+          uint32_t rank = __popc(ballot & lt);
+          for (int w = 0; w < warp; ++w) rank += sCnt[c][w];
+          const uint32_t slot = ray_base + my_hits;
+          MsInterval iv;
+          iv.ray = ray; iv.t_in = t_in; iv.delta = delta; iv.slot = (int)slot;
+          iv.dx = d[0]; iv.dy = d[1]; iv.dz = d[2]; iv.pad = 0;
+          a.intervals[sBase[c] + rank] = iv;
+          MsHit h;
+          h.prim = sPrim[c]; h.t_in = t_in; h.delta = delta; h.pad = 0;
+          a.hits[slot] = h;
+          ++my_hits;
+        }
+      }
+    }
   }
   if (!FILL && valid) a.ray_hits[ray] = my_hits;
 }
