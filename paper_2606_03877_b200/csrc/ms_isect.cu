@@ -6,7 +6,8 @@
 //          ray-major   hits[ray_off[ray] + h]           (stage (e) merges these per ray)
 //          prim-major  intervals[pair_off[pair] + rank]  (stage (d) batches samples by primitive)
 // The prim-major order is (primitive, tile row-major inside its rect, pixel index in tile):
-// deterministic, no atomics.  Bytes: ~48 B written per hit; reads are L1/L2-resident lists.
+// deterministic (the only atomics are integer hit counters in shared memory).  Bytes: ~48 B written per
+// hit; reads are L1/L2-resident lists.
 #include "ms_internal.cuh"
 
 namespace {
