@@ -192,3 +192,35 @@ def test_tile_centre_order(tile):
     cfg1 = synth.shrink(synth.CONFIGS["cfg1"], 32, 18)
     with pytest.raises(api.MsError):
         api.Scene(synth.make_scene(cfg1)).render(synth.make_cameras(cfg1)[0], 18, 32, 8, flags=api.FLAG_TILE_ORDER)
+
+
+def test_more_than_32_hits_per_ray_with_slot_features():
+    """48 nested / overlapping supports around one point: the central rays carry 40+ hits, which takes the
+    general merge of stage (e) (no lane-per-hit fast path) and the unshared path of the feature kernel."""
+    api = _api()
+    mlp = synth.MLPSpec(3, 0, 1, 16, 0, False, synth.MODE_CONTACT)
+    rng = np.random.default_rng(21)
+    n = 48
+    center = rng.normal(size=(n, 3)) * 0.05
+    quat = rng.normal(size=(n, 4))
+    scale = rng.uniform(0.4, 1.2, size=(n, 3))
+    w = synth.draw_weights(rng, n, mlp, -2.0)                 # low density: the rays do not terminate early
+    slots = rng.normal(size=(n, 4, 128)).astype(np.float32)
+    sc = synth.custom_scene(center, quat, scale, w, mlp, slots=slots)
+    W, H = 40, 30
+    cam = synth.pinhole(W, H, 40.0, synth.look_at([0.3, 0.2, 4.0]))
+    gs = api.Scene(sc)
+    rgb, alpha, feat = gs.render(cam, H, W, 1, flags=api.FLAG_KEEP_DEBUG)
+    torch.cuda.synchronize()
+    orc = mso.OracleScene(sc)
+    o_rgb, o_alpha, o_feat, st = orc.render(cam, H, W, 1)
+    h_off, _, _, _ = gs.debug_intervals(H * W)
+    assert np.diff(h_off).max() > 32 and gs.stats().n_intervals == st.n_intervals
+    assert np.abs(rgb.cpu().numpy().reshape(-1, 3) - o_rgb).max() <= TOL_FP32
+    assert np.abs(alpha.cpu().numpy().reshape(-1) - o_alpha).max() <= TOL_FP32
+    scale_f = max(1.0, np.abs(o_feat).max())
+    assert np.abs(feat.cpu().numpy().reshape(-1, 128) - o_feat).max() <= TOL_FP32 * scale_f
+    ray = int(np.argmax(np.diff(h_off)))
+    gp, gk, gt = gs.debug_sample_order(ray)
+    op, ok, ot = orc.ray_samples(cam, H, W, 1, ray)
+    assert np.array_equal(gp, op) and np.array_equal(gt.view(np.uint32), ot.view(np.uint32))
