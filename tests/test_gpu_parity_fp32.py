@@ -182,3 +182,24 @@ def test_render_batch_and_host_entry_match_single_view():
         assert torch.equal(rgb[v], s[0]) and torch.equal(alpha[v], s[1]) and torch.equal(feat[v], s[2])
         assert torch.equal(h_rgb[v], s[0].cpu()) and torch.equal(h_alpha[v], s[1].cpu())
         assert torch.equal(h_feat[v], s[2].cpu())
+
+
+@pytest.mark.parametrize("K,t_stop", [(16, 1e-4), (16, 0.0), (3, 1e-4)])
+def test_more_than_32_hits_and_multi_window_rays(K, t_stop):
+    """48 overlapping supports around one point: the central rays carry 40+ hits and, at K = 16, more than
+    448 samples -- the uncached-hit branch of the merge and the windowed compositing of stage (e),
+    with and without early termination inside a later window."""
+    mlp = synth.MLPSpec(2, 0, 2, 32, 0, False)
+    rng = np.random.default_rng(33)
+    n = 48
+    center = rng.normal(size=(n, 3)) * 0.05
+    quat = rng.normal(size=(n, 4))
+    scale = rng.uniform(0.4, 1.2, size=(n, 3))
+    w = synth.draw_weights(rng, n, mlp, -1.0 if t_stop == 0.0 else 1.0)
+    sc = synth.custom_scene(center, quat, scale, w, mlp)
+    W, H = 24, 18
+    cam = synth.pinhole(W, H, 40.0, synth.look_at([0.3, 0.2, 4.0]))
+    g, o, st = render_both(sc, cam, H, W, K, t_stop=t_stop)
+    assert st.n_intervals > 32 * 20 and (K < 16 or st.n_samples / (W * H) > 448 * 0.5)
+    d = np.maximum(np.abs(g[0] - o[0]).max(axis=1), np.abs(g[1] - o[1]))
+    assert (d > TOL_FP32).sum() <= 2 and d.max() < 1.5e-4          # Q25: stop decision fp32 vs fp64
