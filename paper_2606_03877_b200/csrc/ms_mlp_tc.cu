@@ -336,8 +336,12 @@ __host__ __device__ constexpr int tc_a1_stages(int width) { return width > 64 ? 
 // 64 wide -- groups of 4 warps (a whole row of 64 columns each), group g serving the slots s % groups == g
 __host__ __device__ constexpr int tc_he_groups(int width, int nout) { return width > 64 ? 1 : (nout <= 16 ? 2 : 1); }
 __host__ __device__ constexpr int tc_he_warps(int, int) { return 8; }
+// a warp of its own for the head MMAs (and the weight loads): wide MLPs only.  For the 64- and 32-wide ones the
+// slot warps issue their heads and slot warp 0 loads the weights: 24 warps instead of 25, i.e. 80 registers
+// instead of 72 (ptxas budgets for the warp count rounded up to a multiple of four).
+__host__ __device__ constexpr int tc_head_warp(int width) { return width > 64 ? 1 : 0; }
 __host__ __device__ constexpr int tc_warps(int width, int nout) {
-  return tc_slots(width, nout) + 1 + 4 * tc_en_groups(width) + 4 + tc_he_warps(width, nout);
+  return tc_slots(width, nout) + tc_head_warp(width) + 4 * tc_en_groups(width) + 4 + tc_he_warps(width, nout);
 }
 // warps: one MMA warp per slot, head MMA warp (also weight loader and TMEM owner), EN groups, 4 HD, HE groups
 
@@ -350,7 +354,9 @@ __global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(c
   constexpr int NHS = NSLOT * HPS;
   constexpr int NEG = tc_en_groups(WIDTH), TC_NA1 = tc_a1_stages(WIDTH), NG = tc_he_groups(WIDTH, NOUT), HEW = tc_he_warps(WIDTH, NOUT) / NG;   // HE groups, warps per group
   static_assert(TC_NA1 % NEG == 0, "every ring stage belongs to one EN group");
-  constexpr int W_HM = NSLOT, W_EN = W_HM + 1, W_HD = W_EN + 4 * NEG, W_HE = W_HD + 4;   // first warp of each group
+  constexpr bool HEADW = tc_head_warp(WIDTH) != 0;
+  constexpr int W_HM = HEADW ? NSLOT : 0;          // head warp, or slot warp 0 in its place as loader / TMEM owner
+  constexpr int W_EN = NSLOT + (HEADW ? 1 : 0), W_HD = W_EN + 4 * NEG, W_HE = W_HD + 4;   // first warp of each group
   constexpr int SLOT_COLS = WIDTH + WIDTH / 2 + 8;
   constexpr int HEAD_COL0 = NSLOT * SLOT_COLS;
   static_assert(HEAD_COL0 + NHS * NOUT <= 512, "TMEM columns");
@@ -372,7 +378,7 @@ __global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(c
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   if (tid == 0) {
     mbar_init(bar_w_full, 1);
-    mbar_init(bar_w_free, NSLOT + 1);
+    mbar_init(bar_w_free, NSLOT + (HEADW ? 1 : 0));
     for (int i = 0; i < TC_NA1; ++i) { mbar_init(bar_a1_full + 8 * i, 4); mbar_init(bar_a1_free + 8 * i, 1); }
     for (int i = 0; i < NSLOT; ++i) { mbar_init(bar_d_full + 8 * i, 1); mbar_init(bar_a_ready + 8 * i, HEW); mbar_init(bar_a3_ready + 8 * i, HEW); }
     for (int i = 0; i < NHS; ++i) { mbar_init(bar_h_full + 8 * i, 1); mbar_init(bar_h_free + 8 * i, 4); }
@@ -412,14 +418,38 @@ __global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(c
     const uint32_t a1_base = smem_u32(s_a1);
     const uint32_t d_tmem = tmem + s * SLOT_COLS, a_tmem = d_tmem + WIDTH;
     const uint32_t bar_a_ready_s = bar_a_ready + 8 * s, bar_d_full_s = bar_d_full + 8 * s;
+    uint32_t cnt = 0;                  // !HEADW: heads this warp has issued (head region s*HPS + cnt%HPS, use cnt/HPS)
+    SegWalk wl(p.blk_off, p.n_prims, b0, b1);   // !HEADW, slot warp 0: the weight loader's walk, one segment ahead
+    if (!HEADW && s == 0) {
+      int lp; uint32_t lf, lc;
+      if (wl.next(lp, lf, lc) && lane == 0) {
+        mbar_expect_tx(bar_w_full, IMG_BYTES);
+        bulk_g2s(img, p.image + (size_t)lp * IMG_BYTES, IMG_BYTES, bar_w_full);
+      }
+      __syncwarp();
+    }
     while (w.next(prim, first, count)) {
       mbar_wait(bar_w_full, seg & 1);
       tc_fence_after();
       const uint32_t n_s = (count + NSLOT - 1 - s) / NSLOT;   // blocks of this segment that run in slot s
       for (uint32_t j = 0; j <= n_s; ++j) {
-        if (j > 0) {  // the previous block's last epilogue has read D (its head is the head warp's business)
+        if (j > 0) {  // the previous block's last epilogue has read D; its head: the head warp's business, or issued here
           mbar_wait(bar_a_ready_s, pa);
           pa ^= 1u;
+          if constexpr (!HEADW) {
+            constexpr uint32_t idesc_o = umma_idesc(NOUT);
+            const uint32_t hs = s * HPS + cnt % HPS;
+            mbar_wait(bar_h_free + 8 * hs, ((cnt / HPS) & 1u) ^ 1u);
+            ++cnt;
+            tc_fence_after();
+            const uint32_t h_tmem = tmem + HEAD_COL0 + hs * NOUT;
+#pragma unroll
+            for (int q = 0; q <= WIDTH / 16; ++q) {
+              const uint64_t db = umma_desc(img + tc_off_w(K1, WIDTH, NH) + q * 2 * (NOUT * 16), NOUT * 16, 128);
+              mma_ts(h_tmem, a_tmem + q * 8, db, idesc_o, q > 0);
+            }
+            mma_commit(bar_h_full + 8 * hs);
+          }
         }
         if (j == n_s) break;
         {  // layer 1 of the slot's next block: A from the A1 ring
@@ -450,11 +480,20 @@ __global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(c
         }
       }
       mma_commit(bar_w_free);  // arrives once every MMA this warp issued in the segment has read its weights
+      if (!HEADW && s == 0) {  // loader duty: the next primitive's image once every slot is done with this one
+        mbar_wait(bar_w_free, seg & 1);
+        int lp; uint32_t lf, lc;
+        if (wl.next(lp, lf, lc) && lane == 0) {
+          mbar_expect_tx(bar_w_full, IMG_BYTES);
+          bulk_g2s(img, p.image + (size_t)lp * IMG_BYTES, IMG_BYTES, bar_w_full);
+        }
+        __syncwarp();
+      }
       run0 += count;
       ++seg;
     }
     if (seg > 0) mbar_wait(bar_w_free, (seg - 1) & 1);  // no asynchronous arrive may outlive the CTA
-  } else if (warp == W_HM) {
+  } else if (HEADW && warp == W_HM) {
     // ===== head MMA issuer: the N = NOUT head MMAs are issue-bound (~25 cycles each for a few cycles
     // of tensor work); from a warp of their own they slip into the pipe between the slots' wide MMAs
     // It is also the weight loader: one bulk async copy of the next primitive's image once every
@@ -536,12 +575,12 @@ __global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(c
             pd ^= 1u << s;
             tc_fence_after();
             const uint32_t prev = cum[s] + j;       // blocks the slot has finished before this one
-            if constexpr (WIDTH > 64) {
+            if constexpr (WIDTH > 64 || !HEADW) {
               uint32_t r[HC];
 #pragma unroll
               for (int c0 = 0; c0 < HC; c0 += 32) tmem_ld32(d_tmem + c0, r + c0);
               tmem_ld_wait();
-              if (l == 0 && prev > 0) {             // A still feeds the previous block's head MMAs
+              if (HEADW && l == 0 && prev > 0) {    // A still feeds the previous block's head MMAs
                 mbar_wait(bar_h_full + 8 * (s * HPS + (prev - 1) % HPS), ((prev - 1) / HPS) & 1u);
                 tc_fence_after();
               }
@@ -561,7 +600,7 @@ __global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(c
                 tmem_ld_wait();
 #pragma unroll
                 for (int q = 0; q < 16; ++q) o[q] = relu_pack_bf16(__uint_as_float(r[2 * q]), __uint_as_float(r[2 * q + 1]));
-                if (c0 == 0 && l == 0 && prev > 0) {
+                if (HEADW && c0 == 0 && l == 0 && prev > 0) {
                   mbar_wait(bar_h_full + 8 * (s * HPS + (prev - 1) % HPS), ((prev - 1) / HPS) & 1u);
                   tc_fence_after();
                 }
@@ -573,7 +612,7 @@ __global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(c
             __syncwarp();
             if (lane == 0) {
               mbar_arrive(bar_a_ready + 8 * s);
-              if (l == NH - 1) mbar_arrive(bar_a3_ready + 8 * s);
+              if (HEADW && l == NH - 1) mbar_arrive(bar_a3_ready + 8 * s);
             }
           }
         }
