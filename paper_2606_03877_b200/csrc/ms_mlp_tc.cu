@@ -304,8 +304,9 @@ __device__ __forceinline__ void encode_contact_row(const float *z, uint8_t *dst_
 // kernel
 // ---------------------------------------------------------------------------------------------
 // Warp roles (one CTA per SM):
-//   warp NSLOT        head MMA issuer (N = NOUT MMAs of every block, in block order); also the weight
-//                     loader (one bulk copy per segment) and the TMEM owner
+//   warp NSLOT        (128-wide MLPs only) head MMA issuer (N = NOUT MMAs of every block, in block order);
+//                     also the weight loader (one bulk copy per segment) and the TMEM owner.  Narrower
+//                     MLPs: the slot warps issue their heads, slot warp 0 loads (24 warps -> 80 registers)
 //   warps 0..NSLOT-1  MMA issuers, one per slot: a converged warp, one elected lane issues (see mma_ss).
 //                     One warp per slot because the issue path is latency-bound: ~45 cycles per
 //                     tcgen05.mma (four R2UR each) and ~90 per mbarrier try_wait, 30 MMAs and 6 waits
