@@ -210,7 +210,9 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   // ---- (b) radix sort + tile ranges -------------------------------------------------------
   if (timing) CK(cudaEventRecord(sc->ev[1], st));
   uint64_t *sorted = nullptr;
-  CK(ms_radix_sort_u64((uint64_t *)sc->keys_a.p, (uint64_t *)sc->keys_b.p, P, prim_bits + 32 + tile_bits,
+  // stage (a) emits the keys primitive by primitive, i.e. already ordered by the id in their low prim_bits bits;
+  // the sort is stable, so only the (tile | depth) bits above them need passes
+  CK(ms_radix_sort_u64((uint64_t *)sc->keys_a.p, (uint64_t *)sc->keys_b.p, P, prim_bits, prim_bits + 32 + tile_bits,
                        (uint32_t *)sc->sort_scratch.p, &sorted, st));
   CK(ms_tile_ranges(sorted, P, n_tiles, prim_bits, (uint32_t *)sc->tile_start.p, st));
 

@@ -153,9 +153,9 @@ extern thread_local long long ms_launch_count;
 size_t ms_scan_scratch_elems(size_t n);
 cudaError_t ms_exclusive_scan_u32(const uint32_t *in, uint32_t *out, size_t n, uint32_t *scratch, cudaStream_t s);
 
-// ms_sort.cu: LSD radix sort of 64-bit keys on bits [0, n_bits). Result ends in *result (either a or b).
+// ms_sort.cu: stable LSD radix sort of 64-bit keys on bits [first_bit, n_bits). Result ends in *result (a or b).
 size_t ms_sort_scratch_elems(size_t n);
-cudaError_t ms_radix_sort_u64(uint64_t *a, uint64_t *b, size_t n, int n_bits, uint32_t *scratch,
+cudaError_t ms_radix_sort_u64(uint64_t *a, uint64_t *b, size_t n, int first_bit, int n_bits, uint32_t *scratch,
                               uint64_t **result, cudaStream_t s);
 
 // ms_bin.cu

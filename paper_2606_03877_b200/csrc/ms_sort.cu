@@ -83,8 +83,8 @@ size_t ms_sort_scratch_elems(size_t n) {
   return 2 * (m + 1) + ms_scan_scratch_elems(m) + 8;
 }
 
-cudaError_t ms_radix_sort_u64(uint64_t *a, uint64_t *b, size_t n, int n_bits, uint32_t *scratch, uint64_t **result,
-                              cudaStream_t s) {
+cudaError_t ms_radix_sort_u64(uint64_t *a, uint64_t *b, size_t n, int first_bit, int n_bits, uint32_t *scratch,
+                              uint64_t **result, cudaStream_t s) {
   *result = a;
   if (n <= 1 || n_bits <= 0) return cudaSuccess;
   size_t nb = (n + RS_TILE - 1) / RS_TILE;
@@ -93,7 +93,8 @@ cudaError_t ms_radix_sort_u64(uint64_t *a, uint64_t *b, size_t n, int n_bits, ui
   uint32_t *offsets = scratch + m + 1;
   uint32_t *scan_scratch = scratch + 2 * (m + 1);
   uint64_t *src = a, *dst = b;
-  for (int shift = 0; shift < n_bits; shift += 8) {
+  // LSD and stable: bits below first_bit need no pass when the input is already ordered by them
+  for (int shift = first_bit; shift < n_bits; shift += 8) {
     radix_hist_kernel<<<(unsigned)nb, RS_THREADS, 0, s>>>(src, n, shift, counts, (uint32_t)nb);
   MS_LAUNCHED();
     cudaError_t e = cudaGetLastError();
