@@ -31,8 +31,10 @@ __global__ void __launch_bounds__(RS_THREADS) radix_hist_kernel(const uint64_t *
 __global__ void __launch_bounds__(RS_THREADS) radix_scatter_kernel(const uint64_t *__restrict__ keys,
                                                                    uint64_t *__restrict__ out, size_t n, int shift,
                                                                    const uint32_t *__restrict__ offsets,
+                                                                   const uint32_t *__restrict__ counts,
                                                                    uint32_t n_blocks) {
   __shared__ uint32_t wc[RS_WARPS][256];
+  __shared__ uint32_t wsum[RS_WARPS];
   for (int i = threadIdx.x; i < RS_WARPS * 256; i += RS_THREADS) (&wc[0][0])[i] = 0;
   __syncthreads();
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -55,7 +57,31 @@ __global__ void __launch_bounds__(RS_THREADS) radix_scatter_kernel(const uint64_
   }
   __syncthreads();
   {  // thread t owns digit t: exclusive prefix over warps + global offset of (digit, block)
-    uint32_t run = offsets[(size_t)threadIdx.x * n_blocks + blockIdx.x];
+    uint32_t run;
+    if (offsets) {
+      run = offsets[(size_t)threadIdx.x * n_blocks + blockIdx.x];
+    } else {
+      // few blocks (the usual case: <= 0.5 M keys): the (digit, block) offset straight from the count matrix --
+      // digits below mine over all blocks, plus my digit in the blocks before this one -- no scan launches
+      const uint32_t *row = counts + (size_t)threadIdx.x * n_blocks;
+      uint32_t total = 0, before = 0;
+      for (uint32_t b = 0; b < n_blocks; ++b) {
+        const uint32_t c = row[b];
+        before += b < blockIdx.x ? c : 0u;
+        total += c;
+      }
+      uint32_t incl = total;   // inclusive scan of the digit totals over the 256 threads
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += v;
+      }
+      if (lane == 31) wsum[warp] = incl;
+      __syncthreads();
+      uint32_t wbase = 0;
+      for (int w = 0; w < warp; ++w) wbase += wsum[w];
+      run = wbase + incl - total + before;
+    }
 #pragma unroll
     for (int w = 0; w < RS_WARPS; ++w) {
       uint32_t c = wc[w][threadIdx.x];
@@ -99,9 +125,13 @@ cudaError_t ms_radix_sort_u64(uint64_t *a, uint64_t *b, size_t n, int first_bit,
   MS_LAUNCHED();
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    e = ms_exclusive_scan_u32(counts, offsets, m, scan_scratch, s);
-    if (e != cudaSuccess) return e;
-    radix_scatter_kernel<<<(unsigned)nb, RS_THREADS, 0, s>>>(src, dst, n, shift, offsets, (uint32_t)nb);
+    const bool self_scan = nb <= 256;   // the scatter kernel derives its offsets from the count matrix itself
+    if (!self_scan) {
+      e = ms_exclusive_scan_u32(counts, offsets, m, scan_scratch, s);
+      if (e != cudaSuccess) return e;
+    }
+    radix_scatter_kernel<<<(unsigned)nb, RS_THREADS, 0, s>>>(src, dst, n, shift, self_scan ? nullptr : offsets, counts,
+                                                             (uint32_t)nb);
   MS_LAUNCHED();
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
