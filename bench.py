@@ -190,6 +190,7 @@ def run_ours(args, cfg):
     cams = synth.make_cameras(cfg)
     H, W, K, V = cfg.height, cfg.width, cfg.K, cfg.n_views
     gs = api.Scene(sc)
+    gs.band_bytes, gs.waves = args.band_bytes, args.waves
     stream = torch.cuda.Stream()
     out = None
     with torch.cuda.stream(stream):
@@ -260,7 +261,9 @@ def run_ours(args, cfg):
                    "order": "tile-centre shared order (P:109)" if args.tile_order else "exact per-ray order"},
         "samples_per_s": world * n_samples_view * V / (ms_step * 1e-3),
         "counts_per_view": {"pairs": st.n_pairs, "intervals": st.n_intervals, "samples": st.n_samples,
-                            "row_blocks": st.n_blocks, "scratch_GB": st.scratch_bytes / 1e9},
+                            "row_blocks": st.n_blocks, "scratch_GB": st.scratch_bytes / 1e9,
+                            "samples_evaluated": st.n_samples_evaluated, "bands": st.n_bands, "waves": st.n_waves,
+                            "staging_MB": st.staging_bytes / 1e6},
         "stage_ms_per_view": {k: v / max(1, n_views_timed) for k, v in stage_sum.items()},
         "clocks": clocks,
         "e2e": {"value": world * px_step / (e2e_ms * 1e-3) / 1e6, "unit": UNIT,
@@ -311,6 +314,9 @@ def main():
     ap.add_argument("--tile-order", action="store_true",
                     help="contact-mode configs: the paper's shared per-tile order (P:109) instead of the exact per-ray order")
     ap.add_argument("--tile", type=int, default=0, help="tile edge override (8, 16, 32)")
+    ap.add_argument("--band-bytes", type=int, default=0,
+                    help="staging budget per band in bytes (ms_opts.band_bytes): 0 = library default, -1 = one band")
+    ap.add_argument("--waves", type=int, default=0, help="depth waves (ms_opts.waves): 0 = auto, -1 = off, C > 0 = wave size")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                                  # timing rule: W >= 3

@@ -72,7 +72,7 @@ enum { MS_MODE_LOCAL = 0, MS_MODE_CONTACT = 1 };
  * (d_x,d_y,d_z,delta_x,delta_y,delta_z) and level l, x[2L j + 2l] = sin(2^l pi z_j),
  * x[2L j + 2l + 1] = cos(2^l pi z_j); in_dim = 12 L, no identity, use_viewdir must be 0.
  * alpha = (1 - exp(-sigma l)) g with l = the chord length of the ray inside the support and
- * g = exp(-(9/2) |p* - mu|^2_Lambda) (readings of P:105); hits are
+ * g = exp(-falloff |p* - mu|^2_Lambda), falloff = 9/2 by default (readings of P:105); hits are
  * composited in the order of (t*, primitive id).  ms_opts.K must be 1.  Paths: fp32 for any shape;
  * the tensor path for dtype = MS_BF16 with the paper's shape (L = 6, width 32, two hidden layers, n_feat 0). */
 typedef struct {
@@ -85,7 +85,11 @@ typedef struct {
   const float *weights;
   size_t n_weights;    /* must equal n * P */
   int32_t mode;        /* MS_MODE_LOCAL | MS_MODE_CONTACT */
+  float falloff;       /* MS_MODE_CONTACT: g = exp(-falloff |p* - mu|^2_Lambda), the reading of the "Gaussian falloff"
+                          whose formula the paper omits (Q29).  MS_FALLOFF_DEFAULT = 9/2 puts the
+                          support boundary |.|_Lambda = 1 at three standard deviations; 0 = no falloff; must be >= 0 */
 } ms_mlp;
+#define MS_FALLOFF_DEFAULT 4.5f
 
 /* Pinhole camera (Q14): pixel (x,y), row 0 on top, looks along
  * d_cam = ((x+0.5-cx)/fx, (y+0.5-cy)/fy, 1); c2w = 3x4 row-major [R|t], camera axes
@@ -98,12 +102,14 @@ typedef struct {
 
 enum { MS_PATH_AUTO = 0, MS_PATH_FP32 = 1, MS_PATH_BF16_TC = 2 };
 enum {
-  MS_FLAG_KEEP_DEBUG = 1, /* keep the intermediate buffers of the last view for ms_debug_* */
+  MS_FLAG_KEEP_DEBUG = 1, /* keep the intermediate buffers of the last view for ms_debug_* (tile lists, intervals) */
   MS_FLAG_STAGE_TIMES = 2, /* record CUDA events between stages (ms_last_stage_ms) */
-  MS_FLAG_TILE_ORDER = 4   /* MS_MODE_CONTACT only: composite every pixel of a tile in ONE shared order, that of the
+  MS_FLAG_TILE_ORDER = 4,  /* MS_MODE_CONTACT only: composite every pixel of a tile in ONE shared order, that of the
                               contact points t*_{i,c} of the virtual ray through the tile centre (the
                               paper's approximation), instead of the exact per-ray order; the tile lists are
                               then sorted by (tile, t*_{i,c}, primitive id) */
+  MS_FLAG_KEEP_ORDER = 8   /* stage (e) also records the order it composited every ray's samples in (4 B per sample)
+                              for ms_debug_sample_order*: the order the product really used, not a re-derivation */
 };
 
 typedef struct {
@@ -113,7 +119,23 @@ typedef struct {
   int32_t path;   /* MS_PATH_*; AUTO = BF16_TC when dtype is MS_BF16 and the shape is covered, else FP32 */
   void *stream;   /* cudaStream_t to enqueue on; NULL = the legacy default stream */
   int32_t flags;  /* MS_FLAG_* */
+  int64_t band_bytes; /* Banded rendering (DESIGN.md Sec.6 "Bands and waves"; P:437 tile-local processing): the frame is
+                     cut into bands of neighbouring tiles whose staged samples ((r,g,b,e) + features per sample) fill
+                     about this many bytes, and stages (d), (e) run band by band on ONE staging buffer of that size,
+                     which then lives in the L2 cache instead of HBM.  0 = MS_BAND_BYTES_DEFAULT; < 0 = one band
+                     (staging of the whole frame).  The image does not depend on it. */
+  int32_t waves;  /* Depth waves = early termination that skips MLP work ("early t[ermination]"): > 0 = a tile's
+                     sorted list is evaluated in waves of `waves`, `waves`, 2x, 4x ... entries, and before each
+                     wave the rays that have already stopped (T < t_stop/2 over the samples in front of the wave) drop
+                     their later intervals.  0 = MS_WAVES_AUTO: on when the previous view rendered on this scene
+                     had rays stopping early, else off; < 0 = off.  The image does not depend on it. */
+  float eye_guard; /* Q13: a support whose near depth z_lo <= eye_guard * r_z (it touches or nearly touches the eye
+                     plane) is binned to the whole image instead of through the dual-conic bound, which degenerates
+                     there.  <= 0 = MS_EYE_GUARD_DEFAULT (0.01). */
 } ms_opts;
+#define MS_BAND_BYTES_DEFAULT ((int64_t)48 << 20)
+#define MS_WAVES_AUTO 0
+#define MS_EYE_GUARD_DEFAULT 0.01f
 
 typedef struct {
   int64_t n_visible;   /* primitives with a non-empty screen AABB */
@@ -123,6 +145,12 @@ typedef struct {
   int64_t n_blocks;    /* 128-sample row blocks fed to the MLP stage */
   int64_t scratch_bytes;
   int64_t n_launches;  /* kernels launched for this view (all stages) */
+  int64_t n_samples_evaluated; /* samples whose MLP really ran: n_samples minus those of intervals dropped by the
+                                  depth waves (rays already stopped) */
+  int64_t n_dead_rays; /* rays the depth waves found stopped before their last hit */
+  int64_t n_bands;     /* bands the frame was cut into */
+  int64_t n_waves;     /* depth waves per band (1 = off) */
+  int64_t staging_bytes; /* size of the staging buffers of stages (d) -> (e) */
 } ms_stats;
 
 enum { MS_STAGE_BIN = 0, MS_STAGE_SORT, MS_STAGE_ISECT, MS_STAGE_MLP, MS_STAGE_COMPOSITE, MS_N_STAGES };
@@ -158,7 +186,7 @@ int ms_render_batch(ms_scene *scene, const ms_camera *cameras, int32_t n_views, 
 int ms_render_host(ms_scene *scene, const ms_camera *cameras, int32_t n_views, int32_t H, int32_t W,
                    const ms_opts *opts, float *host_rgb, float *host_alpha, float *host_feat);
 
-/* Counts of the last view rendered on this scene (valid once the stream is idle). */
+/* Counts of the last view rendered on this scene.  Waits for that view to finish (its device counters). */
 int ms_last_stats(ms_scene *scene, ms_stats *out);
 /* Device time of each stage of the last view rendered with MS_FLAG_STAGE_TIMES, in ms,
  * ms[MS_N_STAGES].  Synchronises the recorded events. */
@@ -177,9 +205,13 @@ int ms_debug_tile_lists(ms_scene *scene, int64_t *tile_offsets, int32_t *prim_id
 /* Per-ray hit lists in tile-list order: hit_offsets host [H*W+1]; prim / t_in / delta host [cap]. */
 int ms_debug_intervals(ms_scene *scene, int64_t *hit_offsets, int32_t *prim, float *t_in, float *delta,
                        size_t cap, size_t *n);
-/* Compositing order of one ray (all samples, not truncated): prim / k / t host [cap]. */
+/* Compositing order of one ray (pixel index y*W + x; all samples, not truncated) as stage (e) recorded it while
+ * compositing (MS_FLAG_KEEP_DEBUG | MS_FLAG_KEEP_ORDER): prim / k / t host [cap]. */
 int ms_debug_sample_order(ms_scene *scene, int32_t ray, int32_t *prim, int32_t *k, float *t,
                           size_t cap, size_t *n);
+/* The same for every ray: prim / k host [cap] with cap >= n_samples; ray y*W + x owns the entries
+ * [hit_offsets[ray] * K, hit_offsets[ray + 1] * K) (ms_debug_intervals), in compositing order. */
+int ms_debug_sample_order_all(ms_scene *scene, int32_t *prim, int32_t *k, size_t cap, size_t *n);
 /* Derived per-primitive frames, host [n][9] each (row-major A, M). */
 int ms_debug_prim_frames(ms_scene *scene, float *A, float *M);
 

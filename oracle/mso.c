@@ -27,6 +27,8 @@ struct mso_scene {
   int32_t n_freq, use_viewdir, n_hidden, width, n_feat, mode;
   int32_t c_f;           /* Eq.7 slot embeddings: width (0 = none) */
   int32_t order;         /* MSO_ORDER_EXACT | MSO_ORDER_TILE (contact mode, binned only) */
+  float falloff;         /* contact mode: g = exp(-falloff r2)  (reading Q29; MSO_FALLOFF_DEFAULT = 9/2) */
+  float eye_guard;       /* Q13: z_lo <= eye_guard * r_z -> whole image (MSO_EYE_GUARD_DEFAULT = 0.01) */
   float *slots;          /* [n][4][c_f] */
   int32_t in_dim, out_dim, n_layers, params;
   float *center;  /* [n][3] */
@@ -66,9 +68,12 @@ int mso_scene_create(const mso_prims *p, const mso_mlp *m, mso_scene **out) {
   if (m->n_freq < 0 || m->n_hidden < 1 || m->width < 1 || m->n_feat < 0) return MSO_ERR_ARG;
   if (m->mode != MSO_MODE_LOCAL && m->mode != MSO_MODE_CONTACT) return MSO_ERR_ARG;
   if (m->mode == MSO_MODE_CONTACT && (m->n_freq < 1 || m->use_viewdir)) return MSO_ERR_ARG;
+  if (m->mode == MSO_MODE_CONTACT && !(m->falloff >= 0.0f)) return MSO_ERR_ARG;
   mso_scene *s = (mso_scene *)calloc(1, sizeof(*s));
   if (!s) return MSO_ERR_MEM;
   s->n = p->n;
+  s->falloff = m->falloff;
+  s->eye_guard = MSO_EYE_GUARD_DEFAULT;
   s->n_freq = m->n_freq; s->use_viewdir = m->use_viewdir ? 1 : 0;
   s->n_hidden = m->n_hidden; s->width = m->width; s->n_feat = m->n_feat;
   s->mode = m->mode;
@@ -105,6 +110,12 @@ int mso_scene_create(const mso_prims *p, const mso_mlp *m, mso_scene **out) {
       }
   }
   *out = s;
+  return MSO_OK;
+}
+
+int mso_scene_set_eye_guard(mso_scene *s, float eye_guard) {
+  if (!s || !(eye_guard > 0.0f)) return MSO_ERR_ARG;
+  s->eye_guard = eye_guard;
   return MSO_OK;
 }
 
@@ -243,7 +254,7 @@ static proj_t project(const mso_scene *s, const mso_camera *cam, int H, int W, i
   float z_hi = czv + rz;
   if (!(z_hi > 0.0f)) return r;                       /* entirely behind the eye plane */
   r.z_entry = z_lo > 0.0f ? z_lo : 0.0f;
-  if (z_lo <= 0.01f * rz) {                           /* touches / nears the eye plane: whole image (Q13) */
+  if (z_lo <= s->eye_guard * rz) {                    /* touches / nears the eye plane: whole image (Q13) */
     r.visible = 1; r.px0 = 0; r.px1 = W - 1; r.py0 = 0; r.py1 = H - 1;
     return r;
   }
@@ -648,8 +659,8 @@ int mso_render(const mso_scene *s, const mso_camera *cam, int H, int W, const ms
           encode_contact(s, sp->prim, o, d, sp->t, x, &r2, dlt);
           mlp_forward(s, sp->prim, x, raw);
           activate(s, raw, act);
-          /* alpha = (1 - exp(-sigma l)) g,  g = exp(-(9/2) r2)   (readings: mso.h header) */
-          e = 1.0 - (1.0 - exp(-act[3] * (double)rb.hits[sp->hit].delta)) * exp(-4.5 * r2);
+          /* alpha = (1 - exp(-sigma l)) g,  g = exp(-falloff r2), falloff = 9/2 by default (readings: mso.h header) */
+          e = 1.0 - (1.0 - exp(-act[3] * (double)rb.hits[sp->hit].delta)) * exp(-(double)s->falloff * r2);
         } else {
           float u[3];
           sample_u(s, sp->prim, o, d, sp->t, u);
@@ -771,6 +782,37 @@ int mso_ray_samples(const mso_scene *s, const mso_camera *cam, int H, int W, con
   }
   raybuf_free(&rb);
   return MSO_OK;
+}
+
+/* (primitive, k) of every sample of every pixel in compositing order; pixel q owns [K offsets[q], K offsets[q+1])
+ * of mso_intervals_all's offsets.  The same gather_hits + build_samples the renderer runs. */
+int mso_samples_all(const mso_scene *s, const mso_camera *cam, int H, int W, const mso_opts *opt,
+                    int32_t *prim, int32_t *k, size_t cap, size_t *n) {
+  if (!s || !cam || !opt || opt->K <= 0) return MSO_ERR_ARG;
+  tlists_t tl; memset(&tl, 0, sizeof(tl));
+  if (opt->tile > 0) { int rc = tlists_build(s, cam, H, W, opt->tile, &tl); if (rc) return rc; }
+  const tlists_t *tlp = opt->tile > 0 ? &tl : NULL;
+  raybuf_t rb; memset(&rb, 0, sizeof(rb));
+  size_t tot = 0;
+  int rc = MSO_OK;
+  for (int64_t q = 0; q < (int64_t)H * W; ++q) {
+    float o[3], d[3];
+    long nh = gather_hits(s, cam, tlp, opt->tile, W, (int)q, opt->K, o, d, &rb);
+    if (nh < 0) { rc = MSO_ERR_MEM; break; }
+    long ns = build_samples(s, nh, opt->K, &rb);
+    if (ns < 0) { rc = MSO_ERR_MEM; break; }
+    for (long j = 0; j < ns; ++j, ++tot) {
+      if (tot < cap) {
+        if (prim) prim[tot] = rb.samps[j].prim;
+        if (k) k[tot] = rb.samps[j].k;
+      }
+    }
+  }
+  if (n) *n = tot;
+  raybuf_free(&rb);
+  tlists_free(&tl);
+  if (rc == MSO_OK && tot > cap) rc = MSO_ERR_CAP;
+  return rc;
 }
 
 /* Intervals of every pixel (each ray's list sorted by primitive id): offsets[H*W+1]. */

@@ -29,9 +29,9 @@
  *   (d_x,d_y,d_z,delta_x,delta_y,delta_z), per level l: sin(2^l pi z_j), cos(2^l pi z_j)
  *   -> 12 L dims, no identity                                                P:89-103 Eq.3-5
  *   alpha = (1 - exp(-sigma l)) g, l = chord length of the ray in the support (reading of the
- *   undefined "effective integration length"), g = exp(-(9/2) |p*-mu|^2_Lambda)
- *   (reading of the "Gaussian falloff" whose formula the paper omits: the support
- *   boundary |.|_Lambda = 1 sits at three standard deviations); samples ordered by (t*, primitive id).
+ *   undefined "effective integration length"), g = exp(-falloff |p*-mu|^2_Lambda), falloff = 9/2
+ *   by default (reading of the "Gaussian falloff" whose formula the paper omits: the support
+ *   boundary |.|_Lambda = 1 then sits at three standard deviations); samples ordered by (t*, primitive id).
  *   Both readings are listed in DESIGN.md Sec.11.
  *   Slot features (mso_scene_set_slots; S:Sec.8(f) NEXT-2; Eq.7): u = clip_[-1,1]^3(R^T delta / s),
  *   g_k = softmax_k(a_k^T u) over the canonical tetrahedral frame a_k = (1,1,1), (1,-1,-1), (-1,1,-1),
@@ -74,7 +74,11 @@ typedef struct {
   int32_t n_feat;        /* linear channels after [r,g,b,sigma] */
   const float *weights;  /* [n][params]: per layer W[in][out] row-major, then b[out]   */
   int32_t mode;          /* MSO_MODE_LOCAL (0) | MSO_MODE_CONTACT (1)                  */
+  float falloff;         /* contact mode: g = exp(-falloff |p*-mu|^2_Lambda), >= 0; the reading of P:105's
+                            "Gaussian falloff" (Q29): MSO_FALLOFF_DEFAULT = 9/2               */
 } mso_mlp;
+#define MSO_FALLOFF_DEFAULT 4.5f
+#define MSO_EYE_GUARD_DEFAULT 0.01f
 
 enum { MSO_MODE_LOCAL = 0, MSO_MODE_CONTACT = 1 };
 enum { MSO_ORDER_EXACT = 0, MSO_ORDER_TILE = 1 };
@@ -110,6 +114,9 @@ int  mso_scene_create(const mso_prims *, const mso_mlp *, mso_scene **out);
  * approximation (about 2x faster, -0.35 dB there).  Binned mode only; the tile lists are then sorted by
  * (tile, t*_{i,c}, primitive id).  Default MSO_ORDER_EXACT: per-ray order by (t*, primitive id). */
 int  mso_scene_set_order(mso_scene *, int32_t order);
+/* Q13: a support with z_lo <= eye_guard * r_z (touching or nearly touching the eye plane) is binned to the whole
+ * image; default MSO_EYE_GUARD_DEFAULT = 0.01.  Must be > 0. */
+int  mso_scene_set_eye_guard(mso_scene *, float eye_guard);
 /* contact mode, n_feat == 0: attach slot embeddings emb[n][4][c_f] (copied); mso_render then writes feat[n_pix][c_f] */
 int  mso_scene_set_slots(mso_scene *, int32_t c_f, const float *emb);
 /* gates g[4] of primitive prim for the residual delta = mu - p* (world frame) */
@@ -150,6 +157,11 @@ int mso_intervals_all(const mso_scene *, const mso_camera *, int H, int W, const
 int mso_ray_samples(const mso_scene *, const mso_camera *, int H, int W, const mso_opts *,
                     int32_t pixel, int32_t *prim, int32_t *k, float *t,
                     size_t cap, size_t *n);
+
+/* (primitive, k) of every sample of every pixel in compositing order (not truncated); pixel q owns the entries
+ * [K offsets[q], K offsets[q+1]) of mso_intervals_all's offsets.  cap = 0 to size (*n). */
+int mso_samples_all(const mso_scene *, const mso_camera *, int H, int W, const mso_opts *,
+                    int32_t *prim, int32_t *k, size_t cap, size_t *n);
 
 /* ---- pieces exposed so tests can pin them one by one ---- */
 

@@ -20,7 +20,8 @@ class _Prims(C.Structure):
 
 class _MLP(C.Structure):
     _fields_ = [("n_freq", C.c_int32), ("use_viewdir", C.c_int32), ("n_hidden", C.c_int32),
-                ("width", C.c_int32), ("n_feat", C.c_int32), ("weights", C.c_void_p), ("mode", C.c_int32)]
+                ("width", C.c_int32), ("n_feat", C.c_int32), ("weights", C.c_void_p), ("mode", C.c_int32),
+                ("falloff", C.c_float)]
 
 
 class _Camera(C.Structure):
@@ -84,7 +85,8 @@ class OracleScene:
         self.n = int(self._keep[0].shape[0])
         p = _Prims(self.n, _ptr(self._keep[0]), _ptr(self._keep[1]), _ptr(self._keep[2]))
         m = _MLP(scene.mlp.n_freq, scene.mlp.use_viewdir, scene.mlp.n_hidden, scene.mlp.width,
-                 scene.mlp.n_feat, _ptr(self._keep[3]), int(getattr(scene.mlp, "mode", 0)))
+                 scene.mlp.n_feat, _ptr(self._keep[3]), int(getattr(scene.mlp, "mode", 0)),
+                 float(getattr(scene.mlp, "falloff", 4.5)))
         h = C.c_void_p()
         rc = lib().mso_scene_create(C.byref(p), C.byref(m), C.byref(h))
         if rc != 0:
@@ -191,6 +193,27 @@ class OracleScene:
         if rc != 0:
             raise RuntimeError(f"mso_intervals_all failed: {rc}")
         return off, prim[:n.value], t_in[:n.value], delta[:n.value]
+
+    def samples_all(self, cam, H, W, K, tile=16):
+        """(prim, k) of every sample of every pixel in compositing order (aligned with intervals_all's offsets * K)."""
+        n = C.c_size_t(0)
+        o = _Opts(K, 1e-4, tile, 1)
+        c = _cam(cam)
+        rc = lib().mso_samples_all(self._h, C.byref(c), H, W, C.byref(o), None, None, C.c_size_t(0), C.byref(n))
+        if rc not in (0, -3):
+            raise RuntimeError(f"mso_samples_all failed: {rc}")
+        prim = np.zeros(max(n.value, 1), np.int32)
+        k = np.zeros(max(n.value, 1), np.int32)
+        rc = lib().mso_samples_all(self._h, C.byref(c), H, W, C.byref(o), _ptr(prim), _ptr(k),
+                                   C.c_size_t(prim.size), C.byref(n))
+        if rc != 0:
+            raise RuntimeError(f"mso_samples_all failed: {rc}")
+        return prim[:n.value], k[:n.value]
+
+    def set_eye_guard(self, g: float):
+        rc = lib().mso_scene_set_eye_guard(self._h, C.c_float(g))
+        if rc != 0:
+            raise ValueError(f"mso_scene_set_eye_guard failed: {rc}")
 
     def ray_samples(self, cam, H, W, K, pixel, tile=16):
         cap = self.n * K

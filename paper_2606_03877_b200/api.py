@@ -18,12 +18,14 @@ _LIB_PATH = os.path.join(_HERE, "libmlpsplat.so")
 MS_F32, MS_BF16 = 0, 1
 PATH_AUTO, PATH_FP32, PATH_BF16_TC = 0, 1, 2
 FLAG_KEEP_DEBUG, FLAG_STAGE_TIMES = 1, 2
+FLAG_KEEP_ORDER = 8     # stage (e) records the order it composited in (ms_debug_sample_order*)
+FLAG_DEBUG_ALL = FLAG_KEEP_DEBUG | FLAG_KEEP_ORDER
 FLAG_TILE_ORDER = 4     # contact mode: the paper's shared per-tile order instead of the exact per-ray order
 STAGES = ("bin", "sort", "isect", "mlp", "composite")
 
 EXPORTS = ["ms_scene_create", "ms_scene_set_slots", "ms_scene_destroy", "ms_render", "ms_render_batch", "ms_render_host",
            "ms_last_stats", "ms_last_stage_ms", "ms_stage_accum", "ms_debug_tile_lists", "ms_debug_intervals",
-           "ms_debug_sample_order", "ms_debug_prim_frames", "ms_error_string", "ms_last_cuda_error"]
+           "ms_debug_sample_order", "ms_debug_sample_order_all", "ms_debug_prim_frames", "ms_error_string", "ms_last_cuda_error"]
 
 
 class _Prims(C.Structure):
@@ -33,7 +35,7 @@ class _Prims(C.Structure):
 class _MLP(C.Structure):
     _fields_ = [("n_freq", C.c_int32), ("use_viewdir", C.c_int32), ("n_hidden", C.c_int32),
                 ("width", C.c_int32), ("n_feat", C.c_int32), ("dtype", C.c_int32),
-                ("weights", C.c_void_p), ("n_weights", C.c_size_t), ("mode", C.c_int32)]
+                ("weights", C.c_void_p), ("n_weights", C.c_size_t), ("mode", C.c_int32), ("falloff", C.c_float)]
 
 
 class _Camera(C.Structure):
@@ -43,13 +45,15 @@ class _Camera(C.Structure):
 
 class _Opts(C.Structure):
     _fields_ = [("K", C.c_int32), ("t_stop", C.c_float), ("tile", C.c_int32), ("path", C.c_int32),
-                ("stream", C.c_void_p), ("flags", C.c_int32)]
+                ("stream", C.c_void_p), ("flags", C.c_int32), ("band_bytes", C.c_int64), ("waves", C.c_int32),
+                ("eye_guard", C.c_float)]
 
 
 class _Stats(C.Structure):
     _fields_ = [("n_visible", C.c_int64), ("n_pairs", C.c_int64), ("n_intervals", C.c_int64),
                 ("n_samples", C.c_int64), ("n_blocks", C.c_int64), ("scratch_bytes", C.c_int64),
-                ("n_launches", C.c_int64)]
+                ("n_launches", C.c_int64), ("n_samples_evaluated", C.c_int64), ("n_dead_rays", C.c_int64),
+                ("n_bands", C.c_int64), ("n_waves", C.c_int64), ("staging_bytes", C.c_int64)]
 
 
 def _load() -> C.CDLL:
@@ -98,6 +102,12 @@ class Stats:
     n_blocks: int
     scratch_bytes: int
     n_launches: int
+    n_visible: int = 0
+    n_samples_evaluated: int = 0
+    n_dead_rays: int = 0
+    n_bands: int = 1
+    n_waves: int = 1
+    staging_bytes: int = 0
 
 
 class Scene:
@@ -120,7 +130,8 @@ class Scene:
         self.dtype = dtype
         p = _Prims(self.n, _ptr(center), _ptr(quat), _ptr(scale))
         m = _MLP(scene.mlp.n_freq, scene.mlp.use_viewdir, scene.mlp.n_hidden, scene.mlp.width,
-                 scene.mlp.n_feat, dtype, _ptr(weights), weights.size, int(getattr(scene.mlp, "mode", 0)))
+                 scene.mlp.n_feat, dtype, _ptr(weights), weights.size, int(getattr(scene.mlp, "mode", 0)),
+                 float(getattr(scene.mlp, "falloff", 4.5)))
         h = C.c_void_p()
         rc = _lib.ms_scene_create(C.byref(p), C.byref(m), C.byref(h))
         if rc != 0:
@@ -153,10 +164,16 @@ class Scene:
         if rc != 0:
             raise MsError(rc, where, _lib.ms_last_cuda_error(self._h))
 
+    # band_bytes / waves / eye_guard of every render of this scene (ms_opts; 0 = the library's defaults)
+    band_bytes: int = 0
+    waves: int = 0
+    eye_guard: float = 0.0
+
     def _opts(self, K, t_stop, tile, path, flags, stream=None) -> _Opts:
         if stream is None:
             stream = torch.cuda.current_stream().cuda_stream
-        return _Opts(K, t_stop, tile, path, C.c_void_p(stream), flags)
+        return _Opts(K, t_stop, tile, path, C.c_void_p(stream), flags, int(self.band_bytes), int(self.waves),
+                     float(self.eye_guard))
 
     # -- rendering ---------------------------------------------------------------
     def render(self, cam, H, W, K, *, t_stop=1e-4, tile=16, path=PATH_AUTO, flags=0, out=None,
@@ -214,7 +231,8 @@ class Scene:
     def stats(self) -> Stats:
         st = _Stats()
         self._check(_lib.ms_last_stats(self._h, C.byref(st)), "ms_last_stats")
-        return Stats(st.n_pairs, st.n_intervals, st.n_samples, st.n_blocks, st.scratch_bytes, st.n_launches)
+        return Stats(st.n_pairs, st.n_intervals, st.n_samples, st.n_blocks, st.scratch_bytes, st.n_launches,
+                     st.n_visible, st.n_samples_evaluated, st.n_dead_rays, st.n_bands, st.n_waves, st.staging_bytes)
 
     def stage_ms(self) -> dict[str, float]:
         ms = (C.c_float * len(STAGES))()
@@ -267,6 +285,18 @@ class Scene:
                                                C.c_size_t(prim.size), C.byref(n)),
                     "ms_debug_sample_order")
         return prim[:n.value], k[:n.value], t[:n.value]
+
+    def debug_sample_order_all(self):
+        """(prim, k) of every sample in the order stage (e) composited it, rays in pixel order (FLAG_KEEP_ORDER)."""
+        n = C.c_size_t(0)
+        rc = _lib.ms_debug_sample_order_all(self._h, None, None, C.c_size_t(0), C.byref(n))
+        if rc not in (0, -5):
+            self._check(rc, "ms_debug_sample_order_all")
+        prim = np.zeros(max(n.value, 1), np.int32)
+        k = np.zeros(max(n.value, 1), np.int32)
+        self._check(_lib.ms_debug_sample_order_all(self._h, _ptr(prim), _ptr(k), C.c_size_t(prim.size), C.byref(n)),
+                    "ms_debug_sample_order_all")
+        return prim[:n.value], k[:n.value]
 
     def debug_prim_frames(self):
         A = np.zeros((self.n, 3, 3), np.float32)

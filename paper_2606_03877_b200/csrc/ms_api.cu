@@ -25,8 +25,10 @@ struct Buf {
 struct ms_scene {
   int device = 0;
   int n = 0;
+  int n_sm = 0;
   int dtype = MS_F32;
   MsMlpShape shape{};
+  float falloff = MS_FALLOFF_DEFAULT;
   int last_cuda = 0;
   // scene-lifetime device data
   float *center = nullptr, *quat = nullptr, *scale = nullptr, *A = nullptr, *M = nullptr;
@@ -35,22 +37,28 @@ struct ms_scene {
   int slot_cf = 0;           // Eq.7 slot embeddings: width C_f (0 = none)
   float *slots = nullptr;    // device [N][4][slot_cf]
   // per-view scratch
-  Buf tile_count, emit_off, rect, z_entry, oprime, keys_a, keys_b, sort_scratch, tile_start, pair_hits, pair_off,
-      ray_hits, ray_off, scan_scratch, prim_start, prim_blocks, blk_off, intervals, hits, staging, staging_feat, staging_gate, staging_coef,
-      host_rgb, host_alpha, host_feat, dbg;
-  uint32_t *pinned = nullptr;  // [4] host-pinned readback
-  cudaEvent_t ev[MS_N_STAGES + 1] = {};
+  Buf tile_count, emit_off, rect, z_entry, oprime, keys_a, keys_b, sort_scratch, tile_start, pair_hits_i, pair_hits_j,
+      pair_off, slot_of, key2_a, key2_b, flags, gid, grp_key, grp_prim, grp_iv0, grp_blocks, blk_off, grp_cnt_c,
+      grp_blocks_c, blk_off_c, bw, bands, counters, alive, ray_hits, ray_off, scan_scratch, intervals, hits, staging,
+      staging_feat, staging_gate, staging_coef, dbg_ord, host_rgb, host_alpha, host_feat;
+  uint32_t *pinned = nullptr;  // host-pinned readback: [0] P, [1..] device counters
+  std::vector<cudaEvent_t> ev;     // MS_FLAG_STAGE_TIMES: 4 + 2 per band + 1 events of the last view
+  int ev_bands = 0;
   bool ev_valid = false;
   bool ev_pending = false;         // events of the last view not yet added to stage_sum
+  float last_stage_ms[MS_N_STAGES] = {};
   double stage_sum[MS_N_STAGES] = {};
   int64_t stage_views = 0;
+  cudaEvent_t frame_done = nullptr;  // recorded after the counters' readback copy of the last view
+  bool frame_pending = false;
+  bool prev_terminated = false;      // MS_WAVES_AUTO: the previous view had rays stopping early
   // last view
   ms_stats stats{};
-  bool debug_valid = false;
-  int dbg_H = 0, dbg_W = 0, dbg_tile = 0, dbg_K = 0, dbg_prim_bits = 0, dbg_n_tiles = 0;
+  bool debug_valid = false, order_valid = false;
+  int dbg_H = 0, dbg_W = 0, dbg_K = 0, dbg_prim_bits = 0;
+  MsGrid dbg_grid{};
   uint64_t *dbg_keys = nullptr;
-  float dbg_t_stop = 0.f;
-  int dbg_tile_order = 0;
+  int dbg_contact = 0;
 };
 
 namespace {
@@ -94,13 +102,18 @@ int ensure(ms_scene *sc, Buf &b, size_t bytes) {
     if (_r != MS_OK) return _r;                 \
   } while (0)
 
-size_t scratch_total(const ms_scene *sc) {
-  const Buf *all[] = {&sc->tile_count, &sc->emit_off, &sc->rect, &sc->z_entry, &sc->oprime, &sc->keys_a, &sc->keys_b,
-                      &sc->sort_scratch, &sc->tile_start, &sc->pair_hits, &sc->pair_off, &sc->ray_hits, &sc->ray_off,
-                      &sc->scan_scratch, &sc->prim_start, &sc->prim_blocks, &sc->blk_off, &sc->intervals, &sc->hits,
-                      &sc->staging, &sc->staging_feat, &sc->staging_gate, &sc->staging_coef};
+std::vector<Buf *> scratch_bufs(ms_scene *sc) {
+  return {&sc->tile_count, &sc->emit_off, &sc->rect, &sc->z_entry, &sc->oprime, &sc->keys_a, &sc->keys_b,
+          &sc->sort_scratch, &sc->tile_start, &sc->pair_hits_i, &sc->pair_hits_j, &sc->pair_off, &sc->slot_of,
+          &sc->key2_a, &sc->key2_b, &sc->flags, &sc->gid, &sc->grp_key, &sc->grp_prim, &sc->grp_iv0, &sc->grp_blocks,
+          &sc->blk_off, &sc->grp_cnt_c, &sc->grp_blocks_c, &sc->blk_off_c, &sc->bw, &sc->bands, &sc->counters,
+          &sc->alive, &sc->ray_hits, &sc->ray_off, &sc->scan_scratch, &sc->intervals, &sc->hits, &sc->staging,
+          &sc->staging_feat, &sc->staging_gate, &sc->staging_coef, &sc->dbg_ord};
+}
+
+size_t scratch_total(ms_scene *sc) {
   size_t t = 0;
-  for (const Buf *b : all) t += b->cap;
+  for (const Buf *b : scratch_bufs(sc)) t += b->cap;
   return t;
 }
 
@@ -120,20 +133,39 @@ float round_bf16(float f) {
   return f;
 }
 
-// Adds the stage times of the previous view to the running sums.  Called right after a stream
-// synchronisation (so the events have completed) -- never adds a synchronisation of its own.
+// Event layout of a view rendered with MS_FLAG_STAGE_TIMES: 0 start (a), 1 start (b), 2 start (c), 3 start of the band
+// loop; per band b: 4 + 2b before stage (d), 5 + 2b between (d) and (e); 4 + 2 n_bands the end.
+// Adds the stage times of the previous view to the running sums.  Called right after the last event has completed.
 void harvest_stage_times(ms_scene *sc) {
   if (!sc->ev_pending) return;
   sc->ev_pending = false;
-  for (int i = 0; i < MS_N_STAGES; ++i) {
-    float ms = 0.f;
-    if (cudaEventElapsedTime(&ms, sc->ev[i], sc->ev[i + 1]) != cudaSuccess) {
-      (void)cudaGetLastError();
-      return;
-    }
-    sc->stage_sum[i] += ms;
-  }
+  float ms[MS_N_STAGES] = {0.f, 0.f, 0.f, 0.f, 0.f};
+  auto el = [&](int a, int b, float *out) {
+    float v = 0.f;
+    if (cudaEventElapsedTime(&v, sc->ev[a], sc->ev[b]) != cudaSuccess) { (void)cudaGetLastError(); return false; }
+    *out += v;
+    return true;
+  };
+  bool ok = el(0, 1, &ms[MS_STAGE_BIN]) && el(1, 2, &ms[MS_STAGE_SORT]) && el(2, 3, &ms[MS_STAGE_ISECT]);
+  for (int b = 0; ok && b < sc->ev_bands; ++b)
+    ok = el(3 + 2 * b, 4 + 2 * b, &ms[MS_STAGE_MLP]) && el(4 + 2 * b, 5 + 2 * b, &ms[MS_STAGE_COMPOSITE]);
+  if (!ok) return;
+  for (int i = 0; i < MS_N_STAGES; ++i) { sc->stage_sum[i] += ms[i]; sc->last_stage_ms[i] = ms[i]; }
   sc->stage_views += 1;
+}
+
+// Reads the device counters of the last view (waits for it) into sc->stats.
+int finish_frame(ms_scene *sc) {
+  if (!sc->frame_pending) return MS_OK;
+  CK(cudaEventSynchronize(sc->frame_done));
+  sc->frame_pending = false;
+  const uint32_t *c = sc->pinned + 1;
+  sc->stats.n_blocks = (int64_t)c[MS_CNT_BLOCKS];
+  sc->stats.n_visible = (int64_t)c[MS_CNT_VISIBLE];
+  sc->stats.n_dead_rays = (int64_t)c[MS_CNT_DEAD_RAYS];
+  sc->stats.n_samples_evaluated = sc->stats.n_samples - (int64_t)c[MS_CNT_SKIPPED] * (int64_t)sc->dbg_K;
+  sc->prev_terminated = c[MS_CNT_STOPPED_RAYS] > 0;
+  return MS_OK;
 }
 
 MsCam make_cam(const ms_camera *c, int H, int W) {
@@ -154,12 +186,16 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   const int tile = opts->tile == 0 ? 16 : opts->tile;
   const int K = opts->K;
   const int N = sc->n;
-  const int tiles_x = (W + tile - 1) / tile, tiles_y = (H + tile - 1) / tile;
-  const int64_t n_tiles64 = (int64_t)tiles_x * tiles_y;
-  const int64_t R64 = (int64_t)H * W;
+  MsGrid grid;
+  grid.tile = tile; grid.tiles_x = (W + tile - 1) / tile; grid.tiles_y = (H + tile - 1) / tile;
+  grid.G = 64 / tile < 1 ? 1 : 64 / tile;          // macro-tiles of 64 x 64 pixels
+  grid.W = W; grid.H = H;
+  const int64_t n_tiles64 = (int64_t)grid.tiles_x * grid.tiles_y;
+  const int64_t R64 = n_tiles64 * tile * tile;      // ray slots: every tile padded to tile x tile
   if (R64 >= (1ll << 31) - 1) return MS_ERR_UNSUPPORTED_SHAPE;
-  const int n_tiles = (int)n_tiles64;
-  const int R = (int)R64;
+  grid.n_tiles = (int)n_tiles64;
+  const int n_tiles = grid.n_tiles;
+  const size_t R = (size_t)R64;
   const int prim_bits = ceil_log2((uint64_t)N) < 1 ? 1 : ceil_log2((uint64_t)N);
   const int tile_bits = ceil_log2((uint64_t)n_tiles) < 1 ? 1 : ceil_log2((uint64_t)n_tiles);
   if (prim_bits + tile_bits > 32) return MS_ERR_UNSUPPORTED_SHAPE;
@@ -171,44 +207,69 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   if (path != MS_PATH_BF16_TC && path != MS_PATH_FP32) return MS_ERR_INVALID_ARG;
 
   const bool timing = (opts->flags & MS_FLAG_STAGE_TIMES) != 0;
-  sc->debug_valid = false;
   const MsCam cam = make_cam(camera, H, W);
   const long long launches0 = ms_launch_count;
   if (sc->ev_pending) {  // the previous view's events must be read before they are re-recorded
-    CK(cudaEventSynchronize(sc->ev[MS_N_STAGES]));
+    CK(cudaEventSynchronize(sc->ev[3 + 2 * sc->ev_bands]));
     harvest_stage_times(sc);
   }
+  {  // the previous view's counters (its stats, and whether its rays stopped early: MS_WAVES_AUTO)
+    int rc = finish_frame(sc);
+    if (rc != MS_OK) return rc;
+  }
+  sc->debug_valid = false;
+  sc->order_valid = false;
   sc->ev_valid = false;
+  auto rec = [&](int i) -> cudaError_t {
+    if (!timing) return cudaSuccess;
+    while ((int)sc->ev.size() <= i) {
+      cudaEvent_t e;
+      cudaError_t r = cudaEventCreate(&e);
+      if (r != cudaSuccess) return r;
+      sc->ev.push_back(e);
+    }
+    return cudaEventRecord(sc->ev[i], st);
+  };
 
   // ---- (a) projection + key emit ----------------------------------------------------------
-  if (timing) CK(cudaEventRecord(sc->ev[0], st));
+  CK(rec(0));
+  ENS(sc->counters, (MS_CNT_N + 4) * 4);
+  CK(cudaMemsetAsync(sc->counters.p, 0, (MS_CNT_N + 4) * 4, st));
+  uint32_t *counters = (uint32_t *)sc->counters.p;
   ENS(sc->tile_count, (size_t)N * 4);
   ENS(sc->emit_off, (size_t)(N + 1) * 4);
   ENS(sc->rect, (size_t)N * sizeof(int4));
   ENS(sc->z_entry, (size_t)N * 4);
   ENS(sc->oprime, (size_t)N * 12);
-  ENS(sc->scan_scratch, (ms_scan_scratch_elems((size_t)R > (size_t)N ? (size_t)R : (size_t)N) + 16) * 4);
-  CK(ms_project(N, sc->center, sc->A, sc->M, cam, tile, tiles_x, tiles_y, (uint32_t *)sc->tile_count.p,
-                (int4 *)sc->rect.p, (float *)sc->z_entry.p, (float *)sc->oprime.p, st));
+  ENS(sc->scan_scratch, (ms_scan_scratch_elems(R > (size_t)N ? R : (size_t)N) + 16) * 4);
+  const float eye_guard = opts->eye_guard > 0.0f ? opts->eye_guard : MS_EYE_GUARD_DEFAULT;
+  CK(ms_project(N, sc->center, sc->A, sc->M, cam, tile, eye_guard, (uint32_t *)sc->tile_count.p,
+                (int4 *)sc->rect.p, (float *)sc->z_entry.p, (float *)sc->oprime.p, counters, st));
   CK(ms_exclusive_scan_u32((uint32_t *)sc->tile_count.p, (uint32_t *)sc->emit_off.p, (size_t)N,
                            (uint32_t *)sc->scan_scratch.p, st));
   CK(cudaMemcpyAsync(sc->pinned, (uint32_t *)sc->emit_off.p + N, 4, cudaMemcpyDeviceToHost, st));
+  CK(cudaMemcpyAsync(sc->pinned + 1 + MS_CNT_PAIRS_HI, counters + MS_CNT_PAIRS_HI, 4, cudaMemcpyDeviceToHost, st));
   CK(cudaStreamSynchronize(st));
+  // the 32-bit scan total must agree with the 64-bit count of the projection kernel (a wrapped sum would size
+  // every buffer below too small)
+  if (sc->pinned[1 + MS_CNT_PAIRS_HI] != 0) return MS_ERR_UNSUPPORTED_SHAPE;
   const size_t P = sc->pinned[0];
   if (P >= (1ull << 31)) return MS_ERR_UNSUPPORTED_SHAPE;
   ENS(sc->keys_a, (P + 1) * 8);
   ENS(sc->keys_b, (P + 1) * 8);
   ENS(sc->sort_scratch, ms_sort_scratch_elems(P) * 4);
   ENS(sc->tile_start, (size_t)(n_tiles + 1) * 4);
-  ENS(sc->pair_hits, (P + 1) * 4);
+  ENS(sc->pair_hits_i, (P + 1) * 4);
+  ENS(sc->pair_hits_j, (P + 2) * 4);
   ENS(sc->pair_off, (P + 2) * 4);
+  ENS(sc->slot_of, (P + 1) * 4);
   if (ms_scan_scratch_elems(P) + 16 > sc->scan_scratch.cap / 4) ENS(sc->scan_scratch, (ms_scan_scratch_elems(P) + 16) * 4);
   const int tile_order = (opts->flags & MS_FLAG_TILE_ORDER) != 0;
-  CK(ms_emit_keys(N, (uint32_t *)sc->emit_off.p, (int4 *)sc->rect.p, (float *)sc->z_entry.p, tiles_x, prim_bits,
+  CK(ms_emit_keys(N, (uint32_t *)sc->emit_off.p, (int4 *)sc->rect.p, (float *)sc->z_entry.p, grid.tiles_x, prim_bits,
                   (uint64_t *)sc->keys_a.p, tile_order, cam, tile, sc->A, (float *)sc->oprime.p, st));
 
   // ---- (b) radix sort + tile ranges -------------------------------------------------------
-  if (timing) CK(cudaEventRecord(sc->ev[1], st));
+  CK(rec(1));
   uint64_t *sorted = nullptr;
   // stage (a) emits the keys primitive by primitive, i.e. already ordered by the id in their low prim_bits bits;
   // the sort is stable, so only the (tile | depth) bits above them need passes
@@ -216,67 +277,124 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
                        (uint32_t *)sc->sort_scratch.p, &sorted, st));
   CK(ms_tile_ranges(sorted, P, n_tiles, prim_bits, (uint32_t *)sc->tile_start.p, st));
 
-  // ---- (c) intersection: count, scans, fill -----------------------------------------------
-  if (timing) CK(cudaEventRecord(sc->ev[2], st));
-  ENS(sc->ray_hits, (size_t)R * 4);
-  ENS(sc->ray_off, (size_t)(R + 1) * 4);
-  ENS(sc->prim_start, (size_t)(N + 1) * 4);
-  ENS(sc->prim_blocks, (size_t)(N + 1) * 4);
-  ENS(sc->blk_off, (size_t)(N + 2) * 4);
+  // ---- (c) intersection: count, scan, pair order, fill ---------------------------------------
+  CK(rec(2));
+  ENS(sc->ray_hits, R * 4);
+  ENS(sc->ray_off, (R + 1) * 4);
   MsIsectArgs ia;
-  ia.cam = cam; ia.tile = tile; ia.tiles_x = tiles_x; ia.n_tiles = n_tiles; ia.K = K; ia.prim_bits = prim_bits;
+  ia.cam = cam; ia.grid = grid; ia.K = K; ia.prim_bits = prim_bits;
   ia.contact = sc->shape.mode == MS_MODE_CONTACT;
+  ia.wave_c = 0;
   ia.keys = sorted; ia.tile_start = (uint32_t *)sc->tile_start.p; ia.A = sc->A; ia.oprime = (float *)sc->oprime.p;
-  ia.rect = (int4 *)sc->rect.p; ia.emit_off = (uint32_t *)sc->emit_off.p;
-  ia.pair_hits = (uint32_t *)sc->pair_hits.p; ia.ray_hits = (uint32_t *)sc->ray_hits.p;
-  ia.pair_off = (uint32_t *)sc->pair_off.p; ia.ray_off = (uint32_t *)sc->ray_off.p;
+  ia.pair_hits = (uint32_t *)sc->pair_hits_i.p; ia.ray_hits = (uint32_t *)sc->ray_hits.p;
+  ia.slot_of = (uint32_t *)sc->slot_of.p; ia.pair_off = (uint32_t *)sc->pair_off.p; ia.ray_off = (uint32_t *)sc->ray_off.p;
   ia.intervals = nullptr; ia.hits = nullptr;
   CK(ms_isect_count(ia, st));
-  CK(ms_exclusive_scan_u32((uint32_t *)sc->pair_hits.p, (uint32_t *)sc->pair_off.p, P, (uint32_t *)sc->scan_scratch.p, st));
-  CK(ms_exclusive_scan_u32((uint32_t *)sc->ray_hits.p, (uint32_t *)sc->ray_off.p, (size_t)R,
-                           (uint32_t *)sc->scan_scratch.p, st));
-  CK(ms_prim_blocks(N, (uint32_t *)sc->emit_off.p, (uint32_t *)sc->pair_off.p, K, (uint32_t *)sc->prim_start.p,
-                    (uint32_t *)sc->prim_blocks.p, st));
-  CK(ms_exclusive_scan_u32((uint32_t *)sc->prim_blocks.p, (uint32_t *)sc->blk_off.p, (size_t)N,
-                           (uint32_t *)sc->scan_scratch.p, st));
-  CK(cudaMemcpyAsync(sc->pinned + 1, (uint32_t *)sc->ray_off.p + R, 4, cudaMemcpyDeviceToHost, st));
-  CK(cudaMemcpyAsync(sc->pinned + 2, (uint32_t *)sc->blk_off.p + N, 4, cudaMemcpyDeviceToHost, st));
-  CK(cudaMemcpyAsync(sc->pinned + 3, (uint32_t *)sc->pair_off.p + P, 4, cudaMemcpyDeviceToHost, st));
+  CK(ms_exclusive_scan_u32((uint32_t *)sc->ray_hits.p, (uint32_t *)sc->ray_off.p, R, (uint32_t *)sc->scan_scratch.p, st));
+  CK(ms_tile_stats(grid, (uint32_t *)sc->ray_off.p, (uint32_t *)sc->tile_start.p, counters, st));
+  CK(cudaMemcpyAsync(sc->pinned + 1, counters, MS_CNT_N * 4, cudaMemcpyDeviceToHost, st));
   CK(cudaStreamSynchronize(st));
-  const size_t n_hits = sc->pinned[1];
-  const uint32_t n_blocks = sc->pinned[2];
-  if (sc->pinned[3] != sc->pinned[1]) return MS_ERR_CUDA;  // the two scans must agree
+  if (sc->pinned[1 + MS_CNT_HITS_HI] != 0) return MS_ERR_UNSUPPORTED_SHAPE;   // 64-bit hit total beyond 32 bits
+  const size_t n_hits = sc->pinned[1 + MS_CNT_HITS];
+  const size_t max_tile_hits = sc->pinned[1 + MS_CNT_MAX_TILE_HITS];
+  const uint32_t max_list = sc->pinned[1 + MS_CNT_MAX_LIST];
   if (n_hits >= (1ull << 31)) return MS_ERR_UNSUPPORTED_SHAPE;
   const size_t n_samples = n_hits * (size_t)K;
+  if (n_samples >= (1ull << 40)) return MS_ERR_UNSUPPORTED_SHAPE;
   const bool want_feat = sc->shape.n_feat > 0 && out_feat != nullptr;
+  const bool want_slots = sc->slot_cf > 0 && out_feat != nullptr;   // Eq.7 features (contact mode, K = 1)
+
+  // bands: the staging bytes of one sample decide how many hits fit the budget
+  const size_t sample_bytes = sizeof(float4) + (want_feat ? (size_t)sc->shape.n_feat * 4 : 0) + (want_slots ? 2 * sizeof(float4) : 0);
+  const int64_t budget = opts->band_bytes == 0 ? MS_BAND_BYTES_DEFAULT : opts->band_bytes;
+  size_t cap_hits = n_hits + 1;
+  if (budget > 0) {
+    cap_hits = (size_t)budget / (sample_bytes * (size_t)K);
+    if (cap_hits < 1) cap_hits = 1;
+  }
+  int n_bands = n_hits <= cap_hits ? 1 : (int)(n_hits / cap_hits) + 1;
+  while (n_bands > 1 && prim_bits + 3 + ceil_log2((uint64_t)n_bands) > 32) {   // (band, wave, prim) must fit 32 bits
+    cap_hits *= 2;
+    n_bands = n_hits <= cap_hits ? 1 : (int)(n_hits / cap_hits) + 1;
+  }
+  // depth waves: asked for, or (auto) the previous view had rays stopping early
+  int wave_c = 0;
+  if (opts->t_stop > 0.0f && !tile_order) {
+    if (opts->waves > 0) wave_c = opts->waves;
+    else if (opts->waves == MS_WAVES_AUTO && sc->prev_terminated) wave_c = 4;
+  }
+  int n_waves = 1;
+  if (wave_c > 0 && max_list > 0) n_waves = ms_wave_of_rank(max_list - 1, wave_c) + 1;
+  if (n_waves == 1) wave_c = 0;
+  const bool banded = n_bands > 1 || wave_c > 0;
+  const size_t seg_cap = (banded ? P : (size_t)N) + 2;
+  const size_t band_hits_cap = n_bands == 1 ? n_hits : cap_hits + max_tile_hits;
+
+  ENS(sc->grp_iv0, (seg_cap + 1) * 4);
+  ENS(sc->grp_blocks, (seg_cap + 1) * 4);
+  ENS(sc->blk_off, (seg_cap + 2) * 4);
+  ENS(sc->bw, (size_t)n_bands * MS_MAX_WAVES * sizeof(uint2));
+  ENS(sc->bands, (size_t)n_bands * sizeof(MsBand));
+  if (banded) {
+    ENS(sc->key2_a, (P + 1) * 8);
+    ENS(sc->key2_b, (P + 1) * 8);
+    ENS(sc->flags, (P + 2) * 4);
+    ENS(sc->gid, (P + 2) * 4);
+    ENS(sc->grp_key, seg_cap * 4);
+    ENS(sc->grp_prim, seg_cap * 4);
+  }
+  if (wave_c > 0) {
+    ENS(sc->grp_cnt_c, seg_cap * 4);
+    ENS(sc->grp_blocks_c, seg_cap * 4);
+    ENS(sc->blk_off_c, (seg_cap + 2) * 4);
+    ENS(sc->alive, R);
+    CK(cudaMemsetAsync(sc->alive.p, 1, R, st));
+  }
   ENS(sc->intervals, (n_hits + 1) * sizeof(MsInterval));
   ENS(sc->hits, (n_hits + 1) * sizeof(MsHit));
-  ENS(sc->staging, (n_samples + 1) * sizeof(float4));
-  if (want_feat) ENS(sc->staging_feat, (n_samples + 1) * (size_t)sc->shape.n_feat * 4);
-  const bool want_slots = sc->slot_cf > 0 && out_feat != nullptr;   // Eq.7 features (contact mode, K = 1)
-  if (want_slots) ENS(sc->staging_gate, (n_samples + 1) * sizeof(float4));
-  if (want_slots) ENS(sc->staging_coef, (n_samples + 1) * sizeof(float4));
+  ENS(sc->staging, (band_hits_cap * (size_t)K + 1) * sizeof(float4));
+  if (want_feat) ENS(sc->staging_feat, (band_hits_cap * (size_t)K + 1) * (size_t)sc->shape.n_feat * 4);
+  if (want_slots) ENS(sc->staging_gate, (band_hits_cap * (size_t)K + 1) * sizeof(float4));
+  if (want_slots) ENS(sc->staging_coef, (band_hits_cap * (size_t)K + 1) * sizeof(float4));
+  const bool keep_order = (opts->flags & MS_FLAG_KEEP_ORDER) != 0;
+  if (keep_order) {
+    ENS(sc->dbg_ord, (n_samples + 1) * 4);
+    CK(cudaMemsetAsync(sc->dbg_ord.p, 0xff, (n_samples + 1) * 4, st));   // a rank stage (e) never writes is seen
+  }
+
+  MsBandArgs ba;
+  ba.grid = grid; ba.K = K; ba.prim_bits = prim_bits; ba.n_prims = N; ba.wave_c = wave_c; ba.n_bands = n_bands;
+  ba.cap_hits = (uint32_t)(cap_hits > 0xffffffffull ? 0xffffffffull : cap_hits); ba.P = P;
+  ba.keys = sorted; ba.tile_start = (uint32_t *)sc->tile_start.p; ba.ray_off = (uint32_t *)sc->ray_off.p;
+  ba.emit_off = (uint32_t *)sc->emit_off.p; ba.rect = (int4 *)sc->rect.p; ba.pair_hits_i = (uint32_t *)sc->pair_hits_i.p;
+  ba.key2_a = (uint64_t *)sc->key2_a.p; ba.key2_b = (uint64_t *)sc->key2_b.p;
+  ba.sort_scratch = (uint32_t *)sc->sort_scratch.p; ba.scan_scratch = (uint32_t *)sc->scan_scratch.p;
+  ba.slot_of = (uint32_t *)sc->slot_of.p; ba.pair_hits_j = (uint32_t *)sc->pair_hits_j.p; ba.pair_off = (uint32_t *)sc->pair_off.p;
+  ba.flags = (uint32_t *)sc->flags.p; ba.gid = (uint32_t *)sc->gid.p;
+  ba.grp_key = (uint32_t *)sc->grp_key.p; ba.grp_prim = (uint32_t *)sc->grp_prim.p; ba.grp_iv0 = (uint32_t *)sc->grp_iv0.p;
+  ba.grp_blocks = (uint32_t *)sc->grp_blocks.p; ba.blk_off = (uint32_t *)sc->blk_off.p;
+  ba.bw = (uint2 *)sc->bw.p; ba.bands = (MsBand *)sc->bands.p; ba.counters = counters;
+  if (banded) CK(ms_order_banded(ba, st));
+  else CK(ms_order_single(ba, st));
+
+  ia.wave_c = wave_c;
   ia.intervals = (MsInterval *)sc->intervals.p;
   ia.hits = (MsHit *)sc->hits.p;
   CK(ms_isect_fill(ia, st));
 
-  // ---- (d) grouped per-primitive MLP ------------------------------------------------------
-  if (timing) CK(cudaEventRecord(sc->ev[3], st));
+  // ---- per band: (d) grouped per-primitive MLP, wave by wave, then (e) merge + composite ----------------
   MsMlpArgs ma;
-  ma.shape = sc->shape; ma.cam = cam; ma.K = K; ma.n_prims = N;
+  ma.shape = sc->shape; ma.cam = cam; ma.K = K; ma.falloff = sc->falloff;
   ma.center = sc->center; ma.A = sc->A; ma.weights_f32 = sc->weights_f32;
-  ma.prim_start = (uint32_t *)sc->prim_start.p; ma.blk_off = (uint32_t *)sc->blk_off.p; ma.n_blocks = n_blocks;
+  ma.segs.iv0 = (uint32_t *)sc->grp_iv0.p; ma.segs.cnt = nullptr; ma.segs.blk_off = (uint32_t *)sc->blk_off.p;
+  ma.segs.prim = banded ? (uint32_t *)sc->grp_prim.p : nullptr;
+  ma.n_blocks_hint = 0;
   ma.intervals = (MsInterval *)sc->intervals.p;
   ma.staging = (float4 *)sc->staging.p;
   ma.staging_feat = want_feat ? (float *)sc->staging_feat.p : nullptr;
   ma.staging_gate = want_slots ? (float4 *)sc->staging_gate.p : nullptr;
-  if (path == MS_PATH_BF16_TC) CK(ms_mlp_tc(sc->tc, ma, st));
-  else CK(ms_mlp_f32(ma, st));
-
-  // ---- (e) merge + composite ---------------------------------------------------------------
-  if (timing) CK(cudaEventRecord(sc->ev[4], st));
   MsCompositeArgs ca;
-  ca.n_rays = R; ca.K = K; ca.n_feat = sc->shape.n_feat; ca.t_stop = opts->t_stop;
+  ca.grid = grid; ca.K = K; ca.n_feat = sc->shape.n_feat; ca.t_stop = opts->t_stop;
   ca.contact = sc->shape.mode == MS_MODE_CONTACT;
   ca.tile_order = tile_order;
   ca.ray_off = (uint32_t *)sc->ray_off.p; ca.hits = (MsHit *)sc->hits.p; ca.staging = (float4 *)sc->staging.p;
@@ -284,26 +402,64 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   ca.gates = want_slots ? (const float4 *)sc->staging_gate.p : nullptr;
   ca.coef = want_slots ? (float4 *)sc->staging_coef.p : nullptr;
   ca.slots = sc->slots; ca.c_f = sc->slot_cf;
+  ca.dbg_ord = keep_order ? (uint32_t *)sc->dbg_ord.p : nullptr;
+  ca.counters = counters;
   ca.out_rgb = out_rgb; ca.out_alpha = out_alpha; ca.out_feat = (want_feat || want_slots) ? out_feat : nullptr;
-  CK(ms_composite(ca, st));
+  MsWaveArgs wa;
+  wa.grid = grid; wa.K = K; wa.prim_bits = prim_bits; wa.wave_c = wave_c; wa.contact = ca.contact;
+  wa.t_stop = opts->t_stop;
+  wa.margin = 1e-4f * (1.0f + fabsf(cam.o[0]) + fabsf(cam.o[1]) + fabsf(cam.o[2]));
+  wa.keys = sorted; wa.tile_start = (uint32_t *)sc->tile_start.p; wa.ray_off = (uint32_t *)sc->ray_off.p;
+  wa.hits = (MsHit *)sc->hits.p; wa.staging = (float4 *)sc->staging.p; wa.bands = (MsBand *)sc->bands.p;
+  wa.bw = (uint2 *)sc->bw.p; wa.alive = (uint8_t *)sc->alive.p; wa.intervals = (MsInterval *)sc->intervals.p;
+  wa.grp_iv0 = (uint32_t *)sc->grp_iv0.p; wa.grp_cnt_c = (uint32_t *)sc->grp_cnt_c.p;
+  wa.grp_blocks_c = (uint32_t *)sc->grp_blocks_c.p; wa.blk_off_c = (uint32_t *)sc->blk_off_c.p;
+  wa.counters = counters; wa.n_sm = sc->n_sm;
+  for (int b = 0; b < n_bands; ++b) {
+    CK(rec(3 + 2 * b));
+    ma.segs.band = (MsBand *)sc->bands.p + b;
+    for (int w = 0; w < n_waves; ++w) {
+      ma.segs.range = (uint2 *)sc->bw.p + (size_t)b * MS_MAX_WAVES + w;
+      if (w > 0) {    // rays that have stopped drop out of this wave before their samples are encoded
+        wa.band = b; wa.wave = w;
+        CK(ms_wave_prepare(wa, st));
+        ma.segs.cnt = (uint32_t *)sc->grp_cnt_c.p; ma.segs.blk_off = (uint32_t *)sc->blk_off_c.p;
+      } else {
+        ma.segs.cnt = nullptr; ma.segs.blk_off = (uint32_t *)sc->blk_off.p;
+      }
+      if (path == MS_PATH_BF16_TC) CK(ms_mlp_tc(sc->tc, ma, st));
+      else CK(ms_mlp_f32(ma, st));
+    }
+    CK(rec(4 + 2 * b));
+    ca.band = (MsBand *)sc->bands.p + b;
+    CK(ms_composite(ca, st));
+  }
+  CK(rec(3 + 2 * n_bands));
   if (timing) {
-    CK(cudaEventRecord(sc->ev[5], st));
+    sc->ev_bands = n_bands;
     sc->ev_valid = true;
     sc->ev_pending = true;
   }
+  CK(cudaMemcpyAsync(sc->pinned + 1, counters, MS_CNT_N * 4, cudaMemcpyDeviceToHost, st));
+  CK(cudaEventRecord(sc->frame_done, st));
+  sc->frame_pending = true;
+  sc->stats = ms_stats{};
   sc->stats.n_launches = (int64_t)(ms_launch_count - launches0);
-
   sc->stats.n_pairs = (int64_t)P;
   sc->stats.n_intervals = (int64_t)n_hits;
   sc->stats.n_samples = (int64_t)n_samples;
-  sc->stats.n_blocks = (int64_t)n_blocks;
-  sc->stats.n_visible = -1;
+  sc->stats.n_samples_evaluated = (int64_t)n_samples;
+  sc->stats.n_bands = n_bands;
+  sc->stats.n_waves = n_waves;
+  sc->stats.staging_bytes = (int64_t)(band_hits_cap * (size_t)K * sample_bytes);   // what this view needed
   sc->stats.scratch_bytes = (int64_t)scratch_total(sc);
+  sc->dbg_K = K;
   if (opts->flags & MS_FLAG_KEEP_DEBUG) {
     sc->debug_valid = true;
-    sc->dbg_H = H; sc->dbg_W = W; sc->dbg_tile = tile; sc->dbg_K = K; sc->dbg_prim_bits = prim_bits;
-    sc->dbg_n_tiles = n_tiles; sc->dbg_keys = sorted; sc->dbg_t_stop = opts->t_stop;
-    sc->dbg_tile_order = tile_order;
+    sc->order_valid = keep_order;
+    sc->dbg_H = H; sc->dbg_W = W; sc->dbg_prim_bits = prim_bits;
+    sc->dbg_grid = grid; sc->dbg_keys = sorted;
+    sc->dbg_contact = ca.contact;
   }
   return MS_OK;
 }
@@ -342,6 +498,7 @@ int ms_scene_create(const ms_prims *prims, const ms_mlp *mlp, ms_scene **out) {
   sh.width = mlp->width; sh.n_feat = mlp->n_feat;
   if (mlp->mode != MS_MODE_LOCAL && mlp->mode != MS_MODE_CONTACT) return MS_ERR_INVALID_ARG;
   if (mlp->mode == MS_MODE_CONTACT && (mlp->n_freq < 1 || mlp->use_viewdir)) return MS_ERR_INVALID_ARG;
+  if (mlp->mode == MS_MODE_CONTACT && !(mlp->falloff >= 0.0f)) return MS_ERR_INVALID_ARG;
   sh.mode = mlp->mode;
   sh.in_dim = sh.mode == MS_MODE_CONTACT ? 12 * sh.n_freq : 3 + 6 * sh.n_freq + (sh.use_viewdir ? 3 : 0);
   sh.out_dim = 4 + sh.n_feat;
@@ -363,6 +520,7 @@ int ms_scene_create(const ms_prims *prims, const ms_mlp *mlp, ms_scene **out) {
   sc->n = prims->n;
   sc->dtype = mlp->dtype;
   sc->shape = sh;
+  sc->falloff = mlp->falloff;
   int rc = MS_OK;
   int *d_bad = nullptr;
   std::vector<float> w;
@@ -380,6 +538,7 @@ int ms_scene_create(const ms_prims *prims, const ms_mlp *mlp, ms_scene **out) {
     }                                                                                    \
   } while (0)
   CKC(cudaGetDevice(&sc->device));
+  CKC(cudaDeviceGetAttribute(&sc->n_sm, cudaDevAttrMultiProcessorCount, sc->device));
   CKC(cudaMalloc(&sc->center, n * 12));
   CKC(cudaMalloc(&sc->quat, n * 16));
   CKC(cudaMalloc(&sc->scale, n * 12));
@@ -415,8 +574,9 @@ int ms_scene_create(const ms_prims *prims, const ms_mlp *mlp, ms_scene **out) {
   if (bad) return fail(MS_ERR_INVALID_ARG);
   for (size_t i = 0; i < n * 3; ++i)
     if (!isfinite(prims->center[i])) return fail(MS_ERR_INVALID_ARG);
-  CKC(cudaMallocHost(&sc->pinned, 16));
-  for (int i = 0; i <= MS_N_STAGES; ++i) CKC(cudaEventCreate(&sc->ev[i]));
+  CKC(cudaMallocHost(&sc->pinned, (MS_CNT_N + 4) * 4));
+  memset(sc->pinned, 0, (MS_CNT_N + 4) * 4);
+  CKC(cudaEventCreateWithFlags(&sc->frame_done, cudaEventDisableTiming));
   if (mlp->dtype == MS_BF16) {
     rc = ms_tc_pack(sh, sc->n, w.data(), &sc->tc);  // leaves tc.valid = false if the shape is not covered
     if (rc != MS_OK) return fail(rc);
@@ -450,14 +610,11 @@ int ms_scene_destroy(ms_scene *sc) {
   cudaFree(sc->weights_f32);
   cudaFree(sc->slots);
   ms_tc_free(&sc->tc);
-  Buf *all[] = {&sc->tile_count, &sc->emit_off, &sc->rect, &sc->z_entry, &sc->oprime, &sc->keys_a, &sc->keys_b,
-                &sc->sort_scratch, &sc->tile_start, &sc->pair_hits, &sc->pair_off, &sc->ray_hits, &sc->ray_off,
-                &sc->scan_scratch, &sc->prim_start, &sc->prim_blocks, &sc->blk_off, &sc->intervals, &sc->hits,
-                &sc->staging, &sc->staging_feat, &sc->staging_gate, &sc->staging_coef, &sc->host_rgb, &sc->host_alpha, &sc->host_feat, &sc->dbg};
-  for (Buf *b : all) free_buf(*b);
+  for (Buf *b : scratch_bufs(sc)) free_buf(*b);
+  free_buf(sc->host_rgb); free_buf(sc->host_alpha); free_buf(sc->host_feat);
   if (sc->pinned) cudaFreeHost(sc->pinned);
-  for (int i = 0; i <= MS_N_STAGES; ++i)
-    if (sc->ev[i]) cudaEventDestroy(sc->ev[i]);
+  for (cudaEvent_t e : sc->ev) cudaEventDestroy(e);
+  if (sc->frame_done) cudaEventDestroy(sc->frame_done);
   (void)cudaGetLastError();
   delete sc;
   return MS_OK;
@@ -508,21 +665,26 @@ int ms_render_host(ms_scene *sc, const ms_camera *cams, int32_t n_views, int32_t
 
 int ms_last_stats(ms_scene *sc, ms_stats *out) {
   if (!sc || !out) return MS_ERR_INVALID_ARG;
+  int rc = finish_frame(sc);
+  if (rc != MS_OK) return rc;
   *out = sc->stats;
   return MS_OK;
 }
 
 int ms_last_stage_ms(ms_scene *sc, float *ms) {
   if (!sc || !ms || !sc->ev_valid) return MS_ERR_INVALID_ARG;
-  CK(cudaEventSynchronize(sc->ev[MS_N_STAGES]));
-  for (int i = 0; i < MS_N_STAGES; ++i) CK(cudaEventElapsedTime(&ms[i], sc->ev[i], sc->ev[i + 1]));
+  if (sc->ev_pending) {
+    CK(cudaEventSynchronize(sc->ev[3 + 2 * sc->ev_bands]));
+    harvest_stage_times(sc);
+  }
+  for (int i = 0; i < MS_N_STAGES; ++i) ms[i] = sc->last_stage_ms[i];
   return MS_OK;
 }
 
 int ms_stage_accum(ms_scene *sc, double *ms_sum, int64_t *n_views, int32_t reset) {
   if (!sc) return MS_ERR_INVALID_ARG;
   if (sc->ev_pending) {
-    CK(cudaEventSynchronize(sc->ev[MS_N_STAGES]));
+    CK(cudaEventSynchronize(sc->ev[3 + 2 * sc->ev_bands]));
     harvest_stage_times(sc);
   }
   if (ms_sum)
@@ -542,7 +704,7 @@ int ms_debug_tile_lists(ms_scene *sc, int64_t *tile_offsets, int32_t *prim_ids, 
   if (n) *n = P;
   if (cap < P) return MS_ERR_CAPACITY;
   std::vector<uint64_t> keys(P);
-  std::vector<uint32_t> ts((size_t)sc->dbg_n_tiles + 1);
+  std::vector<uint32_t> ts((size_t)sc->dbg_grid.n_tiles + 1);
   if (P) CK(cudaMemcpy(keys.data(), sc->dbg_keys, P * 8, cudaMemcpyDeviceToHost));
   CK(cudaMemcpy(ts.data(), sc->tile_start.p, ts.size() * 4, cudaMemcpyDeviceToHost));
   if (tile_offsets)
@@ -555,51 +717,99 @@ int ms_debug_tile_lists(ms_scene *sc, int64_t *tile_offsets, int32_t *prim_ids, 
   return MS_OK;
 }
 
+// ray slot of pixel index y*W + x
+static uint32_t slot_of_pixel(const MsGrid &g, size_t pix) {
+  const int x = (int)(pix % (size_t)g.W), y = (int)(pix / (size_t)g.W);
+  const int tx = x / g.tile, ty = y / g.tile;
+  return (uint32_t)ms_tile_pos(g, tx, ty) * (uint32_t)(g.tile * g.tile) + (uint32_t)((y - ty * g.tile) * g.tile + (x - tx * g.tile));
+}
+
 int ms_debug_intervals(ms_scene *sc, int64_t *hit_offsets, int32_t *prim, float *t_in, float *delta, size_t cap,
                        size_t *n) {
   if (!sc || !sc->debug_valid) return MS_ERR_INVALID_ARG;
   CK(cudaDeviceSynchronize());
   const size_t nh = (size_t)sc->stats.n_intervals;
-  const size_t R = (size_t)sc->dbg_H * sc->dbg_W;
+  const MsGrid &g = sc->dbg_grid;
+  const size_t R = (size_t)sc->dbg_H * sc->dbg_W, Rs = (size_t)g.n_tiles * g.tile * g.tile;
   if (n) *n = nh;
   if (cap < nh) return MS_ERR_CAPACITY;
-  std::vector<uint32_t> ro(R + 1);
+  std::vector<uint32_t> ro(Rs + 1);
   std::vector<MsHit> h(nh);
-  CK(cudaMemcpy(ro.data(), sc->ray_off.p, (R + 1) * 4, cudaMemcpyDeviceToHost));
+  CK(cudaMemcpy(ro.data(), sc->ray_off.p, (Rs + 1) * 4, cudaMemcpyDeviceToHost));
   if (nh) CK(cudaMemcpy(h.data(), sc->hits.p, nh * sizeof(MsHit), cudaMemcpyDeviceToHost));
-  if (hit_offsets)
-    for (size_t i = 0; i <= R; ++i) hit_offsets[i] = ro[i];
-  for (size_t i = 0; i < nh; ++i) {
-    if (prim) prim[i] = h[i].prim;
-    if (t_in) t_in[i] = h[i].t_in;
-    if (delta) delta[i] = h[i].delta;
+  // the device numbers its rays tile by tile; the export is in pixel order y*W + x
+  size_t tot = 0;
+  for (size_t pix = 0; pix < R; ++pix) {
+    const uint32_t q = slot_of_pixel(g, pix);
+    if (hit_offsets) hit_offsets[pix] = (int64_t)tot;
+    for (uint32_t i = ro[q]; i < ro[q + 1]; ++i, ++tot) {
+      if (prim) prim[tot] = h[i].prim;
+      if (t_in) t_in[tot] = h[i].t_in;
+      if (delta) delta[tot] = h[i].delta;
+    }
+  }
+  if (hit_offsets) hit_offsets[R] = (int64_t)tot;
+  return MS_OK;
+}
+
+// canonical sample position, host side: this file is compiled without FMA contraction
+static float host_sample_t(float t_in, float delta, int k, int contact) {
+  if (contact) return t_in;
+  volatile float kf = (float)k + 0.5f;
+  volatile float m = kf * delta;
+  return t_in + m;
+}
+
+int ms_debug_sample_order(ms_scene *sc, int32_t ray, int32_t *prim, int32_t *k, float *t, size_t cap, size_t *n) {
+  if (!sc || !sc->debug_valid || !sc->order_valid || ray < 0 || ray >= sc->dbg_H * sc->dbg_W) return MS_ERR_INVALID_ARG;
+  CK(cudaDeviceSynchronize());
+  const uint32_t q = slot_of_pixel(sc->dbg_grid, (size_t)ray);
+  uint32_t ro[2];
+  CK(cudaMemcpy(ro, (uint32_t *)sc->ray_off.p + q, 8, cudaMemcpyDeviceToHost));
+  const size_t K = (size_t)sc->dbg_K, nh = ro[1] - ro[0], ns = nh * K;
+  if (n) *n = ns;
+  if (cap < ns) return MS_ERR_CAPACITY;
+  if (ns == 0) return MS_OK;
+  std::vector<uint32_t> ord(ns);
+  std::vector<MsHit> h(nh);
+  CK(cudaMemcpy(ord.data(), (uint32_t *)sc->dbg_ord.p + (size_t)ro[0] * K, ns * 4, cudaMemcpyDeviceToHost));
+  CK(cudaMemcpy(h.data(), (MsHit *)sc->hits.p + ro[0], nh * sizeof(MsHit), cudaMemcpyDeviceToHost));
+  for (size_t r = 0; r < ns; ++r) {
+    const uint32_t s = ord[r];
+    if (s >= ns) return MS_ERR_CUDA;       // stage (e) never wrote this rank
+    const size_t hh = s / K;
+    const int kk = (int)(s % K);
+    if (prim) prim[r] = h[hh].prim;
+    if (k) k[r] = kk;
+    if (t) t[r] = host_sample_t(h[hh].t_in, h[hh].delta, kk, sc->dbg_contact);
   }
   return MS_OK;
 }
 
-int ms_debug_sample_order(ms_scene *sc, int32_t ray, int32_t *prim, int32_t *k, float *t, size_t cap, size_t *n) {
-  if (!sc || !sc->debug_valid || ray < 0 || ray >= sc->dbg_H * sc->dbg_W) return MS_ERR_INVALID_ARG;
+int ms_debug_sample_order_all(ms_scene *sc, int32_t *prim, int32_t *k, size_t cap, size_t *n) {
+  if (!sc || !sc->debug_valid || !sc->order_valid) return MS_ERR_INVALID_ARG;
   CK(cudaDeviceSynchronize());
-  uint32_t ro[2];
-  CK(cudaMemcpy(ro, (uint32_t *)sc->ray_off.p + ray, 8, cudaMemcpyDeviceToHost));
-  const size_t ns = (size_t)(ro[1] - ro[0]) * (size_t)sc->dbg_K;
+  const MsGrid &g = sc->dbg_grid;
+  const size_t K = (size_t)sc->dbg_K, nh = (size_t)sc->stats.n_intervals, ns = nh * K;
+  const size_t R = (size_t)sc->dbg_H * sc->dbg_W, Rs = (size_t)g.n_tiles * g.tile * g.tile;
   if (n) *n = ns;
   if (cap < ns) return MS_ERR_CAPACITY;
-  if (ns == 0) return MS_OK;
-  ENS(sc->dbg, ns * 12);
-  int *dp = (int *)sc->dbg.p, *dk = dp + ns;
-  float *dt = (float *)(dk + ns);
-  MsCompositeArgs ca;
-  memset(&ca, 0, sizeof(ca));
-  ca.n_rays = sc->dbg_H * sc->dbg_W; ca.K = sc->dbg_K; ca.n_feat = 0; ca.t_stop = 0.f;
-  ca.contact = sc->shape.mode == MS_MODE_CONTACT;
-  ca.tile_order = sc->dbg_tile_order;
-  ca.ray_off = (uint32_t *)sc->ray_off.p; ca.hits = (MsHit *)sc->hits.p; ca.staging = (float4 *)sc->staging.p;
-  CK(ms_sample_order(ca, ray, dp, dk, dt, 0));
-  CK(cudaDeviceSynchronize());
-  if (prim) CK(cudaMemcpy(prim, dp, ns * 4, cudaMemcpyDeviceToHost));
-  if (k) CK(cudaMemcpy(k, dk, ns * 4, cudaMemcpyDeviceToHost));
-  if (t) CK(cudaMemcpy(t, dt, ns * 4, cudaMemcpyDeviceToHost));
+  std::vector<uint32_t> ro(Rs + 1), ord(ns);
+  std::vector<MsHit> h(nh);
+  CK(cudaMemcpy(ro.data(), sc->ray_off.p, (Rs + 1) * 4, cudaMemcpyDeviceToHost));
+  if (ns) CK(cudaMemcpy(ord.data(), sc->dbg_ord.p, ns * 4, cudaMemcpyDeviceToHost));
+  if (nh) CK(cudaMemcpy(h.data(), sc->hits.p, nh * sizeof(MsHit), cudaMemcpyDeviceToHost));
+  size_t tot = 0;
+  for (size_t pix = 0; pix < R; ++pix) {
+    const uint32_t q = slot_of_pixel(g, pix);
+    const size_t base = (size_t)ro[q] * K, cnt = (size_t)(ro[q + 1] - ro[q]) * K;
+    for (size_t r = 0; r < cnt; ++r, ++tot) {
+      const uint32_t s = ord[base + r];
+      if (s >= cnt) return MS_ERR_CUDA;    // stage (e) never wrote this rank
+      if (prim) prim[tot] = h[ro[q] + s / K].prim;
+      if (k) k[tot] = (int32_t)(s % K);
+    }
+  }
   return MS_OK;
 }
 

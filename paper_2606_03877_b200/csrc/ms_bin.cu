@@ -69,8 +69,9 @@ __device__ __forceinline__ int clamp_hi(float v, int n) {
 }
 
 __global__ void project_kernel(int n, const float *__restrict__ center, const float *__restrict__ A,
-                               const float *__restrict__ M, MsCam cam, int tile, uint32_t *__restrict__ tile_count,
-                               int4 *__restrict__ rect, float *__restrict__ z_entry, float *__restrict__ oprime) {
+                               const float *__restrict__ M, MsCam cam, int tile, float eye_guard,
+                               uint32_t *__restrict__ tile_count, int4 *__restrict__ rect, float *__restrict__ z_entry,
+                               float *__restrict__ oprime, uint32_t *__restrict__ counters) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const float *mu = center + 3 * i;
@@ -102,7 +103,7 @@ __global__ void project_kernel(int n, const float *__restrict__ center, const fl
   if (z_hi > 0.0f) {
     ze = z_lo > 0.0f ? z_lo : 0.0f;
     int px0, px1, py0, py1;
-    if (z_lo <= __fmul_rn(0.01f, rz)) {
+    if (z_lo <= __fmul_rn(eye_guard, rz)) {      // Q13: touches / nears the eye plane
       px0 = 0; px1 = cam.W - 1; py0 = 0; py1 = cam.H - 1;
     } else {
       float zz = __fsub_rn(rz2, __fmul_rn(cv[2], cv[2]));
@@ -118,6 +119,10 @@ __global__ void project_kernel(int n, const float *__restrict__ center, const fl
       rc = make_int4(px0 / tile, py0 / tile, px1 / tile, py1 / tile);
       cnt = (uint32_t)(rc.z - rc.x + 1) * (uint32_t)(rc.w - rc.y + 1);
     }
+  }
+  if (cnt) {   // 64-bit pair total (a wrapped 32-bit scan would undersize every buffer) and the visible count
+    atomicAdd(reinterpret_cast<unsigned long long *>(counters + MS_CNT_PAIRS), (unsigned long long)cnt);
+    atomicAdd(&counters[MS_CNT_VISIBLE], 1u);
   }
   tile_count[i] = cnt;
   rect[i] = rc;
@@ -172,10 +177,11 @@ cudaError_t ms_prep_prims(int n, const float *center, const float *quat, const f
   return cudaGetLastError();
 }
 
-cudaError_t ms_project(int n, const float *center, const float *A, const float *M, MsCam cam, int tile, int tiles_x,
-                       int tiles_y, uint32_t *tile_count, int4 *rect, float *z_entry, float *oprime, cudaStream_t s) {
-  (void)tiles_x; (void)tiles_y;
-  project_kernel<<<(n + 127) / 128, 128, 0, s>>>(n, center, A, M, cam, tile, tile_count, rect, z_entry, oprime);
+cudaError_t ms_project(int n, const float *center, const float *A, const float *M, MsCam cam, int tile, float eye_guard,
+                       uint32_t *tile_count, int4 *rect, float *z_entry, float *oprime, uint32_t *counters,
+                       cudaStream_t s) {
+  project_kernel<<<(n + 127) / 128, 128, 0, s>>>(n, center, A, M, cam, tile, eye_guard, tile_count, rect, z_entry, oprime,
+                                                 counters);
   MS_LAUNCHED();
   return cudaGetLastError();
 }

@@ -106,22 +106,30 @@ __device__ __forceinline__ void load_hits(WarpSmem &sm, const MsHit *__restrict_
 }
 
 template <int FEAT>  // 0: rgb/alpha only; 1: + linear head features; 2: + Eq.7 slot features (contact mode, K = 1)
-__global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
+__global__ void __launch_bounds__(CW * 32, FEAT == 0 ? 12 : (FEAT == 1 ? 9 : 8)) composite_kernel(MsCompositeArgs a) {
   __shared__ WarpSmem s_all[CW];
   __shared__ float s_w[FEAT ? CW : 1][FEAT ? CAP : 1];   // weight of the window's r-th merged sample (features only)
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int ray = (int)(blockIdx.x * CW + warp);
-  if (ray >= a.n_rays) return;
+  const MsBand band = *a.band;
   WarpSmem &sm = s_all[warp];
-  const uint32_t off = a.ray_off[ray];
-  const int n = (int)(a.ray_off[ray + 1] - off);
   const int K = a.K, nf = a.n_feat;
+  uint32_t n_stopped = 0;                                   // rays of this warp that stopped before their last sample
+  // one warp per ray slot of the band (tile-major ray order: consecutive slots are neighbouring pixels of one
+  // tile, and their staged samples are consecutive runs of the band's staging buffer)
+  for (uint32_t q = band.q_lo + blockIdx.x * CW + warp; q < band.q_hi; q += gridDim.x * CW) {
+  int px, py;
+  if (!ms_slot_pixel(a.grid, q, &px, &py)) continue;     // padding slot of a tile that overhangs the image
+  const size_t ray = (size_t)py * a.grid.W + px;
+  __syncwarp();                                           // the previous ray is done with the warp's shared memory
+  const uint32_t off = a.ray_off[q];
+  const int n = (int)(a.ray_off[q + 1] - off);
   float T = 1.0f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
   float F[MS_MAX_OUT / 32] = {0.f, 0.f};
   float4 F4 = make_float4(0.f, 0.f, 0.f, 0.f);   // n_feat == 32: channels 4*(lane%8)..+3 of the samples of lane group lane/8
   if (n > 0) {
     const MsHit *hits = a.hits + off;
-    const float4 *stg = a.staging + (size_t)off * (size_t)K;
+    const size_t loc = (size_t)(off - band.slot0);        // the ray's first hit inside the band's staging buffers
+    const float4 *stg = a.staging + loc * (size_t)K;
     const uint32_t S = (uint32_t)n * (uint32_t)K;
     if (FEAT != 1 && K == 1 && n <= 32) {
       // One sample per hit and at most one hit per lane (the contact-point mode's usual ray): lane j holds hit j,
@@ -140,7 +148,10 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
         rank += (j != lane && precedes(t2, t, p2 < prim)) ? 1u : 0u;
       }
       if (a.tile_order) rank = (uint32_t)lane;      // the shared per-tile order: the hits as stage (c) wrote them
-      if (lane < n) sm.ord[rank] = (uint32_t)lane;
+      if (lane < n) {
+        sm.ord[rank] = (uint32_t)lane;
+        if (a.dbg_ord) a.dbg_ord[(size_t)off + rank] = (uint32_t)lane;
+      }
       __syncwarp();
       const bool valid = lane < n;
       uint32_t slot = 0;
@@ -162,17 +173,18 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
       const float w = (valid && lane <= last) ? excl * (1.0f - v.w) : 0.f;
       C0 = w * v.x; C1 = w * v.y; C2 = w * v.z;
       T = __shfl_sync(FULL, p, stop ? last : 31);
+      n_stopped += (stop && last + 1 < n) ? 1u : 0u;
       if (FEAT == 2 && valid) {
-        const float4 g = __ldg(a.gates + off + slot);
-        a.coef[off + slot] = make_float4(w * g.x, w * g.y, w * g.z, w * g.w);
+        const float4 g = __ldg(a.gates + loc + slot);
+        a.coef[loc + slot] = make_float4(w * g.x, w * g.y, w * g.z, w * g.w);
       }
     } else {
     load_hits(sm, hits, n, K, lane, a.contact);
     if (FEAT == 2 && S > (uint32_t)CAP)   // a ray that stops early leaves its later windows unvisited: their coefficients are 0
-      for (uint32_t s = lane; s < S; s += 32) a.coef[off + s] = make_float4(0.f, 0.f, 0.f, 0.f);
+      for (uint32_t s = lane; s < S; s += 32) a.coef[loc + s] = make_float4(0.f, 0.f, 0.f, 0.f);
     __syncwarp();
     bool stopped = false;
-    for (uint32_t r0 = 0; r0 < S && !stopped; r0 += CAP) {
+    for (uint32_t r0 = 0; r0 < S && (!stopped || a.dbg_ord); r0 += CAP) {
       const uint32_t cnt = S - r0 < (uint32_t)CAP ? S - r0 : (uint32_t)CAP;
       // ---- rank pass: ord[] (and, for a multi-window ray, val[] by rank) ----
       int h = lane / K, k = lane - h * K;
@@ -180,11 +192,15 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
       for (uint32_t s = lane; s < S; s += 32) {
         float t;
         const uint32_t rk = (a.tile_order ? s : sample_rank(sm, hits, n, K, h, k, &t, a.contact)) - r0;
-        if (rk < cnt) sm.ord[rk] = s;
+        if (rk < cnt) {
+          sm.ord[rk] = s;
+          if (a.dbg_ord) a.dbg_ord[(size_t)off * (size_t)K + r0 + rk] = s;
+        }
         h += dh; k += dk;
         if (k >= K) { k -= K; ++h; }
       }
       __syncwarp();
+      if (stopped) continue;                       // MS_FLAG_KEEP_ORDER: the windows behind the stop are ranked only
       // ---- composite the window: lane l takes the l-th run of CH consecutive merged samples ----
       // One product scan over the lanes' run products gives every lane its entry transmittance; the
       // run itself is sequential (T <- T e).  The first sample, in merged order, whose T drops
@@ -219,6 +235,7 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
         done = __shfl_sync(FULL, lstop, ls) + 1u;
         T = __shfl_sync(FULL, Tl, ls);
         stopped = true;
+        n_stopped += (r0 + done < S) ? 1u : 0u;
       } else {
         T = __shfl_sync(FULL, Tl, 31);             // lane 31 leaves with T times the product of the whole window
       }
@@ -227,8 +244,8 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
         // Eq.7: F = sum_i (T_i alpha_i) sum_k g_ik e_ik.  This kernel only turns every hit's gates into
         // its coefficients (T alpha) g_k; slot_feature_kernel sums the embeddings (the sum's order is free).
         __syncwarp();
-        const float4 *gates = a.gates + off;
-        float4 *coef = a.coef + off;
+        const float4 *gates = a.gates + loc;
+        float4 *coef = a.coef + loc;
         for (uint32_t r = lane; r < cnt; r += 32) {
           const uint32_t s = sm.ord[r];
           const float w = r < done ? s_w[FEAT ? warp : 0][FEAT ? r : 0] : 0.0f;
@@ -238,7 +255,7 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
       }
       if (FEAT == 1) {
         __syncwarp();
-        const float *fbase = a.staging_feat + (size_t)off * (size_t)K * (size_t)nf;
+        const float *fbase = a.staging_feat + loc * (size_t)K * (size_t)nf;
         if (nf == 32) {
           // lane group g = lane/8 takes sample r+g, lane%8 takes channels 4*(lane%8)..+3: one warp
           // load covers four 128 B rows; four loads in flight per lane before the FMAs.
@@ -285,7 +302,7 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
       C2 += __shfl_xor_sync(FULL, C2, o);
     }
   }
-  if (lane < 3) a.out_rgb[3 * (size_t)ray + lane] = lane == 0 ? C0 : (lane == 1 ? C1 : C2);
+  if (lane < 3) a.out_rgb[3 * ray + lane] = lane == 0 ? C0 : (lane == 1 ? C1 : C2);
   if (lane == 3) a.out_alpha[ray] = 1.0f - T;
   if (FEAT == 1) {
     if (nf == 32) {
@@ -294,15 +311,17 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
         F4.x += __shfl_xor_sync(FULL, F4.x, o); F4.y += __shfl_xor_sync(FULL, F4.y, o);
         F4.z += __shfl_xor_sync(FULL, F4.z, o); F4.w += __shfl_xor_sync(FULL, F4.w, o);
       }
-      if (lane < 8) reinterpret_cast<float4 *>(a.out_feat + (size_t)ray * 32)[lane] = F4;
+      if (lane < 8) reinterpret_cast<float4 *>(a.out_feat + ray * 32)[lane] = F4;
     } else {
 #pragma unroll
-      for (int q = 0; q < MS_MAX_OUT / 32; ++q) {
-        const int c = lane + 32 * q;
-        if (c < nf) a.out_feat[(size_t)ray * nf + c] = F[q];
+      for (int q2 = 0; q2 < MS_MAX_OUT / 32; ++q2) {
+        const int c = lane + 32 * q2;
+        if (c < nf) a.out_feat[ray * nf + c] = F[q2];
       }
     }
   }
+  }
+  if (lane == 0 && n_stopped && a.counters) atomicAdd(&a.counters[MS_CNT_STOPPED_RAYS], n_stopped);
 }
 
 // Eq.7 features: F[ray] = sum over the ray's hits of coef_k e_k[prim], coef = (T alpha) g from
@@ -313,11 +332,17 @@ __global__ void __launch_bounds__(CW * 32) composite_kernel(MsCompositeArgs a) {
 template <int R>
 __global__ void __launch_bounds__(CW * 32) slot_feature_kernel(MsCompositeArgs a) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const long long grp = (long long)blockIdx.x * CW + warp;
-  if (grp * R >= a.n_rays) return;
-  long long ray_of[R];
+  const MsBand band = *a.band;
+  // groups of R consecutive ray slots (R divides the tile edge: one tile row)
+  for (uint32_t q0 = band.q_lo + (blockIdx.x * CW + warp) * R; q0 < band.q_hi; q0 += gridDim.x * CW * R) {
+  long long ray_of[R];     // output pixel index, -1 for a padding slot
+  uint32_t slot_q[R];
 #pragma unroll
-  for (int r = 0; r < R; ++r) ray_of[r] = grp * R + r < a.n_rays ? grp * R + r : -1;
+  for (int r = 0; r < R; ++r) {
+    int px, py;
+    slot_q[r] = q0 + r;
+    ray_of[r] = (q0 + r < band.q_hi && ms_slot_pixel(a.grid, q0 + r, &px, &py)) ? (long long)py * a.grid.W + px : -1;
+  }
   const int cf4 = a.c_f >> 2, nq = a.c_f >> 7;
   float4 F[R][4];
   int prim[R], nh[R];
@@ -329,15 +354,15 @@ __global__ void __launch_bounds__(CW * 32) slot_feature_kernel(MsCompositeArgs a
 #pragma unroll
     for (int q = 0; q < 4; ++q) F[r][q] = make_float4(0.f, 0.f, 0.f, 0.f);
     const bool live = ray_of[r] >= 0;
-    off[r] = live ? a.ray_off[ray_of[r]] : 0u;
-    nh[r] = live ? (int)(a.ray_off[ray_of[r] + 1] - off[r]) : 0;
+    off[r] = live ? a.ray_off[slot_q[r]] : 0u;
+    nh[r] = live ? (int)(a.ray_off[slot_q[r] + 1] - off[r]) : 0;
     big |= nh[r] > 32;
     used[r] = 0u;
     prim[r] = -1;
     cf[r] = make_float4(0.f, 0.f, 0.f, 0.f);
     if (lane < nh[r] && nh[r] <= 32) {
       prim[r] = __ldg(&a.hits[off[r] + lane].prim);
-      cf[r] = __ldg(a.coef + off[r] + lane);
+      cf[r] = __ldg(a.coef + (off[r] - band.slot0) + lane);
     }
   }
   auto add = [&](float4 (&Fr)[4], const float4 c, const float4 *e) {
@@ -395,7 +420,7 @@ __global__ void __launch_bounds__(CW * 32) slot_feature_kernel(MsCompositeArgs a
     for (int r = 0; r < R; ++r)
       for (int j = 0; j < nh[r]; ++j) {
         const int p = __ldg(&a.hits[off[r] + j].prim);
-        add(F[r], __ldg(a.coef + off[r] + j), reinterpret_cast<const float4 *>(a.slots + (size_t)p * 4 * (size_t)a.c_f) + lane);
+        add(F[r], __ldg(a.coef + (off[r] - band.slot0) + j), reinterpret_cast<const float4 *>(a.slots + (size_t)p * 4 * (size_t)a.c_f) + lane);
       }
   }
 #pragma unroll
@@ -404,50 +429,35 @@ __global__ void __launch_bounds__(CW * 32) slot_feature_kernel(MsCompositeArgs a
 #pragma unroll
       for (int q = 0; q < 4; ++q)
         if (q < nq) reinterpret_cast<float4 *>(a.out_feat + (size_t)ray_of[r] * a.c_f)[lane + 32 * q] = F[r][q];
-}
-
-// parity introspection: the merged order of one ray, written by rank (NS: "sample ordering bit-exact")
-__global__ void sample_order_kernel(MsCompositeArgs a, int ray, int *dbg_prim, int *dbg_k, float *dbg_t) {
-  __shared__ WarpSmem sm;
-  const int lane = threadIdx.x;
-  const uint32_t off = a.ray_off[ray];
-  const int n = (int)(a.ray_off[ray + 1] - off);
-  const int K = a.K;
-  const MsHit *hits = a.hits + off;
-  load_hits(sm, hits, n, K, lane, a.contact);
-  __syncwarp();
-  const uint32_t S = (uint32_t)n * (uint32_t)K;
-  for (uint32_t s = lane; s < S; s += 32) {
-    const int h = (int)(s / (uint32_t)K), k = (int)(s - (uint32_t)h * (uint32_t)K);
-    float t;
-    uint32_t rk = sample_rank(sm, hits, n, K, h, k, &t, a.contact);
-    if (a.tile_order) rk = s;   // the shared per-tile order: the hits as stage (c) wrote them
-    dbg_prim[rk] = hits[h].prim; dbg_k[rk] = k; dbg_t[rk] = t;
   }
 }
 
 }  // namespace
 
 cudaError_t ms_composite(const MsCompositeArgs &a, cudaStream_t s) {
-  if (a.n_rays == 0) return cudaSuccess;
-  const unsigned grid = (unsigned)((a.n_rays + CW - 1) / CW);
+  if (a.grid.n_tiles == 0) return cudaSuccess;
+  static int n_sm = 0;
+  if (n_sm == 0) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+  }
+  // persistent warps walking the band's ray slots (the band's extent lives on the device)
+  const size_t slots = (size_t)a.grid.n_tiles * a.grid.tile * a.grid.tile;
+  unsigned grid = (unsigned)n_sm * 12u;
+  if ((slots + CW - 1) / CW < grid) grid = (unsigned)((slots + CW - 1) / CW);
   const bool feat = a.n_feat > 0 && a.out_feat && a.staging_feat;
-  const bool slots = a.c_f > 0 && a.out_feat && a.gates && a.coef && a.slots && a.K == 1;
-  if (slots) composite_kernel<2><<<grid, CW * 32, 0, s>>>(a);
+  const bool slot_feat = a.c_f > 0 && a.out_feat && a.gates && a.coef && a.slots && a.K == 1;
+  if (slot_feat) composite_kernel<2><<<grid, CW * 32, 0, s>>>(a);
   else if (!feat) composite_kernel<0><<<grid, CW * 32, 0, s>>>(a);
   else composite_kernel<1><<<grid, CW * 32, 0, s>>>(a);
   MS_LAUNCHED();
-  if (slots) {
+  if (slot_feat) {
     constexpr int R = 4;
-    const long long groups = ((long long)a.n_rays + R - 1) / R;
-    slot_feature_kernel<R><<<(unsigned)((groups + CW - 1) / CW), CW * 32, 0, s>>>(a);
+    unsigned g2 = (unsigned)n_sm * 12u;
+    if ((slots / R + CW - 1) / CW < g2) g2 = (unsigned)((slots / R + CW - 1) / CW);
+    slot_feature_kernel<R><<<g2, CW * 32, 0, s>>>(a);
     MS_LAUNCHED();
   }
-  return cudaGetLastError();
-}
-
-cudaError_t ms_sample_order(const MsCompositeArgs &a, int ray, int *prim, int *k, float *t, cudaStream_t s) {
-  sample_order_kernel<<<1, 32, 0, s>>>(a, ray, prim, k, t);
-  MS_LAUNCHED();
   return cudaGetLastError();
 }

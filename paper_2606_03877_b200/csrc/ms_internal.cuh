@@ -22,7 +22,7 @@ struct MsCam {
 
 // interval of one (ray, primitive) hit in the primitive-major list consumed by stage (d)
 struct __align__(16) MsInterval {
-  int ray;      // y*W + x
+  int ray;      // ray slot q (tile-major ray order, ms_ray_slot)
   float t_in;
   float delta;  // (t_out - t_in)/K
   int slot;     // global hit index = ray_off[ray] + h ; sample k lives at staging[slot*K + k]
@@ -35,13 +35,80 @@ struct __align__(16) MsHit {
   int prim;
   float t_in;
   float delta;
-  int pad;
+  int wave;     // depth wave of the (tile, primitive) pair the hit comes from (0 when waves are off)
 };
 
 struct MsMlpShape {
   int n_freq, use_viewdir, n_hidden, width, n_feat;
   int in_dim, out_dim, n_layers, params;
   int mode;  // MS_MODE_LOCAL | MS_MODE_CONTACT
+};
+
+// ---------------------------------------------------------------------------------------------
+// tile-major ray order, bands and depth waves (DESIGN.md Sec.6 "Bands and waves"; S:Sec.8(f) NEXT-3)
+// ---------------------------------------------------------------------------------------------
+// Tiles are enumerated macro-tile by macro-tile (G x G tiles, row-major inside), so that a run of
+// consecutive tiles is a compact screen region whose primitives overlap; ray slot q = pos*T*T + ly*T + lx.
+struct MsGrid {
+  int tile, tiles_x, tiles_y, n_tiles, G;   // tile edge, tile grid, macro-tile edge in tiles
+  int W, H;
+};
+__host__ __device__ __forceinline__ int ms_tile_pos(const MsGrid &g, int tx, int ty) {
+  const int mx = tx / g.G, my = ty / g.G;
+  const int h = g.tiles_y - my * g.G < g.G ? g.tiles_y - my * g.G : g.G;
+  const int w = g.tiles_x - mx * g.G < g.G ? g.tiles_x - mx * g.G : g.G;
+  return my * g.G * g.tiles_x + mx * g.G * h + (ty - my * g.G) * w + (tx - mx * g.G);
+}
+__host__ __device__ __forceinline__ void ms_pos_tile(const MsGrid &g, int pos, int *tx, int *ty) {
+  const int my = pos / (g.G * g.tiles_x);
+  const int rem = pos - my * g.G * g.tiles_x;
+  const int h = g.tiles_y - my * g.G < g.G ? g.tiles_y - my * g.G : g.G;
+  const int mcols = (g.tiles_x + g.G - 1) / g.G;
+  int mx = rem / (g.G * h);
+  if (mx > mcols - 1) mx = mcols - 1;
+  const int rem2 = rem - mx * g.G * h;
+  const int w = g.tiles_x - mx * g.G < g.G ? g.tiles_x - mx * g.G : g.G;
+  *ty = my * g.G + rem2 / w;
+  *tx = mx * g.G + rem2 % w;
+}
+// pixel (x, y) of ray slot q; false for the padding slots of tiles that overhang the image
+__host__ __device__ __forceinline__ bool ms_slot_pixel(const MsGrid &g, uint32_t q, int *x, int *y) {
+  const int T2 = g.tile * g.tile;
+  const int pos = (int)(q / (uint32_t)T2), l = (int)(q - (uint32_t)pos * (uint32_t)T2);
+  int tx, ty;
+  ms_pos_tile(g, pos, &tx, &ty);
+  *x = tx * g.tile + l % g.tile;
+  *y = ty * g.tile + l / g.tile;
+  return *x < g.W && *y < g.H;
+}
+
+// Depth waves: wave w covers the ranks [ms_wave_first(w), ms_wave_first(w + 1)) of a tile's sorted list
+// (C, C, 2C, 4C, ... entries; the last wave takes the rest).  C == 0: a single wave.
+#define MS_MAX_WAVES 6
+__host__ __device__ __forceinline__ uint32_t ms_wave_first(int w, int C) {
+  return w <= 0 ? 0u : (uint32_t)C << (w - 1);
+}
+__host__ __device__ __forceinline__ int ms_wave_of_rank(uint32_t r, int C) {
+  if (C <= 0 || r < (uint32_t)C) return 0;
+  int w = 1;
+  while (w < MS_MAX_WAVES - 1 && r >= ((uint32_t)C << w)) ++w;
+  return w;
+}
+
+// One band = a run of consecutive tiles (in ms_tile_pos order) whose hits fill the staging budget.
+struct MsBand {
+  uint32_t q_lo, q_hi;   // ray slots of the band
+  uint32_t slot0;        // first hit slot of the band: sample k of hit slot lives at staging[(slot - slot0) * K + k]
+  uint32_t pad;
+};
+// Segment tables of stage (d): segment g = the intervals of one primitive inside one (band, wave).
+struct MsSegs {
+  const uint32_t *iv0;      // [n_seg + 1] first interval of the segment
+  const uint32_t *cnt;      // [n_seg] intervals of the segment, or NULL: iv0[g + 1] - iv0[g]
+  const uint32_t *blk_off;  // [n_seg + 1] exclusive scan of the segments' 128-row block counts (any base)
+  const uint32_t *prim;     // [n_seg] primitive of the segment, or NULL: the segment index itself
+  const uint2 *range;       // device: segments [x, y) of this launch
+  const MsBand *band;       // device: the launch's band
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -162,8 +229,8 @@ cudaError_t ms_radix_sort_u64(uint64_t *a, uint64_t *b, size_t n, int first_bit,
 cudaError_t ms_prep_prims(int n, const float *center, const float *quat, const float *scale, float *A, float *M,
                           int *bad, cudaStream_t s);
 cudaError_t ms_project(int n, const float *center, const float *A, const float *M, MsCam cam, int tile,
-                       int tiles_x, int tiles_y, uint32_t *tile_count, int4 *rect, float *z_entry, float *oprime,
-                       cudaStream_t s);
+                       float eye_guard, uint32_t *tile_count, int4 *rect, float *z_entry, float *oprime,
+                       uint32_t *counters, cudaStream_t s);
 // tile_order != 0: the depth field of the key is t*_{i,c} of the tile-centre ray (needs cam, tile, A, oprime)
 cudaError_t ms_emit_keys(int n, const uint32_t *emit_off, const int4 *rect, const float *z_entry, int tiles_x,
                          int prim_bits, uint64_t *keys, int tile_order, MsCam cam, int tile, const float *A,
@@ -174,57 +241,125 @@ cudaError_t ms_tile_ranges(const uint64_t *keys, size_t n_pairs, int n_tiles, in
 // ms_isect.cu
 struct MsIsectArgs {
   MsCam cam;
-  int tile, tiles_x, n_tiles, K, prim_bits, contact;
+  MsGrid grid;
+  int K, prim_bits, contact, wave_c;
   const uint64_t *keys;        // sorted
   const uint32_t *tile_start;  // [n_tiles+1]
   const float *A;              // [N][9]
   const float *oprime;         // [N][3]
-  const int4 *rect;            // [N] tile rect (tx0, ty0, tx1, ty1)
-  const uint32_t *emit_off;    // [N+1]
-  uint32_t *pair_hits;         // [P]   (count pass: out)   indexed by emission index
-  uint32_t *ray_hits;          // [R]   (count pass: out)
-  const uint32_t *pair_off;    // [P+1] (fill pass: in)
-  const uint32_t *ray_off;     // [R+1] (fill pass: in)
-  MsInterval *intervals;       // [n_hits] primitive-major (fill pass: out)
-  MsHit *hits;                 // [n_hits] ray-major       (fill pass: out)
+  uint32_t *pair_hits;         // [P]    (count pass: out)   indexed by tile-list index
+  uint32_t *ray_hits;          // [R']   (count pass: out)   indexed by ray slot
+  const uint32_t *slot_of;     // [P]    (fill pass: in)     tile-list index -> pair slot of the prim-major order
+  const uint32_t *pair_off;    // [P+1]  (fill pass: in)     by pair slot
+  const uint32_t *ray_off;     // [R'+1] (fill pass: in)
+  MsInterval *intervals;       // [n_hits] segment-major (fill pass: out)
+  MsHit *hits;                 // [n_hits] ray-major      (fill pass: out)
 };
 cudaError_t ms_isect_count(const MsIsectArgs &a, cudaStream_t s);
 cudaError_t ms_isect_fill(const MsIsectArgs &a, cudaStream_t s);
-// per-primitive interval starts and 128-row block counts
-cudaError_t ms_prim_blocks(int n, const uint32_t *emit_off, const uint32_t *pair_off, int K, uint32_t *prim_start,
-                           uint32_t *prim_blocks, cudaStream_t s);
+
+// ms_band.cu: orders the (tile, primitive) pairs for stage (d) and cuts the frame into bands and waves
+struct MsBandArgs {
+  MsGrid grid;
+  int K, prim_bits, n_prims, wave_c, n_bands;
+  uint32_t cap_hits;           // band budget in hits
+  size_t P;
+  const uint64_t *keys;        // sorted tile lists
+  const uint32_t *tile_start;
+  const uint32_t *ray_off;     // [R'+1]
+  const uint32_t *emit_off;    // [N+1]  (single-band path)
+  const int4 *rect;            // [N]    (single-band path)
+  const uint32_t *pair_hits_i; // [P] by tile-list index
+  uint64_t *key2_a, *key2_b;   // [P]
+  uint32_t *sort_scratch;
+  uint32_t *scan_scratch;
+  uint32_t *slot_of;           // [P]
+  uint32_t *pair_hits_j;       // [P+1] by pair slot
+  uint32_t *pair_off;          // [P+2]
+  uint32_t *flags, *gid;       // [P+2] group boundary flags and their exclusive scan
+  uint32_t *grp_key;           // [n_seg_cap] (band, wave, prim) of segment g
+  uint32_t *grp_prim;          // [n_seg_cap]
+  uint32_t *grp_iv0;           // [n_seg_cap + 1]
+  uint32_t *grp_blocks;        // [n_seg_cap + 1]
+  uint32_t *blk_off;           // [n_seg_cap + 2]
+  uint2 *bw;                   // [n_bands * MS_MAX_WAVES] segment range of (band, wave)
+  MsBand *bands;               // [n_bands]
+  uint32_t *counters;          // device counters (MsCounter)
+};
+// device counters of a view (uint32 each; HITS and PAIRS are 64-bit little-endian pairs, so a total that wrapped the
+// 32-bit scans is seen)
+enum MsCounter { MS_CNT_SEGS = 0, MS_CNT_BLOCKS, MS_CNT_HITS, MS_CNT_HITS_HI, MS_CNT_PAIRS, MS_CNT_PAIRS_HI,
+                 MS_CNT_MAX_TILE_HITS, MS_CNT_MAX_LIST, MS_CNT_SKIPPED, MS_CNT_DEAD_RAYS, MS_CNT_VISIBLE,
+                 MS_CNT_STOPPED_RAYS, MS_CNT_N };
+// after the ray_off scan: the hit total (64-bit), the largest tile's hit count and the longest tile list into counters
+cudaError_t ms_tile_stats(const MsGrid &g, const uint32_t *ray_off, const uint32_t *tile_start, uint32_t *counters,
+                          cudaStream_t s);
+// one band, one wave: segments = primitives in emission order (the layout of small frames)
+cudaError_t ms_order_single(const MsBandArgs &a, cudaStream_t s);
+// bands x waves: pairs sorted by (band, wave, primitive), segments = runs of equal (band, wave, primitive)
+cudaError_t ms_order_banded(const MsBandArgs &a, cudaStream_t s);
+// bits of the (band, wave, primitive, pair index) sort key; the (band, wave, primitive) part must fit 32 bits
+int ms_banded_key_bits(size_t P, int prim_bits, int n_bands, int *group_bits);
+
+// depth waves (real early termination): before wave w >= 1 of a band, rays whose transmittance over the samples
+// in front of the wave's nearest possible sample is already below t_stop/2 are dropped, the wave's interval lists
+// are compacted and its block offsets rebuilt
+struct MsWaveArgs {
+  MsGrid grid;
+  int K, prim_bits, wave_c, band, wave, contact;
+  float t_stop, margin;
+  const uint64_t *keys;
+  const uint32_t *tile_start;
+  const uint32_t *ray_off;
+  const MsHit *hits;
+  const float4 *staging;
+  const MsBand *bands;
+  const uint2 *bw;
+  uint8_t *alive;              // [R'] 1 = the ray still needs its later hits
+  MsInterval *intervals;       // compacted in place
+  const uint32_t *grp_iv0;
+  uint32_t *grp_cnt_c;         // [n_seg_cap] compacted interval count
+  uint32_t *grp_blocks_c;      // [n_seg_cap] compacted 128-row block count
+  uint32_t *blk_off_c;         // [n_seg_cap + 2] block offsets of the compacted wave (relative to its first segment)
+  uint32_t *counters;
+  int n_sm;
+};
+cudaError_t ms_wave_prepare(const MsWaveArgs &a, cudaStream_t s);
 
 // ms_mlp_f32.cu
 struct MsMlpArgs {
   MsMlpShape shape;
   MsCam cam;
-  int K, n_prims;
+  int K;
+  float falloff;                  // contact mode: g = exp(-falloff |p* - mu|^2_Lambda)
   const float *center, *A;
   const float *weights_f32;       // [N][params]
-  const uint32_t *prim_start;     // [N+1] interval offsets
-  const uint32_t *blk_off;        // [N+1] row-block offsets
-  uint32_t n_blocks;
+  MsSegs segs;
+  uint32_t n_blocks_hint;         // blocks of the launch if the host knows them, else 0
   const MsInterval *intervals;
-  float4 *staging;                // [n_hits*K] (r,g,b,e)
-  float *staging_feat;            // [n_hits*K][n_feat] or NULL
-  float4 *staging_gate;           // [n_hits] slot gates g_k of Eq.7 (contact mode) or NULL
+  float4 *staging;                // band-local: [(slot - slot0)*K + k] (r,g,b,e)
+  float *staging_feat;            // same indexing x n_feat, or NULL
+  float4 *staging_gate;           // slot gates g_k of Eq.7 (contact mode) or NULL
 };
 cudaError_t ms_mlp_f32(const MsMlpArgs &a, cudaStream_t s);
 
 // ms_composite.cu
 struct MsCompositeArgs {
-  int n_rays, K, n_feat, contact;
+  MsGrid grid;
+  int K, n_feat, contact;
   int tile_order;        // contact mode: the hits are already in the tile's shared order -- no per-ray merge
   float t_stop;
-  const uint32_t *ray_off;  // [R+1]
+  const MsBand *band;    // device: ray slots and staging origin of this launch
+  const uint32_t *ray_off;  // [R'+1]
   const MsHit *hits;
   const float4 *staging;
   const float *staging_feat;
-  const float4 *gates;   // [n_hits] slot gates (Eq.7) or NULL
-  float4 *coef;          // [n_hits] (T alpha) g_k per hit: composite_kernel<2> -> slot_feature_kernel
+  const float4 *gates;   // slot gates (Eq.7) or NULL
+  float4 *coef;          // (T alpha) g_k per hit: composite_kernel<2> -> slot_feature_kernel
   const float *slots;    // [N][4][c_f] slot embeddings
   int c_f;
+  uint32_t *counters;    // MS_CNT_STOPPED_RAYS
+  uint32_t *dbg_ord;     // MS_FLAG_KEEP_ORDER: [n_hits*K] sample index (h*K + k) by (hit slot of the ray)*K + rank
   float *out_rgb, *out_alpha, *out_feat;
 };
 cudaError_t ms_composite(const MsCompositeArgs &a, cudaStream_t s);
-cudaError_t ms_sample_order(const MsCompositeArgs &a, int ray, int *prim, int *k, float *t, cudaStream_t s);

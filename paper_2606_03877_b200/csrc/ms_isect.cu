@@ -1,12 +1,12 @@
 // ms_isect.cu -- stage (c): per-tile ray/ellipsoid intersection (NS (c)).  One CTA per tile,
 // one thread per pixel; the CTA walks the tile's sorted list and every thread tests its ray
 // against the primitive (canonical fp32 chord).  Two passes:
-//   count: hits per ray and hits per (tile, primitive) pair
-//   fill : after two exclusive scans, each hit is written twice --
-//          ray-major   hits[ray_off[ray] + h]           (stage (e) merges these per ray)
-//          prim-major  intervals[pair_off[pair] + rank]  (stage (d) batches samples by primitive)
-// The prim-major order is (primitive, tile row-major inside its rect, pixel index in tile):
-// deterministic (the only atomics are integer hit counters in shared memory).  Bytes: ~48 B written per
+//   count: hits per ray slot and hits per (tile, primitive) pair (by tile-list index)
+//   fill : after the scans and the pair ordering of ms_band.cu, each hit is written twice --
+//          ray-major      hits[ray_off[q] + h]                       (stage (e) merges these per ray)
+//          segment-major  intervals[pair_off[slot_of[i]] + rank]     (stage (d) batches samples by primitive)
+// Rays are numbered tile by tile (ms_ray_slot order), so a band of tiles owns a contiguous run of hit slots.
+// Deterministic (the only atomics are integer hit counters in shared memory).  Bytes: ~48 B written per
 // hit; reads are L1/L2-resident lists.
 #include "ms_internal.cuh"
 
@@ -20,16 +20,15 @@ __global__ void isect_kernel(MsIsectArgs a) {
   // in shared memory by the first 32 threads: no dependent global load and no block barrier per primitive.
   __shared__ float sA[IS_CHUNK][12];        // A (9), o' = A (o - mu) (3)
   __shared__ int sPrim[IS_CHUNK];
-  __shared__ uint32_t sEmit[IS_CHUNK];      // emission index of the (tile, primitive) pair
-  __shared__ uint32_t sBase[IS_CHUNK];      // FILL: pair_off[emit]
+  __shared__ uint32_t sBase[IS_CHUNK];      // FILL: pair_off[slot_of[i]]
   __shared__ uint32_t sCnt[IS_CHUNK][33];   // hits of the pair per warp (count pass: [c][32] = total)
-  const int T = a.tile;
+  const int T = a.grid.tile;
   const int tile_id = blockIdx.x;
-  const int tile_x = tile_id % a.tiles_x, tile_y = tile_id / a.tiles_x;
+  const int tile_x = tile_id % a.grid.tiles_x, tile_y = tile_id / a.grid.tiles_x;
   const int lx = threadIdx.x % T, ly = threadIdx.x / T;
   const int x = tile_x * T + lx, y = tile_y * T + ly;
   const bool valid = x < a.cam.W && y < a.cam.H;
-  const int ray = y * a.cam.W + x;
+  const uint32_t q = (uint32_t)ms_tile_pos(a.grid, tile_x, tile_y) * (uint32_t)(T * T) + threadIdx.x;   // ray slot
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint32_t lt = (1u << lane) - 1u;
   float d[3] = {0.f, 0.f, 1.f};
@@ -39,7 +38,7 @@ __global__ void isect_kernel(MsIsectArgs a) {
   const uint32_t beg = a.tile_start[tile_id], end = a.tile_start[tile_id + 1];
   uint32_t my_hits = 0;
   uint32_t ray_base = 0;
-  if (FILL && valid) ray_base = a.ray_off[ray];
+  if (FILL) ray_base = a.ray_off[q];
   for (uint32_t base = beg; base < end; base += IS_CHUNK) {
     const int nc = (int)(end - base < (uint32_t)IS_CHUNK ? end - base : (uint32_t)IS_CHUNK);
     __syncthreads();                        // the previous chunk is done with the staging arrays
@@ -49,14 +48,11 @@ __global__ void isect_kernel(MsIsectArgs a) {
       const float *A = a.A + 9 * (size_t)prim;
       const float *op = a.oprime + 3 * (size_t)prim;
 #pragma unroll
-      for (int q = 0; q < 9; ++q) sA[c][q] = __ldg(A + q);
+      for (int qq = 0; qq < 9; ++qq) sA[c][qq] = __ldg(A + qq);
 #pragma unroll
-      for (int q = 0; q < 3; ++q) sA[c][9 + q] = __ldg(op + q);
-      const int4 rc = a.rect[prim];
-      const uint32_t emit = a.emit_off[prim] + (uint32_t)((tile_y - rc.y) * (rc.z - rc.x + 1) + (tile_x - rc.x));
+      for (int qq = 0; qq < 3; ++qq) sA[c][9 + qq] = __ldg(op + qq);
       sPrim[c] = prim;
-      sEmit[c] = emit;
-      if (FILL) sBase[c] = a.pair_off[emit];
+      if (FILL) sBase[c] = a.pair_off[a.slot_of[base + c]];
       if (!FILL) sCnt[c][32] = 0u;
     }
     __syncthreads();
@@ -76,7 +72,7 @@ __global__ void isect_kernel(MsIsectArgs a) {
     }
     __syncthreads();
     if (!FILL) {
-      if ((int)threadIdx.x < nc) a.pair_hits[sEmit[threadIdx.x]] = sCnt[threadIdx.x][32];
+      if ((int)threadIdx.x < nc) a.pair_hits[base + threadIdx.x] = sCnt[threadIdx.x][32];
       my_hits += __popc(hitmask);
     } else {
       // pass 2: the hits are written in list order; rank inside the pair = hits of lower warps + lower lanes
@@ -90,52 +86,33 @@ __global__ void isect_kernel(MsIsectArgs a) {
           for (int w = 0; w < warp; ++w) rank += sCnt[c][w];
           const uint32_t slot = ray_base + my_hits;
           MsInterval iv;
-          iv.ray = ray; iv.t_in = t_in; iv.delta = delta; iv.slot = (int)slot;
+          iv.ray = (int)q; iv.t_in = t_in; iv.delta = delta; iv.slot = (int)slot;
           iv.dx = d[0]; iv.dy = d[1]; iv.dz = d[2]; iv.pad = 0;
           a.intervals[sBase[c] + rank] = iv;
           MsHit h;
-          h.prim = sPrim[c]; h.t_in = t_in; h.delta = delta; h.pad = 0;
+          h.prim = sPrim[c]; h.t_in = t_in; h.delta = delta;
+          h.wave = ms_wave_of_rank(base + (uint32_t)c - beg, a.wave_c);
           a.hits[slot] = h;
           ++my_hits;
         }
       }
     }
   }
-  if (!FILL && valid) a.ray_hits[ray] = my_hits;
-}
-
-__global__ void prim_blocks_kernel(int n, const uint32_t *__restrict__ emit_off, const uint32_t *__restrict__ pair_off,
-                                   int K, uint32_t *__restrict__ prim_start, uint32_t *__restrict__ prim_blocks) {
-  int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i > n) return;
-  uint32_t s = pair_off[emit_off[i]];
-  prim_start[i] = s;
-  if (i < n) {
-    uint32_t e = pair_off[emit_off[i + 1]];
-    uint64_t samples = (uint64_t)(e - s) * (uint64_t)K;
-    prim_blocks[i] = (uint32_t)((samples + MS_ROWS - 1) / MS_ROWS);
-  }
+  if (!FILL) a.ray_hits[q] = my_hits;    // 0 for the padding slots of an overhanging tile
 }
 
 }  // namespace
 
 cudaError_t ms_isect_count(const MsIsectArgs &a, cudaStream_t s) {
-  if (a.n_tiles == 0) return cudaSuccess;
-  isect_kernel<false><<<a.n_tiles, a.tile * a.tile, 0, s>>>(a);
+  if (a.grid.n_tiles == 0) return cudaSuccess;
+  isect_kernel<false><<<a.grid.n_tiles, a.grid.tile * a.grid.tile, 0, s>>>(a);
   MS_LAUNCHED();
   return cudaGetLastError();
 }
 
 cudaError_t ms_isect_fill(const MsIsectArgs &a, cudaStream_t s) {
-  if (a.n_tiles == 0) return cudaSuccess;
-  isect_kernel<true><<<a.n_tiles, a.tile * a.tile, 0, s>>>(a);
-  MS_LAUNCHED();
-  return cudaGetLastError();
-}
-
-cudaError_t ms_prim_blocks(int n, const uint32_t *emit_off, const uint32_t *pair_off, int K, uint32_t *prim_start,
-                           uint32_t *prim_blocks, cudaStream_t s) {
-  prim_blocks_kernel<<<(n + 1 + 127) / 128, 128, 0, s>>>(n, emit_off, pair_off, K, prim_start, prim_blocks);
+  if (a.grid.n_tiles == 0) return cudaSuccess;
+  isect_kernel<true><<<a.grid.n_tiles, a.grid.tile * a.grid.tile, 0, s>>>(a);
   MS_LAUNCHED();
   return cudaGetLastError();
 }

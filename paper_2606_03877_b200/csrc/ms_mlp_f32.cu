@@ -8,31 +8,55 @@
 
 namespace {
 
-__device__ __forceinline__ int find_prim(const uint32_t *__restrict__ blk_off, int n, uint32_t b) {
-  int lo = 0, hi = n;  // largest p with blk_off[p] <= b
+// segment of block b of the launch: largest s with bo[s] - base <= b
+__device__ __forceinline__ int find_seg(const uint32_t *__restrict__ bo, int n, uint32_t base, uint32_t b) {
+  int lo = 0, hi = n;
   while (hi - lo > 1) {
     int mid = (lo + hi) >> 1;
-    if (blk_off[mid] <= b) lo = mid; else hi = mid;
+    if (bo[mid] - base <= b) lo = mid; else hi = mid;
   }
   return lo;
 }
 
+// The launch's segments and band (device tables, ms_band.cu); every CTA walks blocks blockIdx.x, + gridDim.x, ...
+struct LaunchView {
+  uint2 r;
+  MsBand band;
+  const uint32_t *bo;
+  uint32_t base, n_blocks;
+  __device__ LaunchView(const MsSegs &sg) {
+    r = *sg.range;
+    band = *sg.band;
+    bo = sg.blk_off + r.x;
+    base = bo[0];
+    n_blocks = bo[r.y - r.x] - base;
+  }
+};
+
 __global__ void __launch_bounds__(MS_ROWS) mlp_f32_kernel(MsMlpArgs a) {
   extern __shared__ float w_s[];
-  __shared__ int s_prim;
+  __shared__ int s_seg;
   const MsMlpShape &sh = a.shape;
-  if (threadIdx.x == 0) s_prim = find_prim(a.blk_off, a.n_prims, blockIdx.x);
+  const LaunchView lv(a.segs);
+  int cur_prim = -1;
+  for (uint32_t blk = blockIdx.x; blk < lv.n_blocks; blk += gridDim.x) {
+  __syncthreads();                       // the previous block is done with w_s and s_seg
+  if (threadIdx.x == 0) s_seg = find_seg(lv.bo, (int)(lv.r.y - lv.r.x), lv.base, blk);
   __syncthreads();
-  const int prim = s_prim;
-  const float *wg = a.weights_f32 + (size_t)prim * sh.params;
-  for (int i = threadIdx.x; i < sh.params; i += blockDim.x) w_s[i] = wg[i];
+  const uint32_t g = lv.r.x + (uint32_t)s_seg;
+  const int prim = a.segs.prim ? (int)a.segs.prim[g] : (int)g;
+  if (prim != cur_prim) {
+    const float *wg = a.weights_f32 + (size_t)prim * sh.params;
+    for (int i = threadIdx.x; i < sh.params; i += blockDim.x) w_s[i] = wg[i];
+    cur_prim = prim;
+  }
   __syncthreads();
 
-  const uint32_t first = a.prim_start[prim], count = a.prim_start[prim + 1] - first;
-  const uint64_t s = (uint64_t)(blockIdx.x - a.blk_off[prim]) * MS_ROWS + threadIdx.x;
+  const uint32_t first = a.segs.iv0[g], count = a.segs.cnt ? a.segs.cnt[g] : a.segs.iv0[g + 1] - first;
+  const uint64_t s = (uint64_t)(blk - (lv.bo[s_seg] - lv.base)) * MS_ROWS + threadIdx.x;
   const uint32_t j = (uint32_t)(s / (uint32_t)a.K);
   const int k = (int)(s % (uint32_t)a.K);
-  if (j >= count) return;
+  if (j >= count) continue;
   const MsInterval iv = a.intervals[first + j];
   const float d[3] = {iv.dx, iv.dy, iv.dz};
   const bool contact = sh.mode == MS_MODE_CONTACT;
@@ -94,13 +118,14 @@ __global__ void __launch_bounds__(MS_ROWS) mlp_f32_kernel(MsMlpArgs a) {
   r.w = expf(-sigma * iv.delta);  // e = 1 - alpha
   if (contact) {  // alpha = (1 - exp(-sigma l)) g, g = exp(-(9/2) |p* - mu|^2_Lambda)  (include/mlpsplat.h)
     const float r2 = u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
-    r.w = 1.0f - (1.0f - r.w) * expf(-4.5f * r2);
+    r.w = 1.0f - (1.0f - r.w) * expf(-a.falloff * r2);
   }
-  const size_t out = (size_t)(uint32_t)iv.slot * (size_t)a.K + (size_t)k;
+  const size_t out = (size_t)((uint32_t)iv.slot - lv.band.slot0) * (size_t)a.K + (size_t)k;
   a.staging[out] = r;
   if (a.staging_gate) a.staging_gate[out] = ms_slot_gates(u);
   if (a.staging_feat)
     for (int c = 0; c < sh.n_feat; ++c) a.staging_feat[out * sh.n_feat + c] = raw[4 + c];
+  }
 }
 
 
@@ -114,19 +139,26 @@ __global__ void __launch_bounds__(MS_ROWS) mlp_f32_kernel(MsMlpArgs a) {
 template <int NH, int SPT>
 __global__ void __launch_bounds__(MS_ROWS / SPT) mlp_f32_w32_kernel(MsMlpArgs a) {
   extern __shared__ __align__(16) float w_s[];
-  __shared__ int s_prim;
+  __shared__ int s_seg;
   const MsMlpShape &sh = a.shape;
-  if (threadIdx.x == 0) s_prim = find_prim(a.blk_off, a.n_prims, blockIdx.x);
+  const LaunchView lv(a.segs);
+  int cur_prim = -1;
+  for (uint32_t blk = blockIdx.x; blk < lv.n_blocks; blk += gridDim.x) {
+  __syncthreads();                       // the previous block is done with w_s and s_seg
+  if (threadIdx.x == 0) s_seg = find_seg(lv.bo, (int)(lv.r.y - lv.r.x), lv.base, blk);
   __syncthreads();
-  const int prim = s_prim;
-  {
+  const uint32_t g = lv.r.x + (uint32_t)s_seg;
+  const int prim = a.segs.prim ? (int)a.segs.prim[g] : (int)g;
+  if (prim != cur_prim) {
     const float4 *wg = reinterpret_cast<const float4 *>(a.weights_f32 + (size_t)prim * sh.params);   // params % 4 == 0 for these shapes
     float4 *ws4 = reinterpret_cast<float4 *>(w_s);
     for (int i = threadIdx.x; i < sh.params / 4; i += blockDim.x) ws4[i] = __ldg(wg + i);
+    cur_prim = prim;
   }
   __syncthreads();
 
-  const uint32_t first = a.prim_start[prim], count = a.prim_start[prim + 1] - first;
+  const uint32_t first = a.segs.iv0[g], count = a.segs.cnt ? a.segs.cnt[g] : a.segs.iv0[g + 1] - first;
+  const uint32_t blk_in_seg = blk - (lv.bo[s_seg] - lv.base);
   const bool contact = sh.mode == MS_MODE_CONTACT;
   const float *mu = a.center + 3 * (size_t)prim;
   bool live[SPT];
@@ -135,7 +167,7 @@ __global__ void __launch_bounds__(MS_ROWS / SPT) mlp_f32_w32_kernel(MsMlpArgs a)
   float u[SPT][3], z[SPT][6];
 #pragma unroll
   for (int q = 0; q < SPT; ++q) {
-    const uint64_t s = (uint64_t)(blockIdx.x - a.blk_off[prim]) * MS_ROWS + threadIdx.x + q * (MS_ROWS / SPT);
+    const uint64_t s = (uint64_t)blk_in_seg * MS_ROWS + threadIdx.x + q * (MS_ROWS / SPT);
     const uint32_t j = (uint32_t)(s / (uint32_t)a.K);
     kk[q] = (int)(s % (uint32_t)a.K);
     live[q] = j < count;
@@ -148,7 +180,7 @@ __global__ void __launch_bounds__(MS_ROWS / SPT) mlp_f32_w32_kernel(MsMlpArgs a)
 #pragma unroll
     for (int c = 0; c < 3; ++c) z[q][3 + c] = __fsub_rn(mu[c], __fadd_rn(a.cam.o[c], __fmul_rn(t, d[c])));
   }
-  if (count == 0) return;
+  if (count == 0) continue;
 
   float acc[SPT][32];
   const int n_in = sh.in_dim;
@@ -273,9 +305,9 @@ __global__ void __launch_bounds__(MS_ROWS / SPT) mlp_f32_w32_kernel(MsMlpArgs a)
     r.w = expf(-sigma * iv[p].delta);  // e = 1 - alpha
     if (contact) {  // alpha = (1 - exp(-sigma l)) g, g = exp(-(9/2) |p* - mu|^2_Lambda)  (include/mlpsplat.h)
       const float r2 = u[p][0] * u[p][0] + u[p][1] * u[p][1] + u[p][2] * u[p][2];
-      r.w = 1.0f - (1.0f - r.w) * expf(-4.5f * r2);
+      r.w = 1.0f - (1.0f - r.w) * expf(-a.falloff * r2);
     }
-    const size_t out = (size_t)(uint32_t)iv[p].slot * (size_t)a.K + (size_t)kk[p];
+    const size_t out = (size_t)((uint32_t)iv[p].slot - lv.band.slot0) * (size_t)a.K + (size_t)kk[p];
     a.staging[out] = r;
     if (a.staging_gate) a.staging_gate[out] = ms_slot_gates(u[p]);
     if (a.staging_feat)
@@ -286,12 +318,12 @@ __global__ void __launch_bounds__(MS_ROWS / SPT) mlp_f32_w32_kernel(MsMlpArgs a)
         a.staging_feat[out * sh.n_feat + c] = f;
       }
   }
+  }
 }
 
 }  // namespace
 
 cudaError_t ms_mlp_f32(const MsMlpArgs &a, cudaStream_t s) {
-  if (a.n_blocks == 0) return cudaSuccess;
   size_t smem = (size_t)a.shape.params * sizeof(float);
   void (*fn)(MsMlpArgs) = mlp_f32_kernel;
   int threads = MS_ROWS;
@@ -301,7 +333,17 @@ cudaError_t ms_mlp_f32(const MsMlpArgs &a, cudaStream_t s) {
   }
   cudaError_t e = cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  fn<<<a.n_blocks, threads, smem, s>>>(a);
+  // a CTA per block while they fit a few waves of resident CTAs, else a grid-stride walk (the block count of a band
+  // lives on the device)
+  static int n_sm = 0;
+  if (n_sm == 0) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+  }
+  unsigned grid = (unsigned)n_sm * 16u;
+  if (a.n_blocks_hint > 0 && a.n_blocks_hint < grid) grid = a.n_blocks_hint;
+  fn<<<grid, threads, smem, s>>>(a);
   MS_LAUNCHED();
   return cudaGetLastError();
 }

@@ -174,10 +174,10 @@ inline TcLayout tc_layout(int k1, int width, int nh, int nout) {
 
 struct TcParams {
   MsCam cam;
-  int K, n_prims, n_feat;
-  uint32_t n_blocks;
+  int K, n_feat;
+  float falloff;          // CONTACT: g = exp(-falloff |p* - mu|^2_Lambda)
   const float *center, *A;
-  const uint32_t *prim_start, *blk_off;
+  MsSegs segs;            // segment tables, segment range and band of this launch (device)
   const MsInterval *intervals;
   const uint8_t *image;
   float4 *staging;
@@ -185,36 +185,41 @@ struct TcParams {
   float4 *staging_gate;   // CONTACT + Eq.7 slot features: the four gates of every hit, or NULL
 };
 
-__device__ __forceinline__ int find_prim(const uint32_t *__restrict__ blk_off, int n, uint32_t b) {
-  int lo = 0, hi = n;
-  while (hi - lo > 1) {
-    int mid = (lo + hi) >> 1;
-    if (blk_off[mid] <= b) lo = mid; else hi = mid;
-  }
-  return lo;
-}
-
-// Segment walk: the CTA's block range [b0, b1) cut at primitive boundaries.  Every role walks the
-// same segments (a pure function of blk_off), so no role has to tell another what comes next.
+// Segment walk: the CTA's block range [b0, b1) of the launch cut at segment boundaries (a segment = the
+// intervals of one primitive inside the launch's band and wave).  Every role walks the same segments (a pure
+// function of the device tables), so no role has to tell another what comes next.
 struct SegWalk {
-  const uint32_t *blk_off;
-  uint32_t cur, b1;
-  int p;
-  __device__ SegWalk(const uint32_t *bo, int n, uint32_t b0, uint32_t b1_) : blk_off(bo), cur(b0), b1(b1_), p(0) {
-    if (b0 < b1_) p = find_prim(bo, n, b0);
+  const uint32_t *bo;      // block offsets of the launch's segments (absolute: any base)
+  const uint32_t *seg_prim;
+  uint32_t g0, cur, b1;    // cur, b1: absolute block numbers
+  int s;
+  __device__ SegWalk(const MsSegs &sg, uint2 r, uint32_t b0, uint32_t b1_)
+      : bo(sg.blk_off + r.x), seg_prim(sg.prim), g0(r.x), s(0) {
+    const uint32_t base = bo[0];
+    cur = base + b0; b1 = base + b1_;
+    if (b0 < b1_) {
+      int lo = 0, hi = (int)(r.y - r.x);
+      while (hi - lo > 1) {
+        int mid = (lo + hi) >> 1;
+        if (bo[mid] <= cur) lo = mid; else hi = mid;
+      }
+      s = lo;
+    }
   }
-  // returns false when done; else (prim, first block inside prim, number of blocks)
-  __device__ bool next(int &prim, uint32_t &first, uint32_t &count) {
+  // returns false when done; else (segment, its primitive, first block inside the segment, number of blocks)
+  __device__ bool next(uint32_t &seg, int &prim, uint32_t &first, uint32_t &count) {
     while (cur < b1) {
-      uint32_t pe = blk_off[p + 1];
+      uint32_t pe = bo[s + 1];
       uint32_t end = pe < b1 ? pe : b1;
       if (end > cur) {
-        prim = p; first = cur - blk_off[p]; count = end - cur;
+        seg = g0 + (uint32_t)s;
+        prim = seg_prim ? (int)seg_prim[seg] : (int)seg;
+        first = cur - bo[s]; count = end - cur;
         cur = end;
-        if (cur == pe) ++p;
+        if (cur == pe) ++s;
         return true;
       }
-      ++p;
+      ++s;
     }
     return false;
   }
@@ -404,14 +409,17 @@ __global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(c
   __syncthreads();
   tc_fence_after();
 
-  const uint32_t b0 = (uint32_t)(((uint64_t)p.n_blocks * blockIdx.x) / gridDim.x);
-  const uint32_t b1 = (uint32_t)(((uint64_t)p.n_blocks * (blockIdx.x + 1)) / gridDim.x);
+  const uint2 srange = *p.segs.range;
+  const uint32_t n_blocks = p.segs.blk_off[srange.y] - p.segs.blk_off[srange.x];
+  const uint32_t slot0 = p.segs.band->slot0;
+  const uint32_t b0 = (uint32_t)(((uint64_t)n_blocks * blockIdx.x) / gridDim.x);
+  const uint32_t b1 = (uint32_t)(((uint64_t)n_blocks * (blockIdx.x + 1)) / gridDim.x);
 
   if (warp < NSLOT) {
     // ===== MMA issuer of slot s = warp (all 32 lanes walk the schedule; mma_* elect one lane) =====
     const int s = warp;
-    SegWalk w(p.blk_off, p.n_prims, b0, b1);
-    int prim; uint32_t first, count, seg = 0;
+    SegWalk w(p.segs, srange, b0, b1);
+    int prim; uint32_t sg, first, count, seg = 0;
     uint32_t run0 = 0;                 // running index of the segment's first block (ring positions)
     uint32_t pa = 0;                   // parity of the next a_ready[s] completion
     constexpr uint32_t idesc_w = umma_idesc(WIDTH);
@@ -420,16 +428,16 @@ __global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(c
     const uint32_t d_tmem = tmem + s * SLOT_COLS, a_tmem = d_tmem + WIDTH;
     const uint32_t bar_a_ready_s = bar_a_ready + 8 * s, bar_d_full_s = bar_d_full + 8 * s;
     uint32_t cnt = 0;                  // !HEADW: heads this warp has issued (head region s*HPS + cnt%HPS, use cnt/HPS)
-    SegWalk wl(p.blk_off, p.n_prims, b0, b1);   // !HEADW, slot warp 0: the weight loader's walk, one segment ahead
+    SegWalk wl(p.segs, srange, b0, b1);   // !HEADW, slot warp 0: the weight loader's walk, one segment ahead
     if (!HEADW && s == 0) {
-      int lp; uint32_t lf, lc;
-      if (wl.next(lp, lf, lc) && lane == 0) {
+      int lp; uint32_t ls, lf, lc;
+      if (wl.next(ls, lp, lf, lc) && lane == 0) {
         mbar_expect_tx(bar_w_full, IMG_BYTES);
         bulk_g2s(img, p.image + (size_t)lp * IMG_BYTES, IMG_BYTES, bar_w_full);
       }
       __syncwarp();
     }
-    while (w.next(prim, first, count)) {
+    while (w.next(sg, prim, first, count)) {
       mbar_wait(bar_w_full, seg & 1);
       tc_fence_after();
       const uint32_t n_s = (count + NSLOT - 1 - s) / NSLOT;   // blocks of this segment that run in slot s
@@ -483,8 +491,8 @@ __global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(c
       mma_commit(bar_w_free);  // arrives once every MMA this warp issued in the segment has read its weights
       if (!HEADW && s == 0) {  // loader duty: the next primitive's image once every slot is done with this one
         mbar_wait(bar_w_free, seg & 1);
-        int lp; uint32_t lf, lc;
-        if (wl.next(lp, lf, lc) && lane == 0) {
+        int lp; uint32_t ls, lf, lc;
+        if (wl.next(ls, lp, lf, lc) && lane == 0) {
           mbar_expect_tx(bar_w_full, IMG_BYTES);
           bulk_g2s(img, p.image + (size_t)lp * IMG_BYTES, IMG_BYTES, bar_w_full);
         }
@@ -499,22 +507,22 @@ __global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(c
     // of tensor work); from a warp of their own they slip into the pipe between the slots' wide MMAs
     // It is also the weight loader: one bulk async copy of the next primitive's image once every
     // MMA of the segment has read the current one (w_free), issued by lane 0.
-    SegWalk w(p.blk_off, p.n_prims, b0, b1), wl(p.blk_off, p.n_prims, b0, b1);
-    int prim; uint32_t first, count, seg = 0;
+    SegWalk w(p.segs, srange, b0, b1), wl(p.segs, srange, b0, b1);
+    int prim; uint32_t sg, first, count, seg = 0;
     constexpr uint32_t idesc_o = umma_idesc(NOUT);
     const uint32_t img = smem_u32(s_img);
     uint32_t cum[NSLOT];                          // blocks each slot has taken in earlier segments
 #pragma unroll
     for (int s = 0; s < NSLOT; ++s) cum[s] = 0;
     {
-      int lp; uint32_t lf, lc;
-      if (wl.next(lp, lf, lc) && lane == 0) {
+      int lp; uint32_t ls, lf, lc;
+      if (wl.next(ls, lp, lf, lc) && lane == 0) {
         mbar_expect_tx(bar_w_full, IMG_BYTES);
         bulk_g2s(img, p.image + (size_t)lp * IMG_BYTES, IMG_BYTES, bar_w_full);
       }
       __syncwarp();
     }
-    while (w.next(prim, first, count)) {
+    while (w.next(sg, prim, first, count)) {
       mbar_wait(bar_w_full, seg & 1);
       for (uint32_t i = 0; i < count; ++i) {
         const uint32_t slot = i % NSLOT;
@@ -539,8 +547,8 @@ __global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(c
       for (int s = 0; s < NSLOT; ++s) cum[s] += (count + NSLOT - 1 - s) / NSLOT;
       mbar_wait(bar_w_free, seg & 1);             // every MMA of the segment is done with the image
       {
-        int lp; uint32_t lf, lc;
-        if (wl.next(lp, lf, lc) && lane == 0) {
+        int lp; uint32_t ls, lf, lc;
+        if (wl.next(ls, lp, lf, lc) && lane == 0) {
           mbar_expect_tx(bar_w_full, IMG_BYTES);
           bulk_g2s(img, p.image + (size_t)lp * IMG_BYTES, IMG_BYTES, bar_w_full);
         }
@@ -559,9 +567,9 @@ __global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(c
     uint32_t cum[NSLOT];                          // blocks each slot has taken in earlier segments
 #pragma unroll
     for (int s = 0; s < NSLOT; ++s) cum[s] = 0;
-    SegWalk w(p.blk_off, p.n_prims, b0, b1);
-    int prim; uint32_t first, count;
-    while (w.next(prim, first, count)) {
+    SegWalk w(p.segs, srange, b0, b1);
+    int prim; uint32_t sg, first, count;
+    while (w.next(sg, prim, first, count)) {
       const uint32_t jmax = (count + NSLOT - 1) / NSLOT;
       for (uint32_t j = 0; j < jmax; ++j) {
 #pragma unroll 1
@@ -631,10 +639,10 @@ __global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(c
     uint32_t cum[NSLOT];                          // blocks each slot has taken in earlier segments
 #pragma unroll
     for (int s = 0; s < NSLOT; ++s) cum[s] = 0;
-    SegWalk w(p.blk_off, p.n_prims, b0, b1);
-    int prim; uint32_t first, count;
-    while (w.next(prim, first, count)) {
-      const uint32_t iv_first = p.prim_start[prim], iv_count = p.prim_start[prim + 1] - iv_first;
+    SegWalk w(p.segs, srange, b0, b1);
+    int prim; uint32_t sg, first, count;
+    while (w.next(sg, prim, first, count)) {
+      const uint32_t iv_first = p.segs.iv0[sg], iv_count = p.segs.cnt ? p.segs.cnt[sg] : p.segs.iv0[sg + 1] - iv_first;
       const uint64_t s0 = (uint64_t)first * MS_ROWS + (uint32_t)row;
       uint32_t j = (uint32_t)(s0 / K), k = (uint32_t)(s0 - (uint64_t)j * K);
       float4 q0 = make_float4(0.f, 0.f, 0.f, 0.f);   // (ray, t_in, delta, slot) of the row's interval
@@ -658,13 +666,13 @@ __global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(c
         const uint32_t hs = slot * HPS + cnt % HPS;
         const bool valid = j < iv_count;
         const float delta = q0.z;
-        const size_t out_idx = (size_t)(uint32_t)__float_as_int(q0.w) * K + k;
+        const size_t out_idx = (size_t)((uint32_t)__float_as_int(q0.w) - slot0) * K + k;
         float fall = 1.0f;                           // CONTACT: g = exp(-(9/2) |p* - mu|^2_Lambda)
         if (CONTACT && valid) {
           const float dd[3] = {q1.x, q1.y, q1.z};
           float uu[3];
           ms_sample_u(Al, mu, p.cam.o, dd, q0.y, uu);
-          fall = __expf(-4.5f * (uu[0] * uu[0] + uu[1] * uu[1] + uu[2] * uu[2]));
+          fall = __expf(-p.falloff * (uu[0] * uu[0] + uu[1] * uu[1] + uu[2] * uu[2]));
           if (p.staging_gate) p.staging_gate[out_idx] = ms_slot_gates(uu);   // Eq.7 gates for stage (e)
         }
         k += dk; j += dj;
@@ -743,10 +751,10 @@ __global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(c
     const uint32_t K = (uint32_t)p.K;
     const uint32_t dj = (NEG * MS_ROWS) / K, dk = NEG * MS_ROWS - dj * K;   // NEG blocks ahead
     uint32_t run0 = 0;
-    SegWalk w(p.blk_off, p.n_prims, b0, b1);
-    int prim; uint32_t first, count;
-    while (w.next(prim, first, count)) {
-      const uint32_t iv_first = p.prim_start[prim], iv_count = p.prim_start[prim + 1] - iv_first;
+    SegWalk w(p.segs, srange, b0, b1);
+    int prim; uint32_t sg, first, count;
+    while (w.next(sg, prim, first, count)) {
+      const uint32_t iv_first = p.segs.iv0[sg], iv_count = p.segs.cnt ? p.segs.cnt[sg] : p.segs.iv0[sg + 1] - iv_first;
       float Al[9], mu[3];
 #pragma unroll
       for (int q = 0; q < 9; ++q) Al[q] = __ldg(p.A + 9 * (size_t)prim + q);
@@ -909,14 +917,13 @@ void ms_tc_free(MsTcWeights *w) {
 }
 
 cudaError_t ms_mlp_tc(const MsTcWeights &w, const MsMlpArgs &a, cudaStream_t s) {
-  if (a.n_blocks == 0) return cudaSuccess;
   if (!w.valid) return cudaErrorNotSupported;
   KernelFn fn = select_kernel(a.shape.n_freq, a.shape.use_viewdir, a.shape.width, w.n_out_pad, a.shape.n_hidden,
                               a.shape.mode == MS_MODE_CONTACT);
   if (!fn) return cudaErrorNotSupported;
   TcParams p;
-  p.cam = a.cam; p.K = a.K; p.n_prims = a.n_prims; p.n_feat = a.shape.n_feat; p.n_blocks = a.n_blocks;
-  p.center = a.center; p.A = a.A; p.prim_start = a.prim_start; p.blk_off = a.blk_off; p.intervals = a.intervals;
+  p.cam = a.cam; p.K = a.K; p.n_feat = a.shape.n_feat; p.falloff = a.falloff;
+  p.center = a.center; p.A = a.A; p.segs = a.segs; p.intervals = a.intervals;
   p.image = (const uint8_t *)w.image;
   p.staging = a.staging; p.staging_feat = a.staging_feat; p.staging_gate = a.staging_gate;
   size_t smem = w.bytes_per_prim + tc_a1_stages(a.shape.width) * ((size_t)MS_ROWS * w.k1_pad * 2);
@@ -930,7 +937,9 @@ cudaError_t ms_mlp_tc(const MsTcWeights &w, const MsMlpArgs &a, cudaStream_t s) 
   }
   cudaError_t e = cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  unsigned grid = a.n_blocks < (uint32_t)n_sm ? a.n_blocks : (unsigned)n_sm;
+  // one persistent CTA per SM; the launch's block count lives on the device (a CTA with an empty range leaves at once)
+  unsigned grid = (unsigned)n_sm;
+  if (a.n_blocks_hint > 0 && a.n_blocks_hint < grid) grid = a.n_blocks_hint;
   const int threads = 32 * tc_warps(a.shape.width, w.n_out_pad);
   fn<<<grid, threads, smem, s>>>(p);
   MS_LAUNCHED();

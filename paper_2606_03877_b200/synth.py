@@ -44,6 +44,7 @@ class MLPSpec:
     n_feat: int          # extra linear output channels after [r,g,b,sigma]
     bf16: bool           # weights are bf16-representable values
     mode: int = 0        # 0: north-star input (local coords, K samples); 1: the paper's contact-point input (S:§8(f) NEXT-1)
+    falloff: float = 4.5 # contact mode: g = exp(-falloff |p*-mu|^2_Lambda) (Q29; a parameter, default 9/2)
 
     @property
     def in_dim(self) -> int:

@@ -127,7 +127,7 @@ def test_next1_tensor_path(W, H):
     sc, cam = synth.make_scene(cfg), synth.make_cameras(cfg)[0]
     orc = mso.OracleScene(sc)
     gs = api.Scene(sc)
-    rgb, alpha, _ = gs.render(cam, H, W, 1, path=api.PATH_BF16_TC, flags=api.FLAG_KEEP_DEBUG)
+    rgb, alpha, _ = gs.render(cam, H, W, 1, path=api.PATH_BF16_TC, flags=api.FLAG_DEBUG_ALL)
     torch.cuda.synchronize()
     o_rgb, o_alpha, _, st = orc.render(cam, H, W, 1)
     assert check_structures(gs, orc, cam, H, W, 1, 16, n_order_rays=8) == st.n_intervals
@@ -183,7 +183,7 @@ def test_tile_centre_order(tile):
     orc.set_order(1)
     o_rgb, o_alpha, _, st = orc.render(cam, H, W, 1, tile=tile)
     gs = api.Scene(sc)
-    rgb, alpha, _ = gs.render(cam, H, W, 1, tile=tile, flags=api.FLAG_KEEP_DEBUG | api.FLAG_TILE_ORDER)
+    rgb, alpha, _ = gs.render(cam, H, W, 1, tile=tile, flags=api.FLAG_DEBUG_ALL | api.FLAG_TILE_ORDER)
     torch.cuda.synchronize()
     assert check_structures(gs, orc, cam, H, W, 1, tile, n_order_rays=12) == st.n_intervals
     g_rgb, g_alpha = rgb.cpu().numpy().reshape(-1, 3), alpha.cpu().numpy().reshape(-1)
@@ -210,7 +210,7 @@ def test_more_than_32_hits_per_ray_with_slot_features():
     W, H = 40, 30
     cam = synth.pinhole(W, H, 40.0, synth.look_at([0.3, 0.2, 4.0]))
     gs = api.Scene(sc)
-    rgb, alpha, feat = gs.render(cam, H, W, 1, flags=api.FLAG_KEEP_DEBUG)
+    rgb, alpha, feat = gs.render(cam, H, W, 1, flags=api.FLAG_DEBUG_ALL)
     torch.cuda.synchronize()
     orc = mso.OracleScene(sc)
     o_rgb, o_alpha, o_feat, st = orc.render(cam, H, W, 1)
