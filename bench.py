@@ -169,6 +169,146 @@ def run_reference(args, cfg):
 # ------------------------------------------------------------------------------------------------
 # our arm
 # ------------------------------------------------------------------------------------------------
+def algorithmic_bytes(cfg, sc) -> dict:
+    """what the method must move -- the scene read once (primitives; weight matrices in the
+    config's dtype, biases fp32; slot embeddings) and the image written once."""
+    m = cfg.mlp
+    n_w = sum(i * o for i, o in m.layer_dims)
+    n_b = sum(o for _, o in m.layer_dims)
+    scene = sc.n * (40 + n_w * (2 if m.bf16 else 4) + n_b * 4) + (sc.slots.nbytes if sc.slots is not None else 0)
+    feat_w = cfg.c_f or m.n_feat
+    out = cfg.width * cfg.height * (16 + 4 * feat_w)
+    return {"scene": scene, "outputs_per_view": out, "per_view": scene + out}
+
+
+def load_dram_profile():
+    """dram__bytes_read.sum + dram__bytes_write.sum per kernel launch from the committed `ncu --set full` captures
+    (profiles/r2_dram_bytes.json: written by hand from the captures it names; null where none was taken)."""
+    path = os.path.join(ROOT, "profiles", "r2_dram_bytes.json")
+    if os.path.exists(path):
+        return json.load(open(path))
+    return {}
+
+
+def measure(api, cfg, args, peaks, stream, barrier, steps, warmup, sampler=None, shard=None):
+    """Times `steps` steps of one workload (a step = ms_render_batch over its views: stages (a)-(e)) with CUDA
+    events on the launching stream, then the same steps through ms_render_host (e2e).  Returns a dict."""
+    import torch
+    sc = synth.make_scene(cfg)
+    cams = synth.make_cameras(cfg)
+    if shard is not None:                               # this rank's share of the step's views
+        cams = cams[shard[0]:shard[1]] or cams[:1]
+    H, W, K, V = cfg.height, cfg.width, cfg.K, len(cams)
+    t_create = time.perf_counter()
+    gs = api.Scene(sc)
+    create_s = time.perf_counter() - t_create
+    gs.band_bytes, gs.waves = args.band_bytes, args.waves
+    extra_flags = api.FLAG_TILE_ORDER if (args.tile_order and cfg.mlp.mode == 1) else 0
+    tile_kw = {"tile": args.tile} if args.tile else {"tile": cfg.tile}
+    kw = dict(t_stop=cfg.t_stop, **tile_kw)
+    with torch.cuda.stream(stream):
+        out = gs.render_batch(cams, H, W, K, flags=extra_flags, **kw)          # allocates outputs + scratch
+        for _ in range(warmup):
+            gs.render_batch(cams, H, W, K, out=out, flags=extra_flags, **kw)
+    barrier()
+    gs.stage_accum(reset=True)
+    if sampler is not None:
+        sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    launches = api.launch_count()
+    with torch.cuda.stream(stream):
+        ev0.record(stream)
+        for _ in range(steps):
+            gs.render_batch(cams, H, W, K, out=out, flags=api.FLAG_STAGE_TIMES | extra_flags, **kw)
+        ev1.record(stream)
+    launches = api.launch_count() - launches                # kernels this thread launched in the timed region
+    barrier()
+    ms_total = ev0.elapsed_time(ev1)
+    clocks = sampler.stop() if sampler is not None else None
+    stage_sum, n_views_timed = gs.stage_accum()
+    st = gs.stats()                                     # counts of the last view
+
+    # ---- e2e: the same steps through ms_render_host (pinned HOST outputs, D2H inside) ----
+    host_out = gs.render_host(cams, H, W, K, stream=stream.cuda_stream, flags=extra_flags, **kw)
+    barrier()
+    t0 = time.perf_counter()
+    e2e_steps = max(1, min(steps, 10))
+    for _ in range(e2e_steps):
+        gs.render_host(cams, H, W, K, out=host_out, stream=stream.cuda_stream, flags=extra_flags, **kw)   # synchronises the stream itself
+    barrier()
+    e2e_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
+    gs.close()
+    del out, host_out
+    torch.cuda.empty_cache()
+
+    ms_step = ms_total / steps
+    px_step = H * W * V
+    n_samples_view = st.n_samples                       # last view
+    n_eval_view = st.n_samples_evaluated
+    flops_view = cfg.mlp.flop_per_sample * n_eval_view  # the MLP evaluations that really ran
+    nv = max(1, n_views_timed)
+    stage_ms = {k: v / nv for k, v in stage_sum.items()}
+    mlp_ms, comp_ms = stage_ms["mlp"], stage_ms["composite"]
+    achieved = flops_view / (mlp_ms * 1e-3) / 1e12 if mlp_ms > 0 else 0.0
+    peak = peaks["bf16_tflops_sustained"]
+    if not cfg.mlp.bf16:
+        # fp32 SIMT path: 148 SMs x 128 FMA lanes x 2 FLOP at the top SM clock (guide's unit counts)
+        peak = 148 * 128 * 2 * 1.965e9 / 1e12
+    alg = algorithmic_bytes(cfg, sc)
+    feat_w = cfg.c_f or cfg.mlp.n_feat
+    sample_bytes = 16 + 4 * cfg.mlp.n_feat + (32 if cfg.c_f else 0)
+    # bytes the design moves per view by construction: staging written by (d) and read by (e), both hit lists
+    # written by (c) and read by (d) / (e), the outputs
+    stage_bytes_design = 2 * n_eval_view * sample_bytes + 2 * st.n_intervals * 48 + alg["outputs_per_view"]
+    frame_floor_ms = max(flops_view / (peak * 1e12), alg["per_view"] / (peaks["hbm_gbs"] * 1e9)) * 1e3
+    dram = load_dram_profile().get(cfg.name)
+    res = {
+        "workload": workload_desc(cfg), "ms_per_step": ms_step, "Mpixels_per_s": px_step / (ms_step * 1e-3) / 1e6,
+        "samples_per_s": n_eval_view * V / (ms_step * 1e-3), "stage_ms_per_view": stage_ms,
+        "counts_per_view": {"visible": st.n_visible, "pairs": st.n_pairs, "intervals": st.n_intervals,
+                            "samples": st.n_samples, "samples_evaluated": n_eval_view, "dead_rays": st.n_dead_rays,
+                            "row_blocks": st.n_blocks, "bands": st.n_bands, "waves": st.n_waves,
+                            "staging_MB": st.staging_bytes / 1e6, "scratch_GB": st.scratch_bytes / 1e9},
+        "gpu_launches": launches, "scene_create_s": create_s,
+        "e2e": {"value": px_step / (e2e_ms * 1e-3) / 1e6, "unit": UNIT, "h2d_bytes_per_step": 64 * V,
+                "d2h_bytes_per_step": alg["outputs_per_view"] * V, "ms_per_step": e2e_ms},
+        "roofline": {"bound": "tensor" if cfg.mlp.bf16 else "alu",
+                     "kernel": "mlp_tc_kernel (stage d)" if cfg.mlp.bf16 else "mlp_f32_kernel (stage d, fp32 SIMT path)",
+                     "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak if peak else None,
+                     "traffic": (dram or {}).get("mlp"),
+                     "traffic_unit": "bytes per view, all launches of the kernel (ncu dram read + write), " +
+                                     str((dram or {}).get("source", "no capture of this workload")),
+                     "algorithmic_bytes": alg["per_view"],
+                     "algorithmic_bytes_note": "SURVEY.md Sec.8(d): scene read once + outputs written once, per view",
+                     "stage_bytes_design": stage_bytes_design,
+                     "dram_bytes_per_view": (dram or {}).get("total"),
+                     "peak_kind": (f"bf16 dense, sustained, of {peaks['source']}" if cfg.mlp.bf16 else
+                                   "fp32 FMA, 148 SMs x 128 lanes x 2 x 1.965 GHz (derived)"),
+                     "frac_of_burst_peak": achieved / peaks["bf16_tflops"] if cfg.mlp.bf16 else None,
+                     "algorithmic_flop_per_sample": cfg.mlp.flop_per_sample,
+                     "kernel_ms": mlp_ms, "kernel_share_of_step": mlp_ms * V / ms_step},
+        "frame_roofline": {"floor_ms_per_view": frame_floor_ms, "frac": frame_floor_ms * V / ms_step,
+                           "note": "slower of the evaluated MLP FLOPs at the bf16 peak and the algorithmic bytes "
+                                   "(scene + outputs) at the HBM peak, over the whole step"},
+        "clocks": clocks,
+    }
+    if cfg.c_f and comp_ms > mlp_ms:
+        # Eq.7 slot features: stage (e) dominates and is memory-bound.  Algorithmic bytes per view: staging,
+        # gates and hit records once per hit (16 B each), the embeddings once, the outputs once.
+        a2 = st.n_intervals * 48 + sc.slots.nbytes + alg["outputs_per_view"]
+        ach = a2 / (comp_ms * 1e-3) / 1e9
+        res["roofline"] = {"bound": "hbm", "kernel": "composite_kernel<2> + slot_feature_kernel (stage e, slot features)",
+                           "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
+                           "traffic": (dram or {}).get("composite"),
+                           "peak_kind": f"HBM copy bandwidth, of {peaks['source']}", "algorithmic_bytes": a2,
+                           "stage_bytes_design": stage_bytes_design, "dram_bytes_per_view": (dram or {}).get("total"),
+                           "kernel_ms": comp_ms, "kernel_share_of_step": comp_ms * V / ms_step,
+                           "note": "the kernel re-reads each hit's four embedding rows (16 * c_f B per hit) through L1/L2; "
+                                   "that traffic is not algorithmic"}
+    return res, sc, cams
+
+
 def run_ours(args, cfg):
     import torch
     from paper_2606_03877_b200 import api
@@ -186,120 +326,71 @@ def run_ours(args, cfg):
         torch.cuda.synchronize()
 
     peaks = load_peaks()
-    sc = synth.make_scene(cfg)
-    cams = synth.make_cameras(cfg)
-    H, W, K, V = cfg.height, cfg.width, cfg.K, cfg.n_views
-    gs = api.Scene(sc)
-    gs.band_bytes, gs.waves = args.band_bytes, args.waves
     stream = torch.cuda.Stream()
-    out = None
-    with torch.cuda.stream(stream):
-        extra_flags = api.FLAG_TILE_ORDER if args.tile_order else 0
-        tile_kw = {"tile": args.tile} if args.tile else {}
-        out = gs.render_batch(cams, H, W, K, flags=extra_flags, **tile_kw)          # allocates outputs + scratch
-        for _ in range(args.warmup):
-            gs.render_batch(cams, H, W, K, out=out, flags=extra_flags, **tile_kw)
-    barrier()
-    gs.stage_accum(reset=True)
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
-    launches = 0
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    with torch.cuda.stream(stream):
-        ev0.record(stream)
-        for _ in range(args.steps):
-            gs.render_batch(cams, H, W, K, out=out, flags=api.FLAG_STAGE_TIMES | extra_flags, **tile_kw)
-            launches += gs.stats().n_launches * V
-        ev1.record(stream)
-    barrier()
-    ms_total = ev0.elapsed_time(ev1)
-    clocks = sampler.stop() if rank == 0 else None
-    stage_sum, n_views_timed = gs.stage_accum()
-    st = gs.stats()                                     # counts of the last view
+    sampler = ClockSampler(local) if rank == 0 else None
 
-    # ---- e2e: the same steps through ms_render_host (pinned HOST outputs, D2H inside) ----
-    host_out = gs.render_host(cams, H, W, K, stream=stream.cuda_stream, flags=extra_flags, **tile_kw)
-    barrier()
-    t0 = time.perf_counter()
-    e2e_steps = max(1, min(args.steps, 10))
-    for _ in range(e2e_steps):
-        gs.render_host(cams, H, W, K, out=host_out, stream=stream.cuda_stream, flags=extra_flags, **tile_kw)   # synchronises the stream itself
-    barrier()
-    e2e_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
+    # strong scaling (CFG5's batch of poses sharded over the ranks, S:Sec.8(e)): every rank renders its share
+    shard = None
+    if args.shard_views and world > 1:
+        lo, hi = msdist.shard_range(cfg.n_views, rank, world)
+        shard = (lo, hi)
+    r, sc, cams = measure(api, cfg, args, peaks, stream, barrier, args.steps, args.warmup, sampler, shard=shard)
+    ms_step, e2e_ms = msdist.max_over_ranks([r["ms_per_step"], r["e2e"]["ms_per_step"]], "cuda")
 
-    ms_total, e2e_ms = msdist.max_over_ranks([ms_total, e2e_ms], "cuda")
+    others = {}
+    if rank == 0 and world == 1 and args.all_configs:
+        for name in ALL_CONFIGS:
+            if name == cfg.name:
+                continue
+            o, _, _ = measure(api, synth.CONFIGS[name], args, peaks, stream, barrier, max(3, min(args.steps, 10)), 3)
+            others[name] = {k: o[k] for k in ("workload", "ms_per_step", "Mpixels_per_s", "samples_per_s",
+                                              "stage_ms_per_view", "counts_per_view", "gpu_launches", "scene_create_s")}
+            others[name]["e2e_Mpixels_per_s"] = o["e2e"]["value"]
+            others[name]["e2e_ms_per_step"] = o["e2e"]["ms_per_step"]
+            others[name]["roofline"] = {k: o["roofline"].get(k) for k in
+                                        ("bound", "kernel", "achieved", "peak", "unit", "frac", "kernel_ms",
+                                         "algorithmic_bytes", "stage_bytes_design", "dram_bytes_per_view")}
+            others[name]["frame_roofline_frac"] = o["frame_roofline"]["frac"]
     if rank != 0:
         msdist.shutdown()
         return
 
-    ms_step = ms_total / args.steps
-    px_step = H * W * V
-    value = world * px_step / (ms_step * 1e-3) / 1e6
-    n_samples_view = st.n_samples                       # last view; equal for every step of a 1-view workload
-    flops_view = cfg.mlp.flop_per_sample * n_samples_view
-    mlp_ms = stage_sum["mlp"] / max(1, n_views_timed)  # mean duration of the dominant kernel, CUDA events in the timed region
-    achieved = flops_view / (mlp_ms * 1e-3) / 1e12 if mlp_ms > 0 else 0.0
-    peak = peaks["bf16_tflops_sustained"]
-    if not cfg.mlp.bf16:
-        # fp32 SIMT path: 148 SMs x 128 FMA lanes x 2 FLOP at the top SM clock (guide's unit counts)
-        peak = 148 * 128 * 2 * 1.965e9 / 1e12
-    feat_w = cfg.c_f or cfg.mlp.n_feat                  # Eq.7 slot features or the widened head
-    out_bytes = H * W * (16 + 4 * feat_w)
-    frame_floor_ms = max(flops_view / (peak * 1e12), out_bytes / (peaks["hbm_gbs"] * 1e9)) * 1e3
+    H, W, V = cfg.height, cfg.width, cfg.n_views
+    strong = shard is not None
+    px_job = H * W * V * (1 if strong else world)        # strong: the ranks split one step's views
+    n_samp_job = r["counts_per_view"]["samples_evaluated"] * V * (1 if strong else world)
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "metric": METRIC, "value": px_job / (ms_step * 1e-3) / 1e6, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+        "scaling": "strong" if strong else "weak", "vs_baseline": None,
         "dtype": "bf16" if cfg.mlp.bf16 else "f32", "data": "synthetic",
-        "config": {"workload": workload_desc(cfg), "parallelism": f"replicas x{world}, no collective",
-                   "l2": ("inputs larger than L2 (weights %.0f MB, per-view staging %.1f GB)" if
-                          sc.weights.nbytes / 2 + n_samples_view * 16 > 126e6 else
-                          "working set below L2 (weights %.1f MB, per-view staging %.3f GB): no flush, config is launch-bound")
-                         % (sc.weights.nbytes / 2 / 1e6, n_samples_view * 16 / 1e9),
+        "config": {"workload": r["workload"],
+                   "parallelism": (f"views sharded over {world} ranks, no collective" if strong else
+                                   f"replicas x{world}, no collective"),
+                   "l2": ("inputs larger than L2 (weights %.0f MB, staging %.0f MB per band)" if
+                          sc.weights.nbytes / 2 + r["counts_per_view"]["staging_MB"] * 1e6 > 126e6 else
+                          "working set below L2 (weights %.1f MB, staging %.1f MB): no flush, config is launch-bound")
+                         % (sc.weights.nbytes / 2 / 1e6, r["counts_per_view"]["staging_MB"]),
                    "tile": args.tile or cfg.tile, "t_stop": cfg.t_stop,
+                   "band_bytes": args.band_bytes, "waves": args.waves,
                    "order": "tile-centre shared order (P:109)" if args.tile_order else "exact per-ray order"},
-        "samples_per_s": world * n_samples_view * V / (ms_step * 1e-3),
-        "counts_per_view": {"pairs": st.n_pairs, "intervals": st.n_intervals, "samples": st.n_samples,
-                            "row_blocks": st.n_blocks, "scratch_GB": st.scratch_bytes / 1e9,
-                            "samples_evaluated": st.n_samples_evaluated, "bands": st.n_bands, "waves": st.n_waves,
-                            "staging_MB": st.staging_bytes / 1e6},
-        "stage_ms_per_view": {k: v / max(1, n_views_timed) for k, v in stage_sum.items()},
-        "clocks": clocks,
-        "e2e": {"value": world * px_step / (e2e_ms * 1e-3) / 1e6, "unit": UNIT,
-                "h2d_bytes_per_step": 64 * V, "d2h_bytes_per_step": out_bytes * V, "ms_per_step": e2e_ms,
-                "note": "ms_render_host: camera in (kernel parameters), rgb/alpha(/feat) copied to pinned host memory"},
-        "gpu_launches": launches,
-        "roofline": {"bound": "tensor" if cfg.mlp.bf16 else "alu",
-                     "kernel": "mlp_tc_kernel (stage d)" if cfg.mlp.bf16 else "mlp_f32_kernel (stage d, fp32 SIMT path)", "achieved": achieved, "peak": peak,
-                     "unit": "TFLOP/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg.name),
-                     "traffic_unit": "bytes per launch (ncu dram read + write, profiles/r1c_summary.md)",
-                     "algorithmic_bytes": n_samples_view * 16 + st.n_intervals * 32,
-                     "peak_kind": (f"bf16 dense, sustained, of {peaks['source']}" if cfg.mlp.bf16 else
-                                   "fp32 FMA, 148 SMs x 128 lanes x 2 x 1.965 GHz (derived)"),
-                     "frac_of_burst_peak": achieved / peaks["bf16_tflops"] if cfg.mlp.bf16 else None,
-                     "algorithmic_flop_per_sample": cfg.mlp.flop_per_sample,
-                     "kernel_ms": mlp_ms, "kernel_share_of_step": mlp_ms * V / ms_step},
-        "frame_roofline": {"floor_ms_per_view": frame_floor_ms, "frac": frame_floor_ms * V / ms_step,
-                           "note": "slower of MLP FLOPs at the bf16 peak and output bytes at the HBM peak, over the whole step"},
+        "samples_per_s": n_samp_job / (ms_step * 1e-3),
+        "counts_per_view": r["counts_per_view"], "stage_ms_per_view": r["stage_ms_per_view"],
+        "clocks": r["clocks"], "scene_create_s": r["scene_create_s"],
+        "e2e": dict(r["e2e"], value=px_job / (e2e_ms * 1e-3) / 1e6, ms_per_step=e2e_ms,
+                    note="ms_render_host: camera in (kernel parameters), rgb/alpha(/feat) copied to pinned host memory"),
+        "gpu_launches": r["gpu_launches"], "roofline": r["roofline"], "frame_roofline": r["frame_roofline"],
     }
-    comp_ms = stage_sum["composite"] / max(1, n_views_timed)
-    if cfg.c_f and comp_ms > mlp_ms:
-        # Eq.7 slot features: stage (e) dominates and is memory-bound.  Algorithmic bytes per view: staging,
-        # gates and hit records once per hit (16 B each), the embeddings once, the outputs once.
-        alg = st.n_intervals * 48 + sc.slots.nbytes + out_bytes
-        ach = alg / (comp_ms * 1e-3) / 1e9
-        line["roofline"] = {"bound": "hbm", "kernel": "composite_kernel<2> (stage e, slot features)", "achieved": ach,
-                            "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"], "traffic": None,
-                            "peak_kind": f"HBM copy bandwidth, of {peaks['source']}", "algorithmic_bytes": alg,
-                            "kernel_ms": comp_ms, "kernel_share_of_step": comp_ms * V / ms_step,
-                            "note": "the kernel re-reads each hit's four embedding rows (16 * c_f B per hit) through L1/L2; "
-                                    "that traffic is not algorithmic"}
+    if others:
+        line["all_configs"] = others
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = {k: v for k, v in time_oracle(cfg, sc, cams, args.cpu_seconds).items()
                                 if k in ("value", "unit", "cores", "kind", "sample", "samples_per_s")}
     print(json.dumps(line), flush=True)
     msdist.shutdown()
+
+
+ALL_CONFIGS = ["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "next1", "next1b", "next2", "next2b", "cfg4_opaque", "cfg4_inside"]
 
 
 def main():
@@ -316,11 +407,20 @@ def main():
     ap.add_argument("--tile", type=int, default=0, help="tile edge override (8, 16, 32)")
     ap.add_argument("--band-bytes", type=int, default=0,
                     help="staging budget per band in bytes (ms_opts.band_bytes): 0 = library default, -1 = one band")
+    ap.add_argument("--all-configs", action="store_true", default=None,
+                    help="also time every other workload (cfg1-5, next1/1b/2/2b, cfg4_opaque, cfg4_inside) in the same "
+                         "run and add them as `all_configs`; default: on for the default workload at N=1")
+    ap.add_argument("--no-all-configs", dest="all_configs", action="store_false")
+    ap.add_argument("--shard-views", action="store_true",
+                    help="N > 1: shard the workload's views over the ranks (strong scaling; cfg5's 8 poses) instead of "
+                         "one replica of the whole step per rank")
     ap.add_argument("--waves", type=int, default=0, help="depth waves (ms_opts.waves): 0 = auto, -1 = off, C > 0 = wave size")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                                  # timing rule: W >= 3
     cfg = synth.CONFIGS[args.config]
+    if args.all_configs is None:
+        args.all_configs = args.config == "cfg4" and args.gpus == 1
     if args.impl == "reference":
         run_reference(args, cfg)
     else:

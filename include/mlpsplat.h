@@ -133,7 +133,7 @@ typedef struct {
                      plane) is binned to the whole image instead of through the dual-conic bound, which degenerates
                      there.  <= 0 = MS_EYE_GUARD_DEFAULT (0.01). */
 } ms_opts;
-#define MS_BAND_BYTES_DEFAULT ((int64_t)48 << 20)
+#define MS_BAND_BYTES_DEFAULT ((int64_t)1 << 30)
 #define MS_WAVES_AUTO 0
 #define MS_EYE_GUARD_DEFAULT 0.01f
 
@@ -214,6 +214,9 @@ int ms_debug_sample_order(ms_scene *scene, int32_t ray, int32_t *prim, int32_t *
 int ms_debug_sample_order_all(ms_scene *scene, int32_t *prim, int32_t *k, size_t cap, size_t *n);
 /* Derived per-primitive frames, host [n][9] each (row-major A, M). */
 int ms_debug_prim_frames(ms_scene *scene, float *A, float *M);
+
+/* Kernels the calling host thread has launched through this library so far (a running count; no synchronisation). */
+int64_t ms_launch_count_total(void);
 
 const char *ms_error_string(int code);
 /* cudaError_t of the last failing CUDA call on this scene (0 if none). */

@@ -25,7 +25,7 @@ STAGES = ("bin", "sort", "isect", "mlp", "composite")
 
 EXPORTS = ["ms_scene_create", "ms_scene_set_slots", "ms_scene_destroy", "ms_render", "ms_render_batch", "ms_render_host",
            "ms_last_stats", "ms_last_stage_ms", "ms_stage_accum", "ms_debug_tile_lists", "ms_debug_intervals",
-           "ms_debug_sample_order", "ms_debug_sample_order_all", "ms_debug_prim_frames", "ms_error_string", "ms_last_cuda_error"]
+           "ms_debug_sample_order", "ms_debug_sample_order_all", "ms_debug_prim_frames", "ms_launch_count_total", "ms_error_string", "ms_last_cuda_error"]
 
 
 class _Prims(C.Structure):
@@ -65,12 +65,18 @@ def _load() -> C.CDLL:
     for name in EXPORTS:
         getattr(lib, name)  # fail loudly on a stale library
     lib.ms_error_string.restype = C.c_char_p
+    lib.ms_launch_count_total.restype = C.c_int64
     lib.ms_scene_destroy.argtypes = [C.c_void_p]
     lib.ms_scene_set_slots.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
     return lib
 
 
 _lib = _load()
+
+
+def launch_count() -> int:
+    """Kernels this host thread has launched through the library so far (ms_launch_count_total)."""
+    return int(_lib.ms_launch_count_total())
 
 
 class MsError(RuntimeError):

@@ -40,8 +40,10 @@ struct ms_scene {
   Buf tile_count, emit_off, rect, z_entry, oprime, keys_a, keys_b, sort_scratch, tile_start, pair_hits_i, pair_hits_j,
       pair_off, slot_of, key2_a, key2_b, flags, gid, grp_key, grp_prim, grp_iv0, grp_blocks, blk_off, grp_cnt_c,
       grp_blocks_c, blk_off_c, bw, bands, counters, alive, ray_hits, ray_off, scan_scratch, intervals, hits, staging,
-      staging_feat, staging_gate, staging_coef, dbg_ord, host_rgb, host_alpha, host_feat;
+      staging_feat, staging_gate, staging_coef, dbg_ord, pos_xy, host_rgb, host_alpha, host_feat;
   uint32_t *pinned = nullptr;  // host-pinned readback: [0] P, [1..] device counters
+  MsBand *pinned_bands = nullptr;  // host-pinned readback of the band table
+  size_t pinned_bands_cap = 0;
   std::vector<cudaEvent_t> ev;     // MS_FLAG_STAGE_TIMES: 4 + 2 per band + 1 events of the last view
   int ev_bands = 0;
   bool ev_valid = false;
@@ -96,6 +98,19 @@ int ensure(ms_scene *sc, Buf &b, size_t bytes) {
   return MS_OK;
 }
 
+#define ENS_HOST(sc, bytes)                                                     \
+  do {                                                                          \
+    if ((bytes) > (sc)->pinned_bands_cap) {                                     \
+      if ((sc)->pinned_bands) cudaFreeHost((sc)->pinned_bands);                 \
+      (sc)->pinned_bands = nullptr; (sc)->pinned_bands_cap = 0;                 \
+      if (cudaMallocHost(&(sc)->pinned_bands, 2 * (bytes)) != cudaSuccess) {    \
+        (void)cudaGetLastError();                                               \
+        return MS_ERR_OUT_OF_MEMORY;                                            \
+      }                                                                         \
+      (sc)->pinned_bands_cap = 2 * (bytes);                                     \
+    }                                                                           \
+  } while (0)
+
 #define ENS(buf, bytes)                         \
   do {                                          \
     int _r = ensure(sc, buf, (size_t)(bytes));  \
@@ -108,7 +123,7 @@ std::vector<Buf *> scratch_bufs(ms_scene *sc) {
           &sc->key2_a, &sc->key2_b, &sc->flags, &sc->gid, &sc->grp_key, &sc->grp_prim, &sc->grp_iv0, &sc->grp_blocks,
           &sc->blk_off, &sc->grp_cnt_c, &sc->grp_blocks_c, &sc->blk_off_c, &sc->bw, &sc->bands, &sc->counters,
           &sc->alive, &sc->ray_hits, &sc->ray_off, &sc->scan_scratch, &sc->intervals, &sc->hits, &sc->staging,
-          &sc->staging_feat, &sc->staging_gate, &sc->staging_coef, &sc->dbg_ord};
+          &sc->staging_feat, &sc->staging_gate, &sc->staging_coef, &sc->dbg_ord, &sc->pos_xy};
 }
 
 size_t scratch_total(ms_scene *sc) {
@@ -190,6 +205,8 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   grid.tile = tile; grid.tiles_x = (W + tile - 1) / tile; grid.tiles_y = (H + tile - 1) / tile;
   grid.G = 64 / tile < 1 ? 1 : 64 / tile;          // macro-tiles of 64 x 64 pixels
   grid.W = W; grid.H = H;
+  grid.tshift = tile == 8 ? 3 : (tile == 16 ? 4 : 5);
+  grid.pos_xy = nullptr;
   const int64_t n_tiles64 = (int64_t)grid.tiles_x * grid.tiles_y;
   const int64_t R64 = n_tiles64 * tile * tile;      // ray slots: every tile padded to tile x tile
   if (R64 >= (1ll << 31) - 1) return MS_ERR_UNSUPPORTED_SHAPE;
@@ -281,11 +298,14 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   CK(rec(2));
   ENS(sc->ray_hits, R * 4);
   ENS(sc->ray_off, (R + 1) * 4);
+  ENS(sc->pos_xy, (size_t)(n_tiles + 1) * sizeof(ushort2));
+  grid.pos_xy = (const ushort2 *)sc->pos_xy.p;
   MsIsectArgs ia;
   ia.cam = cam; ia.grid = grid; ia.K = K; ia.prim_bits = prim_bits;
   ia.contact = sc->shape.mode == MS_MODE_CONTACT;
   ia.wave_c = 0;
   ia.keys = sorted; ia.tile_start = (uint32_t *)sc->tile_start.p; ia.A = sc->A; ia.oprime = (float *)sc->oprime.p;
+  ia.pos_xy = (ushort2 *)sc->pos_xy.p;
   ia.pair_hits = (uint32_t *)sc->pair_hits_i.p; ia.ray_hits = (uint32_t *)sc->ray_hits.p;
   ia.slot_of = (uint32_t *)sc->slot_of.p; ia.pair_off = (uint32_t *)sc->pair_off.p; ia.ray_off = (uint32_t *)sc->ray_off.p;
   ia.intervals = nullptr; ia.hits = nullptr;
@@ -376,6 +396,17 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   ba.bw = (uint2 *)sc->bw.p; ba.bands = (MsBand *)sc->bands.p; ba.counters = counters;
   if (banded) CK(ms_order_banded(ba, st));
   else CK(ms_order_single(ba, st));
+  // the band table comes back to the host: stage (e) is launched with one CTA per four rays of the band (the
+  // hardware's CTA scheduler balances them; see ms_composite.cu).  A single band is the whole frame: no readback.
+  std::vector<MsBand> band_tab((size_t)n_bands);
+  if (n_bands == 1) {
+    band_tab[0].q_lo = 0u; band_tab[0].q_hi = (uint32_t)R; band_tab[0].slot0 = 0u; band_tab[0].pad = 0u;
+  } else {
+    ENS_HOST(sc, (size_t)n_bands * sizeof(MsBand));
+    CK(cudaMemcpyAsync(sc->pinned_bands, sc->bands.p, (size_t)n_bands * sizeof(MsBand), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    memcpy(band_tab.data(), sc->pinned_bands, (size_t)n_bands * sizeof(MsBand));
+  }
 
   ia.wave_c = wave_c;
   ia.intervals = (MsInterval *)sc->intervals.p;
@@ -431,7 +462,7 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
       else CK(ms_mlp_f32(ma, st));
     }
     CK(rec(4 + 2 * b));
-    ca.band = (MsBand *)sc->bands.p + b;
+    ca.band = band_tab[b];
     CK(ms_composite(ca, st));
   }
   CK(rec(3 + 2 * n_bands));
@@ -613,6 +644,7 @@ int ms_scene_destroy(ms_scene *sc) {
   for (Buf *b : scratch_bufs(sc)) free_buf(*b);
   free_buf(sc->host_rgb); free_buf(sc->host_alpha); free_buf(sc->host_feat);
   if (sc->pinned) cudaFreeHost(sc->pinned);
+  if (sc->pinned_bands) cudaFreeHost(sc->pinned_bands);
   for (cudaEvent_t e : sc->ev) cudaEventDestroy(e);
   if (sc->frame_done) cudaEventDestroy(sc->frame_done);
   (void)cudaGetLastError();
@@ -819,6 +851,8 @@ int ms_debug_prim_frames(ms_scene *sc, float *A, float *M) {
   if (M) CK(cudaMemcpy(M, sc->M, (size_t)sc->n * 36, cudaMemcpyDeviceToHost));
   return MS_OK;
 }
+
+int64_t ms_launch_count_total(void) { return (int64_t)ms_launch_count; }
 
 const char *ms_error_string(int code) {
   switch (code) {

@@ -9,13 +9,13 @@
 // SEGMENTS (= the intervals of one primitive inside one band and wave), of intervals and of 128-row blocks.
 // Stages (d) and (e) are then launched per band on a staging buffer of one band's size.
 //
-// Depth WAVES give the early termination of P:437 real effect: a tile's list is sorted by entry depth z_entry, a
-// lower bound of t for every sample of the primitive (t >= z_cam >= z_entry).  Wave w of a band evaluates the
-// list ranks [first(w), first(w+1)) of every tile.  Before wave w >= 1, every sample in front of
-// B = z_entry(first entry of wave w) has been evaluated, and the transmittance over those samples is a product --
-// independent of their order.  A ray whose product is already below t_stop/2 stops inside that prefix whatever the
-// later hits hold (the factor 2 covers fp32 rounding in the final compositing order), so its later intervals are
-// dropped before they are encoded.  The image is bitwise the one without waves.
+// Depth WAVES give the early termination of P:437 real effect: a tile's list is sorted by entry depth, so wave w of
+// a band -- the list ranks [first(w), first(w+1)) of every tile -- holds the primitives behind those of the earlier
+// waves.  Before wave w >= 1 every ray knows B = the smallest t_in among its own hits still to come; the samples
+// already evaluated with t < B precede everything not yet evaluated, and the transmittance over them is a product,
+// independent of their order.  A ray whose product is already below t_stop/2 stops inside that prefix whatever
+// the later hits hold (the factor 2 covers fp32 rounding in the final compositing order), so its later intervals
+// are dropped before they are encoded.  The image is bitwise the one without waves.
 #include "ms_internal.cuh"
 
 namespace {
@@ -181,35 +181,43 @@ __global__ void __launch_bounds__(256) wave_alive_kernel(MsWaveArgs a) {
   const int lane = threadIdx.x & 31;
   const uint32_t warp_g = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = (gridDim.x * blockDim.x) >> 5;
   const MsBand band = a.bands[a.band];
-  const uint32_t T2 = (uint32_t)(a.grid.tile * a.grid.tile);
   const uint32_t K = (uint32_t)a.K;
-  const uint32_t first = ms_wave_first(a.wave, a.wave_c);
   uint32_t n_dead = 0;
   for (uint32_t q = band.q_lo + warp_g; q < band.q_hi; q += n_warps) {
     if (!a.alive[q]) continue;
     const uint32_t off = a.ray_off[q];
     const uint32_t n = a.ray_off[q + 1] - off;
     if (n == 0) continue;
-    int tx, ty;
-    ms_pos_tile(a.grid, (int)(q / T2), &tx, &ty);
-    const int tile = ty * a.grid.tiles_x + tx;
-    const uint32_t i = a.tile_start[tile] + first;
-    if (i >= a.tile_start[tile + 1]) continue;          // the tile has no entry in this wave or later
-    // every sample of every entry from rank `first` on lies at t >= B (t >= z_cam >= z_entry; the margin covers
-    // the fp32 rounding of both sides)
-    const float B = __uint_as_float((uint32_t)((a.keys[i] >> a.prim_bits) & 0xffffffffull)) - a.margin;
     const MsHit *hits = a.hits + off;
+    // The ray's hits are in list order, so those of earlier waves (all evaluated: the ray is alive) are a prefix
+    // [0, m).  B = the smallest t_in among the hits still to come: every sample not yet evaluated lies at t >= B
+    // (t_k = t_in + (k + 1/2) delta >= t_in in canonical fp32), so the evaluated samples with t < B precede all of
+    // them in the (t, primitive, k) order whatever their values turn out to be.
+    uint32_t m = 0;
+    float B = 3.0e38f;
+    for (uint32_t h = lane; h < n; h += 32) {
+      const MsHit g = hits[h];
+      if (g.wave < a.wave) ++m;
+      else B = fminf(B, g.t_in);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      m += __shfl_xor_sync(FULL, m, o);
+      B = fminf(B, __shfl_xor_sync(FULL, B, o));
+    }
+    if (m == n || m == 0) continue;                      // nothing left to drop / nothing evaluated yet
     const float4 *stg = a.staging + (size_t)(off - band.slot0) * K;
     float p = 1.0f;
-    for (uint32_t s = lane; s < n * K; s += 32) {
+    for (uint32_t s = lane; s < m * K; s += 32) {
       const uint32_t h = s / K, k = s - h * K;
       const MsHit g = hits[h];
-      if (g.wave >= a.wave) break;                       // hits are in list order: earlier waves are a prefix
       const float t = ms_sample_tm(g.t_in, g.delta, (int)k, a.contact);
       if (t < B) p *= __ldg(&stg[s].w);
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) p *= __shfl_xor_sync(FULL, p, o);
+    // the transmittance over that prefix is a product, independent of the order: below t_stop / 2 the ray stops
+    // inside the prefix (the factor 2 covers fp32 rounding in the order the final compositing multiplies in)
     if (lane == 0 && p < 0.5f * a.t_stop) {
       a.alive[q] = 0;
       ++n_dead;
@@ -218,28 +226,43 @@ __global__ void __launch_bounds__(256) wave_alive_kernel(MsWaveArgs a) {
   if (lane == 0 && n_dead) atomicAdd(&a.counters[MS_CNT_DEAD_RAYS], n_dead);
 }
 
-// one warp per segment of the (band, wave): the intervals of dead rays are squeezed out, in place
+// one CTA per segment of the (band, wave), 256 intervals at a time: the intervals of dead rays are squeezed out,
+// in place (a chunk is loaded completely before any of it is stored, and it is stored at or in front of where it
+// was loaded from)
 __global__ void __launch_bounds__(256) wave_compact_kernel(MsWaveArgs a) {
-  const int lane = threadIdx.x & 31;
-  const uint32_t warp_g = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = (gridDim.x * blockDim.x) >> 5;
+  __shared__ uint32_t wsum[8];
+  __shared__ uint32_t kept_s;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint2 r = a.bw[a.band * MS_MAX_WAVES + a.wave];
   const uint32_t lt = (1u << lane) - 1u;
-  for (uint32_t g = r.x + warp_g; g < r.y; g += n_warps) {
+  for (uint32_t g = r.x + blockIdx.x; g < r.y; g += gridDim.x) {
     const uint32_t base = a.grp_iv0[g], n = a.grp_iv0[g + 1] - base;
-    uint32_t kept = 0;
-    for (uint32_t c = 0; c < n; c += 32) {
-      const uint32_t idx = c + lane;
+    __syncthreads();
+    if (threadIdx.x == 0) kept_s = 0u;
+    __syncthreads();
+    for (uint32_t c = 0; c < n; c += 256) {
+      const uint32_t idx = c + threadIdx.x;
       const bool valid = idx < n;
       MsInterval iv;
       iv.ray = 0;
       if (valid) iv = a.intervals[base + idx];
       const bool keep = valid && a.alive[(uint32_t)iv.ray] != 0;
-      const uint32_t ballot = __ballot_sync(FULL, keep);       // also: every lane has loaded before any lane stores
-      if (keep) a.intervals[base + kept + __popc(ballot & lt)] = iv;
-      kept += __popc(ballot);
-      __syncwarp();
+      const uint32_t ballot = __ballot_sync(FULL, keep);
+      if (lane == 0) wsum[warp] = __popc(ballot);
+      __syncthreads();                                   // every interval of the chunk is loaded; warp counts visible
+      uint32_t before = kept_s;
+      for (int w = 0; w < warp; ++w) before += wsum[w];
+      if (keep) a.intervals[base + before + __popc(ballot & lt)] = iv;
+      __syncthreads();
+      if (threadIdx.x == 0) {
+        uint32_t t = kept_s;
+        for (int w = 0; w < 8; ++w) t += wsum[w];
+        kept_s = t;
+      }
+      __syncthreads();
     }
-    if (lane == 0) {
+    if (threadIdx.x == 0) {
+      const uint32_t kept = kept_s;
       a.grp_cnt_c[g] = kept;
       a.grp_blocks_c[g] = (uint32_t)(((uint64_t)kept * (uint64_t)a.K + MS_ROWS - 1) / MS_ROWS);
       if (n > kept) atomicAdd(&a.counters[MS_CNT_SKIPPED], n - kept);
@@ -369,7 +392,7 @@ int ms_banded_key_bits(size_t P, int prim_bits, int n_bands, int *group_bits) {
 cudaError_t ms_wave_prepare(const MsWaveArgs &a, cudaStream_t s) {
   wave_alive_kernel<<<a.n_sm * 8, 256, 0, s>>>(a);
   MS_CHECK_LAUNCH();
-  wave_compact_kernel<<<a.n_sm * 4, 256, 0, s>>>(a);
+  wave_compact_kernel<<<a.n_sm * 8, 256, 0, s>>>(a);
   MS_CHECK_LAUNCH();
   wave_scan_kernel<<<1, 1024, 0, s>>>(a);
   MS_CHECK_LAUNCH();

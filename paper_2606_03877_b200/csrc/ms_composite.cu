@@ -105,20 +105,22 @@ __device__ __forceinline__ void load_hits(WarpSmem &sm, const MsHit *__restrict_
   }
 }
 
-template <int FEAT>  // 0: rgb/alpha only; 1: + linear head features; 2: + Eq.7 slot features (contact mode, K = 1)
+template <int FEAT, bool DBG>  // FEAT 0: rgb/alpha only; 1: + linear head features; 2: + Eq.7 slot features (contact mode, K = 1); DBG: record the order (MS_FLAG_KEEP_ORDER)
 __global__ void __launch_bounds__(CW * 32, FEAT == 0 ? 12 : (FEAT == 1 ? 9 : 8)) composite_kernel(MsCompositeArgs a) {
   __shared__ WarpSmem s_all[CW];
   __shared__ float s_w[FEAT ? CW : 1][FEAT ? CAP : 1];   // weight of the window's r-th merged sample (features only)
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const MsBand band = *a.band;
+  const MsBand band = a.band;
   WarpSmem &sm = s_all[warp];
   const int K = a.K, nf = a.n_feat;
   uint32_t n_stopped = 0;                                   // rays of this warp that stopped before their last sample
   // one warp per ray slot of the band (tile-major ray order: consecutive slots are neighbouring pixels of one
   // tile, and their staged samples are consecutive runs of the band's staging buffer)
-  for (uint32_t q = band.q_lo + blockIdx.x * CW + warp; q < band.q_hi; q += gridDim.x * CW) {
+  // one CTA per CW consecutive slots: the hardware's CTA scheduler balances the rays, which differ widely in cost
+  // (0 .. 40+ hits); a persistent split, static or through a cursor, measured 0.6 - 1.5 ms slower on CFG4
+  for (uint32_t q = band.q_lo + blockIdx.x * CW + warp; q < band.q_hi; q = band.q_hi) {
   int px, py;
-  if (!ms_slot_pixel(a.grid, q, &px, &py)) continue;     // padding slot of a tile that overhangs the image
+  if (!ms_slot_pixel_dev(a.grid, q, &px, &py)) continue;     // padding slot of a tile that overhangs the image
   const size_t ray = (size_t)py * a.grid.W + px;
   __syncwarp();                                           // the previous ray is done with the warp's shared memory
   const uint32_t off = a.ray_off[q];
@@ -150,7 +152,7 @@ __global__ void __launch_bounds__(CW * 32, FEAT == 0 ? 12 : (FEAT == 1 ? 9 : 8))
       if (a.tile_order) rank = (uint32_t)lane;      // the shared per-tile order: the hits as stage (c) wrote them
       if (lane < n) {
         sm.ord[rank] = (uint32_t)lane;
-        if (a.dbg_ord) a.dbg_ord[(size_t)off + rank] = (uint32_t)lane;
+        if (DBG) a.dbg_ord[(size_t)off + rank] = (uint32_t)lane;
       }
       __syncwarp();
       const bool valid = lane < n;
@@ -184,7 +186,7 @@ __global__ void __launch_bounds__(CW * 32, FEAT == 0 ? 12 : (FEAT == 1 ? 9 : 8))
       for (uint32_t s = lane; s < S; s += 32) a.coef[loc + s] = make_float4(0.f, 0.f, 0.f, 0.f);
     __syncwarp();
     bool stopped = false;
-    for (uint32_t r0 = 0; r0 < S && (!stopped || a.dbg_ord); r0 += CAP) {
+    for (uint32_t r0 = 0; r0 < S && (!stopped || DBG); r0 += CAP) {
       const uint32_t cnt = S - r0 < (uint32_t)CAP ? S - r0 : (uint32_t)CAP;
       // ---- rank pass: ord[] (and, for a multi-window ray, val[] by rank) ----
       int h = lane / K, k = lane - h * K;
@@ -194,13 +196,13 @@ __global__ void __launch_bounds__(CW * 32, FEAT == 0 ? 12 : (FEAT == 1 ? 9 : 8))
         const uint32_t rk = (a.tile_order ? s : sample_rank(sm, hits, n, K, h, k, &t, a.contact)) - r0;
         if (rk < cnt) {
           sm.ord[rk] = s;
-          if (a.dbg_ord) a.dbg_ord[(size_t)off * (size_t)K + r0 + rk] = s;
+          if (DBG) a.dbg_ord[(size_t)off * (size_t)K + r0 + rk] = s;
         }
         h += dh; k += dk;
         if (k >= K) { k -= K; ++h; }
       }
       __syncwarp();
-      if (stopped) continue;                       // MS_FLAG_KEEP_ORDER: the windows behind the stop are ranked only
+      if (DBG && stopped) continue;                // MS_FLAG_KEEP_ORDER: the windows behind the stop are ranked only
       // ---- composite the window: lane l takes the l-th run of CH consecutive merged samples ----
       // One product scan over the lanes' run products gives every lane its entry transmittance; the
       // run itself is sequential (T <- T e).  The first sample, in merged order, whose T drops
@@ -332,16 +334,16 @@ __global__ void __launch_bounds__(CW * 32, FEAT == 0 ? 12 : (FEAT == 1 ? 9 : 8))
 template <int R>
 __global__ void __launch_bounds__(CW * 32) slot_feature_kernel(MsCompositeArgs a) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const MsBand band = *a.band;
+  const MsBand band = a.band;
   // groups of R consecutive ray slots (R divides the tile edge: one tile row)
-  for (uint32_t q0 = band.q_lo + (blockIdx.x * CW + warp) * R; q0 < band.q_hi; q0 += gridDim.x * CW * R) {
+  for (uint32_t q0 = band.q_lo + (blockIdx.x * CW + warp) * R; q0 < band.q_hi; q0 = band.q_hi) {
   long long ray_of[R];     // output pixel index, -1 for a padding slot
   uint32_t slot_q[R];
 #pragma unroll
   for (int r = 0; r < R; ++r) {
     int px, py;
     slot_q[r] = q0 + r;
-    ray_of[r] = (q0 + r < band.q_hi && ms_slot_pixel(a.grid, q0 + r, &px, &py)) ? (long long)py * a.grid.W + px : -1;
+    ray_of[r] = (q0 + r < band.q_hi && ms_slot_pixel_dev(a.grid, q0 + r, &px, &py)) ? (long long)py * a.grid.W + px : -1;
   }
   const int cf4 = a.c_f >> 2, nq = a.c_f >> 7;
   float4 F[R][4];
@@ -435,28 +437,19 @@ __global__ void __launch_bounds__(CW * 32) slot_feature_kernel(MsCompositeArgs a
 }  // namespace
 
 cudaError_t ms_composite(const MsCompositeArgs &a, cudaStream_t s) {
-  if (a.grid.n_tiles == 0) return cudaSuccess;
-  static int n_sm = 0;
-  if (n_sm == 0) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-  }
-  // persistent warps walking the band's ray slots (the band's extent lives on the device)
-  const size_t slots = (size_t)a.grid.n_tiles * a.grid.tile * a.grid.tile;
-  unsigned grid = (unsigned)n_sm * 12u;
-  if ((slots + CW - 1) / CW < grid) grid = (unsigned)((slots + CW - 1) / CW);
+  const size_t slots = (size_t)a.band.q_hi - a.band.q_lo;
+  if (slots == 0) return cudaSuccess;
+  const unsigned grid = (unsigned)((slots + CW - 1) / CW);
   const bool feat = a.n_feat > 0 && a.out_feat && a.staging_feat;
   const bool slot_feat = a.c_f > 0 && a.out_feat && a.gates && a.coef && a.slots && a.K == 1;
-  if (slot_feat) composite_kernel<2><<<grid, CW * 32, 0, s>>>(a);
-  else if (!feat) composite_kernel<0><<<grid, CW * 32, 0, s>>>(a);
-  else composite_kernel<1><<<grid, CW * 32, 0, s>>>(a);
+  const bool dbg = a.dbg_ord != nullptr;
+  if (slot_feat) { if (dbg) composite_kernel<2, true><<<grid, CW * 32, 0, s>>>(a); else composite_kernel<2, false><<<grid, CW * 32, 0, s>>>(a); }
+  else if (!feat) { if (dbg) composite_kernel<0, true><<<grid, CW * 32, 0, s>>>(a); else composite_kernel<0, false><<<grid, CW * 32, 0, s>>>(a); }
+  else { if (dbg) composite_kernel<1, true><<<grid, CW * 32, 0, s>>>(a); else composite_kernel<1, false><<<grid, CW * 32, 0, s>>>(a); }
   MS_LAUNCHED();
   if (slot_feat) {
     constexpr int R = 4;
-    unsigned g2 = (unsigned)n_sm * 12u;
-    if ((slots / R + CW - 1) / CW < g2) g2 = (unsigned)((slots / R + CW - 1) / CW);
-    slot_feature_kernel<R><<<g2, CW * 32, 0, s>>>(a);
+    slot_feature_kernel<R><<<(unsigned)((slots / R + CW - 1) / CW), CW * 32, 0, s>>>(a);
     MS_LAUNCHED();
   }
   return cudaGetLastError();

@@ -52,6 +52,8 @@ struct MsMlpShape {
 struct MsGrid {
   int tile, tiles_x, tiles_y, n_tiles, G;   // tile edge, tile grid, macro-tile edge in tiles
   int W, H;
+  int tshift;                               // log2(tile)
+  const ushort2 *pos_xy;                    // device [n_tiles]: tile (tx, ty) at position pos (written by stage (c))
 };
 __host__ __device__ __forceinline__ int ms_tile_pos(const MsGrid &g, int tx, int ty) {
   const int mx = tx / g.G, my = ty / g.G;
@@ -71,6 +73,14 @@ __host__ __device__ __forceinline__ void ms_pos_tile(const MsGrid &g, int pos, i
   *ty = my * g.G + rem2 / w;
   *tx = mx * g.G + rem2 % w;
 }
+// device: the same through the position table (no divisions)
+__device__ __forceinline__ bool ms_slot_pixel_dev(const MsGrid &g, uint32_t q, int *x, int *y) {
+  const uint32_t pos = q >> (2 * g.tshift), l = q & ((1u << (2 * g.tshift)) - 1u);
+  const ushort2 t = __ldg(g.pos_xy + pos);
+  *x = ((int)t.x << g.tshift) + (int)(l & ((1u << g.tshift) - 1u));
+  *y = ((int)t.y << g.tshift) + (int)(l >> g.tshift);
+  return *x < g.W && *y < g.H;
+}
 // pixel (x, y) of ray slot q; false for the padding slots of tiles that overhang the image
 __host__ __device__ __forceinline__ bool ms_slot_pixel(const MsGrid &g, uint32_t q, int *x, int *y) {
   const int T2 = g.tile * g.tile;
@@ -84,7 +94,7 @@ __host__ __device__ __forceinline__ bool ms_slot_pixel(const MsGrid &g, uint32_t
 
 // Depth waves: wave w covers the ranks [ms_wave_first(w), ms_wave_first(w + 1)) of a tile's sorted list
 // (C, C, 2C, 4C, ... entries; the last wave takes the rest).  C == 0: a single wave.
-#define MS_MAX_WAVES 6
+#define MS_MAX_WAVES 4
 __host__ __device__ __forceinline__ uint32_t ms_wave_first(int w, int C) {
   return w <= 0 ? 0u : (uint32_t)C << (w - 1);
 }
@@ -247,6 +257,7 @@ struct MsIsectArgs {
   const uint32_t *tile_start;  // [n_tiles+1]
   const float *A;              // [N][9]
   const float *oprime;         // [N][3]
+  ushort2 *pos_xy;             // [n_tiles] (count pass: out) tile coordinates by position
   uint32_t *pair_hits;         // [P]    (count pass: out)   indexed by tile-list index
   uint32_t *ray_hits;          // [R']   (count pass: out)   indexed by ray slot
   const uint32_t *slot_of;     // [P]    (fill pass: in)     tile-list index -> pair slot of the prim-major order
@@ -349,7 +360,7 @@ struct MsCompositeArgs {
   int K, n_feat, contact;
   int tile_order;        // contact mode: the hits are already in the tile's shared order -- no per-ray merge
   float t_stop;
-  const MsBand *band;    // device: ray slots and staging origin of this launch
+  MsBand band;           // ray slots and staging origin of this launch
   const uint32_t *ray_off;  // [R'+1]
   const MsHit *hits;
   const float4 *staging;

@@ -28,7 +28,9 @@ __global__ void isect_kernel(MsIsectArgs a) {
   const int lx = threadIdx.x % T, ly = threadIdx.x / T;
   const int x = tile_x * T + lx, y = tile_y * T + ly;
   const bool valid = x < a.cam.W && y < a.cam.H;
-  const uint32_t q = (uint32_t)ms_tile_pos(a.grid, tile_x, tile_y) * (uint32_t)(T * T) + threadIdx.x;   // ray slot
+  const int pos = ms_tile_pos(a.grid, tile_x, tile_y);
+  const uint32_t q = (uint32_t)pos * (uint32_t)(T * T) + threadIdx.x;   // ray slot
+  if (!FILL && threadIdx.x == 0) a.pos_xy[pos] = make_ushort2((unsigned short)tile_x, (unsigned short)tile_y);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint32_t lt = (1u << lane) - 1u;
   float d[3] = {0.f, 0.f, 1.f};

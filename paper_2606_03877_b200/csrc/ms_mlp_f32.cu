@@ -39,9 +39,16 @@ __global__ void __launch_bounds__(MS_ROWS) mlp_f32_kernel(MsMlpArgs a) {
   const MsMlpShape &sh = a.shape;
   const LaunchView lv(a.segs);
   int cur_prim = -1;
-  for (uint32_t blk = blockIdx.x; blk < lv.n_blocks; blk += gridDim.x) {
+  // the CTA walks a contiguous run of the launch's blocks: the weights are reloaded only when the primitive changes
+  const uint32_t blk_lo = (uint32_t)(((uint64_t)lv.n_blocks * blockIdx.x) / gridDim.x);
+  const uint32_t blk_hi = (uint32_t)(((uint64_t)lv.n_blocks * (blockIdx.x + 1)) / gridDim.x);
+  for (uint32_t blk = blk_lo; blk < blk_hi; ++blk) {
   __syncthreads();                       // the previous block is done with w_s and s_seg
-  if (threadIdx.x == 0) s_seg = find_seg(lv.bo, (int)(lv.r.y - lv.r.x), lv.base, blk);
+  if (threadIdx.x == 0) {
+    int sgm = blk == blk_lo ? find_seg(lv.bo, (int)(lv.r.y - lv.r.x), lv.base, blk) : s_seg;
+    while (lv.bo[sgm + 1] - lv.base <= blk) ++sgm;     // segments without blocks are skipped
+    s_seg = sgm;
+  }
   __syncthreads();
   const uint32_t g = lv.r.x + (uint32_t)s_seg;
   const int prim = a.segs.prim ? (int)a.segs.prim[g] : (int)g;
@@ -143,9 +150,16 @@ __global__ void __launch_bounds__(MS_ROWS / SPT) mlp_f32_w32_kernel(MsMlpArgs a)
   const MsMlpShape &sh = a.shape;
   const LaunchView lv(a.segs);
   int cur_prim = -1;
-  for (uint32_t blk = blockIdx.x; blk < lv.n_blocks; blk += gridDim.x) {
+  // the CTA walks a contiguous run of the launch's blocks: the weights are reloaded only when the primitive changes
+  const uint32_t blk_lo = (uint32_t)(((uint64_t)lv.n_blocks * blockIdx.x) / gridDim.x);
+  const uint32_t blk_hi = (uint32_t)(((uint64_t)lv.n_blocks * (blockIdx.x + 1)) / gridDim.x);
+  for (uint32_t blk = blk_lo; blk < blk_hi; ++blk) {
   __syncthreads();                       // the previous block is done with w_s and s_seg
-  if (threadIdx.x == 0) s_seg = find_seg(lv.bo, (int)(lv.r.y - lv.r.x), lv.base, blk);
+  if (threadIdx.x == 0) {
+    int sgm = blk == blk_lo ? find_seg(lv.bo, (int)(lv.r.y - lv.r.x), lv.base, blk) : s_seg;
+    while (lv.bo[sgm + 1] - lv.base <= blk) ++sgm;     // segments without blocks are skipped
+    s_seg = sgm;
+  }
   __syncthreads();
   const uint32_t g = lv.r.x + (uint32_t)s_seg;
   const int prim = a.segs.prim ? (int)a.segs.prim[g] : (int)g;
@@ -341,7 +355,7 @@ cudaError_t ms_mlp_f32(const MsMlpArgs &a, cudaStream_t s) {
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
   }
-  unsigned grid = (unsigned)n_sm * 16u;
+  unsigned grid = (unsigned)n_sm * 32u;
   if (a.n_blocks_hint > 0 && a.n_blocks_hint < grid) grid = a.n_blocks_hint;
   fn<<<grid, threads, smem, s>>>(a);
   MS_LAUNCHED();

@@ -119,6 +119,14 @@ CONFIGS: dict[str, SceneConfig] = {
                           MLPSpec(6, 0, 2, 32, 0, True, MODE_CONTACT), 1280, 720, 60.0, 5.0, 1, c_f=512),
     "next2": SceneConfig("next2", 6, 2048, 2.0, 0.05, 0.5,
                          MLPSpec(6, 0, 2, 32, 0, False, MODE_CONTACT), 1280, 720, 60.0, 5.0, 1, c_f=512),
+    # S:§8(f) NEXT-3: CFG4's shape with an opaque medium (density bias 8, as in the early-termination pin P9): the
+    # paper's trained scenes are opaque surfaces ("early t[ermination]"), CFG1-5 never terminate a ray
+    "cfg4_opaque": SceneConfig("cfg4_opaque", 3, 4096, 3.0, 0.03, 0.4,
+                               MLPSpec(6, 0, 3, 128, 0, True), 1920, 1080, 60.0, 5.0, 24, sigma_bias=8.0),
+    # CFG4's scene seen from INSIDE the primitive cloud (the paper's Replica / ScanNet rooms): supports
+    # around and behind the eye, long tile lists
+    "cfg4_inside": SceneConfig("cfg4_inside", 3, 4096, 3.0, 0.03, 0.4,
+                               MLPSpec(6, 0, 3, 128, 0, True), 1920, 1080, 60.0, 0.5, 24),
 }
 
 
