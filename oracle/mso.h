@@ -182,6 +182,19 @@ int mso_contact_eval(const mso_scene *, int32_t prim, const float *o, const floa
 /* encoded input vector x[in_dim] for (u, d). */
 int mso_encode(const mso_scene *, const float *u, const float *d, double *x);
 
+/* ---- backward pass (mso_grad.c; S:Sec.8(f) NEXT-4) ----
+ * fp64 forward + backward of the render of pixels pix[0..n_pix) (all of them, in raster order, if pix == NULL) for
+ * a scene given as fp64 arrays (center[n][3], quat[n][4], scale[n][3], weights[n][params]; mlp->weights is ignored),
+ * north-star mode only.  loss = sum over pixels and channels of |C - target| (the L1 term of Eq.8) when
+ * target != NULL; dL/dC = sign(C - target), or g_in[n_pix][3] if given.  Any of the outputs may be NULL: rgb_out
+ * [n_pix][3], g_weights[n][params], g_center[n][3], g_quat[n][4], g_scale[n][3].  All gradient outputs NULL =
+ * forward only (the finite-difference leg of the pins). */
+int mso_loss_grad_f64(int32_t n, const double *center, const double *quat, const double *scale,
+                      const double *weights, const mso_mlp *mlp, const mso_camera *cam, int H, int W, int K,
+                      double t_stop, const int32_t *pix, int64_t n_pix, const double *target, const double *g_in,
+                      double *loss, double *rgb_out, double *g_weights, double *g_center, double *g_quat,
+                      double *g_scale);
+
 #ifdef __cplusplus
 }
 #endif

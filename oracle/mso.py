@@ -301,3 +301,37 @@ def ray(cam, x, y):
     c = _cam(cam)
     lib().mso_ray(C.byref(c), C.c_int(x), C.c_int(y), _ptr(o), _ptr(d))
     return o, d
+
+
+def loss_grad_f64(scene, cam, H, W, K, *, center=None, quat=None, scale=None, weights=None, t_stop=1e-4,
+                  pixels=None, target=None, g_in=None, want_grad=True):
+    """fp64 forward (+ backward) of the render (mso_grad.c).  The scene's arrays may be overridden by fp64 arrays
+    (the finite-difference pins perturb those).  Returns dict(loss, rgb, g_weights, g_center, g_quat, g_scale)."""
+    n = int(scene.center.shape[0])
+    c64 = np.ascontiguousarray(scene.center if center is None else center, np.float64)
+    q64 = np.ascontiguousarray(scene.quat if quat is None else quat, np.float64)
+    s64 = np.ascontiguousarray(scene.scale if scale is None else scale, np.float64)
+    w64 = np.ascontiguousarray(scene.weights if weights is None else weights, np.float64)
+    m = _MLP(scene.mlp.n_freq, scene.mlp.use_viewdir, scene.mlp.n_hidden, scene.mlp.width, scene.mlp.n_feat,
+             None, int(getattr(scene.mlp, "mode", 0)), float(getattr(scene.mlp, "falloff", 4.5)))
+    if pixels is not None:
+        pixels = np.ascontiguousarray(pixels, np.int32)
+        npx = int(pixels.size)
+    else:
+        npx = H * W
+    tgt = None if target is None else np.ascontiguousarray(target, np.float64).reshape(npx, 3)
+    gin = None if g_in is None else np.ascontiguousarray(g_in, np.float64).reshape(npx, 3)
+    loss = C.c_double(0.0)
+    rgb = np.zeros((npx, 3), np.float64)
+    gw = np.zeros_like(w64) if want_grad else None
+    gc = np.zeros_like(c64) if want_grad else None
+    gq = np.zeros_like(q64) if want_grad else None
+    gs = np.zeros_like(s64) if want_grad else None
+    c = _cam(cam)
+    rc = lib().mso_loss_grad_f64(C.c_int32(n), _ptr(c64), _ptr(q64), _ptr(s64), _ptr(w64), C.byref(m), C.byref(c),
+                                 C.c_int(H), C.c_int(W), C.c_int(K), C.c_double(t_stop), _ptr(pixels),
+                                 C.c_int64(npx), _ptr(tgt), _ptr(gin), C.byref(loss), _ptr(rgb), _ptr(gw), _ptr(gc),
+                                 _ptr(gq), _ptr(gs))
+    if rc != 0:
+        raise RuntimeError(f"mso_loss_grad_f64 failed: {rc}")
+    return dict(loss=loss.value, rgb=rgb, g_weights=gw, g_center=gc, g_quat=gq, g_scale=gs)

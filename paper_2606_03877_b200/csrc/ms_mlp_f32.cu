@@ -144,7 +144,7 @@ __global__ void __launch_bounds__(MS_ROWS) mlp_f32_kernel(MsMlpArgs a) {
 // from shared memory feeds 64 FMAs: with one sample per thread the kernel was bound by the
 // shared-memory wavefronts of the broadcast loads (84 % of peak, profiles/r1e_summary.md).
 template <int NH, int SPT>
-__global__ void __launch_bounds__(MS_ROWS / SPT) mlp_f32_w32_kernel(MsMlpArgs a) {
+__global__ void __launch_bounds__(MS_ROWS / SPT, 6) mlp_f32_w32_kernel(MsMlpArgs a) {
   extern __shared__ __align__(16) float w_s[];
   __shared__ int s_seg;
   const MsMlpShape &sh = a.shape;
@@ -355,7 +355,12 @@ cudaError_t ms_mlp_f32(const MsMlpArgs &a, cudaStream_t s) {
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
   }
-  unsigned grid = (unsigned)n_sm * 32u;
+  int occ = 1;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)fn, threads, smem) != cudaSuccess || occ < 1) {
+    (void)cudaGetLastError();
+    occ = 1;
+  }
+  unsigned grid = (unsigned)(n_sm * occ) * 4u;       // whole rounds of resident CTAs: no ragged last round
   if (a.n_blocks_hint > 0 && a.n_blocks_hint < grid) grid = a.n_blocks_hint;
   fn<<<grid, threads, smem, s>>>(a);
   MS_LAUNCHED();

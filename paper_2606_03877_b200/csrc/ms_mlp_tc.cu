@@ -189,19 +189,16 @@ struct TcParams {
 // intervals of one primitive inside the launch's band and wave).  Every role walks the same segments (a pure
 // function of the device tables), so no role has to tell another what comes next.
 struct SegWalk {
-  const uint32_t *bo;      // block offsets of the launch's segments (absolute: any base)
-  const uint32_t *seg_prim;
-  uint32_t g0, cur, b1;    // cur, b1: absolute block numbers
-  int s;
-  __device__ SegWalk(const MsSegs &sg, uint2 r, uint32_t b0, uint32_t b1_)
-      : bo(sg.blk_off + r.x), seg_prim(sg.prim), g0(r.x), s(0) {
-    const uint32_t base = bo[0];
+  const MsSegs &sg;        // the kernel parameter itself: its pointers stay in the constant bank, not in registers
+  uint32_t s, cur, b1;     // absolute segment index; absolute block numbers (in blk_off's numbering)
+  __device__ SegWalk(const MsSegs &sg_, uint2 r, uint32_t b0, uint32_t b1_) : sg(sg_), s(r.x) {
+    const uint32_t base = sg.blk_off[r.x];
     cur = base + b0; b1 = base + b1_;
     if (b0 < b1_) {
-      int lo = 0, hi = (int)(r.y - r.x);
+      uint32_t lo = r.x, hi = r.y;
       while (hi - lo > 1) {
-        int mid = (lo + hi) >> 1;
-        if (bo[mid] <= cur) lo = mid; else hi = mid;
+        const uint32_t mid = (lo + hi) >> 1;
+        if (sg.blk_off[mid] <= cur) lo = mid; else hi = mid;
       }
       s = lo;
     }
@@ -209,12 +206,12 @@ struct SegWalk {
   // returns false when done; else (segment, its primitive, first block inside the segment, number of blocks)
   __device__ bool next(uint32_t &seg, int &prim, uint32_t &first, uint32_t &count) {
     while (cur < b1) {
-      uint32_t pe = bo[s + 1];
-      uint32_t end = pe < b1 ? pe : b1;
+      const uint32_t pe = sg.blk_off[s + 1];
+      const uint32_t end = pe < b1 ? pe : b1;
       if (end > cur) {
-        seg = g0 + (uint32_t)s;
-        prim = seg_prim ? (int)seg_prim[seg] : (int)seg;
-        first = cur - bo[s]; count = end - cur;
+        seg = s;
+        prim = sg.prim ? (int)sg.prim[s] : (int)s;
+        first = cur - sg.blk_off[s]; count = end - cur;
         cur = end;
         if (cur == pe) ++s;
         return true;

@@ -62,3 +62,51 @@ def test_two_ranks_shard_views_and_reduce_times():
     assert res[0][1] + res[1][1] == list(range(n_views))
     assert all(r[2] == 15.0 for r in res)                   # max over ranks, identical on every rank
     assert all(r[3] == float(n_views) for r in res)         # whole-job units
+
+
+def _render_worker(rank: int, world: int, port: int, out):
+    """Each rank renders its share of CFG5's 8 poses (shrunk) -- here with the CPU oracle standing in for the GPU
+    replica -- and the shares are assembled by render_views_sharded's single all-gather."""
+    import numpy as np
+    from oracle import mso
+    from paper_2606_03877_b200 import synth
+    os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world),
+                      MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    msdist.init("gloo")
+    cfg = synth.shrink(synth.CONFIGS["cfg5"], 24, 14)
+    sc, cams = synth.make_scene(cfg), synth.make_cameras(cfg)
+    orc = mso.OracleScene(sc)
+
+    def render_batch(sub):
+        r = [orc.render(c, cfg.height, cfg.width, 4, n_threads=2) for c in sub]
+        return (torch.from_numpy(np.stack([x[0] for x in r])), torch.from_numpy(np.stack([x[1] for x in r])),
+                torch.from_numpy(np.stack([x[2] for x in r])))
+
+    views, full = msdist.render_views_sharded(render_batch, cams)
+    mine, part = msdist.render_views_sharded(render_batch, cams, gather=False)
+    ref = render_batch(cams) if rank == 0 else None
+    ok = True
+    if rank == 0:
+        ok = all(torch.equal(a, b) for a, b in zip(full, ref))
+    ok = ok and list(views) == list(range(len(cams))) and all(
+        torch.equal(p, f[mine.start:mine.stop]) for p, f in zip(part, full))
+    out.put((rank, list(mine), bool(ok)))
+    msdist.barrier()
+    msdist.shutdown()
+
+
+@pytest.mark.timeout(300)
+@pytest.mark.parametrize("world", [2, 3])
+def test_view_sharded_render_equals_the_single_rank_batch_bitwise(world):
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_render_worker, args=(r, world, port, out)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted(out.get(timeout=280) for _ in range(world))
+    for p in procs:
+        p.join(timeout=30)
+        assert p.exitcode == 0
+    assert sum((r[1] for r in res), []) == list(range(8))    # the shards partition CFG5's 8 poses
+    assert all(r[2] for r in res)                            # gathered batch == single-rank batch, bitwise
