@@ -182,12 +182,15 @@ def algorithmic_bytes(cfg, sc) -> dict:
 
 
 def load_dram_profile():
-    """dram__bytes_read.sum + dram__bytes_write.sum per kernel launch from the committed `ncu --set full` captures
-    (profiles/r2_dram_bytes.json: written by hand from the captures it names; null where none was taken)."""
-    path = os.path.join(ROOT, "profiles", "r2_dram_bytes.json")
+    """dram__bytes_read.sum + dram__bytes_write.sum per view and stage, from the committed `ncu --set full` captures
+    (profiles/r2_dram_bytes.csv, copied by hand from the summaries it names; absent workloads -> null)."""
+    path = os.path.join(ROOT, "profiles", "r2_dram_bytes.csv")
+    out = {}
     if os.path.exists(path):
-        return json.load(open(path))
-    return {}
+        for ln in open(path).read().strip().split("\n")[1:]:
+            w, stage, b, src = ln.split(",", 3)
+            out.setdefault(w, {"source": src})[stage] = float(b)
+    return out
 
 
 def measure(api, cfg, args, peaks, stream, barrier, steps, warmup, sampler=None, shard=None):
