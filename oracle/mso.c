@@ -254,8 +254,35 @@ static proj_t project(const mso_scene *s, const mso_camera *cam, int H, int W, i
   float z_hi = czv + rz;
   if (!(z_hi > 0.0f)) return r;                       /* entirely behind the eye plane */
   r.z_entry = z_lo > 0.0f ? z_lo : 0.0f;
-  if (z_lo <= s->eye_guard * rz) {                    /* touches / nears the eye plane: whole image (Q13) */
+  if (z_lo <= s->eye_guard * rz) {
+    /* Touches / nears the eye plane (Q13): the tangent-plane bound degenerates.  Bound the camera-space box of the
+     * support instead, clipped at a depth z_n in front of which every point of the support projects off the image:
+     * the support lies in c -/+ (r_x, r_y, r_z) (r_a = |row_a(M_c)|), so its points are at least
+     * d_box = |max(|c| - r, 0)| from the eye; one with 0 < z < z_n has (x^2 + y^2)/z^2 > d_box^2/z_n^2 - 1, beyond the
+     * farthest image corner rho_max once z_n < d_box / sqrt(1 + rho_max^2) (half of that is taken).  The part with
+     * z >= z_c = max(z_lo, z_n) projects inside [x_l, x_h] / [z_c, z_hi].  Eye inside the box: whole image. */
+    float rx = sqrtf(dot3(Mc[0], Mc[1], Mc[2], Mc[0], Mc[1], Mc[2]));
+    float ry = sqrtf(dot3(Mc[3], Mc[4], Mc[5], Mc[3], Mc[4], Mc[5]));
+    float ex = fabsf(cxv) - rx, ey = fabsf(cyv) - ry, ez = fabsf(czv) - rz;
+    ex = ex > 0.0f ? ex : 0.0f; ey = ey > 0.0f ? ey : 0.0f; ez = ez > 0.0f ? ez : 0.0f;
+    float d2 = (ex * ex + ey * ey) + ez * ez;
     r.visible = 1; r.px0 = 0; r.px1 = W - 1; r.py0 = 0; r.py1 = H - 1;
+    if (!(d2 > 0.0f)) return r;
+    float wx = (float)W - cam->cx, wy = (float)H - cam->cy;
+    float tx = (cam->cx > wx ? cam->cx : wx) / cam->fx, ty = (cam->cy > wy ? cam->cy : wy) / cam->fy;
+    float zn = (0.5f * sqrtf(d2)) / sqrtf(1.0f + (tx * tx + ty * ty));
+    float zc = z_lo > zn ? z_lo : zn;
+    zc = zc < z_hi ? zc : z_hi;
+    float xl = cxv - rx, xh = cxv + rx, yl = cyv - ry, yh = cyv + ry;
+    float x_lo = cam->fx * (xl < 0.0f ? xl / zc : xl / z_hi) + cam->cx;
+    float x_hi = cam->fx * (xh > 0.0f ? xh / zc : xh / z_hi) + cam->cx;
+    float y_lo = cam->fy * (yl < 0.0f ? yl / zc : yl / z_hi) + cam->cy;
+    float y_hi = cam->fy * (yh > 0.0f ? yh / zc : yh / z_hi) + cam->cy;
+    r.px0 = clamp_lo(x_lo - 0.5f, W);
+    r.px1 = clamp_hi(x_hi - 0.5f, W);
+    r.py0 = clamp_lo(y_lo - 0.5f, H);
+    r.py1 = clamp_hi(y_hi - 0.5f, H);
+    r.visible = (r.px0 <= r.px1) && (r.py0 <= r.py1);
     return r;
   }
   float zz = dot3(Mc[6], Mc[7], Mc[8], Mc[6], Mc[7], Mc[8]) - czv * czv;   /* < 0 here */

@@ -103,8 +103,33 @@ __global__ void project_kernel(int n, const float *__restrict__ center, const fl
   if (z_hi > 0.0f) {
     ze = z_lo > 0.0f ? z_lo : 0.0f;
     int px0, px1, py0, py1;
-    if (z_lo <= __fmul_rn(eye_guard, rz)) {      // Q13: touches / nears the eye plane
+    if (z_lo <= __fmul_rn(eye_guard, rz)) {
+      // Q13: touches / nears the eye plane, where the tangent-plane bound degenerates.  The camera-space box
+      // c -/+ (r_x, r_y, r_z) of the support is bounded instead, clipped at a depth z_n in front of which every point
+      // of the support projects beyond the farthest image corner; eye inside the box: whole image.
       px0 = 0; px1 = cam.W - 1; py0 = 0; py1 = cam.H - 1;
+      const float rx = __fsqrt_rn(ms_dot3(Mc[0], Mc[1], Mc[2], Mc[0], Mc[1], Mc[2]));
+      const float ry = __fsqrt_rn(ms_dot3(Mc[3], Mc[4], Mc[5], Mc[3], Mc[4], Mc[5]));
+      float ex = __fsub_rn(fabsf(cv[0]), rx), ey = __fsub_rn(fabsf(cv[1]), ry), ez = __fsub_rn(fabsf(cv[2]), rz);
+      ex = ex > 0.0f ? ex : 0.0f; ey = ey > 0.0f ? ey : 0.0f; ez = ez > 0.0f ? ez : 0.0f;
+      const float d2 = __fadd_rn(__fadd_rn(__fmul_rn(ex, ex), __fmul_rn(ey, ey)), __fmul_rn(ez, ez));
+      if (d2 > 0.0f) {
+        const float wx = __fsub_rn((float)cam.W, cam.cx), wy = __fsub_rn((float)cam.H, cam.cy);
+        const float tx = __fdiv_rn(cam.cx > wx ? cam.cx : wx, cam.fx), ty = __fdiv_rn(cam.cy > wy ? cam.cy : wy, cam.fy);
+        const float zn = __fdiv_rn(__fmul_rn(0.5f, __fsqrt_rn(d2)),
+                                   __fsqrt_rn(__fadd_rn(1.0f, __fadd_rn(__fmul_rn(tx, tx), __fmul_rn(ty, ty)))));
+        float zc = z_lo > zn ? z_lo : zn;
+        zc = zc < z_hi ? zc : z_hi;
+        const float xl = __fsub_rn(cv[0], rx), xh = __fadd_rn(cv[0], rx), yl = __fsub_rn(cv[1], ry), yh = __fadd_rn(cv[1], ry);
+        const float x_lo = __fadd_rn(__fmul_rn(cam.fx, xl < 0.0f ? __fdiv_rn(xl, zc) : __fdiv_rn(xl, z_hi)), cam.cx);
+        const float x_hi = __fadd_rn(__fmul_rn(cam.fx, xh > 0.0f ? __fdiv_rn(xh, zc) : __fdiv_rn(xh, z_hi)), cam.cx);
+        const float y_lo = __fadd_rn(__fmul_rn(cam.fy, yl < 0.0f ? __fdiv_rn(yl, zc) : __fdiv_rn(yl, z_hi)), cam.cy);
+        const float y_hi = __fadd_rn(__fmul_rn(cam.fy, yh > 0.0f ? __fdiv_rn(yh, zc) : __fdiv_rn(yh, z_hi)), cam.cy);
+        px0 = clamp_lo(__fsub_rn(x_lo, 0.5f), cam.W);
+        px1 = clamp_hi(__fsub_rn(x_hi, 0.5f), cam.W);
+        py0 = clamp_lo(__fsub_rn(y_lo, 0.5f), cam.H);
+        py1 = clamp_hi(__fsub_rn(y_hi, 0.5f), cam.H);
+      }
     } else {
       float zz = __fsub_rn(rz2, __fmul_rn(cv[2], cv[2]));
       float xl, xh, yl, yh;

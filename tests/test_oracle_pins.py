@@ -457,6 +457,53 @@ def test_projection_aabb_is_conservative_and_tight():
     assert n_tight > 50
 
 
+def test_near_eye_box_bound_is_conservative_and_beats_the_whole_image():
+    """Q13: a support that touches or straddles the eye plane is bounded by its camera-space box
+    clipped at the depth in front of which everything projects off the image.  Eye INSIDE CFG4's primitive cloud:
+    points on every such ellipsoid, projected in fp64, land inside the rectangle whenever they land on the image;
+    most of these supports no longer cover the whole image."""
+    cfg = synth.shrink(synth.CONFIGS["cfg4_inside"], 480, 270)
+    sc = synth.make_scene(cfg)
+    cam = synth.make_cameras(cfg)[0]
+    orc = mso.OracleScene(sc)
+    W, H = cfg.width, cfg.height
+    m = cam.c2w.reshape(3, 4).astype(np.float64)
+    rng = np.random.default_rng(1)
+    w = rng.normal(size=(6000, 3))
+    w /= np.linalg.norm(w, axis=1, keepdims=True)
+    n_near = n_full = n_small = 0
+    for i in range(sc.n):
+        _, R = lam(sc.quat[i], sc.scale[i])
+        # surface and interior points: the clip argument is about every point of the support
+        rad = np.concatenate([np.ones(3000), rng.uniform(0, 1, 3000) ** (1 / 3)])[:, None]
+        pts = sc.center[i].astype(np.float64) + (w * rad * sc.scale[i].astype(np.float64)) @ R.T
+        pc = (pts - m[:, 3]) @ m[:, :3]
+        rz = np.linalg.norm((R * sc.scale[i].astype(np.float64)).T @ m[:, 2])      # |row_z(M_c)|
+        cz = (sc.center[i].astype(np.float64) - m[:, 3]) @ m[:, 2]
+        if not (cz + rz > 0 and cz - rz <= 0.01 * rz):
+            continue                                              # not the near-eye branch
+        n_near += 1
+        vis, (x0, x1, y0, y1), z = orc.project(cam, H, W, i)
+        front = pc[:, 2] > 1e-9
+        px = cam.fx * pc[front, 0] / pc[front, 2] + cam.cx - 0.5
+        py = cam.fy * pc[front, 1] / pc[front, 2] + cam.cy - 0.5
+        inside = (px >= -0.5) & (px <= W - 0.5) & (py >= -0.5) & (py <= H - 0.5)
+        if inside.any():
+            assert vis
+            assert x0 <= np.floor(px[inside].min() + 0.5) and x1 >= np.ceil(px[inside].max() - 0.5)
+            assert y0 <= np.floor(py[inside].min() + 0.5) and y1 >= np.ceil(py[inside].max() - 0.5)
+        if vis and (x0, x1, y0, y1) == (0, W - 1, 0, H - 1):
+            n_full += 1
+        else:
+            n_small += 1
+    assert n_near > 100 and n_small > 0.6 * n_near, (n_near, n_full, n_small)
+    # and the image does not notice: binned == brute force bitwise on a sample of pixels
+    pix = rng.choice(W * H, 400, replace=False).astype(np.int32)
+    a = orc.render(cam, H, W, 4, tile=16, pixels=pix)
+    b = orc.render(cam, H, W, 4, tile=0, pixels=pix)
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]) and a[3].n_intervals == b[3].n_intervals
+
+
 def test_tile_lists_sorted_by_tile_depth_id():
     """NS (a),(b): keys = (tile, z_entry bits, primitive id) ascending; rebuilt here from the
     per-primitive AABBs with numpy lexsort (library)."""
