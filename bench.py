@@ -260,7 +260,8 @@ def measure(api, cfg, args, peaks, stream, barrier, steps, warmup, sampler=None,
         peak = 148 * 128 * 2 * 1.965e9 / 1e12
     alg = algorithmic_bytes(cfg, sc)
     feat_w = cfg.c_f or cfg.mlp.n_feat
-    sample_bytes = 16 + 4 * cfg.mlp.n_feat + (32 if cfg.c_f else 0)
+    feat_b = 2 if (cfg.mlp.bf16 and cfg.mlp.n_feat == 32) else 4      # the tensor path stages its features as fp16
+    sample_bytes = 16 + feat_b * cfg.mlp.n_feat + (32 if cfg.c_f else 0)
     # bytes the design moves per view by construction: staging written by (d) and read by (e), both hit lists
     # written by (c) and read by (d) / (e), the outputs
     stage_bytes_design = 2 * n_eval_view * sample_bytes + 2 * st.n_intervals * 48 + alg["outputs_per_view"]

@@ -325,7 +325,10 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   const bool want_slots = sc->slot_cf > 0 && out_feat != nullptr;   // Eq.7 features (contact mode, K = 1)
 
   // bands: the staging bytes of one sample decide how many hits fit the budget
-  const size_t sample_bytes = sizeof(float4) + (want_feat ? (size_t)sc->shape.n_feat * 4 : 0) + (want_slots ? 2 * sizeof(float4) : 0);
+  // the tensor path stages its 32 feature channels as fp16 (its operands are bf16); the fp32 path keeps fp32
+  const bool feat_half = want_feat && path == MS_PATH_BF16_TC && sc->shape.n_feat == 32;
+  const size_t feat_bytes = want_feat ? (size_t)sc->shape.n_feat * (feat_half ? 2 : 4) : 0;
+  const size_t sample_bytes = sizeof(float4) + feat_bytes + (want_slots ? 2 * sizeof(float4) : 0);
   const int64_t budget = opts->band_bytes == 0 ? MS_BAND_BYTES_DEFAULT : opts->band_bytes;
   size_t cap_hits = n_hits + 1;
   if (budget > 0) {
@@ -373,7 +376,7 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   ENS(sc->intervals, (n_hits + 1) * sizeof(MsInterval));
   ENS(sc->hits, (n_hits + 1) * sizeof(MsHit));
   ENS(sc->staging, (band_hits_cap * (size_t)K + 1) * sizeof(float4));
-  if (want_feat) ENS(sc->staging_feat, (band_hits_cap * (size_t)K + 1) * (size_t)sc->shape.n_feat * 4);
+  if (want_feat) ENS(sc->staging_feat, (band_hits_cap * (size_t)K + 1) * feat_bytes);
   if (want_slots) ENS(sc->staging_gate, (band_hits_cap * (size_t)K + 1) * sizeof(float4));
   if (want_slots) ENS(sc->staging_coef, (band_hits_cap * (size_t)K + 1) * sizeof(float4));
   const bool keep_order = (opts->flags & MS_FLAG_KEEP_ORDER) != 0;
@@ -422,14 +425,16 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   ma.n_blocks_hint = 0;
   ma.intervals = (MsInterval *)sc->intervals.p;
   ma.staging = (float4 *)sc->staging.p;
-  ma.staging_feat = want_feat ? (float *)sc->staging_feat.p : nullptr;
+  ma.staging_feat = want_feat ? sc->staging_feat.p : nullptr;
+  ma.feat_half = feat_half ? 1 : 0;
   ma.staging_gate = want_slots ? (float4 *)sc->staging_gate.p : nullptr;
   MsCompositeArgs ca;
   ca.grid = grid; ca.K = K; ca.n_feat = sc->shape.n_feat; ca.t_stop = opts->t_stop;
   ca.contact = sc->shape.mode == MS_MODE_CONTACT;
   ca.tile_order = tile_order;
   ca.ray_off = (uint32_t *)sc->ray_off.p; ca.hits = (MsHit *)sc->hits.p; ca.staging = (float4 *)sc->staging.p;
-  ca.staging_feat = want_feat ? (float *)sc->staging_feat.p : nullptr;
+  ca.staging_feat = want_feat ? sc->staging_feat.p : nullptr;
+  ca.feat_half = feat_half ? 1 : 0;
   ca.gates = want_slots ? (const float4 *)sc->staging_gate.p : nullptr;
   ca.coef = want_slots ? (float4 *)sc->staging_coef.p : nullptr;
   ca.slots = sc->slots; ca.c_f = sc->slot_cf;

@@ -12,6 +12,8 @@
 // scan per window links the runs.  Features
 // (32 channels): four 128 B rows per warp load.
 // HBM-bound by design: reads 16 B (+ 4 n_feat B) per sample and 16 B per hit, once.
+#include <cuda_fp16.h>
+
 #include "ms_internal.cuh"
 
 namespace {
@@ -106,7 +108,7 @@ __device__ __forceinline__ void load_hits(WarpSmem &sm, const MsHit *__restrict_
 }
 
 template <int FEAT, bool DBG>  // FEAT 0: rgb/alpha only; 1: + linear head features; 2: + Eq.7 slot features (contact mode, K = 1); DBG: record the order (MS_FLAG_KEEP_ORDER)
-__global__ void __launch_bounds__(CW * 32, FEAT == 0 ? 12 : (FEAT == 1 ? 9 : 8)) composite_kernel(MsCompositeArgs a) {
+__global__ void __launch_bounds__(CW * 32, FEAT == 0 ? 12 : 8) composite_kernel(MsCompositeArgs a) {
   __shared__ WarpSmem s_all[CW];
   __shared__ float s_w[FEAT ? CW : 1][FEAT ? CAP : 1];   // weight of the window's r-th merged sample (features only)
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -128,6 +130,7 @@ __global__ void __launch_bounds__(CW * 32, FEAT == 0 ? 12 : (FEAT == 1 ? 9 : 8))
   float T = 1.0f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
   float F[MS_MAX_OUT / 32] = {0.f, 0.f};
   float4 F4 = make_float4(0.f, 0.f, 0.f, 0.f);   // n_feat == 32: channels 4*(lane%8)..+3 of the samples of lane group lane/8
+  float4 G4 = make_float4(0.f, 0.f, 0.f, 0.f);   // fp16 staging: F4, G4 = channels 8*(lane%4)..+7 of lane group lane/4
   if (n > 0) {
     const MsHit *hits = a.hits + off;
     const size_t loc = (size_t)(off - band.slot0);        // the ray's first hit inside the band's staging buffers
@@ -257,8 +260,39 @@ __global__ void __launch_bounds__(CW * 32, FEAT == 0 ? 12 : (FEAT == 1 ? 9 : 8))
       }
       if (FEAT == 1) {
         __syncwarp();
-        const float *fbase = a.staging_feat + loc * (size_t)K * (size_t)nf;
-        if (nf == 32) {
+        const float *fbase = reinterpret_cast<const float *>(a.staging_feat) + loc * (size_t)K * (size_t)nf;
+        if (nf == 32 && a.feat_half) {
+          // fp16 rows of 64 B (tensor path): lane group g = lane/4 takes sample r+g, lane%4 the channels
+          // 8*(lane%4)..+7: one warp load covers eight rows; four loads in flight per lane before the FMAs.
+          const uint4 *hbase = reinterpret_cast<const uint4 *>(a.staging_feat) + loc * (size_t)K * 4;
+          const int g = lane >> 2, c8 = lane & 3;
+          for (uint32_t r = 0; r < done; r += 32) {
+            uint4 f[4];
+            float wv[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              const uint32_t rr = r + 8 * q + g;
+              f[q] = make_uint4(0u, 0u, 0u, 0u);
+              wv[q] = 0.f;
+              if (rr < done) {
+                const uint32_t s = sm.ord[rr];
+                wv[q] = s_w[FEAT ? warp : 0][FEAT ? rr : 0];
+                f[q] = __ldg(hbase + (size_t)s * 4 + c8);
+              }
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              const float2 a0 = __half22float2(*reinterpret_cast<const __half2 *>(&f[q].x));
+              const float2 a1 = __half22float2(*reinterpret_cast<const __half2 *>(&f[q].y));
+              const float2 a2 = __half22float2(*reinterpret_cast<const __half2 *>(&f[q].z));
+              const float2 a3 = __half22float2(*reinterpret_cast<const __half2 *>(&f[q].w));
+              F4.x = fmaf(wv[q], a0.x, F4.x); F4.y = fmaf(wv[q], a0.y, F4.y);
+              F4.z = fmaf(wv[q], a1.x, F4.z); F4.w = fmaf(wv[q], a1.y, F4.w);
+              G4.x = fmaf(wv[q], a2.x, G4.x); G4.y = fmaf(wv[q], a2.y, G4.y);
+              G4.z = fmaf(wv[q], a3.x, G4.z); G4.w = fmaf(wv[q], a3.y, G4.w);
+            }
+          }
+        } else if (nf == 32) {
           // lane group g = lane/8 takes sample r+g, lane%8 takes channels 4*(lane%8)..+3: one warp
           // load covers four 128 B rows; four loads in flight per lane before the FMAs.
           const int g = lane >> 3, c4 = lane & 7;
@@ -307,7 +341,19 @@ __global__ void __launch_bounds__(CW * 32, FEAT == 0 ? 12 : (FEAT == 1 ? 9 : 8))
   if (lane < 3) a.out_rgb[3 * ray + lane] = lane == 0 ? C0 : (lane == 1 ? C1 : C2);
   if (lane == 3) a.out_alpha[ray] = 1.0f - T;
   if (FEAT == 1) {
-    if (nf == 32) {
+    if (nf == 32 && a.feat_half) {
+#pragma unroll
+      for (int o = 4; o < 32; o <<= 1) {
+        F4.x += __shfl_xor_sync(FULL, F4.x, o); F4.y += __shfl_xor_sync(FULL, F4.y, o);
+        F4.z += __shfl_xor_sync(FULL, F4.z, o); F4.w += __shfl_xor_sync(FULL, F4.w, o);
+        G4.x += __shfl_xor_sync(FULL, G4.x, o); G4.y += __shfl_xor_sync(FULL, G4.y, o);
+        G4.z += __shfl_xor_sync(FULL, G4.z, o); G4.w += __shfl_xor_sync(FULL, G4.w, o);
+      }
+      if (lane < 4) {
+        reinterpret_cast<float4 *>(a.out_feat + ray * 32)[2 * lane] = F4;
+        reinterpret_cast<float4 *>(a.out_feat + ray * 32)[2 * lane + 1] = G4;
+      }
+    } else if (nf == 32) {
 #pragma unroll
       for (int o = 8; o < 32; o <<= 1) {
         F4.x += __shfl_xor_sync(FULL, F4.x, o); F4.y += __shfl_xor_sync(FULL, F4.y, o);

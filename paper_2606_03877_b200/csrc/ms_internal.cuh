@@ -349,7 +349,8 @@ struct MsMlpArgs {
   uint32_t n_blocks_hint;         // blocks of the launch if the host knows them, else 0
   const MsInterval *intervals;
   float4 *staging;                // band-local: [(slot - slot0)*K + k] (r,g,b,e)
-  float *staging_feat;            // same indexing x n_feat, or NULL
+  void *staging_feat;             // same indexing x n_feat, or NULL: fp32, or fp16 when feat_half
+  int feat_half;                  // tensor path, n_feat == 32: features staged as fp16 rows of 64 B
   float4 *staging_gate;           // slot gates g_k of Eq.7 (contact mode) or NULL
 };
 cudaError_t ms_mlp_f32(const MsMlpArgs &a, cudaStream_t s);
@@ -364,7 +365,8 @@ struct MsCompositeArgs {
   const uint32_t *ray_off;  // [R'+1]
   const MsHit *hits;
   const float4 *staging;
-  const float *staging_feat;
+  const void *staging_feat;
+  int feat_half;         // staging_feat holds fp16 rows (tensor path, n_feat == 32)
   const float4 *gates;   // slot gates (Eq.7) or NULL
   float4 *coef;          // (T alpha) g_k per hit: composite_kernel<2> -> slot_feature_kernel
   const float *slots;    // [N][4][c_f] slot embeddings

@@ -131,7 +131,7 @@ __global__ void __launch_bounds__(MS_ROWS) mlp_f32_kernel(MsMlpArgs a) {
   a.staging[out] = r;
   if (a.staging_gate) a.staging_gate[out] = ms_slot_gates(u);
   if (a.staging_feat)
-    for (int c = 0; c < sh.n_feat; ++c) a.staging_feat[out * sh.n_feat + c] = raw[4 + c];
+    for (int c = 0; c < sh.n_feat; ++c) reinterpret_cast<float *>(a.staging_feat)[out * sh.n_feat + c] = raw[4 + c];
   }
 }
 
@@ -329,7 +329,7 @@ __global__ void __launch_bounds__(MS_ROWS / SPT, 6) mlp_f32_w32_kernel(MsMlpArgs
         float f = bh[4 + c];
 #pragma unroll
         for (int i = 0; i < 32; ++i) f = fmaf(h[p][i], w[i * n_out + 4 + c], f);
-        a.staging_feat[out * sh.n_feat + c] = f;
+        reinterpret_cast<float *>(a.staging_feat)[out * sh.n_feat + c] = f;
       }
   }
   }

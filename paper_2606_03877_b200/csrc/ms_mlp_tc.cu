@@ -138,6 +138,11 @@ __device__ __forceinline__ uint32_t relu_pack_bf16(float lo, float hi) {
   asm("cvt.rn.relu.bf16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
   return d;
 }
+__device__ __forceinline__ uint32_t pack_f16(float lo, float hi) {
+  uint32_t d;
+  asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
+  return d;
+}
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
   uint32_t d;
   asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
@@ -181,7 +186,7 @@ struct TcParams {
   const MsInterval *intervals;
   const uint8_t *image;
   float4 *staging;
-  float *staging_feat;
+  void *staging_feat;     // n_feat == 32: fp16 rows of 64 B; other widths: fp32
   float4 *staging_gate;   // CONTACT + Eq.7 slot features: the four gates of every hit, or NULL
 };
 
@@ -710,30 +715,38 @@ __global__ void __launch_bounds__(32 * tc_warps(WIDTH, NOUT), 1) mlp_tc_kernel(c
           if (CONTACT) v.w = 1.0f - (1.0f - v.w) * fall;   // alpha = (1 - exp(-sigma l)) g
           p.staging[out_idx] = v;
           if constexpr (NOUT > 16) if (feat && p.n_feat != 32) {
-            float *f = p.staging_feat + out_idx * (size_t)p.n_feat;
+            float *f = reinterpret_cast<float *>(p.staging_feat) + out_idx * (size_t)p.n_feat;
 #pragma unroll
             for (int c = 0; c < 32; ++c)
               if (c < p.n_feat) f[c] = __uint_as_float(r[4 + c]);
           }
         }
         if constexpr (NOUT > 16) if (feat && p.n_feat == 32) {
-          // 32 feature channels = one 128 B row per sample.  A lane storing its own row touches 32 lines
-          // per instruction (one LSU wavefront each -- measured: HD was the slowest role of CFG5);
-          // transposed through shared memory, eight lanes store one row and an instruction touches 4.
-          float4 *buf = reinterpret_cast<float4 *>(s_hd + (warp - W_HD) * (32 * TC_HD_ROW));
+          // 32 feature channels, staged as fp16 (the contraction's operands are bf16; fp16 keeps three more bits):
+          // one 64 B row per sample.  A lane storing its own row would touch 32 lines per instruction (one LSU
+          // wavefront each -- measured in round 1: HD was the slowest role of CFG5, and at 128 B per sample the
+          // kernel wrote 2.7 TB/s); transposed through shared memory, four lanes store one row and an instruction
+          // touches 8 rows.  Row stride 80 B: conflict-free for the 16-byte accesses on both sides.
+          constexpr uint32_t HROW = 80;
+          uint8_t *buf = s_hd + (warp - W_HD) * (32 * TC_HD_ROW);
 #pragma unroll
-          for (int c = 0; c < 8; ++c)
-            *reinterpret_cast<float4 *>(reinterpret_cast<uint8_t *>(buf) + lane * TC_HD_ROW + c * 16) =
-                make_float4(__uint_as_float(r[4 + 4 * c]), __uint_as_float(r[5 + 4 * c]),
-                            __uint_as_float(r[6 + 4 * c]), __uint_as_float(r[7 + 4 * c]));
+          for (int c = 0; c < 4; ++c) {
+            uint4 v;
+            v.x = pack_f16(__uint_as_float(r[4 + 8 * c + 0]), __uint_as_float(r[4 + 8 * c + 1]));
+            v.y = pack_f16(__uint_as_float(r[4 + 8 * c + 2]), __uint_as_float(r[4 + 8 * c + 3]));
+            v.z = pack_f16(__uint_as_float(r[4 + 8 * c + 4]), __uint_as_float(r[4 + 8 * c + 5]));
+            v.w = pack_f16(__uint_as_float(r[4 + 8 * c + 6]), __uint_as_float(r[4 + 8 * c + 7]));
+            *reinterpret_cast<uint4 *>(buf + lane * HROW + c * 16) = v;
+          }
           __syncwarp();
           const unsigned long long my = valid ? (unsigned long long)out_idx : ~0ull;
+          uint8_t *fbase = reinterpret_cast<uint8_t *>(p.staging_feat);
 #pragma unroll
-          for (int it = 0; it < 8; ++it) {
-            const int rr = it * 4 + (lane >> 3);
+          for (int it = 0; it < 4; ++it) {
+            const int rr = it * 8 + (lane >> 2);
             const unsigned long long idx = __shfl_sync(0xffffffffu, my, rr);
-            const float4 v = *reinterpret_cast<const float4 *>(reinterpret_cast<const uint8_t *>(buf) + rr * TC_HD_ROW + (lane & 7) * 16);
-            if (idx != ~0ull) reinterpret_cast<float4 *>(p.staging_feat + (size_t)idx * 32)[lane & 7] = v;
+            const uint4 v = *reinterpret_cast<const uint4 *>(buf + rr * HROW + (lane & 3) * 16);
+            if (idx != ~0ull) *reinterpret_cast<uint4 *>(fbase + (size_t)idx * 64 + (lane & 3) * 16) = v;
           }
           __syncwarp();
         }
