@@ -186,6 +186,20 @@ int ms_render_batch(ms_scene *scene, const ms_camera *cameras, int32_t n_views, 
 int ms_render_host(ms_scene *scene, const ms_camera *cameras, int32_t n_views, int32_t H, int32_t W,
                    const ms_opts *opts, float *host_rgb, float *host_alpha, float *host_feat);
 
+/* Backward pass of ms_render (S:Sec.8(f) NEXT-4; the losses of P:132-142 Eq.8-9 need dL/dtheta and dL/d(mu, s, q)):
+ * given d_rgb = dL/d out_rgb (DEVICE [H][W][3]) it ADDS dL/dtheta_i into g_weights (DEVICE [n][P], the layout of
+ * ms_mlp.weights), dL/dmu into g_center [n][3] and, if not NULL, dL/dq into g_quat [n][4] (q as given: the gradient is
+ * tangent to q's sphere, q enters through q/|q|) and dL/ds into g_scale [n][3]; the caller zeroes them, several views
+ * accumulate.  It renders the view first (stages (a)-(e), fp32 path, the whole frame staged, no early-stop waves) and
+ * then walks C = sum_j T_j alpha_j c_j (Eq.6) backwards: compositing, activations, the Linear+ReLU
+ * layers, Eq.5, the chord interval and its K midpoint samples, the frame A = diag(1/s) R(q)^T.  Samples behind
+ * the early stop carry no gradient; a ReLU at exactly 0 has derivative 0; feature channels (n_feat) carry none (their
+ * loss, Eq.9, is not built).  fp32 arithmetic with atomic accumulation (the sums' order is not fixed).
+ * MS_MODE_LOCAL only, and MLPs whose activations of 128 samples fit shared memory (widths <= 64 at three hidden
+ * layers): else MS_ERR_UNSUPPORTED_SHAPE.  Enqueued on opts->stream like ms_render. */
+int ms_backward(ms_scene *scene, const ms_camera *camera, int32_t H, int32_t W, const ms_opts *opts,
+                const float *d_rgb, float *g_weights, float *g_center, float *g_quat, float *g_scale);
+
 /* Counts of the last view rendered on this scene.  Waits for that view to finish (its device counters). */
 int ms_last_stats(ms_scene *scene, ms_stats *out);
 /* Device time of each stage of the last view rendered with MS_FLAG_STAGE_TIMES, in ms,

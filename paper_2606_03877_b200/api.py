@@ -24,7 +24,7 @@ FLAG_TILE_ORDER = 4     # contact mode: the paper's shared per-tile order (P:109
 STAGES = ("bin", "sort", "isect", "mlp", "composite")
 
 EXPORTS = ["ms_scene_create", "ms_scene_set_slots", "ms_scene_destroy", "ms_render", "ms_render_batch", "ms_render_host",
-           "ms_last_stats", "ms_last_stage_ms", "ms_stage_accum", "ms_debug_tile_lists", "ms_debug_intervals",
+           "ms_backward", "ms_last_stats", "ms_last_stage_ms", "ms_stage_accum", "ms_debug_tile_lists", "ms_debug_intervals",
            "ms_debug_sample_order", "ms_debug_sample_order_all", "ms_debug_prim_frames", "ms_launch_count_total", "ms_error_string", "ms_last_cuda_error"]
 
 
@@ -232,6 +232,23 @@ class Scene:
                                         C.byref(o), _ptr(rgb), _ptr(alpha), _ptr(feat)),
                     "ms_render_host")
         return rgb, alpha, feat
+
+    def backward(self, cam, H, W, K, d_rgb, *, t_stop=1e-4, tile=16, grads=None, stream=None):
+        """ms_backward: d_rgb = dL/d out_rgb, float32 CUDA [H, W, 3].  Returns (g_weights [n, P], g_center [n, 3],
+        g_quat [n, 4], g_scale [n, 3]) float32 CUDA tensors; pass `grads` to accumulate into existing ones."""
+        if grads is None:
+            P = self.mlp.params_per_prim
+            grads = (torch.zeros((self.n, P), dtype=torch.float32, device="cuda"),
+                     torch.zeros((self.n, 3), dtype=torch.float32, device="cuda"),
+                     torch.zeros((self.n, 4), dtype=torch.float32, device="cuda"),
+                     torch.zeros((self.n, 3), dtype=torch.float32, device="cuda"))
+        d_rgb = d_rgb.contiguous()
+        assert d_rgb.dtype == torch.float32 and d_rgb.is_cuda and d_rgb.numel() == H * W * 3
+        o = self._opts(K, t_stop, tile, PATH_FP32, 0, stream)
+        c = _cam_struct(cam)
+        self._check(_lib.ms_backward(self._h, C.byref(c), C.c_int32(H), C.c_int32(W), C.byref(o), _ptr(d_rgb),
+                                     _ptr(grads[0]), _ptr(grads[1]), _ptr(grads[2]), _ptr(grads[3])), "ms_backward")
+        return grads
 
     # -- introspection -------------------------------------------------------------
     def stats(self) -> Stats:

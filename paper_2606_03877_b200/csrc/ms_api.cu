@@ -55,6 +55,15 @@ struct ms_scene {
   bool frame_pending = false;
   bool prev_terminated = false;      // MS_WAVES_AUTO: the previous view had rays stopping early
   // last view
+  struct LastView {
+    bool valid = false;
+    MsGrid grid{};
+    MsCam cam{};
+    int K = 0, n_bands = 0, n_waves = 0, banded = 0, path = 0;
+    size_t n_hits = 0;
+    float t_stop = 0.f;
+  } last;
+  Buf bwd_rgb, bwd_alpha, bwd_ord, bwd_gstage, bwd_ivgrad, bwd_gA;   // backward pass scratch
   ms_stats stats{};
   bool debug_valid = false, order_valid = false;
   int dbg_H = 0, dbg_W = 0, dbg_K = 0, dbg_prim_bits = 0;
@@ -490,6 +499,9 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   sc->stats.staging_bytes = (int64_t)(band_hits_cap * (size_t)K * sample_bytes);   // what this view needed
   sc->stats.scratch_bytes = (int64_t)scratch_total(sc);
   sc->dbg_K = K;
+  sc->last.valid = true; sc->last.grid = grid; sc->last.cam = cam; sc->last.K = K; sc->last.n_bands = n_bands;
+  sc->last.n_waves = n_waves; sc->last.banded = banded ? 1 : 0; sc->last.path = path; sc->last.n_hits = n_hits;
+  sc->last.t_stop = opts->t_stop;
   if (opts->flags & MS_FLAG_KEEP_DEBUG) {
     sc->debug_valid = true;
     sc->order_valid = keep_order;
@@ -647,6 +659,8 @@ int ms_scene_destroy(ms_scene *sc) {
   cudaFree(sc->slots);
   ms_tc_free(&sc->tc);
   for (Buf *b : scratch_bufs(sc)) free_buf(*b);
+  free_buf(sc->bwd_rgb); free_buf(sc->bwd_alpha); free_buf(sc->bwd_ord); free_buf(sc->bwd_gstage);
+  free_buf(sc->bwd_ivgrad); free_buf(sc->bwd_gA);
   free_buf(sc->host_rgb); free_buf(sc->host_alpha); free_buf(sc->host_feat);
   if (sc->pinned) cudaFreeHost(sc->pinned);
   if (sc->pinned_bands) cudaFreeHost(sc->pinned_bands);
@@ -697,6 +711,51 @@ int ms_render_host(ms_scene *sc, const ms_camera *cams, int32_t n_views, int32_t
     if (feat) CK(cudaMemcpyAsync(host_feat + v * px * nf, sc->host_feat.p, px * (size_t)nf * 4, cudaMemcpyDeviceToHost, st));
   }
   CK(cudaStreamSynchronize(st));
+  return MS_OK;
+}
+
+int ms_backward(ms_scene *sc, const ms_camera *camera, int32_t H, int32_t W, const ms_opts *opts, const float *d_rgb,
+                float *g_weights, float *g_center, float *g_quat, float *g_scale) {
+  if (!d_rgb || !g_weights || !g_center) return MS_ERR_INVALID_ARG;
+  int rc = check_render_args(sc, camera, 1, H, W, opts, d_rgb, d_rgb);
+  if (rc != MS_OK) return rc;
+  if (sc->shape.mode != MS_MODE_LOCAL || ms_mlp_bwd_smem(sc->shape) == 0) return MS_ERR_UNSUPPORTED_SHAPE;
+  cudaStream_t st = (cudaStream_t)opts->stream;
+  // forward stages (a)-(e) on the fp32 path with the whole frame staged (one band, no waves): the backward kernels
+  // read the staged (rgb, e) of every sample
+  ms_opts o2 = *opts;
+  o2.band_bytes = -1; o2.waves = -1; o2.path = MS_PATH_FP32;
+  o2.flags &= ~(MS_FLAG_KEEP_ORDER | MS_FLAG_TILE_ORDER | MS_FLAG_STAGE_TIMES);
+  const size_t px = (size_t)H * W;
+  ENS(sc->bwd_rgb, px * 12);
+  ENS(sc->bwd_alpha, px * 4);
+  rc = render_view(sc, camera, H, W, &o2, (float *)sc->bwd_rgb.p, (float *)sc->bwd_alpha.p, nullptr);
+  if (rc != MS_OK) return rc;
+  if (!sc->last.valid || sc->last.n_bands != 1 || sc->last.banded) return MS_ERR_CUDA;
+  const size_t n_hits = sc->last.n_hits, n_samples = n_hits * (size_t)sc->last.K;
+  if (n_hits == 0) return MS_OK;
+  const long long launches0 = ms_launch_count;
+  ENS(sc->bwd_ord, (n_samples + 1) * 4);
+  ENS(sc->bwd_gstage, (n_samples + 1) * sizeof(float4));
+  ENS(sc->bwd_ivgrad, (n_hits + 1) * 32);
+  ENS(sc->bwd_gA, (size_t)sc->n * 36);
+  CK(cudaMemsetAsync(sc->bwd_ivgrad.p, 0, (n_hits + 1) * 32, st));
+  CK(cudaMemsetAsync(sc->bwd_gA.p, 0, (size_t)sc->n * 36, st));
+  MsCompositeBwdArgs cb;
+  cb.grid = sc->last.grid; cb.K = sc->last.K; cb.t_stop = sc->last.t_stop;
+  cb.ray_off = (uint32_t *)sc->ray_off.p; cb.hits = (MsHit *)sc->hits.p; cb.staging = (float4 *)sc->staging.p;
+  cb.d_rgb = d_rgb; cb.ord = (uint32_t *)sc->bwd_ord.p; cb.gstage = (float4 *)sc->bwd_gstage.p;
+  CK(ms_composite_bwd(cb, st));
+  MsMlpBwdArgs mb;
+  mb.shape = sc->shape; mb.cam = sc->last.cam; mb.K = sc->last.K; mb.n_prims = sc->n; mb.n_hits = n_hits;
+  mb.center = sc->center; mb.A = sc->A; mb.quat = sc->quat; mb.scale = sc->scale; mb.weights_f32 = sc->weights_f32;
+  mb.segs.iv0 = (uint32_t *)sc->grp_iv0.p; mb.segs.cnt = nullptr; mb.segs.blk_off = (uint32_t *)sc->blk_off.p;
+  mb.segs.prim = nullptr; mb.segs.range = (uint2 *)sc->bw.p; mb.segs.band = (MsBand *)sc->bands.p;
+  mb.intervals = (MsInterval *)sc->intervals.p; mb.staging = (float4 *)sc->staging.p;
+  mb.gstage = (float4 *)sc->bwd_gstage.p; mb.ivgrad = (float *)sc->bwd_ivgrad.p; mb.gA = (float *)sc->bwd_gA.p;
+  mb.g_weights = g_weights; mb.g_center = g_center; mb.g_quat = g_quat; mb.g_scale = g_scale;
+  CK(ms_mlp_bwd(mb, st));
+  sc->stats.n_launches += (int64_t)(ms_launch_count - launches0);
   return MS_OK;
 }
 

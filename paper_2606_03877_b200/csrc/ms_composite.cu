@@ -480,6 +480,94 @@ __global__ void __launch_bounds__(CW * 32) slot_feature_kernel(MsCompositeArgs a
   }
 }
 
+// Backward of the compositing (S:Sec.8(f) NEXT-4; Eq.6, Eq.14): for one ray with dL/dC = g,
+//   dL/dc_j = T_j (1 - e_j) g,     dL/de_j = -T_j (c_j . g) + (sum_{m > j} T_m (1 - e_m) (c_m . g)) / e_j,
+// in the merged (t, primitive, k) order of the forward pass (the same closed-form ranks), samples behind the early
+// stop (Q9) carrying nothing.  One warp per ray: ranks into a global order buffer, a forward product scan that leaves
+// T_j in the output slot, a reverse sum scan that turns it into the two gradients.  Output per sample, at its
+// staging index: (dL/dc_r, dL/dc_g, dL/dc_b, dL/de).
+__global__ void __launch_bounds__(CW * 32) composite_bwd_kernel(MsCompositeBwdArgs a) {
+  __shared__ WarpSmem s_all[CW];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const uint32_t q = blockIdx.x * CW + warp;
+  if (q >= (uint32_t)a.grid.n_tiles << (2 * a.grid.tshift)) return;
+  int px, py;
+  if (!ms_slot_pixel_dev(a.grid, q, &px, &py)) return;
+  WarpSmem &sm = s_all[warp];
+  const uint32_t off = a.ray_off[q];
+  const int n = (int)(a.ray_off[q + 1] - off);
+  if (n == 0) return;
+  const int K = a.K;
+  const size_t ray = (size_t)py * a.grid.W + px;
+  const float g0 = a.d_rgb[3 * ray], g1 = a.d_rgb[3 * ray + 1], g2 = a.d_rgb[3 * ray + 2];
+  const MsHit *hits = a.hits + off;
+  const float4 *stg = a.staging + (size_t)off * (size_t)K;
+  float4 *gst = a.gstage + (size_t)off * (size_t)K;
+  uint32_t *ord = a.ord + (size_t)off * (size_t)K;
+  const uint32_t S = (uint32_t)n * (uint32_t)K;
+  load_hits(sm, hits, n, K, lane, 0);
+  __syncwarp();
+  for (uint32_t s = lane; s < S; s += 32) {
+    const int h = (int)(s / (uint32_t)K), k = (int)(s - (uint32_t)h * (uint32_t)K);
+    float t;
+    ord[sample_rank(sm, hits, n, K, h, k, &t, 0)] = s;
+  }
+  __syncwarp();
+  // forward: transmittance in front of every sample, the stop
+  float T = 1.0f;
+  uint32_t n_used = S;
+  for (uint32_t base = 0; base < S; base += 32) {
+    const uint32_t r = base + lane;
+    const bool valid = r < S;
+    uint32_t s = 0;
+    float e = 1.0f;
+    if (valid) { s = ord[r]; e = stg[s].w; }
+    float p = e;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const float v = __shfl_up_sync(FULL, p, o);
+      if (lane >= o) p *= v;
+    }
+    float excl = __shfl_up_sync(FULL, p, 1);
+    if (lane == 0) excl = 1.0f;
+    if (valid) gst[s].w = T * excl;                           // T_j, replaced by dL/de_j below
+    const unsigned stop = __ballot_sync(FULL, valid && T * p < a.t_stop);
+    if (stop) { n_used = base + (uint32_t)__ffs(stop); break; }   // the stopping sample still counts (Q9)
+    T *= __shfl_sync(FULL, p, 31);
+  }
+  __syncwarp();
+  // backward: suffix sums of T_m (1 - e_m) (c_m . g), from the last used sample to the first
+  float carry = 0.0f;
+  for (int base = (int)((S - 1) / 32) * 32; base >= 0; base -= 32) {
+    const uint32_t r = (uint32_t)base + lane;
+    const bool valid = r < S;
+    const bool used = r < n_used;
+    uint32_t s = 0;
+    float4 v = make_float4(0.f, 0.f, 0.f, 1.f);
+    float Tj = 0.0f;
+    if (valid) { s = ord[r]; v = stg[s]; Tj = gst[s].w; }
+    const float cg = v.x * g0 + v.y * g1 + v.z * g2;
+    const float term = used ? Tj * (1.0f - v.w) * cg : 0.0f;
+    float sum = term;                                          // inclusive sum over the lanes at and above this one
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const float t = __shfl_down_sync(FULL, sum, o);
+      if (lane + o < 32) sum += t;
+    }
+    const float suffix = carry + sum - term;
+    if (valid) {
+      float4 out = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (used) {
+        const float w = Tj * (1.0f - v.w);
+        out.x = w * g0; out.y = w * g1; out.z = w * g2;
+        out.w = -Tj * cg + (v.w > 0.0f ? suffix / v.w : 0.0f);
+      }
+      gst[s] = out;
+    }
+    carry += __shfl_sync(FULL, sum, 0);
+  }
+}
+
 }  // namespace
 
 cudaError_t ms_composite(const MsCompositeArgs &a, cudaStream_t s) {
@@ -498,5 +586,13 @@ cudaError_t ms_composite(const MsCompositeArgs &a, cudaStream_t s) {
     slot_feature_kernel<R><<<(unsigned)((slots / R + CW - 1) / CW), CW * 32, 0, s>>>(a);
     MS_LAUNCHED();
   }
+  return cudaGetLastError();
+}
+
+cudaError_t ms_composite_bwd(const MsCompositeBwdArgs &a, cudaStream_t s) {
+  const size_t slots = (size_t)a.grid.n_tiles * a.grid.tile * a.grid.tile;
+  if (slots == 0) return cudaSuccess;
+  composite_bwd_kernel<<<(unsigned)((slots + CW - 1) / CW), CW * 32, 0, s>>>(a);
+  MS_LAUNCHED();
   return cudaGetLastError();
 }

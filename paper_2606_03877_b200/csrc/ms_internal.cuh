@@ -27,7 +27,7 @@ struct __align__(16) MsInterval {
   float delta;  // (t_out - t_in)/K
   int slot;     // global hit index = ray_off[ray] + h ; sample k lives at staging[slot*K + k]
   float dx, dy, dz;  // unit world-frame ray direction (canonical)
-  int pad;
+  int prim;          // the primitive (the backward pass walks intervals without their segment)
 };
 
 // hit of one ray (ray-major list consumed by stage (e))
@@ -376,3 +376,39 @@ struct MsCompositeArgs {
   float *out_rgb, *out_alpha, *out_feat;
 };
 cudaError_t ms_composite(const MsCompositeArgs &a, cudaStream_t s);
+
+// ---- backward pass (S:Sec.8(f) NEXT-4; ms_backward.cu, ms_composite.cu) -----------------------------------------
+struct MsCompositeBwdArgs {
+  MsGrid grid;
+  int K;
+  float t_stop;
+  const uint32_t *ray_off;
+  const MsHit *hits;
+  const float4 *staging;   // whole frame (one band): (r, g, b, e) at slot * K + k
+  const float *d_rgb;      // [H][W][3] dL/dC
+  uint32_t *ord;           // [n_samples] scratch: sample index by (ray's first sample + rank)
+  float4 *gstage;          // [n_samples] out: (dL/dc_r, dL/dc_g, dL/dc_b, dL/de) at slot * K + k
+};
+cudaError_t ms_composite_bwd(const MsCompositeBwdArgs &a, cudaStream_t s);
+
+struct MsMlpBwdArgs {
+  MsMlpShape shape;
+  MsCam cam;
+  int K, n_prims;
+  size_t n_hits;
+  const float *center, *A, *quat, *scale;
+  const float *weights_f32;
+  MsSegs segs;
+  const MsInterval *intervals;
+  const float4 *staging;
+  const float4 *gstage;
+  float *ivgrad;           // [n_hits][8] scratch, zeroed: dL/d(o'[3], d'[3], t_in, delta) of every interval
+  float *gA;               // [N][9] scratch, zeroed: dL/dA
+  float *g_weights;        // [N][params]  += dL/dtheta
+  float *g_center;         // [N][3]       += dL/dmu
+  float *g_quat;           // [N][4]       += dL/dq
+  float *g_scale;          // [N][3]       += dL/ds
+};
+// smem bytes the MLP backward kernel needs for this shape (0: shape not covered)
+size_t ms_mlp_bwd_smem(const MsMlpShape &sh);
+cudaError_t ms_mlp_bwd(const MsMlpBwdArgs &a, cudaStream_t s);

@@ -89,7 +89,7 @@ __global__ void isect_kernel(MsIsectArgs a) {
           const uint32_t slot = ray_base + my_hits;
           MsInterval iv;
           iv.ray = (int)q; iv.t_in = t_in; iv.delta = delta; iv.slot = (int)slot;
-          iv.dx = d[0]; iv.dy = d[1]; iv.dz = d[2]; iv.pad = 0;
+          iv.dx = d[0]; iv.dy = d[1]; iv.dz = d[2]; iv.prim = sPrim[c];
           a.intervals[sBase[c] + rank] = iv;
           MsHit h;
           h.prim = sPrim[c]; h.t_in = t_in; h.delta = delta;
