@@ -313,6 +313,43 @@ def measure(api, cfg, args, peaks, stream, barrier, steps, warmup, sampler=None,
     return res, sc, cams
 
 
+def measure_backward(api, cfg, args, stream, barrier, steps=5, warmup=3):
+    """ms_backward (S:Sec.8(f) NEXT-4): one call = the forward stages (a)-(e) on the fp32 path + the backward kernels
+    for one view, dL/dC resident in HBM.  Work counted: 3 x the forward MLP FLOPs of the samples (forward recomputed in
+    the backward kernel is not counted twice: forward + dX + dW), against the fp32 FMA peak."""
+    import torch
+    sc = synth.make_scene(cfg)
+    cam = synth.make_cameras(cfg)[0]
+    H, W, K = cfg.height, cfg.width, cfg.K
+    gs = api.Scene(sc)
+    d_rgb = torch.randn((H, W, 3), device="cuda", dtype=torch.float32)
+    with torch.cuda.stream(stream):
+        grads = gs.backward(cam, H, W, K, d_rgb, tile=cfg.tile, t_stop=cfg.t_stop)
+        for _ in range(warmup):
+            gs.backward(cam, H, W, K, d_rgb, tile=cfg.tile, t_stop=cfg.t_stop, grads=grads)
+    barrier()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with torch.cuda.stream(stream):
+        ev0.record(stream)
+        for _ in range(steps):
+            gs.backward(cam, H, W, K, d_rgb, tile=cfg.tile, t_stop=cfg.t_stop, grads=grads)
+        ev1.record(stream)
+    barrier()
+    ms = ev0.elapsed_time(ev1) / steps
+    st = gs.stats()
+    gs.close()
+    del grads, d_rgb
+    torch.cuda.empty_cache()
+    peak = 148 * 128 * 2 * 1.965e9 / 1e12
+    ach = 3 * cfg.mlp.flop_per_sample * st.n_samples / (ms * 1e-3) / 1e12
+    return {"workload": workload_desc(cfg) + ", fp32 path, forward + backward", "ms_per_step": ms,
+            "Mpixels_per_s": H * W / (ms * 1e-3) / 1e6, "samples_per_s": st.n_samples / (ms * 1e-3),
+            "samples": st.n_samples,
+            "roofline": {"bound": "alu", "kernel": "whole call (forward fp32 stages + composite_bwd + mlp_bwd + interval_bwd)",
+                         "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+                         "peak_kind": "fp32 FMA, 148 SMs x 128 lanes x 2 x 1.965 GHz (derived)"}}
+
+
 def run_ours(args, cfg):
     import torch
     from paper_2606_03877_b200 import api
@@ -355,6 +392,10 @@ def run_ours(args, cfg):
                                         ("bound", "kernel", "achieved", "peak", "unit", "frac", "kernel_ms",
                                          "algorithmic_bytes", "stage_bytes_design", "dram_bytes_per_view")}
             others[name]["frame_roofline_frac"] = o["frame_roofline"]["frac"]
+    backward = {}
+    if rank == 0 and world == 1 and args.all_configs:
+        for name in ("cfg1", "cfg3"):
+            backward[name] = measure_backward(api, synth.CONFIGS[name], args, stream, barrier)
     if rank != 0:
         msdist.shutdown()
         return
@@ -387,6 +428,8 @@ def run_ours(args, cfg):
     }
     if others:
         line["all_configs"] = others
+    if backward:
+        line["backward"] = backward
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = {k: v for k, v in time_oracle(cfg, sc, cams, args.cpu_seconds).items()
                                 if k in ("value", "unit", "cores", "kind", "sample", "samples_per_s")}
