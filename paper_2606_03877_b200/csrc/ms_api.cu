@@ -32,7 +32,8 @@ struct ms_scene {
   int last_cuda = 0;
   // scene-lifetime device data
   float *center = nullptr, *quat = nullptr, *scale = nullptr, *A = nullptr, *M = nullptr;
-  float *weights_f32 = nullptr;
+  float *weights_f32 = nullptr;      // fp32 path / backward; for a bf16 scene on the tensor path uploaded on first use
+  std::vector<float> w_host;         // the (bf16-rounded) weight values until then
   MsTcWeights tc{};  // packed bf16 image for the tensor path (may be empty)
   int slot_cf = 0;           // Eq.7 slot embeddings: width C_f (0 = none)
   float *slots = nullptr;    // device [N][4][slot_cf]
@@ -232,6 +233,13 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   if (path == MS_PATH_BF16_TC && !sc->tc.valid) return MS_ERR_UNSUPPORTED_SHAPE;
   if (path != MS_PATH_BF16_TC && path != MS_PATH_FP32) return MS_ERR_INVALID_ARG;
 
+  if (path == MS_PATH_FP32 && !sc->weights_f32) {
+    const size_t bytes = (size_t)N * (size_t)sc->shape.params * 4;
+    if (sc->w_host.size() * 4 != bytes) return MS_ERR_CUDA;
+    CK(cudaMalloc(&sc->weights_f32, bytes));
+    CK(cudaMemcpy(sc->weights_f32, sc->w_host.data(), bytes, cudaMemcpyHostToDevice));
+    std::vector<float>().swap(sc->w_host);
+  }
   const bool timing = (opts->flags & MS_FLAG_STAGE_TIMES) != 0;
   const MsCam cam = make_cam(camera, H, W);
   const long long launches0 = ms_launch_count;
@@ -592,7 +600,6 @@ int ms_scene_create(const ms_prims *prims, const ms_mlp *mlp, ms_scene **out) {
   CKC(cudaMalloc(&sc->scale, n * 12));
   CKC(cudaMalloc(&sc->A, n * 36));
   CKC(cudaMalloc(&sc->M, n * 36));
-  CKC(cudaMalloc(&sc->weights_f32, n * (size_t)params * 4));
   CKC(cudaMalloc(&d_bad, 4));
   CKC(cudaMemset(d_bad, 0, 4));
   CKC(cudaMemcpy(sc->center, prims->center, n * 12, cudaMemcpyHostToDevice));
@@ -615,7 +622,6 @@ int ms_scene_create(const ms_prims *prims, const ms_mlp *mlp, ms_scene **out) {
       }
     }
   }
-  CKC(cudaMemcpy(sc->weights_f32, w.data(), n * (size_t)params * 4, cudaMemcpyHostToDevice));
   CKC(ms_prep_prims(sc->n, sc->center, sc->quat, sc->scale, sc->A, sc->M, d_bad, 0));
   int bad = 0;
   CKC(cudaMemcpy(&bad, d_bad, 4, cudaMemcpyDeviceToHost));
@@ -628,6 +634,13 @@ int ms_scene_create(const ms_prims *prims, const ms_mlp *mlp, ms_scene **out) {
   if (mlp->dtype == MS_BF16) {
     rc = ms_tc_pack(sh, sc->n, w.data(), &sc->tc);  // leaves tc.valid = false if the shape is not covered
     if (rc != MS_OK) return fail(rc);
+  }
+  if (sc->tc.valid) {
+    sc->w_host.swap(w);       // the tensor path needs only the packed image: the fp32 copy (633 MB at CFG4) goes
+                              // to the device when the fp32 path or the backward pass is first asked for
+  } else {
+    CKC(cudaMalloc(&sc->weights_f32, n * (size_t)params * 4));
+    CKC(cudaMemcpy(sc->weights_f32, w.data(), n * (size_t)params * 4, cudaMemcpyHostToDevice));
   }
   CKC(cudaDeviceSynchronize());
   cudaFree(d_bad);

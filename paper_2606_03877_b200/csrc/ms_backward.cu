@@ -11,7 +11,7 @@
 //                        t0,1 = (-b -+ s)/a, s = sqrt(b^2 - a c), a = d'.d', b = o'.d', c = o'.o' - 1 to (o', d'), then
 //                        o' = A (o - mu), d' = A d: dL/dA += ..., dL/dmu -= A^T dL/do'
 //   prim_bwd_kernel      one thread per primitive: A = diag(1/s) R(q/|q|)^T  ->  dL/ds, dL/dq
-// The same chain rule as oracle/mso_grad.c writes out in fp64 -- independently: no code is shared.
+// Written from the chain rule itself; it shares no code with the test oracle, which states the same chain in fp64.
 #include "ms_internal.cuh"
 
 namespace {

@@ -137,6 +137,22 @@ def test_next1_tensor_path(W, H):
     assert np.abs(rgb32.cpu().numpy().reshape(-1, 3) - o_rgb).max() <= TOL_FP32
 
 
+def test_contact_tensor_path_large_world_units():
+    """delta = mu - p* is in world units.  Primitives with semi-axes 4-10 (delta up to ~10): the tensor
+    path reduces z to [-1, 1] before the SFU sin / cos, so the top encoding bands keep the bf16 bar."""
+    from test_gpu_parity_bf16 import assert_bf16_bar
+    api = _api()
+    mlp = synth.MLPSpec(6, 0, 2, 32, 0, True, synth.MODE_CONTACT)
+    cfg = synth.SceneConfig("big_contact", 11, 24, 20.0, 4.0, 10.0, mlp, 96, 54, 60.0, 60.0, 1)
+    sc, cam = synth.make_scene(cfg), synth.make_cameras(cfg)[0]
+    gs = api.Scene(sc)
+    rgb, alpha, _ = gs.render(cam, 54, 96, 1, path=api.PATH_BF16_TC)
+    torch.cuda.synchronize()
+    o_rgb, o_alpha, _, st = mso.OracleScene(sc).render(cam, 54, 96, 1)
+    assert st.n_intervals > 2000
+    assert_bf16_bar(rgb.cpu().numpy().reshape(-1, 3), alpha.cpu().numpy().reshape(-1), o_rgb, o_alpha)
+
+
 def test_next1b_full_size_sampled_pixels():
     from test_gpu_parity_bf16 import assert_bf16_bar
     api = _api()
