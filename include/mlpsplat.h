@@ -125,7 +125,7 @@ typedef struct {
                      which then lives in the L2 cache instead of HBM.  0 = MS_BAND_BYTES_DEFAULT; < 0 = one band
                      (staging of the whole frame).  The image does not depend on it. */
   int32_t waves;  /* Depth waves = early termination that skips MLP work ("early t[ermination]"): > 0 = a tile's
-                     sorted list is evaluated in waves of `waves`, `waves`, 2x, 4x ... entries, and before each
+                     sorted list is evaluated in waves of `waves` entries (at most six, the last takes the rest), and before each
                      wave the rays that have already stopped (T < t_stop/2 over the samples in front of the wave) drop
                      their later intervals.  0 = MS_WAVES_AUTO: on when the previous view rendered on this scene
                      had rays stopping early, else off; < 0 = off.  The image does not depend on it. */

@@ -92,17 +92,16 @@ __host__ __device__ __forceinline__ bool ms_slot_pixel(const MsGrid &g, uint32_t
   return *x < g.W && *y < g.H;
 }
 
-// Depth waves: wave w covers the ranks [ms_wave_first(w), ms_wave_first(w + 1)) of a tile's sorted list
-// (C, C, 2C, 4C, ... entries; the last wave takes the rest).  C == 0: a single wave.
-#define MS_MAX_WAVES 4
+// Depth waves: wave w covers the ranks [w C, (w + 1) C) of a tile's sorted list; the last wave takes the rest.
+// C == 0: a single wave.
+#define MS_MAX_WAVES 6
 __host__ __device__ __forceinline__ uint32_t ms_wave_first(int w, int C) {
-  return w <= 0 ? 0u : (uint32_t)C << (w - 1);
+  return w <= 0 ? 0u : (uint32_t)C * (uint32_t)w;
 }
 __host__ __device__ __forceinline__ int ms_wave_of_rank(uint32_t r, int C) {
-  if (C <= 0 || r < (uint32_t)C) return 0;
-  int w = 1;
-  while (w < MS_MAX_WAVES - 1 && r >= ((uint32_t)C << w)) ++w;
-  return w;
+  if (C <= 0) return 0;
+  const uint32_t w = r / (uint32_t)C;
+  return w < MS_MAX_WAVES - 1 ? (int)w : MS_MAX_WAVES - 1;
 }
 
 // One band = a run of consecutive tiles (in ms_tile_pos order) whose hits fill the staging budget.
@@ -327,9 +326,10 @@ struct MsWaveArgs {
   const MsBand *bands;
   const uint2 *bw;
   uint8_t *alive;              // [R'] 1 = the ray still needs its later hits
-  MsInterval *intervals;       // compacted in place
+  const MsInterval *intervals; // the frame's interval lists (stage (c))
+  MsInterval *intervals_c;     // second buffer: the compacted lists of the waves >= 1
   const uint32_t *grp_iv0;
-  uint32_t *grp_cnt_c;         // [n_seg_cap] compacted interval count
+  uint32_t *grp_cnt_c;         // [n_seg_cap] compacted interval count (zeroed once per frame)
   uint32_t *grp_blocks_c;      // [n_seg_cap] compacted 128-row block count
   uint32_t *blk_off_c;         // [n_seg_cap + 2] block offsets of the compacted wave (relative to its first segment)
   uint32_t *counters;
