@@ -40,7 +40,7 @@ struct ms_scene {
   // per-view scratch
   Buf tile_count, emit_off, rect, z_entry, oprime, keys_a, keys_b, sort_scratch, tile_start, pair_hits_i, pair_hits_j,
       pair_off, slot_of, key2_a, key2_b, flags, gid, grp_key, grp_prim, grp_iv0, grp_blocks, blk_off, grp_cnt_c,
-      grp_blocks_c, blk_off_c, bw, bands, counters, alive, ray_hits, ray_off, scan_scratch, intervals, intervals_c, hits, staging,
+      grp_blocks_c, blk_off_c, bw, bands, counters, alive, ray_hits, ray_off, scan_scratch, intervals, intervals_c, hit_e, hits, staging,
       staging_feat, staging_gate, staging_coef, dbg_ord, pos_xy, host_rgb, host_alpha, host_feat;
   uint32_t *pinned = nullptr;  // host-pinned readback: [0] P, [1..] device counters
   MsBand *pinned_bands = nullptr;  // host-pinned readback of the band table
@@ -132,7 +132,7 @@ std::vector<Buf *> scratch_bufs(ms_scene *sc) {
           &sc->sort_scratch, &sc->tile_start, &sc->pair_hits_i, &sc->pair_hits_j, &sc->pair_off, &sc->slot_of,
           &sc->key2_a, &sc->key2_b, &sc->flags, &sc->gid, &sc->grp_key, &sc->grp_prim, &sc->grp_iv0, &sc->grp_blocks,
           &sc->blk_off, &sc->grp_cnt_c, &sc->grp_blocks_c, &sc->blk_off_c, &sc->bw, &sc->bands, &sc->counters,
-          &sc->alive, &sc->ray_hits, &sc->ray_off, &sc->scan_scratch, &sc->intervals, &sc->intervals_c, &sc->hits, &sc->staging,
+          &sc->alive, &sc->ray_hits, &sc->ray_off, &sc->scan_scratch, &sc->intervals, &sc->intervals_c, &sc->hit_e, &sc->hits, &sc->staging,
           &sc->staging_feat, &sc->staging_gate, &sc->staging_coef, &sc->dbg_ord, &sc->pos_xy};
 }
 
@@ -361,7 +361,7 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   int wave_c = 0;
   if (opts->t_stop > 0.0f && !tile_order) {
     if (opts->waves > 0) wave_c = opts->waves;
-    else if (opts->waves == MS_WAVES_AUTO && sc->prev_terminated) wave_c = 6;   // measured best on cfg4_opaque
+    else if (opts->waves == MS_WAVES_AUTO && sc->prev_terminated) wave_c = 4;   // measured on cfg4_opaque: C = 4 and 6 within noise, 4 skips more
   }
   int n_waves = 1;
   if (wave_c > 0 && max_list > 0) n_waves = ms_wave_of_rank(max_list - 1, wave_c) + 1;
@@ -391,6 +391,8 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
     CK(cudaMemsetAsync(sc->alive.p, 1, R, st));
     CK(cudaMemsetAsync(sc->grp_cnt_c.p, 0, seg_cap * 4, st));
     ENS(sc->intervals_c, (n_hits + 1) * sizeof(MsInterval));
+    ENS(sc->hit_e, (n_hits + 1) * 4);
+    CK(cudaMemsetAsync(sc->hit_e.p, 0xff, (n_hits + 1) * 4, st));   // NaN: no product cached yet
   }
   ENS(sc->intervals, (n_hits + 1) * sizeof(MsInterval));
   ENS(sc->hits, (n_hits + 1) * sizeof(MsHit));
@@ -467,7 +469,7 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   wa.keys = sorted; wa.tile_start = (uint32_t *)sc->tile_start.p; wa.ray_off = (uint32_t *)sc->ray_off.p;
   wa.hits = (MsHit *)sc->hits.p; wa.staging = (float4 *)sc->staging.p; wa.bands = (MsBand *)sc->bands.p;
   wa.bw = (uint2 *)sc->bw.p; wa.alive = (uint8_t *)sc->alive.p; wa.intervals = (MsInterval *)sc->intervals.p;
-  wa.intervals_c = (MsInterval *)sc->intervals_c.p;
+  wa.intervals_c = (MsInterval *)sc->intervals_c.p; wa.hit_e = (float *)sc->hit_e.p;
   wa.grp_iv0 = (uint32_t *)sc->grp_iv0.p; wa.grp_cnt_c = (uint32_t *)sc->grp_cnt_c.p;
   wa.grp_blocks_c = (uint32_t *)sc->grp_blocks_c.p; wa.blk_off_c = (uint32_t *)sc->blk_off_c.p;
   wa.counters = counters; wa.n_sm = sc->n_sm;

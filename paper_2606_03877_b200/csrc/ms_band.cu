@@ -207,12 +207,43 @@ __global__ void __launch_bounds__(256) wave_alive_kernel(MsWaveArgs a) {
     }
     if (m == n || m == 0) continue;                      // nothing left to drop / nothing evaluated yet
     const float4 *stg = a.staging + (size_t)(off - band.slot0) * K;
+    float *hitE = a.hit_e + off;
+    // Lane h takes hit h.  A hit whose last sample lies in front of B contributes the product of all its K samples,
+    // which is cached per hit the first time it is needed (B only grows from wave to wave, so it stays valid): every
+    // staged e is then read about once per frame instead of once per later wave.  A hit that straddles B contributes
+    // its samples with t < B and is not cached.
     float p = 1.0f;
-    for (uint32_t s = lane; s < m * K; s += 32) {
-      const uint32_t h = s / K, k = s - h * K;
-      const MsHit g = hits[h];
-      const float t = ms_sample_tm(g.t_in, g.delta, (int)k, a.contact);
-      if (t < B) p *= __ldg(&stg[s].w);
+    for (uint32_t h0 = 0; h0 < m; h0 += 32) {
+      const uint32_t h = h0 + lane;
+      const bool have = h < m;
+      MsHit g;
+      g.prim = 0; g.t_in = 0.f; g.delta = 0.f; g.wave = 0;
+      if (have) g = hits[h];
+      const float tf = ms_sample_tm(g.t_in, g.delta, 0, a.contact), tl = ms_sample_tm(g.t_in, g.delta, (int)K - 1, a.contact);
+      const bool full = have && tl < B, part = have && !full && tf < B;
+      float val = 1.0f;
+      bool need = part;
+      if (full) {
+        val = hitE[h];
+        need = !(val == val);                             // not cached yet (the buffer starts as NaN)
+      }
+      unsigned todo = __ballot_sync(FULL, need);
+      while (todo) {
+        const int hh = __ffs(todo) - 1;
+        todo &= todo - 1;
+        const float t_in2 = __shfl_sync(FULL, g.t_in, hh), dl2 = __shfl_sync(FULL, g.delta, hh);
+        const bool full2 = __shfl_sync(FULL, full ? 1 : 0, hh) != 0;
+        float pr = 1.0f;
+        for (uint32_t k = lane; k < K; k += 32)
+          if (full2 || ms_sample_tm(t_in2, dl2, (int)k, a.contact) < B) pr *= __ldg(&stg[(size_t)(h0 + hh) * K + k].w);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) pr *= __shfl_xor_sync(FULL, pr, o);
+        if (lane == hh) {
+          val = pr;
+          if (full2) hitE[h] = pr;
+        }
+      }
+      p *= val;
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) p *= __shfl_xor_sync(FULL, p, o);

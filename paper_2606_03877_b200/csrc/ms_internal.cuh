@@ -326,6 +326,7 @@ struct MsWaveArgs {
   const MsBand *bands;
   const uint2 *bw;
   uint8_t *alive;              // [R'] 1 = the ray still needs its later hits
+  float *hit_e;                // [n_hits] product of a hit's K staged e, cached by the wave check (NaN = not yet)
   const MsInterval *intervals; // the frame's interval lists (stage (c))
   MsInterval *intervals_c;     // second buffer: the compacted lists of the waves >= 1
   const uint32_t *grp_iv0;
