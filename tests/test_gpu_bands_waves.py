@@ -137,3 +137,53 @@ def test_waves_never_drop_a_sample_in_front_of_the_stop():
         gs.waves = 1
         out = _render(gs, cam, cfg.height, cfg.width, cfg.K, path=api.PATH_FP32, t_stop=t_stop)
         assert torch.equal(out[0], ref[0]) and torch.equal(out[1], ref[1])
+
+
+@pytest.mark.parametrize("case", ["contact_fp32", "contact_tc_slots", "feat_tc_tile8", "k64_tile32", "k5_ragged"])
+def test_bands_and_waves_across_modes(case):
+    """Bands x waves in every mode that reaches stages (d), (e): the paper's contact-point mode (K = 1, with and
+    without Eq.7 slot features), the widened feature head on the tensor path, the tile sizes 8 and 32, K = 64 and a K
+    that does not divide the 128-row block -- opaque media, so the waves do drop intervals.  Always: bitwise the
+    image (and features) of the one-band, no-wave render, fewer samples evaluated, structures those of the oracle."""
+    api = _api()
+    tile, K, path = 16, 8, api.PATH_FP32
+    if case == "contact_fp32":
+        mlp = synth.MLPSpec(6, 0, 2, 32, 0, False, synth.MODE_CONTACT, falloff=0.0)   # no falloff (Q29's parameter): opaque hits
+        cfg = synth.SceneConfig(case, 21, 160, 1.0, 0.2, 0.6, mlp, 80, 60, 50.0, 3.0, 1, sigma_bias=9.0)
+        K = 1
+    elif case == "contact_tc_slots":
+        mlp = synth.MLPSpec(6, 0, 2, 32, 0, True, synth.MODE_CONTACT, falloff=0.5)
+        cfg = synth.SceneConfig(case, 22, 160, 1.0, 0.2, 0.6, mlp, 80, 60, 50.0, 3.0, 1, sigma_bias=9.0, c_f=128)
+        K, path = 1, api.PATH_BF16_TC
+    elif case == "feat_tc_tile8":
+        mlp = synth.MLPSpec(4, 1, 3, 64, 32, True)
+        cfg = synth.SceneConfig(case, 23, 64, 1.0, 0.3, 0.8, mlp, 72, 50, 50.0, 3.0, 6, sigma_bias=8.0)
+        tile, K, path = 8, 6, api.PATH_BF16_TC
+    elif case == "k64_tile32":
+        mlp = synth.MLPSpec(4, 0, 2, 32, 0, False)
+        cfg = synth.SceneConfig(case, 24, 40, 1.0, 0.3, 0.8, mlp, 70, 45, 50.0, 3.0, 64, sigma_bias=6.0)
+        tile, K = 32, 64
+    else:
+        mlp = synth.MLPSpec(4, 0, 3, 64, 0, True)
+        cfg = synth.SceneConfig(case, 25, 64, 1.0, 0.3, 0.8, mlp, 61, 47, 50.0, 3.0, 5, sigma_bias=8.0)
+        K, path = 5, api.PATH_BF16_TC
+    sc, cam = synth.make_scene(cfg), synth.make_cameras(cfg)[0]
+    H, W = cfg.height, cfg.width
+    gs = api.Scene(sc)
+    gs.waves, gs.band_bytes = -1, -1
+    ref = _render(gs, cam, H, W, K, path=path, tile=tile)
+    st0 = gs.stats()
+    for waves, band_bytes in ((2, -1), (1, 96 << 10), (3, 512 << 10)):
+        gs.waves, gs.band_bytes = waves, band_bytes
+        out = _render(gs, cam, H, W, K, path=path, tile=tile, flags=api.FLAG_DEBUG_ALL)
+        st = gs.stats()
+        for a, b in zip(out, ref):
+            assert (a is None and b is None) or torch.equal(a, b)
+        assert st.n_waves > 1 and st.n_samples == st0.n_samples
+        assert st.n_samples_evaluated < st.n_samples and st.n_dead_rays > 0
+        if band_bytes > 0:
+            assert st.n_bands > 1
+    orc = mso.OracleScene(sc)
+    _, _, _, ost = orc.render(cam, H, W, K, tile=tile)
+    assert ost.n_mlp_evals <= st.n_samples_evaluated
+    assert check_structures(gs, orc, cam, H, W, K, tile, n_order_rays=4) == ost.n_intervals
