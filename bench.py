@@ -207,6 +207,8 @@ def measure(api, cfg, args, peaks, stream, barrier, steps, warmup, sampler=None,
     create_s = time.perf_counter() - t_create
     gs.band_bytes, gs.waves = args.band_bytes, args.waves
     extra_flags = api.FLAG_TILE_ORDER if (args.tile_order and cfg.mlp.mode == 1) else 0
+    if not args.sync:
+        extra_flags |= api.FLAG_NO_SYNC      # views sized from their predecessor: no host synchronisation inside ms_render
     tile_kw = {"tile": args.tile} if args.tile else {"tile": cfg.tile}
     kw = dict(t_stop=cfg.t_stop, **tile_kw)
     with torch.cuda.stream(stream):
@@ -274,7 +276,7 @@ def measure(api, cfg, args, peaks, stream, barrier, steps, warmup, sampler=None,
                             "samples": st.n_samples, "samples_evaluated": n_eval_view, "dead_rays": st.n_dead_rays,
                             "row_blocks": st.n_blocks, "bands": st.n_bands, "waves": st.n_waves,
                             "staging_MB": st.staging_bytes / 1e6, "scratch_GB": st.scratch_bytes / 1e9},
-        "gpu_launches": launches, "scene_create_s": create_s,
+        "gpu_launches": launches, "scene_create_s": create_s, "no_sync_views": bool(st.no_sync), "overflow": bool(st.overflow),
         "e2e": {"value": px_step / (e2e_ms * 1e-3) / 1e6, "unit": UNIT, "h2d_bytes_per_step": 64 * V,
                 "d2h_bytes_per_step": alg["outputs_per_view"] * V, "ms_per_step": e2e_ms},
         "roofline": {"bound": "tensor" if cfg.mlp.bf16 else "alu",
@@ -385,7 +387,8 @@ def run_ours(args, cfg):
                 continue
             o, _, _ = measure(api, synth.CONFIGS[name], args, peaks, stream, barrier, max(3, min(args.steps, 10)), 3)
             others[name] = {k: o[k] for k in ("workload", "ms_per_step", "Mpixels_per_s", "samples_per_s",
-                                              "stage_ms_per_view", "counts_per_view", "gpu_launches", "scene_create_s")}
+                                              "stage_ms_per_view", "counts_per_view", "gpu_launches", "scene_create_s",
+                                              "no_sync_views", "overflow")}
             others[name]["e2e_Mpixels_per_s"] = o["e2e"]["value"]
             others[name]["e2e_ms_per_step"] = o["e2e"]["ms_per_step"]
             others[name]["roofline"] = {k: o["roofline"].get(k) for k in
@@ -418,6 +421,7 @@ def run_ours(args, cfg):
                          % (sc.weights.nbytes / 2 / 1e6, r["counts_per_view"]["staging_MB"]),
                    "tile": args.tile or cfg.tile, "t_stop": cfg.t_stop,
                    "band_bytes": args.band_bytes, "waves": args.waves,
+                   "no_sync": (not args.sync) and bool(r.get("no_sync_views")),
                    "order": "tile-centre shared order (P:109)" if args.tile_order else "exact per-ray order"},
         "samples_per_s": n_samp_job / (ms_step * 1e-3),
         "counts_per_view": r["counts_per_view"], "stage_ms_per_view": r["stage_ms_per_view"],
@@ -461,6 +465,8 @@ def main():
     ap.add_argument("--shard-views", action="store_true",
                     help="N > 1: shard the workload's views over the ranks (strong scaling; cfg5's 8 poses) instead of "
                          "one replica of the whole step per rank")
+    ap.add_argument("--sync", action="store_true",
+                    help="render without MS_FLAG_NO_SYNC (every view reads its counts back to size its scratch)")
     ap.add_argument("--waves", type=int, default=0, help="depth waves (ms_opts.waves): 0 = auto, -1 = off, C > 0 = wave size")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":

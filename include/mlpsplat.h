@@ -108,6 +108,13 @@ enum {
                               contact points t*_{i,c} of the virtual ray through the tile centre (the
                               paper's approximation), instead of the exact per-ray order; the tile lists are
                               then sorted by (tile, t*_{i,c}, primitive id) */
+  MS_FLAG_NO_SYNC = 16,    /* ms_render / ms_render_batch enqueue the whole view without ANY host synchronisation when the
+                              previous synchronising view on this scene had the same H, W, tile, K, path and outputs and was
+                              one band without depth waves: scratch is sized from that view (it carries 25 % of slack) and
+                              every count stays on the device.  A view that needs more than that writes nothing valid:
+                              ms_last_stats then returns MS_ERR_CAPACITY (stats.overflow = 1) and the next render sizes
+                              again.  Ignored (the view synchronises as usual) when there is no such history, with
+                              MS_FLAG_KEEP_DEBUG, or when depth waves are asked for or due. */
   MS_FLAG_KEEP_ORDER = 8   /* stage (e) also records the order it composited every ray's samples in (4 B per sample)
                               for ms_debug_sample_order*: the order the product really used, not a re-derivation */
 };
@@ -151,6 +158,8 @@ typedef struct {
   int64_t n_bands;     /* bands the frame was cut into */
   int64_t n_waves;     /* depth waves per band (1 = off) */
   int64_t staging_bytes; /* size of the staging buffers of stages (d) -> (e) */
+  int64_t overflow;    /* MS_FLAG_NO_SYNC: 1 = the view did not fit the scratch sized from the previous one: invalid */
+  int64_t no_sync;     /* 1 = the view was enqueued without host synchronisation */
 } ms_stats;
 
 enum { MS_STAGE_BIN = 0, MS_STAGE_SORT, MS_STAGE_ISECT, MS_STAGE_MLP, MS_STAGE_COMPOSITE, MS_N_STAGES };
@@ -172,8 +181,9 @@ int ms_scene_destroy(ms_scene *scene);
 /* Renders one view into DEVICE buffers out_rgb [H][W][3], out_alpha [H][W] and, if the MLP has
  * n_feat > 0 and out_feat != NULL, out_feat [H][W][n_feat]; all float32.  rgb / feat are
  * premultiplied sums (no background term, Q14); alpha = 1 - T.  Work is enqueued on
- * opts->stream; the call synchronises that stream twice internally to size its scratch
- * buffers (pair and interval counts), not at the end: outputs are ready once the stream is. */
+ * opts->stream; the call synchronises that stream internally to size its scratch buffers (after the pair count, after
+ * the hit count, and after the band table when the view is cut into several bands), not at the end: outputs are ready
+ * once the stream is.  With MS_FLAG_NO_SYNC and a matching previous view it does not synchronise at all. */
 int ms_render(ms_scene *scene, const ms_camera *camera, int32_t H, int32_t W, const ms_opts *opts,
               float *out_rgb, float *out_alpha, float *out_feat);
 
@@ -200,7 +210,8 @@ int ms_render_host(ms_scene *scene, const ms_camera *cameras, int32_t n_views, i
 int ms_backward(ms_scene *scene, const ms_camera *camera, int32_t H, int32_t W, const ms_opts *opts,
                 const float *d_rgb, float *g_weights, float *g_center, float *g_quat, float *g_scale);
 
-/* Counts of the last view rendered on this scene.  Waits for that view to finish (its device counters). */
+/* Counts of the last view rendered on this scene.  Waits for that view to finish (its device counters).  Returns
+ * MS_ERR_CAPACITY (with *out filled) if that view was a MS_FLAG_NO_SYNC view that overflowed its scratch. */
 int ms_last_stats(ms_scene *scene, ms_stats *out);
 /* Device time of each stage of the last view rendered with MS_FLAG_STAGE_TIMES, in ms,
  * ms[MS_N_STAGES].  Synchronises the recorded events. */

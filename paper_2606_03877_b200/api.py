@@ -19,6 +19,7 @@ MS_F32, MS_BF16 = 0, 1
 PATH_AUTO, PATH_FP32, PATH_BF16_TC = 0, 1, 2
 FLAG_KEEP_DEBUG, FLAG_STAGE_TIMES = 1, 2
 FLAG_KEEP_ORDER = 8     # stage (e) records the order it composited in (ms_debug_sample_order*)
+FLAG_NO_SYNC = 16        # no host synchronisation when the previous view sized the scratch (ms_opts.flags)
 FLAG_DEBUG_ALL = FLAG_KEEP_DEBUG | FLAG_KEEP_ORDER
 FLAG_TILE_ORDER = 4     # contact mode: the paper's shared per-tile order instead of the exact per-ray order
 STAGES = ("bin", "sort", "isect", "mlp", "composite")
@@ -53,7 +54,8 @@ class _Stats(C.Structure):
     _fields_ = [("n_visible", C.c_int64), ("n_pairs", C.c_int64), ("n_intervals", C.c_int64),
                 ("n_samples", C.c_int64), ("n_blocks", C.c_int64), ("scratch_bytes", C.c_int64),
                 ("n_launches", C.c_int64), ("n_samples_evaluated", C.c_int64), ("n_dead_rays", C.c_int64),
-                ("n_bands", C.c_int64), ("n_waves", C.c_int64), ("staging_bytes", C.c_int64)]
+                ("n_bands", C.c_int64), ("n_waves", C.c_int64), ("staging_bytes", C.c_int64), ("overflow", C.c_int64),
+                ("no_sync", C.c_int64)]
 
 
 def _load() -> C.CDLL:
@@ -114,6 +116,8 @@ class Stats:
     n_bands: int = 1
     n_waves: int = 1
     staging_bytes: int = 0
+    overflow: int = 0
+    no_sync: int = 0
 
 
 class Scene:
@@ -253,9 +257,12 @@ class Scene:
     # -- introspection -------------------------------------------------------------
     def stats(self) -> Stats:
         st = _Stats()
-        self._check(_lib.ms_last_stats(self._h, C.byref(st)), "ms_last_stats")
+        rc = _lib.ms_last_stats(self._h, C.byref(st))
+        if rc not in (0, -5):                      # -5: a no-sync view that overflowed its scratch (st.overflow = 1)
+            self._check(rc, "ms_last_stats")
         return Stats(st.n_pairs, st.n_intervals, st.n_samples, st.n_blocks, st.scratch_bytes, st.n_launches,
-                     st.n_visible, st.n_samples_evaluated, st.n_dead_rays, st.n_bands, st.n_waves, st.staging_bytes)
+                     st.n_visible, st.n_samples_evaluated, st.n_dead_rays, st.n_bands, st.n_waves, st.staging_bytes,
+                     st.overflow, st.no_sync)
 
     def stage_ms(self) -> dict[str, float]:
         ms = (C.c_float * len(STAGES))()

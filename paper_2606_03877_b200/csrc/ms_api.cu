@@ -45,10 +45,15 @@ struct ms_scene {
   uint32_t *pinned = nullptr;  // host-pinned readback: [0] P, [1..] device counters
   MsBand *pinned_bands = nullptr;  // host-pinned readback of the band table
   size_t pinned_bands_cap = 0;
-  std::vector<cudaEvent_t> ev;     // MS_FLAG_STAGE_TIMES: 4 + 2 per band + 1 events of the last view
-  int ev_bands = 0;
+  // MS_FLAG_STAGE_TIMES: 4 + 2 per band events per view, in two alternating sets -- a view's events are read when the
+  // view after the next begins (they have long completed then: no wait that would drain the stream)
+  struct EvSet {
+    std::vector<cudaEvent_t> ev;
+    int bands = 0;
+    bool pending = false;          // recorded, not yet added to stage_sum
+  } evs[2];
+  int ev_cur = 0;
   bool ev_valid = false;
-  bool ev_pending = false;         // events of the last view not yet added to stage_sum
   float last_stage_ms[MS_N_STAGES] = {};
   double stage_sum[MS_N_STAGES] = {};
   int64_t stage_views = 0;
@@ -64,6 +69,12 @@ struct ms_scene {
     size_t n_hits = 0;
     float t_stop = 0.f;
   } last;
+  struct History {            // MS_FLAG_NO_SYNC: the last synchronising view, whose scratch sizes the next ones
+    bool valid = false;
+    int H = 0, W = 0, tile = 0, K = 0, path = 0, feat = 0, slots = 0, tile_order = 0;
+  } hist;
+  bool frame_nosync = false;  // the pending view was rendered without host synchronisation
+  bool clear_sticky = false;  // the sticky overflow flag has been seen: clear it before the next view
   Buf bwd_rgb, bwd_alpha, bwd_ord, bwd_gstage, bwd_ivgrad, bwd_gA;   // backward pass scratch
   ms_stats stats{};
   bool debug_valid = false, order_valid = false;
@@ -161,22 +172,25 @@ float round_bf16(float f) {
 // Event layout of a view rendered with MS_FLAG_STAGE_TIMES: 0 start (a), 1 start (b), 2 start (c), 3 start of the band
 // loop; per band b: 4 + 2b before stage (d), 5 + 2b between (d) and (e); 4 + 2 n_bands the end.
 // Adds the stage times of the previous view to the running sums.  Called right after the last event has completed.
-void harvest_stage_times(ms_scene *sc) {
-  if (!sc->ev_pending) return;
-  sc->ev_pending = false;
+int harvest_stage_times(ms_scene *sc, int set) {
+  ms_scene::EvSet &E = sc->evs[set];
+  if (!E.pending) return MS_OK;
+  if (cudaEventSynchronize(E.ev[3 + 2 * E.bands]) != cudaSuccess) { (void)cudaGetLastError(); return MS_ERR_CUDA; }
+  E.pending = false;
   float ms[MS_N_STAGES] = {0.f, 0.f, 0.f, 0.f, 0.f};
   auto el = [&](int a, int b, float *out) {
     float v = 0.f;
-    if (cudaEventElapsedTime(&v, sc->ev[a], sc->ev[b]) != cudaSuccess) { (void)cudaGetLastError(); return false; }
+    if (cudaEventElapsedTime(&v, E.ev[a], E.ev[b]) != cudaSuccess) { (void)cudaGetLastError(); return false; }
     *out += v;
     return true;
   };
   bool ok = el(0, 1, &ms[MS_STAGE_BIN]) && el(1, 2, &ms[MS_STAGE_SORT]) && el(2, 3, &ms[MS_STAGE_ISECT]);
-  for (int b = 0; ok && b < sc->ev_bands; ++b)
+  for (int b = 0; ok && b < E.bands; ++b)
     ok = el(3 + 2 * b, 4 + 2 * b, &ms[MS_STAGE_MLP]) && el(4 + 2 * b, 5 + 2 * b, &ms[MS_STAGE_COMPOSITE]);
-  if (!ok) return;
+  if (!ok) return MS_OK;
   for (int i = 0; i < MS_N_STAGES; ++i) { sc->stage_sum[i] += ms[i]; sc->last_stage_ms[i] = ms[i]; }
   sc->stage_views += 1;
+  return MS_OK;
 }
 
 // Reads the device counters of the last view (waits for it) into sc->stats.
@@ -190,7 +204,30 @@ int finish_frame(ms_scene *sc) {
   sc->stats.n_dead_rays = (int64_t)c[MS_CNT_DEAD_RAYS];
   sc->stats.n_samples_evaluated = sc->stats.n_samples - (int64_t)c[MS_CNT_SKIPPED] * (int64_t)sc->dbg_K;
   sc->prev_terminated = c[MS_CNT_STOPPED_RAYS] > 0;
+  if (sc->frame_nosync) {     // the counts the host never saw
+    sc->frame_nosync = false;
+    sc->stats.n_pairs = (int64_t)c[MS_CNT_PAIRS] | ((int64_t)c[MS_CNT_PAIRS_HI] << 32);
+    sc->stats.n_intervals = (int64_t)c[MS_CNT_HITS] | ((int64_t)c[MS_CNT_HITS_HI] << 32);
+    sc->stats.n_samples = sc->stats.n_intervals * (int64_t)sc->dbg_K;
+    sc->stats.n_samples_evaluated = sc->stats.n_samples;
+    sc->stats.overflow = (c[MS_CNT_OVERFLOW] || c[MS_CNT_STICKY_OVERFLOW]) ? 1 : 0;   // this view, or an earlier one of its batch
+    if (c[MS_CNT_STICKY_OVERFLOW]) sc->clear_sticky = true;
+    if (sc->stats.overflow) {
+      sc->hist.valid = false;  // the next render takes the synchronising path and regrows the scratch
+      sc->stats.n_samples_evaluated = 0;
+    }
+  }
   return MS_OK;
+}
+
+// MS_FLAG_NO_SYNC renders never wait for the previous view: its counters are read only if it has finished
+int finish_frame_if_done(ms_scene *sc, bool no_block) {
+  if (!sc->frame_pending) return MS_OK;
+  if (no_block && cudaEventQuery(sc->frame_done) != cudaSuccess) {
+    (void)cudaGetLastError();
+    return MS_OK;
+  }
+  return finish_frame(sc);
 }
 
 MsCam make_cam(const ms_camera *c, int H, int W) {
@@ -233,6 +270,42 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   if (path == MS_PATH_BF16_TC && !sc->tc.valid) return MS_ERR_UNSUPPORTED_SHAPE;
   if (path != MS_PATH_BF16_TC && path != MS_PATH_FP32) return MS_ERR_INVALID_ARG;
 
+  const int tile_order = (opts->flags & MS_FLAG_TILE_ORDER) != 0;
+  const bool want_feat = sc->shape.n_feat > 0 && out_feat != nullptr;
+  const bool want_slots = sc->slot_cf > 0 && out_feat != nullptr;   // Eq.7 features (contact mode, K = 1)
+  // the tensor path stages its 32 feature channels as fp16 (its operands are bf16); the fp32 path keeps fp32
+  const bool feat_half = want_feat && path == MS_PATH_BF16_TC && sc->shape.n_feat == 32;
+  const size_t feat_bytes = want_feat ? (size_t)sc->shape.n_feat * (feat_half ? 2 : 4) : 0;
+  const size_t sample_bytes = sizeof(float4) + feat_bytes + (want_slots ? 2 * sizeof(float4) : 0);
+  // MS_FLAG_NO_SYNC: no read-back at all if the previous synchronising view had the same shape, was one band without
+  // waves, and left scratch to size this one from (its buffers carry 25 % of slack); the kernels clamp against those
+  // capacities and raise MS_CNT_OVERFLOW, reported by ms_last_stats
+  size_t P_cap = 0, hit_cap = 0;
+  bool nosync = (opts->flags & MS_FLAG_NO_SYNC) != 0 && !(opts->flags & (MS_FLAG_KEEP_DEBUG | MS_FLAG_KEEP_ORDER)) &&
+                sc->hist.valid && sc->hist.H == H && sc->hist.W == W && sc->hist.tile == tile && sc->hist.K == K &&
+                sc->hist.path == path && sc->hist.feat == (want_feat ? 1 : 0) && sc->hist.slots == (want_slots ? 1 : 0) &&
+                sc->hist.tile_order == tile_order && opts->waves <= 0;
+  {  // the previous view's counters (its stats, whether its rays stopped early, whether it overflowed): a view that
+     // may go without synchronisation does not wait for them
+    int rc = finish_frame_if_done(sc, nosync);
+    if (rc != MS_OK) return rc;
+  }
+  if (!sc->hist.valid || (opts->waves == 0 && sc->prev_terminated)) nosync = false;   // overflowed meanwhile / waves due
+  if (nosync) {
+    auto mn = [](size_t a, size_t b) { return a < b ? a : b; };
+    P_cap = mn(mn(sc->keys_a.cap / 8, sc->keys_b.cap / 8), mn(sc->pair_hits_i.cap / 4, sc->slot_of.cap / 4));
+    P_cap = mn(P_cap, mn(sc->pair_hits_j.cap / 4, sc->pair_off.cap / 4));
+    P_cap = P_cap > 4 ? P_cap - 4 : 0;
+    while (P_cap > 0 && (ms_sort_scratch_elems(P_cap) * 4 > sc->sort_scratch.cap ||
+                         (ms_scan_scratch_elems(P_cap) + 16) * 4 > sc->scan_scratch.cap))
+      P_cap = P_cap * 3 / 4;
+    hit_cap = mn(mn(sc->intervals.cap / sizeof(MsInterval), sc->hits.cap / sizeof(MsHit)),
+                 sc->staging.cap / (sizeof(float4) * (size_t)K));
+    if (want_feat) hit_cap = mn(hit_cap, sc->staging_feat.cap / (feat_bytes * (size_t)K));
+    if (want_slots) hit_cap = mn(hit_cap, mn(sc->staging_gate.cap, sc->staging_coef.cap) / (sizeof(float4) * (size_t)K));
+    hit_cap = hit_cap > 2 ? hit_cap - 2 : 0;
+    if (P_cap == 0 || hit_cap == 0 || P_cap >= (1ull << 31) || hit_cap >= (1ull << 31)) nosync = false;
+  }
   if (path == MS_PATH_FP32 && !sc->weights_f32) {
     const size_t bytes = (size_t)N * (size_t)sc->shape.params * 4;
     if (sc->w_host.size() * 4 != bytes) return MS_ERR_CUDA;
@@ -243,32 +316,35 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   const bool timing = (opts->flags & MS_FLAG_STAGE_TIMES) != 0;
   const MsCam cam = make_cam(camera, H, W);
   const long long launches0 = ms_launch_count;
-  if (sc->ev_pending) {  // the previous view's events must be read before they are re-recorded
-    CK(cudaEventSynchronize(sc->ev[3 + 2 * sc->ev_bands]));
-    harvest_stage_times(sc);
-  }
-  {  // the previous view's counters (its stats, and whether its rays stopped early: MS_WAVES_AUTO)
-    int rc = finish_frame(sc);
+  if (timing) {   // this view records into the older set: its events (two views back) are read first
+    sc->ev_cur ^= 1;
+    int rc = harvest_stage_times(sc, sc->ev_cur);
     if (rc != MS_OK) return rc;
   }
-  sc->debug_valid = false;
-  sc->order_valid = false;
   sc->ev_valid = false;
   auto rec = [&](int i) -> cudaError_t {
     if (!timing) return cudaSuccess;
-    while ((int)sc->ev.size() <= i) {
+    std::vector<cudaEvent_t> &ev = sc->evs[sc->ev_cur].ev;
+    while ((int)ev.size() <= i) {
       cudaEvent_t e;
       cudaError_t r = cudaEventCreate(&e);
       if (r != cudaSuccess) return r;
-      sc->ev.push_back(e);
+      ev.push_back(e);
     }
-    return cudaEventRecord(sc->ev[i], st);
+    return cudaEventRecord(ev[i], st);
   };
 
   // ---- (a) projection + key emit ----------------------------------------------------------
   CK(rec(0));
-  ENS(sc->counters, (MS_CNT_N + 4) * 4);
-  CK(cudaMemsetAsync(sc->counters.p, 0, (MS_CNT_N + 4) * 4, st));
+  if (!sc->counters.p) {
+    ENS(sc->counters, (MS_CNT_N + 4) * 4);
+    CK(cudaMemsetAsync(sc->counters.p, 0, (MS_CNT_N + 4) * 4, st));
+  }
+  CK(cudaMemsetAsync(sc->counters.p, 0, MS_CNT_N * 4, st));         // the sticky overflow flag behind them stays
+  if (sc->clear_sticky) {
+    CK(cudaMemsetAsync((uint32_t *)sc->counters.p + MS_CNT_STICKY_OVERFLOW, 0, 4, st));
+    sc->clear_sticky = false;
+  }
   uint32_t *counters = (uint32_t *)sc->counters.p;
   ENS(sc->tile_count, (size_t)N * 4);
   ENS(sc->emit_off, (size_t)(N + 1) * 4);
@@ -281,26 +357,36 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
                 (int4 *)sc->rect.p, (float *)sc->z_entry.p, (float *)sc->oprime.p, counters, st));
   CK(ms_exclusive_scan_u32((uint32_t *)sc->tile_count.p, (uint32_t *)sc->emit_off.p, (size_t)N,
                            (uint32_t *)sc->scan_scratch.p, st));
-  CK(cudaMemcpyAsync(sc->pinned, (uint32_t *)sc->emit_off.p + N, 4, cudaMemcpyDeviceToHost, st));
-  CK(cudaMemcpyAsync(sc->pinned + 1 + MS_CNT_PAIRS_HI, counters + MS_CNT_PAIRS_HI, 4, cudaMemcpyDeviceToHost, st));
-  CK(cudaStreamSynchronize(st));
-  // the 32-bit scan total must agree with the 64-bit count of the projection kernel (a wrapped sum would size
-  // every buffer below too small)
-  if (sc->pinned[1 + MS_CNT_PAIRS_HI] != 0) return MS_ERR_UNSUPPORTED_SHAPE;
-  const size_t P = sc->pinned[0];
-  if (P >= (1ull << 31)) return MS_ERR_UNSUPPORTED_SHAPE;
+  size_t P = 0;                       // the pair count, or (no-sync) the capacity the launches are sized for
+  const uint32_t *P_dev = nullptr;    // no-sync: where the kernels read the count
+  if (nosync) {
+    P = P_cap;
+    CK(ms_frame_guard((uint32_t *)sc->emit_off.p + N, (uint32_t)P_cap, counters, st));
+    P_dev = counters + MS_CNT_P_EFF;
+  } else {
+    CK(cudaMemcpyAsync(sc->pinned, (uint32_t *)sc->emit_off.p + N, 4, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(sc->pinned + 1 + MS_CNT_PAIRS_HI, counters + MS_CNT_PAIRS_HI, 4, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    // the 32-bit scan total must agree with the 64-bit count of the projection kernel (a wrapped sum would size
+    // every buffer below too small)
+    if (sc->pinned[1 + MS_CNT_PAIRS_HI] != 0) return MS_ERR_UNSUPPORTED_SHAPE;
+    P = sc->pinned[0];
+    if (P >= (1ull << 31)) return MS_ERR_UNSUPPORTED_SHAPE;
+  }
   ENS(sc->keys_a, (P + 1) * 8);
   ENS(sc->keys_b, (P + 1) * 8);
-  ENS(sc->sort_scratch, ms_sort_scratch_elems(P) * 4);
+  // sized for the pairs the other buffers' 25 % of slack can hold: a no-sync view may use all of it
+  const size_t P_slack = nosync ? P : P + P / 4 + 4096;
+  ENS(sc->sort_scratch, ms_sort_scratch_elems(P_slack) * 4);
   ENS(sc->tile_start, (size_t)(n_tiles + 1) * 4);
   ENS(sc->pair_hits_i, (P + 1) * 4);
   ENS(sc->pair_hits_j, (P + 2) * 4);
   ENS(sc->pair_off, (P + 2) * 4);
   ENS(sc->slot_of, (P + 1) * 4);
-  if (ms_scan_scratch_elems(P) + 16 > sc->scan_scratch.cap / 4) ENS(sc->scan_scratch, (ms_scan_scratch_elems(P) + 16) * 4);
-  const int tile_order = (opts->flags & MS_FLAG_TILE_ORDER) != 0;
+  if (ms_scan_scratch_elems(P_slack) + 16 > sc->scan_scratch.cap / 4) ENS(sc->scan_scratch, (ms_scan_scratch_elems(P_slack) + 16) * 4);
   CK(ms_emit_keys(N, (uint32_t *)sc->emit_off.p, (int4 *)sc->rect.p, (float *)sc->z_entry.p, grid.tiles_x, prim_bits,
-                  (uint64_t *)sc->keys_a.p, tile_order, cam, tile, sc->A, (float *)sc->oprime.p, st));
+                  (uint64_t *)sc->keys_a.p, tile_order, cam, tile, sc->A, (float *)sc->oprime.p, st,
+                  nosync ? (uint32_t)P_cap : 0xffffffffu));
 
   // ---- (b) radix sort + tile ranges -------------------------------------------------------
   CK(rec(1));
@@ -308,8 +394,8 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   // stage (a) emits the keys primitive by primitive, i.e. already ordered by the id in their low prim_bits bits;
   // the sort is stable, so only the (tile | depth) bits above them need passes
   CK(ms_radix_sort_u64((uint64_t *)sc->keys_a.p, (uint64_t *)sc->keys_b.p, P, prim_bits, prim_bits + 32 + tile_bits,
-                       (uint32_t *)sc->sort_scratch.p, &sorted, st));
-  CK(ms_tile_ranges(sorted, P, n_tiles, prim_bits, (uint32_t *)sc->tile_start.p, st));
+                       (uint32_t *)sc->sort_scratch.p, &sorted, st, P_dev));
+  CK(ms_tile_ranges(sorted, P, n_tiles, prim_bits, (uint32_t *)sc->tile_start.p, st, P_dev));
 
   // ---- (c) intersection: count, scan, pair order, fill ---------------------------------------
   CK(rec(2));
@@ -325,33 +411,33 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   ia.pos_xy = (ushort2 *)sc->pos_xy.p;
   ia.pair_hits = (uint32_t *)sc->pair_hits_i.p; ia.ray_hits = (uint32_t *)sc->ray_hits.p;
   ia.slot_of = (uint32_t *)sc->slot_of.p; ia.pair_off = (uint32_t *)sc->pair_off.p; ia.ray_off = (uint32_t *)sc->ray_off.p;
-  ia.intervals = nullptr; ia.hits = nullptr;
+  ia.intervals = nullptr; ia.hits = nullptr; ia.guard = nullptr;
   CK(ms_isect_count(ia, st));
   CK(ms_exclusive_scan_u32((uint32_t *)sc->ray_hits.p, (uint32_t *)sc->ray_off.p, R, (uint32_t *)sc->scan_scratch.p, st));
-  CK(ms_tile_stats(grid, (uint32_t *)sc->ray_off.p, (uint32_t *)sc->tile_start.p, counters, st));
-  CK(cudaMemcpyAsync(sc->pinned + 1, counters, MS_CNT_N * 4, cudaMemcpyDeviceToHost, st));
-  CK(cudaStreamSynchronize(st));
-  if (sc->pinned[1 + MS_CNT_HITS_HI] != 0) return MS_ERR_UNSUPPORTED_SHAPE;   // 64-bit hit total beyond 32 bits
-  const size_t n_hits = sc->pinned[1 + MS_CNT_HITS];
-  const size_t max_tile_hits = sc->pinned[1 + MS_CNT_MAX_TILE_HITS];
-  const uint32_t max_list = sc->pinned[1 + MS_CNT_MAX_LIST];
-  if (n_hits >= (1ull << 31)) return MS_ERR_UNSUPPORTED_SHAPE;
+  CK(ms_tile_stats(grid, (uint32_t *)sc->ray_off.p, (uint32_t *)sc->tile_start.p, counters, st,
+                   nosync ? (uint32_t)hit_cap : 0u));
+  size_t n_hits = hit_cap, max_tile_hits = 0;     // no-sync: the capacity stands in for the count
+  uint32_t max_list = 0;
+  if (!nosync) {
+    CK(cudaMemcpyAsync(sc->pinned + 1, counters, MS_CNT_N * 4, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    if (sc->pinned[1 + MS_CNT_HITS_HI] != 0) return MS_ERR_UNSUPPORTED_SHAPE;   // 64-bit hit total beyond 32 bits
+    n_hits = sc->pinned[1 + MS_CNT_HITS];
+    max_tile_hits = sc->pinned[1 + MS_CNT_MAX_TILE_HITS];
+    max_list = sc->pinned[1 + MS_CNT_MAX_LIST];
+    if (n_hits >= (1ull << 31)) return MS_ERR_UNSUPPORTED_SHAPE;
+  }
   const size_t n_samples = n_hits * (size_t)K;
   if (n_samples >= (1ull << 40)) return MS_ERR_UNSUPPORTED_SHAPE;
-  const bool want_feat = sc->shape.n_feat > 0 && out_feat != nullptr;
-  const bool want_slots = sc->slot_cf > 0 && out_feat != nullptr;   // Eq.7 features (contact mode, K = 1)
 
   // bands: the staging bytes of one sample decide how many hits fit the budget
-  // the tensor path stages its 32 feature channels as fp16 (its operands are bf16); the fp32 path keeps fp32
-  const bool feat_half = want_feat && path == MS_PATH_BF16_TC && sc->shape.n_feat == 32;
-  const size_t feat_bytes = want_feat ? (size_t)sc->shape.n_feat * (feat_half ? 2 : 4) : 0;
-  const size_t sample_bytes = sizeof(float4) + feat_bytes + (want_slots ? 2 * sizeof(float4) : 0);
   const int64_t budget = opts->band_bytes == 0 ? MS_BAND_BYTES_DEFAULT : opts->band_bytes;
   size_t cap_hits = n_hits + 1;
   if (budget > 0) {
     cap_hits = (size_t)budget / (sample_bytes * (size_t)K);
     if (cap_hits < 1) cap_hits = 1;
   }
+  if (nosync) cap_hits = n_hits + 1;                 // the history says: one band
   int n_bands = n_hits <= cap_hits ? 1 : (int)(n_hits / cap_hits) + 1;
   while (n_bands > 1 && prim_bits + 3 + ceil_log2((uint64_t)n_bands) > 32) {   // (band, wave, prim) must fit 32 bits
     cap_hits *= 2;
@@ -359,7 +445,7 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   }
   // depth waves: asked for, or (auto) the previous view had rays stopping early
   int wave_c = 0;
-  if (opts->t_stop > 0.0f && !tile_order) {
+  if (opts->t_stop > 0.0f && !tile_order && !nosync) {
     if (opts->waves > 0) wave_c = opts->waves;
     else if (opts->waves == MS_WAVES_AUTO && sc->prev_terminated) wave_c = 4;   // measured on cfg4_opaque: C = 4 and 6 within noise, 4 skips more
   }
@@ -408,7 +494,7 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
 
   MsBandArgs ba;
   ba.grid = grid; ba.K = K; ba.prim_bits = prim_bits; ba.n_prims = N; ba.wave_c = wave_c; ba.n_bands = n_bands;
-  ba.cap_hits = (uint32_t)(cap_hits > 0xffffffffull ? 0xffffffffull : cap_hits); ba.P = P;
+  ba.cap_hits = (uint32_t)(cap_hits > 0xffffffffull ? 0xffffffffull : cap_hits); ba.P = P; ba.P_dev = P_dev;
   ba.keys = sorted; ba.tile_start = (uint32_t *)sc->tile_start.p; ba.ray_off = (uint32_t *)sc->ray_off.p;
   ba.emit_off = (uint32_t *)sc->emit_off.p; ba.rect = (int4 *)sc->rect.p; ba.pair_hits_i = (uint32_t *)sc->pair_hits_i.p;
   ba.key2_a = (uint64_t *)sc->key2_a.p; ba.key2_b = (uint64_t *)sc->key2_b.p;
@@ -418,6 +504,7 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   ba.grp_key = (uint32_t *)sc->grp_key.p; ba.grp_prim = (uint32_t *)sc->grp_prim.p; ba.grp_iv0 = (uint32_t *)sc->grp_iv0.p;
   ba.grp_blocks = (uint32_t *)sc->grp_blocks.p; ba.blk_off = (uint32_t *)sc->blk_off.p;
   ba.bw = (uint2 *)sc->bw.p; ba.bands = (MsBand *)sc->bands.p; ba.counters = counters;
+  if (nosync) CK(cudaMemsetAsync(sc->pair_hits_j.p, 0, (P + 2) * 4, st));   // slots beyond the device's pair count
   if (banded) CK(ms_order_banded(ba, st));
   else CK(ms_order_single(ba, st));
   // the band table comes back to the host: stage (e) is launched with one CTA per four rays of the band (the
@@ -433,6 +520,7 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   }
 
   ia.wave_c = wave_c;
+  ia.guard = nosync ? counters : nullptr;
   ia.intervals = (MsInterval *)sc->intervals.p;
   ia.hits = (MsHit *)sc->hits.p;
   CK(ms_isect_fill(ia, st));
@@ -496,19 +584,26 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   }
   CK(rec(3 + 2 * n_bands));
   if (timing) {
-    sc->ev_bands = n_bands;
+    sc->evs[sc->ev_cur].bands = n_bands;
+    sc->evs[sc->ev_cur].pending = true;
     sc->ev_valid = true;
-    sc->ev_pending = true;
   }
-  CK(cudaMemcpyAsync(sc->pinned + 1, counters, MS_CNT_N * 4, cudaMemcpyDeviceToHost, st));
+  CK(cudaMemcpyAsync(sc->pinned + 1, counters, (MS_CNT_N + 2) * 4, cudaMemcpyDeviceToHost, st));
   CK(cudaEventRecord(sc->frame_done, st));
   sc->frame_pending = true;
   sc->stats = ms_stats{};
   sc->stats.n_launches = (int64_t)(ms_launch_count - launches0);
-  sc->stats.n_pairs = (int64_t)P;
+  sc->stats.n_pairs = (int64_t)P;                    // no-sync: capacities, replaced by the counts in finish_frame
   sc->stats.n_intervals = (int64_t)n_hits;
   sc->stats.n_samples = (int64_t)n_samples;
   sc->stats.n_samples_evaluated = (int64_t)n_samples;
+  sc->frame_nosync = nosync;
+  sc->stats.no_sync = nosync ? 1 : 0;
+  if (!nosync) {
+    sc->hist.valid = n_bands == 1 && !banded;
+    sc->hist.H = H; sc->hist.W = W; sc->hist.tile = tile; sc->hist.K = K; sc->hist.path = path;
+    sc->hist.feat = want_feat ? 1 : 0; sc->hist.slots = want_slots ? 1 : 0; sc->hist.tile_order = tile_order;
+  }
   sc->stats.n_bands = n_bands;
   sc->stats.n_waves = n_waves;
   sc->stats.staging_bytes = (int64_t)(band_hits_cap * (size_t)K * sample_bytes);   // what this view needed
@@ -684,7 +779,8 @@ int ms_scene_destroy(ms_scene *sc) {
   free_buf(sc->host_rgb); free_buf(sc->host_alpha); free_buf(sc->host_feat);
   if (sc->pinned) cudaFreeHost(sc->pinned);
   if (sc->pinned_bands) cudaFreeHost(sc->pinned_bands);
-  for (cudaEvent_t e : sc->ev) cudaEventDestroy(e);
+  for (auto &E : sc->evs)
+    for (cudaEvent_t e : E.ev) cudaEventDestroy(e);
   if (sc->frame_done) cudaEventDestroy(sc->frame_done);
   (void)cudaGetLastError();
   delete sc;
@@ -731,6 +827,15 @@ int ms_render_host(ms_scene *sc, const ms_camera *cams, int32_t n_views, int32_t
     if (feat) CK(cudaMemcpyAsync(host_feat + v * px * nf, sc->host_feat.p, px * (size_t)nf * 4, cudaMemcpyDeviceToHost, st));
   }
   CK(cudaStreamSynchronize(st));
+  if (opts->flags & MS_FLAG_NO_SYNC) {   // a view that outgrew the scratch sized from its predecessor: once more, sizing
+    rc = finish_frame(sc);
+    if (rc != MS_OK) return rc;
+    if (sc->stats.overflow) {
+      ms_opts o2 = *opts;
+      o2.flags &= ~MS_FLAG_NO_SYNC;
+      return ms_render_host(sc, cams, n_views, H, W, &o2, host_rgb, host_alpha, host_feat);
+    }
+  }
   return MS_OK;
 }
 
@@ -784,25 +889,23 @@ int ms_last_stats(ms_scene *sc, ms_stats *out) {
   int rc = finish_frame(sc);
   if (rc != MS_OK) return rc;
   *out = sc->stats;
-  return MS_OK;
+  return sc->stats.overflow ? MS_ERR_CAPACITY : MS_OK;
 }
 
 int ms_last_stage_ms(ms_scene *sc, float *ms) {
   if (!sc || !ms || !sc->ev_valid) return MS_ERR_INVALID_ARG;
-  if (sc->ev_pending) {
-    CK(cudaEventSynchronize(sc->ev[3 + 2 * sc->ev_bands]));
-    harvest_stage_times(sc);
-  }
+  int rc = harvest_stage_times(sc, sc->ev_cur ^ 1);      // older view first: last_stage_ms ends as the newest
+  if (rc == MS_OK) rc = harvest_stage_times(sc, sc->ev_cur);
+  if (rc != MS_OK) return rc;
   for (int i = 0; i < MS_N_STAGES; ++i) ms[i] = sc->last_stage_ms[i];
   return MS_OK;
 }
 
 int ms_stage_accum(ms_scene *sc, double *ms_sum, int64_t *n_views, int32_t reset) {
   if (!sc) return MS_ERR_INVALID_ARG;
-  if (sc->ev_pending) {
-    CK(cudaEventSynchronize(sc->ev[3 + 2 * sc->ev_bands]));
-    harvest_stage_times(sc);
-  }
+  int rc = harvest_stage_times(sc, sc->ev_cur ^ 1);
+  if (rc == MS_OK) rc = harvest_stage_times(sc, sc->ev_cur);
+  if (rc != MS_OK) return rc;
   if (ms_sum)
     for (int i = 0; i < MS_N_STAGES; ++i) ms_sum[i] = sc->stage_sum[i];
   if (n_views) *n_views = sc->stage_views;

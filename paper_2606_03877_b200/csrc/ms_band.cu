@@ -24,7 +24,7 @@ constexpr int WB = 3;   // bits of the wave field (MS_MAX_WAVES <= 8)
 static_assert(MS_MAX_WAVES <= (1 << WB), "wave field");
 
 __global__ void tile_stats_kernel(MsGrid g, const uint32_t *__restrict__ ray_off, const uint32_t *__restrict__ tile_start,
-                                  uint32_t *__restrict__ counters) {
+                                  uint32_t *__restrict__ counters, uint32_t hit_cap) {
   const int pos = blockIdx.x * blockDim.x + threadIdx.x;
   const uint32_t T2 = (uint32_t)(g.tile * g.tile);
   if (pos < g.n_tiles) {
@@ -36,12 +36,18 @@ __global__ void tile_stats_kernel(MsGrid g, const uint32_t *__restrict__ ray_off
     const uint32_t len = tile_start[pos + 1] - tile_start[pos];
     if (len) atomicMax(&counters[MS_CNT_MAX_LIST], len);
   }
+  // no-sync renders: the hits must fit the scratch sized from the previous view (hit_cap = 0: no check)
+  if (pos == 0 && hit_cap && ray_off[(size_t)g.n_tiles * T2] > hit_cap) {
+    counters[MS_CNT_OVERFLOW] = 1u;
+    counters[MS_CNT_STICKY_OVERFLOW] = 1u;       // survives the per-view reset: any view of a batch
+  }
 }
 
 // ---- single band, single wave: segments = primitives, pairs in stage (a)'s emission order ----------------------
 __global__ void pair_single_kernel(MsBandArgs a) {
   const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= a.P) return;
+  const size_t P = a.P_dev ? (*a.P_dev < a.P ? (size_t)*a.P_dev : a.P) : a.P;
+  if (i >= P) return;
   const uint64_t key = a.keys[i];
   const int prim = (int)(key & ((1ull << a.prim_bits) - 1ull));
   const int tile = (int)(key >> (32 + a.prim_bits));
@@ -55,17 +61,19 @@ __global__ void pair_single_kernel(MsBandArgs a) {
 __global__ void seg_single_kernel(MsBandArgs a) {
   const int p = blockIdx.x * blockDim.x + threadIdx.x;
   if (p > a.n_prims) return;
-  const uint32_t s = a.pair_off[a.emit_off[p]];
+  const uint32_t cap = (uint32_t)a.P;       // no-sync renders: emit offsets beyond the capacity (an overflowed view)
+  const uint32_t s = a.pair_off[a.emit_off[p] < cap ? a.emit_off[p] : cap];
   a.grp_iv0[p] = s;
   if (p < a.n_prims) {
-    const uint32_t e = a.pair_off[a.emit_off[p + 1]];
+    const uint32_t e = a.pair_off[a.emit_off[p + 1] < cap ? a.emit_off[p + 1] : cap];
     a.grp_blocks[p] = (uint32_t)(((uint64_t)(e - s) * (uint64_t)a.K + MS_ROWS - 1) / MS_ROWS);
   }
 }
 
 __global__ void tables_single_kernel(MsBandArgs a) {
   const uint32_t T2 = (uint32_t)(a.grid.tile * a.grid.tile);
-  a.bw[0] = make_uint2(0u, (uint32_t)a.n_prims);
+  // a no-sync render whose pairs or hits overflowed the scratch evaluates nothing (the view is reported invalid)
+  a.bw[0] = make_uint2(0u, a.counters[MS_CNT_OVERFLOW] ? 0u : (uint32_t)a.n_prims);
   for (int w = 1; w < MS_MAX_WAVES; ++w) a.bw[w] = make_uint2((uint32_t)a.n_prims, (uint32_t)a.n_prims);
   MsBand b;
   b.q_lo = 0u; b.q_hi = (uint32_t)a.grid.n_tiles * T2; b.slot0 = 0u; b.pad = 0u;
@@ -359,8 +367,9 @@ inline unsigned grid_for(size_t n, int threads) { return (unsigned)((n + threads
   } while (0)
 
 cudaError_t ms_tile_stats(const MsGrid &g, const uint32_t *ray_off, const uint32_t *tile_start, uint32_t *counters,
-                          cudaStream_t s) {
-  tile_stats_kernel<<<grid_for((size_t)(g.n_tiles > 0 ? g.n_tiles : 1), 256), 256, 0, s>>>(g, ray_off, tile_start, counters);
+                          cudaStream_t s, uint32_t hit_cap) {
+  tile_stats_kernel<<<grid_for((size_t)(g.n_tiles > 0 ? g.n_tiles : 1), 256), 256, 0, s>>>(g, ray_off, tile_start, counters,
+                                                                                           hit_cap);
   MS_CHECK_LAUNCH();
   return cudaSuccess;
 }

@@ -158,7 +158,7 @@ __global__ void project_kernel(int n, const float *__restrict__ center, const fl
 __global__ void emit_keys_kernel(int n, const uint32_t *__restrict__ emit_off, const int4 *__restrict__ rect,
                                  const float *__restrict__ z_entry, int tiles_x, int prim_bits,
                                  uint64_t *__restrict__ keys, int tile_order, MsCam cam, int tile,
-                                 const float *__restrict__ A, const float *__restrict__ oprime) {
+                                 const float *__restrict__ A, const float *__restrict__ oprime, uint32_t cap) {
   int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   int lane = threadIdx.x & 31;
   if (i >= n) return;
@@ -177,13 +177,18 @@ __global__ void emit_keys_kernel(int n, const uint32_t *__restrict__ emit_off, c
       const float tc = ms_contact_t(A + 9 * (size_t)i, oprime + 3 * (size_t)i, d);
       low = ((uint64_t)__float_as_uint(tc) << prim_bits) | (uint64_t)(uint32_t)i;
     }
-    keys[beg + j] = (t << (32 + prim_bits)) | low;
+    if (beg + j < cap) keys[beg + j] = (t << (32 + prim_bits)) | low;     // cap: the buffer's capacity (no-sync renders)
   }
 }
 
 __global__ void tile_ranges_kernel(const uint64_t *__restrict__ keys, uint32_t n_pairs, int n_tiles, int shift,
-                                   uint32_t *__restrict__ tile_start) {
+                                   uint32_t *__restrict__ tile_start, const uint32_t *__restrict__ n_dev) {
   uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (n_dev) {                                   // the pair count lives on the device; n_pairs is its capacity
+    n_pairs = *n_dev < n_pairs ? *n_dev : n_pairs;
+    if (n_pairs == 0 && i == 0)
+      for (int u = 0; u <= n_tiles; ++u) tile_start[u] = 0u;
+  }
   if (i >= n_pairs) return;
   int t = (int)(keys[i] >> shift);
   int prev = i == 0 ? -1 : (int)(keys[i - 1] >> shift);
@@ -192,7 +197,23 @@ __global__ void tile_ranges_kernel(const uint64_t *__restrict__ keys, uint32_t n
     for (int u = t + 1; u <= n_tiles; ++u) tile_start[u] = n_pairs;
 }
 
+// ms_render without host synchronisation: the pair count against the capacity the scratch was sized for
+__global__ void frame_guard_kernel(const uint32_t *__restrict__ total, uint32_t cap, uint32_t *__restrict__ counters) {
+  const uint32_t P = *total;
+  counters[MS_CNT_P_EFF] = P < cap ? P : cap;
+  if (P > cap) {
+    counters[MS_CNT_OVERFLOW] = 1u;
+    counters[MS_CNT_STICKY_OVERFLOW] = 1u;       // survives the per-view reset: any view of a batch
+  }
+}
+
 }  // namespace
+
+cudaError_t ms_frame_guard(const uint32_t *total, uint32_t cap, uint32_t *counters, cudaStream_t s) {
+  frame_guard_kernel<<<1, 1, 0, s>>>(total, cap, counters);
+  MS_LAUNCHED();
+  return cudaGetLastError();
+}
 
 cudaError_t ms_prep_prims(int n, const float *center, const float *quat, const float *scale, float *A, float *M,
                           int *bad, cudaStream_t s) {
@@ -213,19 +234,19 @@ cudaError_t ms_project(int n, const float *center, const float *A, const float *
 
 cudaError_t ms_emit_keys(int n, const uint32_t *emit_off, const int4 *rect, const float *z_entry, int tiles_x,
                          int prim_bits, uint64_t *keys, int tile_order, MsCam cam, int tile, const float *A,
-                         const float *oprime, cudaStream_t s) {
+                         const float *oprime, cudaStream_t s, uint32_t cap) {
   long threads = (long)n * 32;
   emit_keys_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, s>>>(n, emit_off, rect, z_entry, tiles_x, prim_bits,
-                                                                    keys, tile_order, cam, tile, A, oprime);
+                                                                    keys, tile_order, cam, tile, A, oprime, cap);
   MS_LAUNCHED();
   return cudaGetLastError();
 }
 
 cudaError_t ms_tile_ranges(const uint64_t *keys, size_t n_pairs, int n_tiles, int prim_bits, uint32_t *tile_start,
-                           cudaStream_t s) {
+                           cudaStream_t s, const uint32_t *n_dev) {
   if (n_pairs == 0) return cudaMemsetAsync(tile_start, 0, (size_t)(n_tiles + 1) * sizeof(uint32_t), s);
   tile_ranges_kernel<<<(unsigned)((n_pairs + 255) / 256), 256, 0, s>>>(keys, (uint32_t)n_pairs, n_tiles,
-                                                                      32 + prim_bits, tile_start);
+                                                                      32 + prim_bits, tile_start, n_dev);
   MS_LAUNCHED();
   return cudaGetLastError();
 }

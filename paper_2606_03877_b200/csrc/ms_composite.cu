@@ -112,6 +112,7 @@ __global__ void __launch_bounds__(CW * 32, FEAT == 0 ? 12 : 8) composite_kernel(
   __shared__ WarpSmem s_all[CW];
   __shared__ float s_w[FEAT ? CW : 1][FEAT ? CAP : 1];   // weight of the window's r-th merged sample (features only)
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (a.counters && a.counters[MS_CNT_OVERFLOW]) return;   // a no-sync render that overflowed its scratch: view invalid
   const MsBand band = a.band;
   WarpSmem &sm = s_all[warp];
   const int K = a.K, nf = a.n_feat;
@@ -380,6 +381,7 @@ __global__ void __launch_bounds__(CW * 32, FEAT == 0 ? 12 : 8) composite_kernel(
 template <int R>
 __global__ void __launch_bounds__(CW * 32) slot_feature_kernel(MsCompositeArgs a) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (a.counters && a.counters[MS_CNT_OVERFLOW]) return;
   const MsBand band = a.band;
   // groups of R consecutive ray slots (R divides the tile edge: one tile row)
   for (uint32_t q0 = band.q_lo + (blockIdx.x * CW + warp) * R; q0 < band.q_hi; q0 = band.q_hi) {

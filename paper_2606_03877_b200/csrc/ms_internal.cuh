@@ -231,8 +231,9 @@ cudaError_t ms_exclusive_scan_u32(const uint32_t *in, uint32_t *out, size_t n, u
 
 // ms_sort.cu: stable LSD radix sort of 64-bit keys on bits [first_bit, n_bits). Result ends in *result (a or b).
 size_t ms_sort_scratch_elems(size_t n);
+// n_dev != NULL: the number of keys is read from the device (<= n, the capacity the launches are sized for)
 cudaError_t ms_radix_sort_u64(uint64_t *a, uint64_t *b, size_t n, int first_bit, int n_bits, uint32_t *scratch,
-                              uint64_t **result, cudaStream_t s);
+                              uint64_t **result, cudaStream_t s, const uint32_t *n_dev = nullptr);
 
 // ms_bin.cu
 cudaError_t ms_prep_prims(int n, const float *center, const float *quat, const float *scale, float *A, float *M,
@@ -243,9 +244,11 @@ cudaError_t ms_project(int n, const float *center, const float *A, const float *
 // tile_order != 0: the depth field of the key is t*_{i,c} of the tile-centre ray (needs cam, tile, A, oprime)
 cudaError_t ms_emit_keys(int n, const uint32_t *emit_off, const int4 *rect, const float *z_entry, int tiles_x,
                          int prim_bits, uint64_t *keys, int tile_order, MsCam cam, int tile, const float *A,
-                         const float *oprime, cudaStream_t s);
+                         const float *oprime, cudaStream_t s, uint32_t cap = 0xffffffffu);
 cudaError_t ms_tile_ranges(const uint64_t *keys, size_t n_pairs, int n_tiles, int prim_bits, uint32_t *tile_start,
-                           cudaStream_t s);
+                           cudaStream_t s, const uint32_t *n_dev = nullptr);
+// no-sync renders: counters[MS_CNT_P_EFF] = min(*total, cap); MS_CNT_OVERFLOW if the pairs do not fit
+cudaError_t ms_frame_guard(const uint32_t *total, uint32_t cap, uint32_t *counters, cudaStream_t s);
 
 // ms_isect.cu
 struct MsIsectArgs {
@@ -262,6 +265,7 @@ struct MsIsectArgs {
   const uint32_t *slot_of;     // [P]    (fill pass: in)     tile-list index -> pair slot of the prim-major order
   const uint32_t *pair_off;    // [P+1]  (fill pass: in)     by pair slot
   const uint32_t *ray_off;     // [R'+1] (fill pass: in)
+  const uint32_t *guard;       // counters (MS_CNT_OVERFLOW): a no-sync render that overflowed writes nothing; or NULL
   MsInterval *intervals;       // [n_hits] segment-major (fill pass: out)
   MsHit *hits;                 // [n_hits] ray-major      (fill pass: out)
 };
@@ -273,7 +277,8 @@ struct MsBandArgs {
   MsGrid grid;
   int K, prim_bits, n_prims, wave_c, n_bands;
   uint32_t cap_hits;           // band budget in hits
-  size_t P;
+  size_t P;                    // pairs, or their capacity when P_dev != NULL
+  const uint32_t *P_dev;       // no-sync renders: the pair count on the device
   const uint64_t *keys;        // sorted tile lists
   const uint32_t *tile_start;
   const uint32_t *ray_off;     // [R'+1]
@@ -300,10 +305,11 @@ struct MsBandArgs {
 // 32-bit scans is seen)
 enum MsCounter { MS_CNT_SEGS = 0, MS_CNT_BLOCKS, MS_CNT_HITS, MS_CNT_HITS_HI, MS_CNT_PAIRS, MS_CNT_PAIRS_HI,
                  MS_CNT_MAX_TILE_HITS, MS_CNT_MAX_LIST, MS_CNT_SKIPPED, MS_CNT_DEAD_RAYS, MS_CNT_VISIBLE,
-                 MS_CNT_STOPPED_RAYS, MS_CNT_N };
+                 MS_CNT_STOPPED_RAYS, MS_CNT_P_EFF, MS_CNT_OVERFLOW, MS_CNT_N,
+                 MS_CNT_STICKY_OVERFLOW = MS_CNT_N + 1 /* not cleared per view: read and cleared by the host */ };
 // after the ray_off scan: the hit total (64-bit), the largest tile's hit count and the longest tile list into counters
 cudaError_t ms_tile_stats(const MsGrid &g, const uint32_t *ray_off, const uint32_t *tile_start, uint32_t *counters,
-                          cudaStream_t s);
+                          cudaStream_t s, uint32_t hit_cap = 0);
 // one band, one wave: segments = primitives in emission order (the layout of small frames)
 cudaError_t ms_order_single(const MsBandArgs &a, cudaStream_t s);
 // bands x waves: pairs sorted by (band, wave, primitive), segments = runs of equal (band, wave, primitive)

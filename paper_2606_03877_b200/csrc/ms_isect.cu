@@ -22,6 +22,7 @@ __global__ void isect_kernel(MsIsectArgs a) {
   __shared__ int sPrim[IS_CHUNK];
   __shared__ uint32_t sBase[IS_CHUNK];      // FILL: pair_off[slot_of[i]]
   __shared__ uint32_t sCnt[IS_CHUNK][33];   // hits of the pair per warp (count pass: [c][32] = total)
+  if (FILL && a.guard && a.guard[MS_CNT_OVERFLOW]) return;
   const int T = a.grid.tile;
   const int tile_id = blockIdx.x;
   const int tile_x = tile_id % a.grid.tiles_x, tile_y = tile_id / a.grid.tiles_x;

@@ -12,9 +12,12 @@ constexpr int RS_WARPS = RS_THREADS / 32;
 constexpr int RS_ITEMS = 8;
 constexpr int RS_TILE = RS_THREADS * RS_ITEMS;
 
+// n_dev != NULL: the key count lives on the device (ms_render without host synchronisation); n is then its capacity
 __global__ void __launch_bounds__(RS_THREADS) radix_hist_kernel(const uint64_t *__restrict__ keys, size_t n, int shift,
-                                                                uint32_t *__restrict__ counts, uint32_t n_blocks) {
+                                                                uint32_t *__restrict__ counts, uint32_t n_blocks,
+                                                                const uint32_t *__restrict__ n_dev) {
   __shared__ uint32_t hist[256];
+  if (n_dev) n = *n_dev < n ? (size_t)*n_dev : n;
   hist[threadIdx.x] = 0;
   __syncthreads();
   size_t base = (size_t)blockIdx.x * RS_TILE;
@@ -32,8 +35,9 @@ __global__ void __launch_bounds__(RS_THREADS) radix_scatter_kernel(const uint64_
                                                                    uint64_t *__restrict__ out, size_t n, int shift,
                                                                    const uint32_t *__restrict__ offsets,
                                                                    const uint32_t *__restrict__ counts,
-                                                                   uint32_t n_blocks) {
+                                                                   uint32_t n_blocks, const uint32_t *__restrict__ n_dev) {
   __shared__ uint32_t wc[RS_WARPS][256];
+  if (n_dev) n = *n_dev < n ? (size_t)*n_dev : n;
   __shared__ uint32_t wsum[RS_WARPS];
   for (int i = threadIdx.x; i < RS_WARPS * 256; i += RS_THREADS) (&wc[0][0])[i] = 0;
   __syncthreads();
@@ -110,9 +114,9 @@ size_t ms_sort_scratch_elems(size_t n) {
 }
 
 cudaError_t ms_radix_sort_u64(uint64_t *a, uint64_t *b, size_t n, int first_bit, int n_bits, uint32_t *scratch,
-                              uint64_t **result, cudaStream_t s) {
+                              uint64_t **result, cudaStream_t s, const uint32_t *n_dev) {
   *result = a;
-  if (n <= 1 || n_bits <= 0) return cudaSuccess;
+  if ((n <= 1 && !n_dev) || n == 0 || n_bits <= 0) return cudaSuccess;
   size_t nb = (n + RS_TILE - 1) / RS_TILE;
   size_t m = 256 * nb;
   uint32_t *counts = scratch;
@@ -121,7 +125,7 @@ cudaError_t ms_radix_sort_u64(uint64_t *a, uint64_t *b, size_t n, int first_bit,
   uint64_t *src = a, *dst = b;
   // LSD and stable: bits below first_bit need no pass when the input is already ordered by them
   for (int shift = first_bit; shift < n_bits; shift += 8) {
-    radix_hist_kernel<<<(unsigned)nb, RS_THREADS, 0, s>>>(src, n, shift, counts, (uint32_t)nb);
+    radix_hist_kernel<<<(unsigned)nb, RS_THREADS, 0, s>>>(src, n, shift, counts, (uint32_t)nb, n_dev);
   MS_LAUNCHED();
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
@@ -131,7 +135,7 @@ cudaError_t ms_radix_sort_u64(uint64_t *a, uint64_t *b, size_t n, int first_bit,
       if (e != cudaSuccess) return e;
     }
     radix_scatter_kernel<<<(unsigned)nb, RS_THREADS, 0, s>>>(src, dst, n, shift, self_scan ? nullptr : offsets, counts,
-                                                             (uint32_t)nb);
+                                                             (uint32_t)nb, n_dev);
   MS_LAUNCHED();
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
