@@ -20,6 +20,9 @@ constexpr int BT = MS_ROWS;   // threads per CTA = samples per row block
 
 // odd leading dimension: a thread walking its own row and a warp walking one column are both conflict-free
 __host__ __device__ inline int ld_of(int n) { return n | 1; }
+// leading dimension = 4 (mod 8) for the 4-threads-per-sample kernel: rows are 16-byte aligned and the float4 accesses
+// of the eight threads of a quarter warp (each on its own row) fall on 32 different banks
+__host__ __device__ inline int ld4_of(int n) { int m = (n + 3) & ~3; return (m & 4) ? m : m + 4; }
 
 struct BwdLayout {
   int ld0, ldw, ldg;          // leading dimensions of X0 (encoded input), H_l (hidden), G (gradients)
@@ -27,16 +30,16 @@ struct BwdLayout {
   size_t off_g0, off_g1;      // the two gradient buffers
   size_t floats;
 };
-__host__ __device__ inline BwdLayout bwd_layout(const MsMlpShape &sh) {
+__host__ __device__ inline BwdLayout bwd_layout(const MsMlpShape &sh, bool vec4 = false, int rows = BT) {
   BwdLayout L;
-  L.ld0 = ld_of(sh.in_dim); L.ldw = ld_of(sh.width);
   const int gmax = sh.width > sh.in_dim ? sh.width : sh.in_dim;
-  L.ldg = ld_of(gmax);
+  if (vec4) { L.ld0 = ld4_of(sh.in_dim); L.ldw = ld4_of(sh.width); L.ldg = ld4_of(gmax); }
+  else { L.ld0 = ld_of(sh.in_dim); L.ldw = ld_of(sh.width); L.ldg = ld_of(gmax); }
   size_t o = 0;
-  L.off_h[0] = o; o += (size_t)BT * L.ld0;
-  for (int l = 1; l <= sh.n_hidden; ++l) { L.off_h[l] = o; o += (size_t)BT * L.ldw; }
-  L.off_g0 = o; o += (size_t)BT * L.ldg;
-  L.off_g1 = o; o += (size_t)BT * L.ldg;
+  L.off_h[0] = o; o += (size_t)rows * L.ld0;
+  for (int l = 1; l <= sh.n_hidden; ++l) { L.off_h[l] = o; o += (size_t)rows * L.ldw; }
+  L.off_g0 = o; o += (size_t)rows * L.ldg;
+  L.off_g1 = o; o += (size_t)rows * L.ldg;
   L.floats = o;
   return L;
 }
@@ -206,18 +209,37 @@ __global__ void __launch_bounds__(BT) mlp_bwd_kernel(MsMlpBwdArgs a) {
   }
 }
 
-// The same computation for hidden widths 8 / 16 / 32 / 64 (a multiple of 4: weight rows are 16-byte aligned): the
-// layer outputs and gradients of a thread's sample live in registers while a weight row streams through float4
-// loads (one row feeds WD FMAs), and the weight gradients are register tiles of 4 inputs x (WD / 32 or 1) outputs per
-// lane, so a shared-memory load feeds several FMAs.  Arithmetic order of the sums differs from the generic kernel
-// (and from the oracle) only in the order fp32 atomics arrive.
-template <int WD>
-__global__ void __launch_bounds__(BT) mlp_bwd_fast_kernel(MsMlpBwdArgs a) {
+// The same computation for hidden widths 16 / 32 / 64 / 128 with CG threads per sample (512 threads per CTA; one CTA
+// per SM is resident: the activations of BS samples fill shared memory, so the warps have to come from inside the
+// block.  BS = 128 = one row block, CG = 4 up to width 64; width 128 takes the row block in two halves of BS = 64
+// with CG = 8).  Thread (cg, s) owns the output columns [cg WD/CG, (cg+1) WD/CG) of sample s in the forward pass and
+// every CG-th 4-row chunk of the layer input in the backward pass: accumulators stay in registers, weight rows stream through
+// warp-uniform float4 loads, activations and gradients move as float4 (leading dimensions = 4 mod 8).  The weight
+// gradients X_l^T G_l are register tiles of 8 inputs x (WD / 32) outputs per lane, one (tile, sample range) item per
+// warp.  The sums differ from the generic kernel (and from the fp64 statement of the chain) only in the order of the
+// fp32 additions.
+constexpr int BT4 = 512;              // threads per CTA
+constexpr int NW4 = BT4 / 32;         // warps per CTA
+
+__device__ __forceinline__ float4 lds4(const float *p) { return *reinterpret_cast<const float4 *>(p); }
+__device__ __forceinline__ void sts4(float *p, float x, float y, float z, float w) {
+  *reinterpret_cast<float4 *>(p) = make_float4(x, y, z, w);
+}
+__device__ __forceinline__ float4 ldg4(const float *p) { return __ldg(reinterpret_cast<const float4 *>(p)); }
+
+template <int WD, int CG>
+__global__ void __launch_bounds__(BT4, 1) mlp_bwd_fast_kernel(MsMlpBwdArgs a) {
+  constexpr int BS = BT4 / CG;        // samples per pass
+  constexpr int PASSES = BT / BS;     // passes per 128-row block
+  constexpr int WQ = WD / CG;         // output columns per thread in the forward pass
+  constexpr int OC = WD > 32 ? WD / 32 : 1;
+  static_assert(WQ % 4 == 0, "float4 weight segments");
   extern __shared__ __align__(16) float sm[];
   __shared__ int s_seg;
   const MsMlpShape &sh = a.shape;
-  const BwdLayout L = bwd_layout(sh);
+  const BwdLayout L = bwd_layout(sh, true, BS);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int srow_in = tid & (BS - 1), cg = tid / BS;      // sample row inside the block, column group
   const uint2 r = *a.segs.range;
   const uint32_t *bo = a.segs.blk_off + r.x;
   const uint32_t base = bo[0], n_blocks = bo[r.y - r.x] - base;
@@ -231,14 +253,15 @@ __global__ void __launch_bounds__(BT) mlp_bwd_fast_kernel(MsMlpBwdArgs a) {
       off += nin * no + no; nin = no;
     }
   }
-  for (uint32_t blk = blockIdx.x; blk < n_blocks; blk += gridDim.x) {
+  for (uint32_t unit = blockIdx.x; unit < n_blocks * PASSES; unit += gridDim.x) {
+    const uint32_t blk = unit / PASSES, pass = unit % PASSES;
     __syncthreads();
     if (tid == 0) s_seg = find_seg(bo, (int)(r.y - r.x), base, blk);
     __syncthreads();
     const uint32_t g = r.x + (uint32_t)s_seg;
     const int prim = a.segs.prim ? (int)a.segs.prim[g] : (int)g;
     const uint32_t first = a.segs.iv0[g], count = a.segs.cnt ? a.segs.cnt[g] : a.segs.iv0[g + 1] - first;
-    const uint64_t srow = (uint64_t)(blk - (bo[s_seg] - base)) * BT + tid;
+    const uint64_t srow = (uint64_t)(blk - (bo[s_seg] - base)) * BT + pass * BS + srow_in;
     const uint32_t j = (uint32_t)(srow / (uint32_t)a.K);
     const int k = (int)(srow % (uint32_t)a.K);
     const bool live = j < count;
@@ -249,69 +272,99 @@ __global__ void __launch_bounds__(BT) mlp_bwd_fast_kernel(MsMlpBwdArgs a) {
     if (live) iv = a.intervals[first + j];
     const float d[3] = {iv.dx, iv.dy, iv.dz};
     const float t = ms_sample_t(iv.t_in, iv.delta, k);
-    float u[3];
-    ms_sample_u(Ap, mu, a.cam.o, d, t, u);
-    float *X0 = sm + L.off_h[0] + (size_t)tid * L.ld0;
-    {
-      int ni = 0;
-      X0[ni++] = u[0]; X0[ni++] = u[1]; X0[ni++] = u[2];
-      float scale = 1.0f;
-      for (int l = 0; l < sh.n_freq; ++l) {
+    float *X0 = sm + L.off_h[0] + (size_t)srow_in * L.ld0;
+    {                                 // the encoded input of the sample: frequency l by column group l mod 4
+      float u[3];
+      ms_sample_u(Ap, mu, a.cam.o, d, t, u);
+      if (cg == 0) {
+        X0[0] = u[0]; X0[1] = u[1]; X0[2] = u[2];
+        if (sh.use_viewdir) { float *v = X0 + 3 + 6 * sh.n_freq; v[0] = d[0]; v[1] = d[1]; v[2] = d[2]; }
+      }
+      for (int l = cg; l < sh.n_freq; l += CG) {
+        const float scale = (float)(1 << l);
         float sv[3], cv[3];
 #pragma unroll
         for (int c = 0; c < 3; ++c) sincospif(scale * u[c], &sv[c], &cv[c]);
-        X0[ni++] = sv[0]; X0[ni++] = sv[1]; X0[ni++] = sv[2];
-        X0[ni++] = cv[0]; X0[ni++] = cv[1]; X0[ni++] = cv[2];
-        scale *= 2.0f;
+        float *x = X0 + 3 + 6 * l;
+        x[0] = sv[0]; x[1] = sv[1]; x[2] = sv[2];
+        x[3] = cv[0]; x[4] = cv[1]; x[5] = cv[2];
       }
-      if (sh.use_viewdir) { X0[ni++] = d[0]; X0[ni++] = d[1]; X0[ni++] = d[2]; }
     }
-    // ---- forward ----
-    float acc[WD];
+    __syncthreads();
+    // ---- forward: this thread's WQ columns of every hidden layer ----
     for (int l = 0; l < nh; ++l) {
-      const float *src = sm + L.off_h[l] + (size_t)tid * (l == 0 ? L.ld0 : L.ldw);
-      float *dst = sm + L.off_h[l + 1] + (size_t)tid * L.ldw;
-      const float *w = wp + off_w[l];
+      const float *src = sm + L.off_h[l] + (size_t)srow_in * (l == 0 ? L.ld0 : L.ldw);
+      float *dst = sm + L.off_h[l + 1] + (size_t)srow_in * L.ldw + cg * WQ;
+      const float *w = wp + off_w[l] + cg * WQ;
       const int nin = n_in_l[l];
-      {
-        const float4 *b4 = reinterpret_cast<const float4 *>(w + nin * WD);
+      float acc[WQ];
 #pragma unroll
-        for (int q = 0; q < WD / 4; ++q) {
-          const float4 v = __ldg(b4 + q);
-          acc[4 * q] = v.x; acc[4 * q + 1] = v.y; acc[4 * q + 2] = v.z; acc[4 * q + 3] = v.w;
+      for (int q = 0; q < WQ / 4; ++q) {
+        const float4 v = ldg4(w + nin * WD + 4 * q);
+        acc[4 * q] = v.x; acc[4 * q + 1] = v.y; acc[4 * q + 2] = v.z; acc[4 * q + 3] = v.w;
+      }
+      int i = 0;
+      for (; i + 4 <= nin; i += 4) {
+        const float4 x4 = lds4(src + i);
+        const float xs[4] = {x4.x, x4.y, x4.z, x4.w};
+#pragma unroll
+        for (int ii = 0; ii < 4; ++ii) {
+          const float *wr = w + (i + ii) * WD;
+#pragma unroll
+          for (int q = 0; q < WQ / 4; ++q) {
+            const float4 v = ldg4(wr + 4 * q);
+            acc[4 * q] = fmaf(xs[ii], v.x, acc[4 * q]); acc[4 * q + 1] = fmaf(xs[ii], v.y, acc[4 * q + 1]);
+            acc[4 * q + 2] = fmaf(xs[ii], v.z, acc[4 * q + 2]); acc[4 * q + 3] = fmaf(xs[ii], v.w, acc[4 * q + 3]);
+          }
         }
       }
-      for (int i = 0; i < nin; ++i) {
+      for (; i < nin; ++i) {
         const float xi = src[i];
-        const float4 *w4 = reinterpret_cast<const float4 *>(w + i * WD);
+        const float *wr = w + i * WD;
 #pragma unroll
-        for (int q = 0; q < WD / 4; ++q) {
-          const float4 v = __ldg(w4 + q);
+        for (int q = 0; q < WQ / 4; ++q) {
+          const float4 v = ldg4(wr + 4 * q);
           acc[4 * q] = fmaf(xi, v.x, acc[4 * q]); acc[4 * q + 1] = fmaf(xi, v.y, acc[4 * q + 1]);
           acc[4 * q + 2] = fmaf(xi, v.z, acc[4 * q + 2]); acc[4 * q + 3] = fmaf(xi, v.w, acc[4 * q + 3]);
         }
       }
 #pragma unroll
-      for (int o = 0; o < WD; ++o) dst[o] = acc[o] > 0.0f ? acc[o] : 0.0f;
+      for (int q = 0; q < WQ / 4; ++q)
+        sts4(dst + 4 * q, fmaxf(acc[4 * q], 0.0f), fmaxf(acc[4 * q + 1], 0.0f), fmaxf(acc[4 * q + 2], 0.0f),
+             fmaxf(acc[4 * q + 3], 0.0f));
+      __syncthreads();
     }
-    float raw[4];
-    {
-      const float *src = sm + L.off_h[nh] + (size_t)tid * L.ldw;
-      const float *w = wp + off_w[nh];
-      const int no = sh.out_dim;
-#pragma unroll
-      for (int o = 0; o < 4; ++o) raw[o] = __ldg(w + WD * no + o);
-      for (int i = 0; i < WD; ++i) {
-        const float xi = src[i];
-#pragma unroll
-        for (int o = 0; o < 4; ++o) raw[o] = fmaf(xi, __ldg(w + i * no + o), raw[o]);
-      }
-    }
-    // ---- gradient of the head's four outputs ----
+    // ---- head: partial sums over this thread's WQ inputs, summed by column group 0 ----
     float *G = sm + L.off_g0, *Gn = sm + L.off_g1;
-    float g_delta = 0.0f;
+    const int no_h = sh.out_dim;
     {
-      float gr[4] = {0.f, 0.f, 0.f, 0.f};
+      const float *src = sm + L.off_h[nh] + (size_t)srow_in * L.ldw + cg * WQ;
+      const float *w = wp + off_w[nh] + (size_t)(cg * WQ) * no_h;
+      float pr[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+      for (int q = 0; q < WQ / 4; ++q) {
+        const float4 x4 = lds4(src + 4 * q);
+        const float xs[4] = {x4.x, x4.y, x4.z, x4.w};
+#pragma unroll
+        for (int ii = 0; ii < 4; ++ii)
+#pragma unroll
+          for (int o = 0; o < 4; ++o) pr[o] = fmaf(xs[ii], __ldg(w + (4 * q + ii) * no_h + o), pr[o]);
+      }
+      sts4(Gn + (size_t)srow_in * L.ldg + 4 * cg, pr[0], pr[1], pr[2], pr[3]);
+    }
+    __syncthreads();
+    float g_delta = 0.0f;
+    if (cg == 0) {                    // gradient of the head's four outputs (sigmoid colour, softplus density)
+      float raw[4], gr[4] = {0.f, 0.f, 0.f, 0.f};
+      const float *pp = Gn + (size_t)srow_in * L.ldg;
+      const float *bh = wp + off_w[nh] + WD * no_h;
+      float4 ps = lds4(pp);
+#pragma unroll
+      for (int c = 1; c < CG; ++c) {
+        const float4 pc = lds4(pp + 4 * c);
+        ps.x += pc.x; ps.y += pc.y; ps.z += pc.z; ps.w += pc.w;
+      }
+      raw[0] = __ldg(bh) + ps.x; raw[1] = __ldg(bh + 1) + ps.y; raw[2] = __ldg(bh + 2) + ps.z; raw[3] = __ldg(bh + 3) + ps.w;
       if (live) {
         const size_t idx = (size_t)(uint32_t)iv.slot * (size_t)a.K + (size_t)k;
         const float4 gs = a.gstage[idx];
@@ -322,81 +375,125 @@ __global__ void __launch_bounds__(BT) mlp_bwd_fast_kernel(MsMlpBwdArgs a) {
         gr[3] = -iv.delta * e * gs.w / (1.0f + expf(-raw[3]));
         g_delta = -sigma * e * gs.w;
       }
-      float *gp = G + (size_t)tid * L.ldg;
-#pragma unroll
-      for (int o = 0; o < 4; ++o) gp[o] = gr[o];
+      sts4(G + (size_t)srow_in * L.ldg, gr[0], gr[1], gr[2], gr[3]);
     }
     for (int l = nh; l >= 0; --l) {
       __syncthreads();
       const int nin = n_in_l[l];
-      const int no_ld = l == nh ? sh.out_dim : WD;
-      const int no = l == nh ? 4 : WD;
       const float *Xl = sm + L.off_h[l];
       const int ldx = l == 0 ? L.ld0 : L.ldw;
       float *gw = a.g_weights + (size_t)prim * sh.params + off_w[l];
-      // weight gradients: warp w takes the input rows 4 (w + 4 m) .. + 3, lane the outputs lane (+ 32)
-      constexpr int OC = WD > 32 ? 2 : 1;
-      for (int i0 = 4 * warp; i0 < nin + 1; i0 += 16) {      // row nin = the bias (input 1)
-        float t4[4][OC];
-#pragma unroll
-        for (int ii = 0; ii < 4; ++ii)
-#pragma unroll
-          for (int c = 0; c < OC; ++c) t4[ii][c] = 0.0f;
-        for (int s = 0; s < BT; ++s) {
-          float xv[4];
-#pragma unroll
-          for (int ii = 0; ii < 4; ++ii) {
-            const int i = i0 + ii;
-            xv[ii] = i < nin ? Xl[(size_t)s * ldx + i] : (i == nin ? 1.0f : 0.0f);
-          }
-#pragma unroll
-          for (int c = 0; c < OC; ++c) {
-            const int o = lane + 32 * c;
-            const float gv = o < no ? G[(size_t)s * L.ldg + o] : 0.0f;
-#pragma unroll
-            for (int ii = 0; ii < 4; ++ii) t4[ii][c] = fmaf(xv[ii], gv, t4[ii][c]);
-          }
-        }
-#pragma unroll
-        for (int ii = 0; ii < 4; ++ii)
-#pragma unroll
-          for (int c = 0; c < OC; ++c) {
-            const int i = i0 + ii, o = lane + 32 * c;
-            if (i <= nin && o < no && t4[ii][c] != 0.0f) atomicAdd(gw + i * no_ld + o, t4[ii][c]);
-          }
-      }
-      // gradient of this thread's layer input
-      const float *w = wp + off_w[l];
-      const float *xin = Xl + (size_t)tid * ldx;
-      float *gn = Gn + (size_t)tid * L.ldg;
       if (l == nh) {
-        const float *gp = G + (size_t)tid * L.ldg;
-        const float g0 = gp[0], g1 = gp[1], g2 = gp[2], g3 = gp[3];
-        for (int i = 0; i < nin; ++i) {
-          const float v = __ldg(w + i * no_ld) * g0 + __ldg(w + i * no_ld + 1) * g1 + __ldg(w + i * no_ld + 2) * g2 +
-                          __ldg(w + i * no_ld + 3) * g3;
-          gn[i] = xin[i] > 0.0f ? v : 0.0f;
+        // head weights (WD x 4): lane = input row, four outputs per lane; warps over (row group, sample range)
+        constexpr int RG = (WD + 31) / 32, SSH = NW4 / RG, PER = BS / SSH;
+        const int rg = warp % RG, part = warp / RG, row = rg * 32 + lane;
+        const bool on = row < WD;
+        float t4[4] = {0.f, 0.f, 0.f, 0.f}, tb[4] = {0.f, 0.f, 0.f, 0.f};
+        const float *xr = Xl + (size_t)(part * PER) * ldx + (on ? row : 0);
+        const float *gp = G + (size_t)(part * PER) * L.ldg;
+        for (int s = 0; s < PER; ++s, xr += ldx, gp += L.ldg) {
+          const float4 g4 = lds4(gp);
+          const float x = *xr;
+          t4[0] = fmaf(x, g4.x, t4[0]); t4[1] = fmaf(x, g4.y, t4[1]); t4[2] = fmaf(x, g4.z, t4[2]); t4[3] = fmaf(x, g4.w, t4[3]);
+          tb[0] += g4.x; tb[1] += g4.y; tb[2] += g4.z; tb[3] += g4.w;
+        }
+        if (on) {
+#pragma unroll
+          for (int o = 0; o < 4; ++o) if (t4[o] != 0.0f) atomicAdd(gw + row * no_h + o, t4[o]);
+        }
+        if (rg == 0 && lane == 0) {
+#pragma unroll
+          for (int o = 0; o < 4; ++o) if (tb[o] != 0.0f) atomicAdd(gw + WD * no_h + o, tb[o]);
         }
       } else {
-        const float *gp = G + (size_t)tid * L.ldg;
+        // hidden weights (nin x WD): items = (8-row tile, sample range), lane = output column (+ 32 c)
+        const int n_tiles = (nin + 7) >> 3;
+        int SS = 1;
+        while (2 * SS * n_tiles <= NW4 && SS < 8) SS *= 2;
+        const int per = BS / SS;
+        for (int item = warp; item < n_tiles * SS; item += NW4) {
+          const int tile = item / SS, part = item - tile * SS, i0 = tile * 8;
+          float t8[8][OC], tb[OC];
 #pragma unroll
-        for (int o = 0; o < WD; ++o) acc[o] = gp[o];
-        for (int i = 0; i < nin; ++i) {
-          const float4 *w4 = reinterpret_cast<const float4 *>(w + i * WD);
-          float v = 0.0f;
+          for (int c = 0; c < OC; ++c) {
+            tb[c] = 0.0f;
 #pragma unroll
-          for (int q = 0; q < WD / 4; ++q) {
-            const float4 ww = __ldg(w4 + q);
-            v = fmaf(ww.x, acc[4 * q], v); v = fmaf(ww.y, acc[4 * q + 1], v);
-            v = fmaf(ww.z, acc[4 * q + 2], v); v = fmaf(ww.w, acc[4 * q + 3], v);
+            for (int ii = 0; ii < 8; ++ii) t8[ii][c] = 0.0f;
           }
-          gn[i] = (l > 0 && !(xin[i] > 0.0f)) ? 0.0f : v;
+          const float *xr = Xl + (size_t)(part * per) * ldx + i0;
+          const float *gp = G + (size_t)(part * per) * L.ldg + (WD >= 32 ? lane : (lane & (WD - 1)));
+          for (int s = 0; s < per; ++s, xr += ldx, gp += L.ldg) {
+            const float4 xa = lds4(xr), xb = lds4(xr + 4);
+#pragma unroll
+            for (int c = 0; c < OC; ++c) {
+              const float gv = gp[32 * c];
+              t8[0][c] = fmaf(xa.x, gv, t8[0][c]); t8[1][c] = fmaf(xa.y, gv, t8[1][c]);
+              t8[2][c] = fmaf(xa.z, gv, t8[2][c]); t8[3][c] = fmaf(xa.w, gv, t8[3][c]);
+              t8[4][c] = fmaf(xb.x, gv, t8[4][c]); t8[5][c] = fmaf(xb.y, gv, t8[5][c]);
+              t8[6][c] = fmaf(xb.z, gv, t8[6][c]); t8[7][c] = fmaf(xb.w, gv, t8[7][c]);
+              tb[c] += gv;
+            }
+          }
+          if (WD >= 32 || lane < WD) {
+#pragma unroll
+            for (int c = 0; c < OC; ++c) {
+              const int o = lane + 32 * c;
+#pragma unroll
+              for (int ii = 0; ii < 8; ++ii)
+                if (i0 + ii < nin && t8[ii][c] != 0.0f) atomicAdd(gw + (i0 + ii) * WD + o, t8[ii][c]);
+              if (tile == 0 && tb[c] != 0.0f) atomicAdd(gw + nin * WD + o, tb[c]);
+            }
+          }
+        }
+      }
+      // gradient of the layer input: this thread's 4-row chunks (every fourth chunk)
+      const float *w = wp + off_w[l];
+      const float *xin = Xl + (size_t)srow_in * ldx;
+      const float *gpr = G + (size_t)srow_in * L.ldg;
+      float *gn = Gn + (size_t)srow_in * L.ldg;
+      if (l == nh) {
+        const float4 g4 = lds4(gpr);
+        for (int i0 = 4 * cg; i0 < nin; i0 += 4 * CG) {
+          const float4 x4 = lds4(xin + i0);
+          const float xs[4] = {x4.x, x4.y, x4.z, x4.w};
+          float v[4];
+#pragma unroll
+          for (int ii = 0; ii < 4; ++ii) {
+            const float *wr = w + (i0 + ii) * no_h;
+            const float vv = __ldg(wr) * g4.x + __ldg(wr + 1) * g4.y + __ldg(wr + 2) * g4.z + __ldg(wr + 3) * g4.w;
+            v[ii] = xs[ii] > 0.0f ? vv : 0.0f;
+          }
+          sts4(gn + i0, v[0], v[1], v[2], v[3]);
+        }
+      } else {
+        for (int i0 = 4 * cg; i0 < nin; i0 += 4 * CG) {
+          const float *wr[4];
+#pragma unroll
+          for (int ii = 0; ii < 4; ++ii) wr[ii] = w + (size_t)min(i0 + ii, nin - 1) * WD;   // rows past nin: discarded
+          float v[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll 4
+          for (int o = 0; o < WD; o += 4) {
+            const float4 g4 = lds4(gpr + o);
+#pragma unroll
+            for (int ii = 0; ii < 4; ++ii) {
+              const float4 ww = ldg4(wr[ii] + o);
+              v[ii] = fmaf(ww.x, g4.x, v[ii]); v[ii] = fmaf(ww.y, g4.y, v[ii]);
+              v[ii] = fmaf(ww.z, g4.z, v[ii]); v[ii] = fmaf(ww.w, g4.w, v[ii]);
+            }
+          }
+          if (l > 0) {
+            const float4 x4 = lds4(xin + i0);
+            v[0] = x4.x > 0.0f ? v[0] : 0.0f; v[1] = x4.y > 0.0f ? v[1] : 0.0f;
+            v[2] = x4.z > 0.0f ? v[2] : 0.0f; v[3] = x4.w > 0.0f ? v[3] : 0.0f;
+          }
+          sts4(gn + i0, v[0], v[1], v[2], v[3]);
         }
       }
       float *tmp = G; G = Gn; Gn = tmp;
     }
-    if (live) {
-      const float *gx = G + (size_t)tid * L.ldg;
+    __syncthreads();
+    if (live && cg == 0) {
+      const float *gx = G + (size_t)srow_in * L.ldg;
       float gu[3] = {gx[0], gx[1], gx[2]};
       float scale = 3.14159265358979323846f;
       for (int l = 0; l < sh.n_freq; ++l) {
@@ -496,21 +593,40 @@ __global__ void prim_bwd_kernel(MsMlpBwdArgs a) {
 
 }  // namespace
 
-size_t ms_mlp_bwd_smem(const MsMlpShape &sh) {
-  if (sh.mode != MS_MODE_LOCAL || sh.n_hidden > 4) return 0;
+// which kernel serves the shape: 2 = several threads per sample (widths 16 / 32 / 64 / 128, float4 weight rows),
+// 1 = generic
+static int bwd_kind(const MsMlpShape &sh, size_t *smem) {
+  *smem = 0;
+  if (sh.mode != MS_MODE_LOCAL || sh.n_hidden > 4 || sh.n_hidden < 1) return 0;
+  const size_t cap = 220 * 1024;
+  const bool fast_w = sh.width == 16 || sh.width == 32 || sh.width == 64 || sh.width == 128;
+  if (fast_w && sh.params % 4 == 0) {
+    const size_t b = bwd_layout(sh, true, sh.width == 128 ? 64 : BT).floats * sizeof(float);
+    if (b <= cap) { *smem = b; return 2; }
+  }
   const size_t b = bwd_layout(sh).floats * sizeof(float);
-  return b <= 220 * 1024 ? b : 0;
+  if (b > cap) return 0;
+  *smem = b;
+  return 1;
+}
+
+size_t ms_mlp_bwd_smem(const MsMlpShape &sh) {
+  size_t b = 0;
+  bwd_kind(sh, &b);
+  return b;
 }
 
 cudaError_t ms_mlp_bwd(const MsMlpBwdArgs &a, cudaStream_t s) {
-  const size_t smem = ms_mlp_bwd_smem(a.shape);
-  if (smem == 0) return cudaErrorNotSupported;
+  size_t smem = 0;
+  const int kind = bwd_kind(a.shape, &smem);
+  if (kind == 0) return cudaErrorNotSupported;
   void (*fn)(MsMlpBwdArgs) = mlp_bwd_kernel;
-  const bool aligned = a.shape.params % 4 == 0;       // float4 loads of the weight rows
-  if (aligned && a.shape.width == 8) fn = mlp_bwd_fast_kernel<8>;
-  else if (aligned && a.shape.width == 16) fn = mlp_bwd_fast_kernel<16>;
-  else if (aligned && a.shape.width == 32) fn = mlp_bwd_fast_kernel<32>;
-  else if (aligned && a.shape.width == 64) fn = mlp_bwd_fast_kernel<64>;
+  int threads = BT;
+  if (kind == 2) {
+    threads = BT4;
+    fn = a.shape.width == 16 ? mlp_bwd_fast_kernel<16, 4> : a.shape.width == 32 ? mlp_bwd_fast_kernel<32, 4>
+       : a.shape.width == 64 ? mlp_bwd_fast_kernel<64, 4> : mlp_bwd_fast_kernel<128, 8>;
+  }
   cudaError_t e = cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   static int n_sm = 0;
@@ -520,11 +636,11 @@ cudaError_t ms_mlp_bwd(const MsMlpBwdArgs &a, cudaStream_t s) {
     cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
   }
   int occ = 1;
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)fn, BT, smem) != cudaSuccess || occ < 1) {
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)fn, threads, smem) != cudaSuccess || occ < 1) {
     (void)cudaGetLastError();
     occ = 1;
   }
-  fn<<<(unsigned)(n_sm * occ * 4), BT, smem, s>>>(a);
+  fn<<<(unsigned)(n_sm * occ * (kind == 2 ? 1 : 4)), threads, smem, s>>>(a);
   MS_LAUNCHED();
   e = cudaGetLastError();
   if (e != cudaSuccess) return e;

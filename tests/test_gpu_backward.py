@@ -4,7 +4,11 @@ its family (weights, centres, semi-axes, quaternions).  The bar is set by the FO
 arithmetic: the GPU differentiates the render it runs -- canonical fp32 geometry -- while the oracle's
 backward is fp64 throughout; a sample position that differs by 1 ulp of the eye distance moves the top encoding band's
 phase by 2^(L-1) pi times that (1e-4 at L = 4), and grazing chords carry 1/sqrt(disc).  Measured: <= 5e-3 at L = 4,
-<= 6e-4 at L = 2 (held to 2e-3 there, which a dropped or mis-signed term of the chain rule would break)."""
+<= 6e-4 at L = 2 (held to 2e-3 there, which a dropped or mis-signed term of the chain rule would break); at L = 6 the
+top band's phase error is four times that of L = 4 (measured 1.4e-2; held to 3e-2).  Wide or deep random networks
+amplify the same position error (64 and 128 wide at L = 2: up to 8e-3 on the geometry families, set by one or two
+grazing chords of the scene), so the tight bar is held by every kernel variant on networks up to 32 wide and the 1e-2
+bar on the wide ones."""
 import numpy as np
 import pytest
 import torch
@@ -16,6 +20,7 @@ pytestmark = pytest.mark.gpu
 
 TOL_REL = 1e-2
 TOL_REL_L2 = 2e-3
+TOL_REL_L6 = 3e-2
 
 
 def _api():
@@ -68,15 +73,19 @@ def test_backward_cfg1_shape():
     compare(sc, synth.make_cameras(cfg)[0], 48, 48, cfg.K)
 
 
-@pytest.mark.parametrize("seed,viewdir,width,nh", [(3, 0, 8, 2), (5, 1, 16, 3), (7, 1, 64, 3)])
-def test_backward_overlapping_primitives(seed, viewdir, width, nh):
+@pytest.mark.parametrize("seed,viewdir,width,nh,L", [(3, 0, 8, 2, 2), (5, 1, 16, 3, 2), (7, 1, 64, 3, 4), (11, 1, 32, 2, 2),
+                                                     (13, 0, 24, 2, 2), (9, 0, 128, 3, 2), (9, 0, 128, 3, 6),
+                                                     (15, 1, 64, 4, 2), (17, 0, 16, 1, 2), (19, 0, 64, 2, 2),
+                                                     (21, 0, 32, 3, 2), (23, 0, 64, 1, 2)])
+def test_backward_overlapping_primitives(seed, viewdir, width, nh, L):
     """heavily overlapping supports (interleaved samples of several primitives on every ray), ragged image,
-    with and without the view-direction input, up to CFG3's 30-64-64-64-4"""
-    mlp = synth.MLPSpec(4 if width == 64 else 2, viewdir, nh, width, 0, False)
+    with and without the view-direction input: CFG3's 30-64-64-64-4, CFG4's 39-128-128-128-4 (two 64-sample passes
+    per row block), widths served by the generic one-thread-per-sample kernel (8, 24; 64 with four hidden layers)"""
+    mlp = synth.MLPSpec(L, viewdir, nh, width, 0, False)
     cfg = synth.SceneConfig(f"b{seed}", seed, 9, 0.6, 0.35, 0.8, mlp, 37, 23, 50.0, 3.0, 5)
     sc = with_biases(synth.make_scene(cfg), mlp, seed)
     compare(sc, synth.make_cameras(cfg)[0], cfg.height, cfg.width, cfg.K, seed=seed,
-            tol=TOL_REL if width == 64 else TOL_REL_L2)
+            tol=TOL_REL_L6 if L == 6 else (TOL_REL_L2 if L == 2 and width <= 32 else TOL_REL))
 
 
 def test_backward_stops_at_the_early_termination():
