@@ -335,15 +335,194 @@ __global__ void __launch_bounds__(MS_ROWS / SPT, 6) mlp_f32_w32_kernel(MsMlpArgs
   }
 }
 
+// Wide MLPs (16 / 64 / 128 hidden units; north-star mode): the same arithmetic in the same order as mlp_f32_kernel
+// (acc = b; acc = fma(x_i, W[i][o], acc) for i ascending -- bitwise the same staging), laid out for throughput.  CG
+// threads share a pair of samples: thread (cg, sp) owns the output columns [cg WD/CG, (cg+1) WD/CG) of the samples sp
+// and sp + 64 of the row block, activations live in shared memory (rows 16-byte aligned, leading dimension = 4 mod 8:
+// the float4 reads of a quarter warp fall on 32 different banks), weight rows stream through warp-uniform float4 loads
+// and each serves two samples (8 FMAs per loaded float4).
+__host__ __device__ inline int ld4_of(int n) { int m = (n + 3) & ~3; return (m & 4) ? m : m + 4; }
+__device__ __forceinline__ float4 lds4(const float *p) { return *reinterpret_cast<const float4 *>(p); }
+__device__ __forceinline__ float4 ldg4(const float *p) { return __ldg(reinterpret_cast<const float4 *>(p)); }
+
+template <int WD, int CG>
+__global__ void __launch_bounds__(MS_ROWS * CG / 2) mlp_f32_wide_kernel(MsMlpArgs a) {
+  constexpr int HS = MS_ROWS / 2;     // thread (cg, sp): rows sp and sp + HS
+  constexpr int WQ = WD / CG;
+  static_assert(WQ % 4 == 0, "float4 weight segments");
+  extern __shared__ __align__(16) float sm[];
+  __shared__ int s_seg;
+  const MsMlpShape &sh = a.shape;
+  const LaunchView lv(a.segs);
+  const int ld0 = ld4_of(sh.in_dim), ldw = ld4_of(WD);
+  float *X0 = sm, *HA = X0 + (size_t)MS_ROWS * ld0, *HB = HA + (size_t)MS_ROWS * ldw;
+  const int tid = threadIdx.x, sp = tid & (HS - 1), cg = tid / HS;
+  const uint32_t blk_lo = (uint32_t)(((uint64_t)lv.n_blocks * blockIdx.x) / gridDim.x);
+  const uint32_t blk_hi = (uint32_t)(((uint64_t)lv.n_blocks * (blockIdx.x + 1)) / gridDim.x);
+  for (uint32_t blk = blk_lo; blk < blk_hi; ++blk) {
+    __syncthreads();
+    if (tid == 0) {
+      int sgm = blk == blk_lo ? find_seg(lv.bo, (int)(lv.r.y - lv.r.x), lv.base, blk) : s_seg;
+      while (lv.bo[sgm + 1] - lv.base <= blk) ++sgm;
+      s_seg = sgm;
+    }
+    __syncthreads();
+    const uint32_t g = lv.r.x + (uint32_t)s_seg;
+    const int prim = a.segs.prim ? (int)a.segs.prim[g] : (int)g;
+    const float *wp = a.weights_f32 + (size_t)prim * sh.params;
+    const uint32_t first = a.segs.iv0[g], count = a.segs.cnt ? a.segs.cnt[g] : a.segs.iv0[g + 1] - first;
+    const uint64_t s0 = (uint64_t)(blk - (lv.bo[s_seg] - lv.base)) * MS_ROWS;
+    bool live[2];
+    int kk[2];
+    float delta[2];
+    uint32_t slot[2];
+#pragma unroll
+    for (int p = 0; p < 2; ++p) {
+      const int row = sp + p * HS;
+      const uint64_t s = s0 + row;
+      const uint32_t j = (uint32_t)(s / (uint32_t)a.K);
+      kk[p] = (int)(s % (uint32_t)a.K);
+      live[p] = j < count;
+      MsInterval iv;
+      iv.t_in = 0.f; iv.delta = 0.f; iv.slot = 0; iv.dx = 0.f; iv.dy = 0.f; iv.dz = 1.f; iv.ray = 0; iv.prim = prim;
+      if (live[p]) iv = a.intervals[first + j];
+      delta[p] = iv.delta; slot[p] = (uint32_t)iv.slot;
+      const float d[3] = {iv.dx, iv.dy, iv.dz};
+      const float t = ms_sample_tm(iv.t_in, iv.delta, kk[p], false);
+      float u[3];
+      ms_sample_u(a.A + 9 * (size_t)prim, a.center + 3 * (size_t)prim, a.cam.o, d, t, u);
+      float *x = X0 + (size_t)row * ld0;                  // Eq.5: frequency l by column group l mod CG
+      if (cg == 0) {
+        x[0] = u[0]; x[1] = u[1]; x[2] = u[2];
+        if (sh.use_viewdir) { float *v = x + 3 + 6 * sh.n_freq; v[0] = d[0]; v[1] = d[1]; v[2] = d[2]; }
+        if (a.staging_gate && live[p])
+          a.staging_gate[(size_t)(slot[p] - lv.band.slot0) * (size_t)a.K + (size_t)kk[p]] = ms_slot_gates(u);
+      }
+      for (int l = cg; l < sh.n_freq; l += CG) {
+        const float scale = (float)(1 << l);
+        float sv[3], cv[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) sincospif(scale * u[c], &sv[c], &cv[c]);  // 2^l u is exact
+        float *y = x + 3 + 6 * l;
+        y[0] = sv[0]; y[1] = sv[1]; y[2] = sv[2];
+        y[3] = cv[0]; y[4] = cv[1]; y[5] = cv[2];
+      }
+    }
+    __syncthreads();
+    const float *src = X0;
+    float *dst = HA;
+    int ldx = ld0, n_in = sh.in_dim;
+    const float *w = wp;
+    for (int l = 0; l < sh.n_hidden; ++l) {
+      const float *x0 = src + (size_t)sp * ldx, *x1 = x0 + (size_t)HS * ldx;
+      const float *wc = w + cg * WQ;
+      float acc[2][WQ];
+#pragma unroll
+      for (int q = 0; q < WQ / 4; ++q) {
+        const float4 v = ldg4(wc + n_in * WD + 4 * q);
+        acc[0][4 * q] = acc[1][4 * q] = v.x; acc[0][4 * q + 1] = acc[1][4 * q + 1] = v.y;
+        acc[0][4 * q + 2] = acc[1][4 * q + 2] = v.z; acc[0][4 * q + 3] = acc[1][4 * q + 3] = v.w;
+      }
+      int i = 0;
+      for (; i + 4 <= n_in; i += 4) {
+        const float4 a4 = lds4(x0 + i), b4 = lds4(x1 + i);
+        const float xa[4] = {a4.x, a4.y, a4.z, a4.w}, xb[4] = {b4.x, b4.y, b4.z, b4.w};
+#pragma unroll
+        for (int ii = 0; ii < 4; ++ii) {
+          const float *wr = wc + (i + ii) * WD;
+#pragma unroll
+          for (int q = 0; q < WQ / 4; ++q) {
+            const float4 v = ldg4(wr + 4 * q);
+            acc[0][4 * q] = fmaf(xa[ii], v.x, acc[0][4 * q]); acc[0][4 * q + 1] = fmaf(xa[ii], v.y, acc[0][4 * q + 1]);
+            acc[0][4 * q + 2] = fmaf(xa[ii], v.z, acc[0][4 * q + 2]); acc[0][4 * q + 3] = fmaf(xa[ii], v.w, acc[0][4 * q + 3]);
+            acc[1][4 * q] = fmaf(xb[ii], v.x, acc[1][4 * q]); acc[1][4 * q + 1] = fmaf(xb[ii], v.y, acc[1][4 * q + 1]);
+            acc[1][4 * q + 2] = fmaf(xb[ii], v.z, acc[1][4 * q + 2]); acc[1][4 * q + 3] = fmaf(xb[ii], v.w, acc[1][4 * q + 3]);
+          }
+        }
+      }
+      for (; i < n_in; ++i) {
+        const float xa = x0[i], xb = x1[i];
+        const float *wr = wc + i * WD;
+#pragma unroll
+        for (int q = 0; q < WQ / 4; ++q) {
+          const float4 v = ldg4(wr + 4 * q);
+          acc[0][4 * q] = fmaf(xa, v.x, acc[0][4 * q]); acc[0][4 * q + 1] = fmaf(xa, v.y, acc[0][4 * q + 1]);
+          acc[0][4 * q + 2] = fmaf(xa, v.z, acc[0][4 * q + 2]); acc[0][4 * q + 3] = fmaf(xa, v.w, acc[0][4 * q + 3]);
+          acc[1][4 * q] = fmaf(xb, v.x, acc[1][4 * q]); acc[1][4 * q + 1] = fmaf(xb, v.y, acc[1][4 * q + 1]);
+          acc[1][4 * q + 2] = fmaf(xb, v.z, acc[1][4 * q + 2]); acc[1][4 * q + 3] = fmaf(xb, v.w, acc[1][4 * q + 3]);
+        }
+      }
+#pragma unroll
+      for (int p = 0; p < 2; ++p) {
+        float *y = dst + (size_t)(sp + p * HS) * ldw + cg * WQ;
+#pragma unroll
+        for (int q = 0; q < WQ / 4; ++q)
+          *reinterpret_cast<float4 *>(y + 4 * q) = make_float4(fmaxf(acc[p][4 * q], 0.0f), fmaxf(acc[p][4 * q + 1], 0.0f),
+                                                               fmaxf(acc[p][4 * q + 2], 0.0f), fmaxf(acc[p][4 * q + 3], 0.0f));
+      }
+      __syncthreads();
+      w += n_in * WD + WD;
+      n_in = WD; ldx = ldw;
+      src = dst; dst = dst == HA ? HB : HA;
+    }
+    // head: output o by column group o mod CG, raw values into the free buffer
+    {
+      const int n_out = sh.out_dim;
+      const float *x0 = src + (size_t)sp * ldw, *x1 = x0 + (size_t)HS * ldw;
+      const float *bh = w + WD * n_out;
+      for (int o = cg; o < n_out; o += CG) {
+        float r0 = __ldg(bh + o), r1 = r0;
+#pragma unroll 4
+        for (int i = 0; i < WD; i += 4) {
+          const float4 a4 = lds4(x0 + i), b4 = lds4(x1 + i);
+          const float w0 = __ldg(w + i * n_out + o), w1 = __ldg(w + (i + 1) * n_out + o);
+          const float w2 = __ldg(w + (i + 2) * n_out + o), w3 = __ldg(w + (i + 3) * n_out + o);
+          r0 = fmaf(a4.x, w0, r0); r0 = fmaf(a4.y, w1, r0); r0 = fmaf(a4.z, w2, r0); r0 = fmaf(a4.w, w3, r0);
+          r1 = fmaf(b4.x, w0, r1); r1 = fmaf(b4.y, w1, r1); r1 = fmaf(b4.z, w2, r1); r1 = fmaf(b4.w, w3, r1);
+        }
+        dst[(size_t)sp * ldw + o] = r0;
+        dst[(size_t)(sp + HS) * ldw + o] = r1;
+      }
+    }
+    __syncthreads();
+    if (cg == 0) {
+#pragma unroll
+      for (int p = 0; p < 2; ++p) {
+        if (!live[p]) continue;
+        const float *raw = dst + (size_t)(sp + p * HS) * ldw;
+        float4 r;
+        r.x = 1.0f / (1.0f + expf(-raw[0]));
+        r.y = 1.0f / (1.0f + expf(-raw[1]));
+        r.z = 1.0f / (1.0f + expf(-raw[2]));
+        const float sigma = fmaxf(raw[3], 0.0f) + log1pf(expf(-fabsf(raw[3])));
+        r.w = expf(-sigma * delta[p]);  // e = 1 - alpha
+        const size_t out = (size_t)(slot[p] - lv.band.slot0) * (size_t)a.K + (size_t)kk[p];
+        a.staging[out] = r;
+        if (a.staging_feat)
+          for (int c = 0; c < sh.n_feat; ++c) reinterpret_cast<float *>(a.staging_feat)[out * sh.n_feat + c] = raw[4 + c];
+      }
+    }
+  }
+}
+
 }  // namespace
 
 cudaError_t ms_mlp_f32(const MsMlpArgs &a, cudaStream_t s) {
   size_t smem = (size_t)a.shape.params * sizeof(float);
   void (*fn)(MsMlpArgs) = mlp_f32_kernel;
   int threads = MS_ROWS;
-  if (a.shape.width == 32 && a.shape.params % 4 == 0 && a.shape.n_hidden >= 1 && a.shape.n_hidden <= 3) {
+  const int wd = a.shape.width;
+  const size_t smem_wide = (size_t)MS_ROWS * (ld4_of(a.shape.in_dim) + 2 * ld4_of(wd)) * sizeof(float);
+  if (wd == 32 && a.shape.params % 4 == 0 && a.shape.n_hidden >= 1 && a.shape.n_hidden <= 3) {
     fn = a.shape.n_hidden == 1 ? mlp_f32_w32_kernel<1, 2> : (a.shape.n_hidden == 2 ? mlp_f32_w32_kernel<2, 2> : mlp_f32_w32_kernel<3, 2>);
     threads = MS_ROWS / 2;
+  } else if ((wd == 16 || wd == 32 || wd == 64 || wd == 128) && a.shape.mode == MS_MODE_LOCAL && a.shape.params % 4 == 0 &&
+             a.shape.out_dim <= wd && a.shape.n_hidden >= 1 && smem_wide <= 200 * 1024) {
+    const int cg = wd == 128 ? 8 : 4;
+    fn = wd == 16 ? mlp_f32_wide_kernel<16, 4> : wd == 32 ? mlp_f32_wide_kernel<32, 4>
+       : wd == 64 ? mlp_f32_wide_kernel<64, 4> : mlp_f32_wide_kernel<128, 8>;
+    threads = MS_ROWS * cg / 2;
+    smem = smem_wide;
   }
   cudaError_t e = cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
