@@ -207,6 +207,8 @@ def measure(api, cfg, args, peaks, stream, barrier, steps, warmup, sampler=None,
     create_s = time.perf_counter() - t_create
     gs.band_bytes, gs.waves = args.band_bytes, args.waves
     extra_flags = api.FLAG_TILE_ORDER if (args.tile_order and cfg.mlp.mode == 1) else 0
+    if args.overlap:
+        extra_flags |= api.FLAG_OVERLAP
     if not args.sync:
         extra_flags |= api.FLAG_NO_SYNC      # views sized from their predecessor: no host synchronisation inside ms_render
     tile_kw = {"tile": args.tile} if args.tile else {"tile": cfg.tile}
@@ -465,6 +467,8 @@ def main():
     ap.add_argument("--shard-views", action="store_true",
                     help="N > 1: shard the workload's views over the ranks (strong scaling; cfg5's 8 poses) instead of "
                          "one replica of the whole step per rank")
+    ap.add_argument("--overlap", action="store_true",
+                    help="MS_FLAG_OVERLAP: stage (e) of a band runs beside stage (d) of the next on a second stream")
     ap.add_argument("--sync", action="store_true",
                     help="render without MS_FLAG_NO_SYNC (every view reads its counts back to size its scratch)")
     ap.add_argument("--waves", type=int, default=0, help="depth waves (ms_opts.waves): 0 = auto, -1 = off, C > 0 = wave size")

@@ -115,6 +115,11 @@ enum {
                               ms_last_stats then returns MS_ERR_CAPACITY (stats.overflow = 1) and the next render sizes
                               again.  Ignored (the view synchronises as usual) when there is no such history, with
                               MS_FLAG_KEEP_DEBUG, or when depth waves are asked for or due. */
+  MS_FLAG_OVERLAP = 32,    /* banded views: run stage (e) of band b on a second stream inside the library, beside stage
+                              (d) of band b + 1 (the staging budget split into two halves that alternate).  The image
+                              is bitwise the same and all work is ordered before whatever the caller enqueues next on
+                              its stream.  Off by default: measured on CFG4, both stages contend for the same issue
+                              slots and the view takes as long as without. */
   MS_FLAG_KEEP_ORDER = 8   /* stage (e) also records the order it composited every ray's samples in (4 B per sample)
                               for ms_debug_sample_order*: the order the product really used, not a re-derivation */
 };

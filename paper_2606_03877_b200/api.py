@@ -20,6 +20,7 @@ PATH_AUTO, PATH_FP32, PATH_BF16_TC = 0, 1, 2
 FLAG_KEEP_DEBUG, FLAG_STAGE_TIMES = 1, 2
 FLAG_KEEP_ORDER = 8     # stage (e) records the order it composited in (ms_debug_sample_order*)
 FLAG_NO_SYNC = 16        # no host synchronisation when the previous view sized the scratch (ms_opts.flags)
+FLAG_OVERLAP = 32       # banded views: stage (e) of a band on a second stream beside stage (d) of the next (off by default)
 FLAG_DEBUG_ALL = FLAG_KEEP_DEBUG | FLAG_KEEP_ORDER
 FLAG_TILE_ORDER = 4     # contact mode: the paper's shared per-tile order instead of the exact per-ray order
 STAGES = ("bin", "sort", "isect", "mlp", "composite")

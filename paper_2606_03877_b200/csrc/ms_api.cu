@@ -49,6 +49,8 @@ struct ms_scene {
   // view after the next begins (they have long completed then: no wait that would drain the stream)
   struct EvSet {
     std::vector<cudaEvent_t> ev;
+    std::vector<cudaEvent_t> evc;  // overlapped bands: start / end of stage (e) of band b on the second stream (2b, 2b + 1)
+    bool overlap = false;
     int bands = 0;
     bool pending = false;          // recorded, not yet added to stage_sum
   } evs[2];
@@ -58,6 +60,9 @@ struct ms_scene {
   double stage_sum[MS_N_STAGES] = {};
   int64_t stage_views = 0;
   cudaEvent_t frame_done = nullptr;  // recorded after the counters' readback copy of the last view
+  // banded views: stage (e) of band b runs on st2 while stage (d) of band b + 1 runs on the caller's stream
+  cudaStream_t st2 = nullptr;
+  cudaEvent_t ev_mlp[2] = {nullptr, nullptr}, ev_comp[2] = {nullptr, nullptr};
   bool frame_pending = false;
   bool prev_terminated = false;      // MS_WAVES_AUTO: the previous view had rays stopping early
   // last view
@@ -185,8 +190,17 @@ int harvest_stage_times(ms_scene *sc, int set) {
     return true;
   };
   bool ok = el(0, 1, &ms[MS_STAGE_BIN]) && el(1, 2, &ms[MS_STAGE_SORT]) && el(2, 3, &ms[MS_STAGE_ISECT]);
-  for (int b = 0; ok && b < E.bands; ++b)
-    ok = el(3 + 2 * b, 4 + 2 * b, &ms[MS_STAGE_MLP]) && el(4 + 2 * b, 5 + 2 * b, &ms[MS_STAGE_COMPOSITE]);
+  for (int b = 0; ok && b < E.bands; ++b) {
+    ok = el(3 + 2 * b, 4 + 2 * b, &ms[MS_STAGE_MLP]);
+    if (!ok) break;
+    if (E.overlap) {            // stage (e) ran beside the next band's stage (d): its own duration on the second stream
+      float v = 0.f;
+      if (cudaEventElapsedTime(&v, E.evc[2 * b], E.evc[2 * b + 1]) != cudaSuccess) { (void)cudaGetLastError(); ok = false; }
+      ms[MS_STAGE_COMPOSITE] += v;
+    } else {
+      ok = el(4 + 2 * b, 5 + 2 * b, &ms[MS_STAGE_COMPOSITE]);
+    }
+  }
   if (!ok) return MS_OK;
   for (int i = 0; i < MS_N_STAGES; ++i) { sc->stage_sum[i] += ms[i]; sc->last_stage_ms[i] = ms[i]; }
   sc->stage_views += 1;
@@ -443,6 +457,16 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
     cap_hits *= 2;
     n_bands = n_hits <= cap_hits ? 1 : (int)(n_hits / cap_hits) + 1;
   }
+  // MS_FLAG_OVERLAP, two or more bands: the budget becomes two halves, stage (e) of one beside stage (d) of the next
+  const bool overlap = n_bands > 1 && (opts->flags & MS_FLAG_OVERLAP) != 0;
+  if (overlap) {
+    cap_hits = cap_hits > 1 ? cap_hits / 2 : 1;
+    n_bands = (int)(n_hits / cap_hits) + 1;
+    while (prim_bits + 3 + ceil_log2((uint64_t)n_bands) > 32) {
+      cap_hits *= 2;
+      n_bands = (int)(n_hits / cap_hits) + 1;
+    }
+  }
   // depth waves: asked for, or (auto) the previous view had rays stopping early
   int wave_c = 0;
   if (opts->t_stop > 0.0f && !tile_order && !nosync) {
@@ -482,9 +506,11 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   }
   ENS(sc->intervals, (n_hits + 1) * sizeof(MsInterval));
   ENS(sc->hits, (n_hits + 1) * sizeof(MsHit));
-  ENS(sc->staging, (band_hits_cap * (size_t)K + 1) * sizeof(float4));
-  if (want_feat) ENS(sc->staging_feat, (band_hits_cap * (size_t)K + 1) * feat_bytes);
-  if (want_slots) ENS(sc->staging_gate, (band_hits_cap * (size_t)K + 1) * sizeof(float4));
+  const size_t band_samples = band_hits_cap * (size_t)K + 1;     // per staging half
+  const size_t n_half = overlap ? 2 : 1;
+  ENS(sc->staging, n_half * band_samples * sizeof(float4));
+  if (want_feat) ENS(sc->staging_feat, n_half * band_samples * feat_bytes);
+  if (want_slots) ENS(sc->staging_gate, n_half * band_samples * sizeof(float4));
   if (want_slots) ENS(sc->staging_coef, (band_hits_cap * (size_t)K + 1) * sizeof(float4));
   const bool keep_order = (opts->flags & MS_FLAG_KEEP_ORDER) != 0;
   if (keep_order) {
@@ -561,7 +587,32 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   wa.grp_iv0 = (uint32_t *)sc->grp_iv0.p; wa.grp_cnt_c = (uint32_t *)sc->grp_cnt_c.p;
   wa.grp_blocks_c = (uint32_t *)sc->grp_blocks_c.p; wa.blk_off_c = (uint32_t *)sc->blk_off_c.p;
   wa.counters = counters; wa.n_sm = sc->n_sm;
+  if (overlap && !sc->st2) {
+    CK(cudaStreamCreateWithFlags(&sc->st2, cudaStreamNonBlocking));
+    for (int i = 0; i < 2; ++i) {
+      CK(cudaEventCreateWithFlags(&sc->ev_mlp[i], cudaEventDisableTiming));
+      CK(cudaEventCreateWithFlags(&sc->ev_comp[i], cudaEventDisableTiming));
+    }
+  }
+  auto recc = [&](int i) -> cudaError_t {           // stage (e) events of an overlapped view, on the second stream
+    if (!timing) return cudaSuccess;
+    std::vector<cudaEvent_t> &ev = sc->evs[sc->ev_cur].evc;
+    while ((int)ev.size() <= i) {
+      cudaEvent_t e;
+      cudaError_t r = cudaEventCreate(&e);
+      if (r != cudaSuccess) return r;
+      ev.push_back(e);
+    }
+    return cudaEventRecord(ev[i], sc->st2);
+  };
   for (int b = 0; b < n_bands; ++b) {
+    const int half = overlap ? (b & 1) : 0;
+    ma.staging = (float4 *)sc->staging.p + (size_t)half * band_samples;
+    ma.staging_feat = want_feat ? (void *)((char *)sc->staging_feat.p + (size_t)half * band_samples * feat_bytes) : nullptr;
+    ma.staging_gate = want_slots ? (float4 *)sc->staging_gate.p + (size_t)half * band_samples : nullptr;
+    ca.staging = ma.staging; ca.staging_feat = ma.staging_feat; ca.gates = ma.staging_gate;
+    wa.staging = ma.staging;
+    if (overlap && b >= 2) CK(cudaStreamWaitEvent(st, sc->ev_comp[half], 0));   // stage (e) of band b - 2 has left this half
     CK(rec(3 + 2 * b));
     ma.segs.band = (MsBand *)sc->bands.p + b;
     for (int w = 0; w < n_waves; ++w) {
@@ -580,11 +631,22 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
     }
     CK(rec(4 + 2 * b));
     ca.band = band_tab[b];
-    CK(ms_composite(ca, st));
+    if (overlap) {
+      CK(cudaEventRecord(sc->ev_mlp[half], st));
+      CK(cudaStreamWaitEvent(sc->st2, sc->ev_mlp[half], 0));
+      CK(recc(2 * b));
+      CK(ms_composite(ca, sc->st2));
+      CK(recc(2 * b + 1));
+      CK(cudaEventRecord(sc->ev_comp[half], sc->st2));
+    } else {
+      CK(ms_composite(ca, st));
+    }
   }
+  if (overlap) CK(cudaStreamWaitEvent(st, sc->ev_comp[(n_bands - 1) & 1], 0));   // st2 is in order: this covers every band
   CK(rec(3 + 2 * n_bands));
   if (timing) {
     sc->evs[sc->ev_cur].bands = n_bands;
+    sc->evs[sc->ev_cur].overlap = overlap;
     sc->evs[sc->ev_cur].pending = true;
     sc->ev_valid = true;
   }
@@ -606,7 +668,7 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   }
   sc->stats.n_bands = n_bands;
   sc->stats.n_waves = n_waves;
-  sc->stats.staging_bytes = (int64_t)(band_hits_cap * (size_t)K * sample_bytes);   // what this view needed
+  sc->stats.staging_bytes = (int64_t)(n_half * band_hits_cap * (size_t)K * sample_bytes);   // what this view needed
   sc->stats.scratch_bytes = (int64_t)scratch_total(sc);
   sc->dbg_K = K;
   sc->last.valid = true; sc->last.grid = grid; sc->last.cam = cam; sc->last.K = K; sc->last.n_bands = n_bands;
@@ -779,9 +841,16 @@ int ms_scene_destroy(ms_scene *sc) {
   free_buf(sc->host_rgb); free_buf(sc->host_alpha); free_buf(sc->host_feat);
   if (sc->pinned) cudaFreeHost(sc->pinned);
   if (sc->pinned_bands) cudaFreeHost(sc->pinned_bands);
-  for (auto &E : sc->evs)
+  for (auto &E : sc->evs) {
     for (cudaEvent_t e : E.ev) cudaEventDestroy(e);
+    for (cudaEvent_t e : E.evc) cudaEventDestroy(e);
+  }
   if (sc->frame_done) cudaEventDestroy(sc->frame_done);
+  for (int i = 0; i < 2; ++i) {
+    if (sc->ev_mlp[i]) cudaEventDestroy(sc->ev_mlp[i]);
+    if (sc->ev_comp[i]) cudaEventDestroy(sc->ev_comp[i]);
+  }
+  if (sc->st2) cudaStreamDestroy(sc->st2);
   (void)cudaGetLastError();
   delete sc;
   return MS_OK;

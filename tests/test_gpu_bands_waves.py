@@ -42,6 +42,12 @@ def test_bands_leave_the_image_bitwise_unchanged(name, W, H, path):
         assert st.staging_bytes < st1.staging_bytes
         for a, b in zip(out, ref):
             assert (a is None and b is None) or torch.equal(a, b)
+        # MS_FLAG_OVERLAP: stage (e) of a band on a second stream beside stage (d) of the next, two staging halves
+        ser = _render(gs, cam, H, W, cfg.K, path=p, flags=api.FLAG_OVERLAP)
+        st_s = gs.stats()
+        assert st_s.n_bands >= st.n_bands and st_s.n_intervals == st1.n_intervals
+        for a, b in zip(ser, ref):
+            assert (a is None and b is None) or torch.equal(a, b)
     # the structures of a banded frame against the oracle (tile lists, per-ray intervals, sample order of every ray)
     orc = mso.OracleScene(sc)
     assert check_structures(gs, orc, cam, H, W, cfg.K, 16, n_order_rays=4) == st1.n_intervals
@@ -173,9 +179,9 @@ def test_bands_and_waves_across_modes(case):
     gs.waves, gs.band_bytes = -1, -1
     ref = _render(gs, cam, H, W, K, path=path, tile=tile)
     st0 = gs.stats()
-    for waves, band_bytes in ((2, -1), (1, 96 << 10), (3, 512 << 10)):
+    for waves, band_bytes, fl in ((2, -1, 0), (1, 96 << 10, 0), (3, 512 << 10, 0), (2, 96 << 10, api.FLAG_OVERLAP)):
         gs.waves, gs.band_bytes = waves, band_bytes
-        out = _render(gs, cam, H, W, K, path=path, tile=tile, flags=api.FLAG_DEBUG_ALL)
+        out = _render(gs, cam, H, W, K, path=path, tile=tile, flags=api.FLAG_DEBUG_ALL | fl)
         st = gs.stats()
         for a, b in zip(out, ref):
             assert (a is None and b is None) or torch.equal(a, b)
