@@ -209,37 +209,87 @@ __global__ void __launch_bounds__(BT) mlp_bwd_kernel(MsMlpBwdArgs a) {
   }
 }
 
-// The same computation for hidden widths 16 / 32 / 64 / 128 with CG threads per sample (512 threads per CTA; one CTA
-// per SM is resident: the activations of BS samples fill shared memory, so the warps have to come from inside the
-// block.  BS = 128 = one row block, CG = 4 up to width 64; width 128 takes the row block in two halves of BS = 64
-// with CG = 8).  Thread (cg, s) owns the output columns [cg WD/CG, (cg+1) WD/CG) of sample s in the forward pass and
-// every CG-th 4-row chunk of the layer input in the backward pass: accumulators stay in registers, weight rows stream through
-// warp-uniform float4 loads, activations and gradients move as float4 (leading dimensions = 4 mod 8).  The weight
-// gradients X_l^T G_l are register tiles of 8 inputs x (WD / 32) outputs per lane, one (tile, sample range) item per
-// warp.  The sums differ from the generic kernel (and from the fp64 statement of the chain) only in the order of the
-// fp32 additions.
-constexpr int BT4 = 512;              // threads per CTA
-constexpr int NW4 = BT4 / 32;         // warps per CTA
+// The same computation as three register-tiled fp32 GEMMs per layer (any hidden width that is a multiple of 4).
+// Activations and gradients live in shared memory FEATURE-major, X^T[feature][sample] with leading dimension BS + 4
+// (= 4 mod 32 words): a thread owns a 4 x 4 tile and a warp is 8 tile columns x 4 tile rows, so every operand fetch is
+// one float4 per lane with 8 (or 4) distinct 16-byte chunks per warp -- one shared-memory wavefront per 16 FMA
+// instructions, where a thread per sample needs one wavefront per FMA instruction or four per float4 of weights.
+//   forward   Z^T[o][s]  = b[o] + sum_i W[i][o] X^T[i][s]      tile = 4 outputs x 4 samples, weights staged as W[i][o]
+//   dX        gX^T[i][s] = sum_o W[i][o] gZ^T[o][s]            tile = 4 inputs x 4 samples, weights staged as W^T[o][i]
+//   dW        gW[i][o]   = sum_s X^T[i][s] gZ^T[o][s]          tile = 4 inputs x 4 outputs, a warp = 32 inputs x 16 outputs
+// 512 threads per CTA, one CTA per SM (the activations of BS samples fill shared memory; BS = 128 = one row block, or
+// 64 = half of one when 128 do not fit -- width 128, or four hidden layers of 64).  The forward sums run in the order of
+// the generic kernel (bias first, inputs ascending); the backward sums differ from it only in the order of the fp32
+// additions.
+constexpr int TNT = 512;              // threads per CTA
+constexpr int TNW = TNT / 32;         // warps per CTA
+constexpr int TKP = 64;               // contraction steps of one staged weight panel
 
 __device__ __forceinline__ float4 lds4(const float *p) { return *reinterpret_cast<const float4 *>(p); }
 __device__ __forceinline__ void sts4(float *p, float x, float y, float z, float w) {
   *reinterpret_cast<float4 *>(p) = make_float4(x, y, z, w);
 }
-__device__ __forceinline__ float4 ldg4(const float *p) { return __ldg(reinterpret_cast<const float4 *>(p)); }
 
-template <int WD, int CG>
-__global__ void __launch_bounds__(BT4, 1) mlp_bwd_fast_kernel(MsMlpBwdArgs a) {
-  constexpr int BS = BT4 / CG;        // samples per pass
+struct TLayout {
+  int R0, LS, LW;             // rows of X0^T (in_dim rounded up to 4), leading dimensions of the activations / the panel
+  size_t off_x[5];            // float offsets of X0^T (index 0) and H_1^T..H_nh^T; the gradient of a layer's input
+                              // overwrites that input in place (the owner of a tile reads its mask, then writes)
+  size_t off_g0;              // ... except X0^T, which Eq.5's backward still needs: dL/dX0 has rows of its own
+  size_t off_hd;              // 8 rows: the head's raw outputs (0..3) and their gradients (4..7)
+  size_t off_ws;              // weight panel
+  size_t off_acc;             // weight-gradient accumulators of the primitive being walked (0 floats if they do not fit)
+  int acc_w[5], acc_b[5];     // per layer: float offset of its tile slots / bias slots inside the accumulators
+  int acc_floats;
+  size_t floats;
+};
+// weight-gradient slots of layer l: one per (warp tile, tile element, lane) -- lane-contiguous, so a warp adds its
+// 16 tile elements without a bank conflict
+__host__ __device__ inline int t_warp_tiles(int n_in, int n_out, bool head) {
+  return ((n_in + 31) >> 5) * (head ? 1 : (n_out + 15) >> 4);
+}
+__host__ __device__ inline TLayout t_layout(const MsMlpShape &sh, int bs, bool with_acc) {
+  TLayout L;
+  L.R0 = (sh.in_dim + 3) & ~3;
+  L.LS = bs + 4;
+  L.LW = (sh.width > L.R0 ? sh.width : L.R0) + 4;
+  size_t o = 0;
+  L.off_x[0] = o; o += (size_t)L.R0 * L.LS;
+  for (int l = 1; l <= sh.n_hidden; ++l) { L.off_x[l] = o; o += (size_t)sh.width * L.LS; }
+  L.off_g0 = o; o += (size_t)L.R0 * L.LS;
+  L.off_hd = o; o += (size_t)8 * L.LS;
+  L.off_ws = o; o += (size_t)TKP * L.LW;
+  L.off_acc = o;
+  int ac = 0, nin = sh.in_dim;
+  for (int l = 0; l <= sh.n_hidden; ++l) {
+    const bool head = l == sh.n_hidden;
+    const int no = head ? 4 : sh.width;
+    L.acc_w[l] = ac; ac += t_warp_tiles(nin, no, head) * 512;
+    L.acc_b[l] = ac; ac += (no + 15) & ~15;
+    nin = sh.width;
+  }
+  L.acc_floats = with_acc ? ac : 0;
+  o += (size_t)L.acc_floats;
+  L.floats = o;
+  return L;
+}
+
+template <int BS, bool ACC>
+__global__ void __launch_bounds__(TNT, 1) mlp_bwd_t_kernel(MsMlpBwdArgs a) {
   constexpr int PASSES = BT / BS;     // passes per 128-row block
-  constexpr int WQ = WD / CG;         // output columns per thread in the forward pass
-  constexpr int OC = WD > 32 ? WD / 32 : 1;
-  static_assert(WQ % 4 == 0, "float4 weight segments");
+  constexpr int NCG = TNT / BS;       // threads per sample in the per-sample steps
+  constexpr int NSW = BS / 32;        // warps side by side over the samples (8 sample tiles = 32 samples each)
+  constexpr int NFW = (TNW / NSW) * 4;   // feature tiles (of 4) the CTA covers in one pass of a GEMM
   extern __shared__ __align__(16) float sm[];
   __shared__ int s_seg;
   const MsMlpShape &sh = a.shape;
-  const BwdLayout L = bwd_layout(sh, true, BS);
+  const TLayout L = t_layout(sh, BS, ACC);
+  const int LS = L.LS, LW = L.LW, WD = sh.width;
+  float *const DWS = sm + L.off_acc;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int srow_in = tid & (BS - 1), cg = tid / BS;      // sample row inside the block, column group
+  const int srow_in = tid & (BS - 1), cg = tid / BS;      // per-sample steps: sample, helper index
+  const int sg = (warp % NSW) * 8 + (lane & 7);           // GEMMs: sample tile (samples 4 sg .. 4 sg + 3)
+  const int ft = (warp / NSW) * 4 + (lane >> 3);          //        feature tile inside a pass
+  float *const WS = sm + L.off_ws;
   const uint2 r = *a.segs.range;
   const uint32_t *bo = a.segs.blk_off + r.x;
   const uint32_t base = bo[0], n_blocks = bo[r.y - r.x] - base;
@@ -253,13 +303,227 @@ __global__ void __launch_bounds__(BT4, 1) mlp_bwd_fast_kernel(MsMlpBwdArgs a) {
       off += nin * no + no; nin = no;
     }
   }
-  for (uint32_t unit = blockIdx.x; unit < n_blocks * PASSES; unit += gridDim.x) {
+
+  // Z^T = W^T X^T + b for the n_out (multiple of 4) leading outputs of a layer whose rows are ldw apart
+  auto gemm_fwd = [&](const float *XT, int n_in, const float *Wg, int ldw, int n_out, bool relu, float *OUT) {
+    const int n_ft = n_out >> 2;
+    const float *bias = Wg + (size_t)n_in * ldw;
+    for (int f0 = 0; f0 < n_ft; f0 += NFW) {
+      const int f = f0 + ft;
+      const bool on = f < n_ft;
+      float acc[4][4];
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const float b = on ? __ldg(bias + 4 * f + q) : 0.0f;
+#pragma unroll
+        for (int p = 0; p < 4; ++p) acc[q][p] = b;
+      }
+      for (int i0 = 0; i0 < n_in; i0 += TKP) {
+        const int kp = min(TKP, n_in - i0);
+        __syncthreads();                                   // the panel's previous readers are done
+        for (int e = tid; e < kp * n_out; e += TNT) {
+          const int rr = e / n_out, c = e - rr * n_out;
+          WS[rr * LW + c] = __ldg(Wg + (size_t)(i0 + rr) * ldw + c);
+        }
+        __syncthreads();
+        if (on) {
+          const float *xp = XT + (size_t)i0 * LS + 4 * sg, *wq = WS + 4 * f;
+#pragma unroll 4
+          for (int rr = 0; rr < kp; ++rr) {
+            const float4 x4 = lds4(xp + (size_t)rr * LS), w4 = lds4(wq + rr * LW);
+            const float xs[4] = {x4.x, x4.y, x4.z, x4.w}, ws[4] = {w4.x, w4.y, w4.z, w4.w};
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+#pragma unroll
+              for (int p = 0; p < 4; ++p) acc[q][p] = fmaf(xs[p], ws[q], acc[q][p]);
+          }
+        }
+      }
+      if (on) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          float *y = OUT + (size_t)(4 * f + q) * LS + 4 * sg;
+          if (relu) sts4(y, fmaxf(acc[q][0], 0.0f), fmaxf(acc[q][1], 0.0f), fmaxf(acc[q][2], 0.0f), fmaxf(acc[q][3], 0.0f));
+          else sts4(y, acc[q][0], acc[q][1], acc[q][2], acc[q][3]);
+        }
+      }
+    }
+    __syncthreads();
+  };
+
+  // gX^T = W gZ^T over the n_out leading outputs, masked by the ReLU of the layer below (XT = its output, or null)
+  auto gemm_dx = [&](const float *G, int n_out, const float *Wg, int ldw, int n_in, const float *XT, float *GIN) {
+    const int n_pad = (n_in + 3) & ~3, n_it = n_pad >> 2;
+    for (int f0 = 0; f0 < n_it; f0 += NFW) {
+      const int f = f0 + ft;
+      const bool on = f < n_it;
+      float acc[4][4];
+#pragma unroll
+      for (int q = 0; q < 4; ++q)
+#pragma unroll
+        for (int p = 0; p < 4; ++p) acc[q][p] = 0.0f;
+      for (int o0 = 0; o0 < n_out; o0 += TKP) {
+        const int kp = min(TKP, n_out - o0);
+        __syncthreads();
+        for (int e = tid; e < n_pad * kp; e += TNT) {      // W^T[o][i], inputs past n_in read as 0
+          const int i = e / kp, c = e - i * kp;
+          WS[c * LW + i] = i < n_in ? __ldg(Wg + (size_t)i * ldw + o0 + c) : 0.0f;
+        }
+        __syncthreads();
+        if (on) {
+          const float *gp = G + (size_t)o0 * LS + 4 * sg, *wq = WS + 4 * f;
+#pragma unroll 4
+          for (int c = 0; c < kp; ++c) {
+            const float4 g4 = lds4(gp + (size_t)c * LS), w4 = lds4(wq + c * LW);
+            const float gs[4] = {g4.x, g4.y, g4.z, g4.w}, ws[4] = {w4.x, w4.y, w4.z, w4.w};
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+#pragma unroll
+              for (int p = 0; p < 4; ++p) acc[q][p] = fmaf(ws[q], gs[p], acc[q][p]);
+          }
+        }
+      }
+      if (on) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          const size_t at = (size_t)(4 * f + q) * LS + 4 * sg;
+          if (XT) {
+            const float4 x4 = lds4(XT + at);
+            sts4(GIN + at, x4.x > 0.0f ? acc[q][0] : 0.0f, x4.y > 0.0f ? acc[q][1] : 0.0f,
+                 x4.z > 0.0f ? acc[q][2] : 0.0f, x4.w > 0.0f ? acc[q][3] : 0.0f);
+          } else {
+            sts4(GIN + at, acc[q][0], acc[q][1], acc[q][2], acc[q][3]);
+          }
+        }
+      }
+    }
+  };
+
+  // gW += X G^T over the samples of the pass (and the bias row: sum_s gZ^T[o][s]).  A warp = 32 inputs x 16 outputs:
+  // lane (it, ot) holds the inputs 32 iw + 8 q + it and the outputs 16 ow + 4 q' + ot, rows that sit 4 banks apart.
+  // The head (4 outputs) gives its 4 lane rows to a further split of the samples instead.
+  auto gemm_dw = [&](const float *XT, int n_in, const float *G, int n_out, bool head, float *gw, int ldw, int l) {
+    const int n_iw = (n_in + 31) >> 5, n_ow = head ? 1 : (n_out + 15) >> 4;
+    const int n_wt = n_iw * n_ow;
+    int SS = 1;
+    while (2 * SS * n_wt <= TNW && BS / (2 * SS) >= (head ? 16 : 4)) SS *= 2;
+    const int it = lane & 7, ot = lane >> 3;
+    for (int item = warp; item < n_wt * SS; item += TNW) {
+      const int wt = item / SS, part = item - wt * SS;
+      const int iw = wt / n_ow, ow = wt - iw * n_ow;
+      int s_n = BS / SS, s_lo = part * s_n;
+      if (head) { s_n >>= 2; s_lo += ot * s_n; }
+      const float *xr = XT + (size_t)(32 * iw + it) * LS + s_lo;
+      const float *gr = G + (size_t)(head ? 0 : 16 * ow + ot) * LS + s_lo;
+      const int gstep = head ? LS : 4 * LS;
+      const bool do_bias = iw == 0;                        // warp-uniform
+      float acc[4][4], bsum[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+      for (int q = 0; q < 4; ++q)
+#pragma unroll
+        for (int p = 0; p < 4; ++p) acc[q][p] = 0.0f;
+      for (int s0 = 0; s0 < s_n; s0 += 4) {
+        float4 x[4], g4[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          x[q] = lds4(xr + (size_t)(8 * q) * LS + s0);
+          g4[q] = lds4(gr + (size_t)q * gstep + s0);
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+#pragma unroll
+          for (int p = 0; p < 4; ++p) {
+            float v = acc[q][p];
+            v = fmaf(x[q].x, g4[p].x, v); v = fmaf(x[q].y, g4[p].y, v);
+            v = fmaf(x[q].z, g4[p].z, v); v = fmaf(x[q].w, g4[p].w, v);
+            acc[q][p] = v;
+          }
+        if (do_bias) {
+#pragma unroll
+          for (int p = 0; p < 4; ++p) bsum[p] += (g4[p].x + g4[p].y) + (g4[p].z + g4[p].w);
+        }
+      }
+      if (ACC) {                    // into the primitive's accumulators: slot (warp tile, element, lane)
+        float *slot = DWS + L.acc_w[l] + wt * 512 + lane;
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+#pragma unroll
+          for (int p = 0; p < 4; ++p) atomicAdd(slot + (q * 4 + p) * 32, acc[q][p]);
+        if (do_bias && it == 0) {
+#pragma unroll
+          for (int p = 0; p < 4; ++p) atomicAdd(DWS + L.acc_b[l] + (head ? p : 16 * ow + 4 * p + ot), bsum[p]);
+        }
+        continue;
+      }
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const int i = 32 * iw + 8 * q + it;
+        if (i >= n_in) continue;
+#pragma unroll
+        for (int p = 0; p < 4; ++p) {
+          const int o = head ? p : 16 * ow + 4 * p + ot;
+          if (o < n_out && acc[q][p] != 0.0f) atomicAdd(gw + (size_t)i * ldw + o, acc[q][p]);
+        }
+      }
+      if (do_bias && it == 0) {
+#pragma unroll
+        for (int p = 0; p < 4; ++p) {
+          const int o = head ? p : 16 * ow + 4 * p + ot;
+          if (o < n_out && bsum[p] != 0.0f) atomicAdd(gw + (size_t)n_in * ldw + o, bsum[p]);
+        }
+      }
+    }
+  };
+
+  // the accumulators of one primitive go to g_weights (one atomic per non-zero slot) and are cleared
+  auto flush_acc = [&](int prim) {
+    __syncthreads();
+    float *gwp = a.g_weights + (size_t)prim * sh.params;
+    for (int l = 0; l < NL; ++l) {
+      const bool head = l == nh;
+      const int n_in = n_in_l[l], n_out = head ? 4 : WD, ldw = head ? sh.out_dim : WD;
+      const int n_ow = head ? 1 : (n_out + 15) >> 4;
+      const int n_slots = t_warp_tiles(n_in, n_out, head) * 512;
+      float *gw = gwp + off_w[l];
+      for (int e = tid; e < n_slots; e += TNT) {
+        const float v = DWS[L.acc_w[l] + e];
+        if (v == 0.0f) continue;
+        DWS[L.acc_w[l] + e] = 0.0f;
+        const int wt = e >> 9, qp = (e >> 5) & 15, ln = e & 31;
+        const int iw = wt / n_ow, ow = wt - iw * n_ow;
+        const int i = 32 * iw + 8 * (qp >> 2) + (ln & 7), o = head ? (qp & 3) : 16 * ow + 4 * (qp & 3) + (ln >> 3);
+        if (i < n_in && o < n_out) atomicAdd(gw + (size_t)i * ldw + o, v);
+      }
+      for (int o = tid; o < n_out; o += TNT) {
+        const float v = DWS[L.acc_b[l] + o];
+        DWS[L.acc_b[l] + o] = 0.0f;
+        if (v != 0.0f) atomicAdd(gw + (size_t)n_in * ldw + o, v);
+      }
+    }
+    __syncthreads();
+  };
+
+  if (ACC) {
+    for (int e = tid; e < L.acc_floats; e += TNT) DWS[e] = 0.0f;
+  }
+  int acc_prim = -1;
+  // with accumulators a CTA walks a contiguous run of (row block, pass) units -- consecutive units mostly belong to
+  // one primitive; without, the CTAs interleave (neighbouring CTAs then share a primitive's weights in L2)
+  const uint32_t n_units = n_blocks * PASSES;
+  const uint32_t unit_lo = ACC ? (uint32_t)(((uint64_t)n_units * blockIdx.x) / gridDim.x) : blockIdx.x;
+  const uint32_t unit_hi = ACC ? (uint32_t)(((uint64_t)n_units * (blockIdx.x + 1)) / gridDim.x) : n_units;
+  const uint32_t unit_step = ACC ? 1u : gridDim.x;
+  for (uint32_t unit = unit_lo; unit < unit_hi; unit += unit_step) {
     const uint32_t blk = unit / PASSES, pass = unit % PASSES;
     __syncthreads();
     if (tid == 0) s_seg = find_seg(bo, (int)(r.y - r.x), base, blk);
     __syncthreads();
     const uint32_t g = r.x + (uint32_t)s_seg;
     const int prim = a.segs.prim ? (int)a.segs.prim[g] : (int)g;
+    if (ACC && prim != acc_prim) {                         // block-uniform
+      if (acc_prim >= 0) flush_acc(acc_prim);
+      acc_prim = prim;
+    }
     const uint32_t first = a.segs.iv0[g], count = a.segs.cnt ? a.segs.cnt[g] : a.segs.iv0[g + 1] - first;
     const uint64_t srow = (uint64_t)(blk - (bo[s_seg] - base)) * BT + pass * BS + srow_in;
     const uint32_t j = (uint32_t)(srow / (uint32_t)a.K);
@@ -272,99 +536,36 @@ __global__ void __launch_bounds__(BT4, 1) mlp_bwd_fast_kernel(MsMlpBwdArgs a) {
     if (live) iv = a.intervals[first + j];
     const float d[3] = {iv.dx, iv.dy, iv.dz};
     const float t = ms_sample_t(iv.t_in, iv.delta, k);
-    float *X0 = sm + L.off_h[0] + (size_t)srow_in * L.ld0;
-    {                                 // the encoded input of the sample: frequency l by column group l mod 4
+    float *X0 = sm + L.off_x[0] + srow_in;                 // this sample's column of X0^T: feature i at X0[i LS]
+    {                                 // the encoded input of the sample: frequency l by helper l mod NCG
       float u[3];
       ms_sample_u(Ap, mu, a.cam.o, d, t, u);
       if (cg == 0) {
-        X0[0] = u[0]; X0[1] = u[1]; X0[2] = u[2];
-        if (sh.use_viewdir) { float *v = X0 + 3 + 6 * sh.n_freq; v[0] = d[0]; v[1] = d[1]; v[2] = d[2]; }
+        X0[0] = u[0]; X0[LS] = u[1]; X0[2 * LS] = u[2];
+        if (sh.use_viewdir) { float *v = X0 + (size_t)(3 + 6 * sh.n_freq) * LS; v[0] = d[0]; v[LS] = d[1]; v[2 * LS] = d[2]; }
+        for (int i = sh.in_dim; i < L.R0; ++i) X0[(size_t)i * LS] = 0.0f;
       }
-      for (int l = cg; l < sh.n_freq; l += CG) {
+      for (int l = cg; l < sh.n_freq; l += NCG) {
         const float scale = (float)(1 << l);
         float sv[3], cv[3];
 #pragma unroll
         for (int c = 0; c < 3; ++c) sincospif(scale * u[c], &sv[c], &cv[c]);
-        float *x = X0 + 3 + 6 * l;
-        x[0] = sv[0]; x[1] = sv[1]; x[2] = sv[2];
-        x[3] = cv[0]; x[4] = cv[1]; x[5] = cv[2];
+        float *x = X0 + (size_t)(3 + 6 * l) * LS;
+        x[0] = sv[0]; x[LS] = sv[1]; x[2 * LS] = sv[2];
+        x[3 * LS] = cv[0]; x[4 * LS] = cv[1]; x[5 * LS] = cv[2];
       }
     }
-    __syncthreads();
-    // ---- forward: this thread's WQ columns of every hidden layer ----
-    for (int l = 0; l < nh; ++l) {
-      const float *src = sm + L.off_h[l] + (size_t)srow_in * (l == 0 ? L.ld0 : L.ldw);
-      float *dst = sm + L.off_h[l + 1] + (size_t)srow_in * L.ldw + cg * WQ;
-      const float *w = wp + off_w[l] + cg * WQ;
-      const int nin = n_in_l[l];
-      float acc[WQ];
-#pragma unroll
-      for (int q = 0; q < WQ / 4; ++q) {
-        const float4 v = ldg4(w + nin * WD + 4 * q);
-        acc[4 * q] = v.x; acc[4 * q + 1] = v.y; acc[4 * q + 2] = v.z; acc[4 * q + 3] = v.w;
-      }
-      int i = 0;
-      for (; i + 4 <= nin; i += 4) {
-        const float4 x4 = lds4(src + i);
-        const float xs[4] = {x4.x, x4.y, x4.z, x4.w};
-#pragma unroll
-        for (int ii = 0; ii < 4; ++ii) {
-          const float *wr = w + (i + ii) * WD;
-#pragma unroll
-          for (int q = 0; q < WQ / 4; ++q) {
-            const float4 v = ldg4(wr + 4 * q);
-            acc[4 * q] = fmaf(xs[ii], v.x, acc[4 * q]); acc[4 * q + 1] = fmaf(xs[ii], v.y, acc[4 * q + 1]);
-            acc[4 * q + 2] = fmaf(xs[ii], v.z, acc[4 * q + 2]); acc[4 * q + 3] = fmaf(xs[ii], v.w, acc[4 * q + 3]);
-          }
-        }
-      }
-      for (; i < nin; ++i) {
-        const float xi = src[i];
-        const float *wr = w + i * WD;
-#pragma unroll
-        for (int q = 0; q < WQ / 4; ++q) {
-          const float4 v = ldg4(wr + 4 * q);
-          acc[4 * q] = fmaf(xi, v.x, acc[4 * q]); acc[4 * q + 1] = fmaf(xi, v.y, acc[4 * q + 1]);
-          acc[4 * q + 2] = fmaf(xi, v.z, acc[4 * q + 2]); acc[4 * q + 3] = fmaf(xi, v.w, acc[4 * q + 3]);
-        }
-      }
-#pragma unroll
-      for (int q = 0; q < WQ / 4; ++q)
-        sts4(dst + 4 * q, fmaxf(acc[4 * q], 0.0f), fmaxf(acc[4 * q + 1], 0.0f), fmaxf(acc[4 * q + 2], 0.0f),
-             fmaxf(acc[4 * q + 3], 0.0f));
-      __syncthreads();
-    }
-    // ---- head: partial sums over this thread's WQ inputs, summed by column group 0 ----
-    float *G = sm + L.off_g0, *Gn = sm + L.off_g1;
+    // ---- forward ----
+    for (int l = 0; l < nh; ++l)
+      gemm_fwd(sm + L.off_x[l], n_in_l[l], wp + off_w[l], WD, WD, true, sm + L.off_x[l + 1]);
+    float *const RAW = sm + L.off_hd, *const GH = RAW + 4 * (size_t)LS;
     const int no_h = sh.out_dim;
-    {
-      const float *src = sm + L.off_h[nh] + (size_t)srow_in * L.ldw + cg * WQ;
-      const float *w = wp + off_w[nh] + (size_t)(cg * WQ) * no_h;
-      float pr[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-      for (int q = 0; q < WQ / 4; ++q) {
-        const float4 x4 = lds4(src + 4 * q);
-        const float xs[4] = {x4.x, x4.y, x4.z, x4.w};
-#pragma unroll
-        for (int ii = 0; ii < 4; ++ii)
-#pragma unroll
-          for (int o = 0; o < 4; ++o) pr[o] = fmaf(xs[ii], __ldg(w + (4 * q + ii) * no_h + o), pr[o]);
-      }
-      sts4(Gn + (size_t)srow_in * L.ldg + 4 * cg, pr[0], pr[1], pr[2], pr[3]);
-    }
-    __syncthreads();
+    gemm_fwd(sm + L.off_x[nh], WD, wp + off_w[nh], no_h, 4, false, RAW);    // raw colour and density
     float g_delta = 0.0f;
     if (cg == 0) {                    // gradient of the head's four outputs (sigmoid colour, softplus density)
-      float raw[4], gr[4] = {0.f, 0.f, 0.f, 0.f};
-      const float *pp = Gn + (size_t)srow_in * L.ldg;
-      const float *bh = wp + off_w[nh] + WD * no_h;
-      float4 ps = lds4(pp);
-#pragma unroll
-      for (int c = 1; c < CG; ++c) {
-        const float4 pc = lds4(pp + 4 * c);
-        ps.x += pc.x; ps.y += pc.y; ps.z += pc.z; ps.w += pc.w;
-      }
-      raw[0] = __ldg(bh) + ps.x; raw[1] = __ldg(bh + 1) + ps.y; raw[2] = __ldg(bh + 2) + ps.z; raw[3] = __ldg(bh + 3) + ps.w;
+      const float *pp = RAW + srow_in;
+      const float raw[4] = {pp[0], pp[LS], pp[2 * LS], pp[3 * LS]};
+      float gr[4] = {0.f, 0.f, 0.f, 0.f};
       if (live) {
         const size_t idx = (size_t)(uint32_t)iv.slot * (size_t)a.K + (size_t)k;
         const float4 gs = a.gstage[idx];
@@ -375,132 +576,29 @@ __global__ void __launch_bounds__(BT4, 1) mlp_bwd_fast_kernel(MsMlpBwdArgs a) {
         gr[3] = -iv.delta * e * gs.w / (1.0f + expf(-raw[3]));
         g_delta = -sigma * e * gs.w;
       }
-      sts4(G + (size_t)srow_in * L.ldg, gr[0], gr[1], gr[2], gr[3]);
+      float *gq = GH + srow_in;
+      gq[0] = gr[0]; gq[LS] = gr[1]; gq[2 * LS] = gr[2]; gq[3 * LS] = gr[3];
     }
+    // ---- backward: the gradient of a layer's input replaces that input (X0^T keeps its values: Eq.5 needs them) ----
     for (int l = nh; l >= 0; --l) {
       __syncthreads();
-      const int nin = n_in_l[l];
-      const float *Xl = sm + L.off_h[l];
-      const int ldx = l == 0 ? L.ld0 : L.ldw;
-      float *gw = a.g_weights + (size_t)prim * sh.params + off_w[l];
-      if (l == nh) {
-        // head weights (WD x 4): lane = input row, four outputs per lane; warps over (row group, sample range)
-        constexpr int RG = (WD + 31) / 32, SSH = NW4 / RG, PER = BS / SSH;
-        const int rg = warp % RG, part = warp / RG, row = rg * 32 + lane;
-        const bool on = row < WD;
-        float t4[4] = {0.f, 0.f, 0.f, 0.f}, tb[4] = {0.f, 0.f, 0.f, 0.f};
-        const float *xr = Xl + (size_t)(part * PER) * ldx + (on ? row : 0);
-        const float *gp = G + (size_t)(part * PER) * L.ldg;
-        for (int s = 0; s < PER; ++s, xr += ldx, gp += L.ldg) {
-          const float4 g4 = lds4(gp);
-          const float x = *xr;
-          t4[0] = fmaf(x, g4.x, t4[0]); t4[1] = fmaf(x, g4.y, t4[1]); t4[2] = fmaf(x, g4.z, t4[2]); t4[3] = fmaf(x, g4.w, t4[3]);
-          tb[0] += g4.x; tb[1] += g4.y; tb[2] += g4.z; tb[3] += g4.w;
-        }
-        if (on) {
-#pragma unroll
-          for (int o = 0; o < 4; ++o) if (t4[o] != 0.0f) atomicAdd(gw + row * no_h + o, t4[o]);
-        }
-        if (rg == 0 && lane == 0) {
-#pragma unroll
-          for (int o = 0; o < 4; ++o) if (tb[o] != 0.0f) atomicAdd(gw + WD * no_h + o, tb[o]);
-        }
-      } else {
-        // hidden weights (nin x WD): items = (8-row tile, sample range), lane = output column (+ 32 c)
-        const int n_tiles = (nin + 7) >> 3;
-        int SS = 1;
-        while (2 * SS * n_tiles <= NW4 && SS < 8) SS *= 2;
-        const int per = BS / SS;
-        for (int item = warp; item < n_tiles * SS; item += NW4) {
-          const int tile = item / SS, part = item - tile * SS, i0 = tile * 8;
-          float t8[8][OC], tb[OC];
-#pragma unroll
-          for (int c = 0; c < OC; ++c) {
-            tb[c] = 0.0f;
-#pragma unroll
-            for (int ii = 0; ii < 8; ++ii) t8[ii][c] = 0.0f;
-          }
-          const float *xr = Xl + (size_t)(part * per) * ldx + i0;
-          const float *gp = G + (size_t)(part * per) * L.ldg + (WD >= 32 ? lane : (lane & (WD - 1)));
-          for (int s = 0; s < per; ++s, xr += ldx, gp += L.ldg) {
-            const float4 xa = lds4(xr), xb = lds4(xr + 4);
-#pragma unroll
-            for (int c = 0; c < OC; ++c) {
-              const float gv = gp[32 * c];
-              t8[0][c] = fmaf(xa.x, gv, t8[0][c]); t8[1][c] = fmaf(xa.y, gv, t8[1][c]);
-              t8[2][c] = fmaf(xa.z, gv, t8[2][c]); t8[3][c] = fmaf(xa.w, gv, t8[3][c]);
-              t8[4][c] = fmaf(xb.x, gv, t8[4][c]); t8[5][c] = fmaf(xb.y, gv, t8[5][c]);
-              t8[6][c] = fmaf(xb.z, gv, t8[6][c]); t8[7][c] = fmaf(xb.w, gv, t8[7][c]);
-              tb[c] += gv;
-            }
-          }
-          if (WD >= 32 || lane < WD) {
-#pragma unroll
-            for (int c = 0; c < OC; ++c) {
-              const int o = lane + 32 * c;
-#pragma unroll
-              for (int ii = 0; ii < 8; ++ii)
-                if (i0 + ii < nin && t8[ii][c] != 0.0f) atomicAdd(gw + (i0 + ii) * WD + o, t8[ii][c]);
-              if (tile == 0 && tb[c] != 0.0f) atomicAdd(gw + nin * WD + o, tb[c]);
-            }
-          }
-        }
-      }
-      // gradient of the layer input: this thread's 4-row chunks (every fourth chunk)
-      const float *w = wp + off_w[l];
-      const float *xin = Xl + (size_t)srow_in * ldx;
-      const float *gpr = G + (size_t)srow_in * L.ldg;
-      float *gn = Gn + (size_t)srow_in * L.ldg;
-      if (l == nh) {
-        const float4 g4 = lds4(gpr);
-        for (int i0 = 4 * cg; i0 < nin; i0 += 4 * CG) {
-          const float4 x4 = lds4(xin + i0);
-          const float xs[4] = {x4.x, x4.y, x4.z, x4.w};
-          float v[4];
-#pragma unroll
-          for (int ii = 0; ii < 4; ++ii) {
-            const float *wr = w + (i0 + ii) * no_h;
-            const float vv = __ldg(wr) * g4.x + __ldg(wr + 1) * g4.y + __ldg(wr + 2) * g4.z + __ldg(wr + 3) * g4.w;
-            v[ii] = xs[ii] > 0.0f ? vv : 0.0f;
-          }
-          sts4(gn + i0, v[0], v[1], v[2], v[3]);
-        }
-      } else {
-        for (int i0 = 4 * cg; i0 < nin; i0 += 4 * CG) {
-          const float *wr[4];
-#pragma unroll
-          for (int ii = 0; ii < 4; ++ii) wr[ii] = w + (size_t)min(i0 + ii, nin - 1) * WD;   // rows past nin: discarded
-          float v[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll 4
-          for (int o = 0; o < WD; o += 4) {
-            const float4 g4 = lds4(gpr + o);
-#pragma unroll
-            for (int ii = 0; ii < 4; ++ii) {
-              const float4 ww = ldg4(wr[ii] + o);
-              v[ii] = fmaf(ww.x, g4.x, v[ii]); v[ii] = fmaf(ww.y, g4.y, v[ii]);
-              v[ii] = fmaf(ww.z, g4.z, v[ii]); v[ii] = fmaf(ww.w, g4.w, v[ii]);
-            }
-          }
-          if (l > 0) {
-            const float4 x4 = lds4(xin + i0);
-            v[0] = x4.x > 0.0f ? v[0] : 0.0f; v[1] = x4.y > 0.0f ? v[1] : 0.0f;
-            v[2] = x4.z > 0.0f ? v[2] : 0.0f; v[3] = x4.w > 0.0f ? v[3] : 0.0f;
-          }
-          sts4(gn + i0, v[0], v[1], v[2], v[3]);
-        }
-      }
-      float *tmp = G; G = Gn; Gn = tmp;
+      const bool head = l == nh;
+      const int ldw = head ? no_h : WD, n_out = head ? 4 : WD;
+      float *XT = sm + L.off_x[l];
+      const float *G = head ? GH : sm + L.off_x[l + 1];
+      gemm_dw(XT, n_in_l[l], G, n_out, head, a.g_weights + (size_t)prim * sh.params + off_w[l], ldw, l);
+      gemm_dx(G, n_out, wp + off_w[l], ldw, n_in_l[l], l > 0 ? XT : nullptr, l > 0 ? XT : sm + L.off_g0);
     }
     __syncthreads();
     if (live && cg == 0) {
-      const float *gx = G + (size_t)srow_in * L.ldg;
-      float gu[3] = {gx[0], gx[1], gx[2]};
+      const float *gx = sm + L.off_g0 + srow_in;
+      float gu[3] = {gx[0], gx[LS], gx[2 * LS]};
       float scale = 3.14159265358979323846f;
       for (int l = 0; l < sh.n_freq; ++l) {
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-          const float sn = X0[3 + 6 * l + c], cs = X0[3 + 6 * l + 3 + c];
-          gu[c] += scale * (cs * gx[3 + 6 * l + c] - sn * gx[3 + 6 * l + 3 + c]);
+          const size_t is = (size_t)(3 + 6 * l + c) * LS, ic = (size_t)(3 + 6 * l + 3 + c) * LS;
+          gu[c] += scale * (X0[ic] * gx[is] - X0[is] * gx[ic]);
         }
         scale *= 2.0f;
       }
@@ -515,6 +613,7 @@ __global__ void __launch_bounds__(BT4, 1) mlp_bwd_fast_kernel(MsMlpBwdArgs a) {
       atomicAdd(ig + 7, ((float)k + 0.5f) * gt + g_delta);
     }
   }
+  if (ACC && acc_prim >= 0) flush_acc(acc_prim);
 }
 
 __global__ void interval_bwd_kernel(MsMlpBwdArgs a) {
@@ -593,19 +692,20 @@ __global__ void prim_bwd_kernel(MsMlpBwdArgs a) {
 
 }  // namespace
 
-// which kernel serves the shape: 2 = several threads per sample (widths 16 / 32 / 64 / 128, float4 weight rows),
-// 1 = generic
+// which kernel serves the shape: 2..5 = register-tiled GEMMs (widths that are multiples of 4) over 128 or 64 samples,
+// with or without the primitive's weight-gradient accumulators in shared memory; 1 = generic
 static int bwd_kind(const MsMlpShape &sh, size_t *smem) {
   *smem = 0;
   if (sh.mode != MS_MODE_LOCAL || sh.n_hidden > 4 || sh.n_hidden < 1) return 0;
-  const size_t cap = 220 * 1024;
-  const bool fast_w = sh.width == 16 || sh.width == 32 || sh.width == 64 || sh.width == 128;
-  if (fast_w && sh.params % 4 == 0) {
-    const size_t b = bwd_layout(sh, true, sh.width == 128 ? 64 : BT).floats * sizeof(float);
-    if (b <= cap) { *smem = b; return 2; }
+  const size_t cap = 226 * 1024;
+  if (sh.width % 4 == 0 && sh.width >= 8 && sh.out_dim >= 4) {
+    for (int kind = 2; kind <= 5; ++kind) {              // 128 + acc, 128, 64 + acc, 64
+      const size_t b = t_layout(sh, kind <= 3 ? 128 : 64, (kind & 1) == 0).floats * sizeof(float);
+      if (b <= cap) { *smem = b; return kind; }
+    }
   }
   const size_t b = bwd_layout(sh).floats * sizeof(float);
-  if (b > cap) return 0;
+  if (b > 220 * 1024) return 0;
   *smem = b;
   return 1;
 }
@@ -622,10 +722,10 @@ cudaError_t ms_mlp_bwd(const MsMlpBwdArgs &a, cudaStream_t s) {
   if (kind == 0) return cudaErrorNotSupported;
   void (*fn)(MsMlpBwdArgs) = mlp_bwd_kernel;
   int threads = BT;
-  if (kind == 2) {
-    threads = BT4;
-    fn = a.shape.width == 16 ? mlp_bwd_fast_kernel<16, 4> : a.shape.width == 32 ? mlp_bwd_fast_kernel<32, 4>
-       : a.shape.width == 64 ? mlp_bwd_fast_kernel<64, 4> : mlp_bwd_fast_kernel<128, 8>;
+  if (kind >= 2) {
+    threads = TNT;
+    fn = kind == 2 ? mlp_bwd_t_kernel<128, true> : kind == 3 ? mlp_bwd_t_kernel<128, false>
+       : kind == 4 ? mlp_bwd_t_kernel<64, true> : mlp_bwd_t_kernel<64, false>;
   }
   cudaError_t e = cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
@@ -640,7 +740,7 @@ cudaError_t ms_mlp_bwd(const MsMlpBwdArgs &a, cudaStream_t s) {
     (void)cudaGetLastError();
     occ = 1;
   }
-  fn<<<(unsigned)(n_sm * occ * (kind == 2 ? 1 : 4)), threads, smem, s>>>(a);
+  fn<<<(unsigned)(n_sm * occ * (kind >= 2 ? 1 : 4)), threads, smem, s>>>(a);
   MS_LAUNCHED();
   e = cudaGetLastError();
   if (e != cudaSuccess) return e;
