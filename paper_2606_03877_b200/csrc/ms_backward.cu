@@ -7,12 +7,15 @@
 //                        contractions X_l^T G_l over its 128 samples (threads over (in, out) pairs), added to
 //                        g_weights with one atomic per weight and block; dL/du goes on to the interval:
 //                        u = o' + t d'  ->  dL/do' += du, dL/dd' += t du, dL/dt_in += du.d', dL/ddelta += (k+1/2) du.d'
+//   mlp_bwd_t_kernel     the same chain for widths that are multiples of 4, as register-tiled GEMMs (see its header):
+//                        the kernel that runs for every configuration of the bench; mlp_bwd_kernel serves the rest
 //   interval_bwd_kernel  one thread per (ray, primitive) interval: through delta = (t1 - t_in)/K, t_in = max(t0, t_near),
 //                        t0,1 = (-b -+ s)/a, s = sqrt(b^2 - a c), a = d'.d', b = o'.d', c = o'.o' - 1 to (o', d'), then
 //                        o' = A (o - mu), d' = A d: dL/dA += ..., dL/dmu -= A^T dL/do'
 //   prim_bwd_kernel      one thread per primitive: A = diag(1/s) R(q/|q|)^T  ->  dL/ds, dL/dq
 // Written from the chain rule itself; it shares no code with the test oracle, which states the same chain in fp64.
 #include "ms_internal.cuh"
+#include "ms_tile_gemm.cuh"
 
 namespace {
 
@@ -20,9 +23,6 @@ constexpr int BT = MS_ROWS;   // threads per CTA = samples per row block
 
 // odd leading dimension: a thread walking its own row and a warp walking one column are both conflict-free
 __host__ __device__ inline int ld_of(int n) { return n | 1; }
-// leading dimension = 4 (mod 8) for the 4-threads-per-sample kernel: rows are 16-byte aligned and the float4 accesses
-// of the eight threads of a quarter warp (each on its own row) fall on 32 different banks
-__host__ __device__ inline int ld4_of(int n) { int m = (n + 3) & ~3; return (m & 4) ? m : m + 4; }
 
 struct BwdLayout {
   int ld0, ldw, ldg;          // leading dimensions of X0 (encoded input), H_l (hidden), G (gradients)
@@ -30,16 +30,15 @@ struct BwdLayout {
   size_t off_g0, off_g1;      // the two gradient buffers
   size_t floats;
 };
-__host__ __device__ inline BwdLayout bwd_layout(const MsMlpShape &sh, bool vec4 = false, int rows = BT) {
+__host__ __device__ inline BwdLayout bwd_layout(const MsMlpShape &sh) {
   BwdLayout L;
   const int gmax = sh.width > sh.in_dim ? sh.width : sh.in_dim;
-  if (vec4) { L.ld0 = ld4_of(sh.in_dim); L.ldw = ld4_of(sh.width); L.ldg = ld4_of(gmax); }
-  else { L.ld0 = ld_of(sh.in_dim); L.ldw = ld_of(sh.width); L.ldg = ld_of(gmax); }
+  L.ld0 = ld_of(sh.in_dim); L.ldw = ld_of(sh.width); L.ldg = ld_of(gmax);
   size_t o = 0;
-  L.off_h[0] = o; o += (size_t)rows * L.ld0;
-  for (int l = 1; l <= sh.n_hidden; ++l) { L.off_h[l] = o; o += (size_t)rows * L.ldw; }
-  L.off_g0 = o; o += (size_t)rows * L.ldg;
-  L.off_g1 = o; o += (size_t)rows * L.ldg;
+  L.off_h[0] = o; o += (size_t)BT * L.ld0;
+  for (int l = 1; l <= sh.n_hidden; ++l) { L.off_h[l] = o; o += (size_t)BT * L.ldw; }
+  L.off_g0 = o; o += (size_t)BT * L.ldg;
+  L.off_g1 = o; o += (size_t)BT * L.ldg;
   L.floats = o;
   return L;
 }
@@ -221,14 +220,12 @@ __global__ void __launch_bounds__(BT) mlp_bwd_kernel(MsMlpBwdArgs a) {
 // 64 = half of one when 128 do not fit -- width 128, or four hidden layers of 64).  The forward sums run in the order of
 // the generic kernel (bias first, inputs ascending); the backward sums differ from it only in the order of the fp32
 // additions.
-constexpr int TNT = 512;              // threads per CTA
-constexpr int TNW = TNT / 32;         // warps per CTA
-constexpr int TKP = 64;               // contraction steps of one staged weight panel
+constexpr int TNT = TG_NT;            // threads per CTA
+constexpr int TNW = TG_NW;            // warps per CTA
+constexpr int TKP = TG_KP;            // contraction steps of one staged weight panel
 
-__device__ __forceinline__ float4 lds4(const float *p) { return *reinterpret_cast<const float4 *>(p); }
-__device__ __forceinline__ void sts4(float *p, float x, float y, float z, float w) {
-  *reinterpret_cast<float4 *>(p) = make_float4(x, y, z, w);
-}
+__device__ __forceinline__ float4 lds4(const float *p) { return tg_lds4(p); }
+__device__ __forceinline__ void sts4(float *p, float x, float y, float z, float w) { tg_sts4(p, x, y, z, w); }
 
 struct TLayout {
   int R0, LS, LW;             // rows of X0^T (in_dim rounded up to 4), leading dimensions of the activations / the panel
@@ -304,51 +301,8 @@ __global__ void __launch_bounds__(TNT, 1) mlp_bwd_t_kernel(MsMlpBwdArgs a) {
     }
   }
 
-  // Z^T = W^T X^T + b for the n_out (multiple of 4) leading outputs of a layer whose rows are ldw apart
   auto gemm_fwd = [&](const float *XT, int n_in, const float *Wg, int ldw, int n_out, bool relu, float *OUT) {
-    const int n_ft = n_out >> 2;
-    const float *bias = Wg + (size_t)n_in * ldw;
-    for (int f0 = 0; f0 < n_ft; f0 += NFW) {
-      const int f = f0 + ft;
-      const bool on = f < n_ft;
-      float acc[4][4];
-#pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        const float b = on ? __ldg(bias + 4 * f + q) : 0.0f;
-#pragma unroll
-        for (int p = 0; p < 4; ++p) acc[q][p] = b;
-      }
-      for (int i0 = 0; i0 < n_in; i0 += TKP) {
-        const int kp = min(TKP, n_in - i0);
-        __syncthreads();                                   // the panel's previous readers are done
-        for (int e = tid; e < kp * n_out; e += TNT) {
-          const int rr = e / n_out, c = e - rr * n_out;
-          WS[rr * LW + c] = __ldg(Wg + (size_t)(i0 + rr) * ldw + c);
-        }
-        __syncthreads();
-        if (on) {
-          const float *xp = XT + (size_t)i0 * LS + 4 * sg, *wq = WS + 4 * f;
-#pragma unroll 4
-          for (int rr = 0; rr < kp; ++rr) {
-            const float4 x4 = lds4(xp + (size_t)rr * LS), w4 = lds4(wq + rr * LW);
-            const float xs[4] = {x4.x, x4.y, x4.z, x4.w}, ws[4] = {w4.x, w4.y, w4.z, w4.w};
-#pragma unroll
-            for (int q = 0; q < 4; ++q)
-#pragma unroll
-              for (int p = 0; p < 4; ++p) acc[q][p] = fmaf(xs[p], ws[q], acc[q][p]);
-          }
-        }
-      }
-      if (on) {
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          float *y = OUT + (size_t)(4 * f + q) * LS + 4 * sg;
-          if (relu) sts4(y, fmaxf(acc[q][0], 0.0f), fmaxf(acc[q][1], 0.0f), fmaxf(acc[q][2], 0.0f), fmaxf(acc[q][3], 0.0f));
-          else sts4(y, acc[q][0], acc[q][1], acc[q][2], acc[q][3]);
-        }
-      }
-    }
-    __syncthreads();
+    tg_fwd<BS>(XT, n_in, Wg, ldw, n_out, relu, OUT, WS, LS, LW);
   };
 
   // gX^T = W gZ^T over the n_out leading outputs, masked by the ReLU of the layer below (XT = its output, or null)

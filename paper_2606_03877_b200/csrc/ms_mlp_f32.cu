@@ -5,6 +5,7 @@
 // fp32 FMA accumulation, rgb = sigmoid, sigma = softplus, e = exp(-sigma*delta).
 // This path is the accuracy reference on the device; the throughput path is ms_mlp_tc.cu.
 #include "ms_internal.cuh"
+#include "ms_tile_gemm.cuh"
 
 namespace {
 
@@ -335,28 +336,39 @@ __global__ void __launch_bounds__(MS_ROWS / SPT, 6) mlp_f32_w32_kernel(MsMlpArgs
   }
 }
 
-// Wide MLPs (16 / 64 / 128 hidden units; north-star mode): the same arithmetic in the same order as mlp_f32_kernel
-// (acc = b; acc = fma(x_i, W[i][o], acc) for i ascending -- bitwise the same staging), laid out for throughput.  CG
-// threads share a pair of samples: thread (cg, sp) owns the output columns [cg WD/CG, (cg+1) WD/CG) of the samples sp
-// and sp + 64 of the row block, activations live in shared memory (rows 16-byte aligned, leading dimension = 4 mod 8:
-// the float4 reads of a quarter warp fall on 32 different banks), weight rows stream through warp-uniform float4 loads
-// and each serves two samples (8 FMAs per loaded float4).
-__host__ __device__ inline int ld4_of(int n) { int m = (n + 3) & ~3; return (m & 4) ? m : m + 4; }
-__device__ __forceinline__ float4 lds4(const float *p) { return *reinterpret_cast<const float4 *>(p); }
-__device__ __forceinline__ float4 ldg4(const float *p) { return __ldg(reinterpret_cast<const float4 *>(p)); }
+// North-star mode, hidden widths that are multiples of 4: the layers as register-tiled fp32 GEMMs over the 128 samples
+// of a row block (ms_tile_gemm.cuh: feature-major activations in shared memory, 4 x 4 thread tiles, staged weight
+// panels).  The same arithmetic in the same order as mlp_f32_kernel (acc = b; acc = fma(x_i, W[i][o], acc) for i
+// ascending) -- bitwise the same staging.  Shared memory: X0^T, two buffers that alternate as layer outputs (the head's
+// raw outputs land in the free one), the weight panel.
+struct WideLayout {
+  int R0, LS, LW;
+  size_t off_a, off_b, off_ws, floats;
+};
+__host__ __device__ inline WideLayout wide_layout(const MsMlpShape &sh) {
+  WideLayout L;
+  L.R0 = (sh.in_dim + 3) & ~3;
+  L.LS = MS_ROWS + 4;
+  const int rows = sh.width > sh.out_dim ? sh.width : ((sh.out_dim + 3) & ~3);
+  L.LW = rows + 4;
+  size_t o = (size_t)L.R0 * L.LS;
+  L.off_a = o; o += (size_t)rows * L.LS;
+  L.off_b = o; o += (size_t)rows * L.LS;
+  L.off_ws = o; o += (size_t)TG_KP * L.LW;
+  L.floats = o;
+  return L;
+}
 
-template <int WD, int CG>
-__global__ void __launch_bounds__(MS_ROWS * CG / 2) mlp_f32_wide_kernel(MsMlpArgs a) {
-  constexpr int HS = MS_ROWS / 2;     // thread (cg, sp): rows sp and sp + HS
-  constexpr int WQ = WD / CG;
-  static_assert(WQ % 4 == 0, "float4 weight segments");
+__global__ void __launch_bounds__(TG_NT) mlp_f32_tile_kernel(MsMlpArgs a) {
+  constexpr int BS = MS_ROWS, NCG = TG_NT / BS;
   extern __shared__ __align__(16) float sm[];
   __shared__ int s_seg;
   const MsMlpShape &sh = a.shape;
   const LaunchView lv(a.segs);
-  const int ld0 = ld4_of(sh.in_dim), ldw = ld4_of(WD);
-  float *X0 = sm, *HA = X0 + (size_t)MS_ROWS * ld0, *HB = HA + (size_t)MS_ROWS * ldw;
-  const int tid = threadIdx.x, sp = tid & (HS - 1), cg = tid / HS;
+  const WideLayout L = wide_layout(sh);
+  const int LS = L.LS, LW = L.LW, WD = sh.width;
+  float *const X0T = sm, *const HA = sm + L.off_a, *const HB = sm + L.off_b, *const WS = sm + L.off_ws;
+  const int tid = threadIdx.x, srow_in = tid & (BS - 1), cg = tid / BS;
   const uint32_t blk_lo = (uint32_t)(((uint64_t)lv.n_blocks * blockIdx.x) / gridDim.x);
   const uint32_t blk_hi = (uint32_t)(((uint64_t)lv.n_blocks * (blockIdx.x + 1)) / gridDim.x);
   for (uint32_t blk = blk_lo; blk < blk_hi; ++blk) {
@@ -371,137 +383,70 @@ __global__ void __launch_bounds__(MS_ROWS * CG / 2) mlp_f32_wide_kernel(MsMlpArg
     const int prim = a.segs.prim ? (int)a.segs.prim[g] : (int)g;
     const float *wp = a.weights_f32 + (size_t)prim * sh.params;
     const uint32_t first = a.segs.iv0[g], count = a.segs.cnt ? a.segs.cnt[g] : a.segs.iv0[g + 1] - first;
-    const uint64_t s0 = (uint64_t)(blk - (lv.bo[s_seg] - lv.base)) * MS_ROWS;
-    bool live[2];
-    int kk[2];
-    float delta[2];
-    uint32_t slot[2];
-#pragma unroll
-    for (int p = 0; p < 2; ++p) {
-      const int row = sp + p * HS;
-      const uint64_t s = s0 + row;
-      const uint32_t j = (uint32_t)(s / (uint32_t)a.K);
-      kk[p] = (int)(s % (uint32_t)a.K);
-      live[p] = j < count;
-      MsInterval iv;
-      iv.t_in = 0.f; iv.delta = 0.f; iv.slot = 0; iv.dx = 0.f; iv.dy = 0.f; iv.dz = 1.f; iv.ray = 0; iv.prim = prim;
-      if (live[p]) iv = a.intervals[first + j];
-      delta[p] = iv.delta; slot[p] = (uint32_t)iv.slot;
+    const uint64_t s = (uint64_t)(blk - (lv.bo[s_seg] - lv.base)) * MS_ROWS + srow_in;
+    const uint32_t j = (uint32_t)(s / (uint32_t)a.K);
+    const int k = (int)(s % (uint32_t)a.K);
+    const bool live = j < count;
+    MsInterval iv;
+    iv.t_in = 0.f; iv.delta = 0.f; iv.slot = 0; iv.dx = 0.f; iv.dy = 0.f; iv.dz = 1.f; iv.ray = 0; iv.prim = prim;
+    if (live) iv = a.intervals[first + j];
+    const size_t out = (size_t)((uint32_t)iv.slot - lv.band.slot0) * (size_t)a.K + (size_t)k;
+    {                                 // Eq.5 into this sample's column of X0^T: frequency l by helper l mod NCG
       const float d[3] = {iv.dx, iv.dy, iv.dz};
-      const float t = ms_sample_tm(iv.t_in, iv.delta, kk[p], false);
+      const float t = ms_sample_tm(iv.t_in, iv.delta, k, false);
       float u[3];
       ms_sample_u(a.A + 9 * (size_t)prim, a.center + 3 * (size_t)prim, a.cam.o, d, t, u);
-      float *x = X0 + (size_t)row * ld0;                  // Eq.5: frequency l by column group l mod CG
+      float *x = X0T + srow_in;
       if (cg == 0) {
-        x[0] = u[0]; x[1] = u[1]; x[2] = u[2];
-        if (sh.use_viewdir) { float *v = x + 3 + 6 * sh.n_freq; v[0] = d[0]; v[1] = d[1]; v[2] = d[2]; }
-        if (a.staging_gate && live[p])
-          a.staging_gate[(size_t)(slot[p] - lv.band.slot0) * (size_t)a.K + (size_t)kk[p]] = ms_slot_gates(u);
+        x[0] = u[0]; x[LS] = u[1]; x[2 * LS] = u[2];
+        if (sh.use_viewdir) { float *v = x + (size_t)(3 + 6 * sh.n_freq) * LS; v[0] = d[0]; v[LS] = d[1]; v[2 * LS] = d[2]; }
+        if (a.staging_gate && live) a.staging_gate[out] = ms_slot_gates(u);
       }
-      for (int l = cg; l < sh.n_freq; l += CG) {
+      for (int l = cg; l < sh.n_freq; l += NCG) {
         const float scale = (float)(1 << l);
         float sv[3], cv[3];
 #pragma unroll
         for (int c = 0; c < 3; ++c) sincospif(scale * u[c], &sv[c], &cv[c]);  // 2^l u is exact
-        float *y = x + 3 + 6 * l;
-        y[0] = sv[0]; y[1] = sv[1]; y[2] = sv[2];
-        y[3] = cv[0]; y[4] = cv[1]; y[5] = cv[2];
+        float *y = x + (size_t)(3 + 6 * l) * LS;
+        y[0] = sv[0]; y[LS] = sv[1]; y[2 * LS] = sv[2];
+        y[3 * LS] = cv[0]; y[4 * LS] = cv[1]; y[5 * LS] = cv[2];
       }
     }
-    __syncthreads();
-    const float *src = X0;
+    const float *src = X0T;
     float *dst = HA;
-    int ldx = ld0, n_in = sh.in_dim;
+    int n_in = sh.in_dim;
     const float *w = wp;
     for (int l = 0; l < sh.n_hidden; ++l) {
-      const float *x0 = src + (size_t)sp * ldx, *x1 = x0 + (size_t)HS * ldx;
-      const float *wc = w + cg * WQ;
-      float acc[2][WQ];
-#pragma unroll
-      for (int q = 0; q < WQ / 4; ++q) {
-        const float4 v = ldg4(wc + n_in * WD + 4 * q);
-        acc[0][4 * q] = acc[1][4 * q] = v.x; acc[0][4 * q + 1] = acc[1][4 * q + 1] = v.y;
-        acc[0][4 * q + 2] = acc[1][4 * q + 2] = v.z; acc[0][4 * q + 3] = acc[1][4 * q + 3] = v.w;
-      }
-      int i = 0;
-      for (; i + 4 <= n_in; i += 4) {
-        const float4 a4 = lds4(x0 + i), b4 = lds4(x1 + i);
-        const float xa[4] = {a4.x, a4.y, a4.z, a4.w}, xb[4] = {b4.x, b4.y, b4.z, b4.w};
-#pragma unroll
-        for (int ii = 0; ii < 4; ++ii) {
-          const float *wr = wc + (i + ii) * WD;
-#pragma unroll
-          for (int q = 0; q < WQ / 4; ++q) {
-            const float4 v = ldg4(wr + 4 * q);
-            acc[0][4 * q] = fmaf(xa[ii], v.x, acc[0][4 * q]); acc[0][4 * q + 1] = fmaf(xa[ii], v.y, acc[0][4 * q + 1]);
-            acc[0][4 * q + 2] = fmaf(xa[ii], v.z, acc[0][4 * q + 2]); acc[0][4 * q + 3] = fmaf(xa[ii], v.w, acc[0][4 * q + 3]);
-            acc[1][4 * q] = fmaf(xb[ii], v.x, acc[1][4 * q]); acc[1][4 * q + 1] = fmaf(xb[ii], v.y, acc[1][4 * q + 1]);
-            acc[1][4 * q + 2] = fmaf(xb[ii], v.z, acc[1][4 * q + 2]); acc[1][4 * q + 3] = fmaf(xb[ii], v.w, acc[1][4 * q + 3]);
-          }
-        }
-      }
-      for (; i < n_in; ++i) {
-        const float xa = x0[i], xb = x1[i];
-        const float *wr = wc + i * WD;
-#pragma unroll
-        for (int q = 0; q < WQ / 4; ++q) {
-          const float4 v = ldg4(wr + 4 * q);
-          acc[0][4 * q] = fmaf(xa, v.x, acc[0][4 * q]); acc[0][4 * q + 1] = fmaf(xa, v.y, acc[0][4 * q + 1]);
-          acc[0][4 * q + 2] = fmaf(xa, v.z, acc[0][4 * q + 2]); acc[0][4 * q + 3] = fmaf(xa, v.w, acc[0][4 * q + 3]);
-          acc[1][4 * q] = fmaf(xb, v.x, acc[1][4 * q]); acc[1][4 * q + 1] = fmaf(xb, v.y, acc[1][4 * q + 1]);
-          acc[1][4 * q + 2] = fmaf(xb, v.z, acc[1][4 * q + 2]); acc[1][4 * q + 3] = fmaf(xb, v.w, acc[1][4 * q + 3]);
-        }
-      }
-#pragma unroll
-      for (int p = 0; p < 2; ++p) {
-        float *y = dst + (size_t)(sp + p * HS) * ldw + cg * WQ;
-#pragma unroll
-        for (int q = 0; q < WQ / 4; ++q)
-          *reinterpret_cast<float4 *>(y + 4 * q) = make_float4(fmaxf(acc[p][4 * q], 0.0f), fmaxf(acc[p][4 * q + 1], 0.0f),
-                                                               fmaxf(acc[p][4 * q + 2], 0.0f), fmaxf(acc[p][4 * q + 3], 0.0f));
-      }
-      __syncthreads();
+      tg_fwd<BS>(src, n_in, w, WD, WD, true, dst, WS, LS, LW);
       w += n_in * WD + WD;
-      n_in = WD; ldx = ldw;
+      n_in = WD;
       src = dst; dst = dst == HA ? HB : HA;
     }
-    // head: output o by column group o mod CG, raw values into the free buffer
-    {
-      const int n_out = sh.out_dim;
-      const float *x0 = src + (size_t)sp * ldw, *x1 = x0 + (size_t)HS * ldw;
-      const float *bh = w + WD * n_out;
-      for (int o = cg; o < n_out; o += CG) {
-        float r0 = __ldg(bh + o), r1 = r0;
-#pragma unroll 4
-        for (int i = 0; i < WD; i += 4) {
-          const float4 a4 = lds4(x0 + i), b4 = lds4(x1 + i);
-          const float w0 = __ldg(w + i * n_out + o), w1 = __ldg(w + (i + 1) * n_out + o);
-          const float w2 = __ldg(w + (i + 2) * n_out + o), w3 = __ldg(w + (i + 3) * n_out + o);
-          r0 = fmaf(a4.x, w0, r0); r0 = fmaf(a4.y, w1, r0); r0 = fmaf(a4.z, w2, r0); r0 = fmaf(a4.w, w3, r0);
-          r1 = fmaf(b4.x, w0, r1); r1 = fmaf(b4.y, w1, r1); r1 = fmaf(b4.z, w2, r1); r1 = fmaf(b4.w, w3, r1);
-        }
-        dst[(size_t)sp * ldw + o] = r0;
-        dst[(size_t)(sp + HS) * ldw + o] = r1;
+    const int n_out = sh.out_dim, n_out4 = n_out & ~3;
+    if (n_out4) tg_fwd<BS>(src, WD, w, n_out, n_out4, false, dst, WS, LS, LW);
+    if (n_out4 < n_out) {             // outputs past the last group of four: one thread per (sample, output)
+      const float *x = src + srow_in;
+      for (int o = n_out4 + cg; o < n_out; o += NCG) {
+        float acc = __ldg(w + WD * n_out + o);
+        for (int i = 0; i < WD; ++i) acc = fmaf(x[(size_t)i * LS], __ldg(w + i * n_out + o), acc);
+        dst[(size_t)o * LS + srow_in] = acc;
       }
+      __syncthreads();
     }
-    __syncthreads();
-    if (cg == 0) {
-#pragma unroll
-      for (int p = 0; p < 2; ++p) {
-        if (!live[p]) continue;
-        const float *raw = dst + (size_t)(sp + p * HS) * ldw;
-        float4 r;
-        r.x = 1.0f / (1.0f + expf(-raw[0]));
-        r.y = 1.0f / (1.0f + expf(-raw[1]));
-        r.z = 1.0f / (1.0f + expf(-raw[2]));
-        const float sigma = fmaxf(raw[3], 0.0f) + log1pf(expf(-fabsf(raw[3])));
-        r.w = expf(-sigma * delta[p]);  // e = 1 - alpha
-        const size_t out = (size_t)(slot[p] - lv.band.slot0) * (size_t)a.K + (size_t)kk[p];
-        a.staging[out] = r;
-        if (a.staging_feat)
-          for (int c = 0; c < sh.n_feat; ++c) reinterpret_cast<float *>(a.staging_feat)[out * sh.n_feat + c] = raw[4 + c];
-      }
+    if (cg == 0 && live) {
+      const float *raw = dst + srow_in;
+      float4 r;
+      r.x = 1.0f / (1.0f + expf(-raw[0]));
+      r.y = 1.0f / (1.0f + expf(-raw[LS]));
+      r.z = 1.0f / (1.0f + expf(-raw[2 * LS]));
+      const float r3 = raw[3 * LS];
+      const float sigma = fmaxf(r3, 0.0f) + log1pf(expf(-fabsf(r3)));
+      r.w = expf(-sigma * iv.delta);  // e = 1 - alpha
+      a.staging[out] = r;
     }
+    if (a.staging_feat && live)       // feature channel c by helper c mod NCG
+      for (int c = cg; c < sh.n_feat; c += NCG)
+        reinterpret_cast<float *>(a.staging_feat)[out * sh.n_feat + c] = dst[(size_t)(4 + c) * LS + srow_in];
   }
 }
 
@@ -512,17 +457,14 @@ cudaError_t ms_mlp_f32(const MsMlpArgs &a, cudaStream_t s) {
   void (*fn)(MsMlpArgs) = mlp_f32_kernel;
   int threads = MS_ROWS;
   const int wd = a.shape.width;
-  const size_t smem_wide = (size_t)MS_ROWS * (ld4_of(a.shape.in_dim) + 2 * ld4_of(wd)) * sizeof(float);
+  const size_t smem_tile = wide_layout(a.shape).floats * sizeof(float);
   if (wd == 32 && a.shape.params % 4 == 0 && a.shape.n_hidden >= 1 && a.shape.n_hidden <= 3) {
     fn = a.shape.n_hidden == 1 ? mlp_f32_w32_kernel<1, 2> : (a.shape.n_hidden == 2 ? mlp_f32_w32_kernel<2, 2> : mlp_f32_w32_kernel<3, 2>);
     threads = MS_ROWS / 2;
-  } else if ((wd == 16 || wd == 32 || wd == 64 || wd == 128) && a.shape.mode == MS_MODE_LOCAL && a.shape.params % 4 == 0 &&
-             a.shape.out_dim <= wd && a.shape.n_hidden >= 1 && smem_wide <= 200 * 1024) {
-    const int cg = wd == 128 ? 8 : 4;
-    fn = wd == 16 ? mlp_f32_wide_kernel<16, 4> : wd == 32 ? mlp_f32_wide_kernel<32, 4>
-       : wd == 64 ? mlp_f32_wide_kernel<64, 4> : mlp_f32_wide_kernel<128, 8>;
-    threads = MS_ROWS * cg / 2;
-    smem = smem_wide;
+  } else if (wd % 4 == 0 && wd >= 8 && a.shape.mode == MS_MODE_LOCAL && a.shape.n_hidden >= 1 && smem_tile <= 226 * 1024) {
+    fn = mlp_f32_tile_kernel;
+    threads = TG_NT;
+    smem = smem_tile;
   }
   cudaError_t e = cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
