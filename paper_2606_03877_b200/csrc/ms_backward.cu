@@ -359,11 +359,9 @@ __global__ void __launch_bounds__(TNT, 1) mlp_bwd_t_kernel(MsMlpBwdArgs a) {
   auto gemm_dw = [&](const float *XT, int n_in, const float *G, int n_out, bool head, float *gw, int ldw, int l) {
     const int n_iw = (n_in + 31) >> 5, n_ow = head ? 1 : (n_out + 15) >> 4;
     const int n_wt = n_iw * n_ow;
-    int SS = 1;
-    while (2 * SS * n_wt <= TNW && BS / (2 * SS) >= (head ? 16 : 4)) SS *= 2;
     const int it = lane & 7, ot = lane >> 3;
-    for (int item = warp; item < n_wt * SS; item += TNW) {
-      const int wt = item / SS, part = item - wt * SS;
+    // one (warp tile, sample part) item: acc[q][p] = sum_s X^T[i_q][s] gZ^T[o_p][s], bsum[p] = sum_s gZ^T[o_p][s]
+    auto item_sums = [&](int wt, int part, int SS, float (&acc)[4][4], float (&bsum)[4]) {
       const int iw = wt / n_ow, ow = wt - iw * n_ow;
       int s_n = BS / SS, s_lo = part * s_n;
       if (head) { s_n >>= 2; s_lo += ot * s_n; }
@@ -371,11 +369,12 @@ __global__ void __launch_bounds__(TNT, 1) mlp_bwd_t_kernel(MsMlpBwdArgs a) {
       const float *gr = G + (size_t)(head ? 0 : 16 * ow + ot) * LS + s_lo;
       const int gstep = head ? LS : 4 * LS;
       const bool do_bias = iw == 0;                        // warp-uniform
-      float acc[4][4], bsum[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-      for (int q = 0; q < 4; ++q)
+      for (int q = 0; q < 4; ++q) {
+        bsum[q] = 0.0f;
 #pragma unroll
         for (int p = 0; p < 4; ++p) acc[q][p] = 0.0f;
+      }
       for (int s0 = 0; s0 < s_n; s0 += 4) {
         float4 x[4], g4[4];
 #pragma unroll
@@ -397,18 +396,63 @@ __global__ void __launch_bounds__(TNT, 1) mlp_bwd_t_kernel(MsMlpBwdArgs a) {
           for (int p = 0; p < 4; ++p) bsum[p] += (g4[p].x + g4[p].y) + (g4[p].z + g4[p].w);
         }
       }
-      if (ACC) {                    // into the primitive's accumulators: slot (warp tile, element, lane)
-        float *slot = DWS + L.acc_w[l] + wt * 512 + lane;
+    };
+    // bias slot of output o_p of this lane (the head's four lane rows are sample parts: a slot each)
+    auto bias_slot = [&](int ow, int p) { return head ? 4 * p + ot : 16 * ow + 4 * p + ot; };
+    float acc[4][4], bsum[4];
+    if (ACC) {
+      // into the primitive's accumulators, slot (warp tile, element, lane): every slot has ONE owner -- with two
+      // sample parts per tile the odd part hands its sums over through the idle weight panel
+      float *const BSC = sm + L.off_hd;                    // rows 0..3 (the head's raw outputs, consumed): bias hand-over
+      const bool two = 2 * n_wt <= TNW && BS / 2 >= (head ? 16 : 4) && n_wt * 512 <= TKP * LW;
+      if (!two) {
+        for (int wt = warp; wt < n_wt; wt += TNW) {
+          item_sums(wt, 0, 1, acc, bsum);
+          float *slot = DWS + L.acc_w[l] + wt * 512 + lane;
 #pragma unroll
-        for (int q = 0; q < 4; ++q)
+          for (int q = 0; q < 4; ++q)
 #pragma unroll
-          for (int p = 0; p < 4; ++p) atomicAdd(slot + (q * 4 + p) * 32, acc[q][p]);
-        if (do_bias && it == 0) {
+            for (int p = 0; p < 4; ++p) slot[(q * 4 + p) * 32] += acc[q][p];
+          if (wt < n_ow && it == 0) {
 #pragma unroll
-          for (int p = 0; p < 4; ++p) atomicAdd(DWS + L.acc_b[l] + (head ? p : 16 * ow + 4 * p + ot), bsum[p]);
+            for (int p = 0; p < 4; ++p) DWS[L.acc_b[l] + bias_slot(wt, p)] += bsum[p];
+          }
         }
-        continue;
+      } else {
+        const int wt = warp >> 1, part = warp & 1;
+        const bool active = wt < n_wt;
+        if (active) item_sums(wt, part, 2, acc, bsum);
+        if (active && part == 1) {
+#pragma unroll
+          for (int q = 0; q < 4; ++q)
+#pragma unroll
+            for (int p = 0; p < 4; ++p) WS[wt * 512 + (q * 4 + p) * 32 + lane] = acc[q][p];
+          if (wt < n_ow && it == 0) {
+#pragma unroll
+            for (int p = 0; p < 4; ++p) BSC[bias_slot(wt, p)] = bsum[p];
+          }
+        }
+        __syncthreads();
+        if (active && part == 0) {
+          float *slot = DWS + L.acc_w[l] + wt * 512 + lane;
+#pragma unroll
+          for (int q = 0; q < 4; ++q)
+#pragma unroll
+            for (int p = 0; p < 4; ++p) slot[(q * 4 + p) * 32] += acc[q][p] + WS[wt * 512 + (q * 4 + p) * 32 + lane];
+          if (wt < n_ow && it == 0) {
+#pragma unroll
+            for (int p = 0; p < 4; ++p) DWS[L.acc_b[l] + bias_slot(wt, p)] += bsum[p] + BSC[bias_slot(wt, p)];
+          }
+        }
       }
+      return;
+    }
+    int SS = 1;
+    while (2 * SS * n_wt <= TNW && BS / (2 * SS) >= (head ? 16 : 4)) SS *= 2;
+    for (int item = warp; item < n_wt * SS; item += TNW) {
+      const int wt = item / SS, part = item - wt * SS;
+      const int iw = wt / n_ow, ow = wt - iw * n_ow;
+      item_sums(wt, part, SS, acc, bsum);
 #pragma unroll
       for (int q = 0; q < 4; ++q) {
         const int i = 32 * iw + 8 * q + it;
@@ -419,7 +463,7 @@ __global__ void __launch_bounds__(TNT, 1) mlp_bwd_t_kernel(MsMlpBwdArgs a) {
           if (o < n_out && acc[q][p] != 0.0f) atomicAdd(gw + (size_t)i * ldw + o, acc[q][p]);
         }
       }
-      if (do_bias && it == 0) {
+      if (iw == 0 && it == 0) {
 #pragma unroll
         for (int p = 0; p < 4; ++p) {
           const int o = head ? p : 16 * ow + 4 * p + ot;
@@ -449,8 +493,15 @@ __global__ void __launch_bounds__(TNT, 1) mlp_bwd_t_kernel(MsMlpBwdArgs a) {
         if (i < n_in && o < n_out) atomicAdd(gw + (size_t)i * ldw + o, v);
       }
       for (int o = tid; o < n_out; o += TNT) {
-        const float v = DWS[L.acc_b[l] + o];
-        DWS[L.acc_b[l] + o] = 0.0f;
+        float v;
+        if (head) {                   // a slot per sample part
+          float *b = DWS + L.acc_b[l] + 4 * o;
+          v = (b[0] + b[1]) + (b[2] + b[3]);
+          b[0] = b[1] = b[2] = b[3] = 0.0f;
+        } else {
+          v = DWS[L.acc_b[l] + o];
+          DWS[L.acc_b[l] + o] = 0.0f;
+        }
         if (v != 0.0f) atomicAdd(gw + (size_t)n_in * ldw + o, v);
       }
     }
