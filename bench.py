@@ -354,6 +354,19 @@ def measure_backward(api, cfg, args, stream, barrier, steps=5, warmup=3):
                          "peak_kind": "fp32 FMA, 148 SMs x 128 lanes x 2 x 1.965 GHz (derived)"}}
 
 
+def run_backward_only(args, cfg):
+    import torch
+    from paper_2606_03877_b200 import api
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the backward pass has no CPU fallback")
+    torch.cuda.set_device(0)
+    stream = torch.cuda.Stream()
+    out = measure_backward(api, cfg, args, stream, torch.cuda.synchronize, steps=max(1, min(args.steps, 5)),
+                           warmup=max(1, min(args.warmup, 3)))
+    out["config"] = args.config
+    print(json.dumps(out))
+
+
 def run_ours(args, cfg):
     import torch
     from paper_2606_03877_b200 import api
@@ -399,7 +412,7 @@ def run_ours(args, cfg):
             others[name]["frame_roofline_frac"] = o["frame_roofline"]["frac"]
     backward = {}
     if rank == 0 and world == 1 and args.all_configs:
-        for name in ("cfg1", "cfg3"):
+        for name in ("cfg1", "cfg2", "cfg3"):
             backward[name] = measure_backward(api, synth.CONFIGS[name], args, stream, barrier)
     if rank != 0:
         msdist.shutdown()
@@ -472,7 +485,13 @@ def main():
     ap.add_argument("--sync", action="store_true",
                     help="render without MS_FLAG_NO_SYNC (every view reads its counts back to size its scratch)")
     ap.add_argument("--waves", type=int, default=0, help="depth waves (ms_opts.waves): 0 = auto, -1 = off, C > 0 = wave size")
+    ap.add_argument("--backward-only", action="store_true",
+                    help="time ms_backward (forward + backward of one view, fp32) on --config alone and print its "
+                         "object as one JSON line: the command behind profiles/r2d_backward.md")
     args = ap.parse_args()
+    if args.backward_only:
+        run_backward_only(args, synth.CONFIGS[args.config])
+        return
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                                  # timing rule: W >= 3
     cfg = synth.CONFIGS[args.config]

@@ -595,35 +595,51 @@ __global__ void __launch_bounds__(TNT, 1) mlp_bwd_t_kernel(MsMlpBwdArgs a) {
       gemm_dx(G, n_out, wp + off_w[l], ldw, n_in_l[l], l > 0 ? XT : nullptr, l > 0 ? XT : sm + L.off_g0);
     }
     __syncthreads();
-    if (live && cg == 0) {
-      const float *gx = sm + L.off_g0 + srow_in;
-      float gu[3] = {gx[0], gx[LS], gx[2 * LS]};
-      float scale = 3.14159265358979323846f;
-      for (int l = 0; l < sh.n_freq; ++l) {
+    if (cg == 0) {                    // warps 0 .. BS / 32 - 1, whole
+      float o8[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+      if (live) {
+        const float *gx = sm + L.off_g0 + srow_in;
+        float gu[3] = {gx[0], gx[LS], gx[2 * LS]};
+        float scale = 3.14159265358979323846f;
+        for (int l = 0; l < sh.n_freq; ++l) {
 #pragma unroll
-        for (int c = 0; c < 3; ++c) {
-          const size_t is = (size_t)(3 + 6 * l + c) * LS, ic = (size_t)(3 + 6 * l + 3 + c) * LS;
-          gu[c] += scale * (X0[ic] * gx[is] - X0[is] * gx[ic]);
+          for (int c = 0; c < 3; ++c) {
+            const size_t is = (size_t)(3 + 6 * l + c) * LS, ic = (size_t)(3 + 6 * l + 3 + c) * LS;
+            gu[c] += scale * (X0[ic] * gx[is] - X0[is] * gx[ic]);
+          }
+          scale *= 2.0f;
         }
-        scale *= 2.0f;
-      }
-      float dp[3];
+        float dp[3];
 #pragma unroll
-      for (int rr = 0; rr < 3; ++rr) dp[rr] = Ap[3 * rr] * d[0] + Ap[3 * rr + 1] * d[1] + Ap[3 * rr + 2] * d[2];
-      const float gt = gu[0] * dp[0] + gu[1] * dp[1] + gu[2] * dp[2];
-      float *ig = a.ivgrad + (size_t)(first + j) * 8;
-      atomicAdd(ig + 0, gu[0]); atomicAdd(ig + 1, gu[1]); atomicAdd(ig + 2, gu[2]);
-      atomicAdd(ig + 3, t * gu[0]); atomicAdd(ig + 4, t * gu[1]); atomicAdd(ig + 5, t * gu[2]);
-      atomicAdd(ig + 6, gt);
-      atomicAdd(ig + 7, ((float)k + 0.5f) * gt + g_delta);
+        for (int rr = 0; rr < 3; ++rr) dp[rr] = Ap[3 * rr] * d[0] + Ap[3 * rr + 1] * d[1] + Ap[3 * rr + 2] * d[2];
+        const float gt = gu[0] * dp[0] + gu[1] * dp[1] + gu[2] * dp[2];
+        o8[0] = gu[0]; o8[1] = gu[1]; o8[2] = gu[2];
+        o8[3] = t * gu[0]; o8[4] = t * gu[1]; o8[5] = t * gu[2];
+        o8[6] = gt; o8[7] = ((float)k + 0.5f) * gt + g_delta;
+      }
+      // the K samples of an interval sit in K neighbouring lanes when K is a power of two up to 32 (row blocks start
+      // at multiples of 128): summed by shuffles, one lane adds
+      const int K = a.K;
+      const bool grouped = K <= 32 && (K & (K - 1)) == 0;
+      if (grouped) {
+#pragma unroll
+        for (int e = 0; e < 8; ++e)
+          for (int o = K >> 1; o > 0; o >>= 1) o8[e] += __shfl_xor_sync(0xffffffffu, o8[e], o);
+      }
+      if (live && (!grouped || k == 0)) {
+        float *ig = a.ivgrad + (size_t)(first + j) * 8;
+#pragma unroll
+        for (int e = 0; e < 8; ++e) atomicAdd(ig + e, o8[e]);
+      }
     }
   }
   if (ACC && acc_prim >= 0) flush_acc(acc_prim);
 }
 
 __global__ void interval_bwd_kernel(MsMlpBwdArgs a) {
-  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= a.n_hits) return;
+  const size_t i0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const bool valid = i0 < a.n_hits;
+  const size_t i = valid ? i0 : a.n_hits - 1;             // a lane past the end repeats the last interval and adds zeros
   const MsInterval iv = a.intervals[i];
   const int prim = iv.prim;
   const float *A = a.A + 9 * (size_t)prim, *mu = a.center + 3 * (size_t)prim;
@@ -655,14 +671,37 @@ __global__ void interval_bwd_kernel(MsMlpBwdArgs a) {
     gop[r] = ig[r] + dp[r] * gb + 2.0f * op[r] * gc;
     gdp[r] = ig[3 + r] + 2.0f * dp[r] * ga + op[r] * gb;
   }
-  float *gA = a.gA + 9 * (size_t)prim;
+  // 12 sums per primitive: the intervals of a primitive are contiguous, so a warp mostly holds ONE primitive -- its
+  // lanes are summed by shuffles and one lane adds; a warp that straddles primitives adds lane by lane
+  float out[12];
 #pragma unroll
   for (int r = 0; r < 3; ++r)
 #pragma unroll
-    for (int c = 0; c < 3; ++c) atomicAdd(gA + 3 * r + c, gop[r] * v[c] + gdp[r] * d[c]);
+    for (int c = 0; c < 3; ++c) out[3 * r + c] = valid ? gop[r] * v[c] + gdp[r] * d[c] : 0.0f;
 #pragma unroll
-  for (int c = 0; c < 3; ++c)
-    atomicAdd(a.g_center + 3 * (size_t)prim + c, -(A[c] * gop[0] + A[3 + c] * gop[1] + A[6 + c] * gop[2]));
+  for (int c = 0; c < 3; ++c) out[9 + c] = valid ? -(A[c] * gop[0] + A[3 + c] * gop[1] + A[6 + c] * gop[2]) : 0.0f;
+  float *gA = a.gA + 9 * (size_t)prim, *gc3 = a.g_center + 3 * (size_t)prim;
+  const bool uniform = __all_sync(0xffffffffu, prim == __shfl_sync(0xffffffffu, prim, 0));
+  if (uniform) {
+#pragma unroll
+    for (int e = 0; e < 12; ++e) {
+      float x = out[e];
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+      out[e] = x;
+    }
+    if ((threadIdx.x & 31) == 0) {
+#pragma unroll
+      for (int e = 0; e < 9; ++e) atomicAdd(gA + e, out[e]);
+#pragma unroll
+      for (int c = 0; c < 3; ++c) atomicAdd(gc3 + c, out[9 + c]);
+    }
+  } else if (valid) {
+#pragma unroll
+    for (int e = 0; e < 9; ++e) atomicAdd(gA + e, out[e]);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) atomicAdd(gc3 + c, out[9 + c]);
+  }
 }
 
 __global__ void prim_bwd_kernel(MsMlpBwdArgs a) {
