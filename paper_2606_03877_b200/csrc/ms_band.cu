@@ -17,6 +17,7 @@
 // the later hits hold (the factor 2 covers fp32 rounding in the final compositing order), so its later intervals
 // are dropped before they are encoded.  The image is bitwise the one without waves.
 #include "ms_internal.cuh"
+#include "ms_cta_scan.cuh"
 
 namespace {
 
@@ -44,10 +45,7 @@ __global__ void tile_stats_kernel(MsGrid g, const uint32_t *__restrict__ ray_off
 }
 
 // ---- single band, single wave: segments = primitives, pairs in stage (a)'s emission order ----------------------
-__global__ void pair_single_kernel(MsBandArgs a) {
-  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const size_t P = a.P_dev ? (*a.P_dev < a.P ? (size_t)*a.P_dev : a.P) : a.P;
-  if (i >= P) return;
+__device__ __forceinline__ void pair_single_body(const MsBandArgs &a, size_t i) {
   const uint64_t key = a.keys[i];
   const int prim = (int)(key & ((1ull << a.prim_bits) - 1ull));
   const int tile = (int)(key >> (32 + a.prim_bits));
@@ -58,9 +56,13 @@ __global__ void pair_single_kernel(MsBandArgs a) {
   a.pair_hits_j[emit] = a.pair_hits_i[i];
 }
 
-__global__ void seg_single_kernel(MsBandArgs a) {
-  const int p = blockIdx.x * blockDim.x + threadIdx.x;
-  if (p > a.n_prims) return;
+__global__ void pair_single_kernel(MsBandArgs a) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const size_t P = a.P_dev ? (*a.P_dev < a.P ? (size_t)*a.P_dev : a.P) : a.P;
+  if (i < P) pair_single_body(a, i);
+}
+
+__device__ __forceinline__ void seg_single_body(const MsBandArgs &a, int p) {
   const uint32_t cap = (uint32_t)a.P;       // no-sync renders: emit offsets beyond the capacity (an overflowed view)
   const uint32_t s = a.pair_off[a.emit_off[p] < cap ? a.emit_off[p] : cap];
   a.grp_iv0[p] = s;
@@ -70,7 +72,12 @@ __global__ void seg_single_kernel(MsBandArgs a) {
   }
 }
 
-__global__ void tables_single_kernel(MsBandArgs a) {
+__global__ void seg_single_kernel(MsBandArgs a) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p <= a.n_prims) seg_single_body(a, p);
+}
+
+__device__ __forceinline__ void tables_single_body(const MsBandArgs &a) {
   const uint32_t T2 = (uint32_t)(a.grid.tile * a.grid.tile);
   // a no-sync render whose pairs or hits overflowed the scratch evaluates nothing (the view is reported invalid)
   a.bw[0] = make_uint2(0u, a.counters[MS_CNT_OVERFLOW] ? 0u : (uint32_t)a.n_prims);
@@ -80,6 +87,25 @@ __global__ void tables_single_kernel(MsBandArgs a) {
   a.bands[0] = b;
   a.counters[MS_CNT_SEGS] = (uint32_t)a.n_prims;
   a.counters[MS_CNT_BLOCKS] = a.blk_off[a.n_prims];
+}
+
+__global__ void tables_single_kernel(MsBandArgs a) { tables_single_body(a); }
+
+// small frames: the five steps of ms_order_single by one CTA, one launch
+constexpr int OS_THREADS = 1024;
+constexpr size_t OS_MAX = 32768;
+__global__ void __launch_bounds__(OS_THREADS) order_single_small_kernel(MsBandArgs a) {
+  __shared__ uint32_t wt[OS_THREADS / 32 + 1];
+  const size_t P = a.P_dev ? (*a.P_dev < a.P ? (size_t)*a.P_dev : a.P) : a.P;
+  for (size_t i = threadIdx.x; i < P; i += OS_THREADS) pair_single_body(a, i);
+  __syncthreads();
+  cta_exclusive_scan_u32<OS_THREADS>(a.pair_hits_j, a.pair_off, a.P, wt);
+  __syncthreads();
+  for (int p = threadIdx.x; p <= a.n_prims; p += OS_THREADS) seg_single_body(a, p);
+  __syncthreads();
+  cta_exclusive_scan_u32<OS_THREADS>(a.grp_blocks, a.blk_off, (size_t)a.n_prims, wt);
+  __syncthreads();
+  if (threadIdx.x == 0) tables_single_body(a);
 }
 
 // ---- bands x waves --------------------------------------------------------------------------------------------
@@ -376,6 +402,11 @@ cudaError_t ms_tile_stats(const MsGrid &g, const uint32_t *ray_off, const uint32
 
 cudaError_t ms_order_single(const MsBandArgs &a, cudaStream_t s) {
   cudaError_t e;
+  if (a.P <= OS_MAX && (size_t)a.n_prims <= OS_MAX) {
+    order_single_small_kernel<<<1, OS_THREADS, 0, s>>>(a);
+    MS_CHECK_LAUNCH();
+    return cudaSuccess;
+  }
   if (a.P > 0) {
     pair_single_kernel<<<grid_for(a.P, 256), 256, 0, s>>>(a);
     MS_CHECK_LAUNCH();

@@ -2,6 +2,7 @@
 // per-primitive / per-pair / per-ray counts into offsets).  HBM-bound, one read + one write
 // per element per level; levels shrink by 2048x.
 #include "ms_internal.cuh"
+#include "ms_cta_scan.cuh"
 
 namespace {
 
@@ -65,6 +66,14 @@ __global__ void __launch_bounds__(SCAN_THREADS) scan_add_kernel(uint32_t *__rest
   if (blockIdx.x == 0 && threadIdx.x == 0) out[n] = sums_scan[n_tiles];
 }
 
+// up to SCAN_ONE_CTA elements: one CTA, one launch (three launches of the tiled form cost more than the loop)
+constexpr int SCAN_ONE_THREADS = 1024;
+constexpr size_t SCAN_ONE_CTA = 4 * (size_t)SCAN_ONE_THREADS * 8;
+__global__ void __launch_bounds__(SCAN_ONE_THREADS) scan_one_cta_kernel(const uint32_t *in, uint32_t *out, size_t n) {
+  __shared__ uint32_t wt[SCAN_ONE_THREADS / 32 + 1];
+  cta_exclusive_scan_u32<SCAN_ONE_THREADS>(in, out, n, wt);
+}
+
 }  // namespace
 
 size_t ms_scan_scratch_elems(size_t n) {
@@ -82,6 +91,11 @@ cudaError_t ms_exclusive_scan_u32(const uint32_t *in, uint32_t *out, size_t n, u
   size_t nb = (n + SCAN_TILE - 1) / SCAN_TILE;
   if (nb == 1) {
     scan_tile_kernel<<<1, SCAN_THREADS, 0, s>>>(in, out, n, nullptr);
+  MS_LAUNCHED();
+    return cudaGetLastError();
+  }
+  if (n <= SCAN_ONE_CTA) {
+    scan_one_cta_kernel<<<1, SCAN_ONE_THREADS, 0, s>>>(in, out, n);
   MS_LAUNCHED();
     return cudaGetLastError();
   }
