@@ -375,7 +375,6 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   const uint32_t *P_dev = nullptr;    // no-sync: where the kernels read the count
   if (nosync) {
     P = P_cap;
-    CK(ms_frame_guard((uint32_t *)sc->emit_off.p + N, (uint32_t)P_cap, counters, st));
     P_dev = counters + MS_CNT_P_EFF;
   } else {
     CK(cudaMemcpyAsync(sc->pinned, (uint32_t *)sc->emit_off.p + N, 4, cudaMemcpyDeviceToHost, st));
@@ -400,7 +399,7 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   if (ms_scan_scratch_elems(P_slack) + 16 > sc->scan_scratch.cap / 4) ENS(sc->scan_scratch, (ms_scan_scratch_elems(P_slack) + 16) * 4);
   CK(ms_emit_keys(N, (uint32_t *)sc->emit_off.p, (int4 *)sc->rect.p, (float *)sc->z_entry.p, grid.tiles_x, prim_bits,
                   (uint64_t *)sc->keys_a.p, tile_order, cam, tile, sc->A, (float *)sc->oprime.p, st,
-                  nosync ? (uint32_t)P_cap : 0xffffffffu));
+                  nosync ? (uint32_t)P_cap : 0xffffffffu, nosync ? counters : nullptr));
 
   // ---- (b) radix sort + tile ranges -------------------------------------------------------
   CK(rec(1));

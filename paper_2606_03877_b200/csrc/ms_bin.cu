@@ -158,9 +158,18 @@ __global__ void project_kernel(int n, const float *__restrict__ center, const fl
 __global__ void emit_keys_kernel(int n, const uint32_t *__restrict__ emit_off, const int4 *__restrict__ rect,
                                  const float *__restrict__ z_entry, int tiles_x, int prim_bits,
                                  uint64_t *__restrict__ keys, int tile_order, MsCam cam, int tile,
-                                 const float *__restrict__ A, const float *__restrict__ oprime, uint32_t cap) {
+                                 const float *__restrict__ A, const float *__restrict__ oprime, uint32_t cap,
+                                 uint32_t *__restrict__ counters) {
   int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   int lane = threadIdx.x & 31;
+  if (counters && blockIdx.x == 0 && threadIdx.x == 0) {   // no-sync views: the pair count the later kernels read, and
+    const uint32_t P = emit_off[n];                        // whether it fits the scratch sized from the previous view
+    counters[MS_CNT_P_EFF] = P < cap ? P : cap;
+    if (P > cap) {
+      counters[MS_CNT_OVERFLOW] = 1u;
+      counters[MS_CNT_STICKY_OVERFLOW] = 1u;               // survives the per-view reset: any view of a batch
+    }
+  }
   if (i >= n) return;
   uint32_t beg = emit_off[i], cnt = emit_off[i + 1] - beg;
   if (cnt == 0) return;
@@ -198,22 +207,7 @@ __global__ void tile_ranges_kernel(const uint64_t *__restrict__ keys, uint32_t n
 }
 
 // ms_render without host synchronisation: the pair count against the capacity the scratch was sized for
-__global__ void frame_guard_kernel(const uint32_t *__restrict__ total, uint32_t cap, uint32_t *__restrict__ counters) {
-  const uint32_t P = *total;
-  counters[MS_CNT_P_EFF] = P < cap ? P : cap;
-  if (P > cap) {
-    counters[MS_CNT_OVERFLOW] = 1u;
-    counters[MS_CNT_STICKY_OVERFLOW] = 1u;       // survives the per-view reset: any view of a batch
-  }
-}
-
 }  // namespace
-
-cudaError_t ms_frame_guard(const uint32_t *total, uint32_t cap, uint32_t *counters, cudaStream_t s) {
-  frame_guard_kernel<<<1, 1, 0, s>>>(total, cap, counters);
-  MS_LAUNCHED();
-  return cudaGetLastError();
-}
 
 cudaError_t ms_prep_prims(int n, const float *center, const float *quat, const float *scale, float *A, float *M,
                           int *bad, cudaStream_t s) {
@@ -234,10 +228,10 @@ cudaError_t ms_project(int n, const float *center, const float *A, const float *
 
 cudaError_t ms_emit_keys(int n, const uint32_t *emit_off, const int4 *rect, const float *z_entry, int tiles_x,
                          int prim_bits, uint64_t *keys, int tile_order, MsCam cam, int tile, const float *A,
-                         const float *oprime, cudaStream_t s, uint32_t cap) {
+                         const float *oprime, cudaStream_t s, uint32_t cap, uint32_t *counters) {
   long threads = (long)n * 32;
   emit_keys_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, s>>>(n, emit_off, rect, z_entry, tiles_x, prim_bits,
-                                                                    keys, tile_order, cam, tile, A, oprime, cap);
+                                                                    keys, tile_order, cam, tile, A, oprime, cap, counters);
   MS_LAUNCHED();
   return cudaGetLastError();
 }

@@ -244,11 +244,11 @@ cudaError_t ms_project(int n, const float *center, const float *A, const float *
 // tile_order != 0: the depth field of the key is t*_{i,c} of the tile-centre ray (needs cam, tile, A, oprime)
 cudaError_t ms_emit_keys(int n, const uint32_t *emit_off, const int4 *rect, const float *z_entry, int tiles_x,
                          int prim_bits, uint64_t *keys, int tile_order, MsCam cam, int tile, const float *A,
-                         const float *oprime, cudaStream_t s, uint32_t cap = 0xffffffffu);
+                         const float *oprime, cudaStream_t s, uint32_t cap = 0xffffffffu,
+                         uint32_t *counters = nullptr);   // counters: no-sync views (pair count + overflow guard)
 cudaError_t ms_tile_ranges(const uint64_t *keys, size_t n_pairs, int n_tiles, int prim_bits, uint32_t *tile_start,
                            cudaStream_t s, const uint32_t *n_dev = nullptr);
 // no-sync renders: counters[MS_CNT_P_EFF] = min(*total, cap); MS_CNT_OVERFLOW if the pairs do not fit
-cudaError_t ms_frame_guard(const uint32_t *total, uint32_t cap, uint32_t *counters, cudaStream_t s);
 
 // ms_isect.cu
 struct MsIsectArgs {
