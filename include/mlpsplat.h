@@ -245,6 +245,25 @@ int ms_debug_sample_order_all(ms_scene *scene, int32_t *prim, int32_t *k, size_t
 /* Derived per-primitive frames, host [n][9] each (row-major A, M). */
 int ms_debug_prim_frames(ms_scene *scene, float *A, float *M);
 
+/* ---- the offset scan of stages (a), (c), (d) as entry points of its own ----
+ * out[i] = sum of in[j], j < i, for i in [0, n]: n + 1 values (out[n] = the total), uint32 with wrap-around.
+ * in: device [n]; out: device [n + 1]; they must not overlap.  Enqueued on `stream` (cudaStream_t; NULL = the legacy
+ * default stream).
+ *
+ * ms_exclusive_scan_device: the path the render uses (ms_scan.cu: one CTA up to 32 768 counts, tiled above); it
+ * allocates its scratch with cudaMalloc, synchronises the stream and frees it.
+ *
+ * ms_exclusive_scan_static: allocates NOTHING (no cudaMalloc / cudaFree, no allocating library call) and does not
+ * synchronise: for callers under CUDA graph capture, in serving loops, or in harnesses that forbid allocation.  The
+ * tile sums live in a file-scope device array of 65 KB that every GPU loading the library holds until exit; it covers
+ * n <= MS_SCAN_STATIC_MAX, beyond that the call returns MS_ERR_CAPACITY and enqueues nothing.  Every call shares the
+ * array (the scan writes each scratch word before reading it, so nothing is cleared between calls): calls that
+ * overlap on the GPU -- different streams, concurrent graph replays -- race on it; serialise them.  The first call on
+ * a device looks up the array's address (cudaGetSymbolAddress): make one call before starting a capture. */
+#define MS_SCAN_STATIC_MAX (1u << 24)
+int ms_exclusive_scan_device(const uint32_t *in, uint32_t *out, size_t n, void *stream);
+int ms_exclusive_scan_static(const uint32_t *in, uint32_t *out, size_t n, void *stream);
+
 /* Kernels the calling host thread has launched through this library so far (a running count; no synchronisation). */
 int64_t ms_launch_count_total(void);
 

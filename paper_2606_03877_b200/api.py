@@ -27,7 +27,8 @@ STAGES = ("bin", "sort", "isect", "mlp", "composite")
 
 EXPORTS = ["ms_scene_create", "ms_scene_set_slots", "ms_scene_destroy", "ms_render", "ms_render_batch", "ms_render_host",
            "ms_backward", "ms_last_stats", "ms_last_stage_ms", "ms_stage_accum", "ms_debug_tile_lists", "ms_debug_intervals",
-           "ms_debug_sample_order", "ms_debug_sample_order_all", "ms_debug_prim_frames", "ms_launch_count_total", "ms_error_string", "ms_last_cuda_error"]
+           "ms_debug_sample_order", "ms_debug_sample_order_all", "ms_debug_prim_frames", "ms_launch_count_total", "ms_error_string", "ms_last_cuda_error",
+           "ms_exclusive_scan_device", "ms_exclusive_scan_static"]
 
 
 class _Prims(C.Structure):
@@ -71,6 +72,8 @@ def _load() -> C.CDLL:
     lib.ms_launch_count_total.restype = C.c_int64
     lib.ms_scene_destroy.argtypes = [C.c_void_p]
     lib.ms_scene_set_slots.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
+    for name in ("ms_exclusive_scan_device", "ms_exclusive_scan_static"):
+        getattr(lib, name).argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
     return lib
 
 
@@ -88,6 +91,30 @@ class MsError(RuntimeError):
         self.cuda = cuda
         msg = _lib.ms_error_string(code).decode()
         super().__init__(f"{where}: {msg} ({code})" + (f", cudaError {cuda}" if cuda else ""))
+
+
+SCAN_STATIC_MAX = 1 << 24   # MS_SCAN_STATIC_MAX: the largest n ms_exclusive_scan_static covers
+
+
+def exclusive_scan(counts: "torch.Tensor", out: "torch.Tensor | None" = None, static: bool = False, stream=None):
+    """out[i] = sum(counts[:i]) for i in [0, n] (uint32 arithmetic on int32 CUDA tensors): the offset scan of stages
+    (a), (c), (d).  static=False: ms_exclusive_scan_device (the render's path; allocates its scratch and synchronises).
+    static=True: ms_exclusive_scan_static -- allocates nothing, scratch in a fixed device array, n <= SCAN_STATIC_MAX,
+    calls must not overlap on the GPU (include/mlpsplat.h).  Argument marshalling only."""
+    if not (counts.is_cuda and counts.dtype == torch.int32 and counts.is_contiguous() and counts.dim() == 1):
+        raise ValueError("counts: contiguous 1-D int32 CUDA tensor")
+    n = counts.numel()
+    if out is None:
+        out = torch.empty(n + 1, dtype=torch.int32, device=counts.device)
+    if not (out.is_cuda and out.dtype == torch.int32 and out.is_contiguous() and out.numel() >= n + 1):
+        raise ValueError("out: contiguous int32 CUDA tensor of n + 1 elements")
+    s = torch.cuda.current_stream(counts.device).cuda_stream if stream is None else stream
+    fn = _lib.ms_exclusive_scan_static if static else _lib.ms_exclusive_scan_device
+    with torch.cuda.device(counts.device):
+        rc = fn(_ptr(counts), _ptr(out), n, C.c_void_p(s))
+    if rc != 0:
+        raise MsError(rc, "ms_exclusive_scan_static" if static else "ms_exclusive_scan_device")
+    return out
 
 
 def _ptr(a):
