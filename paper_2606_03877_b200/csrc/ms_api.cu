@@ -77,6 +77,7 @@ struct ms_scene {
   struct History {            // MS_FLAG_NO_SYNC: the last synchronising view, whose scratch sizes the next ones
     bool valid = false;
     int H = 0, W = 0, tile = 0, K = 0, path = 0, feat = 0, slots = 0, tile_order = 0;
+    size_t pairs = 0;         // its pair count
   } hist;
   bool frame_nosync = false;  // the pending view was rendered without host synchronisation
   bool clear_sticky = false;  // the sticky overflow flag has been seen: clear it before the next view
@@ -313,6 +314,8 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
     while (P_cap > 0 && (ms_sort_scratch_elems(P_cap) * 4 > sc->sort_scratch.cap ||
                          (ms_scan_scratch_elems(P_cap) + 16) * 4 > sc->scan_scratch.cap))
       P_cap = P_cap * 3 / 4;
+    // a key set that fits one CTA's sort with a quarter of slack keeps to that capacity: one launch sorts it
+    if (P_cap > MS_BLOCK_SORT_MAX && sc->hist.pairs + sc->hist.pairs / 4 + 64 <= MS_BLOCK_SORT_MAX) P_cap = MS_BLOCK_SORT_MAX;
     hit_cap = mn(mn(sc->intervals.cap / sizeof(MsInterval), sc->hits.cap / sizeof(MsHit)),
                  sc->staging.cap / (sizeof(float4) * (size_t)K));
     if (want_feat) hit_cap = mn(hit_cap, sc->staging_feat.cap / (feat_bytes * (size_t)K));
@@ -354,7 +357,9 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
     ENS(sc->counters, (MS_CNT_N + 4) * 4);
     CK(cudaMemsetAsync(sc->counters.p, 0, (MS_CNT_N + 4) * 4, st));
   }
-  CK(cudaMemsetAsync(sc->counters.p, 0, MS_CNT_N * 4, st));         // the sticky overflow flag behind them stays
+  // small frames without host synchronisation: stages (a) + (b) are one launch of one CTA, which also resets the counters
+  const bool small_ab = nosync && ms_bin_sort_small_fits(N, P_cap);
+  if (!small_ab) CK(cudaMemsetAsync(sc->counters.p, 0, MS_CNT_N * 4, st));         // the sticky overflow flag behind them stays
   if (sc->clear_sticky) {
     CK(cudaMemsetAsync((uint32_t *)sc->counters.p + MS_CNT_STICKY_OVERFLOW, 0, 4, st));
     sc->clear_sticky = false;
@@ -367,10 +372,12 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   ENS(sc->oprime, (size_t)N * 12);
   ENS(sc->scan_scratch, (ms_scan_scratch_elems(R > (size_t)N ? R : (size_t)N) + 16) * 4);
   const float eye_guard = opts->eye_guard > 0.0f ? opts->eye_guard : MS_EYE_GUARD_DEFAULT;
-  CK(ms_project(N, sc->center, sc->A, sc->M, cam, tile, eye_guard, (uint32_t *)sc->tile_count.p,
-                (int4 *)sc->rect.p, (float *)sc->z_entry.p, (float *)sc->oprime.p, counters, st));
-  CK(ms_exclusive_scan_u32((uint32_t *)sc->tile_count.p, (uint32_t *)sc->emit_off.p, (size_t)N,
-                           (uint32_t *)sc->scan_scratch.p, st));
+  if (!small_ab) {
+    CK(ms_project(N, sc->center, sc->A, sc->M, cam, tile, eye_guard, (uint32_t *)sc->tile_count.p,
+                  (int4 *)sc->rect.p, (float *)sc->z_entry.p, (float *)sc->oprime.p, counters, st));
+    CK(ms_exclusive_scan_u32((uint32_t *)sc->tile_count.p, (uint32_t *)sc->emit_off.p, (size_t)N,
+                             (uint32_t *)sc->scan_scratch.p, st));
+  }
   size_t P = 0;                       // the pair count, or (no-sync) the capacity the launches are sized for
   const uint32_t *P_dev = nullptr;    // no-sync: where the kernels read the count
   if (nosync) {
@@ -397,18 +404,28 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   ENS(sc->pair_off, (P + 2) * 4);
   ENS(sc->slot_of, (P + 1) * 4);
   if (ms_scan_scratch_elems(P_slack) + 16 > sc->scan_scratch.cap / 4) ENS(sc->scan_scratch, (ms_scan_scratch_elems(P_slack) + 16) * 4);
-  CK(ms_emit_keys(N, (uint32_t *)sc->emit_off.p, (int4 *)sc->rect.p, (float *)sc->z_entry.p, grid.tiles_x, prim_bits,
-                  (uint64_t *)sc->keys_a.p, tile_order, cam, tile, sc->A, (float *)sc->oprime.p, st,
-                  nosync ? (uint32_t)P_cap : 0xffffffffu, nosync ? counters : nullptr));
-
-  // ---- (b) radix sort + tile ranges -------------------------------------------------------
-  CK(rec(1));
   uint64_t *sorted = nullptr;
-  // stage (a) emits the keys primitive by primitive, i.e. already ordered by the id in their low prim_bits bits;
-  // the sort is stable, so only the (tile | depth) bits above them need passes
-  CK(ms_radix_sort_u64((uint64_t *)sc->keys_a.p, (uint64_t *)sc->keys_b.p, P, prim_bits, prim_bits + 32 + tile_bits,
-                       (uint32_t *)sc->sort_scratch.p, &sorted, st, P_dev));
-  CK(ms_tile_ranges(sorted, P, n_tiles, prim_bits, (uint32_t *)sc->tile_start.p, st, P_dev));
+  if (small_ab) {
+    CK(ms_bin_sort_small(N, sc->center, sc->A, sc->M, cam, tile, eye_guard, grid.tiles_x, n_tiles, prim_bits, tile_order,
+                         prim_bits + 32 + tile_bits, (uint32_t)P_cap, (uint32_t *)sc->tile_count.p,
+                         (uint32_t *)sc->emit_off.p, (int4 *)sc->rect.p, (float *)sc->z_entry.p, (float *)sc->oprime.p,
+                         counters, (uint64_t *)sc->keys_a.p, (uint64_t *)sc->keys_b.p, (uint32_t *)sc->tile_start.p,
+                         (uint32_t *)sc->pair_hits_j.p, st));
+    sorted = (uint64_t *)sc->keys_b.p;
+    CK(rec(1));                      // stage times: the fused launch counts as stage (a); stage (b) reads 0
+  } else {
+    CK(ms_emit_keys(N, (uint32_t *)sc->emit_off.p, (int4 *)sc->rect.p, (float *)sc->z_entry.p, grid.tiles_x, prim_bits,
+                    (uint64_t *)sc->keys_a.p, tile_order, cam, tile, sc->A, (float *)sc->oprime.p, st,
+                    nosync ? (uint32_t)P_cap : 0xffffffffu, nosync ? counters : nullptr));
+
+    // ---- (b) radix sort + tile ranges -------------------------------------------------------
+    CK(rec(1));
+    // stage (a) emits the keys primitive by primitive, i.e. already ordered by the id in their low prim_bits bits;
+    // the sort is stable, so only the (tile | depth) bits above them need passes
+    CK(ms_radix_sort_u64((uint64_t *)sc->keys_a.p, (uint64_t *)sc->keys_b.p, P, prim_bits, prim_bits + 32 + tile_bits,
+                         (uint32_t *)sc->sort_scratch.p, &sorted, st, P_dev));
+    CK(ms_tile_ranges(sorted, P, n_tiles, prim_bits, (uint32_t *)sc->tile_start.p, st, P_dev));
+  }
 
   // ---- (c) intersection: count, scan, pair order, fill ---------------------------------------
   CK(rec(2));
@@ -426,9 +443,15 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   ia.slot_of = (uint32_t *)sc->slot_of.p; ia.pair_off = (uint32_t *)sc->pair_off.p; ia.ray_off = (uint32_t *)sc->ray_off.p;
   ia.intervals = nullptr; ia.hits = nullptr; ia.guard = nullptr;
   CK(ms_isect_count(ia, st));
-  CK(ms_exclusive_scan_u32((uint32_t *)sc->ray_hits.p, (uint32_t *)sc->ray_off.p, R, (uint32_t *)sc->scan_scratch.p, st));
-  CK(ms_tile_stats(grid, (uint32_t *)sc->ray_off.p, (uint32_t *)sc->tile_start.p, counters, st,
-                   nosync ? (uint32_t)hit_cap : 0u));
+  // small frames without host synchronisation: the CTA that orders the pairs (below) takes the tile statistics along,
+  // and the ray scan too when the frame has few enough rays
+  const bool small_c = nosync && ms_order_single_is_small(P, N);
+  const bool small_c_scan = small_c && R <= MS_SMALL_RAYS;
+  if (!small_c_scan)
+    CK(ms_exclusive_scan_u32((uint32_t *)sc->ray_hits.p, (uint32_t *)sc->ray_off.p, R, (uint32_t *)sc->scan_scratch.p, st));
+  if (!small_c)
+    CK(ms_tile_stats(grid, (uint32_t *)sc->ray_off.p, (uint32_t *)sc->tile_start.p, counters, st,
+                     nosync ? (uint32_t)hit_cap : 0u));
   size_t n_hits = hit_cap, max_tile_hits = 0;     // no-sync: the capacity stands in for the count
   uint32_t max_list = 0;
   if (!nosync) {
@@ -529,7 +552,10 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   ba.grp_key = (uint32_t *)sc->grp_key.p; ba.grp_prim = (uint32_t *)sc->grp_prim.p; ba.grp_iv0 = (uint32_t *)sc->grp_iv0.p;
   ba.grp_blocks = (uint32_t *)sc->grp_blocks.p; ba.blk_off = (uint32_t *)sc->blk_off.p;
   ba.bw = (uint2 *)sc->bw.p; ba.bands = (MsBand *)sc->bands.p; ba.counters = counters;
-  if (nosync) CK(cudaMemsetAsync(sc->pair_hits_j.p, 0, (P + 2) * 4, st));   // slots beyond the device's pair count
+  ba.ray_hits = (uint32_t *)sc->ray_hits.p; ba.ray_off_w = (uint32_t *)sc->ray_off.p; ba.R = R;
+  ba.hit_cap = nosync ? (uint32_t)hit_cap : 0u;
+  ba.fuse_ray_scan = small_c_scan && !banded ? 1 : 0; ba.fuse_stats = small_c && !banded ? 1 : 0;
+  if (nosync && !small_ab) CK(cudaMemsetAsync(sc->pair_hits_j.p, 0, (P + 2) * 4, st));   // slots beyond the device's pair count
   if (banded) CK(ms_order_banded(ba, st));
   else CK(ms_order_single(ba, st));
   // the band table comes back to the host: stage (e) is launched with one CTA per four rays of the band (the
@@ -664,6 +690,7 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
     sc->hist.valid = n_bands == 1 && !banded;
     sc->hist.H = H; sc->hist.W = W; sc->hist.tile = tile; sc->hist.K = K; sc->hist.path = path;
     sc->hist.feat = want_feat ? 1 : 0; sc->hist.slots = want_slots ? 1 : 0; sc->hist.tile_order = tile_order;
+    sc->hist.pairs = P;
   }
   sc->stats.n_bands = n_bands;
   sc->stats.n_waves = n_waves;

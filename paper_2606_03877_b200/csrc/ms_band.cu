@@ -24,9 +24,8 @@ namespace {
 constexpr int WB = 3;   // bits of the wave field (MS_MAX_WAVES <= 8)
 static_assert(MS_MAX_WAVES <= (1 << WB), "wave field");
 
-__global__ void tile_stats_kernel(MsGrid g, const uint32_t *__restrict__ ray_off, const uint32_t *__restrict__ tile_start,
-                                  uint32_t *__restrict__ counters, uint32_t hit_cap) {
-  const int pos = blockIdx.x * blockDim.x + threadIdx.x;
+__device__ __forceinline__ void tile_stats_body(const MsGrid &g, int pos, const uint32_t *ray_off, const uint32_t *tile_start,
+                                                uint32_t *counters, uint32_t hit_cap) {
   const uint32_t T2 = (uint32_t)(g.tile * g.tile);
   if (pos < g.n_tiles) {
     const uint32_t h = ray_off[(size_t)(pos + 1) * T2] - ray_off[(size_t)pos * T2];   // exact even if the scan wrapped
@@ -42,6 +41,11 @@ __global__ void tile_stats_kernel(MsGrid g, const uint32_t *__restrict__ ray_off
     counters[MS_CNT_OVERFLOW] = 1u;
     counters[MS_CNT_STICKY_OVERFLOW] = 1u;       // survives the per-view reset: any view of a batch
   }
+}
+
+__global__ void tile_stats_kernel(MsGrid g, const uint32_t *__restrict__ ray_off, const uint32_t *__restrict__ tile_start,
+                                  uint32_t *__restrict__ counters, uint32_t hit_cap) {
+  tile_stats_body(g, blockIdx.x * blockDim.x + threadIdx.x, ray_off, tile_start, counters, hit_cap);
 }
 
 // ---- single band, single wave: segments = primitives, pairs in stage (a)'s emission order ----------------------
@@ -96,6 +100,16 @@ constexpr int OS_THREADS = 1024;
 constexpr size_t OS_MAX = 32768;
 __global__ void __launch_bounds__(OS_THREADS) order_single_small_kernel(MsBandArgs a) {
   __shared__ uint32_t wt[OS_THREADS / 32 + 1];
+  if (a.fuse_ray_scan) {
+    cta_exclusive_scan_u32<OS_THREADS>(a.ray_hits, a.ray_off_w, a.R, wt);
+    __syncthreads();
+  }
+  if (a.fuse_stats) {
+    const int n = a.grid.n_tiles > 0 ? a.grid.n_tiles : 1;
+    for (int pos = threadIdx.x; pos < n; pos += OS_THREADS)
+      tile_stats_body(a.grid, pos, a.ray_off, a.tile_start, a.counters, a.hit_cap);
+    __syncthreads();
+  }
   const size_t P = a.P_dev ? (*a.P_dev < a.P ? (size_t)*a.P_dev : a.P) : a.P;
   for (size_t i = threadIdx.x; i < P; i += OS_THREADS) pair_single_body(a, i);
   __syncthreads();
@@ -400,9 +414,11 @@ cudaError_t ms_tile_stats(const MsGrid &g, const uint32_t *ray_off, const uint32
   return cudaSuccess;
 }
 
+bool ms_order_single_is_small(size_t P, int n_prims) { return P <= OS_MAX && (size_t)n_prims <= OS_MAX; }
+
 cudaError_t ms_order_single(const MsBandArgs &a, cudaStream_t s) {
   cudaError_t e;
-  if (a.P <= OS_MAX && (size_t)a.n_prims <= OS_MAX) {
+  if (ms_order_single_is_small(a.P, a.n_prims)) {
     order_single_small_kernel<<<1, OS_THREADS, 0, s>>>(a);
     MS_CHECK_LAUNCH();
     return cudaSuccess;

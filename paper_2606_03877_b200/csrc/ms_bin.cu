@@ -4,6 +4,8 @@
 //  P:148 "AABB-tile-frustum intersection test"; NS (a)).  All arithmetic is the canonical
 // fp32 sequence of DESIGN.md Sec.2.  Bytes: N*(3+9+9)*4 in, P*8 out -- negligible.
 #include "ms_internal.cuh"
+#include "ms_block_sort.cuh"
+#include "ms_cta_scan.cuh"
 
 namespace {
 
@@ -68,12 +70,10 @@ __device__ __forceinline__ int clamp_hi(float v, int n) {
   return (int)f;
 }
 
-__global__ void project_kernel(int n, const float *__restrict__ center, const float *__restrict__ A,
-                               const float *__restrict__ M, MsCam cam, int tile, float eye_guard,
-                               uint32_t *__restrict__ tile_count, int4 *__restrict__ rect, float *__restrict__ z_entry,
-                               float *__restrict__ oprime, uint32_t *__restrict__ counters) {
-  int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
+__device__ __forceinline__ void project_body(int i, const float *__restrict__ center, const float *__restrict__ A,
+                                             const float *__restrict__ M, const MsCam &cam, int tile, float eye_guard,
+                                             uint32_t *tile_count, int4 *rect, float *z_entry, float *oprime,
+                                             uint32_t *counters) {
   const float *mu = center + 3 * i;
   const float *Mi = M + 9 * i;
   const float *Ai = A + 9 * i;
@@ -154,23 +154,29 @@ __global__ void project_kernel(int n, const float *__restrict__ center, const fl
   z_entry[i] = ze;
 }
 
-// one warp per primitive; emission order: tile rows, then columns (row-major inside the rect)
-__global__ void emit_keys_kernel(int n, const uint32_t *__restrict__ emit_off, const int4 *__restrict__ rect,
-                                 const float *__restrict__ z_entry, int tiles_x, int prim_bits,
-                                 uint64_t *__restrict__ keys, int tile_order, MsCam cam, int tile,
-                                 const float *__restrict__ A, const float *__restrict__ oprime, uint32_t cap,
-                                 uint32_t *__restrict__ counters) {
-  int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  int lane = threadIdx.x & 31;
-  if (counters && blockIdx.x == 0 && threadIdx.x == 0) {   // no-sync views: the pair count the later kernels read, and
-    const uint32_t P = emit_off[n];                        // whether it fits the scratch sized from the previous view
-    counters[MS_CNT_P_EFF] = P < cap ? P : cap;
-    if (P > cap) {
-      counters[MS_CNT_OVERFLOW] = 1u;
-      counters[MS_CNT_STICKY_OVERFLOW] = 1u;               // survives the per-view reset: any view of a batch
-    }
+__global__ void project_kernel(int n, const float *__restrict__ center, const float *__restrict__ A,
+                               const float *__restrict__ M, MsCam cam, int tile, float eye_guard,
+                               uint32_t *__restrict__ tile_count, int4 *__restrict__ rect, float *__restrict__ z_entry,
+                               float *__restrict__ oprime, uint32_t *__restrict__ counters) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) project_body(i, center, A, M, cam, tile, eye_guard, tile_count, rect, z_entry, oprime, counters);
+}
+
+// no-sync views: the pair count the later kernels read, and whether it fits the scratch sized from the previous view
+__device__ __forceinline__ uint32_t pair_guard(uint32_t P, uint32_t cap, uint32_t *counters) {
+  counters[MS_CNT_P_EFF] = P < cap ? P : cap;
+  if (P > cap) {
+    counters[MS_CNT_OVERFLOW] = 1u;
+    counters[MS_CNT_STICKY_OVERFLOW] = 1u;               // survives the per-view reset: any view of a batch
   }
-  if (i >= n) return;
+  return P < cap ? P : cap;
+}
+
+// one warp per primitive; emission order: tile rows, then columns (row-major inside the rect).  Plain pointers: the
+// fused small-frame kernel reads what it has written itself.
+__device__ __forceinline__ void emit_body(int i, int lane, const uint32_t *emit_off, const int4 *rect, const float *z_entry,
+                                          int tiles_x, int prim_bits, uint64_t *keys, int tile_order, const MsCam &cam,
+                                          int tile, const float *A, const float *oprime, uint32_t cap) {
   uint32_t beg = emit_off[i], cnt = emit_off[i + 1] - beg;
   if (cnt == 0) return;
   int4 rc = rect[i];
@@ -190,6 +196,27 @@ __global__ void emit_keys_kernel(int n, const uint32_t *__restrict__ emit_off, c
   }
 }
 
+__global__ void emit_keys_kernel(int n, const uint32_t *__restrict__ emit_off, const int4 *__restrict__ rect,
+                                 const float *__restrict__ z_entry, int tiles_x, int prim_bits,
+                                 uint64_t *__restrict__ keys, int tile_order, MsCam cam, int tile,
+                                 const float *__restrict__ A, const float *__restrict__ oprime, uint32_t cap,
+                                 uint32_t *__restrict__ counters) {
+  int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  int lane = threadIdx.x & 31;
+  if (counters && blockIdx.x == 0 && threadIdx.x == 0) pair_guard(emit_off[n], cap, counters);
+  if (i >= n) return;
+  emit_body(i, lane, emit_off, rect, z_entry, tiles_x, prim_bits, keys, tile_order, cam, tile, A, oprime, cap);
+}
+
+__device__ __forceinline__ void tile_ranges_body(uint32_t i, const uint64_t *keys, uint32_t n_pairs, int n_tiles, int shift,
+                                                 uint32_t *tile_start) {
+  int t = (int)(keys[i] >> shift);
+  int prev = i == 0 ? -1 : (int)(keys[i - 1] >> shift);
+  for (int u = prev + 1; u <= t; ++u) tile_start[u] = i;
+  if (i == n_pairs - 1)
+    for (int u = t + 1; u <= n_tiles; ++u) tile_start[u] = n_pairs;
+}
+
 __global__ void tile_ranges_kernel(const uint64_t *__restrict__ keys, uint32_t n_pairs, int n_tiles, int shift,
                                    uint32_t *__restrict__ tile_start, const uint32_t *__restrict__ n_dev) {
   uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -198,12 +225,53 @@ __global__ void tile_ranges_kernel(const uint64_t *__restrict__ keys, uint32_t n
     if (n_pairs == 0 && i == 0)
       for (int u = 0; u <= n_tiles; ++u) tile_start[u] = 0u;
   }
-  if (i >= n_pairs) return;
-  int t = (int)(keys[i] >> shift);
-  int prev = i == 0 ? -1 : (int)(keys[i - 1] >> shift);
-  for (int u = prev + 1; u <= t; ++u) tile_start[u] = i;
-  if (i == n_pairs - 1)
-    for (int u = t + 1; u <= n_tiles; ++u) tile_start[u] = n_pairs;
+  if (i < n_pairs) tile_ranges_body(i, keys, n_pairs, n_tiles, shift, tile_start);
+}
+
+// Small frames rendered without host synchronisation (N <= MS_SMALL_PRIMS primitives, pair capacity <= SB_MAX): the
+// whole of stages (a) and (b) by ONE CTA in one launch -- counters reset, projection, offset scan, pair guard, key
+// emit, radix sort, tile ranges (7 stream operations otherwise; such a frame is bound by launch latency).  The same
+// device functions as the separate kernels: bitwise the same keys, tile lists and counters.
+struct MsBinSmallArgs {
+  int n;
+  const float *center, *A, *M;
+  MsCam cam;
+  int tile, tiles_x, n_tiles, prim_bits, tile_order, n_bits;
+  float eye_guard;
+  uint32_t cap;                     // pair capacity of keys_a / keys_b / the pair tables
+  uint32_t *tile_count, *emit_off, *counters, *tile_start, *pair_hits_j;
+  int4 *rect;
+  float *z_entry, *oprime;
+  uint64_t *keys_a, *keys_b;
+};
+
+__global__ void __launch_bounds__(SB_THREADS) bin_sort_small_kernel(MsBinSmallArgs a) {
+  extern __shared__ __align__(16) uint8_t sb_smem[];
+  __shared__ uint32_t dsum[8];
+  __shared__ uint32_t wt[SB_THREADS / 32 + 1];
+  __shared__ uint32_t s_P;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (tid < MS_CNT_N) a.counters[tid] = 0u;                // the sticky overflow flag behind them stays
+  for (uint32_t e = tid; e < a.cap + 2; e += SB_THREADS) a.pair_hits_j[e] = 0u;   // slots beyond the pair count (stage (c))
+  __syncthreads();
+  for (int i = tid; i < a.n; i += SB_THREADS)
+    project_body(i, a.center, a.A, a.M, a.cam, a.tile, a.eye_guard, a.tile_count, a.rect, a.z_entry, a.oprime, a.counters);
+  __syncthreads();
+  cta_exclusive_scan_u32<SB_THREADS>(a.tile_count, a.emit_off, (size_t)a.n, wt);
+  __syncthreads();
+  if (tid == 0) s_P = pair_guard(a.emit_off[a.n], a.cap, a.counters);
+  for (int i = warp; i < a.n; i += SB_THREADS / 32)
+    emit_body(i, lane, a.emit_off, a.rect, a.z_entry, a.tiles_x, a.prim_bits, a.keys_a, a.tile_order, a.cam, a.tile, a.A,
+              a.oprime, a.cap);
+  __syncthreads();
+  const uint32_t P = s_P;
+  block_sort(a.keys_a, a.keys_b, P, a.prim_bits, a.n_bits, sb_smem, dsum);
+  __syncthreads();
+  if (P == 0) {
+    for (int u = tid; u <= a.n_tiles; u += SB_THREADS) a.tile_start[u] = 0u;
+  } else {
+    for (uint32_t i = tid; i < P; i += SB_THREADS) tile_ranges_body(i, a.keys_b, P, a.n_tiles, 32 + a.prim_bits, a.tile_start);
+  }
 }
 
 // ms_render without host synchronisation: the pair count against the capacity the scratch was sized for
@@ -232,6 +300,30 @@ cudaError_t ms_emit_keys(int n, const uint32_t *emit_off, const int4 *rect, cons
   long threads = (long)n * 32;
   emit_keys_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, s>>>(n, emit_off, rect, z_entry, tiles_x, prim_bits,
                                                                     keys, tile_order, cam, tile, A, oprime, cap, counters);
+  MS_LAUNCHED();
+  return cudaGetLastError();
+}
+
+bool ms_bin_sort_small_fits(int n_prims, size_t pair_cap) { return n_prims <= MS_SMALL_PRIMS && pair_cap <= (size_t)SB_MAX; }
+
+cudaError_t ms_bin_sort_small(int n, const float *center, const float *A, const float *M, MsCam cam, int tile, float eye_guard,
+                              int tiles_x, int n_tiles, int prim_bits, int tile_order, int n_bits, uint32_t cap,
+                              uint32_t *tile_count, uint32_t *emit_off, int4 *rect, float *z_entry, float *oprime,
+                              uint32_t *counters, uint64_t *keys_a, uint64_t *keys_b, uint32_t *tile_start,
+                              uint32_t *pair_hits_j, cudaStream_t s) {
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute((const void *)bin_sort_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)SB_SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  MsBinSmallArgs a;
+  a.n = n; a.center = center; a.A = A; a.M = M; a.cam = cam; a.tile = tile; a.tiles_x = tiles_x; a.n_tiles = n_tiles;
+  a.prim_bits = prim_bits; a.tile_order = tile_order; a.n_bits = n_bits; a.eye_guard = eye_guard; a.cap = cap;
+  a.tile_count = tile_count; a.emit_off = emit_off; a.counters = counters; a.tile_start = tile_start;
+  a.pair_hits_j = pair_hits_j; a.rect = rect; a.z_entry = z_entry; a.oprime = oprime; a.keys_a = keys_a; a.keys_b = keys_b;
+  bin_sort_small_kernel<<<1, SB_THREADS, SB_SMEM_BYTES, s>>>(a);
   MS_LAUNCHED();
   return cudaGetLastError();
 }

@@ -246,6 +246,15 @@ cudaError_t ms_emit_keys(int n, const uint32_t *emit_off, const int4 *rect, cons
                          int prim_bits, uint64_t *keys, int tile_order, MsCam cam, int tile, const float *A,
                          const float *oprime, cudaStream_t s, uint32_t cap = 0xffffffffu,
                          uint32_t *counters = nullptr);   // counters: no-sync views (pair count + overflow guard)
+// small frames without host synchronisation: stages (a) + (b) in one launch of one CTA (ms_bin.cu)
+constexpr int MS_SMALL_PRIMS = 4096;
+constexpr size_t MS_BLOCK_SORT_MAX = 16384;   // keys one CTA sorts in one launch (ms_block_sort.cuh: SB_MAX)
+bool ms_bin_sort_small_fits(int n_prims, size_t pair_cap);
+cudaError_t ms_bin_sort_small(int n, const float *center, const float *A, const float *M, MsCam cam, int tile, float eye_guard,
+                              int tiles_x, int n_tiles, int prim_bits, int tile_order, int n_bits, uint32_t cap,
+                              uint32_t *tile_count, uint32_t *emit_off, int4 *rect, float *z_entry, float *oprime,
+                              uint32_t *counters, uint64_t *keys_a, uint64_t *keys_b, uint32_t *tile_start,
+                              uint32_t *pair_hits_j, cudaStream_t s);
 cudaError_t ms_tile_ranges(const uint64_t *keys, size_t n_pairs, int n_tiles, int prim_bits, uint32_t *tile_start,
                            cudaStream_t s, const uint32_t *n_dev = nullptr);
 // no-sync renders: counters[MS_CNT_P_EFF] = min(*total, cap); MS_CNT_OVERFLOW if the pairs do not fit
@@ -282,6 +291,14 @@ struct MsBandArgs {
   const uint64_t *keys;        // sorted tile lists
   const uint32_t *tile_start;
   const uint32_t *ray_off;     // [R'+1]
+  // small frames without host synchronisation (ms_order_single): the CTA that orders the pairs also scans the ray hit
+  // counts (fuse_ray_scan: ray_hits [R] -> ray_off_w [R + 1]) and takes the tile statistics (fuse_stats; hit_cap as in
+  // ms_tile_stats)
+  const uint32_t *ray_hits;
+  uint32_t *ray_off_w;
+  size_t R;
+  uint32_t hit_cap;
+  int fuse_ray_scan, fuse_stats;
   const uint32_t *emit_off;    // [N+1]  (single-band path)
   const int4 *rect;            // [N]    (single-band path)
   const uint32_t *pair_hits_i; // [P] by tile-list index
@@ -311,6 +328,9 @@ enum MsCounter { MS_CNT_SEGS = 0, MS_CNT_BLOCKS, MS_CNT_HITS, MS_CNT_HITS_HI, MS
 cudaError_t ms_tile_stats(const MsGrid &g, const uint32_t *ray_off, const uint32_t *tile_start, uint32_t *counters,
                           cudaStream_t s, uint32_t hit_cap = 0);
 // one band, one wave: segments = primitives in emission order (the layout of small frames)
+// one CTA orders the pairs of such a frame; it can take the ray scan and the tile statistics along (MsBandArgs)
+bool ms_order_single_is_small(size_t P, int n_prims);
+constexpr size_t MS_SMALL_RAYS = 65536;   // ray slots one CTA scans along the way
 cudaError_t ms_order_single(const MsBandArgs &a, cudaStream_t s);
 // bands x waves: pairs sorted by (band, wave, primitive), segments = runs of equal (band, wave, primitive)
 cudaError_t ms_order_banded(const MsBandArgs &a, cudaStream_t s);
