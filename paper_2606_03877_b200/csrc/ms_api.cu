@@ -598,6 +598,8 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   ca.gates = want_slots ? (const float4 *)sc->staging_gate.p : nullptr;
   ca.coef = want_slots ? (float4 *)sc->staging_coef.p : nullptr;
   ca.slots = sc->slots; ca.c_f = sc->slot_cf;
+  ca.keys = sorted; ca.tile_start = (uint32_t *)sc->tile_start.p; ca.pair_hits = (uint32_t *)sc->pair_hits_i.p;
+  ca.prim_bits = prim_bits;
   ca.dbg_ord = keep_order ? (uint32_t *)sc->dbg_ord.p : nullptr;
   ca.counters = counters;
   ca.out_rgb = out_rgb; ca.out_alpha = out_alpha; ca.out_feat = (want_feat || want_slots) ? out_feat : nullptr;

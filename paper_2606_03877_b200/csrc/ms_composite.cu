@@ -373,6 +373,128 @@ __global__ void __launch_bounds__(CW * 32, FEAT == 0 ? 12 : 8) composite_kernel(
   if (lane == 0 && n_stopped && a.counters) atomicAdd(&a.counters[MS_CNT_STOPPED_RAYS], n_stopped);
 }
 
+// Eq.7 features, tile-owned accumulation.  A ray's hits are a subsequence of its tile's sorted list (stage (c) writes
+// them in list order), so the CTA of a tile walks that list ONCE: the four embedding rows of a primitive are loaded
+// once per (tile, 128-channel chunk) instead of once per group of four rays, and a primitive that no pixel of the warp
+// hits costs one ballot.  CTA = (tile, block of up to 256 ray slots, chunk of 128 channels); a warp owns 32 consecutive
+// ray slots (two rows of a 16 x 16 tile): lane l keeps the hit-list cursor of slot l AND the accumulators of the channels
+// 4 l .. 4 l + 3 of all 32 slots (128 registers).  Per primitive of the list: ballot of the slots whose next hit it
+// is, their coefficients through shared memory (one broadcast LDS.128 per hit), 16 FMAs per hit and lane.  The sum of
+// a ray runs over its hits in list order whatever the band layout: deterministic.
+constexpr int SF_CHUNK = 32;          // list entries staged per step (one per lane)
+
+// V = the channels a lane owns: float4 (chunks of 128 channels, 128 accumulator registers, one CTA per SM); float2
+// (chunks of 64, two CTAs per SM, the list walked twice as often) is kept for the comparison only
+__device__ __forceinline__ float4 sf_zero(float4) { return make_float4(0.f, 0.f, 0.f, 0.f); }
+__device__ __forceinline__ float2 sf_zero(float2) { return make_float2(0.f, 0.f); }
+__device__ __forceinline__ void sf_fma(float4 &F, const float4 c, const float4 e0, const float4 e1, const float4 e2, const float4 e3) {
+  F.x = fmaf(c.w, e3.x, fmaf(c.z, e2.x, fmaf(c.y, e1.x, fmaf(c.x, e0.x, F.x))));
+  F.y = fmaf(c.w, e3.y, fmaf(c.z, e2.y, fmaf(c.y, e1.y, fmaf(c.x, e0.y, F.y))));
+  F.z = fmaf(c.w, e3.z, fmaf(c.z, e2.z, fmaf(c.y, e1.z, fmaf(c.x, e0.z, F.z))));
+  F.w = fmaf(c.w, e3.w, fmaf(c.z, e2.w, fmaf(c.y, e1.w, fmaf(c.x, e0.w, F.w))));
+}
+__device__ __forceinline__ void sf_fma(float2 &F, const float4 c, const float2 e0, const float2 e1, const float2 e2, const float2 e3) {
+  F.x = fmaf(c.w, e3.x, fmaf(c.z, e2.x, fmaf(c.y, e1.x, fmaf(c.x, e0.x, F.x))));
+  F.y = fmaf(c.w, e3.y, fmaf(c.z, e2.y, fmaf(c.y, e1.y, fmaf(c.x, e0.y, F.y))));
+}
+
+template <typename V>
+__global__ void __launch_bounds__(256, sizeof(V) == 8 ? 2 : 1) slot_feature_tile_kernel(MsCompositeArgs a, int blocks_per_tile, int n_chunks) {
+  constexpr int VW = (int)(sizeof(V) / 4);
+  __shared__ float4 sC[8][32];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (a.counters && a.counters[MS_CNT_OVERFLOW]) return;
+  const MsBand band = a.band;
+  const uint32_t T2 = (uint32_t)(a.grid.tile * a.grid.tile);
+  const int chunk = blockIdx.x % n_chunks;
+  const int blk = (blockIdx.x / n_chunks) % blocks_per_tile;
+  const uint32_t pos = band.q_lo / T2 + blockIdx.x / (uint32_t)(n_chunks * blocks_per_tile);
+  const ushort2 txy = a.grid.pos_xy[pos];
+  const int tile_id = (int)txy.y * a.grid.tiles_x + (int)txy.x;
+  const uint32_t q = pos * T2 + (uint32_t)blk * 256u + threadIdx.x;      // this lane's ray slot
+  int px, py;
+  const bool live = q < band.q_hi && ms_slot_pixel_dev(a.grid, q, &px, &py);
+  const uint32_t off = live ? a.ray_off[q] : 0u;
+  const uint32_t nh = live ? a.ray_off[q + 1] - off : 0u;
+  // the cursor of this lane's hit list, with the next coefficient and the two next primitives already loaded: the
+  // loads a hit triggers are consumed one hit later
+  uint32_t cur = 0;
+  int nxt = nh ? __ldg(&a.hits[off].prim) : -1;
+  int nxt2 = nh > 1 ? __ldg(&a.hits[off + 1].prim) : -1;
+  const float4 *coef = a.coef + (off - band.slot0);
+  float4 cnext = nh ? __ldg(coef) : make_float4(0.f, 0.f, 0.f, 0.f);
+  V F[32];
+#pragma unroll
+  for (int j = 0; j < 32; ++j) F[j] = sf_zero(V());
+  const uint64_t pmask = (1ull << a.prim_bits) - 1ull;
+  const uint32_t beg = a.tile_start[tile_id], end = a.tile_start[tile_id + 1];
+  const size_t cf = (size_t)a.c_f, cf4 = cf / VW, prow = 4 * cf4;     // in units of V: a row, a primitive's four rows
+  const V *slots4 = reinterpret_cast<const V *>(a.slots) + 32 * chunk + lane;
+  const unsigned any_hits = __ballot_sync(FULL, nh > 0);
+  // list entry i: its primitive, or -1 past the end / for a pair without hits
+  auto entry = [&](uint32_t i) -> int {
+    if (i < end && (!a.pair_hits || __ldg(a.pair_hits + i) > 0u)) return (int)(__ldg(a.keys + i) & pmask);
+    return -1;
+  };
+  if (any_hits && beg < end) {
+    int my_p = entry(beg + lane);                          // lane c stages entry base + c of the current chunk ...
+    V e0, e1, e2, e3;                                 // the embedding rows of the current entry (this lane's channels)
+    {
+      const int p0 = __shfl_sync(FULL, my_p, 0);
+      const V *e = slots4 + (size_t)(p0 < 0 ? 0 : p0) * prow;
+      e0 = __ldg(e); e1 = __ldg(e + cf4); e2 = __ldg(e + 2 * cf4); e3 = __ldg(e + 3 * cf4);
+    }
+    for (uint32_t base = beg; base < end; base += SF_CHUNK) {
+      const int my_p2 = entry(base + SF_CHUNK + lane);     // ... and of the one after it
+      const int nc = (int)(end - base < (uint32_t)SF_CHUNK ? end - base : (uint32_t)SF_CHUNK);
+      for (int c = 0; c < nc; ++c) {
+        const int p = __shfl_sync(FULL, my_p, c);
+        // the rows of the entry after this one are on their way while this one is summed
+        const int pn = c + 1 < SF_CHUNK ? __shfl_sync(FULL, my_p, (c + 1) & 31) : __shfl_sync(FULL, my_p2, 0);
+        const V *en = slots4 + (size_t)(pn < 0 ? 0 : pn) * prow;
+        const V n0 = __ldg(en), n1 = __ldg(en + cf4), n2 = __ldg(en + 2 * cf4), n3 = __ldg(en + 3 * cf4);
+        const bool has = p >= 0 && nxt == p;
+        const unsigned m = __ballot_sync(FULL, has);
+        if (m) {
+          sC[warp][lane] = has ? cnext : make_float4(0.f, 0.f, 0.f, 0.f);
+          if (has) {
+            ++cur;
+            nxt = nxt2;
+            if (cur < nh) cnext = __ldg(coef + cur);
+            nxt2 = cur + 1 < nh ? __ldg(&a.hits[off + cur + 1].prim) : -1;
+          }
+          __syncwarp();
+          // groups of four neighbouring slots: a group with a hit is summed whole (zero coefficients where there is
+          // none) -- straight-line code with four independent broadcast loads and sixteen FMA chains in flight
+#pragma unroll
+          for (int g = 0; g < 8; ++g) {
+            if ((m >> (4 * g)) & 15u) {
+              float4 cj[4];
+#pragma unroll
+              for (int u = 0; u < 4; ++u) cj[u] = sC[warp][4 * g + u];
+#pragma unroll
+              for (int u = 0; u < 4; ++u) {
+                sf_fma(F[4 * g + u], cj[u], e0, e1, e2, e3);
+              }
+            }
+          }
+          __syncwarp();
+        }
+        e0 = n0; e1 = n1; e2 = n2; e3 = n3;
+      }
+      my_p = my_p2;
+    }
+  }
+  // pixel j of the warp: 32 lanes x sizeof(V) contiguous bytes of its feature row
+  const unsigned lv = __ballot_sync(FULL, live);
+  const long long my_pix = live ? (long long)py * a.grid.W + px : 0;
+#pragma unroll
+  for (int j = 0; j < 32; ++j) {
+    const long long pix = __shfl_sync(FULL, my_pix, j);
+    if ((lv >> j) & 1u) reinterpret_cast<V *>(a.out_feat + (size_t)pix * cf)[32 * chunk + lane] = F[j];
+  }
+}
+
 // Eq.7 features: F[ray] = sum over the ray's hits of coef_k e_k[prim], coef = (T alpha) g from
 // composite_kernel<2>.  The sum's order is free, so one warp takes R = 4 consecutive rays of a row and walks the
 // UNION of their primitives: the four embedding rows of a primitive (16 c_f bytes, the whole cost of this
@@ -584,8 +706,16 @@ cudaError_t ms_composite(const MsCompositeArgs &a, cudaStream_t s) {
   else { if (dbg) composite_kernel<1, true><<<grid, CW * 32, 0, s>>>(a); else composite_kernel<1, false><<<grid, CW * 32, 0, s>>>(a); }
   MS_LAUNCHED();
   if (slot_feat) {
-    constexpr int R = 4;
-    slot_feature_kernel<R><<<(unsigned)((slots / R + CW - 1) / CW), CW * 32, 0, s>>>(a);
+    const size_t T2 = (size_t)a.grid.tile * a.grid.tile;
+    if (a.keys && a.tile_start && a.grid.pos_xy && a.band.q_lo % T2 == 0 && slots % T2 == 0 && a.c_f % 128 == 0) {
+      const int threads = (int)(T2 < 256 ? T2 : 256), bpt = (int)((T2 + 255) / 256);
+      const size_t n_tiles = slots / T2;
+      // float2 per lane (64-channel chunks, two CTAs per SM) measured slower: 2.75 against 2.64 ms on next2
+      slot_feature_tile_kernel<float4><<<(unsigned)(n_tiles * bpt * (a.c_f / 128)), threads, 0, s>>>(a, bpt, a.c_f / 128);
+    } else {
+      constexpr int R = 4;
+      slot_feature_kernel<R><<<(unsigned)((slots / R + CW - 1) / CW), CW * 32, 0, s>>>(a);
+    }
     MS_LAUNCHED();
   }
   return cudaGetLastError();

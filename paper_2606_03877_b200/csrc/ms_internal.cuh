@@ -398,6 +398,11 @@ struct MsCompositeArgs {
   float4 *coef;          // (T alpha) g_k per hit: composite_kernel<2> -> slot_feature_kernel
   const float *slots;    // [N][4][c_f] slot embeddings
   int c_f;
+  // Eq.7 features, tile-owned accumulation (slot_feature_tile_kernel): the sorted tile lists and the hits per pair
+  const uint64_t *keys;
+  const uint32_t *tile_start;
+  const uint32_t *pair_hits;   // by tile-list index, or NULL
+  int prim_bits;
   uint32_t *counters;    // MS_CNT_STOPPED_RAYS
   uint32_t *dbg_ord;     // MS_FLAG_KEEP_ORDER: [n_hits*K] sample index (h*K + k) by (hit slot of the ray)*K + rank
   float *out_rgb, *out_alpha, *out_feat;

@@ -83,18 +83,19 @@ def test_contact_dense_scene_early_termination_and_t_near():
     assert (d2 > TOL_FP32).sum() <= 2 and d2.max() < 1.5e-4
 
 
-@pytest.mark.parametrize("c_f,W,H", [(128, 96, 54), (512, 64, 36)])
-def test_next2_slot_features(c_f, W, H):
+@pytest.mark.parametrize("c_f,W,H,tile", [(128, 96, 54, 16), (512, 64, 36, 16), (256, 53, 37, 8), (128, 70, 45, 32)])
+def test_next2_slot_features(c_f, W, H, tile):
     """Eq.7 slot features (S:Sec.8(f) NEXT-2): gates, embeddings and the colour weights; C_f = 512 is the
-    paper's width.  Features are linear in O(1) embeddings: 1e-5 relative to their range."""
+    paper's width.  Features are linear in O(1) embeddings: 1e-5 relative to their range.  Tile edges 8 and
+    32 on ragged images: a CTA of the feature kernel owns a whole 64-slot tile, or a quarter of a 1 024-slot one."""
     from dataclasses import replace
     api = _api()
     cfg = synth.shrink(replace(synth.CONFIGS["next2"], c_f=c_f), W, H)
     sc, cam = synth.make_scene(cfg), synth.make_cameras(cfg)[0]
     gs = api.Scene(sc)
-    rgb, alpha, feat = gs.render(cam, H, W, 1)
+    rgb, alpha, feat = gs.render(cam, H, W, 1, tile=tile)
     torch.cuda.synchronize()
-    o_rgb, o_alpha, o_feat, st = mso.OracleScene(sc).render(cam, H, W, 1)
+    o_rgb, o_alpha, o_feat, st = mso.OracleScene(sc).render(cam, H, W, 1, tile=tile)
     assert feat.shape == (H, W, c_f) and gs.stats().n_intervals == st.n_intervals
     assert np.abs(rgb.cpu().numpy().reshape(-1, 3) - o_rgb).max() <= TOL_FP32
     assert np.abs(alpha.cpu().numpy().reshape(-1) - o_alpha).max() <= TOL_FP32
