@@ -77,3 +77,37 @@ def test_no_sync_overflow_is_reported_and_recovered():
     torch.cuda.synchronize()
     assert gs.stats().no_sync == 1 and gs.stats().overflow == 0
     assert torch.equal(out[0], ref[0]) and torch.equal(out[1], ref[1])
+
+
+def test_no_sync_small_frame_in_tile_order_and_with_nothing_in_view():
+    """The fused small-frame launches (stages (a) + (b) by one CTA; ray scan, tile statistics and pair order by one CTA)
+    in the paper's shared per-tile order (MS_FLAG_TILE_ORDER: keys carry the tile-centre contact depth), and on a view
+    that sees no primitive at all after one that saw many (zero pairs: every list empty, background only)."""
+    api = _api()
+    cfg = synth.shrink(synth.CONFIGS["next1"], 96, 54)
+    sc, cam = synth.make_scene(cfg), synth.make_cameras(cfg)[0]
+    H, W = cfg.height, cfg.width
+    gs = api.Scene(sc)
+    fl = api.FLAG_TILE_ORDER
+    ref = [t.clone() for t in gs.render(cam, H, W, 1, flags=fl)[:2]]
+    torch.cuda.synchronize()
+    assert gs.stats().no_sync == 0 and 0 < gs.stats().n_pairs <= 16384
+    launches = []
+    for _ in range(2):
+        n0 = api.launch_count()
+        out = gs.render(cam, H, W, 1, flags=fl | api.FLAG_NO_SYNC)
+        launches.append(api.launch_count() - n0)
+        torch.cuda.synchronize()
+        assert gs.stats().no_sync == 1 and gs.stats().overflow == 0
+        assert torch.equal(out[0], ref[0]) and torch.equal(out[1], ref[1])
+    assert launches[-1] <= 8, launches                     # fused (a)+(b), count, order, fill, MLP, composite (+ scan)
+    # the same scene seen from behind the camera plane: nothing projects
+    away = synth.pinhole(W, H, cfg.fov_deg, synth.look_at([0.0, 0.0, 60.0], target=[0.0, 0.0, 120.0]))
+    blank = gs.render(away, H, W, 1, flags=fl | api.FLAG_NO_SYNC)
+    torch.cuda.synchronize()
+    st = gs.stats()
+    assert st.no_sync == 1 and st.overflow == 0 and st.n_pairs == 0 and st.n_intervals == 0
+    assert float(blank[0].abs().max()) == 0.0 and float(blank[1].abs().max()) == 0.0
+    back = gs.render(cam, H, W, 1, flags=fl | api.FLAG_NO_SYNC)          # and the scratch still serves the full view
+    torch.cuda.synchronize()
+    assert gs.stats().overflow == 0 and torch.equal(back[0], ref[0])
