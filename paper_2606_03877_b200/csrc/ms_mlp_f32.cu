@@ -150,6 +150,7 @@ __global__ void __launch_bounds__(MS_ROWS / SPT, 6) mlp_f32_w32_kernel(MsMlpArgs
   __shared__ int s_seg;
   const MsMlpShape &sh = a.shape;
   const LaunchView lv(a.segs);
+  float *const h_s = w_s + ((sh.params + 3) & ~3);     // [SPT][32][MS_ROWS / SPT]: the inputs of the hidden layers 2..
   int cur_prim = -1;
   // the CTA walks a contiguous run of the launch's blocks: the weights are reloaded only when the primitive changes
   const uint32_t blk_lo = (uint32_t)(((uint64_t)lv.n_blocks * blockIdx.x) / gridDim.x);
@@ -224,13 +225,20 @@ __global__ void __launch_bounds__(MS_ROWS / SPT, 6) mlp_f32_w32_kernel(MsMlpArgs
   };
   if (contact) {
     // x[2L j + 2l] = sin(2^l pi z_j), x[2L j + 2l + 1] = cos(2^l pi z_j)
-#pragma unroll
+    // (a runtime loop: six unrolled copies of this body put the kernel beyond the 32 KB instruction cache and the
+    // warps of an SM, each at a place of its own, stalled on instruction fetch -- 1.3 stall cycles per issue, ncu)
+#pragma unroll 1
     for (int c = 0; c < 6; ++c) {
+      float zc[SPT];
+#pragma unroll
+      for (int p = 0; p < SPT; ++p)
+        zc[p] = c == 0 ? z[p][0] : c == 1 ? z[p][1] : c == 2 ? z[p][2] : c == 3 ? z[p][3] : c == 4 ? z[p][4] : z[p][5];
       float scale = 1.0f;
+#pragma unroll 1
       for (int l = 0; l < sh.n_freq; ++l) {
         float sv[SPT], cv[SPT];
 #pragma unroll
-        for (int p = 0; p < SPT; ++p) sincospif(scale * z[p][c], &sv[p], &cv[p]);  // 2^l z is exact
+        for (int p = 0; p < SPT; ++p) sincospif(scale * zc[p], &sv[p], &cv[p]);  // 2^l z is exact
         feed(sv); feed(cv);
         scale *= 2.0f;
       }
@@ -279,16 +287,27 @@ __global__ void __launch_bounds__(MS_ROWS / SPT, 6) mlp_f32_w32_kernel(MsMlpArgs
 #pragma unroll
       for (int p = 0; p < SPT; ++p) { acc[p][4 * q] = v.x; acc[p][4 * q + 1] = v.y; acc[p][4 * q + 2] = v.z; acc[p][4 * q + 3] = v.w; }
     }
+    // the layer's inputs go through shared memory (column tid of h_s: conflict-free), so that the loop over them need
+    // not be unrolled for register indexing: 2 048 FMAs of straight-line code per layer otherwise
+    __syncwarp();
 #pragma unroll
+    for (int p = 0; p < SPT; ++p)
+#pragma unroll
+      for (int i = 0; i < 32; ++i) h_s[(p * 32 + i) * (MS_ROWS / SPT) + threadIdx.x] = h[p][i];
+    __syncwarp();
+#pragma unroll 2
     for (int i = 0; i < 32; ++i) {
       const float4 *wr = reinterpret_cast<const float4 *>(w + i * 32);
+      float x[SPT];
+#pragma unroll
+      for (int p = 0; p < SPT; ++p) x[p] = h_s[(p * 32 + i) * (MS_ROWS / SPT) + threadIdx.x];
 #pragma unroll
       for (int q = 0; q < 8; ++q) {
         const float4 v = wr[q];
 #pragma unroll
         for (int p = 0; p < SPT; ++p) {
-          acc[p][4 * q] = fmaf(h[p][i], v.x, acc[p][4 * q]); acc[p][4 * q + 1] = fmaf(h[p][i], v.y, acc[p][4 * q + 1]);
-          acc[p][4 * q + 2] = fmaf(h[p][i], v.z, acc[p][4 * q + 2]); acc[p][4 * q + 3] = fmaf(h[p][i], v.w, acc[p][4 * q + 3]);
+          acc[p][4 * q] = fmaf(x[p], v.x, acc[p][4 * q]); acc[p][4 * q + 1] = fmaf(x[p], v.y, acc[p][4 * q + 1]);
+          acc[p][4 * q + 2] = fmaf(x[p], v.z, acc[p][4 * q + 2]); acc[p][4 * q + 3] = fmaf(x[p], v.w, acc[p][4 * q + 3]);
         }
       }
     }
@@ -461,6 +480,7 @@ cudaError_t ms_mlp_f32(const MsMlpArgs &a, cudaStream_t s) {
   if (wd == 32 && a.shape.params % 4 == 0 && a.shape.n_hidden >= 1 && a.shape.n_hidden <= 3) {
     fn = a.shape.n_hidden == 1 ? mlp_f32_w32_kernel<1, 2> : (a.shape.n_hidden == 2 ? mlp_f32_w32_kernel<2, 2> : mlp_f32_w32_kernel<3, 2>);
     threads = MS_ROWS / 2;
+    if (a.shape.n_hidden > 1) smem = ((size_t)((a.shape.params + 3) & ~3) + (size_t)32 * MS_ROWS) * sizeof(float);
   } else if (wd % 4 == 0 && wd >= 8 && a.shape.mode == MS_MODE_LOCAL && a.shape.n_hidden >= 1 && smem_tile <= 226 * 1024) {
     fn = mlp_f32_tile_kernel;
     threads = TG_NT;
