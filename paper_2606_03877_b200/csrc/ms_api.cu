@@ -62,6 +62,11 @@ struct ms_scene {
   cudaEvent_t frame_done = nullptr;  // recorded after the counters' readback copy of the last view
   // banded views: stage (e) of band b runs on st2 while stage (d) of band b + 1 runs on the caller's stream
   cudaStream_t st2 = nullptr;
+  // ms_render_host, several views: the copy of view v to the host runs on copy_st beside the render of view v + 1
+  // (the outputs alternate between two device buffers: host_* and host2_*)
+  cudaStream_t copy_st = nullptr;
+  cudaEvent_t ev_rendered[2] = {nullptr, nullptr}, ev_copied[2] = {nullptr, nullptr};
+  Buf host2_rgb, host2_alpha, host2_feat;
   cudaEvent_t ev_mlp[2] = {nullptr, nullptr}, ev_comp[2] = {nullptr, nullptr};
   bool frame_pending = false;
   bool prev_terminated = false;      // MS_WAVES_AUTO: the previous view had rays stopping early
@@ -163,6 +168,19 @@ int ceil_log2(uint64_t v) {
   int b = 0;
   while ((1ull << b) < v) ++b;
   return b;
+}
+
+// Mid-frame read-backs (pair count, hit counters, band table) are written to pinned host memory by a kernel, not by
+// a device-to-host copy: a copy would queue on the copy engine behind the image copies of the previous view, which
+// ms_render_host runs on a stream of its own beside this view (a 300 MB copy ahead costs 5 ms of waiting).
+__global__ void readback_kernel(uint32_t *dst_host, const uint32_t *src, int n) {
+  for (int i = threadIdx.x; i < n; i += blockDim.x) dst_host[i] = src[i];
+  __threadfence_system();
+}
+cudaError_t readback_words(void *dst_host, const void *src, size_t n_words, cudaStream_t st) {
+  readback_kernel<<<1, 128, 0, st>>>((uint32_t *)dst_host, (const uint32_t *)src, (int)n_words);
+  MS_LAUNCHED();
+  return cudaGetLastError();
 }
 
 float round_bf16(float f) {
@@ -384,8 +402,8 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
     P = P_cap;
     P_dev = counters + MS_CNT_P_EFF;
   } else {
-    CK(cudaMemcpyAsync(sc->pinned, (uint32_t *)sc->emit_off.p + N, 4, cudaMemcpyDeviceToHost, st));
-    CK(cudaMemcpyAsync(sc->pinned + 1 + MS_CNT_PAIRS_HI, counters + MS_CNT_PAIRS_HI, 4, cudaMemcpyDeviceToHost, st));
+    CK(readback_words(sc->pinned, (uint32_t *)sc->emit_off.p + N, 1, st));
+    CK(readback_words(sc->pinned + 1 + MS_CNT_PAIRS_HI, counters + MS_CNT_PAIRS_HI, 1, st));
     CK(cudaStreamSynchronize(st));
     // the 32-bit scan total must agree with the 64-bit count of the projection kernel (a wrapped sum would size
     // every buffer below too small)
@@ -455,7 +473,7 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
   size_t n_hits = hit_cap, max_tile_hits = 0;     // no-sync: the capacity stands in for the count
   uint32_t max_list = 0;
   if (!nosync) {
-    CK(cudaMemcpyAsync(sc->pinned + 1, counters, MS_CNT_N * 4, cudaMemcpyDeviceToHost, st));
+    CK(readback_words(sc->pinned + 1, counters, MS_CNT_N, st));
     CK(cudaStreamSynchronize(st));
     if (sc->pinned[1 + MS_CNT_HITS_HI] != 0) return MS_ERR_UNSUPPORTED_SHAPE;   // 64-bit hit total beyond 32 bits
     n_hits = sc->pinned[1 + MS_CNT_HITS];
@@ -565,7 +583,7 @@ int render_view(ms_scene *sc, const ms_camera *camera, int H, int W, const ms_op
     band_tab[0].q_lo = 0u; band_tab[0].q_hi = (uint32_t)R; band_tab[0].slot0 = 0u; band_tab[0].pad = 0u;
   } else {
     ENS_HOST(sc, (size_t)n_bands * sizeof(MsBand));
-    CK(cudaMemcpyAsync(sc->pinned_bands, sc->bands.p, (size_t)n_bands * sizeof(MsBand), cudaMemcpyDeviceToHost, st));
+    CK(readback_words(sc->pinned_bands, sc->bands.p, (size_t)n_bands * sizeof(MsBand) / 4, st));
     CK(cudaStreamSynchronize(st));
     memcpy(band_tab.data(), sc->pinned_bands, (size_t)n_bands * sizeof(MsBand));
   }
@@ -867,6 +885,12 @@ int ms_scene_destroy(ms_scene *sc) {
   free_buf(sc->bwd_rgb); free_buf(sc->bwd_alpha); free_buf(sc->bwd_ord); free_buf(sc->bwd_gstage);
   free_buf(sc->bwd_ivgrad); free_buf(sc->bwd_gA);
   free_buf(sc->host_rgb); free_buf(sc->host_alpha); free_buf(sc->host_feat);
+  free_buf(sc->host2_rgb); free_buf(sc->host2_alpha); free_buf(sc->host2_feat);
+  for (int i = 0; i < 2; ++i) {
+    if (sc->ev_rendered[i]) cudaEventDestroy(sc->ev_rendered[i]);
+    if (sc->ev_copied[i]) cudaEventDestroy(sc->ev_copied[i]);
+  }
+  if (sc->copy_st) cudaStreamDestroy(sc->copy_st);
   if (sc->pinned) cudaFreeHost(sc->pinned);
   if (sc->pinned_bands) cudaFreeHost(sc->pinned_bands);
   for (auto &E : sc->evs) {
@@ -915,14 +939,41 @@ int ms_render_host(ms_scene *sc, const ms_camera *cams, int32_t n_views, int32_t
   ENS(sc->host_rgb, px * 12);
   ENS(sc->host_alpha, px * 4);
   if (feat) ENS(sc->host_feat, px * (size_t)nf * 4);
-  for (int v = 0; v < n_views; ++v) {
-    rc = render_view(sc, cams + v, H, W, opts, (float *)sc->host_rgb.p, (float *)sc->host_alpha.p,
-                     feat ? (float *)sc->host_feat.p : nullptr);
-    if (rc != MS_OK) return rc;
-    CK(cudaMemcpyAsync(host_rgb + v * px * 3, sc->host_rgb.p, px * 12, cudaMemcpyDeviceToHost, st));
-    CK(cudaMemcpyAsync(host_alpha + v * px, sc->host_alpha.p, px * 4, cudaMemcpyDeviceToHost, st));
-    if (feat) CK(cudaMemcpyAsync(host_feat + v * px * nf, sc->host_feat.p, px * (size_t)nf * 4, cudaMemcpyDeviceToHost, st));
+  const bool two = n_views > 1;            // several views: copy view v beside the render of view v + 1
+  if (two) {
+    ENS(sc->host2_rgb, px * 12);
+    ENS(sc->host2_alpha, px * 4);
+    if (feat) ENS(sc->host2_feat, px * (size_t)nf * 4);
+    if (!sc->copy_st) {
+      CK(cudaStreamCreateWithFlags(&sc->copy_st, cudaStreamNonBlocking));
+      for (int i = 0; i < 2; ++i) {
+        CK(cudaEventCreateWithFlags(&sc->ev_rendered[i], cudaEventDisableTiming));
+        CK(cudaEventCreateWithFlags(&sc->ev_copied[i], cudaEventDisableTiming));
+      }
+    }
   }
+  for (int v = 0; v < n_views; ++v) {
+    const int b = two ? (v & 1) : 0;
+    float *d_rgb = (float *)(b ? sc->host2_rgb.p : sc->host_rgb.p), *d_alpha = (float *)(b ? sc->host2_alpha.p : sc->host_alpha.p);
+    float *d_feat = feat ? (float *)(b ? sc->host2_feat.p : sc->host_feat.p) : nullptr;
+    if (two && v >= 2) CK(cudaStreamWaitEvent(st, sc->ev_copied[b], 0));      // view v - 2 has left this buffer
+    rc = render_view(sc, cams + v, H, W, opts, d_rgb, d_alpha, d_feat);
+    if (rc != MS_OK) {
+      if (two) cudaStreamSynchronize(sc->copy_st);
+      return rc;
+    }
+    cudaStream_t cs = st;
+    if (two) {
+      CK(cudaEventRecord(sc->ev_rendered[b], st));
+      CK(cudaStreamWaitEvent(sc->copy_st, sc->ev_rendered[b], 0));
+      cs = sc->copy_st;
+    }
+    CK(cudaMemcpyAsync(host_rgb + v * px * 3, d_rgb, px * 12, cudaMemcpyDeviceToHost, cs));
+    CK(cudaMemcpyAsync(host_alpha + v * px, d_alpha, px * 4, cudaMemcpyDeviceToHost, cs));
+    if (feat) CK(cudaMemcpyAsync(host_feat + v * px * nf, d_feat, px * (size_t)nf * 4, cudaMemcpyDeviceToHost, cs));
+    if (two) CK(cudaEventRecord(sc->ev_copied[b], sc->copy_st));
+  }
+  if (two) CK(cudaStreamSynchronize(sc->copy_st));
   CK(cudaStreamSynchronize(st));
   if (opts->flags & MS_FLAG_NO_SYNC) {   // a view that outgrew the scratch sized from its predecessor: once more, sizing
     rc = finish_frame(sc);

@@ -177,13 +177,15 @@ def test_empty_and_degenerate_inputs():
 def test_render_batch_and_host_entry_match_single_view():
     api = _api()
     cfg = synth.shrink(synth.CONFIGS["cfg5"], 64, 36)
-    sc, cams = synth.make_scene(cfg), synth.make_cameras(cfg)[:3]
-    gs = api.Scene(sc)
+    sc, cams = synth.make_scene(cfg), synth.make_cameras(cfg)[:5]     # five views: the host entry's two output buffers
+    gs = api.Scene(sc)                                                # are each reused (copy of view v beside view v + 1)
     singles = [gs.render(c, 36, 64, cfg.K, path=api.PATH_FP32) for c in cams]
     singles = [[t.clone() for t in s] for s in singles]
     rgb, alpha, feat = gs.render_batch(cams, 36, 64, cfg.K, path=api.PATH_FP32)
     h_rgb, h_alpha, h_feat = gs.render_host(cams, 36, 64, cfg.K, path=api.PATH_FP32)
+    h1 = gs.render_host(cams[3:4], 36, 64, cfg.K, path=api.PATH_FP32)          # one view: no second stream
     torch.cuda.synchronize()
+    assert torch.equal(h1[0][0], singles[3][0].cpu()) and torch.equal(h1[2][0], singles[3][2].cpu())
     for v, s in enumerate(singles):
         assert torch.equal(rgb[v], s[0]) and torch.equal(alpha[v], s[1]) and torch.equal(feat[v], s[2])
         assert torch.equal(h_rgb[v], s[0].cpu()) and torch.equal(h_alpha[v], s[1].cpu())
