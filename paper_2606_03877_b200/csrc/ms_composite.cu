@@ -10,7 +10,8 @@
 // straight from global memory -- only the order (4 B per sample) lives in shared memory, so 40+
 // warps fit per SM; each lane composites a run of consecutive merged samples, one warp product
 // scan per window links the runs.  Features
-// (32 channels): four 128 B rows per warp load.
+// (32 channels): four 128 B rows per warp load.  Eq.7 slot features: composite_kernel<2> leaves per-hit coefficients,
+// slot_feature_tile_kernel sums the embeddings tile by tile.
 // HBM-bound by design: reads 16 B (+ 4 n_feat B) per sample and 16 B per hit, once.
 #include <cuda_fp16.h>
 
@@ -248,7 +249,7 @@ __global__ void __launch_bounds__(CW * 32, FEAT == 0 ? 12 : 8) composite_kernel(
       C0 += c0; C1 += c1; C2 += c2;
       if (FEAT == 2) {
         // Eq.7: F = sum_i (T_i alpha_i) sum_k g_ik e_ik.  This kernel only turns every hit's gates into
-        // its coefficients (T alpha) g_k; slot_feature_kernel sums the embeddings (the sum's order is free).
+        // its coefficients (T alpha) g_k; slot_feature_tile_kernel sums the embeddings.
         __syncwarp();
         const float4 *gates = a.gates + loc;
         float4 *coef = a.coef + loc;
@@ -383,19 +384,13 @@ __global__ void __launch_bounds__(CW * 32, FEAT == 0 ? 12 : 8) composite_kernel(
 // a ray runs over its hits in list order whatever the band layout: deterministic.
 constexpr int SF_CHUNK = 32;          // list entries staged per step (one per lane)
 
-// V = the channels a lane owns: float4 (chunks of 128 channels, 128 accumulator registers, one CTA per SM); float2
-// (chunks of 64, two CTAs per SM, the list walked twice as often) is kept for the comparison only
+// V = the channels a lane owns: float4 (chunks of 128 channels, 128 accumulator registers, one CTA per SM)
 __device__ __forceinline__ float4 sf_zero(float4) { return make_float4(0.f, 0.f, 0.f, 0.f); }
-__device__ __forceinline__ float2 sf_zero(float2) { return make_float2(0.f, 0.f); }
 __device__ __forceinline__ void sf_fma(float4 &F, const float4 c, const float4 e0, const float4 e1, const float4 e2, const float4 e3) {
   F.x = fmaf(c.w, e3.x, fmaf(c.z, e2.x, fmaf(c.y, e1.x, fmaf(c.x, e0.x, F.x))));
   F.y = fmaf(c.w, e3.y, fmaf(c.z, e2.y, fmaf(c.y, e1.y, fmaf(c.x, e0.y, F.y))));
   F.z = fmaf(c.w, e3.z, fmaf(c.z, e2.z, fmaf(c.y, e1.z, fmaf(c.x, e0.z, F.z))));
   F.w = fmaf(c.w, e3.w, fmaf(c.z, e2.w, fmaf(c.y, e1.w, fmaf(c.x, e0.w, F.w))));
-}
-__device__ __forceinline__ void sf_fma(float2 &F, const float4 c, const float2 e0, const float2 e1, const float2 e2, const float2 e3) {
-  F.x = fmaf(c.w, e3.x, fmaf(c.z, e2.x, fmaf(c.y, e1.x, fmaf(c.x, e0.x, F.x))));
-  F.y = fmaf(c.w, e3.y, fmaf(c.z, e2.y, fmaf(c.y, e1.y, fmaf(c.x, e0.y, F.y))));
 }
 
 template <typename V>
@@ -492,115 +487,6 @@ __global__ void __launch_bounds__(256, sizeof(V) == 8 ? 2 : 1) slot_feature_tile
   for (int j = 0; j < 32; ++j) {
     const long long pix = __shfl_sync(FULL, my_pix, j);
     if ((lv >> j) & 1u) reinterpret_cast<V *>(a.out_feat + (size_t)pix * cf)[32 * chunk + lane] = F[j];
-  }
-}
-
-// Eq.7 features: F[ray] = sum over the ray's hits of coef_k e_k[prim], coef = (T alpha) g from
-// composite_kernel<2>.  The sum's order is free, so one warp takes R = 4 consecutive rays of a row and walks the
-// UNION of their primitives: the four embedding rows of a primitive (16 c_f bytes, the whole cost of this
-// stage) are loaded once and used for every ray of the group that hits it -- neighbouring rays share most
-// of their primitives (a 2 x 2 pixel block instead of 4 in a row measured no better).  Lane l holds channels 4 (l + 32 q)..+3; lane j also holds hit j of each ray.
-template <int R>
-__global__ void __launch_bounds__(CW * 32) slot_feature_kernel(MsCompositeArgs a) {
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  if (a.counters && a.counters[MS_CNT_OVERFLOW]) return;
-  const MsBand band = a.band;
-  // groups of R consecutive ray slots (R divides the tile edge: one tile row)
-  for (uint32_t q0 = band.q_lo + (blockIdx.x * CW + warp) * R; q0 < band.q_hi; q0 = band.q_hi) {
-  long long ray_of[R];     // output pixel index, -1 for a padding slot
-  uint32_t slot_q[R];
-#pragma unroll
-  for (int r = 0; r < R; ++r) {
-    int px, py;
-    slot_q[r] = q0 + r;
-    ray_of[r] = (q0 + r < band.q_hi && ms_slot_pixel_dev(a.grid, q0 + r, &px, &py)) ? (long long)py * a.grid.W + px : -1;
-  }
-  const int cf4 = a.c_f >> 2, nq = a.c_f >> 7;
-  float4 F[R][4];
-  int prim[R], nh[R];
-  uint32_t off[R], used[R];
-  float4 cf[R];
-  bool big = false;
-#pragma unroll
-  for (int r = 0; r < R; ++r) {
-#pragma unroll
-    for (int q = 0; q < 4; ++q) F[r][q] = make_float4(0.f, 0.f, 0.f, 0.f);
-    const bool live = ray_of[r] >= 0;
-    off[r] = live ? a.ray_off[slot_q[r]] : 0u;
-    nh[r] = live ? (int)(a.ray_off[slot_q[r] + 1] - off[r]) : 0;
-    big |= nh[r] > 32;
-    used[r] = 0u;
-    prim[r] = -1;
-    cf[r] = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (lane < nh[r] && nh[r] <= 32) {
-      prim[r] = __ldg(&a.hits[off[r] + lane].prim);
-      cf[r] = __ldg(a.coef + (off[r] - band.slot0) + lane);
-    }
-  }
-  auto add = [&](float4 (&Fr)[4], const float4 c, const float4 *e) {
-#pragma unroll
-    for (int q = 0; q < 4; ++q)
-      if (q < nq) {
-        const float4 e0 = __ldg(e + 32 * q), e1 = __ldg(e + cf4 + 32 * q), e2 = __ldg(e + 2 * cf4 + 32 * q),
-                     e3 = __ldg(e + 3 * cf4 + 32 * q);
-        Fr[q].x += fmaf(c.w, e3.x, fmaf(c.z, e2.x, fmaf(c.y, e1.x, c.x * e0.x)));
-        Fr[q].y += fmaf(c.w, e3.y, fmaf(c.z, e2.y, fmaf(c.y, e1.y, c.x * e0.y)));
-        Fr[q].z += fmaf(c.w, e3.z, fmaf(c.z, e2.z, fmaf(c.y, e1.z, c.x * e0.z)));
-        Fr[q].w += fmaf(c.w, e3.w, fmaf(c.z, e2.w, fmaf(c.y, e1.w, c.x * e0.w)));
-      }
-  };
-  if (!big) {
-#pragma unroll
-    for (int ra = 0; ra < R; ++ra) {
-      for (int j = 0; j < nh[ra]; ++j) {
-        if ((used[ra] >> j) & 1u) continue;
-        const int p = __shfl_sync(FULL, prim[ra], j);
-        const float4 *e = reinterpret_cast<const float4 *>(a.slots + (size_t)p * 4 * (size_t)a.c_f) + lane;
-        float4 c[R];          // coefficients of this primitive in the rays of the group that hit it (0 otherwise)
-#pragma unroll
-        for (int rb = 0; rb < R; ++rb) {
-          c[rb] = make_float4(0.f, 0.f, 0.f, 0.f);
-          if (rb < ra) continue;
-          int jb = j;
-          if (rb > ra) {
-            const unsigned m = __ballot_sync(FULL, prim[rb] == p) & ~used[rb];
-            if (!m) continue;
-            jb = __ffs(m) - 1;
-            used[rb] |= 1u << jb;
-          }
-          c[rb] = make_float4(__shfl_sync(FULL, cf[rb].x, jb), __shfl_sync(FULL, cf[rb].y, jb),
-                              __shfl_sync(FULL, cf[rb].z, jb), __shfl_sync(FULL, cf[rb].w, jb));
-        }
-#pragma unroll
-        for (int q = 0; q < 4; ++q)
-          if (q < nq) {
-            const float4 e0 = __ldg(e + 32 * q), e1 = __ldg(e + cf4 + 32 * q), e2 = __ldg(e + 2 * cf4 + 32 * q),
-                         e3 = __ldg(e + 3 * cf4 + 32 * q);
-#pragma unroll
-            for (int rb = 0; rb < R; ++rb) {
-              if (rb < ra) continue;
-              F[rb][q].x += fmaf(c[rb].w, e3.x, fmaf(c[rb].z, e2.x, fmaf(c[rb].y, e1.x, c[rb].x * e0.x)));
-              F[rb][q].y += fmaf(c[rb].w, e3.y, fmaf(c[rb].z, e2.y, fmaf(c[rb].y, e1.y, c[rb].x * e0.y)));
-              F[rb][q].z += fmaf(c[rb].w, e3.z, fmaf(c[rb].z, e2.z, fmaf(c[rb].y, e1.z, c[rb].x * e0.z)));
-              F[rb][q].w += fmaf(c[rb].w, e3.w, fmaf(c[rb].z, e2.w, fmaf(c[rb].y, e1.w, c[rb].x * e0.w)));
-            }
-          }
-      }
-    }
-  } else {  // a ray with more than 32 hits: no sharing, every ray on its own
-#pragma unroll
-    for (int r = 0; r < R; ++r)
-      for (int j = 0; j < nh[r]; ++j) {
-        const int p = __ldg(&a.hits[off[r] + j].prim);
-        add(F[r], __ldg(a.coef + (off[r] - band.slot0) + j), reinterpret_cast<const float4 *>(a.slots + (size_t)p * 4 * (size_t)a.c_f) + lane);
-      }
-  }
-#pragma unroll
-  for (int r = 0; r < R; ++r)
-    if (ray_of[r] >= 0)
-#pragma unroll
-      for (int q = 0; q < 4; ++q)
-        if (q < nq) reinterpret_cast<float4 *>(a.out_feat + (size_t)ray_of[r] * a.c_f)[lane + 32 * q] = F[r][q];
   }
 }
 
@@ -707,15 +593,13 @@ cudaError_t ms_composite(const MsCompositeArgs &a, cudaStream_t s) {
   MS_LAUNCHED();
   if (slot_feat) {
     const size_t T2 = (size_t)a.grid.tile * a.grid.tile;
-    if (a.keys && a.tile_start && a.grid.pos_xy && a.band.q_lo % T2 == 0 && slots % T2 == 0 && a.c_f % 128 == 0) {
-      const int threads = (int)(T2 < 256 ? T2 : 256), bpt = (int)((T2 + 255) / 256);
-      const size_t n_tiles = slots / T2;
-      // float2 per lane (64-channel chunks, two CTAs per SM) measured slower: 2.75 against 2.64 ms on next2
-      slot_feature_tile_kernel<float4><<<(unsigned)(n_tiles * bpt * (a.c_f / 128)), threads, 0, s>>>(a, bpt, a.c_f / 128);
-    } else {
-      constexpr int R = 4;
-      slot_feature_kernel<R><<<(unsigned)((slots / R + CW - 1) / CW), CW * 32, 0, s>>>(a);
-    }
+    // bands are runs of whole tiles; the tile lists are those of stage (b)
+    if (!(a.keys && a.tile_start && a.grid.pos_xy && a.band.q_lo % T2 == 0 && slots % T2 == 0 && a.c_f % 128 == 0))
+      return cudaErrorInvalidValue;
+    const int threads = (int)(T2 < 256 ? T2 : 256), bpt = (int)((T2 + 255) / 256);
+    const size_t n_tiles = slots / T2;
+    // float2 per lane (64-channel chunks, two CTAs per SM) measured slower: 2.75 against 2.64 ms on next2
+    slot_feature_tile_kernel<float4><<<(unsigned)(n_tiles * bpt * (a.c_f / 128)), threads, 0, s>>>(a, bpt, a.c_f / 128);
     MS_LAUNCHED();
   }
   return cudaGetLastError();

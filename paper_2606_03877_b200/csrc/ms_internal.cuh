@@ -395,7 +395,7 @@ struct MsCompositeArgs {
   const void *staging_feat;
   int feat_half;         // staging_feat holds fp16 rows (tensor path, n_feat == 32)
   const float4 *gates;   // slot gates (Eq.7) or NULL
-  float4 *coef;          // (T alpha) g_k per hit: composite_kernel<2> -> slot_feature_kernel
+  float4 *coef;          // (T alpha) g_k per hit: composite_kernel<2> -> slot_feature_tile_kernel
   const float *slots;    // [N][4][c_f] slot embeddings
   int c_f;
   // Eq.7 features, tile-owned accumulation (slot_feature_tile_kernel): the sorted tile lists and the hits per pair

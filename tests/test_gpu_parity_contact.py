@@ -213,7 +213,7 @@ def test_tile_centre_order(tile):
 
 def test_more_than_32_hits_per_ray_with_slot_features():
     """48 nested / overlapping supports around one point: the central rays carry 40+ hits, which takes the
-    general merge of stage (e) (no lane-per-hit fast path) and the unshared path of the feature kernel."""
+    general merge of stage (e) (no lane-per-hit fast path) and hit-list cursors far into the tile list in the feature kernel."""
     api = _api()
     mlp = synth.MLPSpec(3, 0, 1, 16, 0, False, synth.MODE_CONTACT)
     rng = np.random.default_rng(21)
