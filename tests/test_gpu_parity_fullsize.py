@@ -68,6 +68,10 @@ def test_cfg5_all_eight_views():
         torch.cuda.synchronize()
         assert torch.equal(r1, rgb[v]) and torch.equal(a1, alpha[v]) and torch.equal(f1, feat[v])
         check_full_size_structures(gs, orc, cam, cfg)
+    # the end-to-end entry (ms_render_host: view v copied to the host on a second stream beside the render of view v + 1,
+    # two alternating device buffers, 2.4 GB per call): bitwise the batch
+    h_rgb, h_alpha, h_feat = gs.render_host(cams, H, W, K, tile=cfg.tile)
+    assert torch.equal(h_rgb, rgb.cpu()) and torch.equal(h_alpha, alpha.cpu()) and torch.equal(h_feat, feat.cpu())
 
 
 def test_cfg4_full_size_renders_are_deterministic():
