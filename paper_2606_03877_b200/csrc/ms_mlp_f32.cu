@@ -9,6 +9,15 @@
 
 namespace {
 
+// sin(pi x), cos(pi x) on the special-function unit: exact reduction to [-1, 1], then MUFU.SIN / MUFU.COS, whose
+// absolute error on [-pi, pi] is 2^-21.4 / 2^-21.2 (CUDA C Programming Guide, intrinsic functions)
+__device__ __forceinline__ void sincospi_mufu(float x, float *s, float *c) {
+  const float r = x - 2.0f * rintf(0.5f * x);
+  const float a = 3.14159265358979323846f * r;
+  *s = __sinf(a);
+  *c = __cosf(a);
+}
+
 // segment of block b of the launch: largest s with bo[s] - base <= b
 __device__ __forceinline__ int find_seg(const uint32_t *__restrict__ bo, int n, uint32_t base, uint32_t b) {
   int lo = 0, hi = n;
@@ -238,7 +247,8 @@ __global__ void __launch_bounds__(MS_ROWS / SPT, 6) mlp_f32_w32_kernel(MsMlpArgs
       for (int l = 0; l < sh.n_freq; ++l) {
         float sv[SPT], cv[SPT];
 #pragma unroll
-        for (int p = 0; p < SPT; ++p) sincospif(scale * zc[p], &sv[p], &cv[p]);  // 2^l z is exact
+        for (int p = 0; p < SPT; ++p) sincospi_mufu(scale * zc[p], &sv[p], &cv[p]);  // 2^l z is exact; 36 pairs per hit:
+        // sincospif here was 19 % of the kernel's instructions; with the SFU the image stays 2e-7 from the oracle (bar 1e-5)
         feed(sv); feed(cv);
         scale *= 2.0f;
       }
