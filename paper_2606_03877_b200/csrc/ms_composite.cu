@@ -138,29 +138,34 @@ __global__ void __launch_bounds__(CW * 32, FEAT == 0 ? 12 : 8) composite_kernel(
     const size_t loc = (size_t)(off - band.slot0);        // the ray's first hit inside the band's staging buffers
     const float4 *stg = a.staging + loc * (size_t)K;
     const uint32_t S = (uint32_t)n * (uint32_t)K;
-    if (FEAT != 1 && K == 1 && n <= 32) {
-      // One sample per hit and at most one hit per lane (the contact-point mode's usual ray): lane j holds hit j,
-      // its rank is the number of hits that precede it in (t, prim) order, one product scan composites the ray.
+    const bool one_hit = FEAT == 0 && n == 1 && K > 1 && K <= 32;   // a single interval: its samples are in order
+    if ((FEAT != 1 && K == 1 && n <= 32) || one_hit) {
+      // At most one sample per lane.  K = 1 (the contact-point mode's usual ray): lane j holds hit j, its rank is the
+      // number of hits that precede it in (t, prim) order.  One hit with K <= 32 samples (the usual ray of a sparse
+      // scene): lane k holds sample k, already in order.  One product scan composites the ray.
+      const int m = one_hit ? K : n;
       float t = 0.f;
       int prim = 0x7fffffff;
-      if (lane < n) {
+      if (!one_hit && lane < n) {
         const MsHit g = hits[lane];
         t = ms_sample_tm(g.t_in, g.delta, 0, a.contact);
         prim = g.prim;
       }
       uint32_t rank = 0;
-      for (int j = 0; j < n; ++j) {
-        const float t2 = __shfl_sync(FULL, t, j);
-        const int p2 = __shfl_sync(FULL, prim, j);
-        rank += (j != lane && precedes(t2, t, p2 < prim)) ? 1u : 0u;
+      if (!one_hit) {
+        for (int j = 0; j < n; ++j) {
+          const float t2 = __shfl_sync(FULL, t, j);
+          const int p2 = __shfl_sync(FULL, prim, j);
+          rank += (j != lane && precedes(t2, t, p2 < prim)) ? 1u : 0u;
+        }
       }
-      if (a.tile_order) rank = (uint32_t)lane;      // the shared per-tile order: the hits as stage (c) wrote them
-      if (lane < n) {
+      if (a.tile_order || one_hit) rank = (uint32_t)lane;      // the shared per-tile order: the hits as stage (c) wrote them
+      if (lane < m) {
         sm.ord[rank] = (uint32_t)lane;
-        if (DBG) a.dbg_ord[(size_t)off + rank] = (uint32_t)lane;
+        if (DBG) a.dbg_ord[(size_t)off * (size_t)K + rank] = (uint32_t)lane;
       }
       __syncwarp();
-      const bool valid = lane < n;
+      const bool valid = lane < m;
       uint32_t slot = 0;
       float4 v = make_float4(0.f, 0.f, 0.f, 1.f);
       if (valid) {
@@ -180,7 +185,7 @@ __global__ void __launch_bounds__(CW * 32, FEAT == 0 ? 12 : 8) composite_kernel(
       const float w = (valid && lane <= last) ? excl * (1.0f - v.w) : 0.f;
       C0 = w * v.x; C1 = w * v.y; C2 = w * v.z;
       T = __shfl_sync(FULL, p, stop ? last : 31);
-      n_stopped += (stop && last + 1 < n) ? 1u : 0u;
+      n_stopped += (stop && last + 1 < m) ? 1u : 0u;
       if (FEAT == 2 && valid) {
         const float4 g = __ldg(a.gates + loc + slot);
         a.coef[loc + slot] = make_float4(w * g.x, w * g.y, w * g.z, w * g.w);
