@@ -182,8 +182,8 @@ def algorithmic_bytes(cfg, sc) -> dict:
 
 
 def load_dram_profile():
-    """dram__bytes_read.sum + dram__bytes_write.sum per view and stage, from the committed `ncu --set full` captures
-    (profiles/r2_dram_bytes.csv, copied by hand from the summaries it names; absent workloads -> null)."""
+    """dram__bytes_read.sum + dram__bytes_write.sum per view and stage, from the committed ncu captures
+    (profiles/r2_dram_bytes.csv, copied by hand from the summary it names; absent workloads -> null)."""
     path = os.path.join(ROOT, "profiles", "r2_dram_bytes.csv")
     out = {}
     if os.path.exists(path):
