@@ -154,6 +154,22 @@ def test_contact_tensor_path_large_world_units():
     assert_bf16_bar(rgb.cpu().numpy().reshape(-1, 3), alpha.cpu().numpy().reshape(-1), o_rgb, o_alpha)
 
 
+def test_contact_fp32_path_large_world_units():
+    """The same scene on the fp32 path: its encode reduces 2^l z exactly to [-1, 1] before the SFU sin / cos (absolute
+    error 2^-21 whatever |z|), so the 1e-5 bar holds with delta up to ~10 world units (2^5 z up to ~300)."""
+    api = _api()
+    mlp = synth.MLPSpec(6, 0, 2, 32, 0, False, synth.MODE_CONTACT)
+    cfg = synth.SceneConfig("big_contact32", 11, 24, 20.0, 4.0, 10.0, mlp, 96, 54, 60.0, 60.0, 1)
+    sc, cam = synth.make_scene(cfg), synth.make_cameras(cfg)[0]
+    gs = api.Scene(sc)
+    rgb, alpha, _ = gs.render(cam, 54, 96, 1, path=api.PATH_FP32)
+    torch.cuda.synchronize()
+    o_rgb, o_alpha, _, st = mso.OracleScene(sc).render(cam, 54, 96, 1)
+    assert st.n_intervals > 2000
+    assert np.abs(rgb.cpu().numpy().reshape(-1, 3) - o_rgb).max() <= TOL_FP32
+    assert np.abs(alpha.cpu().numpy().reshape(-1) - o_alpha).max() <= TOL_FP32
+
+
 def test_next1b_full_size_sampled_pixels():
     from test_gpu_parity_bf16 import assert_bf16_bar
     api = _api()
