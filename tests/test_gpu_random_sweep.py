@@ -99,3 +99,37 @@ def test_tensor_path_random_scenes_bands_waves_overlap():
             if fl == api.FLAG_DEBUG_ALL:
                 assert check_structures(gs, orc, cam, H, W, K, tile, n_order_rays=3) == n_int, what
         gs.close()
+
+
+def test_contact_mode_with_slot_features_random_scenes():
+    """The paper's own mode with Eq.7 features on the fp32 path: the tile-owned feature kernel under random tile edges,
+    image sizes (ragged tiles), C_f, band budgets and the shared per-tile order; rays with more than 32 hits included."""
+    api = _api()
+    rng = np.random.default_rng(4242)
+    for seed in range(24):
+        n = int(rng.integers(3, 150)); tile = int(rng.choice([8, 16, 32])); c_f = int(rng.choice([128, 256, 512]))
+        W = int(rng.integers(9, 120)); H = int(rng.integers(9, 90))
+        mlp = synth.MLPSpec(6, 0, 2, 32, 0, False, synth.MODE_CONTACT, falloff=float(rng.choice([0.0, 4.5])))
+        cfg = synth.SceneConfig(f"c{seed}", seed, n, 0.8, 0.2, 0.9, mlp, W, H, 50.0, 3.0, 1,
+                                sigma_bias=float(rng.choice([-1.0, 0.5, 6.0])), c_f=c_f)
+        sc, cam = synth.make_scene(cfg), synth.make_cameras(cfg)[0]
+        order = int(rng.choice([0, api.FLAG_TILE_ORDER]))
+        what = dict(seed=seed, n=n, tile=tile, c_f=c_f, W=W, H=H, order=order)
+        gs, orc = api.Scene(sc), mso.OracleScene(sc)
+        orc.set_order(1 if order else 0)
+        gs.band_bytes = -1
+        ref = [t.clone() for t in gs.render(cam, H, W, 1, tile=tile, flags=order)]
+        torch.cuda.synchronize()
+        n_int = gs.stats().n_intervals
+        o_rgb, o_alpha, o_feat, st = orc.render(cam, H, W, 1, tile=tile)
+        assert n_int == st.n_intervals, what
+        assert np.abs(ref[0].cpu().numpy().reshape(-1, 3) - o_rgb).max() <= TOL_FP32, what
+        assert np.abs(ref[1].cpu().numpy().reshape(-1) - o_alpha).max() <= TOL_FP32, what
+        scale = max(1.0, np.abs(o_feat).max())
+        assert np.abs(ref[2].cpu().numpy().reshape(-1, c_f) - o_feat).max() <= TOL_FP32 * scale, what
+        for budget in (int(rng.choice([24 << 10, 200 << 10])), 0):
+            gs.band_bytes = budget
+            out = gs.render(cam, H, W, 1, tile=tile, flags=order | (api.FLAG_NO_SYNC if budget == 0 else 0))
+            torch.cuda.synchronize()
+            assert all(torch.equal(a, b) for a, b in zip(out, ref)), (what, budget, gs.stats().n_bands)
+        gs.close()
